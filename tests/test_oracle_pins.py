@@ -1,0 +1,530 @@
+"""Pins for the CPU oracle (oracle/vr_oracle.c): closed forms, invariants, special cases and an
+independent brute-force numpy renderer. None of these call the CUDA path. Citations are
+PAPER.md lines; R# are the readings of DESIGN.md."""
+import math
+import os
+
+import numpy as np
+import pytest
+
+import oracle
+import synth
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+
+
+# --------------------------------------------------------------------------- helpers
+def ortho_along_z(nx, ny, nz):
+    """Axis-aligned orthographic camera looking along +z, one pixel per voxel column.
+    Pixel (i, j) looks down the column x = nx-1-i, y = j (the look-at basis mirrors x)."""
+    view = synth.look_at((nx / 2.0, ny / 2.0, -10.0), (nx / 2.0, ny / 2.0, 0.0), (0.0, 1.0, 0.0))
+    proj = synth.orthographic(nx / 2.0, ny / 2.0, 1.0, 30.0 + nz)
+    return view, proj
+
+
+def const_tf(rgb, a, n=4):
+    t = np.zeros((n, 4), dtype=np.float32)
+    t[:, :3] = rgb
+    t[:, 3] = a
+    return t
+
+
+def mats(view, proj):
+    V = np.asarray(view, dtype=np.float64).reshape(4, 4).T
+    P = np.asarray(proj, dtype=np.float64).reshape(4, 4).T
+    return V, P
+
+
+def ray_np(view, proj, W, H, i, j):
+    """Independent statement of R1/R2 with numpy's own inverse."""
+    V, P = mats(view, proj)
+    Minv = np.linalg.inv(P @ V)
+    x, y = 2 * (i + 0.5) / W - 1, 2 * (j + 0.5) / H - 1
+    a = Minv @ np.array([x, y, -1.0, 1.0])
+    b = Minv @ np.array([x, y, 1.0, 1.0])
+    a, b = a[:3] / a[3], b[:3] / b[3]
+    L = np.linalg.norm(b - a)
+    return a, (b - a) / L, L
+
+
+def chord_np(o, d, L, n):
+    """Independent clip of the segment o + t d, t in [0, L], against [0,n] (Liang-Barsky)."""
+    t0, t1 = 0.0, L
+    for a in range(3):
+        if abs(d[a]) < 1e-300:
+            if o[a] < 0 or o[a] > n[a]:
+                return None
+            continue
+        ta, tb = (0 - o[a]) / d[a], (n[a] - o[a]) / d[a]
+        t0, t1 = max(t0, min(ta, tb)), min(t1, max(ta, tb))
+    return (t0, t1) if t1 > t0 else None
+
+
+def brute_force_render(data, tf, vmin, vmax, view, proj, W, H, step, mode):
+    """Independent, unbricked, global renderer written from the definitions (numpy/python)."""
+    nz, ny, nx = data.shape
+    n = (nx, ny, nz)
+    lut = np.asarray(tf, dtype=np.float64)
+    N = lut.shape[0]
+    img = np.zeros((H, W, 4))
+
+    def vox(ix, iy, iz):
+        return float(data[min(max(iz, 0), nz - 1), min(max(iy, 0), ny - 1), min(max(ix, 0), nx - 1)])
+
+    def tri(p):
+        q = [p[0] - 0.5, p[1] - 0.5, p[2] - 0.5]
+        i0 = [math.floor(c) for c in q]
+        f = [q[a] - i0[a] for a in range(3)]
+        acc = 0.0
+        for dz in (0, 1):
+            for dy in (0, 1):
+                for dx in (0, 1):
+                    w = (f[0] if dx else 1 - f[0]) * (f[1] if dy else 1 - f[1]) * (f[2] if dz else 1 - f[2])
+                    acc += w * vox(i0[0] + dx, i0[1] + dy, i0[2] + dz)
+        return acc
+
+    def lut_at(v):
+        u = min(max((v - vmin) / (vmax - vmin), 0.0), 1.0)
+        xs = np.arange(N) / (N - 1.0)
+        return np.array([np.interp(u, xs, lut[:, c]) for c in range(4)])
+
+    for j in range(H):
+        for i in range(W):
+            o, d, L = ray_np(view, proj, W, H, i, j)
+            ch = chord_np(o, d, L, n)
+            if ch is None:
+                continue
+            t0, t1 = ch
+            K = int(math.ceil((t1 - t0) / step))
+            C, A, m, took = np.zeros(3), 0.0, -np.inf, 0
+            for k in range(K):
+                a0, a1 = t0 + k * step, min(t0 + (k + 1) * step, t1)
+                if a1 <= a0:
+                    continue
+                v = tri(o + 0.5 * (a0 + a1) * d)
+                took += 1
+                if mode == oracle.MIP:
+                    m = max(m, v)
+                else:
+                    rgba = lut_at(v)
+                    al = 1 - (1 - rgba[3]) ** (a1 - a0)
+                    C += (1 - A) * al * rgba[:3]
+                    A += (1 - A) * al
+            if mode == oracle.MIP:
+                if took:
+                    img[j, i, :3] = lut_at(m)[:3]
+                    img[j, i, 3] = 1.0
+            else:
+                img[j, i, :3], img[j, i, 3] = C, A
+    return img
+
+
+def small_noise(nx, ny, nz, seed=7, nsrc=3):
+    return synth.Cube(seed, nx, ny, nz, nsrc).fill_host(nthreads=1)
+
+
+# --------------------------------------------------------------------------- golden (paper's printed values)
+def test_table1_sizes_pin_float32_voxels():
+    """dims x 4 B reproduce the printed file sizes => float32 voxels."""
+    for line in open(os.path.join(GOLD, "table1_datasets.txt")):
+        if line.startswith("#") or not line.strip():
+            continue
+        name, nx, ny, nz, gb = [s.strip() for s in line.split("|")]
+        gib = int(nx) * int(ny) * int(nz) * np.dtype(np.float32).itemsize / 2.0 ** 30
+        assert abs(gib - float(gb)) <= 0.7, (name, gib)           # printed values are rounded
+        assert abs(gib * 2 - float(gb)) > 0.7 * float(gb) / 4     # float64 would not fit the table
+
+
+def test_subframe_message_is_one_float_per_pixel():
+    """4 MB per 1024x1024 frame => 4 B/pixel (MIP scalar sub-image, row a8)."""
+    for line in open(os.path.join(GOLD, "subframe_message.txt")):
+        if line.startswith("#") or not line.strip():
+            continue
+        w, h, mb = [float(s) for s in line.split("|")]
+        assert w * h * np.dtype(np.float32).itemsize == mb * 2 ** 20
+
+
+# --------------------------------------------------------------------------- pin 1: homogeneous cube
+@pytest.mark.parametrize("ortho", [False, True])
+def test_homogeneous_cube_closed_form(ortho):
+    """north_star: opacity 1-exp(-sigma L) = 1-(1-a)^L along every ray; exact by R5."""
+    nx, ny, nz = 12, 9, 15
+    a, rgb = float(np.float32(0.07)), (0.2, 0.5, 0.9)   # the LUT stores float32
+    data = np.full((nz, ny, nx), 1.25, dtype=np.float32)
+    W = H = 24
+    fr = synth.Framing(nx, ny, nz, W, H)
+    for bricks in (64, 5):
+        vol = oracle.Volume(nx, ny, nz, bricks, 1, data=data)
+        vol.set_transfer_function(const_tf(rgb, a), -3, 10)
+        vol.set_early_termination(2.0)
+        for k in range(3):
+            view, proj = fr.seeded(99, k), fr.proj(ortho)
+            img = vol.render(view, proj, W, H, 0.37, oracle.ALPHA, nthreads=2)["image"]
+            nhit = 0
+            for j in range(0, H, 3):
+                for i in range(0, W, 3):
+                    o, d, L = ray_np(view, proj, W, H, i, j)
+                    ch = chord_np(o, d, L, (nx, ny, nz))
+                    A = 0.0 if ch is None else 1 - (1 - a) ** (ch[1] - ch[0])
+                    nhit += ch is not None
+                    assert abs(img[j, i, 3] - A) < 1e-12
+                    np.testing.assert_allclose(img[j, i, :3], A * np.array(rgb, dtype=np.float32).astype(np.float64), atol=1e-12)
+            assert nhit > 10
+
+
+def test_camera_inside_volume_starts_at_near_plane():
+    """R2: path length is measured from the near plane when the camera is inside the cube."""
+    n = 20
+    data = np.zeros((n, n, n), dtype=np.float32)
+    a = float(np.float32(0.1))
+    vol = oracle.Volume(n, n, n, 8, 1, data=data)
+    vol.set_transfer_function(const_tf((1, 1, 1), a), -3, 10)
+    vol.set_early_termination(2.0)
+    view = synth.look_at((10.0, 10.0, 4.0), (10.0, 10.0, 20.0), (0.0, 1.0, 0.0))
+    proj = synth.perspective(30.0, 1.0, 2.0, 100.0)
+    W = H = 9
+    img = vol.render(view, proj, W, H, 0.5, oracle.ALPHA)["image"]
+    o, d, L = ray_np(view, proj, W, H, 4, 4)          # centre pixel: straight along +z
+    assert abs(o[2] - 6.0) < 1e-5 and abs(d[2] - 1.0) < 1e-9
+    assert abs(img[4, 4, 3] - (1 - (1 - a) ** (20.0 - o[2]))) < 1e-12
+
+
+# --------------------------------------------------------------------------- pin 2: single bright voxel
+def test_single_voxel_tent_mip():
+    """R3/R11: the interpolant of one bright voxel is a tent; axis-aligned rays sampling the
+    centre plane see V (1-|dx|)(1-|dy|)."""
+    n, V = 8, 8.0                     # n/2 is a power of two: the float32 matrices are exact
+    data = np.zeros((n, n, n), dtype=np.float32)
+    c = (4, 3, 5)                     # (x, y, z) index of the bright voxel
+    data[c[2], c[1], c[0]] = V
+    ident = np.zeros((256, 4), dtype=np.float32)
+    ident[:, 0] = np.linspace(0, 1, 256)
+    ident[:, 3] = 1
+    sub = 4                           # 4 x 4 pixels per voxel => lateral offsets +-1/8, +-3/8 ...
+    W = H = n * sub
+    view, proj = ortho_along_z(n, n, n)
+    for brick in (16, 4):
+        vol = oracle.Volume(n, n, n, brick, 1, data=data)
+        vol.set_transfer_function(ident, 0.0, 10.0)
+        img = vol.render(view, proj, W, H, 1.0, oracle.MIP)["image"]
+        for j in range(H):
+            for i in range(W):
+                x = n - (i + 0.5) / sub            # world x of the ray (mirrored basis)
+                y = (j + 0.5) / sub
+                tent = V * max(0.0, 1 - abs(x - (c[0] + 0.5))) * max(0.0, 1 - abs(y - (c[1] + 0.5)))
+                want = np.interp(tent / 10.0, np.arange(256) / 255.0, ident[:, 0].astype(np.float64))
+                assert abs(img[j, i, 0] - want) < 1e-12 and abs(want - tent / 10.0) < 1e-7
+                assert img[j, i, 3] == 1.0
+
+
+def test_centre_pixel_hits_volume_centre_and_mirror():
+    """R1: a symmetric view puts the volume centre on the centre of the frame; mirroring the
+    camera's x axis mirrors the image."""
+    n = 9
+    data = np.zeros((n, n, n), dtype=np.float32)
+    data[4, 4, 4] = 5.0
+    data[2, 6, 1] = 3.0               # an asymmetric marker
+    vol = oracle.Volume(n, n, n, 4, 1, data=data)
+    vol.set_transfer_function(synth.tf_ramp(), -3, 10)
+    W = H = 15
+    fr = synth.Framing(n, n, n, W, H)
+    view, proj = fr.turntable(0), fr.proj(False)
+    img = vol.render(view, proj, W, H, 0.25, oracle.MIP)["image"]
+    jm, im = np.unravel_index(np.argmax(img[:, :, 0]), (H, W))
+    assert (jm, im) == (H // 2, W // 2)
+    flip = np.diag([-1.0, 1.0, 1.0, 1.0])
+    P = np.asarray(proj, dtype=np.float64).reshape(4, 4).T
+    proj_m = np.ascontiguousarray((flip @ P).T.reshape(16)).astype(np.float32)
+    img_m = vol.render(view, proj_m, W, H, 0.25, oracle.MIP)["image"]
+    np.testing.assert_allclose(img_m, img[:, ::-1, :], atol=1e-12)
+    assert np.abs(img - img[:, ::-1, :]).max() > 1e-3
+
+
+# --------------------------------------------------------------------------- pin 3: axis-aligned orthographic
+def test_axis_aligned_ortho_mip_is_column_max_and_alpha_closed_form():
+    """north_star: axis-aligned orthographic MIP == per-column max; ALPHA == the column's
+    front-to-back product form (samples fall on voxel centres, w = 1). All d_a = 0 on two axes (R4)."""
+    nx, ny, nz = 8, 16, 13            # nx/2, ny/2 powers of two: the float32 matrices are exact
+    data = small_noise(nx, ny, nz)
+    view, proj = ortho_along_z(nx, ny, nz)
+    tf = synth.tf_translucent()
+    tf[:, 3] *= 20.0
+    tf = np.clip(tf, 0, 1).astype(np.float32)
+    vmin, vmax = -3.0, 10.0
+    for brick in (32, 4):
+        vol = oracle.Volume(nx, ny, nz, brick, 1, data=data)
+        vol.set_transfer_function(tf, vmin, vmax)
+        vol.set_early_termination(2.0)
+        mip = vol.render(view, proj, nx, ny, 1.0, oracle.MIP)["image"]
+        alp = vol.render(view, proj, nx, ny, 1.0, oracle.ALPHA)["image"]
+        lut = tf.astype(np.float64)
+        xs = np.arange(256) / 255.0
+        for j in range(ny):
+            for i in range(nx):
+                col = data[:, j, nx - 1 - i].astype(np.float64)
+                u = np.clip((col.max() - vmin) / (vmax - vmin), 0, 1)
+                assert abs(mip[j, i, 0] - np.interp(u, xs, lut[:, 0])) < 1e-12
+                uu = np.clip((col - vmin) / (vmax - vmin), 0, 1)
+                al = np.interp(uu, xs, lut[:, 3])
+                cr = np.interp(uu, xs, lut[:, 0])
+                T = np.concatenate([[1.0], np.cumprod(1 - al)[:-1]])
+                assert abs(alp[j, i, 3] - (1 - np.prod(1 - al))) < 1e-12
+                assert abs(alp[j, i, 0] - np.sum(T * al * cr)) < 1e-12
+
+
+# --------------------------------------------------------------------------- pin 4: 1 brick == N bricks
+@pytest.mark.parametrize("mode", [oracle.ALPHA, oracle.MIP])
+def test_one_brick_equals_n_bricks_ragged(mode):
+    """north_star / R3: with ghost >= 1 and ERT off the image does not depend on the bricking,
+    ragged grids included; no fetch leaves a padded brick. ghost = 0 must differ (seams)."""
+    nx, ny, nz = 19, 11, 13
+    data = small_noise(nx, ny, nz)
+    W, H = 32, 24
+    fr = synth.Framing(nx, ny, nz, W, H)
+    one = oracle.Volume(nx, ny, nz, 64, 1, data=data)
+    many = oracle.Volume(nx, ny, nz, 5, 1, data=data)
+    seam = oracle.Volume(nx, ny, nz, 5, 0, data=data)
+    assert many.nbricks == 4 * 3 * 3
+    for v in (one, many, seam):
+        v.set_transfer_function(synth.tf_ramp(), -3, 10)
+        v.set_early_termination(2.0)
+    worst_seam = 0.0
+    for k, ortho in ((0, False), (1, True), (2, False)):
+        view, proj = fr.seeded(5, k), fr.proj(ortho)
+        a = one.render(view, proj, W, H, 0.5, mode)
+        b = many.render(view, proj, W, H, 0.5, mode)
+        s = seam.render(view, proj, W, H, 0.5, mode)
+        assert np.abs(a["image"] - b["image"]).max() < 1e-12
+        assert np.array_equal(a["counts"][..., 1], b["counts"][..., 1])      # same schedule
+        worst_seam = max(worst_seam, np.abs(a["image"] - s["image"]).max())
+    assert one.ghost_violations() == 0 and many.ghost_violations() == 0
+    assert seam.ghost_violations() > 0 and worst_seam > 1e-3
+
+
+def test_oracle_bricks_are_edge_replicated_copies():
+    """a1 / R3: a padded brick equals the clamped-index gather of the source."""
+    nx, ny, nz = 10, 7, 6
+    data = small_noise(nx, ny, nz)
+    g, B = 2, 4
+    vol = oracle.Volume(nx, ny, nz, B, g, data=data)
+    b = 0
+    for bz in range(2):
+        for by in range(2):
+            for bx in range(3):
+                got = vol.brick_data(b)
+                zs = np.clip(np.arange(bz * B - g, min(bz * B + B, nz) + g), 0, nz - 1)
+                ys = np.clip(np.arange(by * B - g, min(by * B + B, ny) + g), 0, ny - 1)
+                xs = np.clip(np.arange(bx * B - g, min(bx * B + B, nx) + g), 0, nx - 1)
+                assert np.array_equal(got, data[np.ix_(zs, ys, xs)])
+                b += 1
+
+
+# --------------------------------------------------------------------------- pin 5: ERT bound
+def test_ert_within_one_minus_tau():
+    """R8: brick-local termination at tau changes a channel by at most (1 - tau)."""
+    nx = ny = nz = 24
+    data = small_noise(nx, ny, nz)
+    W = H = 24
+    fr = synth.Framing(nx, ny, nz, W, H)
+    view, proj = fr.turntable(3), fr.proj(False)
+    for tau in (0.99, 0.9):
+        vol = oracle.Volume(nx, ny, nz, 8, 1, data=data)
+        vol.set_transfer_function(synth.tf_ramp(), -3, 10)
+        vol.set_early_termination(2.0)
+        off = vol.render(view, proj, W, H, 0.5, oracle.ALPHA)
+        vol.set_early_termination(tau)
+        on = vol.render(view, proj, W, H, 0.5, oracle.ALPHA)
+        diff = np.abs(off["image"] - on["image"]).max()
+        assert 0 < diff <= (1 - tau) + 1e-12
+        assert on["counts"][..., 0].sum() < off["counts"][..., 0].sum()
+        assert np.array_equal(on["counts"][..., 1], off["counts"][..., 1])
+
+
+# --------------------------------------------------------------------------- pin 6/7: ordering
+def test_mip_is_order_independent_alpha_is_not():
+    """MIP composites in arbitrary order; `over` does not."""
+    nx, ny, nz = 16, 16, 16
+    data = small_noise(nx, ny, nz)
+    W = H = 16
+    fr = synth.Framing(nx, ny, nz, W, H)
+    view, proj = fr.seeded(1, 0), fr.proj(False)
+    vol = oracle.Volume(nx, ny, nz, 4, 1, data=data)
+    vol.set_transfer_function(synth.tf_ramp(), -3, 10)
+    vol.set_early_termination(2.0)
+    mip0 = vol.render(view, proj, W, H, 0.5, oracle.MIP)["image"]
+    alp0 = vol.render(view, proj, W, H, 0.5, oracle.ALPHA)["image"]
+    vol.set_order_override(synth.permutation(3, vol.nbricks))
+    assert np.array_equal(vol.render(view, proj, W, H, 0.5, oracle.MIP)["image"], mip0)
+    assert np.abs(vol.render(view, proj, W, H, 0.5, oracle.ALPHA)["image"] - alp0).max() > 1e-3
+
+
+@pytest.mark.parametrize("ortho", [False, True])
+def test_visibility_order_contains_every_ray_order(ortho):
+    """R9/R10: the global order is a permutation; every ray's t_in order is a subsequence of it;
+    consecutive bricks on a ray share a face; bricks holding samples are on the ray's list;
+    no brick holds samples for a pixel outside its rendering rectangle."""
+    nx, ny, nz = 19, 11, 13
+    data = small_noise(nx, ny, nz)
+    W, H = 20, 16
+    fr = synth.Framing(nx, ny, nz, W, H)
+    vol = oracle.Volume(nx, ny, nz, 5, 1, data=data)
+    vol.set_transfer_function(synth.tf_ramp(), -3, 10)
+    vol.set_early_termination(2.0)
+    pix = np.array([(i, j) for j in range(H) for i in range(W)], dtype=np.int32)
+    views = [fr.seeded(11, k) for k in range(4)]
+    # plus an eye inside the brick grid's span on one axis (distance-0 slab)
+    views.append(synth.look_at((9.5, 40.0, 6.0), (9.5, 5.0, 6.0), (0, 0, 1)))
+    for view in views:
+        proj = fr.proj(ortho) if view is not views[-1] else synth.perspective(50.0, W / H, 1.0, 200.0)
+        order = vol.brick_order(view, proj)
+        assert sorted(order.tolist()) == list(range(vol.nbricks))
+        pos = np.empty(vol.nbricks, dtype=np.int64)
+        pos[order] = np.arange(vol.nbricks)
+        counts, lists, graz = vol.ray_bricks(view, proj, W, H, pix, maxlen=16)
+        res = vol.render(view, proj, W, H, 0.5, oracle.MIP, pixels=pix, want_sub=True)
+        rects = vol.rects(view, proj, W, H)
+        hit_any = 0
+        for q in range(len(pix)):
+            if graz[q]:
+                continue
+            lst = lists[q, :counts[q]]
+            assert np.all(np.diff(pos[lst]) > 0), "ray order must embed in the global order"
+            for b0, b1 in zip(lst[:-1], lst[1:]):
+                c0 = np.array([b0 % 4, (b0 // 4) % 3, b0 // 12])
+                c1 = np.array([b1 % 4, (b1 // 4) % 3, b1 // 12])
+                assert np.abs(c0 - c1).sum() == 1, "consecutive bricks share a face"
+            holders = np.nonzero(res["sub"][q, :, 1] > 0)[0]
+            assert set(holders.tolist()) <= set(lst.tolist())
+            assert res["sub"][q, :, 1].sum() == res["counts"][q, 0] == res["counts"][q, 1]
+            i, j = pix[q]
+            for b in holders:
+                x0, y0, x1, y1 = rects[b]
+                assert x0 <= i < x1 and y0 <= j < y1
+            hit_any += len(lst) > 0
+        assert hit_any > 50
+
+
+def test_visibility_order_ragged_grid_close_eyes():
+    """R9 on a strongly ragged grid (slabs 5,5,1 / 4,3 / 6,2) with eyes close to and inside the
+    volume: slab-distance ranks stay valid where centre-distance sorting does not."""
+    nx, ny, nz = 11, 7, 8
+    vol = oracle.Volume(nx, ny, nz, 5, 1, data=np.zeros((nz, ny, nx), dtype=np.float32))
+    g = (3, 2, 2)
+    W = H = 24
+    pix = np.array([(i, j) for j in range(H) for i in range(W)], dtype=np.int32)
+    proj = synth.perspective(70.0, 1.0, 0.05, 60.0)
+    checked = 0
+    for k in range(60):
+        eye = np.array([synth.u01(5, a, k) * (n + 6.0) - 3.0 for a, n in enumerate((nx, ny, nz))])
+        tgt = np.array([synth.u01(6, a, k) * n for a, n in enumerate((nx, ny, nz))])
+        if np.linalg.norm(tgt - eye) < 0.5:
+            continue
+        view = synth.look_at(eye, tgt, (0.123, 0.456, 0.881))
+        order = vol.brick_order(view, proj)
+        pos = np.empty(vol.nbricks, dtype=np.int64)
+        pos[order] = np.arange(vol.nbricks)
+        counts, lists, graz = vol.ray_bricks(view, proj, W, H, pix, maxlen=16)
+        for q in range(len(pix)):
+            if graz[q] or counts[q] < 2:
+                continue
+            assert np.all(np.diff(pos[lists[q, :counts[q]]]) > 0)
+            checked += 1
+    assert checked > 5000
+
+
+# --------------------------------------------------------------------------- pin 8: convergence
+def test_step_halving_converges():
+    """R5: midpoint rule on a smooth field; halving the step shrinks the error."""
+    n = 24
+    z, y, x = np.meshgrid(*(np.arange(n) + 0.5,) * 3, indexing="ij")
+    data = (2.0 + 3.0 * np.sin(x / 5.0) * np.cos(y / 6.0) + 2.0 * np.sin(z / 4.0)).astype(np.float32)
+    W = H = 12
+    fr = synth.Framing(n, n, n, W, H)
+    view, proj = fr.seeded(2, 1), fr.proj(False)
+    vol = oracle.Volume(n, n, n, 8, 1, data=data)
+    tf = synth.tf_translucent()
+    tf[:, 3] *= 8
+    vol.set_transfer_function(tf.astype(np.float32), -3, 10)
+    vol.set_early_termination(2.0)
+    ref = vol.render(view, proj, W, H, 1.0 / 64, oracle.ALPHA)["image"]
+    errs = [np.abs(vol.render(view, proj, W, H, s, oracle.ALPHA)["image"] - ref).max() for s in (1.0, 0.5, 0.25)]
+    assert errs[0] > errs[1] > errs[2] > 0
+    assert errs[2] < errs[0] / 6.0
+
+
+# --------------------------------------------------------------------------- pin 9: brute force
+@pytest.mark.parametrize("mode", [oracle.ALPHA, oracle.MIP])
+@pytest.mark.parametrize("ortho", [False, True])
+def test_against_independent_brute_force_renderer(mode, ortho):
+    """Tiny inputs (<= 16^3, <= 16^2 pixels): the bricked C oracle equals an unbricked numpy
+    renderer written separately from the definitions."""
+    nx, ny, nz = 13, 9, 11
+    data = small_noise(nx, ny, nz, seed=21)
+    W, H = 12, 10
+    fr = synth.Framing(nx, ny, nz, W, H)
+    tf = synth.tf_ramp()
+    tf[:, 1] = tf[::-1, 1]
+    tf[:, 3] *= 0.3
+    view, proj = fr.seeded(4, 2), fr.proj(ortho)
+    vol = oracle.Volume(nx, ny, nz, 4, 1, data=data)
+    vol.set_transfer_function(tf, -2.0, 6.0)
+    vol.set_early_termination(2.0)
+    got = vol.render(view, proj, W, H, 0.4, mode)["image"]
+    want = brute_force_render(data, tf, -2.0, 6.0, view, proj, W, H, 0.4, mode)
+    assert np.abs(got - want).max() < 1e-9
+    assert (want[..., 3] > 0).sum() > 20
+
+
+# --------------------------------------------------------------------------- TF special cases (R7)
+def test_transfer_function_special_cases():
+    n = 12
+    data = small_noise(n, n, n)
+    W = H = 10
+    fr = synth.Framing(n, n, n, W, H)
+    view, proj = fr.seeded(8, 0), fr.proj(False)
+    vol = oracle.Volume(n, n, n, 5, 1, data=data)
+    vol.set_early_termination(2.0)
+    # a = 0: fully transparent frame
+    vol.set_transfer_function(const_tf((1, 1, 1), 0.0), -3, 10)
+    assert np.abs(vol.render(view, proj, W, H, 0.5, oracle.ALPHA)["image"]).max() == 0.0
+    # a = 1: the first sample's colour exactly, opacity 1
+    tf = synth.tf_ramp()
+    tf[:, 3] = 1.0
+    vol.set_transfer_function(tf, -3, 10)
+    img = vol.render(view, proj, W, H, 0.5, oracle.ALPHA)["image"]
+    hit = img[..., 3] > 0
+    assert hit.sum() > 10 and np.all(img[hit][:, 3] == 1.0)
+    one = oracle.Volume(n, n, n, 64, 1, data=data)
+    one.set_transfer_function(tf, -3, 10)
+    one.set_early_termination(0.5)         # stops after the first sample
+    assert np.abs(one.render(view, proj, W, H, 0.5, oracle.ALPHA)["image"] - img).max() < 1e-12
+    # constant colour: C = A c
+    c = np.array([0.3, 0.6, 0.1], dtype=np.float32)
+    tf2 = synth.tf_ramp()
+    tf2[:, :3] = c
+    vol.set_transfer_function(tf2, -3, 10)
+    img = vol.render(view, proj, W, H, 0.5, oracle.ALPHA)["image"]
+    np.testing.assert_allclose(img[..., :3], img[..., 3:4] * c.astype(np.float64), atol=1e-12)
+
+
+# --------------------------------------------------------------------------- compositing (R15)
+def test_composite_over_is_associative_and_matches_numpy():
+    W, H, n = 13, 9, 6
+    rects = [(0, 0, W, H), (2, 1, 9, 7), (5, 0, 13, 4), (0, 3, 6, 9), (4, 4, 5, 5), (1, 1, 12, 8)]
+    layers = []
+    for l, r in enumerate(rects):
+        layers.append(synth.layer_host(77, l, 0, (r[2] - r[0]) * (r[3] - r[1])).reshape(r[3] - r[1], r[2] - r[0], 4))
+    order = synth.permutation(9, n)
+    got = oracle.composite(layers, rects, order, W, H)
+    want = np.zeros((H, W, 4))
+    for l in order:
+        r = rects[l]
+        full = np.zeros((H, W, 4))
+        full[r[1]:r[3], r[0]:r[2]] = layers[l]
+        want += (1 - want[..., 3:4]) * full
+    assert np.abs(got - want).max() < 1e-15
+    # associativity: composite the two halves separately, then merge
+    h1 = oracle.composite([layers[l] for l in order[:3]], [rects[l] for l in order[:3]], np.arange(3), W, H)
+    h2 = oracle.composite([layers[l] for l in order[3:]], [rects[l] for l in order[3:]], np.arange(3), W, H)
+    merged = h1 + (1 - h1[..., 3:4]) * h2
+    assert np.abs(merged - got).max() < 1e-12
