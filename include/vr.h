@@ -1,0 +1,221 @@
+/*
+ * vr.h -- C ABI of libvr: the data-parallel hot path of the bricked ray-casting volume
+ * renderer of Hassan, Fluke & Barnes, "A Distributed GPU-based Framework for real-time 3D
+ * Volume Rendering of Large Astronomical Data Cubes" (arXiv:1205.0282), written from the
+ * paper for one NVIDIA B200 (sm_100a).
+ *
+ * Citations are lines of the paper text with the section they fall in; "R#" are
+ * the readings listed in DESIGN.md for points on which the paper is silent.
+ *
+ * Conventions (all calls)
+ *   - Every function returns a vr_status (0 = VR_OK). No exception or C++ type crosses this
+ *     boundary. vr_last_error() gives a human-readable message for the last failing call on
+ *     a handle (or for a failing vr_volume_create / vr_composite when passed NULL).
+ *   - "device" pointers are CUDA device pointers of the current device; "host" pointers are
+ *     ordinary process memory. Which one a parameter takes is stated per parameter.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream). Calls
+ *     that take a stream are asynchronous on it and never synchronise the host, except where
+ *     a HOST output buffer is written (stated per call). Calls without a stream synchronise.
+ *   - Ownership: the library owns the brick store and its per-view scratch (rectangles,
+ *     visibility order, work list, sub-images). The caller owns every buffer it passes in;
+ *     inputs are read (or copied) before the call's work completes on `stream`, outputs are
+ *     written by it.
+ *   - Geometry: world units are voxels. The volume occupies [0,nx] x [0,ny] x [0,nz]; voxel
+ *     (i,j,k) is centred at (i+1/2, j+1/2, k+1/2) (R3). Cube memory layout is [nz][ny][nx]
+ *     float32, x fastest, z = spectral axis.
+ *   - Matrices: column-major float[16], OpenGL clip conventions, clip = proj * view * world,
+ *     clip z in [-1,1] (sec. 2.3.2 "the OpenGL projection and transformation
+ *     matrices"; R1). Image: [height][width][4] float32 RGBA, row 0 = bottom row, pixel
+ *     centres at half-integers.
+ *
+ * There is no CPU fallback: every call needs a CUDA device and fails with VR_ERR_CUDA
+ * without one.
+ */
+#ifndef VR_H
+#define VR_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum vr_status {
+    VR_OK = 0,
+    VR_ERR_INVALID_ARG = 1,   /* bad sizes, NULL pointers, step <= 0, singular proj*view ... */
+    VR_ERR_OUT_OF_MEMORY = 2, /* a device (or staging) allocation failed */
+    VR_ERR_CUDA = 3,          /* a CUDA call or kernel launch failed; see vr_last_error */
+    VR_ERR_STATE = 4          /* call order: no transfer function set, no data uploaded ... */
+} vr_status;
+
+enum { VR_ALPHA = 0, VR_MIP = 1 };   /* vr_render mode */
+enum { VR_HOST = 0, VR_DEVICE = 1 }; /* memory space of a data pointer */
+
+typedef struct vr_volume vr_volume; /* opaque */
+
+/* Counters of the most recent vr_render on a handle (vr_debug_stats). */
+typedef struct vr_stats {
+    int64_t samples;        /* tri-linear samples taken (after early termination); valid only
+                               if counting was enabled with vr_set_counting, else -1 */
+    int64_t rays;           /* (brick, pixel) rays started = sum of launch-rectangle areas */
+    int64_t work_items;     /* (brick, 8x4-pixel tile) work items of the ray-cast kernel */
+    int64_t subimage_bytes; /* bytes of brick sub-images written by the ray-cast kernel */
+    int32_t nbricks;
+    int32_t overflow;       /* 1 if the view needed more sub-image scratch than was reserved
+                               (frame is then incomplete; never happens unless the host and
+                               device rectangle computations disagree) */
+    float ms_setup;         /* per-stage device times of the last render, from CUDA events  */
+    float ms_raycast;       /*   recorded on the render's stream; valid only if timing was   */
+    float ms_composite;     /*   enabled with vr_set_timing, else -1                         */
+} vr_stats;
+
+/* ------------------------------------------------------------------------------------------
+ * Brick store.
+ * PAPER.md:105,113 (sec. 2.1: the cube is split into sub-cubes, each rendered independently at
+ * full output resolution), :136 (sec. 2.3.1 partitioning), :146 (data moved to GPU memory).
+ * Ghost voxels are not in the paper; R3: each brick carries `ghost` extra voxels per side,
+ * edge-replicated at the volume boundary, so that tri-linear sampling is seam-free; ghost = 1
+ * is exactly sufficient.
+ * ---------------------------------------------------------------------------------------- */
+
+/* Create a volume of nx*ny*nz float32 voxels split into a regular grid of brick^3 cores
+ * (ceil(n/brick) per axis, ragged at the high edges). Allocates grid-many padded bricks of
+ * (brick+2*ghost)^3 floats in device memory, zero-filled.
+ *   nx,ny,nz > 0; brick >= 2; 0 <= ghost <= 8 (ghost = 0 is allowed: seams are then expected).
+ *   out (host): receives the handle. Errors: VR_ERR_INVALID_ARG, VR_ERR_OUT_OF_MEMORY,
+ *   VR_ERR_CUDA (no device). On error *out = NULL. */
+int vr_volume_create(int nx, int ny, int nz, int brick, int ghost, vr_volume** out);
+
+/* Free everything the library allocated for the handle (synchronises the device). NULL ok. */
+void vr_volume_destroy(vr_volume* v);
+
+/* Copy a dense box of the cube into the brick store. `src` is a dense [sz][sy][sx] float32
+ * array (x fastest) holding the voxels of the box with origin (x0,y0,z0); memspace says
+ * whether src is a VR_HOST or VR_DEVICE pointer. Every brick cell (core AND ghost, including
+ * the edge-replicated cells outside the volume) whose clamped global voxel index lies in the
+ * box is written. A whole-cube upload is (0,0,0,nx,ny,nz); z-slab uploads make the ~100 GB
+ * case feasible without a second full copy.
+ *   VR_DEVICE: asynchronous on `stream`; src must stay valid until that work completes.
+ *   VR_HOST: staged through a bounded device buffer; returns after the copy has completed.
+ * Errors: VR_ERR_INVALID_ARG (NULL, box outside the volume, empty box). */
+int vr_volume_upload(vr_volume* v, const float* src, int memspace, int x0, int y0, int z0,
+                     int sx, int sy, int sz, void* stream);
+
+/* Test-only inverse of vr_volume_upload: reads the CORE cells of the bricks back into a dense
+ * [sz][sy][sx] box (dst: VR_HOST or VR_DEVICE). Round trip is bit-exact. VR_HOST synchronises. */
+int vr_volume_download(vr_volume* v, float* dst, int memspace, int x0, int y0, int z0,
+                       int sx, int sy, int sz, void* stream);
+
+/* Test-only: copy the padded cells of brick b, as a dense [dz][dy][dx] box with
+ * d = (core extent + 2*ghost) per axis, to dst (host). dims (host int[3]) receives dx,dy,dz.
+ * dst may be NULL to query dims only. Synchronises. */
+int vr_debug_brick_data(vr_volume* v, int b, float* dst, int* dims);
+
+/* ------------------------------------------------------------------------------------------
+ * Classification (row a6). PAPER.md:45 (sec. 1.2: the transfer function maps a data value to
+ * colour and opacity), :172 (final colour mapping with the user's colour map). R7: n-entry
+ * straight-alpha RGBA table over [vmin,vmax], values clamped, linear interpolation between
+ * entries at x = u*(n-1); the table's alpha is the opacity of one voxel of path length, a
+ * sample standing for a path of length w has opacity 1-(1-a)^w.
+ *   rgba (host): n*4 floats, copied. 2 <= n <= 1024; vmax > vmin. Synchronises the device
+ *   (so that a render in flight is not disturbed). */
+int vr_set_transfer_function(vr_volume* v, const float* rgba, int n, float vmin, float vmax);
+
+/* Early ray termination threshold tau (row a7; "... or opacity is achieved").
+ * R8: a brick's ray stops, before taking a sample, once the brick-local accumulated opacity
+ * is >= tau. Default 0.99; tau > 1 disables early termination. */
+int vr_set_early_termination(vr_volume* v, float tau);
+
+/* ------------------------------------------------------------------------------------------
+ * One frame (rows a2..a9): per-view set-up (inverse of proj*view, rendering rectangle of each
+ * brick = screen bounding box of its 8 projected vertices, Fig. 4 :168),
+ * device-side visibility order of the bricks (PAPER.md:53 names depth sorting; R9), per-brick
+ * ray casting (sec. 2.3.2: ray start, direction, intersection with the bounding
+ * cube, early exit for rays that miss, march to the exit point or until the opacity / the
+ * maximum is reached; tri-linear interpolation :69,:150), then sort-last compositing of the
+ * brick sub-images in visibility order (sec. 2.3.3: `over` is associative;
+ * MIP composites in any order) and, for MIP, the final colour mapping (:172).
+ *   view, proj (host): float[16] each, read before the call returns.
+ *   width,height > 0; step > 0 (voxels); mode VR_ALPHA or VR_MIP.
+ *   out_rgba (device): [height][width][4] float32. VR_ALPHA: premultiplied colour and opacity
+ *   on a transparent black background. VR_MIP: LUT colour of the ray's maximum with alpha 1,
+ *   or (0,0,0,0) if the ray took no sample (R11).
+ * Asynchronous on `stream`; all stages run on the device, the host only validates arguments
+ * and sizes scratch memory (growing the scratch for a larger view than any seen before
+ * allocates, which may synchronise; steady-state frames do not).
+ * Errors: VR_ERR_INVALID_ARG (also: proj*view singular), VR_ERR_STATE (no transfer function
+ * or nothing uploaded), VR_ERR_OUT_OF_MEMORY, VR_ERR_CUDA. */
+int vr_render(vr_volume* v, const float* view, const float* proj, int width, int height,
+              float step, int mode, float* out_rgba, void* stream);
+
+/* Same frame, delivered to HOST memory: renders into a library-owned device frame, copies it
+ * to out_rgba_host ([height][width][4] float32; pinned memory makes the copy asynchronous
+ * with respect to other streams) and waits for the copy. This is the end-to-end entry. */
+int vr_render_host(vr_volume* v, const float* view, const float* proj, int width, int height,
+                   float step, int mode, float* out_rgba_host, void* stream);
+
+/* ------------------------------------------------------------------------------------------
+ * Stand-alone sort-last compositing (row a9; the 64-layer microbenchmark). PAPER.md:114
+ * (compositing is the bottleneck of distributed image-order rendering), :170-174.
+ *   layers (host array of n DEVICE pointers): layer l is a premultiplied RGBA float32
+ *   sub-image covering rects[l], stored [y1-y0][x1-x0][4].
+ *   rects (host): n * (x0,y0,x1,y1), half-open, inside the width x height viewport.
+ *   order (host): n layer indices, front to back.
+ *   out (device): [height][width][4]; pixels no layer covers become (0,0,0,0).
+ * Front-to-back `over`: C += (1-A)*C_l, A += (1-A)*A_l, float32 (R15). Asynchronous on
+ * `stream` after copying the small tables (n <= 4096). */
+int vr_composite(const float* const* layers, const int* rects, const int* order, int n,
+                 int width, int height, float* out, void* stream);
+
+/* ------------------------------------------------------------------------------------------
+ * Debug / test exports. All synchronise and write HOST memory.
+ * ---------------------------------------------------------------------------------------- */
+
+int vr_num_bricks(const vr_volume* v);
+
+/* Front-to-back permutation of the bricks for this view, as computed by the device set-up
+ * kernel (R9). order_out: host int[nbricks]. Brick index b = (bz*gy + by)*gx + bx. */
+int vr_debug_brick_order(vr_volume* v, const float* view, const float* proj, int* order_out);
+
+/* Rendering rectangle (x0,y0,x1,y1), half-open and clipped to the viewport, of every brick,
+ * as computed by the device set-up kernel. rects_out: host int[nbricks*4]. */
+int vr_debug_rects(vr_volume* v, const float* view, const float* proj, int width, int height,
+                   int* rects_out);
+
+/* Per listed pixel (pixels: host int[npix*2] = (i,j) pairs), the bricks whose core box
+ * overlaps the ray's clipped segment with positive length, by increasing entry distance
+ * (R10). counts: host int[npix]; lists: host int[npix*maxlen] (entries beyond the count are
+ * -1); grazing: host uint8[npix] or NULL, 1 where some hit/miss decision had a margin below
+ * 1e-9 voxel (such rays are excluded from exact comparison). */
+int vr_debug_ray_bricks(vr_volume* v, const float* view, const float* proj, int width,
+                        int height, const int* pixels, int npix, int* counts, int* lists,
+                        int maxlen, uint8_t* grazing);
+
+/* Per listed pixel, the sub-image value each brick produced in the most recent vr_render on
+ * this handle with the same width/height (test access to row a8). sub_out: host
+ * float[npix*nbricks*4]: VR_ALPHA premultiplied RGBA; VR_MIP (max, 0, 0, 0) with max = -inf
+ * for "no sample". Bricks whose rectangle does not contain the pixel give zeros / -inf. */
+int vr_debug_subimages(vr_volume* v, const int* pixels, int npix, float* sub_out);
+
+/* Enable (1) / disable (0) counting of samples in the ray-cast kernel (an instrumented
+ * variant of the same kernel: slower, never used for timed runs). */
+int vr_set_counting(vr_volume* v, int enable);
+
+/* Enable (1) / disable (0) CUDA-event timing of the three stages on the render's stream. */
+int vr_set_timing(vr_volume* v, int enable);
+
+/* Counters (and stage times) of the most recent vr_render. Synchronises. */
+int vr_debug_stats(vr_volume* v, vr_stats* out);
+
+/* Number of kernel launches the library has issued on this handle since creation. */
+int64_t vr_launch_count(const vr_volume* v);
+
+/* Message for the last error on the handle (or the last handle-less error if v is NULL).
+ * Never NULL; valid until the next call on the same handle. */
+const char* vr_last_error(const vr_volume* v);
+
+#ifdef __cplusplus
+}
+#endif
+
+#endif /* VR_H */

@@ -1,0 +1,252 @@
+"""paper_1205_0282_b200 -- thin Python binding of libvr (include/vr.h).
+
+Argument marshalling only: every step of the path (brick store, view set-up, visibility sort,
+ray casting, compositing) runs in the CUDA kernels behind the C ABI. PyTorch is used for device
+memory (the caller's tensors) and streams. There is no CPU fallback: a missing library or a
+missing CUDA device raises.
+
+Names follow include/vr.h: Volume.upload / download / set_transfer_function /
+set_early_termination / render / render_host, composite(), and the debug exports.
+"""
+import ctypes
+import os
+
+import numpy as np
+
+ALPHA, MIP = 0, 1
+HOST, DEVICE = 0, 1
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libvr.so")
+
+STATUS = {0: "VR_OK", 1: "VR_ERR_INVALID_ARG", 2: "VR_ERR_OUT_OF_MEMORY", 3: "VR_ERR_CUDA", 4: "VR_ERR_STATE"}
+
+# every symbol include/vr.h declares (tests check the library exports each of them)
+SYMBOLS = (
+    "vr_volume_create", "vr_volume_destroy", "vr_volume_upload", "vr_volume_download", "vr_debug_brick_data",
+    "vr_set_transfer_function", "vr_set_early_termination", "vr_render", "vr_render_host", "vr_composite",
+    "vr_num_bricks", "vr_debug_brick_order", "vr_debug_rects", "vr_debug_ray_bricks", "vr_debug_subimages",
+    "vr_set_counting", "vr_set_timing", "vr_debug_stats", "vr_launch_count", "vr_last_error",
+)
+
+
+class VrError(RuntimeError):
+    def __init__(self, status, message):
+        super().__init__("%s: %s" % (STATUS.get(status, status), message))
+        self.status = status
+
+
+class Stats(ctypes.Structure):
+    _fields_ = [("samples", ctypes.c_int64), ("rays", ctypes.c_int64), ("work_items", ctypes.c_int64),
+                ("subimage_bytes", ctypes.c_int64), ("nbricks", ctypes.c_int32), ("overflow", ctypes.c_int32),
+                ("ms_setup", ctypes.c_float), ("ms_raycast", ctypes.c_float), ("ms_composite", ctypes.c_float)]
+
+
+_lib = None
+
+
+def lib():
+    """Load libvr.so (built in-tree by paper_1205_0282_b200.build). Fails loudly if absent."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError("libvr.so is not built: run `python -m paper_1205_0282_b200.build` "
+                              "(there is no CPU fallback)")
+        L = ctypes.CDLL(LIB_PATH)
+        vp, ci, cf, i64 = ctypes.c_void_p, ctypes.c_int, ctypes.c_float, ctypes.c_int64
+        L.vr_volume_create.argtypes = [ci, ci, ci, ci, ci, ctypes.POINTER(vp)]
+        L.vr_volume_destroy.argtypes = [vp]
+        L.vr_volume_destroy.restype = None
+        L.vr_volume_upload.argtypes = [vp, vp, ci, ci, ci, ci, ci, ci, ci, vp]
+        L.vr_volume_download.argtypes = [vp, vp, ci, ci, ci, ci, ci, ci, ci, vp]
+        L.vr_debug_brick_data.argtypes = [vp, ci, vp, vp]
+        L.vr_set_transfer_function.argtypes = [vp, vp, ci, cf, cf]
+        L.vr_set_early_termination.argtypes = [vp, cf]
+        L.vr_render.argtypes = [vp, vp, vp, ci, ci, cf, ci, vp, vp]
+        L.vr_render_host.argtypes = [vp, vp, vp, ci, ci, cf, ci, vp, vp]
+        L.vr_composite.argtypes = [vp, vp, vp, ci, ci, ci, vp, vp]
+        L.vr_num_bricks.argtypes = [vp]
+        L.vr_debug_brick_order.argtypes = [vp, vp, vp, vp]
+        L.vr_debug_rects.argtypes = [vp, vp, vp, ci, ci, vp]
+        L.vr_debug_ray_bricks.argtypes = [vp, vp, vp, ci, ci, vp, ci, vp, vp, ci, vp]
+        L.vr_debug_subimages.argtypes = [vp, vp, ci, vp]
+        L.vr_set_counting.argtypes = [vp, ci]
+        L.vr_set_timing.argtypes = [vp, ci]
+        L.vr_debug_stats.argtypes = [vp, ctypes.POINTER(Stats)]
+        L.vr_launch_count.argtypes = [vp]
+        L.vr_launch_count.restype = i64
+        L.vr_last_error.argtypes = [vp]
+        L.vr_last_error.restype = ctypes.c_char_p
+        _lib = L
+    return _lib
+
+
+def _mat(m):
+    return np.ascontiguousarray(np.asarray(m, dtype=np.float32).reshape(16))
+
+
+def _stream(stream):
+    if stream is None:
+        import torch
+        return ctypes.c_void_p(torch.cuda.current_stream().cuda_stream)
+    return ctypes.c_void_p(int(stream))
+
+
+def _pixels(pixels):
+    return np.ascontiguousarray(pixels, dtype=np.int32).reshape(-1, 2)
+
+
+class Volume:
+    """Handle of a bricked volume in HBM (vr_volume_create ... vr_volume_destroy)."""
+
+    def __init__(self, nx, ny, nz, brick, ghost=1):
+        self._h = ctypes.c_void_p()
+        self.nx, self.ny, self.nz, self.brick, self.ghost = int(nx), int(ny), int(nz), int(brick), int(ghost)
+        rc = lib().vr_volume_create(self.nx, self.ny, self.nz, self.brick, self.ghost, ctypes.byref(self._h))
+        if rc != 0:
+            self._h = ctypes.c_void_p()
+            raise VrError(rc, lib().vr_last_error(None).decode())
+        self.nbricks = lib().vr_num_bricks(self._h)
+
+    def close(self):
+        if getattr(self, "_h", None) is not None and self._h.value:
+            lib().vr_volume_destroy(self._h)
+            self._h = ctypes.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _check(self, rc):
+        if rc != 0:
+            raise VrError(rc, lib().vr_last_error(self._h).decode())
+
+    # -- brick store (a1) ---------------------------------------------------
+    def _box(self, shape, origin):
+        sz, sy, sx = (int(s) for s in shape)
+        x0, y0, z0 = (int(o) for o in origin)
+        return x0, y0, z0, sx, sy, sz
+
+    def upload(self, data, origin=(0, 0, 0), stream=None):
+        """data: float32 [sz][sy][sx] numpy array (host) or CUDA torch tensor (device)."""
+        if isinstance(data, np.ndarray):
+            d = np.ascontiguousarray(data, dtype=np.float32)
+            assert d.ndim == 3
+            self._check(lib().vr_volume_upload(self._h, d.ctypes.data, HOST, *self._box(d.shape, origin), _stream(stream)))
+        else:
+            assert data.is_cuda and data.is_contiguous() and data.dtype.is_floating_point and data.element_size() == 4
+            assert data.dim() == 3
+            self._check(lib().vr_volume_upload(self._h, data.data_ptr(), DEVICE, *self._box(data.shape, origin), _stream(stream)))
+
+    def download(self, out, origin=(0, 0, 0), stream=None):
+        if isinstance(out, np.ndarray):
+            assert out.dtype == np.float32 and out.flags.c_contiguous and out.ndim == 3
+            self._check(lib().vr_volume_download(self._h, out.ctypes.data, HOST, *self._box(out.shape, origin), _stream(stream)))
+        else:
+            assert out.is_cuda and out.is_contiguous() and out.element_size() == 4 and out.dim() == 3
+            self._check(lib().vr_volume_download(self._h, out.data_ptr(), DEVICE, *self._box(out.shape, origin), _stream(stream)))
+        return out
+
+    def debug_brick_data(self, b):
+        dims = (ctypes.c_int * 3)()
+        self._check(lib().vr_debug_brick_data(self._h, int(b), None, dims))
+        out = np.empty((dims[2], dims[1], dims[0]), dtype=np.float32)
+        self._check(lib().vr_debug_brick_data(self._h, int(b), out.ctypes.data, dims))
+        return out
+
+    # -- classification (a6), termination (a7) --------------------------------
+    def set_transfer_function(self, rgba, vmin, vmax):
+        t = np.ascontiguousarray(rgba, dtype=np.float32)
+        assert t.ndim == 2 and t.shape[1] == 4
+        self._check(lib().vr_set_transfer_function(self._h, t.ctypes.data, t.shape[0], float(vmin), float(vmax)))
+
+    def set_early_termination(self, tau):
+        self._check(lib().vr_set_early_termination(self._h, float(tau)))
+
+    # -- one frame (a2..a9) ---------------------------------------------------
+    def render(self, view, proj, width, height, step, mode, out, stream=None):
+        """out: CUDA float32 tensor [height][width][4]; asynchronous on the stream."""
+        assert out.is_cuda and out.is_contiguous() and out.element_size() == 4 and out.numel() == width * height * 4
+        v, p = _mat(view), _mat(proj)
+        self._check(lib().vr_render(self._h, v.ctypes.data, p.ctypes.data, int(width), int(height), float(step), int(mode),
+                                    out.data_ptr(), _stream(stream)))
+        return out
+
+    def render_host(self, view, proj, width, height, step, mode, out=None, stream=None):
+        """out: float32 numpy array or pinned CPU tensor [height][width][4]; returns when filled."""
+        v, p = _mat(view), _mat(proj)
+        if out is None:
+            out = np.empty((height, width, 4), dtype=np.float32)
+        if isinstance(out, np.ndarray):
+            assert out.dtype == np.float32 and out.flags.c_contiguous and out.size == width * height * 4
+            ptr = out.ctypes.data
+        else:
+            assert (not out.is_cuda) and out.is_contiguous() and out.element_size() == 4 and out.numel() == width * height * 4
+            ptr = out.data_ptr()
+        self._check(lib().vr_render_host(self._h, v.ctypes.data, p.ctypes.data, int(width), int(height), float(step),
+                                         int(mode), ptr, _stream(stream)))
+        return out
+
+    # -- debug / test exports ---------------------------------------------------
+    def debug_brick_order(self, view, proj):
+        v, p = _mat(view), _mat(proj)
+        o = np.empty(self.nbricks, dtype=np.int32)
+        self._check(lib().vr_debug_brick_order(self._h, v.ctypes.data, p.ctypes.data, o.ctypes.data))
+        return o
+
+    def debug_rects(self, view, proj, width, height):
+        v, p = _mat(view), _mat(proj)
+        r = np.empty((self.nbricks, 4), dtype=np.int32)
+        self._check(lib().vr_debug_rects(self._h, v.ctypes.data, p.ctypes.data, int(width), int(height), r.ctypes.data))
+        return r
+
+    def debug_ray_bricks(self, view, proj, width, height, pixels, maxlen=64):
+        v, p = _mat(view), _mat(proj)
+        pix = _pixels(pixels)
+        n = pix.shape[0]
+        counts = np.zeros(n, dtype=np.int32)
+        lists = np.full((n, maxlen), -1, dtype=np.int32)
+        graz = np.zeros(n, dtype=np.uint8)
+        self._check(lib().vr_debug_ray_bricks(self._h, v.ctypes.data, p.ctypes.data, int(width), int(height), pix.ctypes.data,
+                                              n, counts.ctypes.data, lists.ctypes.data, int(maxlen), graz.ctypes.data))
+        return counts, lists, graz
+
+    def debug_subimages(self, pixels):
+        pix = _pixels(pixels)
+        out = np.empty((pix.shape[0], self.nbricks, 4), dtype=np.float32)
+        self._check(lib().vr_debug_subimages(self._h, pix.ctypes.data, pix.shape[0], out.ctypes.data))
+        return out
+
+    def set_counting(self, enable):
+        self._check(lib().vr_set_counting(self._h, int(bool(enable))))
+
+    def set_timing(self, enable):
+        self._check(lib().vr_set_timing(self._h, int(bool(enable))))
+
+    def debug_stats(self):
+        s = Stats()
+        self._check(lib().vr_debug_stats(self._h, ctypes.byref(s)))
+        return {k: getattr(s, k) for k, _ in Stats._fields_}
+
+    def launch_count(self):
+        return int(lib().vr_launch_count(self._h))
+
+
+def composite(layers, rects, order, width, height, out, stream=None):
+    """Stand-alone sort-last compositing (vr_composite). layers: CUDA float32 tensors
+    [y1-y0][x1-x0][4] (premultiplied); rects: n x (x0,y0,x1,y1); order: front-to-back indices;
+    out: CUDA float32 tensor [height][width][4]."""
+    n = len(layers)
+    ptrs = (ctypes.c_void_p * max(n, 1))(*[l.data_ptr() for l in layers])
+    r = np.ascontiguousarray(rects, dtype=np.int32).reshape(n, 4)
+    o = np.ascontiguousarray(order, dtype=np.int32).reshape(n)
+    for l, rc_ in zip(layers, r):
+        assert l.is_cuda and l.is_contiguous() and l.element_size() == 4
+        assert l.numel() == (rc_[2] - rc_[0]) * (rc_[3] - rc_[1]) * 4
+    assert out.is_cuda and out.is_contiguous() and out.numel() == width * height * 4
+    rc = lib().vr_composite(ptrs, r.ctypes.data, o.ctypes.data, n, int(width), int(height), out.data_ptr(), _stream(stream))
+    if rc != 0:
+        raise VrError(rc, lib().vr_last_error(None).decode())
+    return out

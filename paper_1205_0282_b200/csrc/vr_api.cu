@@ -1,0 +1,612 @@
+/*
+ * vr_api.cu -- the C ABI of libvr (include/vr.h): argument validation, device-memory
+ * ownership, scratch sizing and kernel sequencing. No arithmetic of the method lives here;
+ * every step of the path runs in the kernels of vr_bricks.cu, vr_setup.cu, vr_raycast.cu and
+ * vr_composite.cu. There is no CPU fallback: without a CUDA device every call fails.
+ */
+#include <math.h>
+#include <stdarg.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <new>
+
+#include "vr_internal.cuh"
+
+struct vr_volume {
+    VrGrid grid;
+    float* bricks;           /* nbricks * slot floats */
+    bool has_data, has_tf;
+    float4* d_lut_base;      /* VR_MAX_LUT entries each */
+    float4* d_lut_delta;
+    VrLut lut;
+    float tau;
+    /* per-view scratch, written by the set-up kernel */
+    VrViewState* d_vs;
+    VrBrickView* d_bv;
+    int* d_order;
+    int* d_item_prefix;
+    VrCompLayer* d_layers;
+    void* d_sub;             /* sub-image scratch, sub_capacity_px * 16 bytes */
+    long long sub_capacity_px;
+    float* d_frame;          /* vr_render_host's device frame */
+    long long frame_capacity_px;
+    float* d_stage;          /* staging for VR_HOST upload / download */
+    long long stage_floats;
+    int ctas;                /* persistent grid of the ray-cast kernel */
+    bool counting, timing;
+    cudaEvent_t ev[4];
+    bool ev_valid;           /* the four events were recorded by the last render */
+    int last_W, last_H, last_mode;
+    bool last_valid;
+    int64_t launches;
+    char err[512];
+};
+
+static char g_err[512] = "no error";
+
+static int fail(vr_volume* v, int status, const char* fmt, ...) {
+    char* dst = v ? v->err : g_err;
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(dst, 512, fmt, ap);
+    va_end(ap);
+    return status;
+}
+
+#define VR_CUDA(v, call)                                                                                  \
+    do {                                                                                                  \
+        cudaError_t e_ = (call);                                                                          \
+        if (e_ != cudaSuccess) {                                                                          \
+            cudaGetLastError();                                                                           \
+            return fail((v), e_ == cudaErrorMemoryAllocation ? VR_ERR_OUT_OF_MEMORY : VR_ERR_CUDA,        \
+                        "%s failed: %s", #call, cudaGetErrorString(e_));                                  \
+        }                                                                                                 \
+    } while (0)
+
+extern "C" const char* vr_last_error(const vr_volume* v) { return v ? v->err : g_err; }
+
+extern "C" int vr_num_bricks(const vr_volume* v) { return v ? v->grid.nbricks : 0; }
+
+extern "C" int64_t vr_launch_count(const vr_volume* v) { return v ? v->launches : 0; }
+
+static void release(vr_volume* v) {
+    cudaFree(v->bricks);
+    cudaFree(v->d_lut_base);
+    cudaFree(v->d_lut_delta);
+    cudaFree(v->d_vs);
+    cudaFree(v->d_bv);
+    cudaFree(v->d_order);
+    cudaFree(v->d_item_prefix);
+    cudaFree(v->d_layers);
+    cudaFree(v->d_sub);
+    cudaFree(v->d_frame);
+    cudaFree(v->d_stage);
+    for (int i = 0; i < 4; ++i)
+        if (v->ev[i]) cudaEventDestroy(v->ev[i]);
+    cudaGetLastError();
+    delete v;
+}
+
+extern "C" void vr_volume_destroy(vr_volume* v) {
+    if (!v) return;
+    cudaDeviceSynchronize();
+    release(v);
+}
+
+extern "C" int vr_volume_create(int nx, int ny, int nz, int brick, int ghost, vr_volume** out) {
+    if (!out) return fail(NULL, VR_ERR_INVALID_ARG, "vr_volume_create: out is NULL");
+    *out = NULL;
+    if (nx <= 0 || ny <= 0 || nz <= 0) return fail(NULL, VR_ERR_INVALID_ARG, "vr_volume_create: non-positive size %dx%dx%d", nx, ny, nz);
+    if (brick < 2) return fail(NULL, VR_ERR_INVALID_ARG, "vr_volume_create: brick %d < 2", brick);
+    if (ghost < 0 || ghost > 8) return fail(NULL, VR_ERR_INVALID_ARG, "vr_volume_create: ghost %d outside [0,8]", ghost);
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
+        cudaGetLastError();
+        return fail(NULL, VR_ERR_CUDA, "vr_volume_create: no CUDA device (libvr has no CPU path)");
+    }
+    vr_volume* v = new (std::nothrow) vr_volume();
+    if (!v) return fail(NULL, VR_ERR_OUT_OF_MEMORY, "vr_volume_create: host allocation failed");
+    memset(v, 0, sizeof(*v));
+    snprintf(v->err, sizeof(v->err), "no error");
+    VrGrid& g = v->grid;
+    g.n[0] = nx; g.n[1] = ny; g.n[2] = nz;
+    g.brick = brick; g.ghost = ghost;
+    long long nb = 1;
+    for (int a = 0; a < 3; ++a) {
+        g.g[a] = (g.n[a] + brick - 1) / brick;
+        nb *= g.g[a];
+        if (g.g[a] > VR_MAX_AXIS_BRICKS) {
+            delete v;
+            return fail(NULL, VR_ERR_INVALID_ARG, "vr_volume_create: more than %d bricks along an axis", VR_MAX_AXIS_BRICKS);
+        }
+    }
+    if (nb > 65535) {
+        delete v;
+        return fail(NULL, VR_ERR_INVALID_ARG, "vr_volume_create: %lld bricks > 65535", nb);
+    }
+    g.nbricks = (int)nb;
+    /* a volume smaller than one brick needs no larger slot than itself */
+    int core = brick;
+    {
+        int m = nx > ny ? nx : ny;
+        m = m > nz ? m : nz;
+        if (m < core) core = m;
+    }
+    g.P = core + 2 * ghost;
+    g.slot = (long long)g.P * g.P * g.P;
+    g.brick_pow2 = (brick & (brick - 1)) == 0;
+    v->tau = 0.99f;
+
+    cudaError_t e = cudaMalloc(&v->bricks, (size_t)g.slot * (size_t)g.nbricks * sizeof(float));
+    if (e == cudaSuccess) e = cudaMemset(v->bricks, 0, (size_t)g.slot * (size_t)g.nbricks * sizeof(float));
+    if (e == cudaSuccess) e = cudaMalloc(&v->d_lut_base, VR_MAX_LUT * sizeof(float4));
+    if (e == cudaSuccess) e = cudaMalloc(&v->d_lut_delta, VR_MAX_LUT * sizeof(float4));
+    if (e == cudaSuccess) e = cudaMalloc(&v->d_vs, sizeof(VrViewState));
+    if (e == cudaSuccess) e = cudaMemset(v->d_vs, 0, sizeof(VrViewState));
+    if (e == cudaSuccess) e = cudaMalloc(&v->d_bv, sizeof(VrBrickView) * g.nbricks);
+    if (e == cudaSuccess) e = cudaMalloc(&v->d_order, sizeof(int) * g.nbricks);
+    if (e == cudaSuccess) e = cudaMalloc(&v->d_item_prefix, sizeof(int) * (g.nbricks + 1));
+    if (e == cudaSuccess) e = cudaMalloc(&v->d_layers, sizeof(VrCompLayer) * g.nbricks);
+    for (int i = 0; i < 4 && e == cudaSuccess; ++i) e = cudaEventCreate(&v->ev[i]);
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        const int st = (e == cudaErrorMemoryAllocation) ? VR_ERR_OUT_OF_MEMORY : VR_ERR_CUDA;
+        fail(NULL, st, "vr_volume_create: %s (brick store needs %.2f GB)", cudaGetErrorString(e),
+             (double)g.slot * g.nbricks * 4.0 / 1e9);
+        release(v);
+        return st;
+    }
+    v->ctas = vr_raycast_ctas();
+    if (v->ctas <= 0) {
+        release(v);
+        return fail(NULL, VR_ERR_CUDA, "vr_volume_create: cannot size the ray-cast grid (kernel image not loadable on this device?)");
+    }
+    *out = v;
+    return VR_OK;
+}
+
+static int check_box(vr_volume* v, const char* who, const void* p, int memspace, int x0, int y0, int z0, int sx, int sy, int sz) {
+    if (!v) return fail(NULL, VR_ERR_INVALID_ARG, "%s: NULL handle", who);
+    if (!p) return fail(v, VR_ERR_INVALID_ARG, "%s: NULL data pointer", who);
+    if (memspace != VR_HOST && memspace != VR_DEVICE) return fail(v, VR_ERR_INVALID_ARG, "%s: bad memspace %d", who, memspace);
+    if (sx <= 0 || sy <= 0 || sz <= 0) return fail(v, VR_ERR_INVALID_ARG, "%s: empty box %dx%dx%d", who, sx, sy, sz);
+    const VrGrid& g = v->grid;
+    if (x0 < 0 || y0 < 0 || z0 < 0 || (long long)x0 + sx > g.n[0] || (long long)y0 + sy > g.n[1] || (long long)z0 + sz > g.n[2])
+        return fail(v, VR_ERR_INVALID_ARG, "%s: box (%d,%d,%d)+(%d,%d,%d) outside the %dx%dx%d volume", who, x0, y0, z0, sx, sy,
+                    sz, g.n[0], g.n[1], g.n[2]);
+    return VR_OK;
+}
+
+/* planes of an [sy][sx] box per staging chunk: at most 256 MiB, at least one plane */
+static int ensure_stage(vr_volume* v, int sx, int sy, int sz, int* planes) {
+    const long long plane = (long long)sx * sy;
+    long long n = (64ll << 20) / plane;
+    if (n < 1) n = 1;
+    if (n > sz) n = sz;
+    if (v->stage_floats < n * plane) {
+        if (v->d_stage) {
+            cudaDeviceSynchronize();
+            cudaFree(v->d_stage);
+            v->d_stage = NULL;
+            v->stage_floats = 0;
+        }
+        VR_CUDA(v, cudaMalloc(&v->d_stage, (size_t)(n * plane) * sizeof(float)));
+        v->stage_floats = n * plane;
+    }
+    *planes = (int)n;
+    return VR_OK;
+}
+
+extern "C" int vr_volume_upload(vr_volume* v, const float* src, int memspace, int x0, int y0, int z0, int sx, int sy, int sz,
+                                void* stream) {
+    int rc = check_box(v, "vr_volume_upload", src, memspace, x0, y0, z0, sx, sy, sz);
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    if (memspace == VR_DEVICE) {
+        VR_CUDA(v, vr_launch_upload(v->grid, v->bricks, src, x0, y0, z0, sx, sy, sz, st));
+        v->launches++;
+    } else {
+        int planes = 0;
+        rc = ensure_stage(v, sx, sy, sz, &planes);
+        if (rc) return rc;
+        const long long plane = (long long)sx * sy;
+        for (int k = 0; k < sz; k += planes) {
+            const int nk = (sz - k < planes) ? sz - k : planes;
+            VR_CUDA(v, cudaMemcpyAsync(v->d_stage, src + (long long)k * plane, (size_t)(nk * plane) * sizeof(float),
+                                       cudaMemcpyHostToDevice, st));
+            VR_CUDA(v, vr_launch_upload(v->grid, v->bricks, v->d_stage, x0, y0, z0 + k, sx, sy, nk, st));
+            v->launches++;
+            VR_CUDA(v, cudaStreamSynchronize(st)); /* the staging buffer is reused */
+        }
+    }
+    v->has_data = true;
+    return VR_OK;
+}
+
+extern "C" int vr_volume_download(vr_volume* v, float* dst, int memspace, int x0, int y0, int z0, int sx, int sy, int sz,
+                                  void* stream) {
+    int rc = check_box(v, "vr_volume_download", dst, memspace, x0, y0, z0, sx, sy, sz);
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    if (memspace == VR_DEVICE) {
+        VR_CUDA(v, vr_launch_download(v->grid, v->bricks, dst, x0, y0, z0, sx, sy, sz, st));
+        v->launches++;
+        return VR_OK;
+    }
+    int planes = 0;
+    rc = ensure_stage(v, sx, sy, sz, &planes);
+    if (rc) return rc;
+    const long long plane = (long long)sx * sy;
+    for (int k = 0; k < sz; k += planes) {
+        const int nk = (sz - k < planes) ? sz - k : planes;
+        VR_CUDA(v, vr_launch_download(v->grid, v->bricks, v->d_stage, x0, y0, z0 + k, sx, sy, nk, st));
+        v->launches++;
+        VR_CUDA(v, cudaMemcpyAsync(dst + (long long)k * plane, v->d_stage, (size_t)(nk * plane) * sizeof(float),
+                                   cudaMemcpyDeviceToHost, st));
+        VR_CUDA(v, cudaStreamSynchronize(st));
+    }
+    return VR_OK;
+}
+
+extern "C" int vr_debug_brick_data(vr_volume* v, int b, float* dst, int* dims) {
+    if (!v) return fail(NULL, VR_ERR_INVALID_ARG, "vr_debug_brick_data: NULL handle");
+    const VrGrid& g = v->grid;
+    if (b < 0 || b >= g.nbricks || !dims) return fail(v, VR_ERR_INVALID_ARG, "vr_debug_brick_data: bad brick %d or NULL dims", b);
+    const int bx = b % g.g[0], by = (b / g.g[0]) % g.g[1], bz = b / (g.g[0] * g.g[1]);
+    const int bc[3] = {bx, by, bz};
+    int d[3];
+    for (int a = 0; a < 3; ++a) {
+        const int lo = bc[a] * g.brick;
+        int hi = lo + g.brick;
+        if (hi > g.n[a]) hi = g.n[a];
+        d[a] = hi - lo + 2 * g.ghost;
+        dims[a] = d[a];
+    }
+    if (!dst) return VR_OK;
+    VR_CUDA(v, cudaDeviceSynchronize());
+    /* the brick's cells are the low corner of its P^3 slot: a pitched 3-D copy */
+    cudaMemcpy3DParms p;
+    memset(&p, 0, sizeof(p));
+    p.srcPtr = make_cudaPitchedPtr(v->bricks + (long long)b * g.slot, (size_t)g.P * sizeof(float), (size_t)g.P, (size_t)g.P);
+    p.dstPtr = make_cudaPitchedPtr(dst, (size_t)d[0] * sizeof(float), (size_t)d[0], (size_t)d[1]);
+    p.extent = make_cudaExtent((size_t)d[0] * sizeof(float), (size_t)d[1], (size_t)d[2]);
+    p.kind = cudaMemcpyDeviceToHost;
+    VR_CUDA(v, cudaMemcpy3D(&p));
+    return VR_OK;
+}
+
+/* ------------------------------------------------------------------------------------------ */
+extern "C" int vr_set_transfer_function(vr_volume* v, const float* rgba, int n, float vmin, float vmax) {
+    if (!v) return fail(NULL, VR_ERR_INVALID_ARG, "vr_set_transfer_function: NULL handle");
+    if (!rgba) return fail(v, VR_ERR_INVALID_ARG, "vr_set_transfer_function: NULL table");
+    if (n < 2 || n > VR_MAX_LUT) return fail(v, VR_ERR_INVALID_ARG, "vr_set_transfer_function: n = %d outside [2,%d]", n, VR_MAX_LUT);
+    if (!(vmax > vmin) || !isfinite(vmin) || !isfinite(vmax))
+        return fail(v, VR_ERR_INVALID_ARG, "vr_set_transfer_function: need finite vmin < vmax");
+    for (int i = 0; i < 4 * n; ++i)
+        if (!isfinite(rgba[i])) return fail(v, VR_ERR_INVALID_ARG, "vr_set_transfer_function: entry %d is not finite", i / 4);
+    /* the table is stored as (entry, difference to the next entry) pairs; the differences are
+     * plain float32 subtractions of the caller's entries */
+    static float4 base[VR_MAX_LUT], delta[VR_MAX_LUT];
+    for (int i = 0; i < n; ++i) {
+        base[i] = make_float4(rgba[4 * i], rgba[4 * i + 1], rgba[4 * i + 2], rgba[4 * i + 3]);
+        if (i + 1 < n)
+            delta[i] = make_float4(rgba[4 * i + 4] - rgba[4 * i], rgba[4 * i + 5] - rgba[4 * i + 1],
+                                   rgba[4 * i + 6] - rgba[4 * i + 2], rgba[4 * i + 7] - rgba[4 * i + 3]);
+        else
+            delta[i] = make_float4(0.f, 0.f, 0.f, 0.f);
+    }
+    VR_CUDA(v, cudaDeviceSynchronize());
+    VR_CUDA(v, cudaMemcpy(v->d_lut_base, base, sizeof(float4) * n, cudaMemcpyHostToDevice));
+    VR_CUDA(v, cudaMemcpy(v->d_lut_delta, delta, sizeof(float4) * n, cudaMemcpyHostToDevice));
+    v->lut.base = v->d_lut_base;
+    v->lut.delta = v->d_lut_delta;
+    v->lut.n = n;
+    v->lut.vmin = vmin;
+    v->lut.vmax = vmax;
+    v->lut.inv_range = (float)(1.0 / ((double)vmax - (double)vmin));
+    v->has_tf = true;
+    return VR_OK;
+}
+
+extern "C" int vr_set_early_termination(vr_volume* v, float tau) {
+    if (!v) return fail(NULL, VR_ERR_INVALID_ARG, "vr_set_early_termination: NULL handle");
+    if (!(tau > 0.0f)) return fail(v, VR_ERR_INVALID_ARG, "vr_set_early_termination: tau must be > 0");
+    v->tau = tau;
+    return VR_OK;
+}
+
+extern "C" int vr_set_counting(vr_volume* v, int enable) {
+    if (!v) return fail(NULL, VR_ERR_INVALID_ARG, "vr_set_counting: NULL handle");
+    v->counting = enable != 0;
+    return VR_OK;
+}
+
+extern "C" int vr_set_timing(vr_volume* v, int enable) {
+    if (!v) return fail(NULL, VR_ERR_INVALID_ARG, "vr_set_timing: NULL handle");
+    v->timing = enable != 0;
+    v->ev_valid = false;
+    return VR_OK;
+}
+
+/* ------------------------------------------------------------------------------------------ */
+static int check_view(vr_volume* v, const char* who, const float* view, const float* proj, int W, int H, long long* sub_px,
+                      long long* items) {
+    if (!v) return fail(NULL, VR_ERR_INVALID_ARG, "%s: NULL handle", who);
+    if (!view || !proj) return fail(v, VR_ERR_INVALID_ARG, "%s: NULL matrix", who);
+    if (W <= 0 || H <= 0 || W > 32768 || H > 32768) return fail(v, VR_ERR_INVALID_ARG, "%s: bad frame size %dx%d", who, W, H);
+    for (int i = 0; i < 16; ++i)
+        if (!isfinite(view[i]) || !isfinite(proj[i])) return fail(v, VR_ERR_INVALID_ARG, "%s: matrix entry is not finite", who);
+    if (vr_host_view_check(v->grid, view, proj, W, H, sub_px, items))
+        return fail(v, VR_ERR_INVALID_ARG, "%s: proj*view is singular", who);
+    if (*items > 2000000000ll) return fail(v, VR_ERR_INVALID_ARG, "%s: view needs %lld work items (> 2e9)", who, *items);
+    return VR_OK;
+}
+
+static int ensure_sub(vr_volume* v, long long need_px) {
+    if (need_px <= v->sub_capacity_px) return VR_OK;
+    if (v->d_sub) {
+        VR_CUDA(v, cudaDeviceSynchronize());
+        cudaFree(v->d_sub);
+        v->d_sub = NULL;
+        v->sub_capacity_px = 0;
+    }
+    const long long cap = need_px + need_px / 4 + 4096; /* headroom: neighbouring views fit too */
+    VR_CUDA(v, cudaMalloc(&v->d_sub, (size_t)cap * 16));
+    v->sub_capacity_px = cap;
+    return VR_OK;
+}
+
+static int run_setup(vr_volume* v, const float* view, const float* proj, int W, int H, int mode, cudaStream_t st) {
+    VrMatrices m;
+    memcpy(m.view, view, sizeof(m.view));
+    memcpy(m.proj, proj, sizeof(m.proj));
+    VR_CUDA(v, vr_launch_setup(v->grid, m, W, H, mode, v->sub_capacity_px, v->d_sub, v->d_vs, v->d_bv, v->d_order,
+                               v->d_item_prefix, v->d_layers, st));
+    v->launches++;
+    return VR_OK;
+}
+
+extern "C" int vr_render(vr_volume* v, const float* view, const float* proj, int width, int height, float step, int mode,
+                         float* out_rgba, void* stream) {
+    long long sub_px = 0, items = 0;
+    int rc = check_view(v, "vr_render", view, proj, width, height, &sub_px, &items);
+    if (rc) return rc;
+    if (!out_rgba) return fail(v, VR_ERR_INVALID_ARG, "vr_render: NULL output");
+    if (!(step > 0.0f) || !isfinite(step)) return fail(v, VR_ERR_INVALID_ARG, "vr_render: step must be > 0");
+    if (mode != VR_ALPHA && mode != VR_MIP) return fail(v, VR_ERR_INVALID_ARG, "vr_render: bad mode %d", mode);
+    if (!v->has_tf) return fail(v, VR_ERR_STATE, "vr_render: no transfer function set");
+    if (!v->has_data) return fail(v, VR_ERR_STATE, "vr_render: nothing uploaded");
+    rc = ensure_sub(v, sub_px);
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    const bool timing = v->timing;
+
+    if (timing) VR_CUDA(v, cudaEventRecord(v->ev[0], st));
+    rc = run_setup(v, view, proj, width, height, mode, st);
+    if (rc) return rc;
+    if (timing) VR_CUDA(v, cudaEventRecord(v->ev[1], st));
+
+    VrRaycastParams p;
+    p.grid = v->grid;
+    p.bricks = v->bricks;
+    p.vs = v->d_vs;
+    p.bv = v->d_bv;
+    p.order = v->d_order;
+    p.item_prefix = v->d_item_prefix;
+    p.vs_rw = v->d_vs;
+    p.sub = v->d_sub;
+    p.lut = v->lut;
+    p.step = (double)step;
+    p.tau = v->tau;
+    p.mode = mode;
+    long long ctas = v->ctas;
+    const long long want = (items + (VR_RAYCAST_THREADS / 32) - 1) / (VR_RAYCAST_THREADS / 32);
+    if (ctas > want) ctas = want < 1 ? 1 : want;
+    VR_CUDA(v, vr_launch_raycast(p, (int)ctas, v->counting, st));
+    v->launches++;
+    if (timing) VR_CUDA(v, cudaEventRecord(v->ev[2], st));
+
+    VR_CUDA(v, vr_launch_composite(v->d_layers, v->d_order, v->grid.nbricks, width, height, mode, v->lut, out_rgba, st));
+    v->launches++;
+    if (timing) {
+        VR_CUDA(v, cudaEventRecord(v->ev[3], st));
+        v->ev_valid = true;
+    }
+    v->last_W = width;
+    v->last_H = height;
+    v->last_mode = mode;
+    v->last_valid = true;
+    return VR_OK;
+}
+
+extern "C" int vr_render_host(vr_volume* v, const float* view, const float* proj, int width, int height, float step, int mode,
+                              float* out_rgba_host, void* stream) {
+    if (!v) return fail(NULL, VR_ERR_INVALID_ARG, "vr_render_host: NULL handle");
+    if (!out_rgba_host) return fail(v, VR_ERR_INVALID_ARG, "vr_render_host: NULL output");
+    if (width <= 0 || height <= 0 || width > 32768 || height > 32768)
+        return fail(v, VR_ERR_INVALID_ARG, "vr_render_host: bad frame size %dx%d", width, height);
+    const long long px = (long long)width * height;
+    if (px > v->frame_capacity_px) {
+        if (v->d_frame) {
+            VR_CUDA(v, cudaDeviceSynchronize());
+            cudaFree(v->d_frame);
+            v->d_frame = NULL;
+            v->frame_capacity_px = 0;
+        }
+        VR_CUDA(v, cudaMalloc(&v->d_frame, (size_t)px * 16));
+        v->frame_capacity_px = px;
+    }
+    const int rc = vr_render(v, view, proj, width, height, step, mode, v->d_frame, stream);
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    VR_CUDA(v, cudaMemcpyAsync(out_rgba_host, v->d_frame, (size_t)px * 16, cudaMemcpyDeviceToHost, st));
+    VR_CUDA(v, cudaStreamSynchronize(st));
+    return VR_OK;
+}
+
+/* ------------------------------------------------------------------------------------------ */
+extern "C" int vr_composite(const float* const* layers, const int* rects, const int* order, int n, int width, int height,
+                            float* out, void* stream) {
+    if (!layers || !rects || !order || !out) return fail(NULL, VR_ERR_INVALID_ARG, "vr_composite: NULL argument");
+    if (n < 0 || n > 4096) return fail(NULL, VR_ERR_INVALID_ARG, "vr_composite: n = %d outside [0,4096]", n);
+    if (width <= 0 || height <= 0 || width > 32768 || height > 32768)
+        return fail(NULL, VR_ERR_INVALID_ARG, "vr_composite: bad frame size %dx%d", width, height);
+    static VrCompLayer tab[4096];
+    static unsigned char seen[4096];
+    memset(seen, 0, sizeof(seen));
+    for (int l = 0; l < n; ++l) {
+        const int* r = rects + 4 * l;
+        if (r[0] < 0 || r[1] < 0 || r[2] > width || r[3] > height || r[2] < r[0] || r[3] < r[1])
+            return fail(NULL, VR_ERR_INVALID_ARG, "vr_composite: rectangle %d outside the viewport", l);
+        if (!layers[l] && r[2] > r[0] && r[3] > r[1]) return fail(NULL, VR_ERR_INVALID_ARG, "vr_composite: layer %d is NULL", l);
+        if (order[l] < 0 || order[l] >= n || seen[order[l]]) return fail(NULL, VR_ERR_INVALID_ARG, "vr_composite: order is not a permutation");
+        seen[order[l]] = 1;
+        VrCompLayer& L = tab[l];
+        L.x0 = r[0]; L.y0 = r[1]; L.x1 = r[2]; L.y1 = r[3];
+        L.sx0 = r[0]; L.sy0 = r[1];
+        L.pitch = r[2] - r[0];
+        L.pad = 0;
+        L.addr = (unsigned long long)(uintptr_t)layers[l];
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    VrCompLayer* d_tab = NULL;
+    int* d_order = NULL;
+    const size_t nn = n > 0 ? (size_t)n : 1;
+    VR_CUDA(NULL, cudaMallocAsync(&d_tab, sizeof(VrCompLayer) * nn, st));
+    VR_CUDA(NULL, cudaMallocAsync(&d_order, sizeof(int) * nn, st));
+    if (n > 0) {
+        VR_CUDA(NULL, cudaMemcpyAsync(d_tab, tab, sizeof(VrCompLayer) * n, cudaMemcpyHostToDevice, st));
+        VR_CUDA(NULL, cudaMemcpyAsync(d_order, order, sizeof(int) * n, cudaMemcpyHostToDevice, st));
+    }
+    VrLut none;
+    memset(&none, 0, sizeof(none));
+    VR_CUDA(NULL, vr_launch_composite(d_tab, d_order, n, width, height, VR_ALPHA, none, out, st));
+    VR_CUDA(NULL, cudaFreeAsync(d_tab, st));
+    VR_CUDA(NULL, cudaFreeAsync(d_order, st));
+    return VR_OK;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * Debug / test exports. They run the same set-up kernel a frame runs and read its tables.
+ * ---------------------------------------------------------------------------------------- */
+static int debug_setup(vr_volume* v, const char* who, const float* view, const float* proj, int W, int H) {
+    long long sub_px = 0, items = 0;
+    int rc = check_view(v, who, view, proj, W, H, &sub_px, &items);
+    if (rc) return rc;
+    rc = ensure_sub(v, sub_px);
+    if (rc) return rc;
+    rc = run_setup(v, view, proj, W, H, VR_ALPHA, 0);
+    if (rc) return rc;
+    v->last_valid = false; /* the sub-image offsets of the last frame are gone */
+    VR_CUDA(v, cudaDeviceSynchronize());
+    return VR_OK;
+}
+
+extern "C" int vr_debug_brick_order(vr_volume* v, const float* view, const float* proj, int* order_out) {
+    if (v && !order_out) return fail(v, VR_ERR_INVALID_ARG, "vr_debug_brick_order: NULL output");
+    const int rc = debug_setup(v, "vr_debug_brick_order", view, proj, 16, 16);
+    if (rc) return rc;
+    VR_CUDA(v, cudaMemcpy(order_out, v->d_order, sizeof(int) * v->grid.nbricks, cudaMemcpyDeviceToHost));
+    return VR_OK;
+}
+
+extern "C" int vr_debug_rects(vr_volume* v, const float* view, const float* proj, int width, int height, int* rects_out) {
+    if (v && !rects_out) return fail(v, VR_ERR_INVALID_ARG, "vr_debug_rects: NULL output");
+    const int rc = debug_setup(v, "vr_debug_rects", view, proj, width, height);
+    if (rc) return rc;
+    const int nb = v->grid.nbricks;
+    VrBrickView* h = new (std::nothrow) VrBrickView[nb];
+    if (!h) return fail(v, VR_ERR_OUT_OF_MEMORY, "vr_debug_rects: host allocation failed");
+    cudaError_t e = cudaMemcpy(h, v->d_bv, sizeof(VrBrickView) * nb, cudaMemcpyDeviceToHost);
+    if (e == cudaSuccess)
+        for (int b = 0; b < nb; ++b) {
+            rects_out[4 * b + 0] = h[b].rx0;
+            rects_out[4 * b + 1] = h[b].ry0;
+            rects_out[4 * b + 2] = h[b].rx1;
+            rects_out[4 * b + 3] = h[b].ry1;
+        }
+    delete[] h;
+    VR_CUDA(v, e);
+    return VR_OK;
+}
+
+extern "C" int vr_debug_ray_bricks(vr_volume* v, const float* view, const float* proj, int width, int height,
+                                   const int* pixels, int npix, int* counts, int* lists, int maxlen, uint8_t* grazing) {
+    if (v && (!pixels || !counts || !lists || npix <= 0 || maxlen <= 0))
+        return fail(v, VR_ERR_INVALID_ARG, "vr_debug_ray_bricks: NULL or empty argument");
+    int rc = debug_setup(v, "vr_debug_ray_bricks", view, proj, width, height);
+    if (rc) return rc;
+    int *d_pix = NULL, *d_counts = NULL, *d_lists = NULL;
+    double* d_tins = NULL;
+    unsigned char* d_gz = NULL;
+    cudaError_t e = cudaMalloc(&d_pix, sizeof(int) * 2 * (size_t)npix);
+    if (e == cudaSuccess) e = cudaMalloc(&d_counts, sizeof(int) * (size_t)npix);
+    if (e == cudaSuccess) e = cudaMalloc(&d_lists, sizeof(int) * (size_t)npix * maxlen);
+    if (e == cudaSuccess) e = cudaMalloc(&d_tins, sizeof(double) * (size_t)npix * maxlen);
+    if (e == cudaSuccess) e = cudaMalloc(&d_gz, (size_t)npix);
+    if (e == cudaSuccess) e = cudaMemcpy(d_pix, pixels, sizeof(int) * 2 * (size_t)npix, cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) {
+        e = vr_launch_ray_bricks(v->grid, v->d_vs, d_pix, npix, d_counts, d_lists, d_tins, maxlen, d_gz, 0);
+        v->launches++;
+    }
+    if (e == cudaSuccess) e = cudaDeviceSynchronize();
+    if (e == cudaSuccess) e = cudaMemcpy(counts, d_counts, sizeof(int) * (size_t)npix, cudaMemcpyDeviceToHost);
+    if (e == cudaSuccess) e = cudaMemcpy(lists, d_lists, sizeof(int) * (size_t)npix * maxlen, cudaMemcpyDeviceToHost);
+    if (e == cudaSuccess && grazing) e = cudaMemcpy(grazing, d_gz, (size_t)npix, cudaMemcpyDeviceToHost);
+    cudaFree(d_pix);
+    cudaFree(d_counts);
+    cudaFree(d_lists);
+    cudaFree(d_tins);
+    cudaFree(d_gz);
+    VR_CUDA(v, e);
+    return VR_OK;
+}
+
+extern "C" int vr_debug_subimages(vr_volume* v, const int* pixels, int npix, float* sub_out) {
+    if (!v) return fail(NULL, VR_ERR_INVALID_ARG, "vr_debug_subimages: NULL handle");
+    if (!pixels || !sub_out || npix <= 0) return fail(v, VR_ERR_INVALID_ARG, "vr_debug_subimages: NULL or empty argument");
+    if (!v->last_valid) return fail(v, VR_ERR_STATE, "vr_debug_subimages: no vr_render since the last debug call");
+    for (int q = 0; q < npix; ++q)
+        if (pixels[2 * q] < 0 || pixels[2 * q] >= v->last_W || pixels[2 * q + 1] < 0 || pixels[2 * q + 1] >= v->last_H)
+            return fail(v, VR_ERR_INVALID_ARG, "vr_debug_subimages: pixel %d outside the last frame", q);
+    const int nb = v->grid.nbricks;
+    int* d_pix = NULL;
+    float* d_out = NULL;
+    VR_CUDA(v, cudaDeviceSynchronize());
+    cudaError_t e = cudaMalloc(&d_pix, sizeof(int) * 2 * (size_t)npix);
+    if (e == cudaSuccess) e = cudaMalloc(&d_out, sizeof(float) * 4 * (size_t)npix * nb);
+    if (e == cudaSuccess) e = cudaMemcpy(d_pix, pixels, sizeof(int) * 2 * (size_t)npix, cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) {
+        e = vr_launch_gather_sub(v->d_bv, nb, v->d_sub, v->last_mode, d_pix, npix, d_out, 0);
+        v->launches++;
+    }
+    if (e == cudaSuccess) e = cudaDeviceSynchronize();
+    if (e == cudaSuccess) e = cudaMemcpy(sub_out, d_out, sizeof(float) * 4 * (size_t)npix * nb, cudaMemcpyDeviceToHost);
+    cudaFree(d_pix);
+    cudaFree(d_out);
+    VR_CUDA(v, e);
+    return VR_OK;
+}
+
+extern "C" int vr_debug_stats(vr_volume* v, vr_stats* out) {
+    if (!v) return fail(NULL, VR_ERR_INVALID_ARG, "vr_debug_stats: NULL handle");
+    if (!out) return fail(v, VR_ERR_INVALID_ARG, "vr_debug_stats: NULL output");
+    if (!v->last_valid) return fail(v, VR_ERR_STATE, "vr_debug_stats: no vr_render since the last debug call");
+    VR_CUDA(v, cudaDeviceSynchronize());
+    VrViewState vs;
+    VR_CUDA(v, cudaMemcpy(&vs, v->d_vs, sizeof(vs), cudaMemcpyDeviceToHost));
+    out->samples = v->counting ? (int64_t)vs.samples : -1;
+    out->rays = (int64_t)vs.total_sub_pixels;
+    out->work_items = vs.total_items;
+    out->subimage_bytes = (int64_t)vs.total_sub_pixels * (v->last_mode == VR_ALPHA ? 16 : 4);
+    out->nbricks = v->grid.nbricks;
+    out->overflow = vs.overflow;
+    out->ms_setup = out->ms_raycast = out->ms_composite = -1.0f;
+    if (v->timing && v->ev_valid) {
+        VR_CUDA(v, cudaEventElapsedTime(&out->ms_setup, v->ev[0], v->ev[1]));
+        VR_CUDA(v, cudaEventElapsedTime(&out->ms_raycast, v->ev[1], v->ev[2]));
+        VR_CUDA(v, cudaEventElapsedTime(&out->ms_composite, v->ev[2], v->ev[3]));
+    }
+    return VR_OK;
+}

@@ -1,0 +1,108 @@
+/*
+ * vr_bricks.cu -- the brick store.
+ *
+ * PAPER.md:105,113 (sec. 2.1): the cube is split into sub-cubes that are rendered
+ * independently; :136 (sec. 2.3.1) partitioning; :146 the data is moved into GPU memory once,
+ * before rendering. The paper keeps each sub-cube in texture memory (:150); here a brick is a
+ * ghost-padded linear float32 array in HBM (DESIGN.md "Data layout" says why).
+ *
+ * Ghost cells (R3): cell (i,j,k) of brick b holds global voxel clamp(lo_b - ghost + (i,j,k),
+ * 0, n-1), so every tri-linear fetch of a sample the brick owns stays inside the brick and
+ * the volume boundary is edge-replicated.
+ *
+ * Upload is a gather: one warp per padded row of one brick, lanes along x (coalesced writes,
+ * coalesced reads except at the two replicated ends). A cell is written iff its clamped
+ * global index lies in the uploaded box, which makes z-slab uploads of a ~100 GB cube work.
+ */
+#include "vr_view.cuh"
+
+/* range [a0,a1) of padded indices i in [0,ext) with clamp(lo - ghost + i, 0, n-1) in [c0,c1) */
+__device__ __forceinline__ void padded_range(int lo, int ghost, int ext, int n, int c0, int c1, int& a0, int& a1) {
+    /* global index x(i) = clamp(lo - ghost + i, 0, n-1) is non-decreasing in i */
+    const int base = lo - ghost;
+    /* first i with x(i) >= c0 */
+    int f0 = c0 - base;              /* unclamped solution */
+    if (c0 <= 0) f0 = 0;             /* clamped-low cells map to 0 >= c0 */
+    if (c0 > n - 1) f0 = ext;        /* never reached */
+    /* first i with x(i) >= c1 */
+    int f1 = c1 - base;
+    if (c1 <= 0) f1 = 0;
+    if (c1 > n - 1) f1 = ext;
+    a0 = min(max(f0, 0), ext);
+    a1 = min(max(f1, 0), ext);
+}
+
+__global__ void __launch_bounds__(256)
+vr_upload_kernel(VrGrid g, float* __restrict__ bricks, const float* __restrict__ src, int x0, int y0, int z0, int sx, int sy,
+                 int sz) {
+    const int b = blockIdx.y;
+    int bc[3], lo[3], hi[3];
+    vr_brick_coords(g, b, bc);
+    vr_brick_core(g, bc, lo, hi);
+    const int ex = hi[0] - lo[0] + 2 * g.ghost, ey = hi[1] - lo[1] + 2 * g.ghost, ez = hi[2] - lo[2] + 2 * g.ghost;
+    int i0, i1, j0, j1, k0, k1;
+    padded_range(lo[0], g.ghost, ex, g.n[0], x0, x0 + sx, i0, i1);
+    padded_range(lo[1], g.ghost, ey, g.n[1], y0, y0 + sy, j0, j1);
+    padded_range(lo[2], g.ghost, ez, g.n[2], z0, z0 + sz, k0, k1);
+    if (i1 <= i0 || j1 <= j0 || k1 <= k0) return;
+    const int rows = (j1 - j0) * (k1 - k0);
+    const int warps_per_block = blockDim.x >> 5, lane = threadIdx.x & 31;
+    float* __restrict__ dstb = bricks + (long long)b * g.slot;
+    for (int row = blockIdx.x * warps_per_block + (threadIdx.x >> 5); row < rows; row += gridDim.x * warps_per_block) {
+        const int j = j0 + row % (j1 - j0), k = k0 + row / (j1 - j0);
+        const int gy = min(max(lo[1] - g.ghost + j, 0), g.n[1] - 1), gz = min(max(lo[2] - g.ghost + k, 0), g.n[2] - 1);
+        const float* __restrict__ srow = src + ((long long)(gz - z0) * sy + (gy - y0)) * sx;
+        float* __restrict__ drow = dstb + ((long long)k * g.P + j) * g.P;
+        for (int i = i0 + lane; i < i1; i += 32) {
+            const int gx = min(max(lo[0] - g.ghost + i, 0), g.n[0] - 1);
+            drow[i] = __ldcs(srow + (gx - x0));
+        }
+    }
+}
+
+__global__ void __launch_bounds__(256)
+vr_download_kernel(VrGrid g, const float* __restrict__ bricks, float* __restrict__ dst, int x0, int y0, int z0, int sx, int sy,
+                   int sz) {
+    /* one warp per row (y,z) of the requested box; lanes along x */
+    const long long rows = (long long)sy * sz;
+    const int warps_per_block = blockDim.x >> 5, lane = threadIdx.x & 31;
+    for (long long row = (long long)blockIdx.x * warps_per_block + (threadIdx.x >> 5); row < rows;
+         row += (long long)gridDim.x * warps_per_block) {
+        const int y = y0 + (int)(row % sy), z = z0 + (int)(row / sy);
+        const int by = y / g.brick, bz = z / g.brick;
+        for (int xo = lane; xo < sx; xo += 32) {
+            const int x = x0 + xo;
+            const int bx = x / g.brick;
+            const int b = (bz * g.g[1] + by) * g.g[0] + bx;
+            const int i = x - bx * g.brick + g.ghost, j = y - by * g.brick + g.ghost, k = z - bz * g.brick + g.ghost;
+            dst[row * sx + xo] = bricks[(long long)b * g.slot + ((long long)k * g.P + j) * g.P + i];
+        }
+    }
+}
+
+cudaError_t vr_launch_upload(const VrGrid& grid, float* bricks, const float* src, int x0, int y0, int z0, int sx, int sy,
+                             int sz, cudaStream_t st) {
+    /* enough CTAs per brick to cover its rows once at 8 rows per CTA, capped */
+    long long rows = (long long)grid.P * grid.P;
+    int bx = (int)((rows + 7) / 8);
+    if (bx > 4096) bx = 4096;
+    for (int b0 = 0; b0 < grid.nbricks; b0 += 65535) {
+        const int nb = grid.nbricks - b0 < 65535 ? grid.nbricks - b0 : 65535;
+        VrGrid g = grid;
+        (void)g;
+        dim3 gr(bx, nb);
+        if (b0 != 0) return cudaErrorInvalidValue; /* more than 65535 bricks is rejected at create */
+        vr_upload_kernel<<<gr, 256, 0, st>>>(grid, bricks, src, x0, y0, z0, sx, sy, sz);
+    }
+    return cudaGetLastError();
+}
+
+cudaError_t vr_launch_download(const VrGrid& grid, const float* bricks, float* dst, int x0, int y0, int z0, int sx, int sy,
+                               int sz, cudaStream_t st) {
+    long long rows = (long long)sy * sz;
+    long long blocks = (rows + 7) / 8;
+    if (blocks > 148 * 32) blocks = 148 * 32;
+    if (blocks < 1) blocks = 1;
+    vr_download_kernel<<<(unsigned)blocks, 256, 0, st>>>(grid, bricks, dst, x0, y0, z0, sx, sy, sz);
+    return cudaGetLastError();
+}

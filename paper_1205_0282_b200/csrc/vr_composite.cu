@@ -1,0 +1,122 @@
+/*
+ * vr_composite.cu -- sort-last compositing of sub-images into the final frame (SURVEY.md
+ * sec. 8(a) row a9) and, for MIP, the final colour mapping.
+ *
+ * PAPER.md:170-174 (sec. 2.3.3): sub-frames are merged guided by their rendering rectangles;
+ * the alpha blending operator is associative, so sub-images composite in visibility order;
+ * MIP composites in any order; :172 the merged scalar frame is colour-mapped at the end.
+ * :114 names compositing as the bottleneck of distributed image-order rendering, which is
+ * why it is a bandwidth-shaped kernel here: every sub-image pixel is read once with
+ * coalesced 16-byte loads and the frame is written once.
+ *
+ * One CTA per 32x8-pixel tile of the frame. The CTA first filters the layer table, in
+ * visibility order, down to the layers whose rectangle meets its tile (ballot + prefix,
+ * order-preserving), then each thread walks that short list for its pixel:
+ *   ALPHA  C += (1-A) C_l,  A += (1-A) A_l      (float32, R15; no early termination)
+ *   MIP    m = max(m, m_l); at the end RGB = LUT(u(m)), A = 1, or (0,0,0,0) if m = -inf (R11)
+ */
+#include "vr_internal.cuh"
+
+#define COMP_THREADS (VR_COMP_TILE_W * VR_COMP_TILE_H)
+#define COMP_LIST 256
+
+struct CompEntry {
+    unsigned long long addr;
+    int x0, y0, x1, y1;
+    int sx0, sy0, pitch;
+    int inside; /* the whole tile lies inside the layer's rectangle */
+};
+
+template <int MODE>
+__global__ void __launch_bounds__(COMP_THREADS)
+vr_composite_kernel(const VrCompLayer* __restrict__ layers, const int* __restrict__ order, int n, int W, int H, VrLut lut,
+                    float4* __restrict__ out) {
+    __shared__ CompEntry s_list[COMP_LIST];
+    __shared__ int s_warp_cnt[COMP_THREADS / 32];
+    __shared__ int s_count;
+
+    const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+    const int tx0 = blockIdx.x * VR_COMP_TILE_W, ty0 = blockIdx.y * VR_COMP_TILE_H;
+    const int tx1 = min(tx0 + VR_COMP_TILE_W, W), ty1 = min(ty0 + VR_COMP_TILE_H, H);
+    const int px = tx0 + (tid & (VR_COMP_TILE_W - 1)), py = ty0 + tid / VR_COMP_TILE_W;
+    const bool live = px < W && py < H;
+
+    float cr = 0.0f, cg = 0.0f, cb = 0.0f, ca = 0.0f;
+    float m = -INFINITY;
+
+    for (int q0 = 0; q0 < n; q0 += COMP_THREADS) {
+        /* order-preserving filter of up to 256 layers */
+        const int q = q0 + tid;
+        bool hit = false;
+        VrCompLayer L;
+        if (q < n) {
+            L = layers[order[q]];
+            hit = L.x0 < tx1 && L.x1 > tx0 && L.y0 < ty1 && L.y1 > ty0 && L.x1 > L.x0 && L.y1 > L.y0;
+        }
+        const unsigned bal = __ballot_sync(0xffffffffu, hit);
+        if (lane == 0) s_warp_cnt[wid] = __popc(bal);
+        __syncthreads();
+        int base = 0;
+        for (int w = 0; w < wid; ++w) base += s_warp_cnt[w];
+        if (hit) {
+            CompEntry e;
+            e.addr = L.addr;
+            e.x0 = L.x0; e.y0 = L.y0; e.x1 = L.x1; e.y1 = L.y1;
+            e.sx0 = L.sx0; e.sy0 = L.sy0; e.pitch = L.pitch;
+            e.inside = L.x0 <= tx0 && L.x1 >= tx1 && L.y0 <= ty0 && L.y1 >= ty1;
+            s_list[base + __popc(bal & ((1u << lane) - 1u))] = e;
+        }
+        if (tid == COMP_THREADS - 1) s_count = base + __popc(bal);
+        __syncthreads();
+        const int cnt = s_count;
+
+        if (live) {
+#pragma unroll 4
+            for (int k = 0; k < cnt; ++k) {
+                const CompEntry& e = s_list[k];
+                const bool in = e.inside || (px >= e.x0 && px < e.x1 && py >= e.y0 && py < e.y1);
+                if (in) {
+                    const long long off = (long long)(py - e.sy0) * e.pitch + (px - e.sx0);
+                    if (MODE == VR_ALPHA) {
+                        const float4 s = __ldcs(reinterpret_cast<const float4*>(e.addr) + off);
+                        const float t = 1.0f - ca;
+                        cr = fmaf(t, s.x, cr);
+                        cg = fmaf(t, s.y, cg);
+                        cb = fmaf(t, s.z, cb);
+                        ca = fmaf(t, s.w, ca);
+                    } else {
+                        m = fmaxf(m, __ldcs(reinterpret_cast<const float*>(e.addr) + off));
+                    }
+                }
+            }
+        }
+        __syncthreads();
+    }
+
+    if (live) {
+        float4 o;
+        if (MODE == VR_ALPHA) {
+            o = make_float4(cr, cg, cb, ca);
+        } else if (m == -INFINITY) {
+            o = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+        } else {
+            const float u = __saturatef((m - lut.vmin) * lut.inv_range);
+            const float x = u * (float)(lut.n - 1);
+            const int i = min((int)x, lut.n - 2);
+            const float f = x - (float)i;
+            const float4 e = __ldg(lut.base + i), d = __ldg(lut.delta + i);
+            o = make_float4(fmaf(f, d.x, e.x), fmaf(f, d.y, e.y), fmaf(f, d.z, e.z), 1.0f);
+        }
+        __stcs(out + (long long)py * W + px, o);
+    }
+}
+
+cudaError_t vr_launch_composite(const VrCompLayer* layers, const int* order, int n, int W, int H, int mode,
+                                const VrLut& lut, float* out, cudaStream_t st) {
+    dim3 grid((W + VR_COMP_TILE_W - 1) / VR_COMP_TILE_W, (H + VR_COMP_TILE_H - 1) / VR_COMP_TILE_H);
+    if (mode == VR_ALPHA)
+        vr_composite_kernel<VR_ALPHA><<<grid, COMP_THREADS, 0, st>>>(layers, order, n, W, H, lut, reinterpret_cast<float4*>(out));
+    else
+        vr_composite_kernel<VR_MIP><<<grid, COMP_THREADS, 0, st>>>(layers, order, n, W, H, lut, reinterpret_cast<float4*>(out));
+    return cudaGetLastError();
+}

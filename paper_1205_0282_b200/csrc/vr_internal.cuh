@@ -1,0 +1,124 @@
+/*
+ * vr_internal.cuh -- shared declarations of libvr's translation units (not part of the ABI).
+ *
+ * Data layout in HBM:
+ *   bricks        float[nbricks][P][P][P], P = brick + 2*ghost, x fastest. Brick b =
+ *                 (bz*gy + by)*gx + bx. Cell (i,j,k) of brick b holds global voxel
+ *                 clamp(lo_b - ghost + (i,j,k), 0, n-1). Ragged bricks use the low corner of
+ *                 their P^3 slot. 64-bit offsets throughout (a 104 GB store has 2.6e10 cells).
+ *   VrViewState   one per handle: matrices, eye, totals, work counter (written by set-up).
+ *   VrBrickView   one per brick: rendering rectangle, launch rectangle, sub-image offset.
+ *   order         int[nbricks]: brick ids front to back; item_prefix int[nbricks+1]:
+ *                 exclusive prefix of work-item counts by order position.
+ *   sub-images    per brick, launch-rectangle sized, float4 (ALPHA) or float (MIP) per pixel.
+ */
+#ifndef VR_INTERNAL_CUH
+#define VR_INTERNAL_CUH
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/vr.h"
+
+#define VR_MAX_LUT 1024
+#define VR_TILE_W 8 /* a warp renders an 8x4 pixel tile of one brick */
+#define VR_TILE_H 4
+#define VR_MAX_AXIS_BRICKS 1024
+#define VR_RAYCAST_THREADS 256
+#define VR_COMP_TILE_W 32
+#define VR_COMP_TILE_H 8
+
+struct VrGrid {
+    int n[3];     /* nx, ny, nz */
+    int g[3];     /* bricks per axis */
+    int brick, ghost;
+    int nbricks;
+    int P;        /* padded edge of a brick slot */
+    long long slot; /* P^3 */
+    int brick_pow2; /* 1 if brick is a power of two (division by it is an exact scaling) */
+};
+
+/* The caller's matrices travel to the set-up kernel as a kernel argument (no copy, no sync). */
+struct VrMatrices {
+    float view[16];
+    float proj[16];
+};
+
+struct VrViewState {
+    double M[16];    /* proj * view, column-major */
+    double Minv[16];
+    double eye[3];   /* perspective: eye point; orthographic: forward direction (R9) */
+    int ortho;
+    int singular;
+    int W, H;
+    int total_items;
+    int overflow;
+    long long total_sub_pixels;
+    unsigned int work_counter;
+    unsigned int pad0;
+    unsigned long long samples;
+};
+
+struct VrBrickView {
+    int rx0, ry0, rx1, ry1; /* rendering rectangle, half-open, clipped */
+    int lx0, ly0, lx1, ly1; /* launch rectangle: the same, grown to the 8x4 tile grid */
+    int tiles_x, tiles_y;
+    int order_pos;
+    int pad;
+    long long sub_offset;   /* first pixel of this brick's sub-image in the scratch */
+};
+
+/* One layer of the sort-last compositing pass (a brick sub-image or a caller's layer). */
+struct VrCompLayer {
+    int x0, y0, x1, y1;      /* pixels of the frame this layer covers (half-open) */
+    int sx0, sy0;            /* frame position of the layer's stored pixel (0,0) */
+    int pitch;               /* stored pixels per row */
+    int pad;
+    unsigned long long addr; /* device address of stored pixel (0,0) */
+};
+
+struct VrLut {
+    const float4* base;  /* device: entries LUT[i]           (n of them)   */
+    const float4* delta; /* device: LUT[i+1] - LUT[i]         (n-1, last 0) */
+    int n;
+    float vmin, vmax, inv_range;
+};
+
+struct VrRaycastParams {
+    VrGrid grid;
+    const float* bricks;
+    const VrViewState* vs;
+    const VrBrickView* bv;
+    const int* order;
+    const int* item_prefix;
+    VrViewState* vs_rw; /* work counter, sample counter */
+    void* sub;          /* float4[] (ALPHA) or float[] (MIP) */
+    VrLut lut;
+    double step;
+    float tau;
+    int mode;
+};
+
+/* ---- launchers (each returns the cudaError of its launch) ---- */
+cudaError_t vr_launch_setup(const VrGrid& grid, const VrMatrices& mats, int W, int H, int mode,
+                            long long sub_capacity_px, void* sub_base, VrViewState* vs, VrBrickView* bv, int* order,
+                            int* item_prefix, VrCompLayer* layers, cudaStream_t st);
+cudaError_t vr_launch_raycast(const VrRaycastParams& p, int ctas, bool count, cudaStream_t st);
+cudaError_t vr_launch_composite(const VrCompLayer* layers, const int* order, int n, int W, int H, int mode,
+                                const VrLut& lut, float* out, cudaStream_t st);
+cudaError_t vr_launch_upload(const VrGrid& grid, float* bricks, const float* src, int x0, int y0, int z0, int sx,
+                             int sy, int sz, cudaStream_t st);
+cudaError_t vr_launch_download(const VrGrid& grid, const float* bricks, float* dst, int x0, int y0, int z0, int sx,
+                               int sy, int sz, cudaStream_t st);
+cudaError_t vr_launch_ray_bricks(const VrGrid& grid, const VrViewState* vs, const int* d_pixels, int npix,
+                                 int* d_counts, int* d_lists, double* d_tins, int maxlen, unsigned char* d_grazing,
+                                 cudaStream_t st);
+cudaError_t vr_launch_gather_sub(const VrBrickView* bv, int nbricks, const void* sub, int mode, const int* d_pixels,
+                                 int npix, float* d_out, cudaStream_t st);
+int vr_raycast_ctas(); /* persistent grid size: resident CTAs per SM x SM count */
+
+/* host mirror of the set-up arithmetic, for argument validation and scratch sizing only */
+int vr_host_view_check(const VrGrid& grid, const float* view, const float* proj, int W, int H, long long* sub_pixels,
+                       long long* items);
+
+#endif

@@ -1,0 +1,212 @@
+/*
+ * vr_setup.cu -- per-view set-up and device-side visibility sort (SURVEY.md sec. 8(a) rows
+ * a2, a3). One CTA per frame, no host involvement:
+ *   1. M = proj*view, its inverse, the homogeneous eye (vr_view.cuh).
+ *   2. Per-axis slab ranks by distance from the eye (perspective) or by the sign of the view
+ *      direction (orthographic); brick key = (rank_z, rank_y, rank_x) lexicographic. The
+ *      ranks are permutations, so the key IS the brick's position in the front-to-back
+ *      order: the sort is a direct scatter, exact and deterministic (R9). PAPER.md:53 names
+ *      depth sorting as one of the tasks done in CUDA; :174 needs the order for `over`.
+ *   3. Per brick: rendering rectangle = bounding box of its 8 projected vertices
+ *      (Fig. 4 :168), launch rectangle on the 8x4 tile grid, tile counts.
+ *   4. Exclusive scans, in visibility order, of the tile counts (work list of the persistent
+ *      ray-cast kernel) and of the sub-image sizes (scratch offsets); compositing table.
+ */
+#include "vr_view.cuh"
+
+#define SETUP_THREADS 256
+
+struct SetupShared {
+    double M[16];
+    int rank[3][VR_MAX_AXIS_BRICKS];
+    int warp_items[SETUP_THREADS / 32];
+    long long warp_pix[SETUP_THREADS / 32];
+    int carry_items;
+    long long carry_pix;
+    int ortho;
+    double eye[3];
+};
+
+__global__ void __launch_bounds__(SETUP_THREADS)
+vr_setup_kernel(VrGrid grid, VrMatrices mats, int W, int H, int mode, long long sub_capacity_px,
+                unsigned long long sub_base, VrViewState* __restrict__ vs, VrBrickView* __restrict__ bv,
+                int* __restrict__ order, int* __restrict__ item_prefix, VrCompLayer* __restrict__ layers) {
+    __shared__ SetupShared sh;
+    const int tid = threadIdx.x;
+
+    if (tid == 0) {
+        double Minv[16];
+        int ortho = 0;
+        const int bad = vr_view_setup(mats.view, mats.proj, sh.M, Minv, sh.eye, &ortho);
+        sh.ortho = ortho;
+        for (int i = 0; i < 16; ++i) {
+            vs->M[i] = sh.M[i];
+            vs->Minv[i] = Minv[i];
+        }
+        for (int a = 0; a < 3; ++a) vs->eye[a] = sh.eye[a];
+        vs->ortho = ortho;
+        vs->singular = bad;
+        vs->W = W;
+        vs->H = H;
+        vs->work_counter = 0u;
+        vs->samples = 0ull;
+        sh.carry_items = 0;
+        sh.carry_pix = 0;
+    }
+    __syncthreads();
+
+    /* per-axis ranks (R9) */
+    for (int a = 0; a < 3; ++a) {
+        const int n = grid.g[a];
+        for (int i = tid; i < n; i += SETUP_THREADS) {
+            int r;
+            if (sh.ortho) {
+                r = (sh.eye[a] >= 0.0) ? i : (n - 1 - i);
+            } else {
+                const double e = sh.eye[a];
+                double lo = (double)i * (double)grid.brick, hi = lo + (double)grid.brick;
+                if (hi > (double)grid.n[a]) hi = (double)grid.n[a];
+                const double di = (e < lo) ? VR_SUB(lo, e) : ((e > hi) ? VR_SUB(e, hi) : 0.0);
+                r = 0;
+                for (int j = 0; j < n; ++j) {
+                    double lj = (double)j * (double)grid.brick, hj = lj + (double)grid.brick;
+                    if (hj > (double)grid.n[a]) hj = (double)grid.n[a];
+                    const double dj = (e < lj) ? VR_SUB(lj, e) : ((e > hj) ? VR_SUB(e, hj) : 0.0);
+                    if (dj < di || (dj == di && j < i)) ++r;
+                }
+            }
+            sh.rank[a][i] = r;
+        }
+    }
+    __syncthreads();
+
+    /* per brick: order position, rectangles */
+    for (int b = tid; b < grid.nbricks; b += SETUP_THREADS) {
+        int bc[3], lo[3], hi[3], r[4], l[4];
+        vr_brick_coords(grid, b, bc);
+        vr_brick_core(grid, bc, lo, hi);
+        const int key = (sh.rank[2][bc[2]] * grid.g[1] + sh.rank[1][bc[1]]) * grid.g[0] + sh.rank[0][bc[0]];
+        order[key] = b;
+        vr_rect_of_box(sh.M, lo, hi, W, H, r);
+        vr_launch_rect(r, W, H, l);
+        VrBrickView v;
+        v.rx0 = r[0]; v.ry0 = r[1]; v.rx1 = r[2]; v.ry1 = r[3];
+        v.lx0 = l[0]; v.ly0 = l[1]; v.lx1 = l[2]; v.ly1 = l[3];
+        v.tiles_x = (l[2] - l[0] + VR_TILE_W - 1) / VR_TILE_W;
+        v.tiles_y = (l[3] - l[1] + VR_TILE_H - 1) / VR_TILE_H;
+        v.order_pos = key;
+        v.pad = 0;
+        v.sub_offset = 0;
+        bv[b] = v;
+    }
+    __syncthreads();
+    __threadfence_block();
+
+    /* exclusive scans over order positions, 256 at a time with a running carry */
+    const int lane = tid & 31, wid = tid >> 5;
+    for (int q0 = 0; q0 < grid.nbricks; q0 += SETUP_THREADS) {
+        const int q = q0 + tid;
+        int items = 0;
+        long long pix = 0;
+        int b = -1;
+        if (q < grid.nbricks) {
+            b = order[q];
+            const VrBrickView v = bv[b];
+            items = v.tiles_x * v.tiles_y;
+            pix = (long long)(v.lx1 - v.lx0) * (long long)(v.ly1 - v.ly0);
+        }
+        int si = items;
+        long long sp = pix;
+        for (int o = 1; o < 32; o <<= 1) {
+            const int ti = __shfl_up_sync(0xffffffffu, si, o);
+            const long long tp = __shfl_up_sync(0xffffffffu, sp, o);
+            if (lane >= o) {
+                si += ti;
+                sp += tp;
+            }
+        }
+        if (lane == 31) {
+            sh.warp_items[wid] = si;
+            sh.warp_pix[wid] = sp;
+        }
+        __syncthreads();
+        int bi = sh.carry_items;
+        long long bp = sh.carry_pix;
+        for (int w = 0; w < wid; ++w) {
+            bi += sh.warp_items[w];
+            bp += sh.warp_pix[w];
+        }
+        if (q < grid.nbricks) {
+            item_prefix[q] = bi + si - items;
+            bv[b].sub_offset = bp + sp - pix;
+        }
+        __syncthreads();
+        if (tid == SETUP_THREADS - 1) {
+            sh.carry_items = bi + si;
+            sh.carry_pix = bp + sp;
+        }
+        __syncthreads();
+    }
+
+    if (tid == 0) {
+        const int over = sh.carry_pix > sub_capacity_px;
+        item_prefix[grid.nbricks] = sh.carry_items;
+        vs->total_items = over ? 0 : sh.carry_items;
+        vs->total_sub_pixels = sh.carry_pix;
+        vs->overflow = over;
+    }
+    __syncthreads();
+
+    /* compositing table: one layer per brick */
+    const unsigned long long px_bytes = (mode == VR_ALPHA) ? 16ull : 4ull;
+    const bool over = sh.carry_pix > sub_capacity_px;
+    for (int b = tid; b < grid.nbricks; b += SETUP_THREADS) {
+        const VrBrickView v = bv[b];
+        VrCompLayer L;
+        L.x0 = v.rx0; L.y0 = v.ry0; L.x1 = over ? v.rx0 : v.rx1; L.y1 = v.ry1;
+        L.sx0 = v.lx0; L.sy0 = v.ly0;
+        L.pitch = v.lx1 - v.lx0;
+        L.pad = 0;
+        L.addr = sub_base + (unsigned long long)v.sub_offset * px_bytes;
+        layers[b] = L;
+    }
+}
+
+cudaError_t vr_launch_setup(const VrGrid& grid, const VrMatrices& mats, int W, int H, int mode, long long sub_capacity_px,
+                            void* sub_base, VrViewState* vs, VrBrickView* bv, int* order, int* item_prefix,
+                            VrCompLayer* layers, cudaStream_t st) {
+    vr_setup_kernel<<<1, SETUP_THREADS, 0, st>>>(grid, mats, W, H, mode, sub_capacity_px,
+                                                 (unsigned long long)(uintptr_t)sub_base, vs, bv, order, item_prefix, layers);
+    return cudaGetLastError();
+}
+
+/* Host mirror: is proj*view invertible, and how much scratch does this view need. Used for
+ * argument validation and scratch sizing only; the frame itself uses the kernel's values. */
+int vr_host_view_check(const VrGrid& grid, const float* view, const float* proj, int W, int H, long long* sub_pixels,
+                       long long* items) {
+    double M[16], Minv[16], eye[3];
+    int ortho;
+    if (vr_view_setup(view, proj, M, Minv, eye, &ortho)) return 1;
+    long long pix = 0, it = 0;
+    for (int b = 0; b < grid.nbricks; ++b) {
+        int bc[3], lo[3], hi[3], r[4], l[4];
+        vr_brick_coords(grid, b, bc);
+        vr_brick_core(grid, bc, lo, hi);
+        vr_rect_of_box(M, lo, hi, W, H, r);
+        /* one pixel of slack per side in case host and device round a vertex differently */
+        if (r[2] > r[0] && r[3] > r[1]) {
+            r[0] = r[0] > 0 ? r[0] - 1 : 0;
+            r[1] = r[1] > 0 ? r[1] - 1 : 0;
+            r[2] = r[2] < W ? r[2] + 1 : W;
+            r[3] = r[3] < H ? r[3] + 1 : H;
+        } else {
+            r[0] = 0; r[1] = 0; r[2] = 2 < W ? 2 : W; r[3] = 2 < H ? 2 : H;
+        }
+        vr_launch_rect(r, W, H, l);
+        pix += (long long)(l[2] - l[0]) * (l[3] - l[1]);
+        it += (long long)((l[2] - l[0] + VR_TILE_W - 1) / VR_TILE_W) * ((l[3] - l[1] + VR_TILE_H - 1) / VR_TILE_H);
+    }
+    *sub_pixels = pix;
+    *items = it;
+    return 0;
+}

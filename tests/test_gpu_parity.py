@@ -1,0 +1,259 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle on the same seeded
+inputs. Tolerances are north_star's: ALPHA max abs 2e-3 per RGBA channel, MIP 1e-5 relative;
+brick order, rectangles and ray-brick lists exact; brick store bit-exact."""
+import numpy as np
+import pytest
+
+import oracle
+import synth
+from helpers import check_alpha, check_mip, gpu_frame, make_pair, seeded_pixels
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def vr(cuda_device):
+    from paper_1205_0282_b200 import build
+    build.build()
+    import paper_1205_0282_b200 as vr
+    return vr
+
+
+def views_for(cube, W, H, n_rot=3, seed=77):
+    fr = synth.Framing(cube.nx, cube.ny, cube.nz, W, H)
+    out = []
+    for ortho in (False, True):
+        for k in range(n_rot):
+            out.append((("ortho" if ortho else "persp") + str(k), fr.seeded(seed, k), fr.proj(ortho)))
+    return out
+
+
+# --------------------------------------------------------------------------- a1 brick store
+@pytest.mark.parametrize("ghost", [0, 1, 2])
+def test_brick_store_is_bit_exact(vr, ghost):
+    import torch
+    cube = synth.Cube(5, 37, 29, 23, 3)
+    data = cube.fill_host()
+    g = vr.Volume(37, 29, 23, 8, ghost)
+    o = oracle.Volume(37, 29, 23, 8, ghost, data=data)
+    g.upload(data)  # host path
+    for b in range(g.nbricks):
+        assert np.array_equal(g.debug_brick_data(b), o.brick_data(b)), b
+    back = np.zeros_like(data)
+    g.download(back)
+    assert np.array_equal(back, data)
+    # device path, z-slabs and an interior sub-box written last
+    g2 = vr.Volume(37, 29, 23, 8, ghost)
+    d = torch.from_numpy(data).cuda()
+    for z0 in range(0, 23, 5):
+        g2.upload(d[z0:z0 + 5].contiguous(), origin=(0, 0, z0))
+    g2.upload(d[3:9, 4:20, 6:30].contiguous(), origin=(6, 4, 3))
+    for b in range(g2.nbricks):
+        assert np.array_equal(g2.debug_brick_data(b), o.brick_data(b)), b
+    sub = torch.zeros((7, 9, 11), dtype=torch.float32, device="cuda")
+    g2.download(sub, origin=(13, 10, 8))
+    assert np.array_equal(sub.cpu().numpy(), data[8:15, 10:19, 13:24])
+
+
+# --------------------------------------------------------------------------- a2, a3
+@pytest.mark.parametrize("dims,brick", [((64, 64, 64), 64), ((100, 90, 70), 32), ((37, 29, 23), 8)])
+def test_brick_order_and_rectangles_match_exactly(vr, dims, brick):
+    nx, ny, nz = dims
+    g = vr.Volume(nx, ny, nz, brick, 1)
+    o = oracle.Volume(nx, ny, nz, brick, 1)
+    W, H = 203, 117
+    fr = synth.Framing(nx, ny, nz, W, H)
+    cases = [(fr.seeded(3, k), fr.proj(k % 2 == 1)) for k in range(12)]
+    cases += [(fr.turntable(k), fr.proj(False)) for k in range(0, 36, 5)]
+    # eye inside the volume / close to a face: slabs at distance 0
+    cases.append((synth.look_at((nx * 0.4, ny * 0.6, nz * 0.5), (nx, ny, nz), (0, 0, 1)), synth.perspective(60, W / H, 0.5, 500)))
+    for view, proj in cases:
+        assert np.array_equal(g.debug_brick_order(view, proj), o.brick_order(view, proj))
+        assert np.array_equal(g.debug_rects(view, proj, W, H), o.rects(view, proj, W, H))
+
+
+def test_ray_brick_lists_match_exactly(vr):
+    nx, ny, nz, brick = 100, 90, 70, 32
+    g = vr.Volume(nx, ny, nz, brick, 1)
+    o = oracle.Volume(nx, ny, nz, brick, 1)
+    W, H = 160, 120
+    fr = synth.Framing(nx, ny, nz, W, H)
+    pix = seeded_pixels(9, W, H, 4000)
+    for k in range(6):
+        view, proj = fr.seeded(5, k), fr.proj(k % 2 == 1)
+        gc, gl, gg = g.debug_ray_bricks(view, proj, W, H, pix, maxlen=16)
+        oc, ol, og = o.ray_bricks(view, proj, W, H, pix, maxlen=16)
+        ok = (gg == 0) & (og == 0)
+        assert ok.mean() > 0.99
+        assert np.array_equal(gc[ok], oc[ok])
+        assert np.array_equal(gl[ok], ol[ok])
+        assert oc.max() > 3  # the lists are not trivial
+
+
+# --------------------------------------------------------------------------- c0: one brick
+@pytest.mark.parametrize("tf_name", ["ramp", "translucent"])
+def test_config0_full_frames(vr, tf_name):
+    c = synth.CONFIGS["c0"]
+    cube = synth.config_cube("c0")
+    tf = synth.tf_ramp() if tf_name == "ramp" else synth.tf_translucent()
+    g, o = make_pair(cube, c["brick"], c["ghost"], tf=tf)
+    W, H = c["width"], c["height"]
+    for name, view, proj in views_for(cube, W, H):
+        ref = o.render(view, proj, W, H, c["step"], oracle.ALPHA)
+        check_alpha(gpu_frame(g, view, proj, W, H, c["step"], vr.ALPHA), ref["image"], ref["flags"], 0.99, "c0 " + name)
+        ref = o.render(view, proj, W, H, c["step"], oracle.MIP)
+        check_mip(gpu_frame(g, view, proj, W, H, c["step"], vr.MIP), ref["image"], "c0 " + name)
+        assert ref["image"][..., 3].max() == 1.0 and ref["image"][..., 3].min() == 0.0
+
+
+# --------------------------------------------------------------------------- bricked, ragged
+@pytest.mark.parametrize("tau", [0.99, 2.0])
+def test_bricked_ragged_full_frames_and_subimages(vr, tau):
+    cube = synth.Cube(11, 100, 90, 70, 12)
+    tf = synth.tf_translucent() if tau > 1 else synth.tf_ramp()
+    g, o = make_pair(cube, 32, 1, tf=tf, tau=tau)
+    W, H = 203, 117  # not multiples of the 8x4 tile
+    step = 0.5
+    pix = seeded_pixels(4, W, H, 300)
+    for name, view, proj in views_for(cube, W, H, n_rot=2):
+        ref = o.render(view, proj, W, H, step, oracle.ALPHA)
+        img = gpu_frame(g, view, proj, W, H, step, vr.ALPHA)
+        check_alpha(img, ref["image"], ref["flags"], tau, name)
+        # row a8: each brick's sub-image value
+        sub_ref = o.render(view, proj, W, H, step, oracle.ALPHA, pixels=pix, want_sub=True)
+        sub = g.debug_subimages(pix).astype(np.float64)
+        fl = np.repeat(sub_ref["flags"][:, None], g.nbricks, axis=1)
+        check_alpha(sub, sub_ref["sub"], fl, tau, name + " sub-images")
+        ref = o.render(view, proj, W, H, step, oracle.MIP)
+        check_mip(gpu_frame(g, view, proj, W, H, step, vr.MIP), ref["image"], name)
+        sub_ref = o.render(view, proj, W, H, step, oracle.MIP, pixels=pix, want_sub=True)
+        sub = g.debug_subimages(pix).astype(np.float64)[..., 0]
+        m_ref = sub_ref["sub"][..., 0]
+        assert np.array_equal(np.isinf(sub), np.isinf(m_ref))  # same bricks took samples
+        fin = ~np.isinf(m_ref)
+        # the kernel may stop a MIP ray once the running max reaches vmax
+        check_mip(np.minimum(sub[fin], synth.TF_VMAX), np.minimum(m_ref[fin], synth.TF_VMAX), name + " sub-image max")
+
+
+def test_one_brick_equals_n_bricks_on_gpu(vr):
+    """ERT off: the bricked result equals the single-brick result (ghost = 1 suffices, R3)."""
+    cube = synth.Cube(12, 60, 50, 40, 5)
+    data = cube.fill_host()
+    tf = synth.tf_translucent()
+    g1, _ = make_pair(cube, 64, 1, tf=tf, tau=2.0, data=data)
+    gn, _ = make_pair(cube, 16, 1, tf=tf, tau=2.0, data=data)
+    g0, _ = make_pair(cube, 16, 0, tf=tf, tau=2.0, data=data)
+    W, H = 128, 96
+    fr = synth.Framing(60, 50, 40, W, H)
+    view, proj = fr.seeded(2, 0), fr.proj(False)
+    a = gpu_frame(g1, view, proj, W, H, 0.5, vr.ALPHA)
+    b = gpu_frame(gn, view, proj, W, H, 0.5, vr.ALPHA)
+    c = gpu_frame(g0, view, proj, W, H, 0.5, vr.ALPHA)
+    assert np.abs(a - b).max() < 2e-5
+    assert np.abs(a - c).max() > 1e-3  # ghost = 0 must show seams (negative test)
+    am = gpu_frame(g1, view, proj, W, H, 0.5, vr.MIP)
+    bm = gpu_frame(gn, view, proj, W, H, 0.5, vr.MIP)
+    check_mip(bm, am, "1 vs N bricks")
+
+
+# --------------------------------------------------------------------------- edge cases
+def test_edge_cases(vr):
+    import torch
+    cube = synth.Cube(13, 20, 18, 16, 2)
+    g, o = make_pair(cube, 8, 1)
+    fr = synth.Framing(20, 18, 16, 64, 48)
+    # 1x1 frame and a 3x2 frame
+    for (W, H) in ((1, 1), (3, 2), (33, 5)):
+        f2 = synth.Framing(20, 18, 16, W, H)
+        view, proj = f2.seeded(1, 0), f2.proj(False)
+        ref = o.render(view, proj, W, H, 0.5, oracle.ALPHA)
+        check_alpha(gpu_frame(g, view, proj, W, H, 0.5, vr.ALPHA), ref["image"], ref["flags"], 0.99, "%dx%d" % (W, H))
+    W, H = 64, 48
+    # the volume is behind the camera / off screen: transparent black, both modes
+    view = synth.look_at((10, 9, 200), (10, 9, 400), (0, 1, 0))
+    proj = synth.perspective(40, W / H, 1.0, 100.0)
+    for mode in (vr.ALPHA, vr.MIP):
+        assert not gpu_frame(g, view, proj, W, H, 0.5, mode).any()
+    # camera inside the volume (R2: the ray starts on the near plane)
+    view = synth.look_at((10.3, 9.1, 8.2), (30, 20, 12), (0, 0, 1))
+    proj = synth.perspective(70, W / H, 0.25, 100.0)
+    ref = o.render(view, proj, W, H, 0.5, oracle.ALPHA)
+    check_alpha(gpu_frame(g, view, proj, W, H, 0.5, vr.ALPHA), ref["image"], ref["flags"], 0.99, "inside")
+    ref = o.render(view, proj, W, H, 0.5, oracle.MIP)
+    check_mip(gpu_frame(g, view, proj, W, H, 0.5, vr.MIP), ref["image"], "inside")
+    # a step longer than the volume: one (clipped) sample per ray; and a fine step
+    view, proj = fr.seeded(1, 1), fr.proj(True)
+    for step in (100.0, 0.1, 1.0):
+        ref = o.render(view, proj, W, H, step, oracle.ALPHA)
+        check_alpha(gpu_frame(g, view, proj, W, H, step, vr.ALPHA), ref["image"], ref["flags"], 0.99, "step %g" % step)
+        ref = o.render(view, proj, W, H, step, oracle.MIP)
+        check_mip(gpu_frame(g, view, proj, W, H, step, vr.MIP), ref["image"], "step %g" % step)
+    # axis-aligned orthographic view: two direction components are exactly zero (R4)
+    view = synth.look_at((10, 9, -10.0), (10, 9, 0.0), (0.0, 1.0, 0.0))
+    proj = synth.orthographic(10, 9, 1.0, 46.0)
+    ref = o.render(view, proj, 20, 18, 1.0, oracle.MIP)
+    check_mip(gpu_frame(g, view, proj, 20, 18, 1.0, vr.MIP), ref["image"], "axis-aligned")
+    ref = o.render(view, proj, 20, 18, 1.0, oracle.ALPHA)
+    check_alpha(gpu_frame(g, view, proj, 20, 18, 1.0, vr.ALPHA), ref["image"], ref["flags"], 0.99, "axis-aligned")
+    # host-memory entry gives the same frame
+    view, proj = fr.seeded(1, 2), fr.proj(False)
+    a = gpu_frame(g, view, proj, W, H, 0.5, vr.ALPHA)
+    b = g.render_host(view, proj, W, H, 0.5, vr.ALPHA)
+    assert np.array_equal(a.astype(np.float32), b)
+    pinned = torch.empty((H, W, 4), dtype=torch.float32).pin_memory()
+    g.render_host(view, proj, W, H, 0.5, vr.ALPHA, out=pinned)
+    assert np.array_equal(pinned.numpy(), b)
+
+
+def test_errors(vr):
+    import torch
+    g = vr.Volume(16, 16, 16, 8, 1)
+    out = torch.empty((8, 8, 4), dtype=torch.float32, device="cuda")
+    I = np.eye(4, dtype=np.float32).T.reshape(16)
+    with pytest.raises(vr.VrError) as e:
+        g.render(I, I, 8, 8, 0.5, vr.ALPHA, out)
+    assert e.value.status == 4  # no transfer function
+    g.set_transfer_function(synth.tf_ramp(), -3, 10)
+    with pytest.raises(vr.VrError) as e:
+        g.render(I, I, 8, 8, 0.5, vr.ALPHA, out)
+    assert e.value.status == 4  # nothing uploaded
+    g.upload(np.zeros((16, 16, 16), dtype=np.float32))
+    with pytest.raises(vr.VrError) as e:
+        g.render(I, I, 8, 8, 0.0, vr.ALPHA, out)
+    assert e.value.status == 1
+    with pytest.raises(vr.VrError) as e:
+        g.render(I, np.zeros(16, dtype=np.float32), 8, 8, 0.5, vr.ALPHA, out)
+    assert e.value.status == 1 and "singular" in str(e.value)
+    with pytest.raises(vr.VrError):
+        g.render(I, I, 8, 8, 0.5, 7, out)
+    with pytest.raises(vr.VrError):
+        g.set_transfer_function(synth.tf_ramp(), 1.0, 1.0)
+    with pytest.raises(vr.VrError):
+        g.upload(np.zeros((4, 4, 4), dtype=np.float32), origin=(14, 0, 0))
+    g.render(I, I, 8, 8, 0.5, vr.ALPHA, out)  # still usable after errors
+    torch.cuda.synchronize()
+
+
+# --------------------------------------------------------------------------- a9 stand-alone
+def test_composite_matches_oracle(vr):
+    import torch
+    W, H, n = 97, 61, 9
+    rects, layers_h = [], []
+    for l in range(n):
+        x0, y0 = int(synth.u01(1, 1, l) * 60), int(synth.u01(1, 2, l) * 40)
+        x1, y1 = min(W, x0 + 5 + int(synth.u01(1, 3, l) * 70)), min(H, y0 + 3 + int(synth.u01(1, 4, l) * 50))
+        if l == 0:
+            x0, y0, x1, y1 = 0, 0, W, H
+        if l == 1:
+            x1 = x0  # an empty layer
+        rects.append((x0, y0, x1, y1))
+        layers_h.append(synth.layer_host(99, l, 0, (x1 - x0) * (y1 - y0)).reshape(y1 - y0, x1 - x0, 4))
+    order = synth.permutation(5, n)
+    ref = oracle.composite(layers_h, rects, order, W, H)
+    out = torch.full((H, W, 4), 7.0, dtype=torch.float32, device="cuda")
+    layers_d = [torch.from_numpy(l).cuda() if l.size else torch.empty((0, 0, 4), device="cuda") for l in layers_h]
+    vr.composite(layers_d, rects, order, W, H, out)
+    torch.cuda.synchronize()
+    assert np.abs(out.cpu().numpy() - ref).max() < 1e-5  # R15
+    with pytest.raises(vr.VrError):
+        vr.composite(layers_d, rects, np.zeros(n, dtype=np.int32), W, H, out)  # not a permutation
