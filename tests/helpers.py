@@ -60,7 +60,10 @@ def check_alpha(gpu, ref, flags, tau, what=""):
     bad = err > np.where(marg, ALPHA_TOL + max(0.0, 1.0 - tau), ALPHA_TOL)
     assert not bad.any(), "%s ALPHA: %d pixels off, max err %.3e (unflagged max %.3e)" % (
         what, int(bad.sum()), err.max(), err[~marg].max() if (~marg).any() else 0.0)
-    assert marg.mean() < 1e-3, "%s: %.4f%% decision-margin pixels" % (what, 100 * marg.mean())
+    # R12: a ray whose opacity passes tau in steps of dA is flagged with probability ~2e-5/dA
+    # (a few per cent at most); what must stay rare is a flagged pixel that really differs
+    assert marg.mean() < 0.03, "%s: %.4f%% decision-margin pixels" % (what, 100 * marg.mean())
+    assert (err > ALPHA_TOL).mean() < 1e-3, "%s: %.4f%% pixels beyond 2e-3" % (what, 100 * (err > ALPHA_TOL).mean())
     return float(err.max())
 
 
