@@ -1,0 +1,464 @@
+"""bench.py -- frames/s and Gsamples/s of the bricked ray-casting hot path on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload c3|c2|c1|c0]
+                    [--impl ours|reference] [--no-variants] [--no-cpu-baseline]
+
+A step is ONE FRAME: one pass of the whole hot path (view set-up + visibility sort, per-brick
+ray casting, sort-last compositing: rows a2..a9 of SURVEY.md sec. 8) for one view of the
+workload's 36-view cycle, on a synthetic radio-spectral-cube stand-in already resident in HBM
+as ghost-padded bricks (row a1, built once before the timed region, as in the paper:
+PAPER.md:146 loads the data once, :150 renders per view). DESIGN.md "Measurement" states the
+recipe, the algorithmic bytes and the roofline.
+
+Default workload = BASELINE.json configs[3] ("c3"): 4096x4096x1536 float32 (~103 GB) in 512^3
+ghost-padded bricks, 1920x1080, 36-view turntable, ALPHA, step 1.0, early termination 0.99 --
+the configuration the metric ("frames/sec and Gsamples/s at 1920x1080 on 1 B200") and
+north_star's target (">= 100 GB in-core cube at 1920x1080") are quoted on.
+
+N > 1 (torchrun): frames are independent units, so each rank holds its own copy of the cube
+and renders K frames of the cycle (different view offsets); no data-path collective; the
+aggregate is N*K frames over the slowest rank's time ("scaling": "weak").
+
+Prints ONE JSON line (rank 0).
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import synth  # noqa: E402  (seeded inputs only)
+
+METRIC = "frames/s at 1920x1080 (with Gsamples/s and roofline fraction beside it)"
+
+
+# ----------------------------------------------------------------------------- workloads
+def workload(name):
+    """Shapes, cameras and classification of BASELINE.json's configs."""
+    c = dict(synth.CONFIGS[name])
+    c["name"] = name
+    c["seed"] = synth.BASE_SEED + int(name[1:])
+    fr = synth.Framing(c["nx"], c["ny"], c["nz"], c["width"], c["height"])
+    if name == "c2":  # "1920x1080 perspective output, 36 seeded views"
+        c["views"] = [fr.seeded(c["seed"], k) for k in range(36)]
+        c["view_kind"] = "36 seeded rotations"
+    else:             # "36-frame turntable about the spectral axis"
+        c["views"] = [fr.turntable(k) for k in range(36)]
+        c["view_kind"] = "36-view turntable, elevation 20 deg"
+    c["proj"] = fr.proj(False)
+    c["tau"] = 0.99
+    return c
+
+
+def views_for_rank(rank, world, nviews):
+    """Rank r starts its cycle at view r*nviews/world: ranks render different frames."""
+    off = (rank * nviews) // max(world, 1)
+    return [(off + k) % nviews for k in range(nviews)]
+
+
+def aggregate(local_ms, frames_per_rank, world, all_reduce_max=None):
+    """Whole-job frames/s: all ranks' frames over the SLOWEST rank's device time."""
+    ms = all_reduce_max(local_ms) if all_reduce_max is not None else local_ms
+    return frames_per_rank * world / (ms * 1e-3), ms
+
+
+# ----------------------------------------------------------------------------- clocks
+class ClockSampler:
+    """nvidia-smi sampled every 200 ms DURING the timed region (profiling recipe's clocks line)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.proc, self.path = index, None, None
+
+    def start(self):
+        try:
+            fd, self.path = tempfile.mkstemp(suffix=".csv")
+            os.close(fd)
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q, "--format=csv,noheader,nounits",
+                                          "-lms", "200"], stdout=open(self.path, "w"), stderr=subprocess.DEVNULL)
+        except Exception:
+            self.proc = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.proc is None:
+            return out
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, smax, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in open(self.path):
+            f = [x.strip() for x in line.split(",")]
+            if len(f) < 9:
+                continue
+            try:
+                sm.append(float(f[1]))
+                smax.append(float(f[2]))
+            except ValueError:
+                continue
+            for n, val in zip(names, f[5:9]):
+                if val.lower().startswith("active"):
+                    reasons.add(n)
+        os.unlink(self.path)
+        if sm:
+            out.update(sm_mhz=float(np.median(sm)), sm_max_mhz=float(max(smax)), reasons=sorted(reasons), samples=len(sm))
+        return out
+
+
+# ----------------------------------------------------------------------------- product arm
+def build_volume(vr, wl, tf):
+    """Row a1: generate the cube on the device slab by slab (synth's CUDA twin) and upload it."""
+    import torch
+    cube = synth.Cube(wl["seed"], wl["nx"], wl["ny"], wl["nz"], wl["nsrc"], wl["ramp"])
+    g = vr.Volume(wl["nx"], wl["ny"], wl["nz"], wl["brick"], wl["ghost"])
+    plane = wl["nx"] * wl["ny"] * 4
+    nzs = max(1, min(wl["nz"], (1 << 30) // plane))
+    buf = torch.empty((nzs, wl["ny"], wl["nx"]), dtype=torch.float32, device="cuda")
+    st = torch.cuda.current_stream().cuda_stream
+    for z0 in range(0, wl["nz"], nzs):
+        nk = min(nzs, wl["nz"] - z0)
+        cube.fill_device(buf[:nk].data_ptr(), 0, 0, z0, wl["nx"], wl["ny"], nk, st)
+        g.upload(buf[:nk], origin=(0, 0, z0))
+    torch.cuda.synchronize()
+    del buf
+    torch.cuda.empty_cache()
+    g.set_transfer_function(tf, synth.TF_VMIN, synth.TF_VMAX)
+    g.set_early_termination(wl["tau"])
+    return g, cube
+
+
+def count_pass(g, vr, wl, mode, view_ids, out, cells_every):
+    """Instrumented frames (never timed): samples per view, and for every `cells_every`-th view
+    the distinct brick-store cells / 32-byte sectors its samples read (algorithmic bytes)."""
+    import torch
+    res = {}
+    for n, vi in enumerate(view_ids):
+        want_cells = cells_every > 0 and n % cells_every == 0
+        g.set_counting(2 if want_cells else 1)
+        g.render(wl["views"][vi], wl["proj"], wl["width"], wl["height"], wl["step"], mode, out)
+        torch.cuda.synchronize()
+        s = g.debug_stats()
+        assert s["overflow"] == 0
+        res[vi] = s
+    g.set_counting(0)
+    return res
+
+
+def timed_device(g, wl, mode, order, K, W, out, dist=None):
+    """K frames back to back on one stream, CUDA events at both ends, stage events inside."""
+    import torch
+    for k in range(W):
+        g.render(wl["views"][order[k % len(order)]], wl["proj"], wl["width"], wl["height"], wl["step"], mode, out)
+    g.set_timing(1)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    if dist is not None:
+        dist.barrier()
+    torch.cuda.synchronize()
+    l0 = g.launch_count()
+    e0.record()
+    for k in range(K):
+        g.render(wl["views"][order[(W + k) % len(order)]], wl["proj"], wl["width"], wl["height"], wl["step"], mode, out)
+    e1.record()
+    torch.cuda.synchronize()
+    if dist is not None:
+        dist.barrier()
+    ms = e0.elapsed_time(e1)
+    launches = g.launch_count() - l0
+    nst = min(K, 64)
+    stages = g.debug_stage_times(nst)                       # last nst frames, oldest first
+    stage_views = [order[(W + k) % len(order)] for k in range(K - nst, K)]
+    g.set_timing(0)
+    return ms, launches, stages, stage_views
+
+
+def timed_e2e(g, wl, mode, order, K, W, host_out, dist=None):
+    """Same frames through the host-buffer entry (vr_render_host): per frame the matrices go
+    host->device (as kernel arguments) and the finished RGBA frame comes back into pinned host
+    memory; both inside the timed region."""
+    import torch
+    for k in range(W):
+        g.render_host(wl["views"][order[k % len(order)]], wl["proj"], wl["width"], wl["height"], wl["step"], mode, out=host_out)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    if dist is not None:
+        dist.barrier()
+    torch.cuda.synchronize()
+    e0.record()
+    for k in range(K):
+        g.render_host(wl["views"][order[(W + k) % len(order)]], wl["proj"], wl["width"], wl["height"], wl["step"], mode, out=host_out)
+    e1.record()
+    torch.cuda.synchronize()
+    if dist is not None:
+        dist.barrier()
+    return e0.elapsed_time(e1)
+
+
+def roofline_of(counts, stages, stage_views, peak_gbs, peak_src):
+    """Ray-cast kernel (the dominant one): algorithmic bytes = 4 B x distinct brick-store cells
+    its samples read + the sub-image bytes it writes, over the views the
+    counting pass covered; duration = that kernel's device time for the same views inside the
+    timed region (library stage events on the render stream)."""
+    by_view = {}
+    for (ms_setup, ms_ray, ms_comp), vi in zip(stages, stage_views):
+        by_view.setdefault(vi, []).append(float(ms_ray))
+    alg, ms, n = 0.0, 0.0, 0
+    for vi, s in counts.items():
+        if s["cells_touched"] >= 0 and vi in by_view:
+            alg += 4.0 * s["cells_touched"] + s["subimage_bytes"]
+            ms += float(np.mean(by_view[vi]))
+            n += 1
+    if n == 0 or ms <= 0:
+        return None
+    achieved = alg / (ms * 1e-3) / 1e9
+    return {"bound": "hbm", "kernel": "vr_raycast_kernel", "achieved": round(achieved, 1), "peak": peak_gbs, "unit": "GB/s",
+            "frac": round(achieved / peak_gbs, 4), "traffic": None, "peak_source": peak_src,
+            "algorithmic_bytes_per_launch": round(alg / n), "launch_ms": round(ms / n, 4), "views_counted": n}
+
+
+def measured_peak():
+    try:
+        p = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+        return float(p["hbm_gbs"]), "MEASURED_PEAKS.json hbm_gbs (of measured)"
+    except Exception:
+        return 6650.0, "B200_PROFILING.md fallback 6.65 TB/s (of fallback)"
+
+
+# ----------------------------------------------------------------------------- oracle legs
+def oracle_volume(wl, tf):
+    """The CPU oracle as it stands (oracle/, test infrastructure) on the same seeded cube:
+    dense on the host when the cube is small, procedural voxels otherwise (no 103 GB host copy)."""
+    import oracle
+    cube = synth.Cube(wl["seed"], wl["nx"], wl["ny"], wl["nz"], wl["nsrc"], wl["ramp"])
+    nvox = wl["nx"] * wl["ny"] * wl["nz"]
+    if nvox <= 512 ** 3:
+        o = oracle.Volume(wl["nx"], wl["ny"], wl["nz"], wl["brick"], wl["ghost"], data=cube.fill_host())
+        how = "dense host cube"
+    else:
+        o = oracle.Volume(wl["nx"], wl["ny"], wl["nz"], wl["brick"], wl["ghost"], voxel_fn=cube.voxel_fn())
+        how = "procedural voxels"
+    o.set_transfer_function(tf, synth.TF_VMIN, synth.TF_VMAX)
+    o.set_early_termination(wl["tau"])
+    o._cube = cube
+    return o, how
+
+
+def sample_pixels(wl, n, salt):
+    W, H = wl["width"], wl["height"]
+    return np.array([[int(synth.u01(wl["seed"] + salt, 31, k) * W), int(synth.u01(wl["seed"] + salt, 32, k) * H)]
+                     for k in range(n)], dtype=np.int32)
+
+
+def oracle_sample_rate(o, wl, mode_id, view, npix, salt, cores):
+    """Seconds, samples taken, for `npix` seeded pixels of one view."""
+    pix = sample_pixels(wl, npix, salt)
+    t0 = time.perf_counter()
+    r = o.render(view, wl["proj"], wl["width"], wl["height"], wl["step"], mode_id, pixels=pix, nthreads=cores)
+    dt = time.perf_counter() - t0
+    return dt, int(r["counts"][:, 0].sum())
+
+
+def cpu_baseline(wl, tf, mode_id, budget_s=15.0):
+    """Oracle timed on the host cores on a bounded seeded pixel sample of the same frames,
+    extrapolated to frames/s (sample pixels -> all W*H pixels). Baseline only."""
+    cores = synth.default_threads()
+    o, how = oracle_volume(wl, tf)
+    dt, _ = oracle_sample_rate(o, wl, mode_id, wl["views"][0], 512, 1, cores)       # calibration
+    per_pixel = max(dt / 512, 1e-7)
+    views = [0, 9, 18, 27]
+    npix = int(max(256, min(wl["width"] * wl["height"], budget_s / len(views) / per_pixel)))
+    tot_t, tot_s = 0.0, 0
+    for n, vi in enumerate(views):
+        dt, ns = oracle_sample_rate(o, wl, mode_id, wl["views"][vi], npix, 2 + n, cores)
+        tot_t += dt
+        tot_s += ns
+    frame_s = tot_t / len(views) * (wl["width"] * wl["height"] / float(npix))
+    return {"value": 1.0 / frame_s, "unit": "frames/s", "cores": cores, "kind": "oracle",
+            "sample": "%d seeded pixels of each of views %s (%s), extrapolated to %dx%d pixels" % (
+                npix, views, how, wl["width"], wl["height"]),
+            "msamples_per_s": tot_s / tot_t / 1e6}
+
+
+def run_reference(args, wl, tf, mode_id):
+    """--impl reference: the oracle IS the reference arm of this tier. Each step is a bounded
+    seeded pixel sample of one frame of the cycle; value = extrapolated frames/s."""
+    cores = synth.default_threads()
+    o, how = oracle_volume(wl, tf)
+    dt, _ = oracle_sample_rate(o, wl, mode_id, wl["views"][0], 512, 1, cores)
+    per_pixel = max(dt / 512, 1e-7)
+    total = max(1, args.steps + args.warmup)
+    npix = int(max(256, min(wl["width"] * wl["height"], 90.0 / total / per_pixel)))
+    for k in range(args.warmup):
+        oracle_sample_rate(o, wl, mode_id, wl["views"][k % 36], npix, 100 + k, cores)
+    t, ns = 0.0, 0
+    for k in range(args.steps):
+        dt, s = oracle_sample_rate(o, wl, mode_id, wl["views"][(args.warmup + k) % 36], npix, 200 + k, cores)
+        t += dt
+        ns += s
+    scale = wl["width"] * wl["height"] / float(npix)
+    ms_per_step = t / args.steps * scale * 1e3
+    fps = 1e3 / ms_per_step
+    sample = "%d seeded pixels per step (%s), extrapolated to %dx%d pixels" % (npix, how, wl["width"], wl["height"])
+    return {"impl": "reference", "metric": METRIC, "value": fps, "unit": "frames/s", "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic", "config": config_of(wl, args),
+            "gsamples_per_s": ns / t / 1e9,
+            "cpu_baseline": {"value": fps, "unit": "frames/s", "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": fps, "unit": "frames/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+
+
+def config_of(wl, args):
+    return {"workload": "%s: %dx%dx%d float32 cube (noise + %d Gaussian sources%s), %d^3 bricks + %d ghost, %dx%d, %s, %s, "
+                        "step %.1f, tf %s, early termination %.2f" % (
+                            wl["name"], wl["nx"], wl["ny"], wl["nz"], wl["nsrc"], " + spectral ramp" if wl["ramp"] else "",
+                            wl["brick"], wl["ghost"], wl["width"], wl["height"], wl["view_kind"], args.mode.upper(), wl["step"],
+                            args.tf, wl["tau"]),
+            "baseline_config_index": int(wl["name"][1:]),
+            "cube_gb": round(wl["nx"] * wl["ny"] * wl["nz"] * 4 / 1e9, 2),
+            "l2_policy": "inputs larger than L2 (every frame streams a new view's share of the cube); no explicit flush",
+            "frames": "one frame per step, cycling the 36 views"}
+
+
+# ----------------------------------------------------------------------------- main
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=36)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="c3", choices=["c0", "c1", "c2", "c3"])
+    ap.add_argument("--mode", default="alpha", choices=["alpha", "mip"])
+    ap.add_argument("--tf", default="ramp", choices=["ramp", "translucent"])
+    ap.add_argument("--cells-every", type=int, default=6, help="count distinct cells on every n-th view of the cycle (0 = never)")
+    ap.add_argument("--no-variants", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    wl = workload(args.workload)
+    tf = synth.tf_ramp() if args.tf == "ramp" else synth.tf_translucent()
+    mode_id = 0 if args.mode == "alpha" else 1
+
+    if args.impl == "reference":
+        if rank == 0:
+            print(json.dumps(run_reference(args, wl, tf, mode_id)), flush=True)
+        return 0
+
+    import torch
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group(backend="nccl", device_id=torch.device("cuda", local_rank))
+
+    from paper_1205_0282_b200 import build as vr_build
+    if rank == 0:
+        vr_build.build()
+        synth._build.build()
+    if dist is not None:
+        dist.barrier()
+    import paper_1205_0282_b200 as vr
+
+    def reduce_max(x):
+        if dist is None:
+            return x
+        t = torch.tensor([x], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    t_build = time.perf_counter()
+    g, cube = build_volume(vr, wl, tf)
+    t_build = time.perf_counter() - t_build
+    W, H, K, Wm = wl["width"], wl["height"], args.steps, args.warmup
+    out = torch.empty((H, W, 4), dtype=torch.float32, device="cuda")
+    host_out = torch.empty((H, W, 4), dtype=torch.float32).pin_memory()
+    order = views_for_rank(rank, world, len(wl["views"]))
+    timed_views = sorted(set(order[(Wm + k) % len(order)] for k in range(K)))
+
+    def measure(mode, with_e2e, sampler):
+        counts = count_pass(g, vr, wl, mode, timed_views, out, args.cells_every)
+        if sampler:
+            sampler.start()
+        ms, launches, stages, stage_views = timed_device(g, wl, mode, order, K, Wm, out, dist)
+        e2e_ms = timed_e2e(g, wl, mode, order, K, Wm, host_out, dist) if with_e2e else None
+        clocks = sampler.stop() if sampler else None
+        samples = sum(counts[order[(Wm + k) % len(order)]]["samples"] for k in range(K))
+        return dict(ms=ms, launches=launches, stages=stages, stage_views=stage_views, e2e_ms=e2e_ms, clocks=clocks,
+                    samples=samples, counts=counts)
+
+    peak, peak_src = measured_peak()
+    m = measure(mode_id, True, ClockSampler(local_rank) if rank == 0 else None)
+    fps, ms_max = aggregate(m["ms"], K, world, reduce_max)
+    e2e_fps, e2e_ms_max = aggregate(m["e2e_ms"], K, world, reduce_max)
+
+    line = {"metric": METRIC, "value": round(fps, 3), "unit": "frames/s", "n_gpus": world, "steps": K, "warmup": Wm,
+            "ms_per_step": round(ms_max / K, 4), "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32", "data": "synthetic", "config": config_of(wl, args),
+            "gsamples_per_s": round(m["samples"] * world / (ms_max * 1e-3) / 1e9, 3),
+            "samples_per_frame": int(m["samples"] / K),
+            "gpu_launches": int(m["launches"]),
+            "e2e": {"value": round(e2e_fps, 3), "unit": "frames/s", "h2d_bytes_per_step": 128, "d2h_bytes_per_step": W * H * 16,
+                    "what": "vr_render_host: matrices from host memory, finished RGBA frame copied to pinned host memory every step; "
+                            "the cube stays resident in HBM (in-core rendering, PAPER.md:146,206)"},
+            "clocks": m["clocks"],
+            "stage_ms": {"setup": round(float(m["stages"][:, 0].mean()), 4), "raycast": round(float(m["stages"][:, 1].mean()), 4),
+                         "composite": round(float(m["stages"][:, 2].mean()), 4)},
+            "roofline": roofline_of(m["counts"], m["stages"], m["stage_views"], peak, peak_src),
+            "build_s": round(t_build, 1)}
+    cs = [s for s in m["counts"].values() if s["cells_touched"] >= 0]
+    if cs:
+        line["touched_per_frame"] = {"cells_gb": round(np.mean([4.0 * s["cells_touched"] for s in cs]) / 1e9, 3),
+                                     "sectors_gb": round(np.mean([32.0 * s["sectors_touched"] for s in cs]) / 1e9, 3),
+                                     "subimage_gb": round(np.mean([s["subimage_bytes"] for s in cs]) / 1e9, 4)}
+
+    if not args.no_variants and world == 1:
+        variants = []
+        for vmode, vtf in (("alpha", "translucent"), ("mip", "ramp")):
+            if vmode == args.mode and vtf == args.tf:
+                vtf = "ramp"
+            g.set_transfer_function(synth.tf_ramp() if vtf == "ramp" else synth.tf_translucent(), synth.TF_VMIN, synth.TF_VMAX)
+            v = measure(0 if vmode == "alpha" else 1, False, None)
+            variants.append({"mode": vmode, "tf": vtf, "frames_per_s": round(K / (v["ms"] * 1e-3), 3),
+                             "gsamples_per_s": round(v["samples"] / (v["ms"] * 1e-3) / 1e9, 3),
+                             "samples_per_frame": int(v["samples"] / K),
+                             "stage_ms": {"setup": round(float(v["stages"][:, 0].mean()), 4),
+                                          "raycast": round(float(v["stages"][:, 1].mean()), 4),
+                                          "composite": round(float(v["stages"][:, 2].mean()), 4)},
+                             "roofline": roofline_of(v["counts"], v["stages"], v["stage_views"], peak, peak_src)})
+        g.set_transfer_function(tf, synth.TF_VMIN, synth.TF_VMAX)
+        line["variants"] = variants
+
+    if rank == 0 and not args.no_cpu_baseline and world == 1:
+        g.close()
+        torch.cuda.empty_cache()
+        line["cpu_baseline"] = cpu_baseline(wl, tf, mode_id)
+        for k in ("value", "msamples_per_s"):
+            line["cpu_baseline"][k] = round(line["cpu_baseline"][k], 6)
+    elif rank == 0:
+        line["cpu_baseline"] = None
+    if rank == 0:
+        print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.barrier()
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

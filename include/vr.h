@@ -60,6 +60,9 @@ typedef struct vr_stats {
     int64_t rays;           /* (brick, pixel) rays started = sum of launch-rectangle areas */
     int64_t work_items;     /* (brick, 8x4-pixel tile) work items of the ray-cast kernel */
     int64_t subimage_bytes; /* bytes of brick sub-images written by the ray-cast kernel */
+    int64_t cells_touched;  /* distinct brick-store cells (float32 voxels) the frame's samples
+                               read, and distinct 32-byte sectors (8 consecutive cells) they */
+    int64_t sectors_touched;/* fall in; valid only with vr_set_counting(v, 2), else -1 */
     int32_t nbricks;
     int32_t overflow;       /* 1 if the view needed more sub-image scratch than was reserved
                                (frame is then incomplete; never happens unless the host and
@@ -80,7 +83,7 @@ typedef struct vr_stats {
 
 /* Create a volume of nx*ny*nz float32 voxels split into a regular grid of brick^3 cores
  * (ceil(n/brick) per axis, ragged at the high edges). Allocates grid-many padded bricks of
- * (brick+2*ghost)^3 floats in device memory, zero-filled.
+ * (min(brick, max(nx,ny,nz)) + 2*ghost)^3 floats in device memory, zero-filled.
  *   nx,ny,nz > 0; brick >= 2; 0 <= ghost <= 8 (ghost = 0 is allowed: seams are then expected).
  *   out (host): receives the handle. Errors: VR_ERR_INVALID_ARG, VR_ERR_OUT_OF_MEMORY,
  *   VR_ERR_CUDA (no device). On error *out = NULL. */
@@ -197,8 +200,10 @@ int vr_debug_ray_bricks(vr_volume* v, const float* view, const float* proj, int 
  * for "no sample". Bricks whose rectangle does not contain the pixel give zeros / -inf. */
 int vr_debug_subimages(vr_volume* v, const int* pixels, int npix, float* sub_out);
 
-/* Enable (1) / disable (0) counting of samples in the ray-cast kernel (an instrumented
- * variant of the same kernel: slower, never used for timed runs). */
+/* Counting in the ray-cast kernel (an instrumented variant of the same kernel: slower, never
+ * used for timed runs): 0 = off, 1 = count samples, 2 = count samples and keep a bitmap of
+ * the brick-store cells read (1 bit per cell of extra device memory), from which
+ * vr_debug_stats reports the frame's distinct cells and 32-byte sectors. */
 int vr_set_counting(vr_volume* v, int enable);
 
 /* Enable (1) / disable (0) CUDA-event timing of the three stages on the render's stream. */
@@ -206,6 +211,12 @@ int vr_set_timing(vr_volume* v, int enable);
 
 /* Counters (and stage times) of the most recent vr_render. Synchronises. */
 int vr_debug_stats(vr_volume* v, vr_stats* out);
+
+/* Device times (ms) of set-up, ray casting and compositing of the last `nframes` frames
+ * rendered since vr_set_timing(v, 1), oldest first: ms_out (host) float[nframes*3],
+ * 1 <= nframes <= 64. Lets a caller time frames back to back without synchronising between
+ * them and read every frame's stage times afterwards. Synchronises. */
+int vr_debug_stage_times(vr_volume* v, int nframes, float* ms_out);
 
 /* Number of kernel launches the library has issued on this handle since creation. */
 int64_t vr_launch_count(const vr_volume* v);

@@ -26,7 +26,7 @@ SYMBOLS = (
     "vr_volume_create", "vr_volume_destroy", "vr_volume_upload", "vr_volume_download", "vr_debug_brick_data",
     "vr_set_transfer_function", "vr_set_early_termination", "vr_render", "vr_render_host", "vr_composite",
     "vr_num_bricks", "vr_debug_brick_order", "vr_debug_rects", "vr_debug_ray_bricks", "vr_debug_subimages",
-    "vr_set_counting", "vr_set_timing", "vr_debug_stats", "vr_launch_count", "vr_last_error",
+    "vr_set_counting", "vr_set_timing", "vr_debug_stats", "vr_debug_stage_times", "vr_launch_count", "vr_last_error",
 )
 
 
@@ -38,7 +38,8 @@ class VrError(RuntimeError):
 
 class Stats(ctypes.Structure):
     _fields_ = [("samples", ctypes.c_int64), ("rays", ctypes.c_int64), ("work_items", ctypes.c_int64),
-                ("subimage_bytes", ctypes.c_int64), ("nbricks", ctypes.c_int32), ("overflow", ctypes.c_int32),
+                ("subimage_bytes", ctypes.c_int64), ("cells_touched", ctypes.c_int64), ("sectors_touched", ctypes.c_int64),
+                ("nbricks", ctypes.c_int32), ("overflow", ctypes.c_int32),
                 ("ms_setup", ctypes.c_float), ("ms_raycast", ctypes.c_float), ("ms_composite", ctypes.c_float)]
 
 
@@ -73,6 +74,7 @@ def lib():
         L.vr_set_counting.argtypes = [vp, ci]
         L.vr_set_timing.argtypes = [vp, ci]
         L.vr_debug_stats.argtypes = [vp, ctypes.POINTER(Stats)]
+        L.vr_debug_stage_times.argtypes = [vp, ci, vp]
         L.vr_launch_count.argtypes = [vp]
         L.vr_launch_count.restype = i64
         L.vr_last_error.argtypes = [vp]
@@ -219,8 +221,9 @@ class Volume:
         self._check(lib().vr_debug_subimages(self._h, pix.ctypes.data, pix.shape[0], out.ctypes.data))
         return out
 
-    def set_counting(self, enable):
-        self._check(lib().vr_set_counting(self._h, int(bool(enable))))
+    def set_counting(self, mode):
+        """0 off, 1 count samples, 2 also track the distinct cells / sectors read."""
+        self._check(lib().vr_set_counting(self._h, int(mode)))
 
     def set_timing(self, enable):
         self._check(lib().vr_set_timing(self._h, int(bool(enable))))
@@ -229,6 +232,12 @@ class Volume:
         s = Stats()
         self._check(lib().vr_debug_stats(self._h, ctypes.byref(s)))
         return {k: getattr(s, k) for k, _ in Stats._fields_}
+
+    def debug_stage_times(self, nframes):
+        """[nframes][3] ms of (set-up, ray cast, compositing) of the last nframes timed frames."""
+        out = np.empty((int(nframes), 3), dtype=np.float32)
+        self._check(lib().vr_debug_stage_times(self._h, int(nframes), out.ctypes.data))
+        return out
 
     def launch_count(self):
         return int(lib().vr_launch_count(self._h))

@@ -34,9 +34,13 @@ struct vr_volume {
     float* d_stage;          /* staging for VR_HOST upload / download */
     long long stage_floats;
     int ctas;                /* persistent grid of the ray-cast kernel */
-    bool counting, timing;
-    cudaEvent_t ev[4];
-    bool ev_valid;           /* the four events were recorded by the last render */
+    int counting;            /* 0 off, 1 samples, 2 samples + touched-cells bitmap */
+    bool timing;
+    unsigned* d_bitmap;      /* one bit per brick-store cell (counting == 2) */
+    long long bitmap_words;
+    unsigned long long* d_counts2;
+    cudaEvent_t ev[VR_EV_RING][4]; /* stage boundaries of the last VR_EV_RING timed frames */
+    long long timed_frames;  /* frames rendered since timing was switched on */
     int last_W, last_H, last_mode;
     bool last_valid;
     int64_t launches;
@@ -82,8 +86,11 @@ static void release(vr_volume* v) {
     cudaFree(v->d_sub);
     cudaFree(v->d_frame);
     cudaFree(v->d_stage);
-    for (int i = 0; i < 4; ++i)
-        if (v->ev[i]) cudaEventDestroy(v->ev[i]);
+    cudaFree(v->d_bitmap);
+    cudaFree(v->d_counts2);
+    for (int r = 0; r < VR_EV_RING; ++r)
+        for (int i = 0; i < 4; ++i)
+            if (v->ev[r][i]) cudaEventDestroy(v->ev[r][i]);
     cudaGetLastError();
     delete v;
 }
@@ -148,7 +155,8 @@ extern "C" int vr_volume_create(int nx, int ny, int nz, int brick, int ghost, vr
     if (e == cudaSuccess) e = cudaMalloc(&v->d_order, sizeof(int) * g.nbricks);
     if (e == cudaSuccess) e = cudaMalloc(&v->d_item_prefix, sizeof(int) * (g.nbricks + 1));
     if (e == cudaSuccess) e = cudaMalloc(&v->d_layers, sizeof(VrCompLayer) * g.nbricks);
-    for (int i = 0; i < 4 && e == cudaSuccess; ++i) e = cudaEventCreate(&v->ev[i]);
+    for (int r = 0; r < VR_EV_RING && e == cudaSuccess; ++r)
+        for (int i = 0; i < 4 && e == cudaSuccess; ++i) e = cudaEventCreate(&v->ev[r][i]);
     if (e != cudaSuccess) {
         cudaGetLastError();
         const int st = (e == cudaErrorMemoryAllocation) ? VR_ERR_OUT_OF_MEMORY : VR_ERR_CUDA;
@@ -318,14 +326,21 @@ extern "C" int vr_set_early_termination(vr_volume* v, float tau) {
 
 extern "C" int vr_set_counting(vr_volume* v, int enable) {
     if (!v) return fail(NULL, VR_ERR_INVALID_ARG, "vr_set_counting: NULL handle");
-    v->counting = enable != 0;
+    if (enable < 0 || enable > 2) return fail(v, VR_ERR_INVALID_ARG, "vr_set_counting: mode %d outside [0,2]", enable);
+    if (enable == 2 && !v->d_bitmap) {
+        const long long words = (v->grid.slot * v->grid.nbricks + 31) / 32;
+        VR_CUDA(v, cudaMalloc(&v->d_bitmap, (size_t)words * sizeof(unsigned)));
+        VR_CUDA(v, cudaMalloc(&v->d_counts2, 2 * sizeof(unsigned long long)));
+        v->bitmap_words = words;
+    }
+    v->counting = enable;
     return VR_OK;
 }
 
 extern "C" int vr_set_timing(vr_volume* v, int enable) {
     if (!v) return fail(NULL, VR_ERR_INVALID_ARG, "vr_set_timing: NULL handle");
     v->timing = enable != 0;
-    v->ev_valid = false;
+    v->timed_frames = 0;
     return VR_OK;
 }
 
@@ -381,11 +396,12 @@ extern "C" int vr_render(vr_volume* v, const float* view, const float* proj, int
     if (rc) return rc;
     cudaStream_t st = (cudaStream_t)stream;
     const bool timing = v->timing;
+    cudaEvent_t* ev = v->ev[v->timed_frames % VR_EV_RING];
 
-    if (timing) VR_CUDA(v, cudaEventRecord(v->ev[0], st));
+    if (timing) VR_CUDA(v, cudaEventRecord(ev[0], st));
     rc = run_setup(v, view, proj, width, height, mode, st);
     if (rc) return rc;
-    if (timing) VR_CUDA(v, cudaEventRecord(v->ev[1], st));
+    if (timing) VR_CUDA(v, cudaEventRecord(ev[1], st));
 
     VrRaycastParams p;
     p.grid = v->grid;
@@ -396,6 +412,11 @@ extern "C" int vr_render(vr_volume* v, const float* view, const float* proj, int
     p.item_prefix = v->d_item_prefix;
     p.vs_rw = v->d_vs;
     p.sub = v->d_sub;
+    p.bitmap = NULL;
+    if (v->counting == 2) {
+        VR_CUDA(v, cudaMemsetAsync(v->d_bitmap, 0, (size_t)v->bitmap_words * sizeof(unsigned), st));
+        p.bitmap = v->d_bitmap;
+    }
     p.lut = v->lut;
     p.step = (double)step;
     p.tau = v->tau;
@@ -403,15 +424,15 @@ extern "C" int vr_render(vr_volume* v, const float* view, const float* proj, int
     long long ctas = v->ctas;
     const long long want = (items + (VR_RAYCAST_THREADS / 32) - 1) / (VR_RAYCAST_THREADS / 32);
     if (ctas > want) ctas = want < 1 ? 1 : want;
-    VR_CUDA(v, vr_launch_raycast(p, (int)ctas, v->counting, st));
+    VR_CUDA(v, vr_launch_raycast(p, (int)ctas, v->counting != 0, st));
     v->launches++;
-    if (timing) VR_CUDA(v, cudaEventRecord(v->ev[2], st));
+    if (timing) VR_CUDA(v, cudaEventRecord(ev[2], st));
 
     VR_CUDA(v, vr_launch_composite(v->d_layers, v->d_order, v->grid.nbricks, width, height, mode, v->lut, out_rgba, st));
     v->launches++;
     if (timing) {
-        VR_CUDA(v, cudaEventRecord(v->ev[3], st));
-        v->ev_valid = true;
+        VR_CUDA(v, cudaEventRecord(ev[3], st));
+        v->timed_frames++;
     }
     v->last_W = width;
     v->last_H = height;
@@ -600,13 +621,38 @@ extern "C" int vr_debug_stats(vr_volume* v, vr_stats* out) {
     out->rays = (int64_t)vs.total_sub_pixels;
     out->work_items = vs.total_items;
     out->subimage_bytes = (int64_t)vs.total_sub_pixels * (v->last_mode == VR_ALPHA ? 16 : 4);
+    out->cells_touched = out->sectors_touched = -1;
+    if (v->counting == 2) {
+        unsigned long long c2[2] = {0, 0};
+        VR_CUDA(v, cudaMemset(v->d_counts2, 0, sizeof(c2)));
+        VR_CUDA(v, vr_launch_count_bits(v->d_bitmap, v->bitmap_words, v->d_counts2, 0));
+        v->launches++;
+        VR_CUDA(v, cudaMemcpy(c2, v->d_counts2, sizeof(c2), cudaMemcpyDeviceToHost));
+        out->cells_touched = (int64_t)c2[0];
+        out->sectors_touched = (int64_t)c2[1];
+    }
     out->nbricks = v->grid.nbricks;
     out->overflow = vs.overflow;
     out->ms_setup = out->ms_raycast = out->ms_composite = -1.0f;
-    if (v->timing && v->ev_valid) {
-        VR_CUDA(v, cudaEventElapsedTime(&out->ms_setup, v->ev[0], v->ev[1]));
-        VR_CUDA(v, cudaEventElapsedTime(&out->ms_raycast, v->ev[1], v->ev[2]));
-        VR_CUDA(v, cudaEventElapsedTime(&out->ms_composite, v->ev[2], v->ev[3]));
+    if (v->timing && v->timed_frames > 0) {
+        cudaEvent_t* ev = v->ev[(v->timed_frames - 1) % VR_EV_RING];
+        VR_CUDA(v, cudaEventElapsedTime(&out->ms_setup, ev[0], ev[1]));
+        VR_CUDA(v, cudaEventElapsedTime(&out->ms_raycast, ev[1], ev[2]));
+        VR_CUDA(v, cudaEventElapsedTime(&out->ms_composite, ev[2], ev[3]));
+    }
+    return VR_OK;
+}
+
+extern "C" int vr_debug_stage_times(vr_volume* v, int nframes, float* ms_out) {
+    if (!v) return fail(NULL, VR_ERR_INVALID_ARG, "vr_debug_stage_times: NULL handle");
+    if (!ms_out || nframes <= 0 || nframes > VR_EV_RING)
+        return fail(v, VR_ERR_INVALID_ARG, "vr_debug_stage_times: need 1 <= nframes <= %d and an output", VR_EV_RING);
+    if (!v->timing || v->timed_frames < nframes)
+        return fail(v, VR_ERR_STATE, "vr_debug_stage_times: only %lld frames rendered since vr_set_timing(1)", v->timed_frames);
+    VR_CUDA(v, cudaDeviceSynchronize());
+    for (int f = 0; f < nframes; ++f) {
+        cudaEvent_t* ev = v->ev[(v->timed_frames - nframes + f) % VR_EV_RING];
+        for (int s3 = 0; s3 < 3; ++s3) VR_CUDA(v, cudaEventElapsedTime(ms_out + 3 * f + s3, ev[s3], ev[s3 + 1]));
     }
     return VR_OK;
 }

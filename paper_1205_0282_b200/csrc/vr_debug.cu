@@ -164,3 +164,27 @@ cudaError_t vr_launch_gather_sub(const VrBrickView* bv, int nbricks, const void*
                                                                      reinterpret_cast<float4*>(d_out));
     return cudaGetLastError();
 }
+
+/* Touched-cells bitmap (bench instrumentation): out2[0] += set bits (distinct brick-store
+ * cells read), out2[1] += non-zero bytes (distinct 32-byte sectors: 8 consecutive cells). */
+__global__ void vr_count_bits_kernel(const unsigned* __restrict__ bitmap, long long words, unsigned long long* __restrict__ out2) {
+    unsigned long long cells = 0, sectors = 0;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < words; i += (long long)gridDim.x * blockDim.x) {
+        const unsigned w = bitmap[i];
+        cells += __popc(w);
+        sectors += ((w & 0xffu) != 0) + ((w & 0xff00u) != 0) + ((w & 0xff0000u) != 0) + ((w & 0xff000000u) != 0);
+    }
+    for (int o = 16; o > 0; o >>= 1) {
+        cells += __shfl_xor_sync(0xffffffffu, cells, o);
+        sectors += __shfl_xor_sync(0xffffffffu, sectors, o);
+    }
+    if ((threadIdx.x & 31) == 0) {
+        atomicAdd(out2, cells);
+        atomicAdd(out2 + 1, sectors);
+    }
+}
+
+cudaError_t vr_launch_count_bits(const unsigned* bitmap, long long words, unsigned long long* d_out2, cudaStream_t st) {
+    vr_count_bits_kernel<<<148 * 8, 256, 0, st>>>(bitmap, words, d_out2);
+    return cudaGetLastError();
+}

@@ -27,6 +27,7 @@
 #define VR_RAYCAST_THREADS 256
 #define VR_COMP_TILE_W 32
 #define VR_COMP_TILE_H 8
+#define VR_EV_RING 64 /* timed frames whose stage events are kept */
 
 struct VrGrid {
     int n[3];     /* nx, ny, nz */
@@ -93,6 +94,7 @@ struct VrRaycastParams {
     const int* item_prefix;
     VrViewState* vs_rw; /* work counter, sample counter */
     void* sub;          /* float4[] (ALPHA) or float[] (MIP) */
+    unsigned* bitmap;   /* counting variant only: one bit per brick-store cell, or NULL */
     VrLut lut;
     double step;
     float tau;
@@ -115,6 +117,7 @@ cudaError_t vr_launch_ray_bricks(const VrGrid& grid, const VrViewState* vs, cons
                                  cudaStream_t st);
 cudaError_t vr_launch_gather_sub(const VrBrickView* bv, int nbricks, const void* sub, int mode, const int* d_pixels,
                                  int npix, float* d_out, cudaStream_t st);
+cudaError_t vr_launch_count_bits(const unsigned* bitmap, long long words, unsigned long long* d_out2, cudaStream_t st);
 int vr_raycast_ctas(); /* persistent grid size: resident CTAs per SM x SM count */
 
 /* host mirror of the set-up arithmetic, for argument validation and scratch sizing only */

@@ -225,8 +225,14 @@ __device__ __forceinline__ long long to_fixed(double x) { return __double2ll_rn(
 
 /* Tri-linear interpolation (R3) at a fixed-point brick-local position. PT > 0: the padded
  * edge is a compile-time constant so the 8 loads share one address register pair. */
-template <int PT, bool CLAMP>
-__device__ __forceinline__ float trilinear(const float* __restrict__ brick, int P, const int ext[3], const Lattice& L) {
+/* Instrumented variant only: mark brick-store cell `cell` in the touched-cells bitmap. */
+__device__ __forceinline__ void mark_cell(unsigned* __restrict__ bitmap, long long cell) {
+    atomicOr(bitmap + (cell >> 5), 1u << (unsigned)(cell & 31));
+}
+
+template <int PT, bool CLAMP, bool COUNT>
+__device__ __forceinline__ float trilinear(const float* __restrict__ brick, int P, const int ext[3], const Lattice& L,
+                                           unsigned* __restrict__ bitmap, long long brick_cell0) {
     const int Pe = PT > 0 ? PT : P;
     int ix = (int)(L.q[0] >> 32), iy = (int)(L.q[1] >> 32), iz = (int)(L.q[2] >> 32);
     const float fx = __uint_as_float(0x3F800000u | ((unsigned)L.q[0] >> 9)) - 1.0f;
@@ -243,6 +249,17 @@ __device__ __forceinline__ float trilinear(const float* __restrict__ brick, int 
         c101 = __ldg(p + Pe * Pe + 1);
         c110 = __ldg(p + Pe * Pe + Pe);
         c111 = __ldg(p + Pe * Pe + Pe + 1);
+        if (COUNT && bitmap) {
+            const long long c = brick_cell0 + (p - brick);
+            mark_cell(bitmap, c);
+            mark_cell(bitmap, c + 1);
+            mark_cell(bitmap, c + Pe);
+            mark_cell(bitmap, c + Pe + 1);
+            mark_cell(bitmap, c + Pe * Pe);
+            mark_cell(bitmap, c + Pe * Pe + 1);
+            mark_cell(bitmap, c + Pe * Pe + Pe);
+            mark_cell(bitmap, c + Pe * Pe + Pe + 1);
+        }
     } else {
         /* ghost = 0: indices leaving the brick's own cells are clamped into them (seams) */
         const int x0 = min(max(ix, 0), ext[0] - 1), x1 = min(max(ix + 1, 0), ext[0] - 1);
@@ -258,6 +275,16 @@ __device__ __forceinline__ float trilinear(const float* __restrict__ brick, int 
         c101 = __ldg(brick + r10 + x1);
         c110 = __ldg(brick + r11 + x0);
         c111 = __ldg(brick + r11 + x1);
+        if (COUNT && bitmap) {
+            mark_cell(bitmap, brick_cell0 + r00 + x0);
+            mark_cell(bitmap, brick_cell0 + r00 + x1);
+            mark_cell(bitmap, brick_cell0 + r01 + x0);
+            mark_cell(bitmap, brick_cell0 + r01 + x1);
+            mark_cell(bitmap, brick_cell0 + r10 + x0);
+            mark_cell(bitmap, brick_cell0 + r10 + x1);
+            mark_cell(bitmap, brick_cell0 + r11 + x0);
+            mark_cell(bitmap, brick_cell0 + r11 + x1);
+        }
     }
     const float c00 = fmaf(fx, c001 - c000, c000);
     const float c01 = fmaf(fx, c011 - c010, c010);
@@ -383,7 +410,7 @@ vr_raycast_kernel(const VrRaycastParams prm) {
         bool active = n > 0 && !stopped;
         while (__any_sync(FULL_MASK, active)) {
             if (active) {
-                const float v = trilinear<PT, CLAMP>(brick, g.P, ext, L);
+                const float v = trilinear<PT, CLAMP, COUNT>(brick, g.P, ext, L, prm.bitmap, (long long)b * g.slot);
                 if (COUNT) ++nsamples;
                 if (MODE == VR_MIP) {
                     acc.r = fmaxf(acc.r, v);
@@ -410,7 +437,7 @@ vr_raycast_kernel(const VrRaycastParams prm) {
                     const double p = VR_FMA(s, ray.d[a], ray.o[a]);
                     L.q[a] = to_fixed(p - ((double)(blo[a] - g.ghost) + 0.5));
                 }
-                const float v = trilinear<PT, CLAMP>(brick, g.P, ext, L);
+                const float v = trilinear<PT, CLAMP, COUNT>(brick, g.P, ext, L, prm.bitmap, (long long)b * g.slot);
                 if (COUNT) ++nsamples;
                 if (MODE == VR_MIP) {
                     acc.r = fmaxf(acc.r, v);
