@@ -7,6 +7,7 @@
 #include <math.h>
 #include <stdarg.h>
 #include <stdio.h>
+#include <stdlib.h>
 #include <string.h>
 
 #include <new>
@@ -164,6 +165,10 @@ extern "C" int vr_volume_create(int nx, int ny, int nz, int brick, int ghost, vr
              (double)g.slot * g.nbricks * 4.0 / 1e9);
         release(v);
         return st;
+    }
+    if (const char* e = getenv("VR_L2_FETCH_GRANULARITY")) { /* experiment knob: 32, 64 or 128 bytes */
+        cudaDeviceSetLimit(cudaLimitMaxL2FetchGranularity, (size_t)atoi(e));
+        cudaGetLastError();
     }
     v->ctas = vr_raycast_ctas();
     if (v->ctas <= 0) {
