@@ -1,0 +1,116 @@
+"""GPU parity at BASELINE.json's full sizes, in the launch configuration bench.py times
+(bench.workload / bench.build_volume): seeded pixel samples the oracle computes one by one
+(procedural voxels for the 4 GB and 103 GB cubes), plus the exact integer results per view."""
+import numpy as np
+import pytest
+
+import bench
+import oracle
+import synth
+from helpers import check_alpha, check_mip, gpu_frame, seeded_pixels
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def vr(cuda_device):
+    from paper_1205_0282_b200 import build
+    build.build()
+    import paper_1205_0282_b200 as vr
+    return vr
+
+
+def pair(vr, name, tf):
+    import torch
+    wl = bench.workload(name)
+    g, cube = bench.build_volume(vr, wl, tf)
+    if wl["nx"] * wl["ny"] * wl["nz"] <= 512 ** 3:
+        o = oracle.Volume(wl["nx"], wl["ny"], wl["nz"], wl["brick"], wl["ghost"], data=cube.fill_host())
+    else:
+        o = oracle.Volume(wl["nx"], wl["ny"], wl["nz"], wl["brick"], wl["ghost"], voxel_fn=cube.voxel_fn())
+    o.set_transfer_function(tf, synth.TF_VMIN, synth.TF_VMAX)
+    o.set_early_termination(wl["tau"])
+    torch.cuda.synchronize()
+    return wl, g, o, cube
+
+
+def check_views(vr, wl, g, o, view_ids, npix, modes, tau):
+    W, H = wl["width"], wl["height"]
+    for vi in view_ids:
+        view, proj = wl["views"][vi], wl["proj"]
+        assert np.array_equal(g.debug_brick_order(view, proj), o.brick_order(view, proj))
+        assert np.array_equal(g.debug_rects(view, proj, W, H), o.rects(view, proj, W, H))
+        pix = seeded_pixels(1000 + vi, W, H, npix)
+        gc, gl, gg = g.debug_ray_bricks(view, proj, W, H, pix, maxlen=32)
+        oc, ol, og = o.ray_bricks(view, proj, W, H, pix, maxlen=32)
+        ok = (gg == 0) & (og == 0)
+        assert ok.mean() > 0.99 and np.array_equal(gc[ok], oc[ok]) and np.array_equal(gl[ok], ol[ok])
+        for mode in modes:
+            img = gpu_frame(g, view, proj, W, H, wl["step"], mode)[pix[:, 1], pix[:, 0]]
+            ref = o.render(view, proj, W, H, wl["step"], mode, pixels=pix)
+            assert (ref["counts"][:, 0] > 0).mean() > 0.05  # the sample is not all background
+            if mode == vr.ALPHA:
+                check_alpha(img, ref["image"], ref["flags"], tau, "%s view %d" % (wl["name"], vi))
+            else:
+                check_mip(img, ref["image"], "%s view %d" % (wl["name"], vi))
+
+
+def test_config1_512cube_8_bricks(vr):
+    wl, g, o, cube = pair(vr, "c1", synth.tf_ramp())
+    # the device generator and the host generator made the same cube
+    back = np.empty((3, wl["ny"], wl["nx"]), dtype=np.float32)
+    g.download(back, origin=(0, 0, 255))
+    assert np.array_equal(back, cube.fill_host(0, 0, 255, wl["nx"], wl["ny"], 3))
+    check_views(vr, wl, g, o, (0, 7, 20), 3000, (vr.ALPHA,), 0.99)
+    g.set_transfer_function(synth.tf_translucent(), synth.TF_VMIN, synth.TF_VMAX)
+    o.set_transfer_function(synth.tf_translucent(), synth.TF_VMIN, synth.TF_VMAX)
+    check_views(vr, wl, g, o, (13,), 2000, (vr.ALPHA, vr.MIP), 0.99)
+
+
+def test_config2_1024cube_64_bricks(vr):
+    wl, g, o, cube = pair(vr, "c2", synth.tf_ramp())
+    check_views(vr, wl, g, o, (0, 5, 17), 1500, (vr.ALPHA, vr.MIP), 0.99)
+
+
+def test_config3_103GB_cube_192_bricks(vr):
+    import torch
+    free, total = torch.cuda.mem_get_info()
+    if free < 120e9:
+        pytest.skip("needs ~110 GB of free device memory")
+    wl, g, o, cube = pair(vr, "c3", synth.tf_ramp())
+    check_views(vr, wl, g, o, (0, 11), 1500, (vr.ALPHA, vr.MIP), 0.99)
+    g.set_transfer_function(synth.tf_translucent(), synth.TF_VMIN, synth.TF_VMAX)
+    o.set_transfer_function(synth.tf_translucent(), synth.TF_VMIN, synth.TF_VMAX)
+    check_views(vr, wl, g, o, (23,), 1000, (vr.ALPHA,), 0.99)
+    # spot-check the brick store itself against the procedural voxels (interior, seam and far corner)
+    for (x, y, z) in ((0, 0, 0), (511, 512, 513), (4095, 4095, 1535), (2047, 1024, 1000)):
+        box = np.empty((1, 1, 2 if x < 4095 else 1), dtype=np.float32)
+        g.download(box, origin=(x, y, z))
+        assert box[0, 0, 0] == np.float32(cube.voxel(x, y, z))
+    g.close()
+
+
+def test_composite_microbenchmark_shape(vr):
+    """c4's compositing case at reduced layer count: full-frame 4096^2 layers, seeded order."""
+    import torch
+    W = H = 4096
+    n = 6
+    layers = []
+    for l in range(n):
+        t = torch.empty((H, W, 4), dtype=torch.float32, device="cuda")
+        synth.layer_device(synth.BASE_SEED + 4, l, 0, W * H, t.data_ptr(), torch.cuda.current_stream().cuda_stream)
+        layers.append(t)
+    rects = [(0, 0, W, H)] * n
+    order = synth.permutation(synth.BASE_SEED + 4, n)
+    out = torch.empty((H, W, 4), dtype=torch.float32, device="cuda")
+    vr.composite(layers, rects, order, W, H, out)
+    torch.cuda.synchronize()
+    pix = seeded_pixels(5, W, H, 4000)
+    # the oracle composites the same pixels from host copies of the same seeded layers
+    lin = (pix[:, 1].astype(np.int64) * W + pix[:, 0])
+    ref = np.zeros((len(pix), 4))
+    for q, p in enumerate(lin):
+        host_layers = [synth.layer_host(synth.BASE_SEED + 4, l, int(p), 1).reshape(1, 1, 4) for l in range(n)]
+        ref[q] = oracle.composite(host_layers, [(0, 0, 1, 1)] * n, order, 1, 1)[0, 0]
+    got = out.cpu().numpy()[pix[:, 1], pix[:, 0]]
+    assert np.abs(got - ref).max() < 1e-5
