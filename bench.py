@@ -433,6 +433,7 @@ def main():
     if cs:
         line["touched_per_frame"] = {"cells_gb": round(np.mean([4.0 * s["cells_touched"] for s in cs]) / 1e9, 3),
                                      "sectors_gb": round(np.mean([32.0 * s["sectors_touched"] for s in cs]) / 1e9, 3),
+                                     "lines_gb": round(np.mean([128.0 * s["lines_touched"] for s in cs]) / 1e9, 3),
                                      "subimage_gb": round(np.mean([s["subimage_bytes"] for s in cs]) / 1e9, 4)}
 
     if not args.no_variants and world == 1:

@@ -50,6 +50,13 @@ typedef enum vr_status {
 
 enum { VR_ALPHA = 0, VR_MIP = 1 };   /* vr_render mode */
 enum { VR_HOST = 0, VR_DEVICE = 1 }; /* memory space of a data pointer */
+/* Layout of a ghost-padded brick in HBM (north_star: "a tiled linear layout ... whichever ncu
+ * shows is faster"). LINEAR: rows of P = brick + 2*ghost cells, x fastest. TILED: 4x4x2-cell
+ * micro-tiles of 32 floats = one 128-byte DRAM line each, tiles x fastest, so that the 2x2x2
+ * neighbourhoods of consecutive samples of a ray fall into few lines. DEFAULT = TILED (the
+ * faster one on every config measured, see DESIGN.md and profiles/). Results do not depend
+ * on the layout. */
+enum { VR_LAYOUT_DEFAULT = 0, VR_LAYOUT_LINEAR = 1, VR_LAYOUT_TILED = 2 };
 
 typedef struct vr_volume vr_volume; /* opaque */
 
@@ -63,6 +70,8 @@ typedef struct vr_stats {
     int64_t cells_touched;  /* distinct brick-store cells (float32 voxels) the frame's samples
                                read, and distinct 32-byte sectors (8 consecutive cells) they */
     int64_t sectors_touched;/* fall in; valid only with vr_set_counting(v, 2), else -1 */
+    int64_t lines_touched;  /* distinct 128-byte lines (32 consecutive cells) of the brick store
+                               they fall in; valid only with vr_set_counting(v, 2), else -1 */
     int32_t nbricks;
     int32_t overflow;       /* 1 if the view needed more sub-image scratch than was reserved
                                (frame is then incomplete; never happens unless the host and
@@ -88,6 +97,12 @@ typedef struct vr_stats {
  *   out (host): receives the handle. Errors: VR_ERR_INVALID_ARG, VR_ERR_OUT_OF_MEMORY,
  *   VR_ERR_CUDA (no device). On error *out = NULL. */
 int vr_volume_create(int nx, int ny, int nz, int brick, int ghost, vr_volume** out);
+
+/* Same, with the brick layout chosen by the caller (VR_LAYOUT_*): vr_volume_create is this
+ * call with VR_LAYOUT_DEFAULT. A TILED slot is padded to whole micro-tiles per axis (514^3
+ * cells -> 516 x 516 x 514, +0.8 %). Errors as above, plus VR_ERR_INVALID_ARG for an unknown
+ * layout. */
+int vr_volume_create_layout(int nx, int ny, int nz, int brick, int ghost, int layout, vr_volume** out);
 
 /* Free everything the library allocated for the handle (synchronises the device). NULL ok. */
 void vr_volume_destroy(vr_volume* v);

@@ -15,6 +15,7 @@ import numpy as np
 
 ALPHA, MIP = 0, 1
 HOST, DEVICE = 0, 1
+LAYOUT_DEFAULT, LAYOUT_LINEAR, LAYOUT_TILED = 0, 1, 2
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libvr.so")
@@ -23,7 +24,7 @@ STATUS = {0: "VR_OK", 1: "VR_ERR_INVALID_ARG", 2: "VR_ERR_OUT_OF_MEMORY", 3: "VR
 
 # every symbol include/vr.h declares (tests check the library exports each of them)
 SYMBOLS = (
-    "vr_volume_create", "vr_volume_destroy", "vr_volume_upload", "vr_volume_download", "vr_debug_brick_data",
+    "vr_volume_create", "vr_volume_create_layout", "vr_volume_destroy", "vr_volume_upload", "vr_volume_download", "vr_debug_brick_data",
     "vr_set_transfer_function", "vr_set_early_termination", "vr_render", "vr_render_host", "vr_composite",
     "vr_num_bricks", "vr_debug_brick_order", "vr_debug_rects", "vr_debug_ray_bricks", "vr_debug_subimages",
     "vr_set_counting", "vr_set_timing", "vr_debug_stats", "vr_debug_stage_times", "vr_launch_count", "vr_last_error",
@@ -39,6 +40,7 @@ class VrError(RuntimeError):
 class Stats(ctypes.Structure):
     _fields_ = [("samples", ctypes.c_int64), ("rays", ctypes.c_int64), ("work_items", ctypes.c_int64),
                 ("subimage_bytes", ctypes.c_int64), ("cells_touched", ctypes.c_int64), ("sectors_touched", ctypes.c_int64),
+                ("lines_touched", ctypes.c_int64),
                 ("nbricks", ctypes.c_int32), ("overflow", ctypes.c_int32),
                 ("ms_setup", ctypes.c_float), ("ms_raycast", ctypes.c_float), ("ms_composite", ctypes.c_float)]
 
@@ -56,6 +58,7 @@ def lib():
         L = ctypes.CDLL(LIB_PATH)
         vp, ci, cf, i64 = ctypes.c_void_p, ctypes.c_int, ctypes.c_float, ctypes.c_int64
         L.vr_volume_create.argtypes = [ci, ci, ci, ci, ci, ctypes.POINTER(vp)]
+        L.vr_volume_create_layout.argtypes = [ci, ci, ci, ci, ci, ci, ctypes.POINTER(vp)]
         L.vr_volume_destroy.argtypes = [vp]
         L.vr_volume_destroy.restype = None
         L.vr_volume_upload.argtypes = [vp, vp, ci, ci, ci, ci, ci, ci, ci, vp]
@@ -101,10 +104,15 @@ def _pixels(pixels):
 class Volume:
     """Handle of a bricked volume in HBM (vr_volume_create ... vr_volume_destroy)."""
 
-    def __init__(self, nx, ny, nz, brick, ghost=1):
+    def __init__(self, nx, ny, nz, brick, ghost=1, layout=LAYOUT_DEFAULT):
         self._h = ctypes.c_void_p()
         self.nx, self.ny, self.nz, self.brick, self.ghost = int(nx), int(ny), int(nz), int(brick), int(ghost)
-        rc = lib().vr_volume_create(self.nx, self.ny, self.nz, self.brick, self.ghost, ctypes.byref(self._h))
+        self.layout = int(layout)
+        if self.layout == LAYOUT_DEFAULT:
+            rc = lib().vr_volume_create(self.nx, self.ny, self.nz, self.brick, self.ghost, ctypes.byref(self._h))
+        else:
+            rc = lib().vr_volume_create_layout(self.nx, self.ny, self.nz, self.brick, self.ghost, self.layout,
+                                               ctypes.byref(self._h))
         if rc != 0:
             self._h = ctypes.c_void_p()
             raise VrError(rc, lib().vr_last_error(None).decode())

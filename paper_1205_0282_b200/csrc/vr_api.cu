@@ -102,12 +102,62 @@ extern "C" void vr_volume_destroy(vr_volume* v) {
     release(v);
 }
 
+/* Fill the layout part of the grid: per-axis offset functions and the slot size. */
+static void set_layout(VrGrid& g, int layout, const int tl[3], const int ml[3]) {
+    g.layout = layout;
+    const int P = g.P;
+    if (layout == VR_LAYOUT_LINEAR) {
+        for (int a = 0; a < 3; ++a) {
+            g.tl[a] = g.ml[a] = 0;
+            g.nt[a] = P;
+            VrAxisLayout& A = g.ax[a];
+            memset(&A, 0, sizeof(A));
+        }
+        g.ax[0].lo_mask = 0x7fffffff; /* x: the index itself */
+        g.ax[0].hi_in = 31;
+        g.ax[1].hi_stride = (unsigned)P;
+        g.ax[2].hi_stride = (unsigned)P * (unsigned)P;
+        g.slot = (((long long)P * P * P + 31) / 32) * 32;
+        return;
+    }
+    const int tbits = tl[0] + tl[1] + tl[2];          /* 5: 32 floats per micro-tile */
+    const int mbits = ml[0] + ml[1] + ml[2];
+    const unsigned block = 1u << (tbits + mbits);      /* floats per macro block */
+    int lo_shift = 0, mid_shift = tbits;
+    unsigned stride = block;
+    for (int a = 0; a < 3; ++a) {
+        g.tl[a] = tl[a];
+        g.ml[a] = ml[a];
+        const int span = 1 << (tl[a] + ml[a]);         /* cells per macro block along a */
+        g.nt[a] = (P + span - 1) / span;
+        VrAxisLayout& A = g.ax[a];
+        A.lo_mask = (1 << tl[a]) - 1;
+        A.lo_shift = lo_shift;
+        A.mid_in = tl[a];
+        A.mid_mask = (1 << ml[a]) - 1;
+        A.mid_shift = mid_shift;
+        A.hi_in = tl[a] + ml[a];
+        A.hi_stride = stride;
+        lo_shift += tl[a];
+        mid_shift += ml[a];
+        stride *= (unsigned)g.nt[a];
+    }
+    g.slot = (long long)block * g.nt[0] * g.nt[1] * g.nt[2];
+}
+
 extern "C" int vr_volume_create(int nx, int ny, int nz, int brick, int ghost, vr_volume** out) {
+    return vr_volume_create_layout(nx, ny, nz, brick, ghost, VR_LAYOUT_DEFAULT, out);
+}
+
+extern "C" int vr_volume_create_layout(int nx, int ny, int nz, int brick, int ghost, int layout, vr_volume** out) {
     if (!out) return fail(NULL, VR_ERR_INVALID_ARG, "vr_volume_create: out is NULL");
     *out = NULL;
     if (nx <= 0 || ny <= 0 || nz <= 0) return fail(NULL, VR_ERR_INVALID_ARG, "vr_volume_create: non-positive size %dx%dx%d", nx, ny, nz);
     if (brick < 2) return fail(NULL, VR_ERR_INVALID_ARG, "vr_volume_create: brick %d < 2", brick);
     if (ghost < 0 || ghost > 8) return fail(NULL, VR_ERR_INVALID_ARG, "vr_volume_create: ghost %d outside [0,8]", ghost);
+    if (layout != VR_LAYOUT_DEFAULT && layout != VR_LAYOUT_LINEAR && layout != VR_LAYOUT_TILED)
+        return fail(NULL, VR_ERR_INVALID_ARG, "vr_volume_create_layout: unknown layout %d", layout);
+    if (layout == VR_LAYOUT_DEFAULT) layout = VR_LAYOUT_TILED;
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
         cudaGetLastError();
@@ -142,8 +192,18 @@ extern "C" int vr_volume_create(int nx, int ny, int nz, int brick, int ghost, vr
         if (m < core) core = m;
     }
     g.P = core + 2 * ghost;
-    g.slot = (long long)g.P * g.P * g.P;
     g.brick_pow2 = (brick & (brick - 1)) == 0;
+    {
+        int tl[3] = {2, 2, 1}, ml[3] = {0, 0, 0};
+        if (const char* e = getenv("VR_TILE")) /* experiment knob: "lx,ly,lz,mx,my,mz" (log2) */
+            sscanf(e, "%d,%d,%d,%d,%d,%d", &tl[0], &tl[1], &tl[2], &ml[0], &ml[1], &ml[2]);
+        if (const char* e = getenv("VR_LAYOUT")) layout = atoi(e) == 1 ? VR_LAYOUT_LINEAR : VR_LAYOUT_TILED;
+        set_layout(g, layout, tl, ml);
+    }
+    if (g.slot >= (1ll << 31)) {
+        delete v;
+        return fail(NULL, VR_ERR_INVALID_ARG, "vr_volume_create: a padded brick of %d^3 cells exceeds 2^31 floats", g.P);
+    }
     v->tau = 0.99f;
 
     cudaError_t e = cudaMalloc(&v->bricks, (size_t)g.slot * (size_t)g.nbricks * sizeof(float));
@@ -165,10 +225,6 @@ extern "C" int vr_volume_create(int nx, int ny, int nz, int brick, int ghost, vr
              (double)g.slot * g.nbricks * 4.0 / 1e9);
         release(v);
         return st;
-    }
-    if (const char* e = getenv("VR_L2_FETCH_GRANULARITY")) { /* experiment knob: 32, 64 or 128 bytes */
-        cudaDeviceSetLimit(cudaLimitMaxL2FetchGranularity, (size_t)atoi(e));
-        cudaGetLastError();
     }
     v->ctas = vr_raycast_ctas();
     if (v->ctas <= 0) {
@@ -278,14 +334,14 @@ extern "C" int vr_debug_brick_data(vr_volume* v, int b, float* dst, int* dims) {
     }
     if (!dst) return VR_OK;
     VR_CUDA(v, cudaDeviceSynchronize());
-    /* the brick's cells are the low corner of its P^3 slot: a pitched 3-D copy */
-    cudaMemcpy3DParms p;
-    memset(&p, 0, sizeof(p));
-    p.srcPtr = make_cudaPitchedPtr(v->bricks + (long long)b * g.slot, (size_t)g.P * sizeof(float), (size_t)g.P, (size_t)g.P);
-    p.dstPtr = make_cudaPitchedPtr(dst, (size_t)d[0] * sizeof(float), (size_t)d[0], (size_t)d[1]);
-    p.extent = make_cudaExtent((size_t)d[0] * sizeof(float), (size_t)d[1], (size_t)d[2]);
-    p.kind = cudaMemcpyDeviceToHost;
-    VR_CUDA(v, cudaMemcpy3D(&p));
+    float* d_tmp = NULL;
+    const size_t bytes = (size_t)d[0] * d[1] * d[2] * sizeof(float);
+    VR_CUDA(v, cudaMalloc(&d_tmp, bytes));
+    cudaError_t e = vr_launch_brick_copy(g, v->bricks, b, d, d_tmp, 0);
+    v->launches++;
+    if (e == cudaSuccess) e = cudaMemcpy(dst, d_tmp, bytes, cudaMemcpyDeviceToHost);
+    cudaFree(d_tmp);
+    VR_CUDA(v, e);
     return VR_OK;
 }
 
@@ -335,7 +391,7 @@ extern "C" int vr_set_counting(vr_volume* v, int enable) {
     if (enable == 2 && !v->d_bitmap) {
         const long long words = (v->grid.slot * v->grid.nbricks + 31) / 32;
         VR_CUDA(v, cudaMalloc(&v->d_bitmap, (size_t)words * sizeof(unsigned)));
-        VR_CUDA(v, cudaMalloc(&v->d_counts2, 2 * sizeof(unsigned long long)));
+        VR_CUDA(v, cudaMalloc(&v->d_counts2, 3 * sizeof(unsigned long long)));
         v->bitmap_words = words;
     }
     v->counting = enable;
@@ -626,15 +682,16 @@ extern "C" int vr_debug_stats(vr_volume* v, vr_stats* out) {
     out->rays = (int64_t)vs.total_sub_pixels;
     out->work_items = vs.total_items;
     out->subimage_bytes = (int64_t)vs.total_sub_pixels * (v->last_mode == VR_ALPHA ? 16 : 4);
-    out->cells_touched = out->sectors_touched = -1;
+    out->cells_touched = out->sectors_touched = out->lines_touched = -1;
     if (v->counting == 2) {
-        unsigned long long c2[2] = {0, 0};
+        unsigned long long c2[3] = {0, 0, 0};
         VR_CUDA(v, cudaMemset(v->d_counts2, 0, sizeof(c2)));
         VR_CUDA(v, vr_launch_count_bits(v->d_bitmap, v->bitmap_words, v->d_counts2, 0));
         v->launches++;
         VR_CUDA(v, cudaMemcpy(c2, v->d_counts2, sizeof(c2), cudaMemcpyDeviceToHost));
         out->cells_touched = (int64_t)c2[0];
         out->sectors_touched = (int64_t)c2[1];
+        out->lines_touched = (int64_t)c2[2];
     }
     out->nbricks = v->grid.nbricks;
     out->overflow = vs.overflow;

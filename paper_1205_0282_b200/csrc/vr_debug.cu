@@ -165,26 +165,47 @@ cudaError_t vr_launch_gather_sub(const VrBrickView* bv, int nbricks, const void*
     return cudaGetLastError();
 }
 
-/* Touched-cells bitmap (bench instrumentation): out2[0] += set bits (distinct brick-store
- * cells read), out2[1] += non-zero bytes (distinct 32-byte sectors: 8 consecutive cells). */
-__global__ void vr_count_bits_kernel(const unsigned* __restrict__ bitmap, long long words, unsigned long long* __restrict__ out2) {
-    unsigned long long cells = 0, sectors = 0;
+/* Test export: the padded cells of brick b as a dense [dz][dy][dx] box (any layout). */
+__global__ void vr_brick_copy_kernel(VrGrid g, const float* __restrict__ bricks, int b, int dx, int dy, int dz,
+                                     float* __restrict__ out) {
+    const long long n = (long long)dx * dy * dz;
+    const float* __restrict__ src = bricks + (long long)b * g.slot;
+    for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < n; t += (long long)gridDim.x * blockDim.x) {
+        const int i = (int)(t % dx), j = (int)((t / dx) % dy), k = (int)(t / ((long long)dx * dy));
+        out[t] = src[vr_cell_offset(g, i, j, k)];
+    }
+}
+
+cudaError_t vr_launch_brick_copy(const VrGrid& grid, const float* bricks, int b, const int dims[3], float* d_out,
+                                 cudaStream_t st) {
+    vr_brick_copy_kernel<<<148 * 8, 256, 0, st>>>(grid, bricks, b, dims[0], dims[1], dims[2], d_out);
+    return cudaGetLastError();
+}
+
+/* Touched-cells bitmap (bench instrumentation): out3[0] += set bits (distinct brick-store
+ * cells read), out3[1] += non-zero bytes (distinct 32-byte sectors: 8 consecutive cells),
+ * out3[2] += non-zero words (distinct 128-byte lines: 32 consecutive cells). */
+__global__ void vr_count_bits_kernel(const unsigned* __restrict__ bitmap, long long words, unsigned long long* __restrict__ out3) {
+    unsigned long long cells = 0, sectors = 0, lines = 0;
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < words; i += (long long)gridDim.x * blockDim.x) {
         const unsigned w = bitmap[i];
         cells += __popc(w);
         sectors += ((w & 0xffu) != 0) + ((w & 0xff00u) != 0) + ((w & 0xff0000u) != 0) + ((w & 0xff000000u) != 0);
+        lines += (w != 0);
     }
     for (int o = 16; o > 0; o >>= 1) {
         cells += __shfl_xor_sync(0xffffffffu, cells, o);
         sectors += __shfl_xor_sync(0xffffffffu, sectors, o);
+        lines += __shfl_xor_sync(0xffffffffu, lines, o);
     }
     if ((threadIdx.x & 31) == 0) {
-        atomicAdd(out2, cells);
-        atomicAdd(out2 + 1, sectors);
+        atomicAdd(out3, cells);
+        atomicAdd(out3 + 1, sectors);
+        atomicAdd(out3 + 2, lines);
     }
 }
 
-cudaError_t vr_launch_count_bits(const unsigned* bitmap, long long words, unsigned long long* d_out2, cudaStream_t st) {
-    vr_count_bits_kernel<<<148 * 8, 256, 0, st>>>(bitmap, words, d_out2);
+cudaError_t vr_launch_count_bits(const unsigned* bitmap, long long words, unsigned long long* d_out3, cudaStream_t st) {
+    vr_count_bits_kernel<<<148 * 8, 256, 0, st>>>(bitmap, words, d_out3);
     return cudaGetLastError();
 }

@@ -2,10 +2,12 @@
  * vr_internal.cuh -- shared declarations of libvr's translation units (not part of the ABI).
  *
  * Data layout in HBM:
- *   bricks        float[nbricks][P][P][P], P = brick + 2*ghost, x fastest. Brick b =
- *                 (bz*gy + by)*gx + bx. Cell (i,j,k) of brick b holds global voxel
- *                 clamp(lo_b - ghost + (i,j,k), 0, n-1). Ragged bricks use the low corner of
- *                 their P^3 slot. 64-bit offsets throughout (a 104 GB store has 2.6e10 cells).
+ *   bricks        float[nbricks][slot], P = brick + 2*ghost padded cells per axis. Brick b =
+ *                 (bz*gy + by)*gx + bx. Padded cell (i,j,k) of brick b holds global voxel
+ *                 clamp(lo_b - ghost + (i,j,k), 0, n-1) and sits at vr_cell_offset(i,j,k):
+ *                 x-linear rows (VR_LAYOUT_LINEAR) or 128-byte 3-D micro-tiles
+ *                 (VR_LAYOUT_TILED), see VrAxisLayout. Ragged bricks use the low corner of
+ *                 their slot. 64-bit offsets throughout (a 104 GB store has 2.6e10 cells).
  *   VrViewState   one per handle: matrices, eye, totals, work counter (written by set-up).
  *   VrBrickView   one per brick: rendering rectangle, launch rectangle, sub-image offset.
  *   order         int[nbricks]: brick ids front to back; item_prefix int[nbricks+1]:
@@ -29,14 +31,32 @@
 #define VR_COMP_TILE_H 8
 #define VR_EV_RING 64 /* timed frames whose stage events are kept */
 
+/* Where padded cell i of one axis sits inside a brick slot. Every supported layout is
+ * SEPARABLE: offset(i,j,k) = ax[0](i) + ax[1](j) + ax[2](k) floats, with
+ *   ax(i) = ((i & lo_mask) << lo_shift)                        position inside a 128-byte micro-tile
+ *         + (((i >> mid_in) & mid_mask) << mid_shift)          micro-tile inside a macro block
+ *         + (i >> hi_in) * hi_stride                           macro block (or tile) along this axis
+ * x-linear rows are the special case lo_mask = ~0 (x) / hi_in = 0, hi_stride = P, P*P (y, z). */
+struct VrAxisLayout {
+    int lo_mask, lo_shift;
+    int mid_in, mid_mask, mid_shift;
+    int hi_in;
+    unsigned hi_stride;
+};
+
 struct VrGrid {
     int n[3];     /* nx, ny, nz */
     int g[3];     /* bricks per axis */
     int brick, ghost;
     int nbricks;
     int P;        /* padded edge of a brick slot */
-    long long slot; /* P^3 */
+    long long slot; /* floats per brick slot (a multiple of 32: slots start on 128-byte lines) */
     int brick_pow2; /* 1 if brick is a power of two (division by it is an exact scaling) */
+    int layout;     /* VR_LAYOUT_LINEAR or VR_LAYOUT_TILED */
+    int tl[3];      /* log2 edge of a micro-tile (tiled: 2^(tl0+tl1+tl2) = 32 floats = 128 bytes) */
+    int ml[3];      /* log2 micro-tiles per macro block and axis (0,0,0: tiles in x-fastest order) */
+    int nt[3];      /* tiled: macro blocks (or tiles) per axis of a slot */
+    VrAxisLayout ax[3];
 };
 
 /* The caller's matrices travel to the set-up kernel as a kernel argument (no copy, no sync). */
@@ -101,6 +121,15 @@ struct VrRaycastParams {
     int mode;
 };
 
+/* Offset (floats) of padded cell (i,j,k) inside a brick slot; < 2^32 for every legal slot. */
+__host__ __device__ __forceinline__ unsigned vr_axis_offset(const VrAxisLayout& A, int i) {
+    return ((unsigned)(i & A.lo_mask) << A.lo_shift) + ((unsigned)((i >> A.mid_in) & A.mid_mask) << A.mid_shift) +
+           (unsigned)(i >> A.hi_in) * A.hi_stride;
+}
+__host__ __device__ __forceinline__ unsigned vr_cell_offset(const VrGrid& g, int i, int j, int k) {
+    return vr_axis_offset(g.ax[0], i) + vr_axis_offset(g.ax[1], j) + vr_axis_offset(g.ax[2], k);
+}
+
 /* ---- launchers (each returns the cudaError of its launch) ---- */
 cudaError_t vr_launch_setup(const VrGrid& grid, const VrMatrices& mats, int W, int H, int mode,
                             long long sub_capacity_px, void* sub_base, VrViewState* vs, VrBrickView* bv, int* order,
@@ -117,7 +146,9 @@ cudaError_t vr_launch_ray_bricks(const VrGrid& grid, const VrViewState* vs, cons
                                  cudaStream_t st);
 cudaError_t vr_launch_gather_sub(const VrBrickView* bv, int nbricks, const void* sub, int mode, const int* d_pixels,
                                  int npix, float* d_out, cudaStream_t st);
-cudaError_t vr_launch_count_bits(const unsigned* bitmap, long long words, unsigned long long* d_out2, cudaStream_t st);
+cudaError_t vr_launch_brick_copy(const VrGrid& grid, const float* bricks, int b, const int dims[3], float* d_out,
+                                 cudaStream_t st);
+cudaError_t vr_launch_count_bits(const unsigned* bitmap, long long words, unsigned long long* d_out3, cudaStream_t st);
 int vr_raycast_ctas(); /* persistent grid size: resident CTAs per SM x SM count */
 
 /* host mirror of the set-up arithmetic, for argument validation and scratch sizing only */

@@ -230,16 +230,62 @@ __device__ __forceinline__ void mark_cell(unsigned* __restrict__ bitmap, long lo
     atomicOr(bitmap + (cell >> 5), 1u << (unsigned)(cell & 31));
 }
 
-template <int PT, bool CLAMP, bool COUNT>
-__device__ __forceinline__ float trilinear(const float* __restrict__ brick, int P, const int ext[3], const Lattice& L,
+/* Brick layouts the kernel is instantiated for:
+ *   LAY_LINEAR  x-linear rows of PT (compile time) or g.P cells;
+ *   LAY_TILE442 4x4x2-cell micro-tiles, tiles x fastest: per axis two integer operations,
+ *               ox(i) = i + (i>>2)*28, oy(j) = 4j + (j>>2)*(SY-16), oz(k) = 16k + (k>>1)*(SZ-32);
+ *   LAY_GENERIC any separable layout of VrAxisLayout (micro-tile shape, macro blocks). */
+enum { LAY_LINEAR = 0, LAY_TILE442 = 1, LAY_GENERIC = 2 };
+
+template <int LAY>
+__device__ __forceinline__ int axis_off(const VrGrid& g, int a, int i) {
+    if (LAY == LAY_TILE442) {
+        if (a == 0) return i + (i >> 2) * 28;
+        if (a == 1) return 4 * i + (i >> 2) * ((int)g.ax[1].hi_stride - 16);
+        return 16 * i + (i >> 1) * ((int)g.ax[2].hi_stride - 32);
+    }
+    return (int)vr_axis_offset(g.ax[a], i);
+}
+
+template <int LAY, int PT, bool CLAMP, bool COUNT>
+__device__ __forceinline__ float trilinear(const float* __restrict__ brick, const VrGrid& g, const int ext[3], const Lattice& L,
                                            unsigned* __restrict__ bitmap, long long brick_cell0) {
-    const int Pe = PT > 0 ? PT : P;
+    const int Pe = PT > 0 ? PT : g.P;
     int ix = (int)(L.q[0] >> 32), iy = (int)(L.q[1] >> 32), iz = (int)(L.q[2] >> 32);
     const float fx = __uint_as_float(0x3F800000u | ((unsigned)L.q[0] >> 9)) - 1.0f;
     const float fy = __uint_as_float(0x3F800000u | ((unsigned)L.q[1] >> 9)) - 1.0f;
     const float fz = __uint_as_float(0x3F800000u | ((unsigned)L.q[2] >> 9)) - 1.0f;
     float c000, c001, c010, c011, c100, c101, c110, c111;
-    if (!CLAMP) {
+    if (LAY != LAY_LINEAR) {
+        int x0 = ix, x1 = ix + 1, y0 = iy, y1 = iy + 1, z0 = iz, z1 = iz + 1;
+        if (CLAMP) { /* ghost = 0: indices leaving the brick's own cells are clamped into them (seams) */
+            x0 = min(max(x0, 0), ext[0] - 1), x1 = min(max(x1, 0), ext[0] - 1);
+            y0 = min(max(y0, 0), ext[1] - 1), y1 = min(max(y1, 0), ext[1] - 1);
+            z0 = min(max(z0, 0), ext[2] - 1), z1 = min(max(z1, 0), ext[2] - 1);
+        }
+        const int ox0 = axis_off<LAY>(g, 0, x0), ox1 = axis_off<LAY>(g, 0, x1);
+        const int oy0 = axis_off<LAY>(g, 1, y0), oy1 = axis_off<LAY>(g, 1, y1);
+        const int oz0 = axis_off<LAY>(g, 2, z0), oz1 = axis_off<LAY>(g, 2, z1);
+        const int r00 = oz0 + oy0, r01 = oz0 + oy1, r10 = oz1 + oy0, r11 = oz1 + oy1;
+        c000 = __ldg(brick + (r00 + ox0));
+        c001 = __ldg(brick + (r00 + ox1));
+        c010 = __ldg(brick + (r01 + ox0));
+        c011 = __ldg(brick + (r01 + ox1));
+        c100 = __ldg(brick + (r10 + ox0));
+        c101 = __ldg(brick + (r10 + ox1));
+        c110 = __ldg(brick + (r11 + ox0));
+        c111 = __ldg(brick + (r11 + ox1));
+        if (COUNT && bitmap) {
+            mark_cell(bitmap, brick_cell0 + (r00 + ox0));
+            mark_cell(bitmap, brick_cell0 + (r00 + ox1));
+            mark_cell(bitmap, brick_cell0 + (r01 + ox0));
+            mark_cell(bitmap, brick_cell0 + (r01 + ox1));
+            mark_cell(bitmap, brick_cell0 + (r10 + ox0));
+            mark_cell(bitmap, brick_cell0 + (r10 + ox1));
+            mark_cell(bitmap, brick_cell0 + (r11 + ox0));
+            mark_cell(bitmap, brick_cell0 + (r11 + ox1));
+        }
+    } else if (!CLAMP) {
         const float* p = brick + ((long long)(iz * Pe + iy) * Pe + ix);
         c000 = __ldg(p);
         c001 = __ldg(p + 1);
@@ -316,7 +362,7 @@ __device__ __forceinline__ void shade_alpha(Accum& acc, float v, float w, const 
     acc.a += ta;
 }
 
-template <int MODE, int PT, bool CLAMP, bool COUNT>
+template <int MODE, int LAY, int PT, bool CLAMP, bool COUNT>
 __global__ void __launch_bounds__(VR_RAYCAST_THREADS)
 vr_raycast_kernel(const VrRaycastParams prm) {
     __shared__ float4 s_lut_base[MODE == VR_ALPHA ? VR_MAX_LUT : 1];
@@ -410,7 +456,7 @@ vr_raycast_kernel(const VrRaycastParams prm) {
         bool active = n > 0 && !stopped;
         while (__any_sync(FULL_MASK, active)) {
             if (active) {
-                const float v = trilinear<PT, CLAMP, COUNT>(brick, g.P, ext, L, prm.bitmap, (long long)b * g.slot);
+                const float v = trilinear<LAY, PT, CLAMP, COUNT>(brick, g, ext, L, prm.bitmap, (long long)b * g.slot);
                 if (COUNT) ++nsamples;
                 if (MODE == VR_MIP) {
                     acc.r = fmaxf(acc.r, v);
@@ -437,7 +483,7 @@ vr_raycast_kernel(const VrRaycastParams prm) {
                     const double p = VR_FMA(s, ray.d[a], ray.o[a]);
                     L.q[a] = to_fixed(p - ((double)(blo[a] - g.ghost) + 0.5));
                 }
-                const float v = trilinear<PT, CLAMP, COUNT>(brick, g.P, ext, L, prm.bitmap, (long long)b * g.slot);
+                const float v = trilinear<LAY, PT, CLAMP, COUNT>(brick, g, ext, L, prm.bitmap, (long long)b * g.slot);
                 if (COUNT) ++nsamples;
                 if (MODE == VR_MIP) {
                     acc.r = fmaxf(acc.r, v);
@@ -464,20 +510,33 @@ vr_raycast_kernel(const VrRaycastParams prm) {
 }
 
 /* ------------------------------------------------------------------------------------------ */
-template <int MODE, int PT, bool CLAMP, bool COUNT>
+template <int MODE, int LAY, int PT, bool CLAMP, bool COUNT>
 static cudaError_t launch_variant(const VrRaycastParams& p, int ctas, cudaStream_t st) {
-    vr_raycast_kernel<MODE, PT, CLAMP, COUNT><<<ctas, VR_RAYCAST_THREADS, 0, st>>>(p);
+    vr_raycast_kernel<MODE, LAY, PT, CLAMP, COUNT><<<ctas, VR_RAYCAST_THREADS, 0, st>>>(p);
     return cudaGetLastError();
+}
+
+static bool is_tile442(const VrGrid& g) {
+    return g.layout == VR_LAYOUT_TILED && g.tl[0] == 2 && g.tl[1] == 2 && g.tl[2] == 1 && g.ml[0] == 0 && g.ml[1] == 0 &&
+           g.ml[2] == 0;
 }
 
 template <int MODE, bool COUNT>
 static cudaError_t launch_mode(const VrRaycastParams& p, int ctas, cudaStream_t st) {
-    if (p.grid.ghost == 0) return launch_variant<MODE, 0, true, COUNT>(p, ctas, st);
-    switch (p.grid.P) {
-        case 258: return launch_variant<MODE, 258, false, COUNT>(p, ctas, st);
-        case 514: return launch_variant<MODE, 514, false, COUNT>(p, ctas, st);
-        default: return launch_variant<MODE, 0, false, COUNT>(p, ctas, st);
+    const bool clamp = p.grid.ghost == 0;
+    if (p.grid.layout == VR_LAYOUT_LINEAR) {
+        if (clamp) return launch_variant<MODE, LAY_LINEAR, 0, true, COUNT>(p, ctas, st);
+        switch (p.grid.P) {
+            case 258: return launch_variant<MODE, LAY_LINEAR, 258, false, COUNT>(p, ctas, st);
+            case 514: return launch_variant<MODE, LAY_LINEAR, 514, false, COUNT>(p, ctas, st);
+            default: return launch_variant<MODE, LAY_LINEAR, 0, false, COUNT>(p, ctas, st);
+        }
     }
+    if (is_tile442(p.grid))
+        return clamp ? launch_variant<MODE, LAY_TILE442, 0, true, COUNT>(p, ctas, st)
+                     : launch_variant<MODE, LAY_TILE442, 0, false, COUNT>(p, ctas, st);
+    return clamp ? launch_variant<MODE, LAY_GENERIC, 0, true, COUNT>(p, ctas, st)
+                 : launch_variant<MODE, LAY_GENERIC, 0, false, COUNT>(p, ctas, st);
 }
 
 cudaError_t vr_launch_raycast(const VrRaycastParams& p, int ctas, bool count, cudaStream_t st) {
@@ -489,7 +548,7 @@ int vr_raycast_ctas() {
     int dev = 0, sms = 0, per_sm = 0;
     if (cudaGetDevice(&dev) != cudaSuccess) return 0;
     if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return 0;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, vr_raycast_kernel<VR_ALPHA, 258, false, false>,
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, vr_raycast_kernel<VR_ALPHA, LAY_TILE442, 0, false, false>,
                                                       VR_RAYCAST_THREADS, 0) != cudaSuccess)
         return 0;
     if (per_sm < 1) per_sm = 1;
