@@ -34,7 +34,6 @@ struct vr_volume {
     long long frame_capacity_px;
     float* d_stage;          /* staging for VR_HOST upload / download */
     long long stage_floats;
-    int ctas;                /* persistent grid of the ray-cast kernel */
     int counting;            /* 0 off, 1 samples, 2 samples + touched-cells bitmap */
     bool timing;
     unsigned* d_bitmap;      /* one bit per brick-store cell (counting == 2) */
@@ -225,11 +224,6 @@ extern "C" int vr_volume_create_layout(int nx, int ny, int nz, int brick, int gh
              (double)g.slot * g.nbricks * 4.0 / 1e9);
         release(v);
         return st;
-    }
-    v->ctas = vr_raycast_ctas();
-    if (v->ctas <= 0) {
-        release(v);
-        return fail(NULL, VR_ERR_CUDA, "vr_volume_create: cannot size the ray-cast grid (kernel image not loadable on this device?)");
     }
     *out = v;
     return VR_OK;
@@ -482,10 +476,7 @@ extern "C" int vr_render(vr_volume* v, const float* view, const float* proj, int
     p.step = (double)step;
     p.tau = v->tau;
     p.mode = mode;
-    long long ctas = v->ctas;
-    const long long want = (items + (VR_RAYCAST_THREADS / 32) - 1) / (VR_RAYCAST_THREADS / 32);
-    if (ctas > want) ctas = want < 1 ? 1 : want;
-    VR_CUDA(v, vr_launch_raycast(p, (int)ctas, v->counting != 0, st));
+    VR_CUDA(v, vr_launch_raycast(p, items, v->counting != 0, st));
     v->launches++;
     if (timing) VR_CUDA(v, cudaEventRecord(ev[2], st));
 

@@ -134,7 +134,8 @@ __host__ __device__ __forceinline__ unsigned vr_cell_offset(const VrGrid& g, int
 cudaError_t vr_launch_setup(const VrGrid& grid, const VrMatrices& mats, int W, int H, int mode,
                             long long sub_capacity_px, void* sub_base, VrViewState* vs, VrBrickView* bv, int* order,
                             int* item_prefix, VrCompLayer* layers, cudaStream_t st);
-cudaError_t vr_launch_raycast(const VrRaycastParams& p, int ctas, bool count, cudaStream_t st);
+/* items = work items of the view (sizes the persistent grid) */
+cudaError_t vr_launch_raycast(const VrRaycastParams& p, long long items, bool count, cudaStream_t st);
 cudaError_t vr_launch_composite(const VrCompLayer* layers, const int* order, int n, int W, int H, int mode,
                                 const VrLut& lut, float* out, cudaStream_t st);
 cudaError_t vr_launch_upload(const VrGrid& grid, float* bricks, const float* src, int x0, int y0, int z0, int sx,
@@ -149,7 +150,6 @@ cudaError_t vr_launch_gather_sub(const VrBrickView* bv, int nbricks, const void*
 cudaError_t vr_launch_brick_copy(const VrGrid& grid, const float* bricks, int b, const int dims[3], float* d_out,
                                  cudaStream_t st);
 cudaError_t vr_launch_count_bits(const unsigned* bitmap, long long words, unsigned long long* d_out3, cudaStream_t st);
-int vr_raycast_ctas(); /* persistent grid size: resident CTAs per SM x SM count */
 
 /* host mirror of the set-up arithmetic, for argument validation and scratch sizing only */
 int vr_host_view_check(const VrGrid& grid, const float* view, const float* proj, int W, int H, long long* sub_pixels,

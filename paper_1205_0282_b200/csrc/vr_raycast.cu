@@ -23,9 +23,20 @@
  *   - the LUT is staged in shared memory as (entry, delta) pairs;
  *   - early ray termination and loop exit are warp votes.
  */
+#include <limits.h>
+
 #include "vr_view.cuh"
 
 #define FULL_MASK 0xffffffffu
+#ifndef VR_REUSE
+#define VR_REUSE 1 /* keep the 8 voxels while consecutive samples stay in the same cell */
+#endif
+#ifndef VR_RECOMPUTE_TAIL
+#define VR_RECOMPUTE_TAIL 1 /* rebuild the FP64 ray for the exit samples instead of keeping it live */
+#endif
+#ifndef VR_MIN_CTAS
+#define VR_MIN_CTAS 3 /* resident CTAs per SM the register budget is cut for (80 registers) */
+#endif
 
 struct RaySetup {
     double o[3], d[3];
@@ -247,14 +258,16 @@ __device__ __forceinline__ int axis_off(const VrGrid& g, int a, int i) {
     return (int)vr_axis_offset(g.ax[a], i);
 }
 
+/* The 8 voxels around a lattice position (cell = integer words of L), x fastest in c[]. */
+struct Corners {
+    float c000, c001, c010, c011, c100, c101, c110, c111;
+};
+
 template <int LAY, int PT, bool CLAMP, bool COUNT>
-__device__ __forceinline__ float trilinear(const float* __restrict__ brick, const VrGrid& g, const int ext[3], const Lattice& L,
-                                           unsigned* __restrict__ bitmap, long long brick_cell0) {
+__device__ __forceinline__ void fetch8(const float* __restrict__ brick, const VrGrid& g, const int ext[3], const Lattice& L,
+                                       unsigned* __restrict__ bitmap, long long brick_cell0, Corners& C) {
     const int Pe = PT > 0 ? PT : g.P;
     int ix = (int)(L.q[0] >> 32), iy = (int)(L.q[1] >> 32), iz = (int)(L.q[2] >> 32);
-    const float fx = __uint_as_float(0x3F800000u | ((unsigned)L.q[0] >> 9)) - 1.0f;
-    const float fy = __uint_as_float(0x3F800000u | ((unsigned)L.q[1] >> 9)) - 1.0f;
-    const float fz = __uint_as_float(0x3F800000u | ((unsigned)L.q[2] >> 9)) - 1.0f;
     float c000, c001, c010, c011, c100, c101, c110, c111;
     if (LAY != LAY_LINEAR) {
         int x0 = ix, x1 = ix + 1, y0 = iy, y1 = iy + 1, z0 = iz, z1 = iz + 1;
@@ -332,13 +345,30 @@ __device__ __forceinline__ float trilinear(const float* __restrict__ brick, cons
             mark_cell(bitmap, brick_cell0 + r11 + x1);
         }
     }
-    const float c00 = fmaf(fx, c001 - c000, c000);
-    const float c01 = fmaf(fx, c011 - c010, c010);
-    const float c10 = fmaf(fx, c101 - c100, c100);
-    const float c11 = fmaf(fx, c111 - c110, c110);
+    C.c000 = c000, C.c001 = c001, C.c010 = c010, C.c011 = c011;
+    C.c100 = c100, C.c101 = c101, C.c110 = c110, C.c111 = c111;
+}
+
+/* Tri-linear interpolation (R3): the fraction words of L are the float32 weights. */
+__device__ __forceinline__ float lerp8(const Corners& C, const Lattice& L) {
+    const float fx = __uint_as_float(0x3F800000u | ((unsigned)L.q[0] >> 9)) - 1.0f;
+    const float fy = __uint_as_float(0x3F800000u | ((unsigned)L.q[1] >> 9)) - 1.0f;
+    const float fz = __uint_as_float(0x3F800000u | ((unsigned)L.q[2] >> 9)) - 1.0f;
+    const float c00 = fmaf(fx, C.c001 - C.c000, C.c000);
+    const float c01 = fmaf(fx, C.c011 - C.c010, C.c010);
+    const float c10 = fmaf(fx, C.c101 - C.c100, C.c100);
+    const float c11 = fmaf(fx, C.c111 - C.c110, C.c110);
     const float c0 = fmaf(fy, c01 - c00, c00);
     const float c1 = fmaf(fy, c11 - c10, c10);
     return fmaf(fz, c1 - c0, c0);
+}
+
+template <int LAY, int PT, bool CLAMP, bool COUNT>
+__device__ __forceinline__ float trilinear(const float* __restrict__ brick, const VrGrid& g, const int ext[3], const Lattice& L,
+                                           unsigned* __restrict__ bitmap, long long brick_cell0) {
+    Corners C;
+    fetch8<LAY, PT, CLAMP, COUNT>(brick, g, ext, L, bitmap, brick_cell0, C);
+    return lerp8(C, L);
 }
 
 struct Accum {
@@ -363,18 +393,21 @@ __device__ __forceinline__ void shade_alpha(Accum& acc, float v, float w, const 
 }
 
 template <int MODE, int LAY, int PT, bool CLAMP, bool COUNT>
-__global__ void __launch_bounds__(VR_RAYCAST_THREADS)
+__global__ void __launch_bounds__(VR_RAYCAST_THREADS, VR_MIN_CTAS)
 vr_raycast_kernel(const VrRaycastParams prm) {
-    __shared__ float4 s_lut_base[MODE == VR_ALPHA ? VR_MAX_LUT : 1];
-    __shared__ float4 s_lut_delta[MODE == VR_ALPHA ? VR_MAX_LUT : 1];
+    /* dynamic: 2 * lut.n float4 (ALPHA) - a 256-entry table takes 8 KB, not the 32 KB of the
+     * largest one, and what it does not take stays L1 cache */
+    extern __shared__ float4 s_lut[];
+    const float4* s_lut_base = s_lut;
+    const float4* s_lut_delta = s_lut + prm.lut.n;
     __shared__ double s_minv[16];
 
     const VrGrid& g = prm.grid;
     const int lane = threadIdx.x & 31;
     if (MODE == VR_ALPHA) {
         for (int i = threadIdx.x; i < prm.lut.n; i += blockDim.x) {
-            s_lut_base[i] = prm.lut.base[i];
-            s_lut_delta[i] = prm.lut.delta[i];
+            s_lut[i] = prm.lut.base[i];
+            s_lut[prm.lut.n + i] = prm.lut.delta[i];
         }
     }
     if (threadIdx.x < 16) s_minv[threadIdx.x] = prm.vs->Minv[threadIdx.x];
@@ -454,9 +487,19 @@ vr_raycast_kernel(const VrRaycastParams prm) {
         }
         bool stopped = (MODE == VR_ALPHA) ? !(acc.a < tau) : false;
         bool active = n > 0 && !stopped;
+        /* With step < 1 consecutive samples of a ray often fall into the same cell: the 8
+         * voxels stay in registers and only the weights change (fewer L1 wavefronts, the
+         * bound of densely sampled views). */
+        Corners C;
+        int pcx = INT_MIN, pcy = 0, pcz = 0;
         while (__any_sync(FULL_MASK, active)) {
             if (active) {
-                const float v = trilinear<LAY, PT, CLAMP, COUNT>(brick, g, ext, L, prm.bitmap, (long long)b * g.slot);
+                const int cx = (int)(L.q[0] >> 32), cy = (int)(L.q[1] >> 32), cz = (int)(L.q[2] >> 32);
+                if (!VR_REUSE || cx != pcx || cy != pcy || cz != pcz) {
+                    fetch8<LAY, PT, CLAMP, COUNT>(brick, g, ext, L, prm.bitmap, (long long)b * g.slot, C);
+                    pcx = cx, pcy = cy, pcz = cz;
+                }
+                const float v = lerp8(C, L);
                 if (COUNT) ++nsamples;
                 if (MODE == VR_MIP) {
                     acc.r = fmaxf(acc.r, v);
@@ -465,9 +508,7 @@ vr_raycast_kernel(const VrRaycastParams prm) {
                     shade_alpha(acc, v, stepf, s_lut_base, s_lut_delta, prm.lut.n, vmin, inv_range);
                     stopped = !(acc.a < tau);
                 }
-                L.q[0] += D[0];
-                L.q[1] += D[1];
-                L.q[2] += D[2];
+                L.q[0] += D[0], L.q[1] += D[1], L.q[2] += D[2];
                 --n;
                 active = n > 0 && !stopped;
             }
@@ -475,6 +516,13 @@ vr_raycast_kernel(const VrRaycastParams prm) {
         /* the (at most two) samples next to the exit point */
         const int k_tail = max(k_lat, k_lo);
         if (__any_sync(FULL_MASK, k_tail < k_hi && !stopped)) {
+#if VR_RECOMPUTE_TAIL
+            if (k_tail < k_hi && !stopped) {
+                int qi = pi, qj = pj; /* opaque copies: the ray is rebuilt, not kept in registers */
+                asm volatile("" : "+r"(qi), "+r"(qj));
+                ray_setup(s_minv, W, H, qi, qj, g, step, ray);
+            }
+#endif
             for (int k = k_tail; k < k_hi && !stopped; ++k) {
                 double s, w;
                 if (!sample_sw(ray, step, k, s, w)) continue;
@@ -510,9 +558,28 @@ vr_raycast_kernel(const VrRaycastParams prm) {
 }
 
 /* ------------------------------------------------------------------------------------------ */
+/* Persistent grid: resident CTAs per SM (for this instance and its shared memory) x SMs,
+ * but no more CTAs than there are groups of 8 work items. */
 template <int MODE, int LAY, int PT, bool CLAMP, bool COUNT>
-static cudaError_t launch_variant(const VrRaycastParams& p, int ctas, cudaStream_t st) {
-    vr_raycast_kernel<MODE, LAY, PT, CLAMP, COUNT><<<ctas, VR_RAYCAST_THREADS, 0, st>>>(p);
+static cudaError_t launch_variant(const VrRaycastParams& p, long long items, cudaStream_t st) {
+    static int sms = 0, cached_per_sm = 0;
+    static size_t cached_smem = (size_t)-1;
+    const size_t smem = MODE == VR_ALPHA ? 2 * sizeof(float4) * (size_t)p.lut.n : 0;
+    if (smem != cached_smem) {
+        int dev = 0;
+        cudaError_t e = cudaGetDevice(&dev);
+        if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        if (e == cudaSuccess)
+            e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&cached_per_sm, vr_raycast_kernel<MODE, LAY, PT, CLAMP, COUNT>,
+                                                              VR_RAYCAST_THREADS, smem);
+        if (e != cudaSuccess) return e;
+        if (cached_per_sm < 1) return cudaErrorLaunchOutOfResources;
+        cached_smem = smem;
+    }
+    long long ctas = (long long)sms * cached_per_sm;
+    const long long want = (items + (VR_RAYCAST_THREADS / 32) - 1) / (VR_RAYCAST_THREADS / 32);
+    if (ctas > want) ctas = want < 1 ? 1 : want;
+    vr_raycast_kernel<MODE, LAY, PT, CLAMP, COUNT><<<(int)ctas, VR_RAYCAST_THREADS, smem, st>>>(p);
     return cudaGetLastError();
 }
 
@@ -522,7 +589,7 @@ static bool is_tile442(const VrGrid& g) {
 }
 
 template <int MODE, bool COUNT>
-static cudaError_t launch_mode(const VrRaycastParams& p, int ctas, cudaStream_t st) {
+static cudaError_t launch_mode(const VrRaycastParams& p, long long ctas, cudaStream_t st) {
     const bool clamp = p.grid.ghost == 0;
     if (p.grid.layout == VR_LAYOUT_LINEAR) {
         if (clamp) return launch_variant<MODE, LAY_LINEAR, 0, true, COUNT>(p, ctas, st);
@@ -539,18 +606,7 @@ static cudaError_t launch_mode(const VrRaycastParams& p, int ctas, cudaStream_t 
                  : launch_variant<MODE, LAY_GENERIC, 0, false, COUNT>(p, ctas, st);
 }
 
-cudaError_t vr_launch_raycast(const VrRaycastParams& p, int ctas, bool count, cudaStream_t st) {
+cudaError_t vr_launch_raycast(const VrRaycastParams& p, long long ctas, bool count, cudaStream_t st) {
     if (p.mode == VR_ALPHA) return count ? launch_mode<VR_ALPHA, true>(p, ctas, st) : launch_mode<VR_ALPHA, false>(p, ctas, st);
     return count ? launch_mode<VR_MIP, true>(p, ctas, st) : launch_mode<VR_MIP, false>(p, ctas, st);
-}
-
-int vr_raycast_ctas() {
-    int dev = 0, sms = 0, per_sm = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess) return 0;
-    if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return 0;
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, vr_raycast_kernel<VR_ALPHA, LAY_TILE442, 0, false, false>,
-                                                      VR_RAYCAST_THREADS, 0) != cudaSuccess)
-        return 0;
-    if (per_sm < 1) per_sm = 1;
-    return sms * per_sm;
 }
