@@ -191,47 +191,79 @@ def timed_device(g, wl, mode, order, K, W, out, dist=None):
     return ms, launches, stages, stage_views
 
 
-def timed_e2e(g, wl, mode, order, K, W, host_out, dist=None):
-    """Same frames through the host-buffer entry (vr_render_host): per frame the matrices go
-    host->device (as kernel arguments) and the finished RGBA frame comes back into pinned host
-    memory; both inside the timed region."""
+def timed_e2e(g, wl, mode, order, K, W, host_bufs, dist=None, pipelined=True):
+    """Same frames through the host-buffer entries: per frame the matrices go host->device (as
+    kernel arguments) and the finished RGBA frame comes back into pinned host memory; both
+    inside the timed region. pipelined: vr_render_host_async (frame i's copy overlaps frame
+    i+1's rendering, two frames in flight, three rotating pinned buffers) and one
+    vr_render_host_wait before the closing event; else vr_render_host, which waits per frame."""
     import torch
+
+    def frame(k):
+        view = wl["views"][order[k % len(order)]]
+        if pipelined:
+            g.render_host_async(view, wl["proj"], wl["width"], wl["height"], wl["step"], mode, host_bufs[k % len(host_bufs)])
+        else:
+            g.render_host(view, wl["proj"], wl["width"], wl["height"], wl["step"], mode, out=host_bufs[0])
+
     for k in range(W):
-        g.render_host(wl["views"][order[k % len(order)]], wl["proj"], wl["width"], wl["height"], wl["step"], mode, out=host_out)
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        frame(k)
+    g.render_host_wait()
     if dist is not None:
         dist.barrier()
     torch.cuda.synchronize()
-    e0.record()
+    t0 = time.perf_counter()
     for k in range(K):
-        g.render_host(wl["views"][order[(W + k) % len(order)]], wl["proj"], wl["width"], wl["height"], wl["step"], mode, out=host_out)
-    e1.record()
+        frame(W + k)
+    g.render_host_wait()
     torch.cuda.synchronize()
+    ms = (time.perf_counter() - t0) * 1e3
     if dist is not None:
         dist.barrier()
-    return e0.elapsed_time(e1)
+    return ms
 
 
-def roofline_of(counts, stages, stage_views, peak_gbs, peak_src):
+def traffic_of(workload, mode, tf):
+    """DRAM bytes (read + write) of ONE ray-cast launch from the committed `ncu --set full`
+    capture of this workload (profiles/r1_traffic.csv, written from the .ncu-rep files as
+    profiles/r1_traffic.md describes), or None. Quoted, not measured in this run."""
+    try:
+        import csv
+        with open(os.path.join(ROOT, "profiles", "r1_traffic.csv")) as f:
+            for row in csv.DictReader(f):
+                if (row["workload"], row["mode"], row["tf"]) == (workload, mode, tf):
+                    return int(row["dram_read_bytes"]) + int(row["dram_write_bytes"])
+    except Exception:
+        pass
+    return None
+
+
+def roofline_of(counts, stages, stage_views, peak_gbs, peak_src, traffic=None):
     """Ray-cast kernel (the dominant one): algorithmic bytes = 4 B x distinct brick-store cells
     its samples read + the sub-image bytes it writes, over the views the
     counting pass covered; duration = that kernel's device time for the same views inside the
-    timed region (library stage events on the render stream)."""
+    timed region (library stage events on the render stream). `lines_*`: the same with the
+    distinct 128-byte lines of the brick store instead of the cells - what DRAM must deliver
+    for this layout at least."""
     by_view = {}
     for (ms_setup, ms_ray, ms_comp), vi in zip(stages, stage_views):
         by_view.setdefault(vi, []).append(float(ms_ray))
-    alg, ms, n = 0.0, 0.0, 0
+    alg, lines, ms, n = 0.0, 0.0, 0.0, 0
     for vi, s in counts.items():
         if s["cells_touched"] >= 0 and vi in by_view:
             alg += 4.0 * s["cells_touched"] + s["subimage_bytes"]
+            lines += 128.0 * s["lines_touched"] + s["subimage_bytes"]
             ms += float(np.mean(by_view[vi]))
             n += 1
     if n == 0 or ms <= 0:
         return None
     achieved = alg / (ms * 1e-3) / 1e9
+    lines_gbs = lines / (ms * 1e-3) / 1e9
     return {"bound": "hbm", "kernel": "vr_raycast_kernel", "achieved": round(achieved, 1), "peak": peak_gbs, "unit": "GB/s",
-            "frac": round(achieved / peak_gbs, 4), "traffic": None, "peak_source": peak_src,
-            "algorithmic_bytes_per_launch": round(alg / n), "launch_ms": round(ms / n, 4), "views_counted": n}
+            "frac": round(achieved / peak_gbs, 4), "traffic": traffic, "peak_source": peak_src,
+            "algorithmic_bytes_per_launch": round(alg / n), "launch_ms": round(ms / n, 4), "views_counted": n,
+            "lines_bytes_per_launch": round(lines / n), "lines_gbs": round(lines_gbs, 1),
+            "lines_frac": round(lines_gbs / peak_gbs, 4)}
 
 
 def measured_peak():
@@ -338,6 +370,85 @@ def config_of(wl, args):
             "frames": "one frame per step, cycling the 36 views"}
 
 
+# ----------------------------------------------------------------------------- config 4
+def run_c4(args, vr, peak, peak_src, sampler):
+    """BASELINE.json configs[4]: (i) the 1024^3 cube of config 2 rendered at 512^2 .. 4096^2 in
+    ALPHA mode (seeded views, ramp TF, tau 0.99); (ii) the compositing microbenchmark: 64 seeded
+    premultiplied full-frame 4096^2 RGBA layers composited in a seeded visibility order
+    (vr_composite, row a9 alone). The roofline object is the compositing kernel's: pure HBM
+    streaming, algorithmic bytes = every layer pixel read once + the frame written once."""
+    import torch
+    K, Wm = args.steps, args.warmup
+    st = torch.cuda.current_stream().cuda_stream
+    # (ii) first, while HBM is empty: 64 x 268 MB layers
+    W = H = 4096
+    n = 64
+    layers = []
+    for l in range(n):
+        t = torch.empty((H, W, 4), dtype=torch.float32, device="cuda")
+        synth.layer_device(synth.BASE_SEED + 4, l, 0, W * H, t.data_ptr(), st)
+        layers.append(t)
+    rects = [(0, 0, W, H)] * n
+    order = synth.permutation(synth.BASE_SEED + 4, n)
+    out = torch.empty((H, W, 4), dtype=torch.float32, device="cuda")
+    for _ in range(Wm):
+        vr.composite(layers, rects, order, W, H, out)
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(K + 1)]
+    torch.cuda.synchronize()
+    sampler.start()
+    ev[0].record()
+    for k in range(K):
+        vr.composite(layers, rects, order, W, H, out)
+        ev[k + 1].record()
+    torch.cuda.synchronize()
+    clocks = sampler.stop()
+    comp_ms = np.array([ev[k].elapsed_time(ev[k + 1]) for k in range(K)])
+    comp_bytes = (n + 1) * W * H * 16
+    achieved = comp_bytes / (comp_ms.mean() * 1e-3) / 1e9
+    comp = {"layers": n, "width": W, "height": H, "ms": round(float(comp_ms.mean()), 4), "ms_min": round(float(comp_ms.min()), 4),
+            "bytes": comp_bytes, "gb_per_s": round(achieved, 1), "launches": K}
+    roof = {"bound": "hbm", "kernel": "vr_composite_kernel", "achieved": round(achieved, 1), "peak": peak, "unit": "GB/s",
+            "frac": round(achieved / peak, 4), "traffic": traffic_of("c4", "composite", "-"), "peak_source": peak_src,
+            "algorithmic_bytes_per_launch": comp_bytes, "launch_ms": round(float(comp_ms.mean()), 4)}
+    del layers, out
+    torch.cuda.empty_cache()
+
+    # (i) resolution sweep on config 2's cube
+    wl = workload("c2")
+    g, _ = build_volume(vr, wl, synth.tf_ramp())
+    sweep, launches = [], K
+    for res in (512, 1024, 2048, 4096):
+        w = dict(wl)
+        w["width"] = w["height"] = res
+        fr = synth.Framing(w["nx"], w["ny"], w["nz"], res, res)
+        w["views"] = [fr.seeded(w["seed"], k) for k in range(36)]
+        w["proj"] = fr.proj(False)
+        img = torch.empty((res, res, 4), dtype=torch.float32, device="cuda")
+        ids = list(range(36))
+        timed = sorted(set(ids[(Wm + k) % 36] for k in range(K)))
+        counts = count_pass(g, vr, w, 0, timed, img, 0)
+        ms, nl, stages, _ = timed_device(g, w, 0, ids, K, Wm, img)
+        launches += nl
+        samples = sum(counts[ids[(Wm + k) % 36]]["samples"] for k in range(K))
+        sweep.append({"width": res, "height": res, "frames_per_s": round(K / (ms * 1e-3), 3),
+                      "gsamples_per_s": round(samples / (ms * 1e-3) / 1e9, 3), "samples_per_frame": int(samples / K),
+                      "stage_ms": {"setup": round(float(stages[:, 0].mean()), 4), "raycast": round(float(stages[:, 1].mean()), 4),
+                                   "composite": round(float(stages[:, 2].mean()), 4)}})
+        del img
+    g.close()
+    top = sweep[-1]
+    return {"metric": METRIC, "value": top["frames_per_s"], "unit": "frames/s", "n_gpus": 1, "steps": K, "warmup": Wm,
+            "ms_per_step": round(1e3 / top["frames_per_s"], 4), "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32", "data": "synthetic",
+            "config": {"workload": "c4: value = frames/s of config 2's 1024^3 cube at 4096x4096 (ALPHA, step 0.5, ramp TF, tau 0.99, "
+                                   "36 seeded views); `sweep` = the same at 512^2..4096^2; `compositing` = 64 seeded premultiplied "
+                                   "4096^2 RGBA layers through vr_composite in a seeded order",
+                       "baseline_config_index": 4,
+                       "l2_policy": "inputs larger than L2 (17 GB of layers per compositing launch; 4.3 GB cube); no explicit flush"},
+            "gsamples_per_s": top["gsamples_per_s"], "gpu_launches": launches, "sweep": sweep, "compositing": comp,
+            "roofline": roof, "clocks": clocks, "e2e": None, "cpu_baseline": None}
+
+
 # ----------------------------------------------------------------------------- main
 def main():
     ap = argparse.ArgumentParser()
@@ -345,7 +456,7 @@ def main():
     ap.add_argument("--steps", type=int, default=36)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="c3", choices=["c0", "c1", "c2", "c3"])
+    ap.add_argument("--workload", default="c3", choices=["c0", "c1", "c2", "c3", "c4"])
     ap.add_argument("--mode", default="alpha", choices=["alpha", "mip"])
     ap.add_argument("--tf", default="ramp", choices=["ramp", "translucent"])
     ap.add_argument("--cells-every", type=int, default=6, help="count distinct cells on every n-th view of the cycle (0 = never)")
@@ -357,7 +468,7 @@ def main():
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
-    wl = workload(args.workload)
+    wl = workload(args.workload if args.workload != "c4" else "c2")
     tf = synth.tf_ramp() if args.tf == "ramp" else synth.tf_translucent()
     mode_id = 0 if args.mode == "alpha" else 1
 
@@ -390,12 +501,19 @@ def main():
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         return float(t.item())
 
+    if args.workload == "c4":
+        if world > 1:
+            raise SystemExit("bench.py: --workload c4 is a single-GPU microbenchmark")
+        peak, peak_src = measured_peak()
+        print(json.dumps(run_c4(args, vr, peak, peak_src, ClockSampler(local_rank))), flush=True)
+        return 0
+
     t_build = time.perf_counter()
     g, cube = build_volume(vr, wl, tf)
     t_build = time.perf_counter() - t_build
     W, H, K, Wm = wl["width"], wl["height"], args.steps, args.warmup
     out = torch.empty((H, W, 4), dtype=torch.float32, device="cuda")
-    host_out = torch.empty((H, W, 4), dtype=torch.float32).pin_memory()
+    host_bufs = [torch.empty((H, W, 4), dtype=torch.float32).pin_memory() for _ in range(3)]
     order = views_for_rank(rank, world, len(wl["views"]))
     timed_views = sorted(set(order[(Wm + k) % len(order)] for k in range(K)))
 
@@ -404,16 +522,18 @@ def main():
         if sampler:
             sampler.start()
         ms, launches, stages, stage_views = timed_device(g, wl, mode, order, K, Wm, out, dist)
-        e2e_ms = timed_e2e(g, wl, mode, order, K, Wm, host_out, dist) if with_e2e else None
+        e2e_ms = timed_e2e(g, wl, mode, order, K, Wm, host_bufs, dist, True) if with_e2e else None
+        e2e_sync_ms = timed_e2e(g, wl, mode, order, K, Wm, host_bufs, dist, False) if with_e2e else None
         clocks = sampler.stop() if sampler else None
         samples = sum(counts[order[(Wm + k) % len(order)]]["samples"] for k in range(K))
-        return dict(ms=ms, launches=launches, stages=stages, stage_views=stage_views, e2e_ms=e2e_ms, clocks=clocks,
+        return dict(ms=ms, launches=launches, stages=stages, stage_views=stage_views, e2e_ms=e2e_ms, e2e_sync_ms=e2e_sync_ms, clocks=clocks,
                     samples=samples, counts=counts)
 
     peak, peak_src = measured_peak()
     m = measure(mode_id, True, ClockSampler(local_rank) if rank == 0 else None)
     fps, ms_max = aggregate(m["ms"], K, world, reduce_max)
     e2e_fps, e2e_ms_max = aggregate(m["e2e_ms"], K, world, reduce_max)
+    e2e_sync_fps, _ = aggregate(m["e2e_sync_ms"], K, world, reduce_max)
 
     line = {"metric": METRIC, "value": round(fps, 3), "unit": "frames/s", "n_gpus": world, "steps": K, "warmup": Wm,
             "ms_per_step": round(ms_max / K, 4), "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -422,12 +542,17 @@ def main():
             "samples_per_frame": int(m["samples"] / K),
             "gpu_launches": int(m["launches"]),
             "e2e": {"value": round(e2e_fps, 3), "unit": "frames/s", "h2d_bytes_per_step": 128, "d2h_bytes_per_step": W * H * 16,
-                    "what": "vr_render_host: matrices from host memory, finished RGBA frame copied to pinned host memory every step; "
-                            "the cube stays resident in HBM (in-core rendering, PAPER.md:146,206)"},
+                    "what": "vr_render_host_async + one vr_render_host_wait: matrices from host memory, every finished RGBA frame "
+                            "copied to pinned host memory inside the timed region (frame i's copy overlaps frame i+1's rendering); "
+                            "host wall clock around K frames with a device synchronise on both sides; the cube stays resident in "
+                            "HBM (in-core rendering, PAPER.md:146,206)",
+                    "synchronous_value": round(e2e_sync_fps, 3),
+                    "synchronous_what": "vr_render_host: the caller waits for each frame's copy before queueing the next"},
             "clocks": m["clocks"],
             "stage_ms": {"setup": round(float(m["stages"][:, 0].mean()), 4), "raycast": round(float(m["stages"][:, 1].mean()), 4),
                          "composite": round(float(m["stages"][:, 2].mean()), 4)},
-            "roofline": roofline_of(m["counts"], m["stages"], m["stage_views"], peak, peak_src),
+            "roofline": roofline_of(m["counts"], m["stages"], m["stage_views"], peak, peak_src,
+                                    traffic_of(args.workload, args.mode, args.tf)),
             "build_s": round(t_build, 1)}
     cs = [s for s in m["counts"].values() if s["cells_touched"] >= 0]
     if cs:
@@ -449,7 +574,8 @@ def main():
                              "stage_ms": {"setup": round(float(v["stages"][:, 0].mean()), 4),
                                           "raycast": round(float(v["stages"][:, 1].mean()), 4),
                                           "composite": round(float(v["stages"][:, 2].mean()), 4)},
-                             "roofline": roofline_of(v["counts"], v["stages"], v["stage_views"], peak, peak_src)})
+                             "roofline": roofline_of(v["counts"], v["stages"], v["stage_views"], peak, peak_src,
+                                                     traffic_of(args.workload, vmode, vtf))})
         g.set_transfer_function(tf, synth.TF_VMIN, synth.TF_VMAX)
         line["variants"] = variants
 

@@ -172,6 +172,21 @@ int vr_render(vr_volume* v, const float* view, const float* proj, int width, int
 int vr_render_host(vr_volume* v, const float* view, const float* proj, int width, int height,
                    float step, int mode, float* out_rgba_host, void* stream);
 
+/* The same end-to-end frame, PIPELINED: the call returns once the frame's kernels and its
+ * device->host copy are queued, and the copy of frame i (on a library-owned copy stream, out
+ * of one of two library-owned device frames) overlaps the rendering of frame i+1 on `stream`.
+ * This is how a frame server uses the renderer (the server renders while the
+ * previous frame travels to the viewer).
+ *   out_rgba_host (host, should be pinned): [height][width][4] float32; its contents are
+ *   defined only after vr_render_host_wait returns. The caller must not reuse the buffer for
+ *   another frame before that (use one buffer per frame in flight; two frames are in flight).
+ * vr_render_host_wait blocks until every frame queued by vr_render_host_async on this handle
+ * has arrived in host memory. Errors as vr_render; the wait returns VR_ERR_CUDA if a queued
+ * copy failed. */
+int vr_render_host_async(vr_volume* v, const float* view, const float* proj, int width,
+                         int height, float step, int mode, float* out_rgba_host, void* stream);
+int vr_render_host_wait(vr_volume* v);
+
 /* ------------------------------------------------------------------------------------------
  * Stand-alone sort-last compositing (row a9; the 64-layer microbenchmark). PAPER.md:114
  * (compositing is the bottleneck of distributed image-order rendering), :170-174.

@@ -25,7 +25,7 @@ STATUS = {0: "VR_OK", 1: "VR_ERR_INVALID_ARG", 2: "VR_ERR_OUT_OF_MEMORY", 3: "VR
 # every symbol include/vr.h declares (tests check the library exports each of them)
 SYMBOLS = (
     "vr_volume_create", "vr_volume_create_layout", "vr_volume_destroy", "vr_volume_upload", "vr_volume_download", "vr_debug_brick_data",
-    "vr_set_transfer_function", "vr_set_early_termination", "vr_render", "vr_render_host", "vr_composite",
+    "vr_set_transfer_function", "vr_set_early_termination", "vr_render", "vr_render_host", "vr_render_host_async", "vr_render_host_wait", "vr_composite",
     "vr_num_bricks", "vr_debug_brick_order", "vr_debug_rects", "vr_debug_ray_bricks", "vr_debug_subimages",
     "vr_set_counting", "vr_set_timing", "vr_debug_stats", "vr_debug_stage_times", "vr_launch_count", "vr_last_error",
 )
@@ -68,6 +68,8 @@ def lib():
         L.vr_set_early_termination.argtypes = [vp, cf]
         L.vr_render.argtypes = [vp, vp, vp, ci, ci, cf, ci, vp, vp]
         L.vr_render_host.argtypes = [vp, vp, vp, ci, ci, cf, ci, vp, vp]
+        L.vr_render_host_async.argtypes = [vp, vp, vp, ci, ci, cf, ci, vp, vp]
+        L.vr_render_host_wait.argtypes = [vp]
         L.vr_composite.argtypes = [vp, vp, vp, ci, ci, ci, vp, vp]
         L.vr_num_bricks.argtypes = [vp]
         L.vr_debug_brick_order.argtypes = [vp, vp, vp, vp]
@@ -198,6 +200,23 @@ class Volume:
         self._check(lib().vr_render_host(self._h, v.ctypes.data, p.ctypes.data, int(width), int(height), float(step),
                                          int(mode), ptr, _stream(stream)))
         return out
+
+    def render_host_async(self, view, proj, width, height, step, mode, out, stream=None):
+        """Pipelined render_host: `out` (pinned CPU tensor or numpy array) is filled once
+        render_host_wait() has returned; use one buffer per frame in flight (two are)."""
+        v, p = _mat(view), _mat(proj)
+        if isinstance(out, np.ndarray):
+            assert out.dtype == np.float32 and out.flags.c_contiguous and out.size == width * height * 4
+            ptr = out.ctypes.data
+        else:
+            assert (not out.is_cuda) and out.is_contiguous() and out.element_size() == 4 and out.numel() == width * height * 4
+            ptr = out.data_ptr()
+        self._check(lib().vr_render_host_async(self._h, v.ctypes.data, p.ctypes.data, int(width), int(height), float(step),
+                                               int(mode), ptr, _stream(stream)))
+        return out
+
+    def render_host_wait(self):
+        self._check(lib().vr_render_host_wait(self._h))
 
     # -- debug / test exports ---------------------------------------------------
     def debug_brick_order(self, view, proj):

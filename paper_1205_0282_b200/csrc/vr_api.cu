@@ -32,6 +32,11 @@ struct vr_volume {
     long long sub_capacity_px;
     float* d_frame;          /* vr_render_host's device frame */
     long long frame_capacity_px;
+    float* d_pipe[2];        /* vr_render_host_async: two device frames, ... */
+    long long pipe_capacity_px;
+    cudaStream_t copy_stream; /* ... a copy stream, and per frame slot: */
+    cudaEvent_t ev_rendered[2], ev_copied[2];
+    long long pipe_frames;
     float* d_stage;          /* staging for VR_HOST upload / download */
     long long stage_floats;
     int counting;            /* 0 off, 1 samples, 2 samples + touched-cells bitmap */
@@ -85,6 +90,12 @@ static void release(vr_volume* v) {
     cudaFree(v->d_layers);
     cudaFree(v->d_sub);
     cudaFree(v->d_frame);
+    for (int i = 0; i < 2; ++i) {
+        cudaFree(v->d_pipe[i]);
+        if (v->ev_rendered[i]) cudaEventDestroy(v->ev_rendered[i]);
+        if (v->ev_copied[i]) cudaEventDestroy(v->ev_copied[i]);
+    }
+    if (v->copy_stream) cudaStreamDestroy(v->copy_stream);
     cudaFree(v->d_stage);
     cudaFree(v->d_bitmap);
     cudaFree(v->d_counts2);
@@ -368,6 +379,8 @@ extern "C" int vr_set_transfer_function(vr_volume* v, const float* rgba, int n, 
     v->lut.vmin = vmin;
     v->lut.vmax = vmax;
     v->lut.inv_range = (float)(1.0 / ((double)vmax - (double)vmin));
+    v->lut.nm2 = n - 2;
+    v->lut.scale = (float)(n - 1);
     v->has_tf = true;
     return VR_OK;
 }
@@ -474,6 +487,7 @@ extern "C" int vr_render(vr_volume* v, const float* view, const float* proj, int
     }
     p.lut = v->lut;
     p.step = (double)step;
+    p.stepf = step;
     p.tau = v->tau;
     p.mode = mode;
     VR_CUDA(v, vr_launch_raycast(p, items, v->counting != 0, st));
@@ -504,6 +518,12 @@ extern "C" int vr_render_host(vr_volume* v, const float* view, const float* proj
         if (v->d_frame) {
             VR_CUDA(v, cudaDeviceSynchronize());
             cudaFree(v->d_frame);
+    for (int i = 0; i < 2; ++i) {
+        cudaFree(v->d_pipe[i]);
+        if (v->ev_rendered[i]) cudaEventDestroy(v->ev_rendered[i]);
+        if (v->ev_copied[i]) cudaEventDestroy(v->ev_copied[i]);
+    }
+    if (v->copy_stream) cudaStreamDestroy(v->copy_stream);
             v->d_frame = NULL;
             v->frame_capacity_px = 0;
         }
@@ -515,6 +535,50 @@ extern "C" int vr_render_host(vr_volume* v, const float* view, const float* proj
     cudaStream_t st = (cudaStream_t)stream;
     VR_CUDA(v, cudaMemcpyAsync(out_rgba_host, v->d_frame, (size_t)px * 16, cudaMemcpyDeviceToHost, st));
     VR_CUDA(v, cudaStreamSynchronize(st));
+    return VR_OK;
+}
+
+extern "C" int vr_render_host_async(vr_volume* v, const float* view, const float* proj, int width, int height, float step,
+                                    int mode, float* out_rgba_host, void* stream) {
+    if (!v) return fail(NULL, VR_ERR_INVALID_ARG, "vr_render_host_async: NULL handle");
+    if (!out_rgba_host) return fail(v, VR_ERR_INVALID_ARG, "vr_render_host_async: NULL output");
+    if (width <= 0 || height <= 0 || width > 32768 || height > 32768)
+        return fail(v, VR_ERR_INVALID_ARG, "vr_render_host_async: bad frame size %dx%d", width, height);
+    const long long px = (long long)width * height;
+    if (!v->copy_stream) {
+        VR_CUDA(v, cudaStreamCreateWithFlags(&v->copy_stream, cudaStreamNonBlocking));
+        for (int i = 0; i < 2; ++i) {
+            VR_CUDA(v, cudaEventCreateWithFlags(&v->ev_rendered[i], cudaEventDisableTiming));
+            VR_CUDA(v, cudaEventCreateWithFlags(&v->ev_copied[i], cudaEventDisableTiming));
+        }
+    }
+    if (px > v->pipe_capacity_px) {
+        VR_CUDA(v, cudaDeviceSynchronize());
+        for (int i = 0; i < 2; ++i) {
+            cudaFree(v->d_pipe[i]);
+            v->d_pipe[i] = NULL;
+        }
+        v->pipe_capacity_px = 0;
+        for (int i = 0; i < 2; ++i) VR_CUDA(v, cudaMalloc(&v->d_pipe[i], (size_t)px * 16));
+        v->pipe_capacity_px = px;
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    const int slot = (int)(v->pipe_frames & 1);
+    /* the frame that last used this slot must have left it */
+    if (v->pipe_frames >= 2) VR_CUDA(v, cudaStreamWaitEvent(st, v->ev_copied[slot], 0));
+    const int rc = vr_render(v, view, proj, width, height, step, mode, v->d_pipe[slot], stream);
+    if (rc) return rc;
+    VR_CUDA(v, cudaEventRecord(v->ev_rendered[slot], st));
+    VR_CUDA(v, cudaStreamWaitEvent(v->copy_stream, v->ev_rendered[slot], 0));
+    VR_CUDA(v, cudaMemcpyAsync(out_rgba_host, v->d_pipe[slot], (size_t)px * 16, cudaMemcpyDeviceToHost, v->copy_stream));
+    VR_CUDA(v, cudaEventRecord(v->ev_copied[slot], v->copy_stream));
+    v->pipe_frames++;
+    return VR_OK;
+}
+
+extern "C" int vr_render_host_wait(vr_volume* v) {
+    if (!v) return fail(NULL, VR_ERR_INVALID_ARG, "vr_render_host_wait: NULL handle");
+    if (v->copy_stream) VR_CUDA(v, cudaStreamSynchronize(v->copy_stream));
     return VR_OK;
 }
 

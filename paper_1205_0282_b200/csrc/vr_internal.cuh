@@ -103,6 +103,8 @@ struct VrLut {
     const float4* delta; /* device: LUT[i+1] - LUT[i]         (n-1, last 0) */
     int n;
     float vmin, vmax, inv_range;
+    int nm2;     /* n - 2: last interval */
+    float scale; /* n - 1 as float: u -> table coordinate */
 };
 
 struct VrRaycastParams {
@@ -117,6 +119,7 @@ struct VrRaycastParams {
     unsigned* bitmap;   /* counting variant only: one bit per brick-store cell, or NULL */
     VrLut lut;
     double step;
+    float stepf; /* (float)step */
     float tau;
     int mode;
 };

@@ -269,7 +269,35 @@ __device__ __forceinline__ void fetch8(const float* __restrict__ brick, const Vr
     const int Pe = PT > 0 ? PT : g.P;
     int ix = (int)(L.q[0] >> 32), iy = (int)(L.q[1] >> 32), iz = (int)(L.q[2] >> 32);
     float c000, c001, c010, c011, c100, c101, c110, c111;
-    if (LAY != LAY_LINEAR) {
+    if (LAY == LAY_TILE442 && !CLAMP) {
+        /* ghost >= 1: every index is >= 0, so the offsets are
+         * unsigned 32-bit and each address is one 32x32+64 multiply-add on a kept base */
+        const unsigned ux0 = (unsigned)ix, ux1 = ux0 + 1u, uy0 = (unsigned)iy, uy1 = uy0 + 1u, uz0 = (unsigned)iz, uz1 = uz0 + 1u;
+        const unsigned sy = g.ax[1].hi_stride - 16u, sz = g.ax[2].hi_stride - 32u;
+        const unsigned ox0 = ux0 + (ux0 >> 2) * 28u, ox1 = ux1 + (ux1 >> 2) * 28u;
+        const unsigned oy0 = (uy0 << 2) + (uy0 >> 2) * sy, oy1 = (uy1 << 2) + (uy1 >> 2) * sy;
+        const unsigned oz0 = (uz0 << 4) + (uz0 >> 1) * sz, oz1 = (uz1 << 4) + (uz1 >> 1) * sz;
+        const unsigned r00 = oz0 + oy0, r01 = oz0 + oy1, r10 = oz1 + oy0, r11 = oz1 + oy1;
+        c000 = __ldg(brick + (r00 + ox0));
+        c001 = __ldg(brick + (r00 + ox1));
+        c010 = __ldg(brick + (r01 + ox0));
+        c011 = __ldg(brick + (r01 + ox1));
+        c100 = __ldg(brick + (r10 + ox0));
+        c101 = __ldg(brick + (r10 + ox1));
+        c110 = __ldg(brick + (r11 + ox0));
+        c111 = __ldg(brick + (r11 + ox1));
+        if (COUNT && bitmap) {
+            const long long c0 = brick_cell0 + ox0, c1 = brick_cell0 + ox1;
+            mark_cell(bitmap, c0 + r00);
+            mark_cell(bitmap, c1 + r00);
+            mark_cell(bitmap, c0 + r01);
+            mark_cell(bitmap, c1 + r01);
+            mark_cell(bitmap, c0 + r10);
+            mark_cell(bitmap, c1 + r10);
+            mark_cell(bitmap, c0 + r11);
+            mark_cell(bitmap, c1 + r11);
+        }
+    } else if (LAY != LAY_LINEAR) {
         int x0 = ix, x1 = ix + 1, y0 = iy, y1 = iy + 1, z0 = iz, z1 = iz + 1;
         if (CLAMP) { /* ghost = 0: indices leaving the brick's own cells are clamped into them (seams) */
             x0 = min(max(x0, 0), ext[0] - 1), x1 = min(max(x1, 0), ext[0] - 1);
@@ -375,16 +403,43 @@ struct Accum {
     float r, g, b, a; /* ALPHA: premultiplied colour and opacity; MIP: r = running max */
 };
 
-/* R7: classification and opacity of a sample standing for a path of length w; R8 blending. */
-__device__ __forceinline__ void shade_alpha(Accum& acc, float v, float w, const float4* __restrict__ lut_base,
-                                            const float4* __restrict__ lut_delta, int n, float vmin, float inv_range) {
-    const float u = __saturatef((v - vmin) * inv_range);
-    const float x = u * (float)(n - 1);
-    const int i = min((int)x, n - 2);
+/* The LUT as the kernel sees it: (entry, delta) pairs interleaved in shared memory, addressed
+ * through one 32-bit shared-window address kept in a register. */
+struct LutView {
+    unsigned base; /* shared-memory byte address of pair 0 */
+};
+
+template <int OFF>
+__device__ __forceinline__ float4 lds128(unsigned addr) {
+    float4 v;
+    asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4+%5];"
+                 : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w)
+                 : "r"(addr), "n"(OFF));
+    return v;
+}
+__device__ __forceinline__ float lg2_approx(float x) {
+    float y;
+    asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+__device__ __forceinline__ float ex2_approx(float x) {
+    float y;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
+/* R7: classification and opacity of a sample standing for a path of length w; R8 blending.
+ * alpha = 1 - (1-a)^w = 1 - 2^(w log2(1-a)) on the two MUFU approximations (2^-22 relative,
+ * DESIGN.md "Tolerances"); a = 1 gives log2(0) = -inf and alpha = 1, a = 0 gives alpha = 0. */
+__device__ __forceinline__ void shade_alpha(Accum& acc, float v, float w, const LutView& lut, const VrLut& P) {
+    const float u = __saturatef((v - P.vmin) * P.inv_range);
+    const float x = u * P.scale;
+    const int i = min((int)x, P.nm2);
     const float f = x - (float)i;
-    const float4 e = lut_base[i], dl = lut_delta[i];
+    const unsigned a = lut.base + 32u * (unsigned)i;
+    const float4 e = lds128<0>(a), dl = lds128<16>(a);
     const float cr = fmaf(f, dl.x, e.x), cg = fmaf(f, dl.y, e.y), cb = fmaf(f, dl.z, e.z), ca = fmaf(f, dl.w, e.w);
-    const float alpha = 1.0f - exp2f(w * __log2f(1.0f - ca));
+    const float alpha = 1.0f - ex2_approx(w * lg2_approx(1.0f - ca));
     const float ta = (1.0f - acc.a) * alpha;
     acc.r = fmaf(ta, cr, acc.r);
     acc.g = fmaf(ta, cg, acc.g);
@@ -398,16 +453,14 @@ vr_raycast_kernel(const VrRaycastParams prm) {
     /* dynamic: 2 * lut.n float4 (ALPHA) - a 256-entry table takes 8 KB, not the 32 KB of the
      * largest one, and what it does not take stays L1 cache */
     extern __shared__ float4 s_lut[];
-    const float4* s_lut_base = s_lut;
-    const float4* s_lut_delta = s_lut + prm.lut.n;
     __shared__ double s_minv[16];
 
     const VrGrid& g = prm.grid;
     const int lane = threadIdx.x & 31;
     if (MODE == VR_ALPHA) {
         for (int i = threadIdx.x; i < prm.lut.n; i += blockDim.x) {
-            s_lut[i] = prm.lut.base[i];
-            s_lut[prm.lut.n + i] = prm.lut.delta[i];
+            s_lut[2 * i] = prm.lut.base[i];
+            s_lut[2 * i + 1] = prm.lut.delta[i];
         }
     }
     if (threadIdx.x < 16) s_minv[threadIdx.x] = prm.vs->Minv[threadIdx.x];
@@ -417,9 +470,13 @@ vr_raycast_kernel(const VrRaycastParams prm) {
     const int W = prm.vs->W, H = prm.vs->H;
     const int total = prm.vs->total_items;
     const double step = prm.step;
-    const float stepf = (float)step;
     const float tau = prm.tau;
-    const float vmin = prm.lut.vmin, inv_range = prm.lut.inv_range;
+    LutView lut;
+    lut.base = 0;
+    if (MODE == VR_ALPHA) {
+        lut.base = (unsigned)__cvta_generic_to_shared(s_lut);
+        asm volatile("" : "+r"(lut.base)); /* one register, not rebuilt per sample */
+    }
     const float mip_stop = prm.lut.vmax; /* the output saturates at vmax */
     unsigned long long nsamples = 0;
 
@@ -454,6 +511,7 @@ vr_raycast_kernel(const VrRaycastParams prm) {
 #pragma unroll
         for (int a = 0; a < 3; ++a) ext[a] = bhi[a] - blo[a] + 2 * g.ghost;
         const float* __restrict__ brick = prm.bricks + (long long)b * g.slot;
+        asm volatile("" : "+l"(brick)); /* keep the base in registers: do not rebuild it per load */
 
         RaySetup ray;
         ray.K = 0;
@@ -505,7 +563,7 @@ vr_raycast_kernel(const VrRaycastParams prm) {
                     acc.r = fmaxf(acc.r, v);
                     stopped = acc.r >= mip_stop;
                 } else {
-                    shade_alpha(acc, v, stepf, s_lut_base, s_lut_delta, prm.lut.n, vmin, inv_range);
+                    shade_alpha(acc, v, prm.stepf, lut, prm.lut);
                     stopped = !(acc.a < tau);
                 }
                 L.q[0] += D[0], L.q[1] += D[1], L.q[2] += D[2];
@@ -537,7 +595,7 @@ vr_raycast_kernel(const VrRaycastParams prm) {
                     acc.r = fmaxf(acc.r, v);
                     stopped = acc.r >= mip_stop;
                 } else {
-                    shade_alpha(acc, v, (float)w, s_lut_base, s_lut_delta, prm.lut.n, vmin, inv_range);
+                    shade_alpha(acc, v, (float)w, lut, prm.lut);
                     stopped = !(acc.a < tau);
                 }
             }

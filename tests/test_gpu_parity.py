@@ -156,6 +156,30 @@ def test_one_brick_equals_n_bricks_on_gpu(vr):
     check_mip(bm, am, "1 vs N bricks")
 
 
+def test_pipelined_host_frames_equal_synchronous_ones(vr):
+    """vr_render_host_async / vr_render_host_wait: six frames in flight two at a time arrive
+    bit-identical to vr_render_host's, and the first one matches the oracle."""
+    import torch
+    cube = synth.Cube(21, 72, 40, 56, 6)
+    g, o = make_pair(cube, 32, 1)
+    W, H = 144, 100
+    fr = synth.Framing(cube.nx, cube.ny, cube.nz, W, H)
+    views = [fr.turntable(k) for k in range(6)]
+    proj = fr.proj(False)
+    bufs = [torch.empty((H, W, 4), dtype=torch.float32).pin_memory() for _ in views]
+    for mode in (vr.ALPHA, vr.MIP):
+        for b in bufs:
+            b.fill_(-1.0)
+        for v, b in zip(views, bufs):
+            g.render_host_async(v, proj, W, H, 0.5, mode, b)
+        g.render_host_wait()
+        for v, b in zip(views, bufs):
+            sync = g.render_host(v, proj, W, H, 0.5, mode)
+            assert np.array_equal(b.numpy(), sync)
+    ref = o.render(views[0], proj, W, H, 0.5, oracle.MIP)
+    check_mip(bufs[0].numpy().astype(np.float64), ref["image"], "pipelined frame 0")
+
+
 # --------------------------------------------------------------------------- edge cases
 def test_edge_cases(vr):
     import torch
