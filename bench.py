@@ -132,18 +132,32 @@ def build_volume(vr, wl, tf):
     cube = synth.Cube(wl["seed"], wl["nx"], wl["ny"], wl["nz"], wl["nsrc"], wl["ramp"])
     g = vr.Volume(wl["nx"], wl["ny"], wl["nz"], wl["brick"], wl["ghost"])
     plane = wl["nx"] * wl["ny"] * 4
-    nzs = max(1, min(wl["nz"], (1 << 30) // plane))
+    nzs = max(1, min(wl["nz"], (4 << 30) // plane))  # 4 GiB slabs: 64 planes of config 3
     buf = torch.empty((nzs, wl["ny"], wl["nx"]), dtype=torch.float32, device="cuda")
     st = torch.cuda.current_stream().cuda_stream
+    evs = []
     for z0 in range(0, wl["nz"], nzs):
         nk = min(nzs, wl["nz"] - z0)
         cube.fill_device(buf[:nk].data_ptr(), 0, 0, z0, wl["nx"], wl["ny"], nk, st)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
         g.upload(buf[:nk], origin=(0, 0, z0))
+        e1.record()
+        evs.append((e0, e1))
     torch.cuda.synchronize()
     del buf
     torch.cuda.empty_cache()
     g.set_transfer_function(tf, synth.TF_VMIN, synth.TF_VMAX)
     g.set_early_termination(wl["tau"])
+    # row a1 (once per cube): every source voxel read once, every padded brick cell written once
+    pad = 1
+    for n in (wl["nx"], wl["ny"], wl["nz"]):
+        nb = -(-n // wl["brick"])
+        pad *= n + 2 * wl["ghost"] * nb
+    up_bytes = 4 * (wl["nx"] * wl["ny"] * wl["nz"] + pad)
+    up_ms = sum(a.elapsed_time(b) for a, b in evs)
+    g.upload_stats = {"kernel": "vr_upload_tile442_kernel", "launches": len(evs), "ms": round(up_ms, 3), "bytes": up_bytes,
+                      "gb_per_s": round(up_bytes / (up_ms * 1e-3) / 1e9, 1)}
     return g, cube
 
 
@@ -553,7 +567,7 @@ def main():
                          "composite": round(float(m["stages"][:, 2].mean()), 4)},
             "roofline": roofline_of(m["counts"], m["stages"], m["stage_views"], peak, peak_src,
                                     traffic_of(args.workload, args.mode, args.tf)),
-            "build_s": round(t_build, 1)}
+            "build_s": round(t_build, 1), "upload": dict(g.upload_stats, frac_of_hbm_peak=round(g.upload_stats["gb_per_s"] / peak, 4))}
     cs = [s for s in m["counts"].values() if s["cells_touched"] >= 0]
     if cs:
         line["touched_per_frame"] = {"cells_gb": round(np.mean([4.0 * s["cells_touched"] for s in cs]) / 1e9, 3),

@@ -12,10 +12,10 @@
  * the volume boundary is edge-replicated.
  *
  * Upload is a gather. LINEAR: one warp per padded row of one brick, lanes along x (coalesced
- * writes, coalesced reads except at the two replicated ends). TILED: one warp per micro-tile
- * (one coalesced 128-byte line written; the 16-byte source segments it reads are shared with
- * the neighbouring warps of the CTA through L1). A cell is written iff its clamped global
- * index lies in the uploaded box, which makes z-slab uploads of a ~100 GB cube work.
+ * writes, coalesced reads except at the two replicated ends). TILED: one CTA per row of
+ * micro-tiles, source rows staged in shared memory so that both the reads and the writes are
+ * whole 128-byte lines. A cell is written iff its clamped global index lies in the uploaded
+ * box, which makes z-slab uploads of a ~100 GB cube work.
  */
 #include "vr_view.cuh"
 
@@ -63,11 +63,19 @@ vr_upload_kernel(VrGrid g, float* __restrict__ bricks, const float* __restrict__
     }
 }
 
-/* TILED: CTA = one row of micro-tiles (fixed tile y, z) of one brick; warp w takes tiles
- * w, w+8, ... along x; lane = cell inside the tile. */
+/* TILED: a CTA takes groups of TR consecutive rows of micro-tiles (same tile z) of one brick,
+ * TR * 2^(tl1+tl2) <= 32 source rows at a time. Phase 1 stages those source rows in shared
+ * memory: each warp owns up to 4 rows and keeps 8 coalesced 128-byte reads in flight (lanes
+ * along x; the replicated ends re-read one cell). Phase 2 writes the micro-tiles, one warp per
+ * tile = one 128-byte line, lane = cell inside the tile. The row pitch is = 4 (mod 32) floats
+ * so that the rows x cells a warp gathers fall into different banks. Both sides of the copy
+ * move whole lines: an HBM streaming kernel. */
+#define UP_ROWS 32 /* staged source rows per group (at most) */
+
 __global__ void __launch_bounds__(256)
 vr_upload_tiled_kernel(VrGrid g, float* __restrict__ bricks, const float* __restrict__ src, int x0, int y0, int z0, int sx,
-                       int sy, int sz) {
+                       int sy, int sz, int pitch) {
+    extern __shared__ float s_rows[];
     const int b = blockIdx.y;
     int bc[3], lo[3], hi[3];
     vr_brick_coords(g, b, bc);
@@ -78,25 +86,148 @@ vr_upload_tiled_kernel(VrGrid g, float* __restrict__ bricks, const float* __rest
     padded_range(lo[1], g.ghost, ey, g.n[1], y0, y0 + sy, j0, j1);
     padded_range(lo[2], g.ghost, ez, g.n[2], z0, z0 + sz, k0, k1);
     if (i1 <= i0 || j1 <= j0 || k1 <= k0) return;
-    const int tx0 = i0 >> g.tl[0], tx1 = ((i1 - 1) >> g.tl[0]) + 1;
+    const int tx0 = i0 >> g.tl[0], tx1 = ((i1 - 1) >> g.tl[0]) + 1, ntx = tx1 - tx0;
     const int ty0 = j0 >> g.tl[1], ty1 = ((j1 - 1) >> g.tl[1]) + 1;
     const int tz0 = k0 >> g.tl[2], tz1 = ((k1 - 1) >> g.tl[2]) + 1;
-    const int rows = (ty1 - ty0) * (tz1 - tz0);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, nwarps = blockDim.x >> 5;
-    const int li = lane & ((1 << g.tl[0]) - 1), lj = (lane >> g.tl[0]) & ((1 << g.tl[1]) - 1), lk = lane >> (g.tl[0] + g.tl[1]);
+    const int rbits = g.tl[1] + g.tl[2], nrow = 1 << rbits; /* source rows per tile row */
+    const int TR = UP_ROWS >> rbits;                        /* tile rows per group */
+    const int ngy = (ty1 - ty0 + TR - 1) / TR, groups = ngy * (tz1 - tz0);
+    const int li = lane & ((1 << g.tl[0]) - 1), ljk = lane >> g.tl[0];
+    const int lj = ljk & ((1 << g.tl[1]) - 1), lk = ljk >> g.tl[1];
+    const int ibase = tx0 << g.tl[0]; /* first staged padded x index */
     float* __restrict__ dstb = bricks + (long long)b * g.slot;
-    for (int row = blockIdx.x; row < rows; row += gridDim.x) {
-        const int j = ((ty0 + row % (ty1 - ty0)) << g.tl[1]) + lj, k = ((tz0 + row / (ty1 - ty0)) << g.tl[2]) + lk;
-        if (j < j0 || j >= j1 || k < k0 || k >= k1) continue;
-        const int gy = min(max(lo[1] - g.ghost + j, 0), g.n[1] - 1), gz = min(max(lo[2] - g.ghost + k, 0), g.n[2] - 1);
-        const float* __restrict__ srow = src + ((long long)(gz - z0) * sy + (gy - y0)) * sx;
-        const unsigned oyz = vr_axis_offset(g.ax[1], j) + vr_axis_offset(g.ax[2], k);
-        for (int t = tx0 + warp; t < tx1; t += nwarps) {
-            const int i = (t << g.tl[0]) + li;
-            if (i < i0 || i >= i1) continue;
-            const int gx = min(max(lo[0] - g.ghost + i, 0), g.n[0] - 1);
-            dstb[oyz + vr_axis_offset(g.ax[0], i)] = __ldg(srow + (gx - x0));
+    for (int grp = blockIdx.x; grp < groups; grp += gridDim.x) {
+        const int tyg = ty0 + (grp % ngy) * TR, kt = (tz0 + grp / ngy) << g.tl[2];
+        const int ntr = min(TR, ty1 - tyg); /* tile rows in this group */
+        /* phase 1: rows r = warp, warp + 8, ... of the group; r = (tile row, lk, lj) */
+        const float* srow[4];
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            const int r = warp + q * nwarps;
+            const int j = ((tyg + (r >> rbits)) << g.tl[1]) + (r & ((1 << g.tl[1]) - 1));
+            const int k = kt + ((r >> g.tl[1]) & ((1 << g.tl[2]) - 1));
+            srow[q] = NULL;
+            if (r < (ntr << rbits) && j >= j0 && j < j1 && k >= k0 && k < k1) {
+                const int gy = min(max(lo[1] - g.ghost + j, 0), g.n[1] - 1), gz = min(max(lo[2] - g.ghost + k, 0), g.n[2] - 1);
+                srow[q] = src + ((long long)(gz - z0) * sy + (gy - y0)) * sx - x0;
+            }
         }
+        for (int i = i0 + lane; i < i1; i += 64) {
+            float v[4][2];
+#pragma unroll
+            for (int q = 0; q < 4; ++q)
+#pragma unroll
+                for (int u = 0; u < 2; ++u) {
+                    const int gx = min(max(lo[0] - g.ghost + min(i + 32 * u, i1 - 1), 0), g.n[0] - 1);
+                    v[q][u] = srow[q] ? __ldcs(srow[q] + gx) : 0.0f;
+                }
+#pragma unroll
+            for (int q = 0; q < 4; ++q)
+#pragma unroll
+                for (int u = 0; u < 2; ++u)
+                    if (srow[q] && i + 32 * u < i1) s_rows[(warp + q * nwarps) * pitch + (i + 32 * u - ibase)] = v[q][u];
+        }
+        __syncthreads();
+        /* phase 2: tile t of the group = (tile row t / ntx, tile x t % ntx) */
+        for (int t = warp; t < ntr * ntx; t += nwarps) {
+            const int tr = t / ntx, tx = tx0 + (t - tr * ntx);
+            const int i = (tx << g.tl[0]) + li, j = ((tyg + tr) << g.tl[1]) + lj, k = kt + lk;
+            if (i >= i0 && i < i1 && j >= j0 && j < j1 && k >= k0 && k < k1)
+                dstb[vr_cell_offset(g, i, j, k)] = s_rows[((tr << rbits) + ljk) * pitch + (i - ibase)];
+        }
+        __syncthreads();
+    }
+}
+
+/* TILED, the default 4x4x2 micro-tiles in x-fastest tile order: the same two phases with the
+ * index arithmetic hoisted out of the element loops. Groups of TR = 2^TRL tile rows = 8 TR
+ * source rows (TRL = 2 for small bricks, 1 when 32 rows of a large brick would take too much
+ * shared memory for 6 CTAs per SM). Phase 1: warp w stages rows w, w+8, ... with 8 independent
+ * 128-byte reads in flight; phase 2: 8/TR warps per tile row, a lane writes one 16-byte row
+ * of a micro-tile (LDS.128 -> STG.128), so a warp instruction writes four whole 128-byte lines. */
+template <int TRL>
+__global__ void __launch_bounds__(256)
+vr_upload_tile442_kernel(VrGrid g, float* __restrict__ bricks, const float* __restrict__ src, int x0, int y0, int z0, int sx,
+                         int sy, int sz, int pitch) {
+    constexpr int TR = 1 << TRL;  /* tile rows per group */
+    constexpr int RW = TR;        /* staged rows per warp (8 TR rows, 8 warps) */
+    constexpr int CH = 8 / RW;    /* 32-cell chunks per row and iteration */
+    constexpr int WPT = 8 >> TRL; /* phase 2: warps per tile row */
+    extern __shared__ __align__(16) float s_rows[];
+    const int b = blockIdx.y;
+    int bc[3], lo[3], hi[3];
+    vr_brick_coords(g, b, bc);
+    vr_brick_core(g, bc, lo, hi);
+    const int ex = hi[0] - lo[0] + 2 * g.ghost, ey = hi[1] - lo[1] + 2 * g.ghost, ez = hi[2] - lo[2] + 2 * g.ghost;
+    int i0, i1, j0, j1, k0, k1;
+    padded_range(lo[0], g.ghost, ex, g.n[0], x0, x0 + sx, i0, i1);
+    padded_range(lo[1], g.ghost, ey, g.n[1], y0, y0 + sy, j0, j1);
+    padded_range(lo[2], g.ghost, ez, g.n[2], z0, z0 + sz, k0, k1);
+    if (i1 <= i0 || j1 <= j0 || k1 <= k0) return;
+    const int tx0 = i0 >> 2, tx1 = ((i1 - 1) >> 2) + 1;
+    const int ty0 = j0 >> 2, ty1 = ((j1 - 1) >> 2) + 1;
+    const int tz0 = k0 >> 1, tz1 = ((k1 - 1) >> 1) + 1;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int ngy = (ty1 - ty0 + TR - 1) >> TRL, groups = ngy * (tz1 - tz0);
+    const int ibase = tx0 << 2;
+    const int xbase = lo[0] - g.ghost; /* global x of padded cell 0 */
+    const bool clamp_x = xbase < 0 || xbase + ex - 1 > g.n[0] - 1;
+    float* __restrict__ dstb = bricks + (long long)b * g.slot;
+    /* phase-2 role of this lane: tile row tr, row r = lj + 4 lk of the tile, x tile q (+ 4 per warp of the row) */
+    const int tr = warp / WPT, r = lane & 7, q = (lane >> 3) + ((warp % WPT) << 2);
+    for (int grp = blockIdx.x; grp < groups; grp += gridDim.x) {
+        const int tyg = ty0 + ((grp % ngy) << TRL), kt = (tz0 + grp / ngy) << 1;
+        const int ntr = min(TR, ty1 - tyg);
+        const float* srow[RW];
+#pragma unroll
+        for (int u = 0; u < RW; ++u) {
+            const int rr = warp + 8 * u; /* staged row: tile row rr >> 3, lk = (rr >> 2) & 1, lj = rr & 3 */
+            const int j = ((tyg + (rr >> 3)) << 2) + (rr & 3), k = kt + ((rr >> 2) & 1);
+            srow[u] = NULL;
+            if ((rr >> 3) < ntr && j >= j0 && j < j1 && k >= k0 && k < k1) {
+                const int gy = min(max(lo[1] - g.ghost + j, 0), g.n[1] - 1), gz = min(max(lo[2] - g.ghost + k, 0), g.n[2] - 1);
+                srow[u] = src + ((long long)(gz - z0) * sy + (gy - y0)) * sx + (xbase - x0);
+            }
+        }
+        for (int i = i0 + lane; i < i1; i += 32 * CH) {
+            int ic[CH], gc[CH];
+#pragma unroll
+            for (int c = 0; c < CH; ++c) {
+                ic[c] = min(i + 32 * c, i1 - 1); /* clamped into the row: its last cell may be staged twice */
+                gc[c] = clamp_x ? min(max(xbase + ic[c], 0), g.n[0] - 1) - xbase : ic[c];
+            }
+            float v[RW][CH];
+#pragma unroll
+            for (int u = 0; u < RW; ++u)
+#pragma unroll
+                for (int c = 0; c < CH; ++c) v[u][c] = srow[u] ? __ldcs(srow[u] + gc[c]) : 0.0f;
+#pragma unroll
+            for (int u = 0; u < RW; ++u) {
+                float* d = s_rows + (warp + 8 * u) * pitch - ibase;
+#pragma unroll
+                for (int c = 0; c < CH; ++c) d[ic[c]] = v[u][c];
+            }
+        }
+        __syncthreads();
+        {
+            const int j = ((tyg + tr) << 2) + (r & 3), k = kt + (r >> 2);
+            if (tr < ntr && j >= j0 && j < j1 && k >= k0 && k < k1) {
+                const float* __restrict__ srw = s_rows + ((tr << 3) + r) * pitch - ibase;
+                float* __restrict__ out = dstb + (vr_axis_offset(g.ax[1], j) + vr_axis_offset(g.ax[2], k));
+                for (int tx = tx0 + q; tx < tx1; tx += 4 * WPT) {
+                    const int i = tx << 2;
+                    if (i >= i0 && i + 3 < i1) {
+                        *reinterpret_cast<float4*>(out + (tx << 5)) = *reinterpret_cast<const float4*>(srw + i);
+                    } else {
+#pragma unroll
+                        for (int c = 0; c < 4; ++c)
+                            if (i + c >= i0 && i + c < i1) out[(tx << 5) + c] = srw[i + c];
+                    }
+                }
+            }
+        }
+        __syncthreads();
     }
 }
 
@@ -130,12 +261,40 @@ cudaError_t vr_launch_upload(const VrGrid& grid, float* bricks, const float* src
         if (bx > 4096) bx = 4096;
         vr_upload_kernel<<<dim3(bx, grid.nbricks), 256, 0, st>>>(grid, bricks, src, x0, y0, z0, sx, sy, sz);
     } else {
-        /* one CTA per row of micro-tiles the box can touch in one brick, capped */
-        const long long ty = ((long long)grid.P >> grid.tl[1]) + 1;
+        /* one CTA per group of tile rows the box can touch in one brick, capped */
+        const int rbits = grid.tl[1] + grid.tl[2];
+        if (rbits > 5) return cudaErrorInvalidValue; /* a micro-tile spans at most 32 rows */
+        const int TR = UP_ROWS >> rbits;
+        const long long ty = (((long long)grid.P >> grid.tl[1]) + 1 + TR - 1) / TR;
         long long tz = (((long long)(sz < grid.P ? sz + 2 * grid.ghost : grid.P)) >> grid.tl[2]) + 2;
         long long bx = ty * tz;
         if (bx > 8192) bx = 8192;
-        vr_upload_tiled_kernel<<<dim3((unsigned)bx, grid.nbricks), 256, 0, st>>>(grid, bricks, src, x0, y0, z0, sx, sy, sz);
+        const int span = ((grid.P >> grid.tl[0]) + 1) << grid.tl[0];     /* staged cells per row */
+        const int pitch = ((span + 31) / 32) * 32 + 4;                    /* = 4 (mod 32) */
+        const size_t smem = sizeof(float) * (size_t)pitch * UP_ROWS;
+        if (smem > 48 * 1024) {
+            cudaError_t e = cudaFuncSetAttribute(vr_upload_tiled_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            if (e != cudaSuccess) return e;
+        }
+        const bool t442 = grid.tl[0] == 2 && grid.tl[1] == 2 && grid.tl[2] == 1 && grid.ml[0] == 0 && grid.ml[1] == 0 &&
+                          grid.ml[2] == 0;
+        if (t442) {
+            /* 32 staged rows while six CTAs of them fit an SM's shared memory, else 16 */
+            const bool big = smem > 40 * 1024;
+            const size_t sm2 = big ? smem / 2 : smem;
+            const long long ty2 = big ? (((long long)grid.P >> 2) + 2) / 2 : ty;
+            long long bx2 = ty2 * tz;
+            if (bx2 > 16384) bx2 = 16384;
+            if (big)
+                vr_upload_tile442_kernel<1><<<dim3((unsigned)bx2, grid.nbricks), 256, sm2, st>>>(grid, bricks, src, x0, y0, z0, sx,
+                                                                                                 sy, sz, pitch);
+            else
+                vr_upload_tile442_kernel<2><<<dim3((unsigned)bx2, grid.nbricks), 256, sm2, st>>>(grid, bricks, src, x0, y0, z0, sx,
+                                                                                                 sy, sz, pitch);
+        } else {
+            vr_upload_tiled_kernel<<<dim3((unsigned)bx, grid.nbricks), 256, smem, st>>>(grid, bricks, src, x0, y0, z0, sx, sy,
+                                                                                        sz, pitch);
+        }
     }
     return cudaGetLastError();
 }

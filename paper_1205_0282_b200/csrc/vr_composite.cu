@@ -19,6 +19,10 @@
 
 #define COMP_THREADS (VR_COMP_TILE_W * VR_COMP_TILE_H)
 #define COMP_LIST 256
+#ifndef VR_COMP_UNROLL
+#define VR_COMP_UNROLL 16 /* layers whose loads are in flight per pixel */
+#endif
+static constexpr int COMP_UNROLL = VR_COMP_UNROLL;
 
 struct CompEntry {
     unsigned long long addr;
@@ -71,7 +75,7 @@ vr_composite_kernel(const VrCompLayer* __restrict__ layers, const int* __restric
         const int cnt = s_count;
 
         if (live) {
-#pragma unroll 4
+#pragma unroll COMP_UNROLL
             for (int k = 0; k < cnt; ++k) {
                 const CompEntry& e = s_list[k];
                 const bool in = e.inside || (px >= e.x0 && px < e.x1 && py >= e.y0 && py < e.y1);
