@@ -33,6 +33,8 @@ def lib():
         L.vro_brick_data.restype = vp
         L.vro_brick_data.argtypes = [vp, ci, vp]
         L.vro_set_tf.argtypes = [vp, vp, ci, dbl, dbl]
+        L.vro_brick_minmax.argtypes = [vp, ci, vp, vp]
+        L.vro_brick_transparent.argtypes = [vp, ci]
         L.vro_set_tau.argtypes = [vp, dbl]
         L.vro_set_order_override.argtypes = [vp, vp]
         L.vro_brick_order.argtypes = [vp, vp, vp, vp]
@@ -111,6 +113,20 @@ class Volume:
         d0, d1, d2 = dims[0], dims[1], dims[2]
         buf = (ctypes.c_float * (d0 * d1 * d2)).from_address(p)
         return np.frombuffer(buf, dtype=np.float32).reshape(d2, d1, d0).copy()
+
+    def brick_minmax(self, b=-1):
+        """(min, max) as float32 over brick b's ghost-padded cells; b = -1: the whole volume (row f1)."""
+        mn, mx = ctypes.c_float(), ctypes.c_float()
+        if lib().vro_brick_minmax(self._h, int(b), ctypes.byref(mn), ctypes.byref(mx)) != 0:
+            raise ValueError("no data")
+        return np.float32(mn.value), np.float32(mx.value)
+
+    def brick_transparent(self, b):
+        """R16: True iff the current transfer function is zero-alpha over everything brick b can sample."""
+        r = lib().vro_brick_transparent(self._h, int(b))
+        if r < 0:
+            raise ValueError("no data or no transfer function")
+        return bool(r)
 
     def brick_order(self, view, proj):
         o = np.empty(self.nbricks, dtype=np.int32)

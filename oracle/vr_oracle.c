@@ -18,7 +18,8 @@
  *                                                         PAPER.md:150, Fig.4 :168
  *   - final colour mapping with the user's colour map
  * The paper gives no formulas; every constant and convention is a documented reading
- * R1..R15 (restated in DESIGN.md "Readings").
+ * R1..R15 (restated in DESIGN.md "Readings"), plus R16 (row f1: per-brick
+ * data range, and the transparent-brick rule built on it).
  *
  * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference leg
  * may load this. It shares no code with paper_1205_0282_b200/ (the CUDA path); only the
@@ -28,7 +29,8 @@
  * axis-aligned orthographic MIP = column max and ALPHA closed form, 1 brick == N bricks,
  * ERT bound, order independence of MIP, per-ray order within global order, each sample
  * owned once, rectangle conservativeness, step-halving convergence, brute force against an
- * independent numpy renderer. Parity unpinned (pure conventions): R1 row orientation,
+ * independent numpy renderer; data range: planted extremes incl. ghost-only cells, brute
+ * force; transparent bricks: their sub-images are exactly zero. Parity unpinned (pure conventions): R1 row orientation,
  * R11 MIP alpha, R13 form of the relative tolerance, R14 NaN handling (excluded).
  *
  * Build: gcc -O2 -std=c11 -ffp-contract=off -fopenmp -shared -fPIC (oracle/build.py).
@@ -144,6 +146,67 @@ const float* vro_brick_data(const vro_volume* v, int b, int64_t dims[3]) {
     brick_core(v, b, lo, hi);
     for (int a = 0; a < 3; ++a) dims[a] = hi[a] - lo[a] + 2 * v->ghost;
     return v->bricks ? v->bricks[b] : NULL;
+}
+
+/* ------------------------------------------------------------------ data range (row f1)
+ * PAPER.md:146 (sec. 2.3.1): "An independent task to determine the local minimum and maximum
+ * starts when the data is loaded into the GPU memory"; :152 the march may stop at "the
+ * maximum pixel value (defined by the global maximum of the data)".
+ * Local = per brick, over the brick's own ghost-padded copy (every value a sample of that
+ * brick can interpolate between); b < 0: over all bricks = the range of the whole volume
+ * (ghost cells are copies of voxels). Plain loops over the cells. */
+int vro_brick_minmax(const vro_volume* v, int b, float* mn_out, float* mx_out) {
+    if (!v || b >= v->nbricks || (!v->bricks && !v->fn)) return 1;
+    float mn = INFINITY, mx = -INFINITY;
+    const int b0 = b < 0 ? 0 : b, b1 = b < 0 ? v->nbricks : b + 1;
+    const int g = v->ghost;
+    for (int q = b0; q < b1; ++q) {
+        int64_t lo[3], hi[3];
+        brick_core(v, q, lo, hi);
+        const int64_t d0 = hi[0] - lo[0] + 2 * g, d1 = hi[1] - lo[1] + 2 * g, d2 = hi[2] - lo[2] + 2 * g;
+        for (int64_t k = 0; k < d2; ++k)
+            for (int64_t j = 0; j < d1; ++j)
+                for (int64_t i = 0; i < d0; ++i) {
+                    float x;
+                    if (v->bricks) x = v->bricks[q][(k * d1 + j) * d0 + i];
+                    else x = v->fn(v->ctx, clamp64(lo[0] - g + i, 0, v->n[0] - 1), clamp64(lo[1] - g + j, 0, v->n[1] - 1),
+                                   clamp64(lo[2] - g + k, 0, v->n[2] - 1));
+                    if (x < mn) mn = x;
+                    if (x > mx) mx = x;
+                }
+    }
+    *mn_out = mn;
+    *mx_out = mx;
+    return 0;
+}
+
+/* R16: a brick is TRANSPARENT for the current transfer function - and may be skipped in ALPHA
+ * mode without changing a single output bit - iff every table entry a sample of the brick can
+ * interpolate between has alpha == 0. The entry range is an integer decision taken in
+ * float32 (the precision the kernel classifies in), widened by one entry below and two above
+ * so that a rounding of the interpolated value cannot leave it:
+ *   I(x) = min(floor(sat((x - vmin) * inv_range) * (n-1)), n-2),  inv_range = (float)(1/(vmax-vmin))
+ *   transparent <=> a_i == 0 for all i in [max(0, I(min_b) - 1), min(n-1, I(max_b) + 2)].  */
+static int tf_index_f32(const vro_volume* v, float x) {
+    const float vminf = (float)v->vmin;
+    const float inv_range = (float)(1.0 / ((double)(float)v->vmax - (double)(float)v->vmin));
+    float u = (x - vminf) * inv_range;
+    if (!(u > 0.0f)) u = 0.0f;
+    if (u > 1.0f) u = 1.0f;
+    const float t = u * (float)(v->ntf - 1);
+    int i = (int)t;
+    if (i > v->ntf - 2) i = v->ntf - 2;
+    return i;
+}
+int vro_brick_transparent(const vro_volume* v, int b) {
+    float mn, mx;
+    if (!v || !v->tf || b < 0 || vro_brick_minmax(v, b, &mn, &mx)) return -1;
+    int i0 = tf_index_f32(v, mn) - 1, i1 = tf_index_f32(v, mx) + 2;
+    if (i0 < 0) i0 = 0;
+    if (i1 > v->ntf - 1) i1 = v->ntf - 1;
+    for (int i = i0; i <= i1; ++i)
+        if (v->tf[4 * i + 3] != 0.0f) return 0;
+    return 1;
 }
 
 int vro_set_tf(vro_volume* v, const float* rgba, int n, double vmin, double vmax) {

@@ -528,3 +528,93 @@ def test_composite_over_is_associative_and_matches_numpy():
     h2 = oracle.composite([layers[l] for l in order[3:]], [rects[l] for l in order[3:]], np.arange(3), W, H)
     merged = h1 + (1 - h1[..., 3:4]) * h2
     assert np.abs(merged - got).max() < 1e-12
+
+
+# --------------------------------------------------------------------------- data range (row f1, R16)
+def test_brick_minmax_planted_extremes_and_ghost_cells():
+    """PAPER.md:146 local minimum and maximum: per brick over its ghost-padded cells. A voxel on
+    a brick face belongs to the neighbour's ghost layer, so BOTH bricks see it; a voxel two
+    cells inside does not leak; the global range is the range of the volume."""
+    nx, ny, nz, B = 12, 8, 8, 4                      # 3 x 2 x 2 bricks
+    data = np.zeros((nz, ny, nx), dtype=np.float32)
+    data[1, 1, 3] = 7.5                              # last core cell of brick 0 along x -> ghost of brick 1
+    data[1, 1, 4] = -2.25                            # first core cell of brick 1 -> ghost of brick 0
+    data[6, 6, 10] = 9.0                             # two cells inside brick 11: nobody else sees it
+    vol = oracle.Volume(nx, ny, nz, B, 1, data=data)
+    assert vol.brick_minmax(0) == (np.float32(-2.25), np.float32(7.5))
+    assert vol.brick_minmax(1) == (np.float32(-2.25), np.float32(7.5))
+    assert vol.brick_minmax(2) == (np.float32(0.0), np.float32(0.0))
+    assert vol.brick_minmax(11) == (np.float32(0.0), np.float32(9.0))
+    for b in (3, 4, 5, 6, 7, 8, 9, 10):
+        assert vol.brick_minmax(b) == (np.float32(0.0), np.float32(0.0)), b
+    assert vol.brick_minmax(-1) == (np.float32(-2.25), np.float32(9.0))
+    # ghost = 0: the face voxels stay private
+    vol0 = oracle.Volume(nx, ny, nz, B, 0, data=data)
+    assert vol0.brick_minmax(0) == (np.float32(0.0), np.float32(7.5))
+    assert vol0.brick_minmax(1) == (np.float32(-2.25), np.float32(0.0))
+
+
+@pytest.mark.parametrize("ghost", [0, 1, 2])
+def test_brick_minmax_brute_force_ragged(ghost):
+    """Against numpy's edge padding (an independent statement of the clamp rule) on a ragged grid,
+    dense and procedural storage."""
+    cube = synth.Cube(31, 11, 9, 7, 2)
+    data = cube.fill_host()
+    B = 4
+    pad = np.pad(data, ghost, mode="edge")
+    for vol in (oracle.Volume(11, 9, 7, B, ghost, data=data), oracle.Volume(11, 9, 7, B, ghost, voxel_fn=cube.voxel_fn())):
+        b = 0
+        for bz in range(2):
+            for by in range(3):
+                for bx in range(3):
+                    x0, y0, z0 = bx * B, by * B, bz * B
+                    x1, y1, z1 = min(x0 + B, 11), min(y0 + B, 9), min(z0 + B, 7)
+                    box = pad[z0:z1 + 2 * ghost, y0:y1 + 2 * ghost, x0:x1 + 2 * ghost]
+                    assert vol.brick_minmax(b) == (box.min(), box.max()), b
+                    b += 1
+        assert vol.brick_minmax(-1) == (data.min(), data.max())
+
+
+def test_transparent_brick_rule_boundaries():
+    """R16 on constant bricks: entry range [I(min)-1, I(max)+2] must be all zero-alpha."""
+    n = 101                                          # table coordinate = value when vmin, vmax = 0, 100
+    def vol_of(value, alpha_nonzero):
+        v = oracle.Volume(4, 4, 4, 4, 1, data=np.full((4, 4, 4), value, dtype=np.float32))
+        tf = np.zeros((n, 4), dtype=np.float32)
+        tf[:, :3] = 0.5
+        tf[list(alpha_nonzero), 3] = 0.25
+        v.set_transfer_function(tf, 0.0, 100.0)
+        return v
+    hi = range(50, n)                                # opaque from entry 50 up
+    assert vol_of(47.5, hi).brick_transparent(0)     # I = 47 -> entries 46..49
+    assert not vol_of(48.5, hi).brick_transparent(0)  # I = 48 -> entries 47..50
+    assert not vol_of(60.0, hi).brick_transparent(0)
+    lo = range(0, 11)                                # opaque up to entry 10
+    assert not vol_of(11.5, lo).brick_transparent(0)  # I = 11 -> entries 10..13
+    assert vol_of(12.5, lo).brick_transparent(0)     # I = 12 -> entries 11..14
+    assert vol_of(-5.0, hi).brick_transparent(0)     # clamped below the table
+    assert not vol_of(500.0, hi).brick_transparent(0)  # clamped above: I = n-2 -> entries n-3..n-1
+    assert vol_of(500.0, lo).brick_transparent(0)
+
+
+def test_transparent_bricks_render_exactly_nothing():
+    """The point of R16: skipping a transparent brick changes no output bit, because all of its
+    samples classify to alpha 0 - its sub-image is exactly zero for every ray (ALPHA)."""
+    nx, ny, nz, B = 24, 16, 16, 8                    # 3 x 2 x 2 bricks
+    data = synth.Cube(5, nx, ny, nz, 3).fill_host()
+    faint = np.clip(data, -2.9, -1.2)
+    for (bx, by, bz) in ((0, 0, 0), (2, 1, 0), (1, 0, 1)):   # these bricks (with a margin for the ghosts) hold faint values only
+        x0, y0, z0 = max(bx * B - 1, 0), max(by * B - 1, 0), max(bz * B - 1, 0)
+        data[z0:bz * B + B + 1, y0:by * B + B + 1, x0:bx * B + B + 1] = faint[z0:bz * B + B + 1, y0:by * B + B + 1, x0:bx * B + B + 1]
+    vol = oracle.Volume(nx, ny, nz, B, 1, data=data)
+    tf = synth.tf_ramp()
+    tf[:64, 3] = 0.0                                 # zero opacity below u = 0.25 (value 0.25)
+    vol.set_transfer_function(tf, synth.TF_VMIN, synth.TF_VMAX)
+    transparent = [b for b in range(vol.nbricks) if vol.brick_transparent(b)]
+    assert transparent == [0, 5, 7]
+    W, H = 48, 36
+    fr = synth.Framing(nx, ny, nz, W, H)
+    r = vol.render(fr.seeded(3, 1), fr.proj(False), W, H, 0.5, oracle.ALPHA, want_sub=True)
+    sub = r["sub"].reshape(H * W, vol.nbricks, 4)
+    assert np.all(sub[:, transparent, :] == 0.0)
+    assert np.abs(sub[:, [b for b in range(vol.nbricks) if b not in transparent], 3]).max() > 0.1
