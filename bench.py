@@ -158,6 +158,15 @@ def build_volume(vr, wl, tf):
     up_ms = sum(a.elapsed_time(b) for a, b in evs)
     g.upload_stats = {"kernel": "vr_upload_tile442_kernel", "launches": len(evs), "ms": round(up_ms, 3), "bytes": up_bytes,
                       "gb_per_s": round(up_bytes / (up_ms * 1e-3) / 1e9, 1)}
+    # row f1 (once per upload): one streaming read of the padded brick store
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    lo, hi = g.minmax()
+    e1.record()
+    torch.cuda.synchronize()
+    mm_ms = e0.elapsed_time(e1)
+    g.minmax_stats = {"kernel": "vr_brick_minmax_kernel", "ms": round(mm_ms, 3), "bytes": 4 * pad,
+                      "gb_per_s": round(4 * pad / (mm_ms * 1e-3) / 1e9, 1), "data_min": float(lo), "data_max": float(hi)}
     return g, cube
 
 
@@ -278,6 +287,26 @@ def roofline_of(counts, stages, stage_views, peak_gbs, peak_src, traffic=None):
             "algorithmic_bytes_per_launch": round(alg / n), "launch_ms": round(ms / n, 4), "views_counted": n,
             "lines_bytes_per_launch": round(lines / n), "lines_gbs": round(lines_gbs, 1),
             "lines_frac": round(lines_gbs / peak_gbs, 4)}
+
+
+# SASS instructions of one trip of the ray-cast kernel's sample loop (4x4x2 layout, timed instance;
+# counted with `cuobjdump -sass` between the loop head and the backward branch after VOTE.ANY:
+# DESIGN.md "Kernels" lists them by kind). One trip = one sample for each of the warp's 32 rays.
+LOOP_INSTRUCTIONS = {"alpha": 123, "mip": 99}
+SM_COUNT, SCHEDULERS_PER_SM = 148, 4
+
+
+def roofline_alu(gsamples_per_s, mode, sm_mhz, traffic=None):
+    """Issue-slot bound of the sample loop, the bound of DENSELY sampled views (configs 0, 1, 2, 4:
+    >= 0.6 samples per voxel, every line is reused from L1/L2 and DRAM idles): peak = SMs x 4
+    warp schedulers x SM clock issue slots per second, x 32 samples per loop trip / instructions
+    per trip. `frac` therefore = issue-slot utilisation x the fraction of lanes doing a sample."""
+    clock = (sm_mhz or 1965.0) * 1e6
+    peak = SM_COUNT * SCHEDULERS_PER_SM * clock * 32.0 / LOOP_INSTRUCTIONS[mode] / 1e9
+    return {"bound": "alu", "kernel": "vr_raycast_kernel", "achieved": round(gsamples_per_s, 2), "peak": round(peak, 1),
+            "unit": "Gsamples/s", "frac": round(gsamples_per_s / peak, 4), "traffic": traffic,
+            "peak_source": "%d SMs x %d schedulers x %.0f MHz (max SM clock) x 32 lanes / %d SASS instructions per loop trip" % (
+                SM_COUNT, SCHEDULERS_PER_SM, clock / 1e6, LOOP_INSTRUCTIONS[mode])}
 
 
 def measured_peak():
@@ -444,7 +473,9 @@ def run_c4(args, vr, peak, peak_src, sampler):
         ms, nl, stages, _ = timed_device(g, w, 0, ids, K, Wm, img)
         launches += nl
         samples = sum(counts[ids[(Wm + k) % 36]]["samples"] for k in range(K))
+        ray_gs = samples / K / (float(stages[:, 1].mean()) * 1e-3) / 1e9
         sweep.append({"width": res, "height": res, "frames_per_s": round(K / (ms * 1e-3), 3),
+                      "roofline_alu": roofline_alu(ray_gs, "alpha", None),
                       "gsamples_per_s": round(samples / (ms * 1e-3) / 1e9, 3), "samples_per_frame": int(samples / K),
                       "stage_ms": {"setup": round(float(stages[:, 0].mean()), 4), "raycast": round(float(stages[:, 1].mean()), 4),
                                    "composite": round(float(stages[:, 2].mean()), 4)}})
@@ -567,7 +598,17 @@ def main():
                          "composite": round(float(m["stages"][:, 2].mean()), 4)},
             "roofline": roofline_of(m["counts"], m["stages"], m["stage_views"], peak, peak_src,
                                     traffic_of(args.workload, args.mode, args.tf)),
-            "build_s": round(t_build, 1), "upload": dict(g.upload_stats, frac_of_hbm_peak=round(g.upload_stats["gb_per_s"] / peak, 4))}
+            "build_s": round(t_build, 1), "upload": dict(g.upload_stats, frac_of_hbm_peak=round(g.upload_stats["gb_per_s"] / peak, 4)),
+            "minmax": dict(g.minmax_stats, frac_of_hbm_peak=round(g.minmax_stats["gb_per_s"] / peak, 4))}
+    # which roofline bounds the ray-cast kernel: DRAM for the sparsely sampled 103 GB cube (0.03 samples per
+    # voxel), issue slots for the densely sampled small cubes; the other one is reported beside it
+    smax = (m["clocks"] or {}).get("sm_max_mhz") if rank == 0 else None
+    ray_gs = m["samples"] / K / (float(m["stages"][:, 1].mean()) * 1e-3) / 1e9
+    alu = roofline_alu(ray_gs, args.mode, smax, traffic_of(args.workload, args.mode, args.tf))
+    if args.workload == "c3":
+        line["roofline_alu"] = alu
+    else:
+        line["roofline_hbm"], line["roofline"] = line["roofline"], alu
     cs = [s for s in m["counts"].values() if s["cells_touched"] >= 0]
     if cs:
         line["touched_per_frame"] = {"cells_gb": round(np.mean([4.0 * s["cells_touched"] for s in cs]) / 1e9, 3),

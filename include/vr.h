@@ -79,6 +79,8 @@ typedef struct vr_stats {
     float ms_setup;         /* per-stage device times of the last render, from CUDA events  */
     float ms_raycast;       /*   recorded on the render's stream; valid only if timing was   */
     float ms_composite;     /*   enabled with vr_set_timing, else -1                         */
+    int32_t bricks_culled;  /* bricks the view skipped as transparent (R16); 0 in MIP mode or
+                               with culling off */
 } vr_stats;
 
 /* ------------------------------------------------------------------------------------------
@@ -143,6 +145,27 @@ int vr_set_transfer_function(vr_volume* v, const float* rgba, int n, float vmin,
  * R8: a brick's ray stops, before taking a sample, once the brick-local accumulated opacity
  * is >= tau. Default 0.99; tau > 1 disables early termination. */
 int vr_set_early_termination(vr_volume* v, float tau);
+
+/* ------------------------------------------------------------------------------------------
+ * Data range. PAPER.md:146 (sec. 2.3.1): "An independent task to
+ * determine the local minimum and maximum starts when the data is loaded into the GPU memory";
+ * :152 the march may stop at "the maximum pixel value (defined by the global maximum of the
+ * data)". Local = per brick, over the brick's ghost-padded cells. The range is computed by one
+ * streaming pass over the brick store on the device, lazily, after the last upload: by
+ * vr_volume_minmax, or by the first vr_render that wants it (culling on). It gives the caller
+ * the data min/max for vr_set_transfer_function, lets MIP rays stop at the global maximum, and
+ * lets ALPHA frames skip transparent bricks.
+ *   vmin_out, vmax_out (host): range of the whole volume. Runs on `stream`, then waits for it.
+ * Errors: VR_ERR_STATE (nothing uploaded), VR_ERR_CUDA. */
+int vr_volume_minmax(vr_volume* v, float* vmin_out, float* vmax_out, void* stream);
+
+/* Transparent-brick culling (R16), default ON. In VR_ALPHA mode a brick is skipped for a frame
+ * (no rays, no sub-image, not composited) iff every transfer-function entry with index in
+ * [max(0, I(min_b) - 1), min(n - 1, I(max_b) + 2)] has alpha == 0, where
+ * I(x) = min((int)(sat((x - vmin) * inv_range) * (n - 1)), n - 2) in float32 is the entry a
+ * value classifies to; the widening absorbs the rounding of interpolated values. Such a brick
+ * contributes exact zeros, so the frame is bit-identical with culling on or off. */
+int vr_set_culling(vr_volume* v, int enable);
 
 /* ------------------------------------------------------------------------------------------
  * One frame (rows a2..a9): per-view set-up (inverse of proj*view, rendering rectangle of each
@@ -228,6 +251,9 @@ int vr_debug_ray_bricks(vr_volume* v, const float* view, const float* proj, int 
  * this handle with the same width/height (test access to row a8). sub_out: host
  * float[npix*nbricks*4]: VR_ALPHA premultiplied RGBA; VR_MIP (max, 0, 0, 0) with max = -inf
  * for "no sample". Bricks whose rectangle does not contain the pixel give zeros / -inf. */
+/* mm_out (host): nbricks * 2 floats, (min, max) per brick over its ghost-padded cells. */
+int vr_debug_brick_minmax(vr_volume* v, float* mm_out);
+
 int vr_debug_subimages(vr_volume* v, const int* pixels, int npix, float* sub_out);
 
 /* Counting in the ray-cast kernel (an instrumented variant of the same kernel: slower, never

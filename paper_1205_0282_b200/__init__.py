@@ -25,7 +25,7 @@ STATUS = {0: "VR_OK", 1: "VR_ERR_INVALID_ARG", 2: "VR_ERR_OUT_OF_MEMORY", 3: "VR
 # every symbol include/vr.h declares (tests check the library exports each of them)
 SYMBOLS = (
     "vr_volume_create", "vr_volume_create_layout", "vr_volume_destroy", "vr_volume_upload", "vr_volume_download", "vr_debug_brick_data",
-    "vr_set_transfer_function", "vr_set_early_termination", "vr_render", "vr_render_host", "vr_render_host_async", "vr_render_host_wait", "vr_composite",
+    "vr_set_transfer_function", "vr_set_early_termination", "vr_volume_minmax", "vr_set_culling", "vr_debug_brick_minmax", "vr_render", "vr_render_host", "vr_render_host_async", "vr_render_host_wait", "vr_composite",
     "vr_num_bricks", "vr_debug_brick_order", "vr_debug_rects", "vr_debug_ray_bricks", "vr_debug_subimages",
     "vr_set_counting", "vr_set_timing", "vr_debug_stats", "vr_debug_stage_times", "vr_launch_count", "vr_last_error",
 )
@@ -42,7 +42,8 @@ class Stats(ctypes.Structure):
                 ("subimage_bytes", ctypes.c_int64), ("cells_touched", ctypes.c_int64), ("sectors_touched", ctypes.c_int64),
                 ("lines_touched", ctypes.c_int64),
                 ("nbricks", ctypes.c_int32), ("overflow", ctypes.c_int32),
-                ("ms_setup", ctypes.c_float), ("ms_raycast", ctypes.c_float), ("ms_composite", ctypes.c_float)]
+                ("ms_setup", ctypes.c_float), ("ms_raycast", ctypes.c_float), ("ms_composite", ctypes.c_float),
+                ("bricks_culled", ctypes.c_int32)]
 
 
 _lib = None
@@ -66,6 +67,9 @@ def lib():
         L.vr_debug_brick_data.argtypes = [vp, ci, vp, vp]
         L.vr_set_transfer_function.argtypes = [vp, vp, ci, cf, cf]
         L.vr_set_early_termination.argtypes = [vp, cf]
+        L.vr_volume_minmax.argtypes = [vp, vp, vp, vp]
+        L.vr_set_culling.argtypes = [vp, ci]
+        L.vr_debug_brick_minmax.argtypes = [vp, vp]
         L.vr_render.argtypes = [vp, vp, vp, ci, ci, cf, ci, vp, vp]
         L.vr_render_host.argtypes = [vp, vp, vp, ci, ci, cf, ci, vp, vp]
         L.vr_render_host_async.argtypes = [vp, vp, vp, ci, ci, cf, ci, vp, vp]
@@ -176,6 +180,22 @@ class Volume:
 
     def set_early_termination(self, tau):
         self._check(lib().vr_set_early_termination(self._h, float(tau)))
+
+    # -- data range (f1) ---------------------------------------------------------
+    def minmax(self, stream=None):
+        """(min, max) of the uploaded volume as float32 (vr_volume_minmax)."""
+        mn, mx = ctypes.c_float(), ctypes.c_float()
+        self._check(lib().vr_volume_minmax(self._h, ctypes.byref(mn), ctypes.byref(mx), _stream(stream)))
+        return np.float32(mn.value), np.float32(mx.value)
+
+    def set_culling(self, enable):
+        self._check(lib().vr_set_culling(self._h, int(bool(enable))))
+
+    def debug_brick_minmax(self):
+        """[nbricks][2] float32: (min, max) per brick over its ghost-padded cells."""
+        mm = np.empty((self.nbricks, 2), dtype=np.float32)
+        self._check(lib().vr_debug_brick_minmax(self._h, mm.ctypes.data))
+        return mm
 
     # -- one frame (a2..a9) ---------------------------------------------------
     def render(self, view, proj, width, height, step, mode, out, stream=None):

@@ -39,6 +39,10 @@ struct vr_volume {
     long long pipe_frames;
     float* d_stage;          /* staging for VR_HOST upload / download */
     long long stage_floats;
+    int2* d_mm_enc;          /* row f1: per-brick range, order-preserving integer encoding */
+    float2* d_mm;            /* nbricks + 1 entries: per brick, then the whole volume */
+    bool mm_valid;           /* d_mm describes the current contents of the store */
+    bool culling;
     int counting;            /* 0 off, 1 samples, 2 samples + touched-cells bitmap */
     bool timing;
     unsigned* d_bitmap;      /* one bit per brick-store cell (counting == 2) */
@@ -98,6 +102,8 @@ static void release(vr_volume* v) {
     if (v->copy_stream) cudaStreamDestroy(v->copy_stream);
     cudaFree(v->d_stage);
     cudaFree(v->d_bitmap);
+    cudaFree(v->d_mm_enc);
+    cudaFree(v->d_mm);
     cudaFree(v->d_counts2);
     for (int r = 0; r < VR_EV_RING; ++r)
         for (int i = 0; i < 4; ++i)
@@ -215,6 +221,7 @@ extern "C" int vr_volume_create_layout(int nx, int ny, int nz, int brick, int gh
         return fail(NULL, VR_ERR_INVALID_ARG, "vr_volume_create: a padded brick of %d^3 cells exceeds 2^31 floats", g.P);
     }
     v->tau = 0.99f;
+    v->culling = true;
 
     cudaError_t e = cudaMalloc(&v->bricks, (size_t)g.slot * (size_t)g.nbricks * sizeof(float));
     if (e == cudaSuccess) e = cudaMemset(v->bricks, 0, (size_t)g.slot * (size_t)g.nbricks * sizeof(float));
@@ -226,6 +233,8 @@ extern "C" int vr_volume_create_layout(int nx, int ny, int nz, int brick, int gh
     if (e == cudaSuccess) e = cudaMalloc(&v->d_order, sizeof(int) * g.nbricks);
     if (e == cudaSuccess) e = cudaMalloc(&v->d_item_prefix, sizeof(int) * (g.nbricks + 1));
     if (e == cudaSuccess) e = cudaMalloc(&v->d_layers, sizeof(VrCompLayer) * g.nbricks);
+    if (e == cudaSuccess) e = cudaMalloc(&v->d_mm_enc, sizeof(int2) * g.nbricks);
+    if (e == cudaSuccess) e = cudaMalloc(&v->d_mm, sizeof(float2) * (g.nbricks + 1));
     for (int r = 0; r < VR_EV_RING && e == cudaSuccess; ++r)
         for (int i = 0; i < 4 && e == cudaSuccess; ++i) e = cudaEventCreate(&v->ev[r][i]);
     if (e != cudaSuccess) {
@@ -295,6 +304,7 @@ extern "C" int vr_volume_upload(vr_volume* v, const float* src, int memspace, in
         }
     }
     v->has_data = true;
+    v->mm_valid = false;
     return VR_OK;
 }
 
@@ -440,13 +450,59 @@ static int ensure_sub(vr_volume* v, long long need_px) {
     return VR_OK;
 }
 
-static int run_setup(vr_volume* v, const float* view, const float* proj, int W, int H, int mode, cudaStream_t st) {
+/* Row f1: bring the range table up to date with the store (three launches, after an upload only). */
+static int ensure_minmax(vr_volume* v, cudaStream_t st) {
+    if (v->mm_valid) return VR_OK;
+    VR_CUDA(v, vr_launch_minmax(v->grid, v->bricks, v->d_mm_enc, v->d_mm, st));
+    v->launches += 3;
+    v->mm_valid = true;
+    return VR_OK;
+}
+
+static int run_setup(vr_volume* v, const float* view, const float* proj, int W, int H, int mode, bool use_range,
+                     cudaStream_t st) {
     VrMatrices m;
     memcpy(m.view, view, sizeof(m.view));
     memcpy(m.proj, proj, sizeof(m.proj));
+    if (use_range) {
+        const int rc = ensure_minmax(v, st);
+        if (rc) return rc;
+    }
     VR_CUDA(v, vr_launch_setup(v->grid, m, W, H, mode, v->sub_capacity_px, v->d_sub, v->d_vs, v->d_bv, v->d_order,
-                               v->d_item_prefix, v->d_layers, st));
+                               v->d_item_prefix, v->d_layers, use_range ? v->d_mm : NULL, v->lut, st));
     v->launches++;
+    return VR_OK;
+}
+
+extern "C" int vr_volume_minmax(vr_volume* v, float* vmin_out, float* vmax_out, void* stream) {
+    if (!v) return fail(NULL, VR_ERR_INVALID_ARG, "vr_volume_minmax: NULL handle");
+    if (!vmin_out || !vmax_out) return fail(v, VR_ERR_INVALID_ARG, "vr_volume_minmax: NULL output");
+    if (!v->has_data) return fail(v, VR_ERR_STATE, "vr_volume_minmax: nothing uploaded");
+    cudaStream_t st = (cudaStream_t)stream;
+    const int rc = ensure_minmax(v, st);
+    if (rc) return rc;
+    float2 mm;
+    VR_CUDA(v, cudaMemcpyAsync(&mm, v->d_mm + v->grid.nbricks, sizeof(mm), cudaMemcpyDeviceToHost, st));
+    VR_CUDA(v, cudaStreamSynchronize(st));
+    *vmin_out = mm.x;
+    *vmax_out = mm.y;
+    return VR_OK;
+}
+
+extern "C" int vr_set_culling(vr_volume* v, int enable) {
+    if (!v) return fail(NULL, VR_ERR_INVALID_ARG, "vr_set_culling: NULL handle");
+    v->culling = enable != 0;
+    return VR_OK;
+}
+
+extern "C" int vr_debug_brick_minmax(vr_volume* v, float* mm_out) {
+    if (!v) return fail(NULL, VR_ERR_INVALID_ARG, "vr_debug_brick_minmax: NULL handle");
+    if (!mm_out) return fail(v, VR_ERR_INVALID_ARG, "vr_debug_brick_minmax: NULL output");
+    if (!v->has_data) return fail(v, VR_ERR_STATE, "vr_debug_brick_minmax: nothing uploaded");
+    const int rc = ensure_minmax(v, 0);
+    if (rc) return rc;
+    VR_CUDA(v, cudaDeviceSynchronize());
+    VR_CUDA(v, cudaMemcpy(mm_out, v->d_mm, sizeof(float2) * v->grid.nbricks, cudaMemcpyDeviceToHost));
     return VR_OK;
 }
 
@@ -466,8 +522,12 @@ extern "C" int vr_render(vr_volume* v, const float* view, const float* proj, int
     const bool timing = v->timing;
     cudaEvent_t* ev = v->ev[v->timed_frames % VR_EV_RING];
 
+    if (v->culling) { /* after an upload only: the range pass is not part of the frame's stages */
+        rc = ensure_minmax(v, st);
+        if (rc) return rc;
+    }
     if (timing) VR_CUDA(v, cudaEventRecord(ev[0], st));
-    rc = run_setup(v, view, proj, width, height, mode, st);
+    rc = run_setup(v, view, proj, width, height, mode, v->culling, st);
     if (rc) return rc;
     if (timing) VR_CUDA(v, cudaEventRecord(ev[1], st));
 
@@ -633,7 +693,7 @@ static int debug_setup(vr_volume* v, const char* who, const float* view, const f
     if (rc) return rc;
     rc = ensure_sub(v, sub_px);
     if (rc) return rc;
-    rc = run_setup(v, view, proj, W, H, VR_ALPHA, 0);
+    rc = run_setup(v, view, proj, W, H, VR_ALPHA, false, 0);
     if (rc) return rc;
     v->last_valid = false; /* the sub-image offsets of the last frame are gone */
     VR_CUDA(v, cudaDeviceSynchronize());
@@ -750,6 +810,7 @@ extern "C" int vr_debug_stats(vr_volume* v, vr_stats* out) {
     }
     out->nbricks = v->grid.nbricks;
     out->overflow = vs.overflow;
+    out->bricks_culled = vs.culled;
     out->ms_setup = out->ms_raycast = out->ms_composite = -1.0f;
     if (v->timing && v->timed_frames > 0) {
         cudaEvent_t* ev = v->ev[(v->timed_frames - 1) % VR_EV_RING];

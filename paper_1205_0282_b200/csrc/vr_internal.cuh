@@ -78,6 +78,8 @@ struct VrViewState {
     unsigned int work_counter;
     unsigned int pad0;
     unsigned long long samples;
+    float data_max; /* global maximum of the data if known, else +inf (MIP stop) */
+    int culled;     /* bricks skipped as transparent in this view (R16) */
 };
 
 struct VrBrickView {
@@ -134,9 +136,11 @@ __host__ __device__ __forceinline__ unsigned vr_cell_offset(const VrGrid& g, int
 }
 
 /* ---- launchers (each returns the cudaError of its launch) ---- */
+/* range: float2[nbricks + 1] (per brick, then the whole volume) or NULL = unknown, no culling */
 cudaError_t vr_launch_setup(const VrGrid& grid, const VrMatrices& mats, int W, int H, int mode,
                             long long sub_capacity_px, void* sub_base, VrViewState* vs, VrBrickView* bv, int* order,
-                            int* item_prefix, VrCompLayer* layers, cudaStream_t st);
+                            int* item_prefix, VrCompLayer* layers, const float2* range, const VrLut& lut, cudaStream_t st);
+cudaError_t vr_launch_minmax(const VrGrid& grid, const float* bricks, int2* enc, float2* table, cudaStream_t st);
 /* items = work items of the view (sizes the persistent grid) */
 cudaError_t vr_launch_raycast(const VrRaycastParams& p, long long items, bool count, cudaStream_t st);
 cudaError_t vr_launch_composite(const VrCompLayer* layers, const int* order, int n, int W, int H, int mode,

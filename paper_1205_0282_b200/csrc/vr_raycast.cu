@@ -477,7 +477,9 @@ vr_raycast_kernel(const VrRaycastParams prm) {
         lut.base = (unsigned)__cvta_generic_to_shared(s_lut);
         asm volatile("" : "+r"(lut.base)); /* one register, not rebuilt per sample */
     }
-    const float mip_stop = prm.lut.vmax; /* the output saturates at vmax */
+    /* MIP may stop where the output saturates (vmax) or at the global maximum of the data when
+     * it is known ("the maximum pixel value (defined by the global maximum of the data)") */
+    const float mip_stop = fminf(prm.lut.vmax, prm.vs->data_max);
     unsigned long long nsamples = 0;
 
     /* one atomic per item; the next item is requested before the current one is processed */

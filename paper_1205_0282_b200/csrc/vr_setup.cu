@@ -11,6 +11,10 @@
  *      (Fig. 4 :168), launch rectangle on the 8x4 tile grid, tile counts.
  *   4. Exclusive scans, in visibility order, of the tile counts (work list of the persistent
  *      ray-cast kernel) and of the sub-image sizes (scratch offsets); compositing table.
+ *   5. Row f1: with the per-brick data range known (vr_minmax.cu), ALPHA frames skip the bricks
+ *      the transfer function makes transparent (R16: every table entry the brick's values can
+ *      interpolate between has alpha 0, entry range widened by -1/+2): no work items, no
+ *      sub-image, an empty compositing rectangle. Exact: such a brick contributes zeros.
  */
 #include "vr_view.cuh"
 
@@ -25,12 +29,15 @@ struct SetupShared {
     long long carry_pix;
     int ortho;
     double eye[3];
+    int culled;
+    unsigned short nz_prefix[VR_MAX_LUT + 1]; /* nz_prefix[i] = entries < i with alpha != 0 */
 };
 
 __global__ void __launch_bounds__(SETUP_THREADS)
 vr_setup_kernel(VrGrid grid, VrMatrices mats, int W, int H, int mode, long long sub_capacity_px,
                 unsigned long long sub_base, VrViewState* __restrict__ vs, VrBrickView* __restrict__ bv,
-                int* __restrict__ order, int* __restrict__ item_prefix, VrCompLayer* __restrict__ layers) {
+                int* __restrict__ order, int* __restrict__ item_prefix, VrCompLayer* __restrict__ layers,
+                const float2* __restrict__ range, VrLut lut) {
     __shared__ SetupShared sh;
     const int tid = threadIdx.x;
 
@@ -52,6 +59,17 @@ vr_setup_kernel(VrGrid grid, VrMatrices mats, int W, int H, int mode, long long 
         vs->samples = 0ull;
         sh.carry_items = 0;
         sh.carry_pix = 0;
+        sh.culled = 0;
+        vs->data_max = range ? range[grid.nbricks].y : INFINITY;
+    }
+    const bool cull = range != NULL && mode == VR_ALPHA && lut.base != NULL;
+    if (cull) { /* flags in parallel, then a serial prefix over at most 1024 entries of shared memory */
+        for (int i = tid; i < lut.n; i += SETUP_THREADS) sh.nz_prefix[i + 1] = lut.base[i].w != 0.0f ? 1 : 0;
+        __syncthreads();
+        if (tid == 0) {
+            sh.nz_prefix[0] = 0;
+            for (int i = 1; i <= lut.n; ++i) sh.nz_prefix[i] = (unsigned short)(sh.nz_prefix[i] + sh.nz_prefix[i - 1]);
+        }
     }
     __syncthreads();
 
@@ -88,6 +106,17 @@ vr_setup_kernel(VrGrid grid, VrMatrices mats, int W, int H, int mode, long long 
         const int key = (sh.rank[2][bc[2]] * grid.g[1] + sh.rank[1][bc[1]]) * grid.g[0] + sh.rank[0][bc[0]];
         order[key] = b;
         vr_rect_of_box(sh.M, lo, hi, W, H, r);
+        if (cull) { /* R16, float32 as the ray-cast kernel classifies */
+            const float2 mm = range[b];
+            const float ulo = __saturatef(__fmul_rn(__fsub_rn(mm.x, lut.vmin), lut.inv_range));
+            const float uhi = __saturatef(__fmul_rn(__fsub_rn(mm.y, lut.vmin), lut.inv_range));
+            const int i0 = max(min((int)__fmul_rn(ulo, lut.scale), lut.nm2) - 1, 0);
+            const int i1 = min(min((int)__fmul_rn(uhi, lut.scale), lut.nm2) + 2, lut.n - 1);
+            if (sh.nz_prefix[i1 + 1] == sh.nz_prefix[i0] && r[2] > r[0] && r[3] > r[1]) {
+                r[2] = r[0]; /* empty rectangle: nothing to cast, nothing to composite */
+                atomicAdd(&sh.culled, 1);
+            }
+        }
         vr_launch_rect(r, W, H, l);
         VrBrickView v;
         v.rx0 = r[0]; v.ry0 = r[1]; v.rx1 = r[2]; v.ry1 = r[3];
@@ -154,6 +183,7 @@ vr_setup_kernel(VrGrid grid, VrMatrices mats, int W, int H, int mode, long long 
         vs->total_items = over ? 0 : sh.carry_items;
         vs->total_sub_pixels = sh.carry_pix;
         vs->overflow = over;
+        vs->culled = sh.culled;
     }
     __syncthreads();
 
@@ -174,9 +204,10 @@ vr_setup_kernel(VrGrid grid, VrMatrices mats, int W, int H, int mode, long long 
 
 cudaError_t vr_launch_setup(const VrGrid& grid, const VrMatrices& mats, int W, int H, int mode, long long sub_capacity_px,
                             void* sub_base, VrViewState* vs, VrBrickView* bv, int* order, int* item_prefix,
-                            VrCompLayer* layers, cudaStream_t st) {
+                            VrCompLayer* layers, const float2* range, const VrLut& lut, cudaStream_t st) {
     vr_setup_kernel<<<1, SETUP_THREADS, 0, st>>>(grid, mats, W, H, mode, sub_capacity_px,
-                                                 (unsigned long long)(uintptr_t)sub_base, vs, bv, order, item_prefix, layers);
+                                                 (unsigned long long)(uintptr_t)sub_base, vs, bv, order, item_prefix, layers,
+                                                 range, lut);
     return cudaGetLastError();
 }
 

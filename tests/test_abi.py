@@ -35,7 +35,7 @@ def test_library_exports_every_declared_symbol(vr):
 
 
 def test_stats_struct_layout(vr):
-    # int64 x7, int32 x2, float x3 (+ padding to 8)
+    # int64 x7, int32 x2, float x3, int32 (bricks_culled, in what used to be tail padding)
     assert ctypes.sizeof(vr.Stats) == 80
 
 

@@ -180,6 +180,87 @@ def test_pipelined_host_frames_equal_synchronous_ones(vr):
     check_mip(bufs[0].numpy().astype(np.float64), ref["image"], "pipelined frame 0")
 
 
+# --------------------------------------------------------------------------- f1 data range, culling
+@pytest.mark.parametrize("layout", ["tiled", "linear"])
+@pytest.mark.parametrize("ghost", [0, 1, 2])
+def test_brick_minmax_is_exact(vr, layout, ghost):
+    """Per-brick and global data range on a ragged grid: bit-equal to the oracle's."""
+    cube = synth.Cube(41, 45, 38, 27, 4)
+    data = cube.fill_host()
+    lay = vr.LAYOUT_TILED if layout == "tiled" else vr.LAYOUT_LINEAR
+    g = vr.Volume(45, 38, 27, 16, ghost, layout=lay)
+    g.upload(data)
+    o = oracle.Volume(45, 38, 27, 16, ghost, data=data)
+    mm = g.debug_brick_minmax()
+    for b in range(g.nbricks):
+        assert tuple(mm[b]) == o.brick_minmax(b), b
+    assert g.minmax() == o.brick_minmax(-1) == (data.min(), data.max())
+    # a second upload invalidates the table: overwrite one voxel with a new maximum
+    spike = np.full((1, 1, 1), 99.0, dtype=np.float32)
+    g.upload(spike, origin=(44, 37, 26))
+    assert g.minmax() == (data.min(), np.float32(99.0))
+
+
+def sparse_cube(nx, ny, nz, B, seed):
+    """N-body-like stand-in (Table 1 :221, the paper's other data family): most bricks hold
+    only faint values (below the opacity threshold of the test's transfer function), a few hold
+    the usual noise + sources."""
+    data = synth.Cube(seed, nx, ny, nz, 6).fill_host()
+    faint = np.clip(data, -2.9, -1.2)
+    gx, gy, gz = -(-nx // B), -(-ny // B), -(-nz // B)
+    for bz in range(gz):
+        for by in range(gy):
+            for bx in range(gx):
+                if synth.u01(seed, 91, (bz * gy + by) * gx + bx) < 0.6:
+                    x0, y0, z0 = max(bx * B - 1, 0), max(by * B - 1, 0), max(bz * B - 1, 0)
+                    sl = (slice(z0, bz * B + B + 1), slice(y0, by * B + B + 1), slice(x0, bx * B + B + 1))
+                    data[sl] = faint[sl]
+    return data
+
+
+def test_transparent_bricks_are_culled_exactly(vr):
+    """R16: the set of culled bricks equals the oracle's transparent set, the frame still matches
+    the oracle, and it is bit-identical with culling switched off."""
+    import torch
+    nx, ny, nz, B = 96, 72, 64, 16
+    data = sparse_cube(nx, ny, nz, B, 17)
+    tf = synth.tf_ramp()
+    tf[:64, 3] = 0.0
+    g = vr.Volume(nx, ny, nz, B, 1)
+    g.upload(data)
+    o = oracle.Volume(nx, ny, nz, B, 1, data=data)
+    for v in (g, o):
+        v.set_transfer_function(tf, synth.TF_VMIN, synth.TF_VMAX)
+        v.set_early_termination(0.99)
+    transparent = [b for b in range(o.nbricks) if o.brick_transparent(b)]
+    assert 10 < len(transparent) < o.nbricks - 10
+    W, H = 200, 150
+    fr = synth.Framing(nx, ny, nz, W, H)
+    view, proj = fr.seeded(8, 2), fr.proj(False)
+    on = gpu_frame(g, view, proj, W, H, 0.5, vr.ALPHA)
+    st = g.debug_stats()
+    rects = o.rects(view, proj, W, H)
+    visible = [b for b in transparent if rects[b][2] > rects[b][0] and rects[b][3] > rects[b][1]]
+    assert st["bricks_culled"] == len(visible)
+    pix = seeded_pixels(3, W, H, 64)
+    subs = g.debug_subimages(pix)                    # [npix][nbricks][4]: culled bricks deliver nothing
+    assert np.all(subs[:, transparent, :] == 0.0)
+    ref = o.render(view, proj, W, H, 0.5, oracle.ALPHA)
+    check_alpha(on, ref["image"], ref["flags"], 0.99, "culled frame")
+    g.set_culling(False)
+    off = gpu_frame(g, view, proj, W, H, 0.5, vr.ALPHA)
+    assert g.debug_stats()["bricks_culled"] == 0
+    assert np.array_equal(on, off)
+    # MIP never culls, and stops at the global maximum of the data without changing the frame
+    g.set_culling(True)
+    m_on = gpu_frame(g, view, proj, W, H, 0.5, vr.MIP)
+    assert g.debug_stats()["bricks_culled"] == 0
+    g.set_culling(False)
+    m_off = gpu_frame(g, view, proj, W, H, 0.5, vr.MIP)
+    assert np.array_equal(m_on, m_off)
+    check_mip(m_on, o.render(view, proj, W, H, 0.5, oracle.MIP)["image"], "MIP with data-max stop")
+
+
 # --------------------------------------------------------------------------- edge cases
 def test_edge_cases(vr):
     import torch
