@@ -458,9 +458,11 @@ def run_c4(args, vr, peak, peak_src, sampler):
 
     # (i) resolution sweep on config 2's cube
     wl = workload("c2")
-    g, _ = build_volume(vr, wl, synth.tf_ramp())
     sweep, launches = [], K
-    for res in (512, 1024, 2048, 4096):
+    g = None
+    if args.c4_part != "composite":
+        g, _ = build_volume(vr, wl, synth.tf_ramp())
+    for res in ((512, 1024, 2048, 4096) if g is not None else ()):
         w = dict(wl)
         w["width"] = w["height"] = res
         fr = synth.Framing(w["nx"], w["ny"], w["nz"], res, res)
@@ -480,8 +482,9 @@ def run_c4(args, vr, peak, peak_src, sampler):
                       "stage_ms": {"setup": round(float(stages[:, 0].mean()), 4), "raycast": round(float(stages[:, 1].mean()), 4),
                                    "composite": round(float(stages[:, 2].mean()), 4)}})
         del img
-    g.close()
-    top = sweep[-1]
+    if g is not None:
+        g.close()
+    top = sweep[-1] if sweep else {"frames_per_s": round(1e3 / float(comp_ms.mean()), 3), "gsamples_per_s": None}
     return {"metric": METRIC, "value": top["frames_per_s"], "unit": "frames/s", "n_gpus": 1, "steps": K, "warmup": Wm,
             "ms_per_step": round(1e3 / top["frames_per_s"], 4), "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32", "data": "synthetic",
@@ -505,6 +508,8 @@ def main():
     ap.add_argument("--mode", default="alpha", choices=["alpha", "mip"])
     ap.add_argument("--tf", default="ramp", choices=["ramp", "translucent"])
     ap.add_argument("--cells-every", type=int, default=6, help="count distinct cells on every n-th view of the cycle (0 = never)")
+    ap.add_argument("--c4-part", default="both", choices=["both", "composite"],
+                    help="--workload c4: `composite` runs only the compositing microbenchmark (profiling)")
     ap.add_argument("--no-variants", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
