@@ -189,6 +189,19 @@ int vr_set_culling(vr_volume* v, int enable);
 int vr_render(vr_volume* v, const float* view, const float* proj, int width, int height,
               float step, int mode, float* out_rgba, void* stream);
 
+/* Traversal. VR_SORT_LAST (default) is the path above: every brick
+ * renders its own sub-image with BRICK-LOCAL early termination (R8) and the sub-images are
+ * composited in visibility order, as the paper's GPUs do.
+ * VR_FUSED marches one ray per frame pixel through all the bricks it crosses, front to back,
+ * with one accumulator and GLOBAL early termination, and writes the frame directly: no
+ * sub-images, no compositing pass. R17: the result is what VR_SORT_LAST gives for a volume
+ * held in a single brick (same sample schedule, R5; same voxels, R3), early termination
+ * included; with early termination off the two traversals agree to rounding.
+ * vr_debug_subimages and the transparent-brick counter do not apply to fused frames. */
+#define VR_SORT_LAST 0
+#define VR_FUSED 1
+int vr_set_traversal(vr_volume* v, int traversal);
+
 /* Same frame, delivered to HOST memory: renders into a library-owned device frame, copies it
  * to out_rgba_host ([height][width][4] float32; pinned memory makes the copy asynchronous
  * with respect to other streams) and waits for the copy. This is the end-to-end entry. */

@@ -43,6 +43,7 @@ struct vr_volume {
     float2* d_mm;            /* nbricks + 1 entries: per brick, then the whole volume */
     bool mm_valid;           /* d_mm describes the current contents of the store */
     bool culling;
+    int traversal;           /* VR_SORT_LAST or VR_FUSED */
     int counting;            /* 0 off, 1 samples, 2 samples + touched-cells bitmap */
     bool timing;
     unsigned* d_bitmap;      /* one bit per brick-store cell (counting == 2) */
@@ -51,7 +52,8 @@ struct vr_volume {
     cudaEvent_t ev[VR_EV_RING][4]; /* stage boundaries of the last VR_EV_RING timed frames */
     long long timed_frames;  /* frames rendered since timing was switched on */
     int last_W, last_H, last_mode;
-    bool last_valid;
+    bool last_valid;       /* the last frame's sub-images are still in the scratch */
+    bool last_stats_valid; /* the last frame's counters are still in the view state */
     int64_t launches;
     char err[512];
 };
@@ -489,6 +491,14 @@ extern "C" int vr_volume_minmax(vr_volume* v, float* vmin_out, float* vmax_out, 
     return VR_OK;
 }
 
+extern "C" int vr_set_traversal(vr_volume* v, int traversal) {
+    if (!v) return fail(NULL, VR_ERR_INVALID_ARG, "vr_set_traversal: NULL handle");
+    if (traversal != VR_SORT_LAST && traversal != VR_FUSED)
+        return fail(v, VR_ERR_INVALID_ARG, "vr_set_traversal: unknown traversal %d", traversal);
+    v->traversal = traversal;
+    return VR_OK;
+}
+
 extern "C" int vr_set_culling(vr_volume* v, int enable) {
     if (!v) return fail(NULL, VR_ERR_INVALID_ARG, "vr_set_culling: NULL handle");
     v->culling = enable != 0;
@@ -550,12 +560,17 @@ extern "C" int vr_render(vr_volume* v, const float* view, const float* proj, int
     p.stepf = step;
     p.tau = v->tau;
     p.mode = mode;
-    VR_CUDA(v, vr_launch_raycast(p, items, v->counting != 0, st));
-    v->launches++;
-    if (timing) VR_CUDA(v, cudaEventRecord(ev[2], st));
-
-    VR_CUDA(v, vr_launch_composite(v->d_layers, v->d_order, v->grid.nbricks, width, height, mode, v->lut, out_rgba, st));
-    v->launches++;
+    if (v->traversal == VR_FUSED) {
+        VR_CUDA(v, vr_launch_fused(p, out_rgba, width, height, v->counting != 0, st));
+        v->launches++;
+        if (timing) VR_CUDA(v, cudaEventRecord(ev[2], st));
+    } else {
+        VR_CUDA(v, vr_launch_raycast(p, items, v->counting != 0, st));
+        v->launches++;
+        if (timing) VR_CUDA(v, cudaEventRecord(ev[2], st));
+        VR_CUDA(v, vr_launch_composite(v->d_layers, v->d_order, v->grid.nbricks, width, height, mode, v->lut, out_rgba, st));
+        v->launches++;
+    }
     if (timing) {
         VR_CUDA(v, cudaEventRecord(ev[3], st));
         v->timed_frames++;
@@ -563,7 +578,8 @@ extern "C" int vr_render(vr_volume* v, const float* view, const float* proj, int
     v->last_W = width;
     v->last_H = height;
     v->last_mode = mode;
-    v->last_valid = true;
+    v->last_valid = v->traversal == VR_SORT_LAST; /* fused frames leave no sub-images to inspect */
+    v->last_stats_valid = true;
     return VR_OK;
 }
 
@@ -696,6 +712,7 @@ static int debug_setup(vr_volume* v, const char* who, const float* view, const f
     rc = run_setup(v, view, proj, W, H, VR_ALPHA, false, 0);
     if (rc) return rc;
     v->last_valid = false; /* the sub-image offsets of the last frame are gone */
+    v->last_stats_valid = false;
     VR_CUDA(v, cudaDeviceSynchronize());
     return VR_OK;
 }
@@ -789,7 +806,7 @@ extern "C" int vr_debug_subimages(vr_volume* v, const int* pixels, int npix, flo
 extern "C" int vr_debug_stats(vr_volume* v, vr_stats* out) {
     if (!v) return fail(NULL, VR_ERR_INVALID_ARG, "vr_debug_stats: NULL handle");
     if (!out) return fail(v, VR_ERR_INVALID_ARG, "vr_debug_stats: NULL output");
-    if (!v->last_valid) return fail(v, VR_ERR_STATE, "vr_debug_stats: no vr_render since the last debug call");
+    if (!v->last_stats_valid) return fail(v, VR_ERR_STATE, "vr_debug_stats: no vr_render since the last debug call");
     VR_CUDA(v, cudaDeviceSynchronize());
     VrViewState vs;
     VR_CUDA(v, cudaMemcpy(&vs, v->d_vs, sizeof(vs), cudaMemcpyDeviceToHost));

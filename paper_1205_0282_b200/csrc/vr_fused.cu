@@ -1,0 +1,228 @@
+/*
+ * vr_fused.cu -- fused front-to-back traversal: one ray per
+ * frame pixel walks the bricks it crosses in order, with ONE accumulator, and writes the frame
+ * directly. No sub-images, no compositing pass, and early ray termination is GLOBAL: a ray
+ * that is opaque after its first brick never touches the bricks behind it.
+ *
+ * PAPER.md:152 (sec. 2.3.2) is the march of one ray through "the bounding cube" until the exit
+ * point, the maximum or the opacity is reached; the paper splits that march into sub-cubes
+ * only because its cube does not fit one GPU (:105, :113) and then pays for sub-frames and
+ * compositing (:114, :156-184). On one B200 the whole cube is resident, so the split is only a
+ * memory layout: the sample schedule is the ray's own (R5: anchored at the entry into the
+ * whole volume), each sample is read from the brick that owns it (R6; ghosts make it
+ * seam-free, R3), and the result is what the sort-last path gives for a single brick covering
+ * the volume (R17) - with early termination ON as well, which sort-last cannot offer (R8).
+ *
+ * Work decomposition: persistent warps pull 8x4-pixel tiles of the FRAME (one atomic per
+ * tile). Per ray: FP64 set-up once; per brick crossed: the owner brick of the next sample and
+ * the integer sample range it owns (the same exact arithmetic as vr_raycast.cu), then the
+ * float32 lattice march of vr_march.cuh.
+ */
+#include "vr_march.cuh"
+
+template <int MODE, int LAY, bool CLAMP, bool COUNT>
+__global__ void __launch_bounds__(VR_RAYCAST_THREADS, VR_MIN_CTAS)
+vr_fused_kernel(const VrRaycastParams prm, float4* __restrict__ frame) {
+    extern __shared__ float4 s_lut[]; /* (entry, delta) pairs: shading (ALPHA), final colour map (MIP) */
+    __shared__ double s_minv[16];
+
+    const VrGrid& g = prm.grid;
+    const int lane = threadIdx.x & 31;
+    for (int i = threadIdx.x; i < prm.lut.n; i += blockDim.x) {
+        s_lut[2 * i] = prm.lut.base[i];
+        s_lut[2 * i + 1] = prm.lut.delta[i];
+    }
+    if (threadIdx.x < 16) s_minv[threadIdx.x] = prm.vs->Minv[threadIdx.x];
+    __syncthreads();
+    if (prm.vs->singular) return;
+
+    const int W = prm.vs->W, H = prm.vs->H;
+    const int tiles_x = (W + VR_TILE_W - 1) / VR_TILE_W, tiles_y = (H + VR_TILE_H - 1) / VR_TILE_H;
+    const unsigned total = (unsigned)(tiles_x * tiles_y);
+    const double step = prm.step;
+    const float tau = prm.tau;
+    LutView lut;
+    lut.base = (unsigned)__cvta_generic_to_shared(s_lut);
+    asm volatile("" : "+r"(lut.base));
+    const float mip_stop = fminf(prm.lut.vmax, prm.vs->data_max);
+    unsigned long long nsamples = 0;
+
+    unsigned next = 0;
+    if (lane == 0) next = atomicAdd(&prm.vs_rw->work_counter, 1u);
+    next = __shfl_sync(FULL_MASK, next, 0);
+
+    while (next < total) {
+        const int item = (int)next;
+        if (lane == 0) next = atomicAdd(&prm.vs_rw->work_counter, 1u);
+        const int ty = item / tiles_x, tx = item - ty * tiles_x;
+        const int pi = tx * VR_TILE_W + (lane & 7), pj = ty * VR_TILE_H + (lane >> 3);
+        const bool in_frame = pi < W && pj < H;
+
+        RaySetup ray;
+        ray.K = 0;
+        if (in_frame) ray_setup(s_minv, W, H, pi, pj, g, step, ray);
+
+        Accum acc;
+        acc.r = (MODE == VR_MIP) ? -INFINITY : 0.0f;
+        acc.g = acc.b = acc.a = 0.0f;
+        bool stopped = (MODE == VR_ALPHA) ? !(acc.a < tau) : false;
+        int k = 0; /* next sample of the ray's schedule */
+
+        /* one trip per brick the ray crosses */
+        while (__any_sync(FULL_MASK, k < ray.K && !stopped)) {
+            const bool live = k < ray.K && !stopped;
+            int bc[3] = {0, 0, 0}, blo[3], bhi[3], ext[3];
+            int k_lo = k, k_hi = k + 1;
+            bool owned = false;
+            if (live) {
+                double s, w;
+                owned = sample_sw(ray, step, k, s, w); /* an empty interval is dropped (R5) */
+                if (owned) {
+#pragma unroll
+                    for (int a = 0; a < 3; ++a) bc[a] = owner_axis(ray, g, s, a); /* R6: the brick that owns sample k */
+                }
+            }
+            vr_brick_core(g, bc, blo, bhi);
+#pragma unroll
+            for (int a = 0; a < 3; ++a) ext[a] = bhi[a] - blo[a] + 2 * g.ghost;
+            if (owned) {
+                brick_range(ray, g, step, bc, blo, bhi, k_lo, k_hi);
+                if (k_hi <= k) k_hi = k + 1; /* cannot happen (sample k is owned by bc); guarantees progress */
+            }
+            const int b = (bc[2] * g.g[1] + bc[1]) * g.g[0] + bc[0];
+            const float* __restrict__ brick = prm.bricks + (long long)b * g.slot;
+
+            const int k_lat = min(k_hi, max(k, ray.K - 2));
+            int n = owned ? k_lat - k : 0;
+            Lattice L;
+            long long D[3];
+            if (n > 0) {
+                double s, w;
+                sample_sw(ray, step, k, s, w);
+#pragma unroll
+                for (int a = 0; a < 3; ++a) {
+                    const double p = VR_FMA(s, ray.d[a], ray.o[a]);
+                    L.q[a] = to_fixed(p - ((double)(blo[a] - g.ghost) + 0.5));
+                    D[a] = to_fixed(step * ray.d[a]);
+                }
+            } else {
+                L.q[0] = L.q[1] = L.q[2] = 0;
+                D[0] = D[1] = D[2] = 0;
+            }
+            bool active = n > 0 && !stopped;
+            Corners C;
+            int pcx = INT_MIN, pcy = 0, pcz = 0;
+            while (__any_sync(FULL_MASK, active)) {
+                if (active) {
+                    const int cx = (int)(L.q[0] >> 32), cy = (int)(L.q[1] >> 32), cz = (int)(L.q[2] >> 32);
+                    if (!VR_REUSE || cx != pcx || cy != pcy || cz != pcz) {
+                        fetch8<LAY, 0, CLAMP, COUNT>(brick, g, ext, L, prm.bitmap, (long long)b * g.slot, C);
+                        pcx = cx, pcy = cy, pcz = cz;
+                    }
+                    const float v = lerp8(C, L);
+                    if (COUNT) ++nsamples;
+                    if (MODE == VR_MIP) {
+                        acc.r = fmaxf(acc.r, v);
+                        stopped = acc.r >= mip_stop;
+                    } else {
+                        shade_alpha(acc, v, prm.stepf, lut, prm.lut);
+                        stopped = !(acc.a < tau);
+                    }
+                    L.q[0] += D[0], L.q[1] += D[1], L.q[2] += D[2];
+                    --n;
+                    active = n > 0 && !stopped;
+                }
+            }
+            /* the (at most two) samples next to the exit point, one by one in FP64 (R5) */
+            if (live) {
+                for (int kk = max(k_lat, k); owned && kk < k_hi && !stopped; ++kk) {
+                    double s, w;
+                    if (!sample_sw(ray, step, kk, s, w)) continue;
+#pragma unroll
+                    for (int a = 0; a < 3; ++a) {
+                        const double p = VR_FMA(s, ray.d[a], ray.o[a]);
+                        L.q[a] = to_fixed(p - ((double)(blo[a] - g.ghost) + 0.5));
+                    }
+                    const float v = trilinear<LAY, 0, CLAMP, COUNT>(brick, g, ext, L, prm.bitmap, (long long)b * g.slot);
+                    if (COUNT) ++nsamples;
+                    if (MODE == VR_MIP) {
+                        acc.r = fmaxf(acc.r, v);
+                        stopped = acc.r >= mip_stop;
+                    } else {
+                        shade_alpha(acc, v, (float)w, lut, prm.lut);
+                        stopped = !(acc.a < tau);
+                    }
+                }
+                k = k_hi;
+            }
+        }
+
+        if (in_frame) {
+            float4 o;
+            if (MODE == VR_ALPHA) {
+                o = make_float4(acc.r, acc.g, acc.b, acc.a);
+            } else if (acc.r == -INFINITY) {
+                o = make_float4(0.0f, 0.0f, 0.0f, 0.0f); /* R11: the ray took no sample */
+            } else {
+                const float u = __saturatef((acc.r - prm.lut.vmin) * prm.lut.inv_range);
+                const float x = u * prm.lut.scale;
+                const int i = min((int)x, prm.lut.nm2);
+                const float f = x - (float)i;
+                const float4 e = s_lut[2 * i], d = s_lut[2 * i + 1];
+                o = make_float4(fmaf(f, d.x, e.x), fmaf(f, d.y, e.y), fmaf(f, d.z, e.z), 1.0f);
+            }
+            __stcs(frame + ((long long)pj * W + pi), o);
+        }
+        next = __shfl_sync(FULL_MASK, next, 0);
+    }
+    if (COUNT) {
+        for (int o = 16; o > 0; o >>= 1) nsamples += __shfl_xor_sync(FULL_MASK, nsamples, o);
+        if (lane == 0 && nsamples) atomicAdd(&prm.vs_rw->samples, nsamples);
+    }
+}
+
+template <int MODE, int LAY, bool CLAMP, bool COUNT>
+static cudaError_t launch_fused(const VrRaycastParams& p, float* frame, long long items, cudaStream_t st) {
+    static int sms = 0, cached_per_sm = 0;
+    static size_t cached_smem = (size_t)-1;
+    const size_t smem = 2 * sizeof(float4) * (size_t)p.lut.n;
+    if (smem != cached_smem) {
+        int dev = 0;
+        cudaError_t e = cudaGetDevice(&dev);
+        if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        if (e == cudaSuccess)
+            e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&cached_per_sm, vr_fused_kernel<MODE, LAY, CLAMP, COUNT>,
+                                                              VR_RAYCAST_THREADS, smem);
+        if (e != cudaSuccess) return e;
+        if (cached_per_sm < 1) return cudaErrorLaunchOutOfResources;
+        cached_smem = smem;
+    }
+    long long ctas = (long long)sms * cached_per_sm;
+    const long long want = (items + (VR_RAYCAST_THREADS / 32) - 1) / (VR_RAYCAST_THREADS / 32);
+    if (ctas > want) ctas = want < 1 ? 1 : want;
+    vr_fused_kernel<MODE, LAY, CLAMP, COUNT><<<(int)ctas, VR_RAYCAST_THREADS, smem, st>>>(p, reinterpret_cast<float4*>(frame));
+    return cudaGetLastError();
+}
+
+template <int MODE, bool COUNT>
+static cudaError_t launch_fused_mode(const VrRaycastParams& p, float* frame, long long items, cudaStream_t st) {
+    const bool clamp = p.grid.ghost == 0;
+    const VrGrid& g = p.grid;
+    const bool t442 = g.layout == VR_LAYOUT_TILED && g.tl[0] == 2 && g.tl[1] == 2 && g.tl[2] == 1 && g.ml[0] == 0 && g.ml[1] == 0 &&
+                      g.ml[2] == 0;
+    if (g.layout == VR_LAYOUT_LINEAR)
+        return clamp ? launch_fused<MODE, LAY_LINEAR, true, COUNT>(p, frame, items, st)
+                     : launch_fused<MODE, LAY_LINEAR, false, COUNT>(p, frame, items, st);
+    if (t442)
+        return clamp ? launch_fused<MODE, LAY_TILE442, true, COUNT>(p, frame, items, st)
+                     : launch_fused<MODE, LAY_TILE442, false, COUNT>(p, frame, items, st);
+    return clamp ? launch_fused<MODE, LAY_GENERIC, true, COUNT>(p, frame, items, st)
+                 : launch_fused<MODE, LAY_GENERIC, false, COUNT>(p, frame, items, st);
+}
+
+cudaError_t vr_launch_fused(const VrRaycastParams& p, float* frame, int W, int H, bool count, cudaStream_t st) {
+    const long long items = (long long)((W + VR_TILE_W - 1) / VR_TILE_W) * ((H + VR_TILE_H - 1) / VR_TILE_H);
+    if (p.mode == VR_ALPHA)
+        return count ? launch_fused_mode<VR_ALPHA, true>(p, frame, items, st) : launch_fused_mode<VR_ALPHA, false>(p, frame, items, st);
+    return count ? launch_fused_mode<VR_MIP, true>(p, frame, items, st) : launch_fused_mode<VR_MIP, false>(p, frame, items, st);
+}

@@ -143,6 +143,8 @@ cudaError_t vr_launch_setup(const VrGrid& grid, const VrMatrices& mats, int W, i
 cudaError_t vr_launch_minmax(const VrGrid& grid, const float* bricks, int2* enc, float2* table, cudaStream_t st);
 /* items = work items of the view (sizes the persistent grid) */
 cudaError_t vr_launch_raycast(const VrRaycastParams& p, long long items, bool count, cudaStream_t st);
+/* fused traversal (row f2): one ray per frame pixel through all bricks, writes the frame */
+cudaError_t vr_launch_fused(const VrRaycastParams& p, float* frame, int W, int H, bool count, cudaStream_t st);
 cudaError_t vr_launch_composite(const VrCompLayer* layers, const int* order, int n, int W, int H, int mode,
                                 const VrLut& lut, float* out, cudaStream_t st);
 cudaError_t vr_launch_upload(const VrGrid& grid, float* bricks, const float* src, int x0, int y0, int z0, int sx,

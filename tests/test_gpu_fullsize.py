@@ -55,6 +55,32 @@ def check_views(vr, wl, g, o, view_ids, npix, modes, tau):
                 check_mip(img, ref["image"], "%s view %d" % (wl["name"], vi))
 
 
+def check_fused(vr, wl, g, cube, tf, view_ids, npix, modes, tau):
+    """Row f2 at full size: VR_FUSED frames of the bricked volume against the oracle holding the
+    same cube in ONE brick (R17), on seeded pixels."""
+    W, H = wl["width"], wl["height"]
+    big = max(wl["nx"], wl["ny"], wl["nz"])
+    if wl["nx"] * wl["ny"] * wl["nz"] <= 512 ** 3:
+        one = oracle.Volume(wl["nx"], wl["ny"], wl["nz"], big, 1, data=cube.fill_host())
+    else:
+        one = oracle.Volume(wl["nx"], wl["ny"], wl["nz"], big, 1, voxel_fn=cube.voxel_fn())
+    one.set_transfer_function(tf, synth.TF_VMIN, synth.TF_VMAX)
+    one.set_early_termination(tau)
+    g.set_traversal(vr.FUSED)
+    for vi in view_ids:
+        view, proj = wl["views"][vi], wl["proj"]
+        pix = seeded_pixels(2000 + vi, W, H, npix)
+        for mode in modes:
+            img = gpu_frame(g, view, proj, W, H, wl["step"], mode)[pix[:, 1], pix[:, 0]]
+            ref = one.render(view, proj, W, H, wl["step"], mode, pixels=pix)
+            assert (ref["counts"][:, 0] > 0).mean() > 0.05
+            if mode == vr.ALPHA:
+                check_alpha(img, ref["image"], ref["flags"], tau, "fused %s view %d" % (wl["name"], vi))
+            else:
+                check_mip(img, ref["image"], "fused %s view %d" % (wl["name"], vi))
+    g.set_traversal(vr.SORT_LAST)
+
+
 def test_config1_512cube_8_bricks(vr):
     wl, g, o, cube = pair(vr, "c1", synth.tf_ramp())
     # the device generator and the host generator made the same cube
@@ -62,6 +88,7 @@ def test_config1_512cube_8_bricks(vr):
     g.download(back, origin=(0, 0, 255))
     assert np.array_equal(back, cube.fill_host(0, 0, 255, wl["nx"], wl["ny"], 3))
     check_views(vr, wl, g, o, (0, 7, 20), 3000, (vr.ALPHA,), 0.99)
+    check_fused(vr, wl, g, cube, synth.tf_ramp(), (3,), 2000, (vr.ALPHA, vr.MIP), 0.99)
     g.set_transfer_function(synth.tf_translucent(), synth.TF_VMIN, synth.TF_VMAX)
     o.set_transfer_function(synth.tf_translucent(), synth.TF_VMIN, synth.TF_VMAX)
     check_views(vr, wl, g, o, (13,), 2000, (vr.ALPHA, vr.MIP), 0.99)
@@ -70,6 +97,7 @@ def test_config1_512cube_8_bricks(vr):
 def test_config2_1024cube_64_bricks(vr):
     wl, g, o, cube = pair(vr, "c2", synth.tf_ramp())
     check_views(vr, wl, g, o, (0, 5, 17), 1500, (vr.ALPHA, vr.MIP), 0.99)
+    check_fused(vr, wl, g, cube, synth.tf_ramp(), (9,), 1000, (vr.ALPHA,), 0.99)
 
 
 def test_config3_103GB_cube_192_bricks(vr):
@@ -79,6 +107,7 @@ def test_config3_103GB_cube_192_bricks(vr):
         pytest.skip("needs ~110 GB of free device memory")
     wl, g, o, cube = pair(vr, "c3", synth.tf_ramp())
     check_views(vr, wl, g, o, (0, 11), 1500, (vr.ALPHA, vr.MIP), 0.99)
+    check_fused(vr, wl, g, cube, synth.tf_ramp(), (5,), 1000, (vr.ALPHA,), 0.99)
     g.set_transfer_function(synth.tf_translucent(), synth.TF_VMIN, synth.TF_VMAX)
     o.set_transfer_function(synth.tf_translucent(), synth.TF_VMIN, synth.TF_VMAX)
     check_views(vr, wl, g, o, (23,), 1000, (vr.ALPHA,), 0.99)

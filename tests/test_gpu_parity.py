@@ -261,6 +261,89 @@ def test_transparent_bricks_are_culled_exactly(vr):
     check_mip(m_on, o.render(view, proj, W, H, 0.5, oracle.MIP)["image"], "MIP with data-max stop")
 
 
+# --------------------------------------------------------------------------- f2 fused traversal (R17)
+@pytest.mark.parametrize("tau", [0.99, 2.0])
+@pytest.mark.parametrize("ortho", [False, True])
+def test_fused_traversal_equals_single_brick_oracle(vr, tau, ortho):
+    """VR_FUSED on a ragged grid of bricks == the oracle holding the volume in ONE brick (R17):
+    same sample schedule, global early termination. Also: the same frame on both layouts, and
+    within rounding of the sort-last frame when early termination is off."""
+    cube = synth.Cube(23, 70, 52, 44, 6)
+    data = cube.fill_host()
+    tf = synth.tf_ramp() if tau < 1 else synth.tf_translucent()
+    g, _ = make_pair(cube, 16, 1, tf=tf, tau=tau, data=data)          # 5 x 4 x 3 bricks, ragged
+    one = oracle.Volume(cube.nx, cube.ny, cube.nz, 128, 1, data=data)  # a single brick
+    one.set_transfer_function(tf, synth.TF_VMIN, synth.TF_VMAX)
+    one.set_early_termination(tau)
+    W, H = 176, 132
+    fr = synth.Framing(cube.nx, cube.ny, cube.nz, W, H)
+    view, proj = fr.seeded(5, 1), fr.proj(ortho)
+    g.set_traversal(vr.FUSED)
+    g.minmax()                                                         # the once-per-upload range pass (f1)
+    l0 = g.launch_count()
+    fa = gpu_frame(g, view, proj, W, H, 0.5, vr.ALPHA)
+    assert g.launch_count() - l0 == 2                                  # set-up + one fused kernel, no compositing
+    ref = one.render(view, proj, W, H, 0.5, oracle.ALPHA)
+    check_alpha(fa, ref["image"], ref["flags"], tau, "fused alpha")
+    fm = gpu_frame(g, view, proj, W, H, 0.5, vr.MIP)
+    check_mip(fm, one.render(view, proj, W, H, 0.5, oracle.MIP)["image"], "fused mip")
+    g.set_traversal(vr.SORT_LAST)
+    sm = gpu_frame(g, view, proj, W, H, 0.5, vr.MIP)
+    check_mip(fm, sm, "fused vs sort-last mip")
+    if tau > 1:
+        sa = gpu_frame(g, view, proj, W, H, 0.5, vr.ALPHA)
+        assert np.abs(sa - fa).max() < 2e-5
+    # sample count: global termination takes no more samples than brick-local termination
+    g.set_counting(1)
+    gpu_frame(g, view, proj, W, H, 0.5, vr.ALPHA)
+    n_sort = g.debug_stats()["samples"]
+    g.set_traversal(vr.FUSED)
+    gpu_frame(g, view, proj, W, H, 0.5, vr.ALPHA)
+    n_fused = g.debug_stats()["samples"]
+    assert n_fused == int(ref["counts"][..., 0].sum())                 # exactly the oracle's sample set
+    assert n_fused <= n_sort
+    g.set_counting(0)
+    lin = vr.Volume(cube.nx, cube.ny, cube.nz, 16, 1, layout=vr.LAYOUT_LINEAR)
+    lin.upload(data)
+    lin.set_transfer_function(tf, synth.TF_VMIN, synth.TF_VMAX)
+    lin.set_early_termination(tau)
+    lin.set_traversal(vr.FUSED)
+    assert np.array_equal(gpu_frame(lin, view, proj, W, H, 0.5, vr.ALPHA), fa)
+
+
+def test_fused_traversal_edge_cases(vr):
+    """Camera inside the volume, a volume behind the camera, tiny frames, axis-aligned orthographic
+    rays, a step longer than the volume, and one brick (fused == sort-last bit for bit)."""
+    cube = synth.Cube(29, 40, 36, 30, 3)
+    data = cube.fill_host()
+    g, _ = make_pair(cube, 16, 1, data=data)
+    one = oracle.Volume(40, 36, 30, 64, 1, data=data)
+    one.set_transfer_function(synth.tf_ramp(), synth.TF_VMIN, synth.TF_VMAX)
+    g.set_traversal(vr.FUSED)
+    W, H = 64, 48
+    fr = synth.Framing(40, 36, 30, W, H)
+
+    def both(view, proj, w, h, step, what):
+        ref = one.render(view, proj, w, h, step, oracle.ALPHA)
+        check_alpha(gpu_frame(g, view, proj, w, h, step, vr.ALPHA), ref["image"], ref["flags"], 0.99, what)
+        check_mip(gpu_frame(g, view, proj, w, h, step, vr.MIP), one.render(view, proj, w, h, step, oracle.MIP)["image"], what)
+
+    both(synth.look_at((20.3, 18.1, 14.2), (60, 40, 22), (0, 0, 1)), synth.perspective(70, W / H, 0.25, 200.0), W, H, 0.5, "inside")
+    behind = synth.look_at((20, 18, 300), (20, 18, 600), (0, 1, 0))
+    for mode in (vr.ALPHA, vr.MIP):
+        assert not gpu_frame(g, behind, synth.perspective(40, W / H, 1.0, 100.0), W, H, 0.5, mode).any()
+    for (w, h) in ((1, 1), (3, 2), (33, 5)):
+        f2 = synth.Framing(40, 36, 30, w, h)
+        both(f2.seeded(1, 0), f2.proj(False), w, h, 0.5, "%dx%d" % (w, h))
+    both(synth.look_at((20, 18, -10.0), (20, 18, 0.0), (0.0, 1.0, 0.0)), synth.orthographic(20, 18, 1.0, 60.0), 40, 36, 1.0, "axis-aligned")
+    for step in (200.0, 0.1):
+        both(fr.seeded(1, 1), fr.proj(True), W, H, step, "step %g" % step)
+    g1, _ = make_pair(cube, 64, 1, data=data)
+    a = gpu_frame(g1, fr.turntable(3), fr.proj(False), W, H, 0.5, vr.ALPHA)
+    g1.set_traversal(vr.FUSED)
+    assert np.array_equal(gpu_frame(g1, fr.turntable(3), fr.proj(False), W, H, 0.5, vr.ALPHA), a)
+
+
 # --------------------------------------------------------------------------- edge cases
 def test_edge_cases(vr):
     import torch
