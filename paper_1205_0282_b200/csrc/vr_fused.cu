@@ -37,8 +37,11 @@ vr_fused_kernel(const VrRaycastParams prm, float4* __restrict__ frame) {
     if (prm.vs->singular) return;
 
     const int W = prm.vs->W, H = prm.vs->H;
+    /* tiles are handed out block by block (4 x 8 tiles = 32 x 32 pixels, row-major inside a block) so that
+     * the warps in flight work on neighbouring rays - the same bricks and lines - instead of one frame row */
     const int tiles_x = (W + VR_TILE_W - 1) / VR_TILE_W, tiles_y = (H + VR_TILE_H - 1) / VR_TILE_H;
-    const unsigned total = (unsigned)(tiles_x * tiles_y);
+    const int blocks_x = (tiles_x + 3) >> 2, blocks_y = (tiles_y + 7) >> 3;
+    const unsigned total = (unsigned)(blocks_x * blocks_y) << 5;
     const double step = prm.step;
     const float tau = prm.tau;
     LutView lut;
@@ -54,9 +57,10 @@ vr_fused_kernel(const VrRaycastParams prm, float4* __restrict__ frame) {
     while (next < total) {
         const int item = (int)next;
         if (lane == 0) next = atomicAdd(&prm.vs_rw->work_counter, 1u);
-        const int ty = item / tiles_x, tx = item - ty * tiles_x;
+        const int blk = item >> 5, by = blk / blocks_x, bx = blk - by * blocks_x;
+        const int tx = (bx << 2) + (item & 3), ty = (by << 3) + ((item >> 2) & 7);
         const int pi = tx * VR_TILE_W + (lane & 7), pj = ty * VR_TILE_H + (lane >> 3);
-        const bool in_frame = pi < W && pj < H;
+        const bool in_frame = pi < W && pj < H; /* also false for the tiles a ragged block has beyond the frame */
 
         RaySetup ray;
         ray.K = 0;
@@ -91,6 +95,7 @@ vr_fused_kernel(const VrRaycastParams prm, float4* __restrict__ frame) {
             }
             const int b = (bc[2] * g.g[1] + bc[1]) * g.g[0] + bc[0];
             const float* __restrict__ brick = prm.bricks + (long long)b * g.slot;
+            asm volatile("" : "+l"(brick)); /* keep the base in registers: do not rebuild it per load */
 
             const int k_lat = min(k_hi, max(k, ray.K - 2));
             int n = owned ? k_lat - k : 0;
@@ -221,7 +226,8 @@ static cudaError_t launch_fused_mode(const VrRaycastParams& p, float* frame, lon
 }
 
 cudaError_t vr_launch_fused(const VrRaycastParams& p, float* frame, int W, int H, bool count, cudaStream_t st) {
-    const long long items = (long long)((W + VR_TILE_W - 1) / VR_TILE_W) * ((H + VR_TILE_H - 1) / VR_TILE_H);
+    const long long tiles_x = (W + VR_TILE_W - 1) / VR_TILE_W, tiles_y = (H + VR_TILE_H - 1) / VR_TILE_H;
+    const long long items = ((tiles_x + 3) / 4) * ((tiles_y + 7) / 8) * 32;
     if (p.mode == VR_ALPHA)
         return count ? launch_fused_mode<VR_ALPHA, true>(p, frame, items, st) : launch_fused_mode<VR_ALPHA, false>(p, frame, items, st);
     return count ? launch_fused_mode<VR_MIP, true>(p, frame, items, st) : launch_fused_mode<VR_MIP, false>(p, frame, items, st);
