@@ -411,7 +411,7 @@ def config_of(wl, args):
                         "step %.1f, tf %s, early termination %.2f" % (
                             wl["name"], wl["nx"], wl["ny"], wl["nz"], wl["nsrc"], " + spectral ramp" if wl["ramp"] else "",
                             wl["brick"], wl["ghost"], wl["width"], wl["height"], wl["view_kind"], args.mode.upper(), wl["step"],
-                            args.tf, wl["tau"]),
+                            args.tf, wl["tau"]) + (", fused traversal" if getattr(args, "traversal", "sort_last") == "fused" else ""),
             "baseline_config_index": int(wl["name"][1:]),
             "cube_gb": round(wl["nx"] * wl["ny"] * wl["nz"] * 4 / 1e9, 2),
             "l2_policy": "inputs larger than L2 (every frame streams a new view's share of the cube); no explicit flush",
@@ -512,6 +512,8 @@ def main():
     ap.add_argument("--workload", default="c3", choices=["c0", "c1", "c2", "c3", "c4"])
     ap.add_argument("--mode", default="alpha", choices=["alpha", "mip"])
     ap.add_argument("--tf", default="ramp", choices=["ramp", "translucent"])
+    ap.add_argument("--traversal", default="sort_last", choices=["sort_last", "fused"],
+                    help="main arm: per-brick sub-images + compositing (the headline path) or the fused traversal (row f2)")
     ap.add_argument("--cells-every", type=int, default=6, help="count distinct cells on every n-th view of the cycle (0 = never)")
     ap.add_argument("--c4-part", default="both", choices=["both", "composite"],
                     help="--workload c4: `composite` runs only the compositing microbenchmark (profiling)")
@@ -585,7 +587,9 @@ def main():
                     samples=samples, counts=counts)
 
     peak, peak_src = measured_peak()
+    g.set_traversal(vr.FUSED if args.traversal == "fused" else vr.SORT_LAST)
     m = measure(mode_id, True, ClockSampler(local_rank) if rank == 0 else None)
+    g.set_traversal(vr.SORT_LAST)
     fps, ms_max = aggregate(m["ms"], K, world, reduce_max)
     e2e_fps, e2e_ms_max = aggregate(m["e2e_ms"], K, world, reduce_max)
     e2e_sync_fps, _ = aggregate(m["e2e_sync_ms"], K, world, reduce_max)
@@ -607,7 +611,7 @@ def main():
             "stage_ms": {"setup": round(float(m["stages"][:, 0].mean()), 4), "raycast": round(float(m["stages"][:, 1].mean()), 4),
                          "composite": round(float(m["stages"][:, 2].mean()), 4)},
             "roofline": roofline_of(m["counts"], m["stages"], m["stage_views"], peak, peak_src,
-                                    traffic_of(args.workload, args.mode, args.tf)),
+                                    traffic_of(args.workload, args.mode, args.tf + ("" if args.traversal == "sort_last" else "/fused"))),
             "build_s": round(t_build, 1), "upload": dict(g.upload_stats, frac_of_hbm_peak=round(g.upload_stats["gb_per_s"] / peak, 4)),
             "minmax": dict(g.minmax_stats, frac_of_hbm_peak=round(g.minmax_stats["gb_per_s"] / peak, 4))}
     # which roofline bounds the ray-cast kernel: DRAM for the sparsely sampled 103 GB cube (0.03 samples per
@@ -645,7 +649,7 @@ def main():
                                           "raycast": round(float(v["stages"][:, 1].mean()), 4),
                                           "composite": round(float(v["stages"][:, 2].mean()), 4)},
                              "roofline": roofline_of(v["counts"], v["stages"], v["stage_views"], peak, peak_src,
-                                                     traffic_of(args.workload, vmode, vtf) if vtrav == "sort_last" else None)})
+                                                     traffic_of(args.workload, vmode, vtf + ("" if vtrav == "sort_last" else "/fused")))})
         g.set_transfer_function(tf, synth.TF_VMIN, synth.TF_VMAX)
         line["variants"] = variants
 
