@@ -23,6 +23,9 @@
  *   - the LUT is staged in shared memory as (entry, delta) pairs;
  *   - early ray termination and loop exit are warp votes.
  */
+#include <stdlib.h>
+#include <string.h>
+
 #include "vr_march.cuh"
 
 template <int MODE, int LAY, int PT, bool CLAMP, bool COUNT>
@@ -212,6 +215,10 @@ static cudaError_t launch_variant(const VrRaycastParams& p, long long items, cud
                                                               VR_RAYCAST_THREADS, smem);
         if (e != cudaSuccess) return e;
         if (cached_per_sm < 1) return cudaErrorLaunchOutOfResources;
+        if (const char* e = getenv("VR_CTAS_PER_SM")) { /* experiment knob: fewer resident CTAs */
+            const int cap = atoi(e + (MODE == VR_MIP && strchr(e, ',') ? (strchr(e, ',') - e + 1) : 0));
+            if (cap >= 1 && cap < cached_per_sm) cached_per_sm = cap;
+        }
         cached_smem = smem;
     }
     long long ctas = (long long)sms * cached_per_sm;
