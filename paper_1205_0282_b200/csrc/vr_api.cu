@@ -565,7 +565,9 @@ extern "C" int vr_render(vr_volume* v, const float* view, const float* proj, int
         v->launches++;
         if (timing) VR_CUDA(v, cudaEventRecord(ev[2], st));
     } else {
-        VR_CUDA(v, vr_launch_raycast(p, items, v->counting != 0, st));
+        /* brick faces of brick^2 voxels project onto sub_px pixels in all: > 4 voxels per pixel = sparse */
+        const bool sparse = (double)v->grid.nbricks * v->grid.brick * v->grid.brick > 4.0 * (double)sub_px;
+        VR_CUDA(v, vr_launch_raycast(p, items, v->counting != 0, sparse, st));
         v->launches++;
         if (timing) VR_CUDA(v, cudaEventRecord(ev[2], st));
         VR_CUDA(v, vr_launch_composite(v->d_layers, v->d_order, v->grid.nbricks, width, height, mode, v->lut, out_rgba, st));

@@ -141,8 +141,9 @@ cudaError_t vr_launch_setup(const VrGrid& grid, const VrMatrices& mats, int W, i
                             long long sub_capacity_px, void* sub_base, VrViewState* vs, VrBrickView* bv, int* order,
                             int* item_prefix, VrCompLayer* layers, const float2* range, const VrLut& lut, cudaStream_t st);
 cudaError_t vr_launch_minmax(const VrGrid& grid, const float* bricks, int2* enc, float2* table, cudaStream_t st);
-/* items = work items of the view (sizes the persistent grid) */
-cudaError_t vr_launch_raycast(const VrRaycastParams& p, long long items, bool count, cudaStream_t st);
+/* items = work items of the view (sizes the persistent grid); sparse = the view samples the store at
+ * more than two voxels per pixel (launch heuristic only) */
+cudaError_t vr_launch_raycast(const VrRaycastParams& p, long long items, bool count, bool sparse, cudaStream_t st);
 /* fused traversal (row f2): one ray per frame pixel through all bricks, writes the frame */
 cudaError_t vr_launch_fused(const VrRaycastParams& p, float* frame, int W, int H, bool count, cudaStream_t st);
 cudaError_t vr_launch_composite(const VrCompLayer* layers, const int* order, int n, int W, int H, int mode,

@@ -10,8 +10,8 @@
  *
  * One streaming pass over the store after an upload (not per frame): grid (x, brick), every
  * thread reads 16-byte words in memory order (4x4x2 layout: one x-row of a micro-tile, the
- * cells beyond the brick's extent masked out), warp min/max by shuffles, one pair of atomics
- * per warp on an order-preserving integer encoding of the floats. A second one-CTA kernel
+ * cells beyond the brick's extent masked out), min/max by warp shuffles and shared memory, one
+ * pair of atomics per CTA on an order-preserving integer encoding of the floats. A second one-CTA kernel
  * decodes the table and reduces it to the range of the whole volume.
  */
 #include <math.h>
@@ -72,9 +72,16 @@ vr_brick_minmax_kernel(VrGrid g, const float* __restrict__ bricks, int2* __restr
         mn = fminf(mn, __shfl_xor_sync(0xffffffffu, mn, o));
         mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, o));
     }
-    if ((threadIdx.x & 31) == 0 && mn <= mx) {
-        atomicMin(&enc[b].x, mm_encode(mn));
-        atomicMax(&enc[b].y, mm_encode(mx));
+    /* one pair of atomics per CTA: same-address atomics serialise in L2 (~2 ns each) */
+    __shared__ float s_mn[8], s_mx[8];
+    if ((threadIdx.x & 31) == 0) s_mn[threadIdx.x >> 5] = mn, s_mx[threadIdx.x >> 5] = mx;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int w = 1; w < (int)(blockDim.x >> 5); ++w) mn = fminf(mn, s_mn[w]), mx = fmaxf(mx, s_mx[w]);
+        if (mn <= mx) {
+            atomicMin(&enc[b].x, mm_encode(mn));
+            atomicMax(&enc[b].y, mm_encode(mx));
+        }
     }
 }
 
@@ -106,8 +113,8 @@ cudaError_t vr_launch_minmax(const VrGrid& grid, const float* bricks, int2* enc,
     const bool t442 = grid.layout == VR_LAYOUT_TILED && grid.tl[0] == 2 && grid.tl[1] == 2 && grid.tl[2] == 1 &&
                       grid.ml[0] == 0 && grid.ml[1] == 0 && grid.ml[2] == 0;
     /* enough CTAs per brick to fill the machine several times over, few enough to keep the atomics rare */
-    long long per_brick = t442 ? (grid.slot / 4 + 256 * 16 - 1) / (256 * 16) : ((long long)grid.P * grid.P + 7) / 8;
-    if (per_brick > 2048) per_brick = 2048;
+    long long per_brick = t442 ? (grid.slot / 4 + 256 * 32 - 1) / (256 * 32) : ((long long)grid.P * grid.P + 7) / 8;
+    if (per_brick > 1024) per_brick = 1024;
     if (per_brick < 1) per_brick = 1;
     const dim3 gr((unsigned)per_brick, grid.nbricks);
     if (t442) vr_brick_minmax_kernel<true><<<gr, 256, 0, st>>>(grid, bricks, enc);

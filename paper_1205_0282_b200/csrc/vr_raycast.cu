@@ -23,9 +23,6 @@
  *   - the LUT is staged in shared memory as (entry, delta) pairs;
  *   - early ray termination and loop exit are warp votes.
  */
-#include <stdlib.h>
-#include <string.h>
-
 #include "vr_march.cuh"
 
 template <int MODE, int LAY, int PT, bool CLAMP, bool COUNT>
@@ -202,7 +199,7 @@ vr_raycast_kernel(const VrRaycastParams prm) {
 /* Persistent grid: resident CTAs per SM (for this instance and its shared memory) x SMs,
  * but no more CTAs than there are groups of 8 work items. */
 template <int MODE, int LAY, int PT, bool CLAMP, bool COUNT>
-static cudaError_t launch_variant(const VrRaycastParams& p, long long items, cudaStream_t st) {
+static cudaError_t launch_variant(const VrRaycastParams& p, long long items, bool sparse, cudaStream_t st) {
     static int sms = 0, cached_per_sm = 0;
     static size_t cached_smem = (size_t)-1;
     const size_t smem = MODE == VR_ALPHA ? 2 * sizeof(float4) * (size_t)p.lut.n : 0;
@@ -215,13 +212,13 @@ static cudaError_t launch_variant(const VrRaycastParams& p, long long items, cud
                                                               VR_RAYCAST_THREADS, smem);
         if (e != cudaSuccess) return e;
         if (cached_per_sm < 1) return cudaErrorLaunchOutOfResources;
-        if (const char* e = getenv("VR_CTAS_PER_SM")) { /* experiment knob: fewer resident CTAs */
-            const int cap = atoi(e + (MODE == VR_MIP && strchr(e, ',') ? (strchr(e, ',') - e + 1) : 0));
-            if (cap >= 1 && cap < cached_per_sm) cached_per_sm = cap;
-        }
         cached_smem = smem;
     }
-    long long ctas = (long long)sms * cached_per_sm;
+    /* Sparse MIP frames (several voxels per pixel: every load is a DRAM line of its own) run faster with two
+     * resident CTAs per SM than with three - the lighter MIP loop keeps more lines in flight than L1/L2 hold
+     * (c3: 14.5 -> 12.3 ms); dense frames and ALPHA want all three. */
+    const int per_sm = (MODE == VR_MIP && sparse && cached_per_sm > 2) ? 2 : cached_per_sm;
+    long long ctas = (long long)sms * per_sm;
     const long long want = (items + (VR_RAYCAST_THREADS / 32) - 1) / (VR_RAYCAST_THREADS / 32);
     if (ctas > want) ctas = want < 1 ? 1 : want;
     vr_raycast_kernel<MODE, LAY, PT, CLAMP, COUNT><<<(int)ctas, VR_RAYCAST_THREADS, smem, st>>>(p);
@@ -234,24 +231,24 @@ static bool is_tile442(const VrGrid& g) {
 }
 
 template <int MODE, bool COUNT>
-static cudaError_t launch_mode(const VrRaycastParams& p, long long ctas, cudaStream_t st) {
+static cudaError_t launch_mode(const VrRaycastParams& p, long long ctas, bool sparse, cudaStream_t st) {
     const bool clamp = p.grid.ghost == 0;
     if (p.grid.layout == VR_LAYOUT_LINEAR) {
-        if (clamp) return launch_variant<MODE, LAY_LINEAR, 0, true, COUNT>(p, ctas, st);
+        if (clamp) return launch_variant<MODE, LAY_LINEAR, 0, true, COUNT>(p, ctas, sparse, st);
         switch (p.grid.P) {
-            case 258: return launch_variant<MODE, LAY_LINEAR, 258, false, COUNT>(p, ctas, st);
-            case 514: return launch_variant<MODE, LAY_LINEAR, 514, false, COUNT>(p, ctas, st);
-            default: return launch_variant<MODE, LAY_LINEAR, 0, false, COUNT>(p, ctas, st);
+            case 258: return launch_variant<MODE, LAY_LINEAR, 258, false, COUNT>(p, ctas, sparse, st);
+            case 514: return launch_variant<MODE, LAY_LINEAR, 514, false, COUNT>(p, ctas, sparse, st);
+            default: return launch_variant<MODE, LAY_LINEAR, 0, false, COUNT>(p, ctas, sparse, st);
         }
     }
     if (is_tile442(p.grid))
-        return clamp ? launch_variant<MODE, LAY_TILE442, 0, true, COUNT>(p, ctas, st)
-                     : launch_variant<MODE, LAY_TILE442, 0, false, COUNT>(p, ctas, st);
-    return clamp ? launch_variant<MODE, LAY_GENERIC, 0, true, COUNT>(p, ctas, st)
-                 : launch_variant<MODE, LAY_GENERIC, 0, false, COUNT>(p, ctas, st);
+        return clamp ? launch_variant<MODE, LAY_TILE442, 0, true, COUNT>(p, ctas, sparse, st)
+                     : launch_variant<MODE, LAY_TILE442, 0, false, COUNT>(p, ctas, sparse, st);
+    return clamp ? launch_variant<MODE, LAY_GENERIC, 0, true, COUNT>(p, ctas, sparse, st)
+                 : launch_variant<MODE, LAY_GENERIC, 0, false, COUNT>(p, ctas, sparse, st);
 }
 
-cudaError_t vr_launch_raycast(const VrRaycastParams& p, long long ctas, bool count, cudaStream_t st) {
-    if (p.mode == VR_ALPHA) return count ? launch_mode<VR_ALPHA, true>(p, ctas, st) : launch_mode<VR_ALPHA, false>(p, ctas, st);
-    return count ? launch_mode<VR_MIP, true>(p, ctas, st) : launch_mode<VR_MIP, false>(p, ctas, st);
+cudaError_t vr_launch_raycast(const VrRaycastParams& p, long long ctas, bool count, bool sparse, cudaStream_t st) {
+    if (p.mode == VR_ALPHA) return count ? launch_mode<VR_ALPHA, true>(p, ctas, sparse, st) : launch_mode<VR_ALPHA, false>(p, ctas, sparse, st);
+    return count ? launch_mode<VR_MIP, true>(p, ctas, sparse, st) : launch_mode<VR_MIP, false>(p, ctas, sparse, st);
 }
