@@ -373,7 +373,7 @@ extern "C" int vr_set_transfer_function(vr_volume* v, const float* rgba, int n, 
         if (!isfinite(rgba[i])) return fail(v, VR_ERR_INVALID_ARG, "vr_set_transfer_function: entry %d is not finite", i / 4);
     /* the table is stored as (entry, difference to the next entry) pairs; the differences are
      * plain float32 subtractions of the caller's entries */
-    static float4 base[VR_MAX_LUT], delta[VR_MAX_LUT];
+    float4 base[VR_MAX_LUT], delta[VR_MAX_LUT]; /* 32 KB of stack: no state shared between handles or threads */
     for (int i = 0; i < n; ++i) {
         base[i] = make_float4(rgba[4 * i], rgba[4 * i + 1], rgba[4 * i + 2], rgba[4 * i + 3]);
         if (i + 1 < n)
@@ -667,9 +667,19 @@ extern "C" int vr_composite(const float* const* layers, const int* rects, const 
     if (n < 0 || n > 4096) return fail(NULL, VR_ERR_INVALID_ARG, "vr_composite: n = %d outside [0,4096]", n);
     if (width <= 0 || height <= 0 || width > 32768 || height > 32768)
         return fail(NULL, VR_ERR_INVALID_ARG, "vr_composite: bad frame size %dx%d", width, height);
-    static VrCompLayer tab[4096];
-    static unsigned char seen[4096];
-    memset(seen, 0, sizeof(seen));
+    VrCompLayer* tab = new (std::nothrow) VrCompLayer[n > 0 ? n : 1];
+    unsigned char* seen = new (std::nothrow) unsigned char[n > 0 ? n : 1];
+    if (!tab || !seen) {
+        delete[] tab;
+        delete[] seen;
+        return fail(NULL, VR_ERR_OUT_OF_MEMORY, "vr_composite: host allocation failed");
+    }
+    struct Free { /* released on every return path */
+        VrCompLayer* t;
+        unsigned char* s;
+        ~Free() { delete[] t; delete[] s; }
+    } free_tables = {tab, seen};
+    memset(seen, 0, (size_t)(n > 0 ? n : 1));
     for (int l = 0; l < n; ++l) {
         const int* r = rects + 4 * l;
         if (r[0] < 0 || r[1] < 0 || r[2] > width || r[3] > height || r[2] < r[0] || r[3] < r[1])
