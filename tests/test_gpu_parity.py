@@ -180,6 +180,48 @@ def test_pipelined_host_frames_equal_synchronous_ones(vr):
     check_mip(bufs[0].numpy().astype(np.float64), ref["image"], "pipelined frame 0")
 
 
+# --------------------------------------------------------------------------- other bricks, ghosts, layouts
+@pytest.mark.parametrize("brick,ghost,tile", [(20, 1, None), (7, 2, None), (24, 1, "3,1,1,0,0,0"), (20, 2, "1,2,2,1,1,1"),
+                                               (12, 1, "linear")])
+def test_odd_bricks_ghosts_and_generic_layouts(vr, monkeypatch, brick, ghost, tile):
+    """Bricks that are not powers of two (the owner rule divides instead of scaling), wider ghost
+    layers, x-linear rows and the generic separable micro-tile layouts (8x2x2 tiles; 2x4x4 tiles
+    in 2x2x2 macro blocks) all render the same frames: parity with the oracle in both modes and
+    both traversals, brick store and data range bit-exact."""
+    cube = synth.Cube(57, 61, 47, 39, 5)
+    data = cube.fill_host()
+    layout = vr.LAYOUT_DEFAULT
+    if tile == "linear":
+        layout = vr.LAYOUT_LINEAR
+    elif tile:
+        monkeypatch.setenv("VR_TILE", tile)
+    g = vr.Volume(61, 47, 39, brick, ghost, layout=layout)
+    monkeypatch.delenv("VR_TILE", raising=False)
+    g.upload(data)
+    o = oracle.Volume(61, 47, 39, brick, ghost, data=data)
+    one = oracle.Volume(61, 47, 39, 64, 1, data=data)
+    for v in (g, o, one):
+        v.set_transfer_function(synth.tf_ramp(), synth.TF_VMIN, synth.TF_VMAX)
+        v.set_early_termination(0.99)
+    back = np.empty_like(data)
+    g.download(back)
+    assert np.array_equal(back, data)
+    for b in (0, g.nbricks // 2, g.nbricks - 1):
+        assert np.array_equal(g.debug_brick_data(b), o.brick_data(b))
+        assert tuple(g.debug_brick_minmax()[b]) == o.brick_minmax(b)
+    W, H = 120, 90
+    fr = synth.Framing(61, 47, 39, W, H)
+    view, proj = fr.seeded(4, 2), fr.proj(False)
+    assert np.array_equal(g.debug_brick_order(view, proj), o.brick_order(view, proj))
+    ref = o.render(view, proj, W, H, 0.5, oracle.ALPHA)
+    check_alpha(gpu_frame(g, view, proj, W, H, 0.5, vr.ALPHA), ref["image"], ref["flags"], 0.99, "sort-last")
+    check_mip(gpu_frame(g, view, proj, W, H, 0.5, vr.MIP), o.render(view, proj, W, H, 0.5, oracle.MIP)["image"], "sort-last")
+    g.set_traversal(vr.FUSED)
+    ref = one.render(view, proj, W, H, 0.5, oracle.ALPHA)
+    check_alpha(gpu_frame(g, view, proj, W, H, 0.5, vr.ALPHA), ref["image"], ref["flags"], 0.99, "fused")
+    check_mip(gpu_frame(g, view, proj, W, H, 0.5, vr.MIP), one.render(view, proj, W, H, 0.5, oracle.MIP)["image"], "fused")
+
+
 # --------------------------------------------------------------------------- f1 data range, culling
 @pytest.mark.parametrize("layout", ["tiled", "linear"])
 @pytest.mark.parametrize("ghost", [0, 1, 2])
