@@ -610,6 +610,12 @@ def main():
             "clocks": m["clocks"],
             "stage_ms": {"setup": round(float(m["stages"][:, 0].mean()), 4), "raycast": round(float(m["stages"][:, 1].mean()), 4),
                          "composite": round(float(m["stages"][:, 2].mean()), 4)},
+            # the paper's estimator: frame time per rotation angle, then its 75th percentile
+            # over the angles; here one device-timed frame per view of the cycle (stage events summed)
+            "frame_ms": {"p50": round(float(np.percentile(m["stages"].sum(axis=1), 50)), 4),
+                         "p75": round(float(np.percentile(m["stages"].sum(axis=1), 75)), 4),
+                         "min": round(float(m["stages"].sum(axis=1).min()), 4),
+                         "max": round(float(m["stages"].sum(axis=1).max()), 4), "views": int(len(m["stages"]))},
             "roofline": roofline_of(m["counts"], m["stages"], m["stage_views"], peak, peak_src,
                                     traffic_of(args.workload, args.mode, args.tf + ("" if args.traversal == "sort_last" else "/fused"))),
             "build_s": round(t_build, 1), "upload": dict(g.upload_stats, frac_of_hbm_peak=round(g.upload_stats["gb_per_s"] / peak, 4)),
