@@ -19,7 +19,8 @@
  *   - final colour mapping with the user's colour map
  * The paper gives no formulas; every constant and convention is a documented reading
  * R1..R15 (restated in DESIGN.md "Readings"), plus R16 (row f1: per-brick
- * data range, and the transparent-brick rule built on it).
+ * data range, and the transparent-brick rule built on it) and R18 (the paper's
+ * per-ray step, selected with step == 0).
  *
  * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference leg
  * may load this. It shares no code with paper_1205_0282_b200/ (the CUDA path); only the
@@ -505,6 +506,15 @@ static void render_pixel(vro_volume* v, const vro_view* vw, const int* order, in
     }
     if (mg < 1e-9) fl |= VRO_FLAG_GRAZING;
     if (hit) {
+        /* R18 (row f2 (i)): step == 0 asks for the paper's per-ray step, "a discrete ray-casting with
+         * at least one sample for each voxel intersected" (after Kaufman): one sample per
+         * unit advance along the ray's major axis, step = 1 / max_a |d_a| (d is a unit vector). */
+        if (step == 0.0) {
+            double m = fabs(d[0]);
+            if (fabs(d[1]) > m) m = fabs(d[1]);
+            if (fabs(d[2]) > m) m = fabs(d[2]);
+            step = 1.0 / m;
+        }
         /* step 3: sample schedule anchored at the global entry (R5) */
         int64_t K = (int64_t)ceil((t1 - t0) / step);
         double min_owner_margin = INFINITY;
@@ -591,7 +601,7 @@ static void render_pixel(vro_volume* v, const vro_view* vw, const int* order, in
  * counts[2*p] = samples taken, counts[2*p+1] = samples scheduled (before ERT). */
 int vro_render(vro_volume* v, const float* view, const float* proj, int W, int H, double step, int mode,
                const int* pixels, int64_t npix, double* out, uint8_t* flags, int64_t* counts, double* sub, int nthreads) {
-    if (!v || !view || !proj || W <= 0 || H <= 0 || !(step > 0.0) || !out) return 1;
+    if (!v || !view || !proj || W <= 0 || H <= 0 || !(step >= 0.0) || !out) return 1;
     if (mode != VRO_ALPHA && mode != VRO_MIP) return 1;
     if (!v->tf) return 3;
     if (!v->bricks && !v->fn) return 3;

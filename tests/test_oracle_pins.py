@@ -618,3 +618,50 @@ def test_transparent_bricks_render_exactly_nothing():
     sub = r["sub"].reshape(H * W, vol.nbricks, 4)
     assert np.all(sub[:, transparent, :] == 0.0)
     assert np.abs(sub[:, [b for b in range(vol.nbricks) if b not in transparent], 3]).max() > 0.1
+
+
+# --------------------------------------------------------------------------- per-ray step (row f2 (i), R18)
+def test_auto_step_is_one_sample_per_major_axis_voxel():
+    """PAPER.md:152 "at least one sample for each voxel intersected": step = 0 selects
+    1 / max|d_a| per ray. Closed forms: the number of scheduled samples is ceil(chord * max|d_a|)
+    = the number of unit slabs crossed along the major axis; an axis-aligned view is the
+    step-1 render; the homogeneous cube keeps its exact opacity (the weights sum to the chord)."""
+    n = 24
+    data = small_noise(n, n, n, seed=11)
+    vol = oracle.Volume(n, n, n, 8, 1, data=data)
+    vol.set_transfer_function(synth.tf_translucent(), -3, 10)
+    vol.set_early_termination(2.0)
+    W, H = 40, 30
+    fr = synth.Framing(n, n, n, W, H)
+    for ortho in (False, True):
+        view, proj = fr.seeded(3, 1), fr.proj(ortho)
+        r = vol.render(view, proj, W, H, 0.0, oracle.ALPHA)
+        sched = r["counts"][..., 1]
+        checked = 0
+        for (i, j) in ((W // 2, H // 2), (W // 3, H // 2), (W // 2, H // 3), (2 * W // 3, 2 * H // 3), (5, 5)):
+            o, d, tfar = ray_np(view, proj, W, H, i, j)
+            c = chord_np(o, d, tfar, [n, n, n])
+            if c is not None:
+                t0, t1 = c
+                expect = math.ceil((t1 - t0) * np.abs(d).max() - 1e-9)
+                assert abs(int(sched[j, i]) - expect) <= 1 and sched[j, i] >= expect - 1e-9, (i, j, sched[j, i], expect)
+                checked += 1
+            else:
+                assert sched[j, i] == 0
+        assert checked >= 3
+    view, proj = ortho_along_z(n, n, n)
+    a = vol.render(view, proj, n, n, 0.0, oracle.ALPHA)["image"]
+    b = vol.render(view, proj, n, n, 1.0, oracle.ALPHA)["image"]
+    assert np.array_equal(a, b)
+    # homogeneous cube: opacity 1 - (1 - a)^L whatever the step, so also with the per-ray step
+    hom = oracle.Volume(n, n, n, 8, 1, data=np.full((n, n, n), 2.0, dtype=np.float32))
+    hom.set_transfer_function(const_tf((0.2, 0.5, 0.9), 0.05), -3, 10)
+    hom.set_early_termination(2.0)
+    view, proj = fr.seeded(3, 2), fr.proj(False)
+    img = hom.render(view, proj, W, H, 0.0, oracle.ALPHA)["image"]
+    for (i, j) in ((W // 2, H // 2), (W // 3, H // 2), (W // 2, 2 * H // 3)):
+        o, d, tfar = ray_np(view, proj, W, H, i, j)
+        c = chord_np(o, d, tfar, [n, n, n])
+        L = (c[1] - c[0]) if c is not None else 0.0
+        a32 = float(np.float32(0.05))                # the table holds float32 opacities
+        assert L > 5 and abs(img[j, i, 3] - (1.0 - (1.0 - a32) ** L)) < 1e-12
