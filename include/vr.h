@@ -49,6 +49,7 @@ typedef enum vr_status {
 } vr_status;
 
 enum { VR_ALPHA = 0, VR_MIP = 1 };   /* vr_render mode */
+#define VR_STEP_AUTO 0.0f            /* vr_render step: the paper's per-ray step (R18) */
 enum { VR_HOST = 0, VR_DEVICE = 1 }; /* memory space of a data pointer */
 /* Layout of a ghost-padded brick in HBM (north_star: "a tiled linear layout ... whichever ncu
  * shows is faster"). LINEAR: rows of P = brick + 2*ghost cells, x fastest. TILED: 4x4x2-cell
@@ -177,7 +178,11 @@ int vr_set_culling(vr_volume* v, int enable);
  * brick sub-images in visibility order (sec. 2.3.3: `over` is associative;
  * MIP composites in any order) and, for MIP, the final colour mapping (:172).
  *   view, proj (host): float[16] each, read before the call returns.
- *   width,height > 0; step > 0 (voxels); mode VR_ALPHA or VR_MIP.
+ *   width,height > 0; mode VR_ALPHA or VR_MIP.
+ *   step > 0: sample spacing along every ray, in voxels (R5). step == VR_STEP_AUTO (0): the
+ *   paper's own rule, "a discrete ray-casting with at least one sample for each voxel
+ *   intersected": per ray, one sample per unit advance along the ray's major
+ *   axis, step = 1 / max(|d_x|,|d_y|,|d_z|) for the unit direction d (R18; 1 .. sqrt(3) voxels).
  *   out_rgba (device): [height][width][4] float32. VR_ALPHA: premultiplied colour and opacity
  *   on a transparent black background. VR_MIP: LUT colour of the ray's maximum with alpha 1,
  *   or (0,0,0,0) if the ray took no sample (R11).

@@ -15,6 +15,7 @@ import numpy as np
 
 ALPHA, MIP = 0, 1
 SORT_LAST, FUSED = 0, 1
+STEP_AUTO = 0.0  # vr_render step: the paper's per-ray step (R18)
 HOST, DEVICE = 0, 1
 LAYOUT_DEFAULT, LAYOUT_LINEAR, LAYOUT_TILED = 0, 1, 2
 

@@ -522,7 +522,7 @@ extern "C" int vr_render(vr_volume* v, const float* view, const float* proj, int
     int rc = check_view(v, "vr_render", view, proj, width, height, &sub_px, &items);
     if (rc) return rc;
     if (!out_rgba) return fail(v, VR_ERR_INVALID_ARG, "vr_render: NULL output");
-    if (!(step > 0.0f) || !isfinite(step)) return fail(v, VR_ERR_INVALID_ARG, "vr_render: step must be > 0");
+    if (!(step >= 0.0f) || !isfinite(step)) return fail(v, VR_ERR_INVALID_ARG, "vr_render: step must be > 0, or VR_STEP_AUTO (0)");
     if (mode != VR_ALPHA && mode != VR_MIP) return fail(v, VR_ERR_INVALID_ARG, "vr_render: bad mode %d", mode);
     if (!v->has_tf) return fail(v, VR_ERR_STATE, "vr_render: no transfer function set");
     if (!v->has_data) return fail(v, VR_ERR_STATE, "vr_render: nothing uploaded");
@@ -557,7 +557,6 @@ extern "C" int vr_render(vr_volume* v, const float* view, const float* proj, int
     }
     p.lut = v->lut;
     p.step = (double)step;
-    p.stepf = step;
     p.tau = v->tau;
     p.mode = mode;
     if (v->traversal == VR_FUSED) {

@@ -64,7 +64,9 @@ vr_fused_kernel(const VrRaycastParams prm, float4* __restrict__ frame) {
 
         RaySetup ray;
         ray.K = 0;
+        ray.step = step;
         if (in_frame) ray_setup(s_minv, W, H, pi, pj, g, step, ray);
+        const float stepf = (float)ray.step; /* path length a lattice sample stands for */
 
         Accum acc;
         acc.r = (MODE == VR_MIP) ? -INFINITY : 0.0f;
@@ -80,7 +82,7 @@ vr_fused_kernel(const VrRaycastParams prm, float4* __restrict__ frame) {
             bool owned = false;
             if (live) {
                 double s, w;
-                owned = sample_sw(ray, step, k, s, w); /* an empty interval is dropped (R5) */
+                owned = sample_sw(ray, k, s, w); /* an empty interval is dropped (R5) */
                 if (owned) {
 #pragma unroll
                     for (int a = 0; a < 3; ++a) bc[a] = owner_axis(ray, g, s, a); /* R6: the brick that owns sample k */
@@ -90,7 +92,7 @@ vr_fused_kernel(const VrRaycastParams prm, float4* __restrict__ frame) {
 #pragma unroll
             for (int a = 0; a < 3; ++a) ext[a] = bhi[a] - blo[a] + 2 * g.ghost;
             if (owned) {
-                brick_range(ray, g, step, bc, blo, bhi, k_lo, k_hi);
+                brick_range(ray, g, bc, blo, bhi, k_lo, k_hi);
                 if (k_hi <= k) k_hi = k + 1; /* cannot happen (sample k is owned by bc); guarantees progress */
             }
             const int b = (bc[2] * g.g[1] + bc[1]) * g.g[0] + bc[0];
@@ -103,12 +105,12 @@ vr_fused_kernel(const VrRaycastParams prm, float4* __restrict__ frame) {
             long long D[3];
             if (n > 0) {
                 double s, w;
-                sample_sw(ray, step, k, s, w);
+                sample_sw(ray, k, s, w);
 #pragma unroll
                 for (int a = 0; a < 3; ++a) {
                     const double p = VR_FMA(s, ray.d[a], ray.o[a]);
                     L.q[a] = to_fixed(p - ((double)(blo[a] - g.ghost) + 0.5));
-                    D[a] = to_fixed(step * ray.d[a]);
+                    D[a] = to_fixed(ray.step * ray.d[a]);
                 }
             } else {
                 L.q[0] = L.q[1] = L.q[2] = 0;
@@ -130,7 +132,7 @@ vr_fused_kernel(const VrRaycastParams prm, float4* __restrict__ frame) {
                         acc.r = fmaxf(acc.r, v);
                         stopped = acc.r >= mip_stop;
                     } else {
-                        shade_alpha(acc, v, prm.stepf, lut, prm.lut);
+                        shade_alpha(acc, v, stepf, lut, prm.lut);
                         stopped = !(acc.a < tau);
                     }
                     L.q[0] += D[0], L.q[1] += D[1], L.q[2] += D[2];
@@ -142,7 +144,7 @@ vr_fused_kernel(const VrRaycastParams prm, float4* __restrict__ frame) {
             if (live) {
                 for (int kk = max(k_lat, k); owned && kk < k_hi && !stopped; ++kk) {
                     double s, w;
-                    if (!sample_sw(ray, step, kk, s, w)) continue;
+                    if (!sample_sw(ray, kk, s, w)) continue;
 #pragma unroll
                     for (int a = 0; a < 3; ++a) {
                         const double p = VR_FMA(s, ray.d[a], ray.o[a]);

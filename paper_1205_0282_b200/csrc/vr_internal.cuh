@@ -120,8 +120,7 @@ struct VrRaycastParams {
     void* sub;          /* float4[] (ALPHA) or float[] (MIP) */
     unsigned* bitmap;   /* counting variant only: one bit per brick-store cell, or NULL */
     VrLut lut;
-    double step;
-    float stepf; /* (float)step */
+    double step; /* > 0: sample spacing in voxels; 0: per ray, 1 / max|d_a| (R18) */
     float tau;
     int mode;
 };

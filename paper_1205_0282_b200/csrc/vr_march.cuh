@@ -26,11 +26,14 @@
 struct RaySetup {
     double o[3], d[3];
     double t0, t1;
+    double step; /* sample spacing along this ray (R5); per ray when the caller asks for the paper's rule (R18) */
     int K; /* number of scheduled samples; 0 = miss */
 };
 
 /* R1, R2: pixel (i,j), centres at half-integers, row 0 at the bottom; ray from the near plane
- * (clip z = -1) to the far plane (+1). R4: slab test against the closed global box. */
+ * (clip z = -1) to the far plane (+1). R4: slab test against the closed global box.
+ * step > 0: the caller's spacing; step == 0: R18, the paper's "at least one sample for each voxel
+ * intersected", one sample per unit advance along the major axis, 1 / max|d_a|. */
 __device__ __forceinline__ void ray_setup(const double* __restrict__ Minv, int W, int H, int i, int j, const VrGrid& g,
                                           double step, RaySetup& r) {
     const double x = VR_SUB(VR_DIV(VR_MUL(2.0, VR_ADD((double)i, 0.5)), (double)W), 1.0);
@@ -56,6 +59,13 @@ __device__ __forceinline__ void ray_setup(const double* __restrict__ Minv, int W
 #pragma unroll
     for (int a = 0; a < 3; ++a) r.d[a] = VR_DIV(r.d[a], len);
     const double tfar = len;
+    if (step == 0.0) {
+        double m = fabs(r.d[0]);
+        if (fabs(r.d[1]) > m) m = fabs(r.d[1]);
+        if (fabs(r.d[2]) > m) m = fabs(r.d[2]);
+        step = VR_DIV(1.0, m);
+    }
+    r.step = step;
 
     double tin = -INFINITY, tout = INFINITY;
     bool hit = true;
@@ -93,7 +103,8 @@ __device__ __forceinline__ void ray_setup(const double* __restrict__ Minv, int W
 
 /* R5: sample k stands for the interval [t0 + k step, min(t0 + (k+1) step, t1)]: s = its
  * midpoint, w = its length; intervals of non-positive length are dropped. */
-__device__ __forceinline__ bool sample_sw(const RaySetup& r, double step, int k, double& s, double& w) {
+__device__ __forceinline__ bool sample_sw(const RaySetup& r, int k, double& s, double& w) {
+    const double step = r.step;
     const double a0 = VR_ADD(r.t0, VR_MUL((double)k, step));
     double a1 = VR_ADD(r.t0, VR_MUL((double)(k + 1), step));
     if (a1 > r.t1) a1 = r.t1;
@@ -115,10 +126,10 @@ __device__ __forceinline__ int owner_axis(const RaySetup& r, const VrGrid& g, do
  *   entered(k): every axis has reached the brick's slab      (false ... false true ... true)
  *   left(k):    some axis has gone past the brick's slab     (false ... false true ... true)
  * Sample k belongs to the brick iff entered(k) && !left(k). */
-__device__ __forceinline__ void owner_flags(const RaySetup& r, const VrGrid& g, double step, const int bc[3], int k,
+__device__ __forceinline__ void owner_flags(const RaySetup& r, const VrGrid& g, const int bc[3], int k,
                                             bool& entered, bool& left) {
     double s, w;
-    sample_sw(r, step, k, s, w);
+    sample_sw(r, k, s, w);
     entered = true;
     left = false;
 #pragma unroll
@@ -137,19 +148,19 @@ __device__ __forceinline__ void owner_flags(const RaySetup& r, const VrGrid& g, 
 }
 
 template <bool WANT_LEFT>
-__device__ __forceinline__ bool owner_pred(const RaySetup& r, const VrGrid& g, double step, const int bc[3], int k) {
+__device__ __forceinline__ bool owner_pred(const RaySetup& r, const VrGrid& g, const int bc[3], int k) {
     bool e, l;
-    owner_flags(r, g, step, bc, k, e, l);
+    owner_flags(r, g, bc, k, e, l);
     return WANT_LEFT ? l : e;
 }
 
 /* Smallest k in [0,K] with pred(k) (pred(K) taken as true); `est` is a guess. */
 template <bool WANT_LEFT>
-__device__ __forceinline__ int first_true(const RaySetup& r, const VrGrid& g, double step, const int bc[3], int est) {
+__device__ __forceinline__ int first_true(const RaySetup& r, const VrGrid& g, const int bc[3], int est) {
     const int K = r.K;
     est = est < 0 ? 0 : (est > K ? K : est);
-    const bool at = (est == K) || owner_pred<WANT_LEFT>(r, g, step, bc, est);
-    const bool before = (est > 0) && owner_pred<WANT_LEFT>(r, g, step, bc, est - 1);
+    const bool at = (est == K) || owner_pred<WANT_LEFT>(r, g, bc, est);
+    const bool before = (est > 0) && owner_pred<WANT_LEFT>(r, g, bc, est - 1);
     if (at && !before) return est;
     int lo, hi; /* invariant: pred(lo-1) false (or lo == 0), pred(hi) true */
     if (at) {
@@ -161,14 +172,14 @@ __device__ __forceinline__ int first_true(const RaySetup& r, const VrGrid& g, do
     }
     while (lo < hi) {
         const int mid = lo + ((hi - lo) >> 1);
-        if (owner_pred<WANT_LEFT>(r, g, step, bc, mid)) hi = mid;
+        if (owner_pred<WANT_LEFT>(r, g, bc, mid)) hi = mid;
         else lo = mid + 1;
     }
     return lo;
 }
 
 /* The integer sample range [k_lo, k_hi) of the ray that brick bc owns (R6). */
-__device__ __forceinline__ void brick_range(const RaySetup& r, const VrGrid& g, double step, const int bc[3],
+__device__ __forceinline__ void brick_range(const RaySetup& r, const VrGrid& g, const int bc[3],
                                             const int lo[3], const int hi[3], int& k_lo, int& k_hi) {
     k_lo = 0;
     k_hi = 0;
@@ -198,17 +209,17 @@ __device__ __forceinline__ void brick_range(const RaySetup& r, const VrGrid& g, 
         }
     }
     if (miss || tout < tin - 1e-6 * (1.0 + fabs(tin))) return;
-    const double inv_step = 1.0 / step;
+    const double inv_step = 1.0 / r.step;
     const double e_lo = ceil((tin - r.t0) * inv_step - 0.5);
     const double e_hi = ceil((tout - r.t0) * inv_step - 0.5);
     const int est_lo = e_lo < 0.0 ? 0 : (e_lo > (double)r.K ? r.K : (int)e_lo);
     const int est_hi = e_hi < 0.0 ? 0 : (e_hi > (double)r.K ? r.K : (int)e_hi);
-    k_lo = first_true<false>(r, g, step, bc, est_lo);
+    k_lo = first_true<false>(r, g, bc, est_lo);
     if (k_lo >= r.K) {
         k_hi = k_lo;
         return;
     }
-    k_hi = first_true<true>(r, g, step, bc, est_hi);
+    k_hi = first_true<true>(r, g, bc, est_hi);
     if (k_hi < k_lo) k_hi = k_lo;
 }
 

@@ -95,10 +95,11 @@ vr_raycast_kernel(const VrRaycastParams prm) {
 
         RaySetup ray;
         ray.K = 0;
+        ray.step = step;
         int k_lo = 0, k_hi = 0;
         if (in_rect) {
             ray_setup(s_minv, W, H, pi, pj, g, step, ray);
-            brick_range(ray, g, step, bc, blo, bhi, k_lo, k_hi);
+            brick_range(ray, g, bc, blo, bhi, k_lo, k_hi);
         }
         /* lattice samples: k in [k_lo, k_lat); samples k >= K-2 (whose interval may be clipped
          * by the exit point) are evaluated one by one in FP64 below */
@@ -110,14 +111,15 @@ vr_raycast_kernel(const VrRaycastParams prm) {
         acc.g = acc.b = acc.a = 0.0f;
         Lattice L;
         long long D[3];
+        const float stepf = (float)ray.step; /* path length a lattice sample stands for */
         if (n > 0) {
             double s, w;
-            sample_sw(ray, step, k_lo, s, w);
+            sample_sw(ray, k_lo, s, w);
 #pragma unroll
             for (int a = 0; a < 3; ++a) {
                 const double p = VR_FMA(s, ray.d[a], ray.o[a]);
                 L.q[a] = to_fixed(p - ((double)(blo[a] - g.ghost) + 0.5));
-                D[a] = to_fixed(step * ray.d[a]);
+                D[a] = to_fixed(ray.step * ray.d[a]);
             }
         } else {
             L.q[0] = L.q[1] = L.q[2] = 0;
@@ -143,7 +145,7 @@ vr_raycast_kernel(const VrRaycastParams prm) {
                     acc.r = fmaxf(acc.r, v);
                     stopped = acc.r >= mip_stop;
                 } else {
-                    shade_alpha(acc, v, prm.stepf, lut, prm.lut);
+                    shade_alpha(acc, v, stepf, lut, prm.lut);
                     stopped = !(acc.a < tau);
                 }
                 L.q[0] += D[0], L.q[1] += D[1], L.q[2] += D[2];
@@ -163,7 +165,7 @@ vr_raycast_kernel(const VrRaycastParams prm) {
 #endif
             for (int k = k_tail; k < k_hi && !stopped; ++k) {
                 double s, w;
-                if (!sample_sw(ray, step, k, s, w)) continue;
+                if (!sample_sw(ray, k, s, w)) continue;
 #pragma unroll
                 for (int a = 0; a < 3; ++a) {
                     const double p = VR_FMA(s, ray.d[a], ray.o[a]);

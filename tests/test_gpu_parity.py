@@ -180,6 +180,33 @@ def test_pipelined_host_frames_equal_synchronous_ones(vr):
     check_mip(bufs[0].numpy().astype(np.float64), ref["image"], "pipelined frame 0")
 
 
+# --------------------------------------------------------------------------- f2 (i) per-ray step (R18)
+@pytest.mark.parametrize("ortho", [False, True])
+def test_auto_step_matches_oracle(vr, ortho):
+    """step = VR_STEP_AUTO: 1 / max|d_a| per ray, sort-last and fused, ALPHA and MIP,
+    with the exact sample count of the oracle."""
+    cube = synth.Cube(61, 66, 50, 41, 5)
+    data = cube.fill_host()
+    g, o = make_pair(cube, 16, 1, data=data)
+    one = oracle.Volume(cube.nx, cube.ny, cube.nz, 128, 1, data=data)
+    one.set_transfer_function(synth.tf_ramp(), synth.TF_VMIN, synth.TF_VMAX)
+    W, H = 150, 110
+    fr = synth.Framing(cube.nx, cube.ny, cube.nz, W, H)
+    view, proj = fr.seeded(6, 0), fr.proj(ortho)
+    g.set_counting(1)
+    for trav, orc in ((vr.SORT_LAST, o), (vr.FUSED, one)):
+        g.set_traversal(trav)
+        ref = orc.render(view, proj, W, H, 0.0, oracle.ALPHA)
+        check_alpha(gpu_frame(g, view, proj, W, H, vr.STEP_AUTO, vr.ALPHA), ref["image"], ref["flags"], 0.99, "auto step")
+        assert g.debug_stats()["samples"] == int(ref["counts"][..., 0].sum())
+        check_mip(gpu_frame(g, view, proj, W, H, vr.STEP_AUTO, vr.MIP), orc.render(view, proj, W, H, 0.0, oracle.MIP)["image"], "auto step")
+    # axis-aligned orthographic view: the per-ray step is exactly 1
+    g.set_traversal(vr.SORT_LAST)
+    view = synth.look_at((33, 25, -10.0), (33, 25, 0.0), (0.0, 1.0, 0.0))
+    proj = synth.orthographic(33, 25, 1.0, 70.0)
+    assert np.array_equal(gpu_frame(g, view, proj, 66, 50, vr.STEP_AUTO, vr.ALPHA), gpu_frame(g, view, proj, 66, 50, 1.0, vr.ALPHA))
+
+
 # --------------------------------------------------------------------------- other bricks, ghosts, layouts
 @pytest.mark.parametrize("brick,ghost,tile", [(20, 1, None), (7, 2, None), (24, 1, "3,1,1,0,0,0"), (20, 2, "1,2,2,1,1,1"),
                                                (12, 1, "linear")])
@@ -449,7 +476,10 @@ def test_errors(vr):
     assert e.value.status == 4  # nothing uploaded
     g.upload(np.zeros((16, 16, 16), dtype=np.float32))
     with pytest.raises(vr.VrError) as e:
-        g.render(I, I, 8, 8, 0.0, vr.ALPHA, out)
+        g.render(I, I, 8, 8, -0.5, vr.ALPHA, out)   # 0 is VR_STEP_AUTO; negative and NaN steps are errors
+    assert e.value.status == 1
+    with pytest.raises(vr.VrError) as e:
+        g.render(I, I, 8, 8, float("nan"), vr.ALPHA, out)
     assert e.value.status == 1
     with pytest.raises(vr.VrError) as e:
         g.render(I, np.zeros(16, dtype=np.float32), 8, 8, 0.5, vr.ALPHA, out)
