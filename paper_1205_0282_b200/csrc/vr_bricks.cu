@@ -37,8 +37,8 @@ __device__ __forceinline__ void padded_range(int lo, int ghost, int ext, int n, 
 
 __global__ void __launch_bounds__(256)
 vr_upload_kernel(VrGrid g, float* __restrict__ bricks, const float* __restrict__ src, int x0, int y0, int z0, int sx, int sy,
-                 int sz) {
-    const int b = blockIdx.y;
+                 int sz, int b0) {
+    const int b = blockIdx.y + b0; /* b0: first brick of the z range the box can touch */
     int bc[3], lo[3], hi[3];
     vr_brick_coords(g, b, bc);
     vr_brick_core(g, bc, lo, hi);
@@ -74,9 +74,9 @@ vr_upload_kernel(VrGrid g, float* __restrict__ bricks, const float* __restrict__
 
 __global__ void __launch_bounds__(256)
 vr_upload_tiled_kernel(VrGrid g, float* __restrict__ bricks, const float* __restrict__ src, int x0, int y0, int z0, int sx,
-                       int sy, int sz, int pitch) {
+                       int sy, int sz, int pitch, int b0) {
     extern __shared__ float s_rows[];
-    const int b = blockIdx.y;
+    const int b = blockIdx.y + b0; /* b0: first brick of the z range the box can touch */
     int bc[3], lo[3], hi[3];
     vr_brick_coords(g, b, bc);
     vr_brick_core(g, bc, lo, hi);
@@ -143,19 +143,24 @@ vr_upload_tiled_kernel(VrGrid g, float* __restrict__ bricks, const float* __rest
 /* TILED, the default 4x4x2 micro-tiles in x-fastest tile order: the same two phases with the
  * index arithmetic hoisted out of the element loops. Groups of TR = 2^TRL tile rows = 8 TR
  * source rows (TRL = 2 for small bricks, 1 when 32 rows of a large brick would take too much
- * shared memory for 6 CTAs per SM). Phase 1: warp w stages rows w, w+8, ... with 8 independent
- * 128-byte reads in flight; phase 2: 8/TR warps per tile row, a lane writes one 16-byte row
+ * shared memory for 6 CTAs per SM). Phase 1: warp w stages rows w, w+8, ... with cp.async (global ->
+ * shared, no register stage: all of a group's 128-byte reads are in flight together); phase 2: 8/TR warps per tile row, a lane writes one 16-byte row
  * of a micro-tile (LDS.128 -> STG.128), so a warp instruction writes four whole 128-byte lines. */
+__device__ __forceinline__ void cp_async4(float* smem_dst, const float* gmem_src) {
+    const unsigned sa = (unsigned)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(sa), "l"(gmem_src) : "memory");
+}
+
 template <int TRL>
 __global__ void __launch_bounds__(256)
 vr_upload_tile442_kernel(VrGrid g, float* __restrict__ bricks, const float* __restrict__ src, int x0, int y0, int z0, int sx,
-                         int sy, int sz, int pitch) {
+                         int sy, int sz, int pitch, int b0) {
     constexpr int TR = 1 << TRL;  /* tile rows per group */
     constexpr int RW = TR;        /* staged rows per warp (8 TR rows, 8 warps) */
     constexpr int CH = 8 / RW;    /* 32-cell chunks per row and iteration */
     constexpr int WPT = 8 >> TRL; /* phase 2: warps per tile row */
     extern __shared__ __align__(16) float s_rows[];
-    const int b = blockIdx.y;
+    const int b = blockIdx.y + b0; /* b0: first brick of the z range the box can touch */
     int bc[3], lo[3], hi[3];
     vr_brick_coords(g, b, bc);
     vr_brick_core(g, bc, lo, hi);
@@ -190,25 +195,21 @@ vr_upload_tile442_kernel(VrGrid g, float* __restrict__ bricks, const float* __re
                 srow[u] = src + ((long long)(gz - z0) * sy + (gy - y0)) * sx + (xbase - x0);
             }
         }
+        /* global -> shared without a register stage (cp.async, 4 bytes per lane): every request of the
+         * group is in flight at once, whatever the compiler's scheduling; one wait before the barrier */
         for (int i = i0 + lane; i < i1; i += 32 * CH) {
-            int ic[CH], gc[CH];
 #pragma unroll
             for (int c = 0; c < CH; ++c) {
-                ic[c] = min(i + 32 * c, i1 - 1); /* clamped into the row: its last cell may be staged twice */
-                gc[c] = clamp_x ? min(max(xbase + ic[c], 0), g.n[0] - 1) - xbase : ic[c];
-            }
-            float v[RW][CH];
+                const int ic = i + 32 * c;
+                if (ic < i1) {
+                    const int gc = clamp_x ? min(max(xbase + ic, 0), g.n[0] - 1) - xbase : ic;
 #pragma unroll
-            for (int u = 0; u < RW; ++u)
-#pragma unroll
-                for (int c = 0; c < CH; ++c) v[u][c] = srow[u] ? __ldcs(srow[u] + gc[c]) : 0.0f;
-#pragma unroll
-            for (int u = 0; u < RW; ++u) {
-                float* d = s_rows + (warp + 8 * u) * pitch - ibase;
-#pragma unroll
-                for (int c = 0; c < CH; ++c) d[ic[c]] = v[u][c];
+                    for (int u = 0; u < RW; ++u)
+                        if (srow[u]) cp_async4(s_rows + (warp + 8 * u) * pitch + (ic - ibase), srow[u] + gc);
+                }
             }
         }
+        asm volatile("cp.async.commit_group;\n\tcp.async.wait_group 0;" ::: "memory");
         __syncthreads();
         {
             const int j = ((tyg + tr) << 2) + (r & 3), k = kt + (r >> 2);
@@ -253,13 +254,19 @@ vr_download_kernel(VrGrid g, const float* __restrict__ bricks, float* __restrict
 
 cudaError_t vr_launch_upload(const VrGrid& grid, float* bricks, const float* src, int x0, int y0, int z0, int sx, int sy,
                              int sz, cudaStream_t st) {
-    /* nbricks <= 65535 (checked at create): bricks along grid.y */
+    /* nbricks <= 65535 (checked at create): bricks along grid.y - only those brick z-slabs whose padded
+     * extent can hold a plane of the box (a z-slab upload of a tall cube touches one or two of them) */
+    const int bz0 = (z0 - grid.ghost) > 0 ? (z0 - grid.ghost) / grid.brick : 0;
+    int bz1 = (z0 + sz - 1 + grid.ghost) / grid.brick;
+    if (bz1 > grid.g[2] - 1) bz1 = grid.g[2] - 1;
+    const int b0 = bz0 * grid.g[0] * grid.g[1];
+    const unsigned nby = (unsigned)((bz1 - bz0 + 1) * grid.g[0] * grid.g[1]);
     if (grid.layout == VR_LAYOUT_LINEAR) {
         /* enough CTAs per brick to cover its rows once at 8 rows per CTA, capped */
         long long rows = (long long)grid.P * grid.P;
         int bx = (int)((rows + 7) / 8);
         if (bx > 4096) bx = 4096;
-        vr_upload_kernel<<<dim3(bx, grid.nbricks), 256, 0, st>>>(grid, bricks, src, x0, y0, z0, sx, sy, sz);
+        vr_upload_kernel<<<dim3(bx, nby), 256, 0, st>>>(grid, bricks, src, x0, y0, z0, sx, sy, sz, b0);
     } else {
         /* one CTA per group of tile rows the box can touch in one brick, capped */
         const int rbits = grid.tl[1] + grid.tl[2];
@@ -286,14 +293,13 @@ cudaError_t vr_launch_upload(const VrGrid& grid, float* bricks, const float* src
             long long bx2 = ty2 * tz;
             if (bx2 > 16384) bx2 = 16384;
             if (big)
-                vr_upload_tile442_kernel<1><<<dim3((unsigned)bx2, grid.nbricks), 256, sm2, st>>>(grid, bricks, src, x0, y0, z0, sx,
-                                                                                                 sy, sz, pitch);
+                vr_upload_tile442_kernel<1><<<dim3((unsigned)bx2, nby), 256, sm2, st>>>(grid, bricks, src, x0, y0, z0, sx, sy, sz, pitch,
+                                                                                        b0);
             else
-                vr_upload_tile442_kernel<2><<<dim3((unsigned)bx2, grid.nbricks), 256, sm2, st>>>(grid, bricks, src, x0, y0, z0, sx,
-                                                                                                 sy, sz, pitch);
+                vr_upload_tile442_kernel<2><<<dim3((unsigned)bx2, nby), 256, sm2, st>>>(grid, bricks, src, x0, y0, z0, sx, sy, sz, pitch,
+                                                                                        b0);
         } else {
-            vr_upload_tiled_kernel<<<dim3((unsigned)bx, grid.nbricks), 256, smem, st>>>(grid, bricks, src, x0, y0, z0, sx, sy,
-                                                                                        sz, pitch);
+            vr_upload_tiled_kernel<<<dim3((unsigned)bx, nby), 256, smem, st>>>(grid, bricks, src, x0, y0, z0, sx, sy, sz, pitch, b0);
         }
     }
     return cudaGetLastError();
