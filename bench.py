@@ -44,7 +44,8 @@ def workload(name):
     """Shapes, cameras and classification of BASELINE.json's configs."""
     c = dict(synth.CONFIGS[name])
     c["name"] = name
-    c["seed"] = synth.BASE_SEED + int(name[1:])
+    c["seed"] = synth.BASE_SEED + int(name[1:]) + (10 if name[0] == "n" else 0)
+    c.setdefault("kind", 0)
     fr = synth.Framing(c["nx"], c["ny"], c["nz"], c["width"], c["height"])
     if name == "c2":  # "1920x1080 perspective output, 36 seeded views"
         c["views"] = [fr.seeded(c["seed"], k) for k in range(36)]
@@ -134,7 +135,7 @@ def build_volume(vr, wl, tf):
     toy.upload(torch.zeros((36, 40, 48), dtype=torch.float32, device="cuda"))
     toy.minmax()
     toy.close()
-    cube = synth.Cube(wl["seed"], wl["nx"], wl["ny"], wl["nz"], wl["nsrc"], wl["ramp"])
+    cube = synth.Cube(wl["seed"], wl["nx"], wl["ny"], wl["nz"], wl["nsrc"], wl["ramp"], wl.get("kind", 0))
     g = vr.Volume(wl["nx"], wl["ny"], wl["nz"], wl["brick"], wl["ghost"])
     plane = wl["nx"] * wl["ny"] * 4
     nzs = max(1, min(wl["nz"], (4 << 30) // plane))  # 4 GiB slabs: 64 planes of config 3
@@ -152,7 +153,7 @@ def build_volume(vr, wl, tf):
     torch.cuda.synchronize()
     del buf
     torch.cuda.empty_cache()
-    g.set_transfer_function(tf, synth.TF_VMIN, synth.TF_VMAX)
+    g.set_transfer_function(tf, *tf_range(wl))
     g.set_early_termination(wl["tau"])
     # row a1 (once per cube): every source voxel read once, every padded brick cell written once
     pad = 1
@@ -173,6 +174,20 @@ def build_volume(vr, wl, tf):
     g.minmax_stats = {"kernel": "vr_brick_minmax_kernel", "ms": round(mm_ms, 3), "bytes": 4 * pad,
                       "gb_per_s": round(4 * pad / (mm_ms * 1e-3) / 1e9, 1), "data_min": float(lo), "data_max": float(hi)}
     return g, cube
+
+
+def tf_range(wl):
+    """Data range the transfer function spans: [-3, 10] sigma for the spectral cubes, [0, 20] for density cubes."""
+    return (0.0, synth.NBODY_VMAX) if wl.get("kind", 0) == synth.NBODY else (synth.TF_VMIN, synth.TF_VMAX)
+
+
+def pick_tf(wl, name):
+    if wl.get("kind", 0) == synth.NBODY:  # zero-opacity toe: empty space is exactly transparent (R16)
+        t = synth.tf_density()
+        if name == "translucent":
+            t[:, 3] /= 64.0
+        return t
+    return synth.tf_ramp() if name == "ramp" else synth.tf_translucent()
 
 
 def count_pass(g, vr, wl, mode, view_ids, out, cells_every):
@@ -327,7 +342,7 @@ def oracle_volume(wl, tf):
     """The CPU oracle as it stands (oracle/, test infrastructure) on the same seeded cube:
     dense on the host when the cube is small, procedural voxels otherwise (no 103 GB host copy)."""
     import oracle
-    cube = synth.Cube(wl["seed"], wl["nx"], wl["ny"], wl["nz"], wl["nsrc"], wl["ramp"])
+    cube = synth.Cube(wl["seed"], wl["nx"], wl["ny"], wl["nz"], wl["nsrc"], wl["ramp"], wl.get("kind", 0))
     nvox = wl["nx"] * wl["ny"] * wl["nz"]
     if nvox <= 512 ** 3:
         o = oracle.Volume(wl["nx"], wl["ny"], wl["nz"], wl["brick"], wl["ghost"], data=cube.fill_host())
@@ -335,7 +350,7 @@ def oracle_volume(wl, tf):
     else:
         o = oracle.Volume(wl["nx"], wl["ny"], wl["nz"], wl["brick"], wl["ghost"], voxel_fn=cube.voxel_fn())
         how = "procedural voxels"
-    o.set_transfer_function(tf, synth.TF_VMIN, synth.TF_VMAX)
+    o.set_transfer_function(tf, *tf_range(wl))
     o.set_early_termination(wl["tau"])
     o._cube = cube
     return o, how
@@ -407,12 +422,14 @@ def run_reference(args, wl, tf, mode_id):
 
 
 def config_of(wl, args):
-    return {"workload": "%s: %dx%dx%d float32 cube (noise + %d Gaussian sources%s), %d^3 bricks + %d ghost, %dx%d, %s, %s, "
-                        "step %.1f, tf %s, early termination %.2f" % (
-                            wl["name"], wl["nx"], wl["ny"], wl["nz"], wl["nsrc"], " + spectral ramp" if wl["ramp"] else "",
-                            wl["brick"], wl["ghost"], wl["width"], wl["height"], wl["view_kind"], args.mode.upper(), wl["step"],
-                            args.tf, wl["tau"]) + (", fused traversal" if getattr(args, "traversal", "sort_last") == "fused" else ""),
-            "baseline_config_index": int(wl["name"][1:]),
+    what = "density cube: zero + %d extended halos" % wl["nsrc"] if wl.get("kind", 0) else \
+        "noise + %d Gaussian sources%s" % (wl["nsrc"], " + spectral ramp" if wl["ramp"] else "")
+    return {"workload": "%s: %dx%dx%d float32 cube (%s), %d^3 bricks + %d ghost, %dx%d, %s, %s, step %.1f, tf %s, "
+                        "early termination %.2f%s" % (
+                            wl["name"], wl["nx"], wl["ny"], wl["nz"], what, wl["brick"], wl["ghost"], wl["width"], wl["height"],
+                            wl["view_kind"], args.mode.upper(), wl["step"], args.tf, wl["tau"],
+                            ", fused traversal" if getattr(args, "traversal", "sort_last") == "fused" else ""),
+            "baseline_config_index": int(wl["name"][1:]) if wl["name"][0] == "c" else None,
             "cube_gb": round(wl["nx"] * wl["ny"] * wl["nz"] * 4 / 1e9, 2),
             "l2_policy": "inputs larger than L2 (every frame streams a new view's share of the cube); no explicit flush",
             "frames": "one frame per step, cycling the 36 views"}
@@ -509,7 +526,7 @@ def main():
     ap.add_argument("--steps", type=int, default=36)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="c3", choices=["c0", "c1", "c2", "c3", "c4"])
+    ap.add_argument("--workload", default="c3", choices=["c0", "c1", "c2", "c3", "c4", "n1"])
     ap.add_argument("--mode", default="alpha", choices=["alpha", "mip"])
     ap.add_argument("--tf", default="ramp", choices=["ramp", "translucent"])
     ap.add_argument("--traversal", default="sort_last", choices=["sort_last", "fused"],
@@ -526,7 +543,7 @@ def main():
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     wl = workload(args.workload if args.workload != "c4" else "c2")
-    tf = synth.tf_ramp() if args.tf == "ramp" else synth.tf_translucent()
+    tf = pick_tf(wl, args.tf)
     mode_id = 0 if args.mode == "alpha" else 1
 
     if args.impl == "reference":
@@ -629,6 +646,15 @@ def main():
         line["roofline_alu"] = alu
     else:
         line["roofline_hbm"], line["roofline"] = line["roofline"], alu
+    # row f1: bricks the transfer function makes transparent are skipped (exactly); report what that buys
+    culled = [s["bricks_culled"] for s in m["counts"].values()]
+    if max(culled) > 0 and args.traversal == "sort_last" and world == 1:
+        g.set_culling(False)
+        ms_off, _, st_off, _ = timed_device(g, wl, mode_id, order, K, Wm, out, dist)
+        g.set_culling(True)
+        line["culling"] = {"bricks": g.nbricks, "bricks_culled_mean": round(float(np.mean(culled)), 1),
+                           "frames_per_s_culling_off": round(K / (ms_off * 1e-3), 3),
+                           "raycast_ms_culling_off": round(float(st_off[:, 1].mean()), 4)}
     cs = [s for s in m["counts"].values() if s["cells_touched"] >= 0]
     if cs:
         line["touched_per_frame"] = {"cells_gb": round(np.mean([4.0 * s["cells_touched"] for s in cs]) / 1e9, 3),
@@ -644,7 +670,7 @@ def main():
                                   ("alpha", "ramp", "fused"), ("alpha", "translucent", "fused")):
             if vtrav == "sort_last" and vmode == args.mode and vtf == args.tf:
                 vtf = "ramp"
-            g.set_transfer_function(synth.tf_ramp() if vtf == "ramp" else synth.tf_translucent(), synth.TF_VMIN, synth.TF_VMAX)
+            g.set_transfer_function(pick_tf(wl, vtf), *tf_range(wl))
             g.set_traversal(vr.FUSED if vtrav == "fused" else vr.SORT_LAST)
             v = measure(0 if vmode == "alpha" else 1, False, None)
             g.set_traversal(vr.SORT_LAST)
@@ -656,7 +682,7 @@ def main():
                                           "composite": round(float(v["stages"][:, 2].mean()), 4)},
                              "roofline": roofline_of(v["counts"], v["stages"], v["stage_views"], peak, peak_src,
                                                      traffic_of(args.workload, vmode, vtf + ("" if vtrav == "sort_last" else "/fused")))})
-        g.set_transfer_function(tf, synth.TF_VMIN, synth.TF_VMAX)
+        g.set_transfer_function(tf, *tf_range(wl))
         line["variants"] = variants
 
     if rank == 0 and not args.no_cpu_baseline and world == 1:

@@ -202,7 +202,8 @@ int vr_render(vr_volume* v, const float* view, const float* proj, int width, int
  * sub-images, no compositing pass. R17: the result is what VR_SORT_LAST gives for a volume
  * held in a single brick (same sample schedule, R5; same voxels, R3), early termination
  * included; with early termination off the two traversals agree to rounding.
- * vr_debug_subimages and the transparent-brick counter do not apply to fused frames. */
+ * vr_debug_subimages does not apply to fused frames; transparent bricks (R16) are skipped along
+ * the ray, exactly as they are skipped as sub-images. */
 #define VR_SORT_LAST 0
 #define VR_FUSED 1
 int vr_set_traversal(vr_volume* v, int traversal);

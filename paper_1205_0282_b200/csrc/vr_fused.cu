@@ -99,6 +99,9 @@ vr_fused_kernel(const VrRaycastParams prm, float4* __restrict__ frame) {
             const float* __restrict__ brick = prm.bricks + (long long)b * g.slot;
             asm volatile("" : "+l"(brick)); /* keep the base in registers: do not rebuild it per load */
 
+            /* a brick the set-up kernel found transparent (R16: empty rendering rectangle) contributes exact
+             * zeros: its samples are skipped, the schedule moves on to the next brick */
+            if (owned && prm.bv[b].rx1 <= prm.bv[b].rx0) owned = false;
             const int k_lat = min(k_hi, max(k, ray.K - 2));
             int n = owned ? k_lat - k : 0;
             Lattice L;

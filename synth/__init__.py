@@ -25,6 +25,8 @@ def _cpu_lib():
         i64, u64, i32, vp, dbl = ctypes.c_int64, ctypes.c_uint64, ctypes.c_int32, ctypes.c_void_p, ctypes.c_double
         lib.vs_cube_create.restype = vp
         lib.vs_cube_create.argtypes = [u64, i64, i64, i64, i32, dbl]
+        lib.vs_cube_create_kind.restype = vp
+        lib.vs_cube_create_kind.argtypes = [u64, i64, i64, i64, i32, dbl, i32]
         lib.vs_cube_destroy.argtypes = [vp]
         for f in (lib.vs_cube_nprof, lib.vs_cube_ncell, lib.vs_cube_nitems):
             f.restype = i64
@@ -62,9 +64,12 @@ def default_threads():
 class Cube:
     """A seeded synthetic spectral cube, evaluable anywhere (host box, device box, one voxel)."""
 
-    def __init__(self, seed, nx, ny, nz, nsrc, ramp=0.0):
+    def __init__(self, seed, nx, ny, nz, nsrc, ramp=0.0, kind=0):
+        """kind SPECTRAL (0): N(0,1) noise + compact sources (+ spectral ramp); NBODY (1): the paper's other
+        data family (Table 1 "Nbody"), a density cube that is zero except for nsrc extended halos."""
         self.seed, self.nx, self.ny, self.nz, self.nsrc, self.ramp = int(seed), int(nx), int(ny), int(nz), int(nsrc), float(ramp)
-        self._h = _cpu_lib().vs_cube_create(self.seed, self.nx, self.ny, self.nz, self.nsrc, self.ramp)
+        self.kind = int(kind)
+        self._h = _cpu_lib().vs_cube_create_kind(self.seed, self.nx, self.ny, self.nz, self.nsrc, self.ramp, self.kind)
         if not self._h:
             raise ValueError("bad cube parameters")
         self._d = None
@@ -158,6 +163,18 @@ def tf_ramp(n=256):
     """Primary: literal linear ramp, all four channels = u (BASELINE.json configs)."""
     u = np.linspace(0.0, 1.0, n, dtype=np.float64)
     return np.stack([u, u, u, u], axis=1).astype(np.float32)
+
+
+def tf_density(n=256, toe=6):
+    """For NBODY cubes over [0, NBODY_VMAX]: the ramp with a zero-opacity toe (entries < toe), so
+    that empty space is exactly transparent and empty bricks can be skipped (R16)."""
+    t = tf_ramp(n)
+    t[:toe, 3] = 0.0
+    return t
+
+
+NBODY_VMAX = 20.0
+SPECTRAL, NBODY = 0, 1
 
 
 def tf_translucent(n=256):
@@ -262,10 +279,13 @@ CONFIGS = {
     "c1": dict(nx=512, ny=512, nz=512, brick=256, ghost=1, nsrc=200, ramp=0.0, width=1024, height=1024, step=0.5),
     "c2": dict(nx=1024, ny=1024, nz=1024, brick=256, ghost=1, nsrc=2000, ramp=1.0, width=1920, height=1080, step=0.5),
     "c3": dict(nx=4096, ny=4096, nz=1536, brick=512, ghost=1, nsrc=50000, ramp=0.0, width=1920, height=1080, step=1.0),
+    # row f4 (not a BASELINE.json config): the paper's other data family (Table 1 "Nbody" 1024^3, "scaled Nbody"
+    # 2600^3): a 2048^3 density cube (34 GB), zero except for 200 extended halos, in 512 bricks of 256^3
+    "n1": dict(nx=2048, ny=2048, nz=2048, brick=256, ghost=1, nsrc=200, ramp=0.0, width=1920, height=1080, step=0.5, kind=1),
 }
 
 
 def config_cube(name):
     c = CONFIGS[name]
-    k = int(name[1:])
-    return Cube(BASE_SEED + k, c["nx"], c["ny"], c["nz"], c["nsrc"], c["ramp"])
+    k = int(name[1:]) + (10 if name[0] == "n" else 0)
+    return Cube(BASE_SEED + k, c["nx"], c["ny"], c["nz"], c["nsrc"], c["ramp"], c.get("kind", 0))

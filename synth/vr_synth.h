@@ -11,12 +11,14 @@
  * The same functions compile for the host (gcc, -ffp-contract=off) and for the
  * device (nvcc, -fmad=false). Every floating-point step is an individually
  * IEEE-rounded operation (+, *, /, sqrt, fma), so host and device produce
- * bit-identical voxels; tests/test_synth.py and tests/test_gpu_synth.py check it.
+ * bit-identical voxels; tests/test_synth.py and tests/test_gpu_parity.py (test_device_generator_is_the_host_generator) check it.
  *
  * voxel(x,y,z) = noise(seed, linear index)                 i.i.d. N(0,1)
  *              + sum over sources s (ascending s) of
  *                peak_s * gx_s[x-x0_s] * gy_s[y-y0_s] * gz_s[z-z0_s]
  *              + ramp * (z + 1/2) / nz                      continuum-like gradient
+ * kind VS_NBODY (the paper's other data family, Table 1 "Nbody": a density cube, zero where
+ * there are no particles): no noise term, and the sources are extended halos (vr_synth_cpu.c).
  */
 #ifndef VR_SYNTH_H
 #define VR_SYNTH_H
@@ -68,7 +70,11 @@ typedef struct vs_cube {
     int32_t cgx, cgy, cgz;
     const int32_t* cell_start; /* [cgx*cgy*cgz + 1] */
     const int32_t* cell_items;
+    int32_t kind;        /* VS_SPECTRAL: noise + compact sources; VS_NBODY: no noise, extended halos on zero */
 } vs_cube;
+
+#define VS_SPECTRAL 0
+#define VS_NBODY 1
 
 /* 64-bit finaliser (splitmix64 constants). Counter-based: any index, any order. */
 VS_HD uint64_t vs_mix64(uint64_t x) {
@@ -163,7 +169,7 @@ VS_HD float vs_noise(uint64_t seed, uint64_t idx) {
 /* The synthetic cube's voxel (x fastest, z = spectral axis). */
 VS_HD float vs_voxel(const vs_cube* c, int64_t x, int64_t y, int64_t z) {
     uint64_t idx = (uint64_t)((z * c->ny + y) * c->nx + x);
-    float v = vs_noise(c->seed, idx);
+    float v = c->kind == VS_NBODY ? 0.0f : vs_noise(c->seed, idx);
     if (c->nsrc > 0) {
         int64_t cell = ((z / VS_CELL) * c->cgy + (y / VS_CELL)) * c->cgx + (x / VS_CELL);
         int32_t b = c->cell_start[cell], e = c->cell_start[cell + 1];

@@ -25,10 +25,18 @@ static double u01(uint64_t seed, uint64_t stream, uint64_t i) {
 
 static int64_t clampi(int64_t v, int64_t lo, int64_t hi) { return v < lo ? lo : (v > hi ? hi : v); }
 
+vs_cube* vs_cube_create_kind(uint64_t seed, int64_t nx, int64_t ny, int64_t nz, int32_t nsrc, double ramp, int32_t kind);
+
 vs_cube* vs_cube_create(uint64_t seed, int64_t nx, int64_t ny, int64_t nz, int32_t nsrc, double ramp) {
-    if (nx <= 0 || ny <= 0 || nz <= 0 || nsrc < 0) return NULL;
+    return vs_cube_create_kind(seed, nx, ny, nz, nsrc, ramp, VS_SPECTRAL);
+}
+
+/* kind VS_NBODY: density-cube stand-in (Table 1 "Nbody"): zero background, nsrc halos with
+ * log-uniform central density 0.5..30 and FWHM 4..32 voxels per axis, truncated at 5 sigma. */
+vs_cube* vs_cube_create_kind(uint64_t seed, int64_t nx, int64_t ny, int64_t nz, int32_t nsrc, double ramp, int32_t kind) {
+    if (nx <= 0 || ny <= 0 || nz <= 0 || nsrc < 0 || (kind != VS_SPECTRAL && kind != VS_NBODY)) return NULL;
     vs_cube* c = (vs_cube*)calloc(1, sizeof(vs_cube));
-    c->seed = seed; c->nx = nx; c->ny = ny; c->nz = nz; c->ramp = ramp; c->nsrc = nsrc;
+    c->seed = seed; c->nx = nx; c->ny = ny; c->nz = nz; c->ramp = ramp; c->nsrc = nsrc; c->kind = kind;
     c->cgx = (int32_t)((nx + VS_CELL - 1) / VS_CELL);
     c->cgy = (int32_t)((ny + VS_CELL - 1) / VS_CELL);
     c->cgz = (int32_t)((nz + VS_CELL - 1) / VS_CELL);
@@ -52,6 +60,10 @@ vs_cube* vs_cube_create(uint64_t seed, int64_t nx, int64_t ny, int64_t nz, int32
         sig[0] = (3.0 + 5.0 * u01(seed, 5, s)) / 2.3548;
         sig[1] = (3.0 + 5.0 * u01(seed, 6, s)) / 2.3548;
         sig[2] = (2.0 + 18.0 * u01(seed, 7, s)) / 2.3548;
+        if (kind == VS_NBODY) {
+            peak[s] = (float)(0.5 * exp(u01(seed, 4, s) * log(60.0)));
+            for (int a = 0; a < 3; ++a) sig[a] = (4.0 + 28.0 * u01(seed, 5 + a, s)) / 2.3548;
+        }
         int32_t org[3], len[3], off[3];
         for (int a = 0; a < 3; ++a) {
             int64_t lo = clampi((int64_t)floor(ctr[a] - 5.0 * sig[a]), 0, dims[a] - 1);

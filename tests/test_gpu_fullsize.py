@@ -24,11 +24,12 @@ def pair(vr, name, tf):
     import torch
     wl = bench.workload(name)
     g, cube = bench.build_volume(vr, wl, tf)
+    lo, hi = bench.tf_range(wl)
     if wl["nx"] * wl["ny"] * wl["nz"] <= 512 ** 3:
         o = oracle.Volume(wl["nx"], wl["ny"], wl["nz"], wl["brick"], wl["ghost"], data=cube.fill_host())
     else:
         o = oracle.Volume(wl["nx"], wl["ny"], wl["nz"], wl["brick"], wl["ghost"], voxel_fn=cube.voxel_fn())
-    o.set_transfer_function(tf, synth.TF_VMIN, synth.TF_VMAX)
+    o.set_transfer_function(tf, lo, hi)
     o.set_early_termination(wl["tau"])
     torch.cuda.synchronize()
     return wl, g, o, cube
@@ -143,3 +144,23 @@ def test_composite_microbenchmark_shape(vr):
         ref[q] = oracle.composite(host_layers, [(0, 0, 1, 1)] * n, order, 1, 1)[0, 0]
     got = out.cpu().numpy()[pix[:, 1], pix[:, 0]]
     assert np.abs(got - ref).max() < 1e-5
+
+
+def test_nbody_34GB_density_cube_with_culling(vr):
+    """Row f4 workload (bench.py --workload n1): 2048^3 density cube, 512 bricks, transfer function
+    with a zero-opacity toe. The device generator matches the host one, a good share of the
+    bricks is culled, and frames match the oracle (which renders every brick)."""
+    import torch
+    free, total = torch.cuda.mem_get_info()
+    if free < 45e9:
+        pytest.skip("needs ~40 GB of free device memory")
+    wl, g, o, cube = pair(vr, "n1", bench.pick_tf(bench.workload("n1"), "ramp"))
+    back = np.empty((2, wl["ny"], wl["nx"]), dtype=np.float32)
+    g.download(back, origin=(0, 0, 1023))
+    assert np.array_equal(back, cube.fill_host(0, 0, 1023, wl["nx"], wl["ny"], 2))
+    assert g.minmax()[0] == 0.0
+    check_views(vr, wl, g, o, (0, 13), 1200, (vr.ALPHA, vr.MIP), 0.99)
+    culled = g.debug_stats()["bricks_culled"]    # the last frame was MIP: never culled
+    assert culled == 0
+    gpu_frame(g, wl["views"][13], wl["proj"], wl["width"], wl["height"], wl["step"], vr.ALPHA)
+    assert g.debug_stats()["bricks_culled"] > 50

@@ -28,6 +28,18 @@ def views_for(cube, W, H, n_rot=3, seed=77):
     return out
 
 
+# --------------------------------------------------------------------------- inputs
+@pytest.mark.parametrize("kind", [0, 1])
+def test_device_generator_is_the_host_generator(vr, kind):
+    """synth's CUDA twin makes bit-identical cubes (it is what fills the 103 GB store), both kinds."""
+    import torch
+    c = synth.Cube(77, 70, 45, 33, 9, ramp=0.5, kind=kind)
+    dev = torch.empty((20, 30, 50), dtype=torch.float32, device="cuda")
+    c.fill_device(dev.data_ptr(), 11, 7, 5, 50, 30, 20, torch.cuda.current_stream().cuda_stream)
+    torch.cuda.synchronize()
+    assert np.array_equal(dev.cpu().numpy(), c.fill_host(11, 7, 5, 50, 30, 20))
+
+
 # --------------------------------------------------------------------------- a1 brick store
 @pytest.mark.parametrize("ghost", [0, 1, 2])
 def test_brick_store_is_bit_exact(vr, ghost):
@@ -320,6 +332,22 @@ def test_transparent_bricks_are_culled_exactly(vr):
     off = gpu_frame(g, view, proj, W, H, 0.5, vr.ALPHA)
     assert g.debug_stats()["bricks_culled"] == 0
     assert np.array_equal(on, off)
+    # the fused traversal skips the same bricks along each ray: same frame as with culling off, fewer samples
+    one = oracle.Volume(nx, ny, nz, 128, 1, data=data)
+    one.set_transfer_function(tf, synth.TF_VMIN, synth.TF_VMAX)
+    g.set_traversal(vr.FUSED)
+    g.set_counting(1)
+    f_off = gpu_frame(g, view, proj, W, H, 0.5, vr.ALPHA)
+    n_off = g.debug_stats()["samples"]
+    g.set_culling(True)
+    f_on = gpu_frame(g, view, proj, W, H, 0.5, vr.ALPHA)
+    n_on = g.debug_stats()["samples"]
+    assert np.array_equal(f_on, f_off) and n_on < 0.8 * n_off
+    r1 = one.render(view, proj, W, H, 0.5, oracle.ALPHA)
+    check_alpha(f_on, r1["image"], r1["flags"], 0.99, "fused, culled")
+    g.set_counting(0)
+    g.set_traversal(vr.SORT_LAST)
+    g.set_culling(False)
     # MIP never culls, and stops at the global maximum of the data without changing the frame
     g.set_culling(True)
     m_on = gpu_frame(g, view, proj, W, H, 0.5, vr.MIP)
