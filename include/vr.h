@@ -28,6 +28,14 @@
  *     matrices"; R1). Image: [height][width][4] float32 RGBA, row 0 = bottom row, pixel
  *     centres at half-integers.
  *
+ *   - Threads and devices: a handle belongs to the CUDA device that was current when it was
+ *     created and must be used with that device current. Calls on ONE handle must not
+ *     overlap in time (no internal locking); different handles may be used from different
+ *     threads. One process drives one GPU (the multi-GPU launch is one process per GPU).
+ *   - Environment (experiments only, read by vr_volume_create*): VR_TILE="lx,ly,lz,mx,my,mz"
+ *     (log2 micro-tile edge and log2 micro-tiles per macro block and axis; default 2,2,1,0,0,0)
+ *     and VR_LAYOUT=1|2 override the brick layout. Results never depend on the layout.
+ *
  * There is no CPU fallback: every call needs a CUDA device and fails with VR_ERR_CUDA
  * without one.
  */
@@ -42,7 +50,7 @@ extern "C" {
 
 typedef enum vr_status {
     VR_OK = 0,
-    VR_ERR_INVALID_ARG = 1,   /* bad sizes, NULL pointers, step <= 0, singular proj*view ... */
+    VR_ERR_INVALID_ARG = 1,   /* bad sizes, NULL pointers, step < 0, singular proj*view ... */
     VR_ERR_OUT_OF_MEMORY = 2, /* a device (or staging) allocation failed */
     VR_ERR_CUDA = 3,          /* a CUDA call or kernel launch failed; see vr_last_error */
     VR_ERR_STATE = 4          /* call order: no transfer function set, no data uploaded ... */
