@@ -187,6 +187,8 @@ def pick_tf(wl, name):
         if name == "translucent":
             t[:, 3] /= 64.0
         return t
+    if name == "threshold":  # noise hidden: zero opacity below 3.5 sigma (macro-cell skipping, R19)
+        return synth.tf_threshold()
     return synth.tf_ramp() if name == "ramp" else synth.tf_translucent()
 
 
@@ -528,7 +530,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="c3", choices=["c0", "c1", "c2", "c3", "c4", "n1"])
     ap.add_argument("--mode", default="alpha", choices=["alpha", "mip"])
-    ap.add_argument("--tf", default="ramp", choices=["ramp", "translucent"])
+    ap.add_argument("--tf", default="ramp", choices=["ramp", "translucent", "threshold"])
     ap.add_argument("--traversal", default="sort_last", choices=["sort_last", "fused"],
                     help="main arm: per-brick sub-images + compositing (the headline path) or the fused traversal (row f2)")
     ap.add_argument("--cells-every", type=int, default=6, help="count distinct cells on every n-th view of the cycle (0 = never)")
@@ -667,14 +669,21 @@ def main():
         # sort-last (the headline path) with the other transfer function / mode, then the fused traversal
         # (row f2: one ray through all bricks, global early termination, no sub-images, no compositing)
         for vmode, vtf, vtrav in (("alpha", "translucent", "sort_last"), ("mip", "ramp", "sort_last"),
-                                  ("alpha", "ramp", "fused"), ("alpha", "translucent", "fused")):
+                                  ("alpha", "ramp", "fused"), ("alpha", "translucent", "fused"),
+                                  ("alpha", "threshold", "sort_last"), ("alpha", "threshold", "fused")):
             if vtrav == "sort_last" and vmode == args.mode and vtf == args.tf:
                 vtf = "ramp"
             g.set_transfer_function(pick_tf(wl, vtf), *tf_range(wl))
             g.set_traversal(vr.FUSED if vtrav == "fused" else vr.SORT_LAST)
             v = measure(0 if vmode == "alpha" else 1, False, None)
+            extra = {}
+            if vtf == "threshold":  # the same frames (bit-identical) without brick culling and macro-cell skipping
+                g.set_culling(False)
+                ms_off = timed_device(g, wl, 0, order, K, Wm, out, dist)[0]
+                g.set_culling(True)
+                extra = {"frames_per_s_skipping_off": round(K / (ms_off * 1e-3), 3)}
             g.set_traversal(vr.SORT_LAST)
-            variants.append({"mode": vmode, "tf": vtf, "traversal": vtrav, "frames_per_s": round(K / (v["ms"] * 1e-3), 3),
+            variants.append({"mode": vmode, "tf": vtf, "traversal": vtrav, "frames_per_s": round(K / (v["ms"] * 1e-3), 3), **extra,
                              "gsamples_per_s": round(v["samples"] / (v["ms"] * 1e-3) / 1e9, 3),
                              "samples_per_frame": int(v["samples"] / K),
                              "stage_ms": {"setup": round(float(v["stages"][:, 0].mean()), 4),

@@ -175,6 +175,14 @@ int vr_volume_minmax(vr_volume* v, float* vmin_out, float* vmax_out, void* strea
  * value classifies to; the widening absorbs the rounding of interpolated values. Such a brick
  * contributes exact zeros, so the frame is bit-identical with culling on or off. */
 int vr_set_culling(vr_volume* v, int enable);
+/* With culling on, VR_ALPHA frames also skip transparent space INSIDE bricks (R19; 4x4x2 layout,
+ * ghost >= 1, and only when the transfer function has an entry with alpha == 0). The padded
+ * cells of a brick are cut into 8x8x8 macro-cells; macro-cell m is transparent iff R16's rule
+ * holds for the (min, max) of cells 8m .. 8m+8 per axis (the macro-cell plus one layer on its
+ * high sides) - every voxel a sample based in m can interpolate between. Samples based in a transparent macro-cell
+ * are not fetched: their opacity is exactly zero, so frames are bit-identical with culling on or
+ * off. The per-cell ranges are computed once after an upload (one streaming pass, 8 bytes per 512
+ * voxels of extra memory), the transparency bits once per transfer function. */
 
 /* ------------------------------------------------------------------------------------------
  * One frame (rows a2..a9): per-view set-up (inverse of proj*view, rendering rectangle of each
@@ -278,6 +286,11 @@ int vr_debug_ray_bricks(vr_volume* v, const float* view, const float* proj, int 
  * this handle with the same width/height (test access to row a8). sub_out: host
  * float[npix*nbricks*4]: VR_ALPHA premultiplied RGBA; VR_MIP (max, 0, 0, 0) with max = -inf
  * for "no sample". Bricks whose rectangle does not contain the pixel give zeros / -inf. */
+/* Macro-cell transparency flags of brick b under the current transfer function (R19).
+ * dims (host): 3 ints, macro-cells per axis of a brick slot; flags_out (host, may be NULL to ask
+ * for dims only): dims[0]*dims[1]*dims[2] bytes, x fastest, 1 = transparent. */
+int vr_debug_cell_flags(vr_volume* v, int b, unsigned char* flags_out, int* dims);
+
 /* mm_out (host): nbricks * 2 floats, (min, max) per brick over its ghost-padded cells. */
 int vr_debug_brick_minmax(vr_volume* v, float* mm_out);
 

@@ -27,7 +27,7 @@ STATUS = {0: "VR_OK", 1: "VR_ERR_INVALID_ARG", 2: "VR_ERR_OUT_OF_MEMORY", 3: "VR
 # every symbol include/vr.h declares (tests check the library exports each of them)
 SYMBOLS = (
     "vr_volume_create", "vr_volume_create_layout", "vr_volume_destroy", "vr_volume_upload", "vr_volume_download", "vr_debug_brick_data",
-    "vr_set_transfer_function", "vr_set_early_termination", "vr_volume_minmax", "vr_set_culling", "vr_set_traversal", "vr_debug_brick_minmax", "vr_render", "vr_render_host", "vr_render_host_async", "vr_render_host_wait", "vr_composite",
+    "vr_set_transfer_function", "vr_set_early_termination", "vr_volume_minmax", "vr_set_culling", "vr_set_traversal", "vr_debug_brick_minmax", "vr_debug_cell_flags", "vr_render", "vr_render_host", "vr_render_host_async", "vr_render_host_wait", "vr_composite",
     "vr_num_bricks", "vr_debug_brick_order", "vr_debug_rects", "vr_debug_ray_bricks", "vr_debug_subimages",
     "vr_set_counting", "vr_set_timing", "vr_debug_stats", "vr_debug_stage_times", "vr_launch_count", "vr_last_error",
 )
@@ -73,6 +73,7 @@ def lib():
         L.vr_set_culling.argtypes = [vp, ci]
         L.vr_set_traversal.argtypes = [vp, ci]
         L.vr_debug_brick_minmax.argtypes = [vp, vp]
+        L.vr_debug_cell_flags.argtypes = [vp, ci, vp, vp]
         L.vr_render.argtypes = [vp, vp, vp, ci, ci, cf, ci, vp, vp]
         L.vr_render_host.argtypes = [vp, vp, vp, ci, ci, cf, ci, vp, vp]
         L.vr_render_host_async.argtypes = [vp, vp, vp, ci, ci, cf, ci, vp, vp]
@@ -193,6 +194,14 @@ class Volume:
 
     def set_culling(self, enable):
         self._check(lib().vr_set_culling(self._h, int(bool(enable))))
+
+    def debug_cell_flags(self, b):
+        """[ncz][ncy][ncx] uint8: 1 where the 8x8x8 macro-cell of brick b is transparent under the current LUT (R19)."""
+        dims = (ctypes.c_int * 3)()
+        self._check(lib().vr_debug_cell_flags(self._h, int(b), None, dims))
+        out = np.empty((dims[2], dims[1], dims[0]), dtype=np.uint8)
+        self._check(lib().vr_debug_cell_flags(self._h, int(b), out.ctypes.data, dims))
+        return out
 
     def set_traversal(self, traversal):
         """SORT_LAST (per-brick sub-images + compositing, the default) or FUSED (one ray through all bricks)."""

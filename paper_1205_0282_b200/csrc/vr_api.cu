@@ -42,6 +42,11 @@ struct vr_volume {
     int2* d_mm_enc;          /* row f1: per-brick range, order-preserving integer encoding */
     float2* d_mm;            /* nbricks + 1 entries: per brick, then the whole volume */
     bool mm_valid;           /* d_mm describes the current contents of the store */
+    float2* d_cell_mm;       /* R19: (min, max) per 8x8x8 macro-cell, nbricks * nc^3 (allocated on first use) */
+    unsigned* d_cell_bits;   /* 1 = macro-cell transparent under the current LUT */
+    int nc[3], cell_words;   /* macro-cells per axis of a slot; words of d_cell_bits per brick */
+    bool cell_mm_valid, cell_bits_valid;
+    bool tf_has_zero;        /* the LUT has a run of >= 3 zero-alpha entries: skipping can do something */
     bool culling;
     int traversal;           /* VR_SORT_LAST or VR_FUSED */
     int counting;            /* 0 off, 1 samples, 2 samples + touched-cells bitmap */
@@ -106,6 +111,8 @@ static void release(vr_volume* v) {
     cudaFree(v->d_bitmap);
     cudaFree(v->d_mm_enc);
     cudaFree(v->d_mm);
+    cudaFree(v->d_cell_mm);
+    cudaFree(v->d_cell_bits);
     cudaFree(v->d_counts2);
     for (int r = 0; r < VR_EV_RING; ++r)
         for (int i = 0; i < 4; ++i)
@@ -307,6 +314,7 @@ extern "C" int vr_volume_upload(vr_volume* v, const float* src, int memspace, in
     }
     v->has_data = true;
     v->mm_valid = false;
+    v->cell_mm_valid = v->cell_bits_valid = false;
     return VR_OK;
 }
 
@@ -393,6 +401,14 @@ extern "C" int vr_set_transfer_function(vr_volume* v, const float* rgba, int n, 
     v->lut.inv_range = (float)(1.0 / ((double)vmax - (double)vmin));
     v->lut.nm2 = n - 2;
     v->lut.scale = (float)(n - 1);
+    /* R16 needs every entry of [I(min)-1, I(max)+2] transparent: at least three consecutive zero-alpha entries
+     * (a lone zero at entry 0, as in a linear ramp, can never make anything transparent) */
+    v->tf_has_zero = false;
+    for (int i = 0, run = 0; i < n; ++i) {
+        run = rgba[4 * i + 3] == 0.0f ? run + 1 : 0;
+        if (run >= 3) v->tf_has_zero = true;
+    }
+    v->cell_bits_valid = false;
     v->has_tf = true;
     return VR_OK;
 }
@@ -461,6 +477,37 @@ static int ensure_minmax(vr_volume* v, cudaStream_t st) {
     return VR_OK;
 }
 
+/* R19: macro-cell ranges (after an upload) and transparency bits (after an upload or a new transfer
+ * function). Only for the 4x4x2 layout with ghost cells; memory is taken on first use. */
+static bool cells_supported(const vr_volume* v) {
+    const VrGrid& g = v->grid;
+    return g.layout == VR_LAYOUT_TILED && g.tl[0] == 2 && g.tl[1] == 2 && g.tl[2] == 1 && g.ml[0] == 0 && g.ml[1] == 0 &&
+           g.ml[2] == 0 && g.ghost >= 1;
+}
+
+static int ensure_cells(vr_volume* v, cudaStream_t st) {
+    const VrGrid& g = v->grid;
+    if (!v->d_cell_mm) {
+        for (int a = 0; a < 3; ++a) v->nc[a] = (g.nt[a] * (1 << g.tl[a]) + 7) / 8;
+        const long long ncell = (long long)v->nc[0] * v->nc[1] * v->nc[2];
+        v->cell_words = (int)((ncell + 31) / 32);
+        VR_CUDA(v, cudaMalloc(&v->d_cell_mm, sizeof(float2) * (size_t)ncell * g.nbricks));
+        VR_CUDA(v, cudaMalloc(&v->d_cell_bits, sizeof(unsigned) * (size_t)v->cell_words * g.nbricks));
+    }
+    if (!v->cell_mm_valid) {
+        VR_CUDA(v, vr_launch_cell_minmax(g, v->bricks, v->d_cell_mm, v->nc, st));
+        v->launches++;
+        v->cell_mm_valid = true;
+        v->cell_bits_valid = false;
+    }
+    if (!v->cell_bits_valid) {
+        VR_CUDA(v, vr_launch_cell_flags(v->d_cell_mm, v->d_cell_bits, g.nbricks, v->nc, v->cell_words, v->lut, st));
+        v->launches++;
+        v->cell_bits_valid = true;
+    }
+    return VR_OK;
+}
+
 static int run_setup(vr_volume* v, const float* view, const float* proj, int W, int H, int mode, bool use_range,
                      cudaStream_t st) {
     VrMatrices m;
@@ -505,6 +552,27 @@ extern "C" int vr_set_culling(vr_volume* v, int enable) {
     return VR_OK;
 }
 
+extern "C" int vr_debug_cell_flags(vr_volume* v, int b, unsigned char* flags_out, int* dims) {
+    if (!v) return fail(NULL, VR_ERR_INVALID_ARG, "vr_debug_cell_flags: NULL handle");
+    if (!dims || b < 0 || b >= v->grid.nbricks) return fail(v, VR_ERR_INVALID_ARG, "vr_debug_cell_flags: bad brick %d or NULL dims", b);
+    if (!v->has_data || !v->has_tf) return fail(v, VR_ERR_STATE, "vr_debug_cell_flags: needs data and a transfer function");
+    if (!cells_supported(v)) return fail(v, VR_ERR_STATE, "vr_debug_cell_flags: macro-cells need the 4x4x2 layout and ghost >= 1");
+    const int rc = ensure_cells(v, 0);
+    if (rc) return rc;
+    for (int a = 0; a < 3; ++a) dims[a] = v->nc[a];
+    if (!flags_out) return VR_OK;
+    VR_CUDA(v, cudaDeviceSynchronize());
+    unsigned* words = new (std::nothrow) unsigned[v->cell_words];
+    if (!words) return fail(v, VR_ERR_OUT_OF_MEMORY, "vr_debug_cell_flags: host allocation failed");
+    const cudaError_t e = cudaMemcpy(words, v->d_cell_bits + (size_t)b * v->cell_words, sizeof(unsigned) * v->cell_words,
+                                     cudaMemcpyDeviceToHost);
+    if (e == cudaSuccess)
+        for (int m = 0; m < v->nc[0] * v->nc[1] * v->nc[2]; ++m) flags_out[m] = (unsigned char)((words[m >> 5] >> (m & 31)) & 1u);
+    delete[] words;
+    VR_CUDA(v, e);
+    return VR_OK;
+}
+
 extern "C" int vr_debug_brick_minmax(vr_volume* v, float* mm_out) {
     if (!v) return fail(NULL, VR_ERR_INVALID_ARG, "vr_debug_brick_minmax: NULL handle");
     if (!mm_out) return fail(v, VR_ERR_INVALID_ARG, "vr_debug_brick_minmax: NULL output");
@@ -536,6 +604,12 @@ extern "C" int vr_render(vr_volume* v, const float* view, const float* proj, int
         rc = ensure_minmax(v, st);
         if (rc) return rc;
     }
+    /* after an upload or a new transfer function only, and only if the table has a transparent range */
+    const bool skipping = v->culling && v->tf_has_zero && mode == VR_ALPHA && cells_supported(v);
+    if (skipping) {
+        rc = ensure_cells(v, st);
+        if (rc) return rc;
+    }
     if (timing) VR_CUDA(v, cudaEventRecord(ev[0], st));
     rc = run_setup(v, view, proj, width, height, mode, v->culling, st);
     if (rc) return rc;
@@ -551,6 +625,9 @@ extern "C" int vr_render(vr_volume* v, const float* view, const float* proj, int
     p.vs_rw = v->d_vs;
     p.sub = v->d_sub;
     p.bitmap = NULL;
+    p.cell_bits = skipping ? v->d_cell_bits : NULL;
+    p.nc[0] = v->nc[0]; p.nc[1] = v->nc[1]; p.nc[2] = v->nc[2];
+    p.cell_words = v->cell_words;
     if (v->counting == 2) {
         VR_CUDA(v, cudaMemsetAsync(v->d_bitmap, 0, (size_t)v->bitmap_words * sizeof(unsigned), st));
         p.bitmap = v->d_bitmap;

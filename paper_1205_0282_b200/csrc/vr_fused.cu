@@ -20,7 +20,7 @@
  */
 #include "vr_march.cuh"
 
-template <int MODE, int LAY, bool CLAMP, bool COUNT>
+template <int MODE, int LAY, bool CLAMP, bool COUNT, bool SKIP>
 __global__ void __launch_bounds__(VR_RAYCAST_THREADS, VR_MIN_CTAS)
 vr_fused_kernel(const VrRaycastParams prm, float4* __restrict__ frame) {
     extern __shared__ float4 s_lut[]; /* (entry, delta) pairs: shading (ALPHA), final colour map (MIP) */
@@ -122,21 +122,38 @@ vr_fused_kernel(const VrRaycastParams prm, float4* __restrict__ frame) {
             bool active = n > 0 && !stopped;
             Corners C;
             int pcx = INT_MIN, pcy = 0, pcz = 0;
+            /* R19: samples based in a transparent macro-cell are skipped (see vr_raycast.cu) */
+            const unsigned* __restrict__ cbits = SKIP ? prm.cell_bits + (long long)b * prm.cell_words : NULL;
+            int pm = -1;
+            bool ptransp = false;
             while (__any_sync(FULL_MASK, active)) {
                 if (active) {
                     const int cx = (int)(L.q[0] >> 32), cy = (int)(L.q[1] >> 32), cz = (int)(L.q[2] >> 32);
+                    bool skip = false;
                     if (!VR_REUSE || cx != pcx || cy != pcy || cz != pcz) {
-                        fetch8<LAY, 0, CLAMP, COUNT>(brick, g, ext, L, prm.bitmap, (long long)b * g.slot, C);
-                        pcx = cx, pcy = cy, pcz = cz;
+                        if (SKIP) {
+                            const int m = ((cz >> 3) * prm.nc[1] + (cy >> 3)) * prm.nc[0] + (cx >> 3);
+                            if (m != pm) {
+                                pm = m;
+                                ptransp = (__ldg(cbits + (m >> 5)) >> (m & 31)) & 1u;
+                            }
+                            skip = ptransp;
+                        }
+                        if (!skip) {
+                            fetch8<LAY, 0, CLAMP, COUNT>(brick, g, ext, L, prm.bitmap, (long long)b * g.slot, C);
+                            pcx = cx, pcy = cy, pcz = cz;
+                        }
                     }
-                    const float v = lerp8(C, L);
-                    if (COUNT) ++nsamples;
-                    if (MODE == VR_MIP) {
-                        acc.r = fmaxf(acc.r, v);
-                        stopped = acc.r >= mip_stop;
-                    } else {
-                        shade_alpha(acc, v, stepf, lut, prm.lut);
-                        stopped = !(acc.a < tau);
+                    if (!skip) {
+                        const float v = lerp8(C, L);
+                        if (COUNT) ++nsamples;
+                        if (MODE == VR_MIP) {
+                            acc.r = fmaxf(acc.r, v);
+                            stopped = acc.r >= mip_stop;
+                        } else {
+                            shade_alpha(acc, v, stepf, lut, prm.lut);
+                            stopped = !(acc.a < tau);
+                        }
                     }
                     L.q[0] += D[0], L.q[1] += D[1], L.q[2] += D[2];
                     --n;
@@ -191,7 +208,7 @@ vr_fused_kernel(const VrRaycastParams prm, float4* __restrict__ frame) {
     }
 }
 
-template <int MODE, int LAY, bool CLAMP, bool COUNT>
+template <int MODE, int LAY, bool CLAMP, bool COUNT, bool SKIP = false>
 static cudaError_t launch_fused(const VrRaycastParams& p, float* frame, long long items, cudaStream_t st) {
     static int sms = 0, cached_per_sm = 0;
     static size_t cached_smem = (size_t)-1;
@@ -201,7 +218,7 @@ static cudaError_t launch_fused(const VrRaycastParams& p, float* frame, long lon
         cudaError_t e = cudaGetDevice(&dev);
         if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
         if (e == cudaSuccess)
-            e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&cached_per_sm, vr_fused_kernel<MODE, LAY, CLAMP, COUNT>,
+            e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&cached_per_sm, vr_fused_kernel<MODE, LAY, CLAMP, COUNT, SKIP>,
                                                               VR_RAYCAST_THREADS, smem);
         if (e != cudaSuccess) return e;
         if (cached_per_sm < 1) return cudaErrorLaunchOutOfResources;
@@ -210,7 +227,7 @@ static cudaError_t launch_fused(const VrRaycastParams& p, float* frame, long lon
     long long ctas = (long long)sms * cached_per_sm;
     const long long want = (items + (VR_RAYCAST_THREADS / 32) - 1) / (VR_RAYCAST_THREADS / 32);
     if (ctas > want) ctas = want < 1 ? 1 : want;
-    vr_fused_kernel<MODE, LAY, CLAMP, COUNT><<<(int)ctas, VR_RAYCAST_THREADS, smem, st>>>(p, reinterpret_cast<float4*>(frame));
+    vr_fused_kernel<MODE, LAY, CLAMP, COUNT, SKIP><<<(int)ctas, VR_RAYCAST_THREADS, smem, st>>>(p, reinterpret_cast<float4*>(frame));
     return cudaGetLastError();
 }
 
@@ -223,9 +240,12 @@ static cudaError_t launch_fused_mode(const VrRaycastParams& p, float* frame, lon
     if (g.layout == VR_LAYOUT_LINEAR)
         return clamp ? launch_fused<MODE, LAY_LINEAR, true, COUNT>(p, frame, items, st)
                      : launch_fused<MODE, LAY_LINEAR, false, COUNT>(p, frame, items, st);
-    if (t442)
+    if (t442) {
+        if (MODE == VR_ALPHA && !clamp && p.cell_bits) /* R19: macro-cell skipping */
+            return launch_fused<MODE, LAY_TILE442, false, COUNT, MODE == VR_ALPHA>(p, frame, items, st);
         return clamp ? launch_fused<MODE, LAY_TILE442, true, COUNT>(p, frame, items, st)
                      : launch_fused<MODE, LAY_TILE442, false, COUNT>(p, frame, items, st);
+    }
     return clamp ? launch_fused<MODE, LAY_GENERIC, true, COUNT>(p, frame, items, st)
                  : launch_fused<MODE, LAY_GENERIC, false, COUNT>(p, frame, items, st);
 }

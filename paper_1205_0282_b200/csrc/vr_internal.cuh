@@ -119,6 +119,9 @@ struct VrRaycastParams {
     VrViewState* vs_rw; /* work counter, sample counter */
     void* sub;          /* float4[] (ALPHA) or float[] (MIP) */
     unsigned* bitmap;   /* counting variant only: one bit per brick-store cell, or NULL */
+    const unsigned* cell_bits; /* R19: one bit per 8x8x8 macro-cell, 1 = transparent under the LUT; NULL = no skipping */
+    int nc[3];          /* macro-cells per axis of a brick slot */
+    int cell_words;     /* 32-bit words of cell_bits per brick */
     VrLut lut;
     double step; /* > 0: sample spacing in voxels; 0: per ray, 1 / max|d_a| (R18) */
     float tau;
@@ -140,6 +143,10 @@ cudaError_t vr_launch_setup(const VrGrid& grid, const VrMatrices& mats, int W, i
                             long long sub_capacity_px, void* sub_base, VrViewState* vs, VrBrickView* bv, int* order,
                             int* item_prefix, VrCompLayer* layers, const float2* range, const VrLut& lut, cudaStream_t st);
 cudaError_t vr_launch_minmax(const VrGrid& grid, const float* bricks, int2* enc, float2* table, cudaStream_t st);
+/* macro-cells (R19): per-cell (min, max) of the 4x4x2-tiled store; transparency bits for a LUT */
+cudaError_t vr_launch_cell_minmax(const VrGrid& grid, const float* bricks, float2* cell_mm, const int nc[3], cudaStream_t st);
+cudaError_t vr_launch_cell_flags(const float2* cell_mm, unsigned* bits, int nbricks, const int nc[3], int words_per_brick,
+                                 const VrLut& lut, cudaStream_t st);
 /* items = work items of the view (sizes the persistent grid); sparse = the view samples the store at
  * more than two voxels per pixel (launch heuristic only) */
 cudaError_t vr_launch_raycast(const VrRaycastParams& p, long long items, bool count, bool sparse, cudaStream_t st);

@@ -122,3 +122,111 @@ cudaError_t vr_launch_minmax(const VrGrid& grid, const float* bricks, int2* enc,
     vr_minmax_finish_kernel<<<1, 256, 0, st>>>(enc, grid.nbricks, table);
     return cudaGetLastError();
 }
+
+/* ------------------------------------------------------------------------------------------
+ * Macro-cells (empty-space skipping inside a brick, R19). A brick's padded cells are cut into
+ * 8x8x8 macro-cells (4x4x2 layout: 2x2x4 micro-tiles = 16 whole lines). A sample whose base
+ * cell lies in macro-cell m reads cells 8m .. 8m+8 per axis only, so cell_mm[b][m] is the
+ * (min, max) over that 9x9x9 block (the macro-cell plus one layer on its high sides): it
+ * bounds everything such a sample can interpolate between. A macro-cell is flagged
+ * TRANSPARENT for the current transfer function with R16's rule on that range; the ray-cast
+ * kernels then skip the samples based in it: their opacity is exactly zero, so the frame does
+ * not change by a bit.
+ * ---------------------------------------------------------------------------------------- */
+__global__ void __launch_bounds__(256)
+vr_cell_minmax_kernel(VrGrid g, const float* __restrict__ bricks, float2* __restrict__ cell_mm, int nc0, int nc1, int nc2) {
+    /* one warp per macro-cell: 16 micro-tiles x 8 rows = 128 float4 words, 4 per lane */
+    const int b = blockIdx.y;
+    int bc[3], lo[3], hi[3];
+    vr_brick_coords(g, b, bc);
+    vr_brick_core(g, bc, lo, hi);
+    const int ex = hi[0] - lo[0] + 2 * g.ghost, ey = hi[1] - lo[1] + 2 * g.ghost, ez = hi[2] - lo[2] + 2 * g.ghost;
+    const float* __restrict__ base = bricks + (long long)b * g.slot;
+    const int lane = threadIdx.x & 31, ncell = nc0 * nc1 * nc2;
+    for (int m = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); m < ncell; m += gridDim.x * (blockDim.x >> 5)) {
+        const int m2 = m / (nc0 * nc1), rem = m - m2 * (nc0 * nc1), m1 = rem / nc0, m0 = rem - m1 * nc0;
+        float mn = INFINITY, mx = -INFINITY;
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            const int w = lane + 32 * q;           /* word of the macro-cell: tile (w >> 3), row (w & 7) */
+            const int t = w >> 3, r = w & 7;
+            const int tx = (m0 << 1) + (t & 1), ty = (m1 << 1) + ((t >> 1) & 1), tz = (m2 << 2) + (t >> 2);
+            const int i = tx << 2, j = (ty << 2) + (r & 3), k = (tz << 1) + (r >> 2);
+            if (tx < g.nt[0] && ty < g.nt[1] && tz < g.nt[2] && i < ex && j < ey && k < ez) {
+                const long long word = ((long long)((tz * g.nt[1] + ty) * g.nt[0] + tx) << 3) + r;
+                const float4 v = __ldcs(reinterpret_cast<const float4*>(base) + word);
+                mn = fminf(mn, v.x), mx = fmaxf(mx, v.x);
+                if (i + 1 < ex) mn = fminf(mn, v.y), mx = fmaxf(mx, v.y);
+                if (i + 2 < ex) mn = fminf(mn, v.z), mx = fmaxf(mx, v.z);
+                if (i + 3 < ex) mn = fminf(mn, v.w), mx = fmaxf(mx, v.w);
+            }
+        }
+        /* the layer on the high sides: planes x = 8 (9x9), y = 8 (8x9), z = 8 (8x8) of the 9x9x9 block */
+        for (int h = lane; h < 217; h += 32) {
+            int a, c, d;
+            if (h < 81) a = 8, c = h % 9, d = h / 9;
+            else if (h < 153) a = (h - 81) & 7, c = 8, d = (h - 81) >> 3;
+            else a = (h - 153) & 7, c = (h - 153) >> 3, d = 8;
+            const int i = (m0 << 3) + a, j = (m1 << 3) + c, k = (m2 << 3) + d;
+            if (i < ex && j < ey && k < ez) {
+                const float x = __ldg(base + vr_cell_offset(g, i, j, k));
+                mn = fminf(mn, x), mx = fmaxf(mx, x);
+            }
+        }
+        for (int o = 16; o > 0; o >>= 1) {
+            mn = fminf(mn, __shfl_xor_sync(0xffffffffu, mn, o));
+            mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+        }
+        if (lane == 0) cell_mm[(long long)b * ncell + m] = make_float2(mn + 0.0f, mx + 0.0f);
+    }
+}
+
+/* bits[b][m] = 1 iff macro-cell m of brick b is transparent under the LUT (R19). One thread per cell. */
+__global__ void __launch_bounds__(256)
+vr_cell_flags_kernel(const float2* __restrict__ cell_mm, unsigned* __restrict__ bits, int nbricks, int nc0, int nc1, int nc2,
+                     int words_per_brick, VrLut lut) {
+    __shared__ unsigned short nz_prefix[VR_MAX_LUT + 1];
+    for (int i = threadIdx.x; i < lut.n; i += blockDim.x) nz_prefix[i + 1] = lut.base[i].w != 0.0f ? 1 : 0;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        nz_prefix[0] = 0;
+        for (int i = 1; i <= lut.n; ++i) nz_prefix[i] = (unsigned short)(nz_prefix[i] + nz_prefix[i - 1]);
+    }
+    __syncthreads();
+    const int ncell = nc0 * nc1 * nc2;
+    const long long total = (long long)nbricks * words_per_brick * 32;
+    for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < total; t += (long long)gridDim.x * blockDim.x) {
+        const int b = (int)(t / (words_per_brick * 32)), m = (int)(t - (long long)b * words_per_brick * 32);
+        bool transparent = false;
+        if (m < ncell) {
+            const float2 rr = cell_mm[(long long)b * ncell + m];
+            const float mn = rr.x, mx = rr.y;
+            if (mn <= mx) { /* R16's entry range in float32 */
+                const float ulo = __saturatef(__fmul_rn(__fsub_rn(mn, lut.vmin), lut.inv_range));
+                const float uhi = __saturatef(__fmul_rn(__fsub_rn(mx, lut.vmin), lut.inv_range));
+                const int i0 = max(min((int)__fmul_rn(ulo, lut.scale), lut.nm2) - 1, 0);
+                const int i1 = min(min((int)__fmul_rn(uhi, lut.scale), lut.nm2) + 2, lut.n - 1);
+                transparent = nz_prefix[i1 + 1] == nz_prefix[i0];
+            }
+        }
+        const unsigned word = __ballot_sync(0xffffffffu, transparent);
+        if ((threadIdx.x & 31) == 0) bits[t >> 5] = word;
+    }
+}
+
+cudaError_t vr_launch_cell_minmax(const VrGrid& grid, const float* bricks, float2* cell_mm, const int nc[3], cudaStream_t st) {
+    const long long ncell = (long long)nc[0] * nc[1] * nc[2];
+    long long bx = (ncell + 7) / 8;
+    if (bx > 4096) bx = 4096;
+    vr_cell_minmax_kernel<<<dim3((unsigned)bx, grid.nbricks), 256, 0, st>>>(grid, bricks, cell_mm, nc[0], nc[1], nc[2]);
+    return cudaGetLastError();
+}
+
+cudaError_t vr_launch_cell_flags(const float2* cell_mm, unsigned* bits, int nbricks, const int nc[3], int words_per_brick,
+                                 const VrLut& lut, cudaStream_t st) {
+    const long long total = (long long)nbricks * words_per_brick * 32;
+    long long blocks = (total + 255) / 256;
+    if (blocks > 148 * 16) blocks = 148 * 16;
+    vr_cell_flags_kernel<<<(unsigned)blocks, 256, 0, st>>>(cell_mm, bits, nbricks, nc[0], nc[1], nc[2], words_per_brick, lut);
+    return cudaGetLastError();
+}

@@ -25,7 +25,7 @@
  */
 #include "vr_march.cuh"
 
-template <int MODE, int LAY, int PT, bool CLAMP, bool COUNT>
+template <int MODE, int LAY, int PT, bool CLAMP, bool COUNT, bool SKIP>
 __global__ void __launch_bounds__(VR_RAYCAST_THREADS, VR_MIN_CTAS)
 vr_raycast_kernel(const VrRaycastParams prm) {
     /* dynamic: 2 * lut.n float4 (ALPHA) - a 256-entry table takes 8 KB, not the 32 KB of the
@@ -132,21 +132,39 @@ vr_raycast_kernel(const VrRaycastParams prm) {
          * bound of densely sampled views). */
         Corners C;
         int pcx = INT_MIN, pcy = 0, pcz = 0;
+        /* R19: samples based in a macro-cell the transfer function makes transparent are skipped (their
+         * opacity is exactly 0): no voxel is fetched. The flag is looked up when the macro-cell changes. */
+        const unsigned* __restrict__ cbits = SKIP ? prm.cell_bits + (long long)b * prm.cell_words : NULL;
+        int pm = -1;
+        bool ptransp = false;
         while (__any_sync(FULL_MASK, active)) {
             if (active) {
                 const int cx = (int)(L.q[0] >> 32), cy = (int)(L.q[1] >> 32), cz = (int)(L.q[2] >> 32);
+                bool skip = false;
                 if (!VR_REUSE || cx != pcx || cy != pcy || cz != pcz) {
-                    fetch8<LAY, PT, CLAMP, COUNT>(brick, g, ext, L, prm.bitmap, (long long)b * g.slot, C);
-                    pcx = cx, pcy = cy, pcz = cz;
+                    if (SKIP) {
+                        const int m = ((cz >> 3) * prm.nc[1] + (cy >> 3)) * prm.nc[0] + (cx >> 3);
+                        if (m != pm) {
+                            pm = m;
+                            ptransp = (__ldg(cbits + (m >> 5)) >> (m & 31)) & 1u;
+                        }
+                        skip = ptransp;
+                    }
+                    if (!skip) {
+                        fetch8<LAY, PT, CLAMP, COUNT>(brick, g, ext, L, prm.bitmap, (long long)b * g.slot, C);
+                        pcx = cx, pcy = cy, pcz = cz;
+                    }
                 }
-                const float v = lerp8(C, L);
-                if (COUNT) ++nsamples;
-                if (MODE == VR_MIP) {
-                    acc.r = fmaxf(acc.r, v);
-                    stopped = acc.r >= mip_stop;
-                } else {
-                    shade_alpha(acc, v, stepf, lut, prm.lut);
-                    stopped = !(acc.a < tau);
+                if (!skip) {
+                    const float v = lerp8(C, L);
+                    if (COUNT) ++nsamples;
+                    if (MODE == VR_MIP) {
+                        acc.r = fmaxf(acc.r, v);
+                        stopped = acc.r >= mip_stop;
+                    } else {
+                        shade_alpha(acc, v, stepf, lut, prm.lut);
+                        stopped = !(acc.a < tau);
+                    }
                 }
                 L.q[0] += D[0], L.q[1] += D[1], L.q[2] += D[2];
                 --n;
@@ -200,7 +218,7 @@ vr_raycast_kernel(const VrRaycastParams prm) {
 /* ------------------------------------------------------------------------------------------ */
 /* Persistent grid: resident CTAs per SM (for this instance and its shared memory) x SMs,
  * but no more CTAs than there are groups of 8 work items. */
-template <int MODE, int LAY, int PT, bool CLAMP, bool COUNT>
+template <int MODE, int LAY, int PT, bool CLAMP, bool COUNT, bool SKIP = false>
 static cudaError_t launch_variant(const VrRaycastParams& p, long long items, bool sparse, cudaStream_t st) {
     static int sms = 0, cached_per_sm = 0;
     static size_t cached_smem = (size_t)-1;
@@ -210,7 +228,7 @@ static cudaError_t launch_variant(const VrRaycastParams& p, long long items, boo
         cudaError_t e = cudaGetDevice(&dev);
         if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
         if (e == cudaSuccess)
-            e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&cached_per_sm, vr_raycast_kernel<MODE, LAY, PT, CLAMP, COUNT>,
+            e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&cached_per_sm, vr_raycast_kernel<MODE, LAY, PT, CLAMP, COUNT, SKIP>,
                                                               VR_RAYCAST_THREADS, smem);
         if (e != cudaSuccess) return e;
         if (cached_per_sm < 1) return cudaErrorLaunchOutOfResources;
@@ -223,7 +241,7 @@ static cudaError_t launch_variant(const VrRaycastParams& p, long long items, boo
     long long ctas = (long long)sms * per_sm;
     const long long want = (items + (VR_RAYCAST_THREADS / 32) - 1) / (VR_RAYCAST_THREADS / 32);
     if (ctas > want) ctas = want < 1 ? 1 : want;
-    vr_raycast_kernel<MODE, LAY, PT, CLAMP, COUNT><<<(int)ctas, VR_RAYCAST_THREADS, smem, st>>>(p);
+    vr_raycast_kernel<MODE, LAY, PT, CLAMP, COUNT, SKIP><<<(int)ctas, VR_RAYCAST_THREADS, smem, st>>>(p);
     return cudaGetLastError();
 }
 
@@ -243,9 +261,12 @@ static cudaError_t launch_mode(const VrRaycastParams& p, long long ctas, bool sp
             default: return launch_variant<MODE, LAY_LINEAR, 0, false, COUNT>(p, ctas, sparse, st);
         }
     }
-    if (is_tile442(p.grid))
+    if (is_tile442(p.grid)) {
+        if (MODE == VR_ALPHA && !clamp && p.cell_bits) /* R19: macro-cell skipping, the transfer function has a transparent range */
+            return launch_variant<MODE, LAY_TILE442, 0, false, COUNT, MODE == VR_ALPHA>(p, ctas, sparse, st);
         return clamp ? launch_variant<MODE, LAY_TILE442, 0, true, COUNT>(p, ctas, sparse, st)
                      : launch_variant<MODE, LAY_TILE442, 0, false, COUNT>(p, ctas, sparse, st);
+    }
     return clamp ? launch_variant<MODE, LAY_GENERIC, 0, true, COUNT>(p, ctas, sparse, st)
                  : launch_variant<MODE, LAY_GENERIC, 0, false, COUNT>(p, ctas, sparse, st);
 }

@@ -177,6 +177,14 @@ NBODY_VMAX = 20.0
 SPECTRAL, NBODY = 0, 1
 
 
+def tf_threshold(n=256, cut=0.5):
+    """The usual way to look at a noisy spectral cube: the ramp with zero opacity below u = cut
+    (value 3.5 sigma for cut = 0.5 over [-3, 10]), so that only the sources show."""
+    t = tf_ramp(n)
+    t[:int(round(cut * (n - 1))) + 1, 3] = 0.0
+    return t
+
+
 def tf_translucent(n=256):
     """Secondary: same colours, opacity u/64 per voxel (rays cross most of the cube)."""
     u = np.linspace(0.0, 1.0, n, dtype=np.float64)

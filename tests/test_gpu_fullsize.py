@@ -99,6 +99,14 @@ def test_config2_1024cube_64_bricks(vr):
     wl, g, o, cube = pair(vr, "c2", synth.tf_ramp())
     check_views(vr, wl, g, o, (0, 5, 17), 1500, (vr.ALPHA, vr.MIP), 0.99)
     check_fused(vr, wl, g, cube, synth.tf_ramp(), (9,), 1000, (vr.ALPHA,), 0.99)
+    # config 4's resolution sweep uses this cube at square frames up to 4096^2 (0.4 voxels per pixel)
+    w4 = dict(wl)
+    w4["width"] = w4["height"] = 4096
+    fr = synth.Framing(wl["nx"], wl["ny"], wl["nz"], 4096, 4096)
+    w4["views"] = [fr.seeded(wl["seed"], k) for k in range(36)]
+    w4["proj"] = fr.proj(False)
+    w4["name"] = "c4@4096"
+    check_views(vr, w4, g, o, (21,), 1000, (vr.ALPHA, vr.MIP), 0.99)
 
 
 def test_config3_103GB_cube_192_bricks(vr):

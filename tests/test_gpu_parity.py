@@ -358,6 +358,75 @@ def test_transparent_bricks_are_culled_exactly(vr):
     check_mip(m_on, o.render(view, proj, W, H, 0.5, oracle.MIP)["image"], "MIP with data-max stop")
 
 
+# --------------------------------------------------------------------------- R19 macro-cell skipping
+def test_macro_cell_skipping_is_exact(vr):
+    """A transfer function that hides the noise (alpha 0 below ~3.5 sigma, the usual way to look
+    at a spectral cube): the 8x8x8 macro-cell flags equal an independent numpy statement of R19,
+    frames are bit-identical with skipping on and off in both traversals, match the oracle, and
+    most samples are never fetched."""
+    nx, ny, nz, B = 100, 84, 60, 32                  # ragged 4 x 3 x 2 bricks
+    cube = synth.Cube(71, nx, ny, nz, 10)
+    data = cube.fill_host()
+    tf = synth.tf_ramp()
+    tf[:128, 3] = 0.0                                # opacity only above u = 0.5 (value 3.5)
+    g = vr.Volume(nx, ny, nz, B, 1)
+    g.upload(data)
+    o = oracle.Volume(nx, ny, nz, B, 1, data=data)
+    one = oracle.Volume(nx, ny, nz, 128, 1, data=data)
+    for v in (g, o, one):
+        v.set_transfer_function(tf, synth.TF_VMIN, synth.TF_VMAX)
+        v.set_early_termination(0.99)
+    # flags: numpy on the oracle's padded copy of the brick (float32 arithmetic of R16's entry rule)
+    n = tf.shape[0]
+    inv = np.float32(1.0 / (np.float64(np.float32(synth.TF_VMAX)) - np.float64(np.float32(synth.TF_VMIN))))
+
+    def entry(x):
+        u = np.clip((np.float32(x) - np.float32(synth.TF_VMIN)) * inv, np.float32(0), np.float32(1))
+        return min(int(np.float32(u) * np.float32(n - 1)), n - 2)
+
+    for b in (0, 5, g.nbricks - 1):
+        pad = o.brick_data(b)                        # [dz][dy][dx] ghost-padded
+        flags = g.debug_cell_flags(b)
+        ncz, ncy, ncx = flags.shape
+        seen = 0
+        for mz in range(ncz):
+            for my in range(ncy):
+                for mx in range(ncx):
+                    blk = pad[8 * mz:8 * mz + 9, 8 * my:8 * my + 9, 8 * mx:8 * mx + 9]   # the macro-cell + one layer
+                    if blk.size == 0:
+                        continue
+                    i0, i1 = max(entry(blk.min()) - 1, 0), min(entry(blk.max()) + 2, n - 1)
+                    assert flags[mz, my, mx] == int(not tf[i0:i1 + 1, 3].any()), (b, mx, my, mz)
+                    seen += 1
+        assert seen >= 8 and 0 < flags.sum()
+    W, H = 200, 150
+    fr = synth.Framing(nx, ny, nz, W, H)
+    view, proj = fr.seeded(2, 1), fr.proj(False)
+    g.set_counting(1)
+    for trav, orc in ((vr.SORT_LAST, o), (vr.FUSED, one)):
+        g.set_traversal(trav)
+        g.set_culling(True)
+        on = gpu_frame(g, view, proj, W, H, 0.5, vr.ALPHA)
+        n_on = g.debug_stats()["samples"]
+        g.set_culling(False)
+        off = gpu_frame(g, view, proj, W, H, 0.5, vr.ALPHA)
+        n_off = g.debug_stats()["samples"]
+        assert np.array_equal(on, off) and on[..., 3].max() > 0.2
+        assert n_on < 0.5 * n_off
+        ref = orc.render(view, proj, W, H, 0.5, oracle.ALPHA)
+        check_alpha(on, ref["image"], ref["flags"], 0.99, "macro-cell skipping")
+        assert n_off == int(ref["counts"][..., 0].sum())
+    # a new transfer function re-flags the cells; one without transparent entries switches skipping off
+    g.set_traversal(vr.SORT_LAST)
+    g.set_culling(True)
+    g.set_transfer_function(synth.tf_ramp(), synth.TF_VMIN, synth.TF_VMAX)
+    o.set_transfer_function(synth.tf_ramp(), synth.TF_VMIN, synth.TF_VMAX)
+    ref = o.render(view, proj, W, H, 0.5, oracle.ALPHA)
+    check_alpha(gpu_frame(g, view, proj, W, H, 0.5, vr.ALPHA), ref["image"], ref["flags"], 0.99, "ramp after threshold")
+    # nothing is skipped any more (a termination decided in float32 may differ by one sample on a few rays, R12)
+    assert abs(g.debug_stats()["samples"] - int(ref["counts"][..., 0].sum())) <= 1e-4 * ref["counts"][..., 0].sum()
+
+
 # --------------------------------------------------------------------------- f2 fused traversal (R17)
 @pytest.mark.parametrize("tau", [0.99, 2.0])
 @pytest.mark.parametrize("ortho", [False, True])
