@@ -20,8 +20,14 @@
  *     int<->float conversion in the loop, and a position error below 1e-7 voxel;
  *   - tri-linear interpolation is hand-rolled in float32 on 8 read-only loads (hardware
  *     texture filtering has 8-bit weights and cannot meet the MIP tolerance);
- *   - the LUT is staged in shared memory as (entry, delta) pairs;
- *   - early ray termination and loop exit are warp votes.
+ *   - the LUT is staged in dynamic shared memory as interleaved (entry, delta) pairs;
+ *   - early ray termination and loop exit are warp votes;
+ *   - 80 registers (3 CTAs per SM): the FP64 ray is rebuilt for the exit samples instead of
+ *     living through the loop; the 8 voxels are kept while a ray stays in one cell;
+ *   - with a transfer function that has a transparent range, samples based in a transparent
+ *     8x8x8 macro-cell are not fetched (R19; the SKIP instances).
+ * Measured bounds: DRAM lines on the 103 GB cube, issue slots / L1 data stage on the small
+ * cubes (DESIGN.md sections 8 and 9; profiles/).
  */
 #include "vr_march.cuh"
 
