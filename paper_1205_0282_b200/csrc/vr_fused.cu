@@ -129,7 +129,7 @@ vr_fused_kernel(const VrRaycastParams prm, float4* __restrict__ frame) {
             while (__any_sync(FULL_MASK, active)) {
                 if (active) {
                     const int cx = (int)(L.q[0] >> 32), cy = (int)(L.q[1] >> 32), cz = (int)(L.q[2] >> 32);
-                    bool skip = false;
+                    int adv = 1; /* lattice steps this trip takes */
                     if (!VR_REUSE || cx != pcx || cy != pcy || cz != pcz) {
                         if (SKIP) {
                             const int m = ((cz >> 3) * prm.nc[1] + (cy >> 3)) * prm.nc[0] + (cx >> 3);
@@ -137,14 +137,14 @@ vr_fused_kernel(const VrRaycastParams prm, float4* __restrict__ frame) {
                                 pm = m;
                                 ptransp = (__ldg(cbits + (m >> 5)) >> (m & 31)) & 1u;
                             }
-                            skip = ptransp;
+                            if (ptransp) adv = -leap_steps(L, D, n); /* negative: a leap over transparent samples, nothing fetched */
                         }
-                        if (!skip) {
+                        if (adv > 0) {
                             fetch8<LAY, 0, CLAMP, COUNT>(brick, g, ext, L, prm.bitmap, (long long)b * g.slot, C);
                             pcx = cx, pcy = cy, pcz = cz;
                         }
                     }
-                    if (!skip) {
+                    if (adv > 0) {
                         const float v = lerp8(C, L);
                         if (COUNT) ++nsamples;
                         if (MODE == VR_MIP) {
@@ -154,9 +154,12 @@ vr_fused_kernel(const VrRaycastParams prm, float4* __restrict__ frame) {
                             shade_alpha(acc, v, stepf, lut, prm.lut);
                             stopped = !(acc.a < tau);
                         }
+                        L.q[0] += D[0], L.q[1] += D[1], L.q[2] += D[2];
+                    } else {
+                        adv = -adv;
+                        L.q[0] += D[0] * adv, L.q[1] += D[1] * adv, L.q[2] += D[2] * adv;
                     }
-                    L.q[0] += D[0], L.q[1] += D[1], L.q[2] += D[2];
-                    --n;
+                    n -= adv;
                     active = n > 0 && !stopped;
                 }
             }

@@ -395,6 +395,27 @@ __device__ __forceinline__ float trilinear(const float* __restrict__ brick, cons
     return lerp8(C, L);
 }
 
+/* R19: how many lattice steps (at least 1, at most n) can be taken from position L without leaving the
+ * 8x8x8 macro-cell it is in. An UNDER-estimate by construction (quotients rounded down from values scaled
+ * down by 2^-20), so every position stepped over lies inside the macro-cell; landing short only means
+ * another leap. 32.32 fixed point: a macro-cell spans 2^35 units per axis. */
+__device__ __forceinline__ int leap_steps(const Lattice& L, const long long D[3], int n) {
+    float t = (float)n;
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        const long long d = D[a];
+        if (d != 0) {
+            const long long lo = L.q[a] & ~((1ll << 35) - 1);
+            /* d > 0: positions j with q + j d < lo + 2^35 are inside: ceil(dist / d) of them; d < 0: floor((q - lo) / -d) + 1 */
+            const long long dist = d > 0 ? lo + (1ll << 35) - L.q[a] : L.q[a] - lo;
+            const float e = __fdividef(__ll2float_rz(dist), __ll2float_ru(d > 0 ? d : -d)) * 0.999999f;
+            t = fminf(t, d > 0 ? e : e + 1.0f);
+        }
+    }
+    const int j = (int)t; /* rounds toward zero */
+    return j < 1 ? 1 : j;
+}
+
 struct Accum {
     float r, g, b, a; /* ALPHA: premultiplied colour and opacity; MIP: r = running max */
 };
