@@ -182,7 +182,12 @@ int vr_set_culling(vr_volume* v, int enable);
  * high sides) - every voxel a sample based in m can interpolate between. Samples based in a transparent macro-cell
  * are not fetched: their opacity is exactly zero, so frames are bit-identical with culling on or
  * off. The per-cell ranges are computed once after an upload (one streaming pass, 8 bytes per 512
- * voxels of extra memory), the transparency bits once per transfer function. */
+ * voxels of extra memory), the transparency bits once per transfer function.
+ * VR_MIP frames use the same per-cell ranges where the cube has empty space (at least an eighth
+ * of the macro-cells hold nothing but the global minimum, e.g. the zero background of a density
+ * cube): a macro-cell whose maximum (plus a rounding margin) cannot raise the ray's running
+ * maximum is stepped over; frames stay bit-identical. That decision is taken once per upload by
+ * the first VR_MIP frame, which therefore waits once for an 8-byte read-back on its stream. */
 
 /* ------------------------------------------------------------------------------------------
  * One frame (rows a2..a9): per-view set-up (inverse of proj*view, rendering rectangle of each

@@ -46,6 +46,8 @@ struct vr_volume {
     unsigned* d_cell_bits;   /* 1 = macro-cell transparent under the current LUT */
     int nc[3], cell_words;   /* macro-cells per axis of a slot; words of d_cell_bits per brick */
     bool cell_mm_valid, cell_bits_valid;
+    bool mip_skip_known, mip_skip_useful; /* decided once per upload: does the cube have empty space (R19, MIP) */
+    unsigned long long* d_cell_count;
     bool tf_has_zero;        /* the LUT has a run of >= 3 zero-alpha entries: skipping can do something */
     bool culling;
     int traversal;           /* VR_SORT_LAST or VR_FUSED */
@@ -113,6 +115,7 @@ static void release(vr_volume* v) {
     cudaFree(v->d_mm);
     cudaFree(v->d_cell_mm);
     cudaFree(v->d_cell_bits);
+    cudaFree(v->d_cell_count);
     cudaFree(v->d_counts2);
     for (int r = 0; r < VR_EV_RING; ++r)
         for (int i = 0; i < 4; ++i)
@@ -315,6 +318,7 @@ extern "C" int vr_volume_upload(vr_volume* v, const float* src, int memspace, in
     v->has_data = true;
     v->mm_valid = false;
     v->cell_mm_valid = v->cell_bits_valid = false;
+    v->mip_skip_known = false;
     return VR_OK;
 }
 
@@ -485,7 +489,7 @@ static bool cells_supported(const vr_volume* v) {
            g.ml[2] == 0 && g.ghost >= 1;
 }
 
-static int ensure_cells(vr_volume* v, cudaStream_t st) {
+static int ensure_cells(vr_volume* v, bool want_bits, cudaStream_t st) {
     const VrGrid& g = v->grid;
     if (!v->d_cell_mm) {
         for (int a = 0; a < 3; ++a) v->nc[a] = (g.nt[a] * (1 << g.tl[a]) + 7) / 8;
@@ -500,11 +504,32 @@ static int ensure_cells(vr_volume* v, cudaStream_t st) {
         v->cell_mm_valid = true;
         v->cell_bits_valid = false;
     }
-    if (!v->cell_bits_valid) {
+    if (want_bits && !v->cell_bits_valid) {
         VR_CUDA(v, vr_launch_cell_flags(v->d_cell_mm, v->d_cell_bits, g.nbricks, v->nc, v->cell_words, v->lut, st));
         v->launches++;
         v->cell_bits_valid = true;
     }
+    return VR_OK;
+}
+
+/* MIP (R19): stepping over macro-cells that cannot raise a ray's maximum pays only if the cube has empty
+ * space - macro-cells that hold nothing but the global minimum (the zero background of a density cube).
+ * Decided once per upload (one pass over the cell table and one 8-byte read-back): at least an eighth. */
+static int decide_mip_skip(vr_volume* v, cudaStream_t st) {
+    if (v->mip_skip_known) return VR_OK;
+    int rc = ensure_minmax(v, st);
+    if (!rc) rc = ensure_cells(v, false, st);
+    if (rc) return rc;
+    if (!v->d_cell_count) VR_CUDA(v, cudaMalloc(&v->d_cell_count, sizeof(unsigned long long)));
+    const long long ncells = (long long)v->nc[0] * v->nc[1] * v->nc[2] * v->grid.nbricks;
+    unsigned long long empty = 0;
+    VR_CUDA(v, cudaMemsetAsync(v->d_cell_count, 0, sizeof(unsigned long long), st));
+    VR_CUDA(v, vr_launch_cell_count_empty(v->d_cell_mm, ncells, v->d_mm + v->grid.nbricks, v->d_cell_count, st));
+    v->launches++;
+    VR_CUDA(v, cudaMemcpyAsync(&empty, v->d_cell_count, sizeof(empty), cudaMemcpyDeviceToHost, st));
+    VR_CUDA(v, cudaStreamSynchronize(st));
+    v->mip_skip_useful = empty * 8ull >= (unsigned long long)ncells;
+    v->mip_skip_known = true;
     return VR_OK;
 }
 
@@ -557,7 +582,7 @@ extern "C" int vr_debug_cell_flags(vr_volume* v, int b, unsigned char* flags_out
     if (!dims || b < 0 || b >= v->grid.nbricks) return fail(v, VR_ERR_INVALID_ARG, "vr_debug_cell_flags: bad brick %d or NULL dims", b);
     if (!v->has_data || !v->has_tf) return fail(v, VR_ERR_STATE, "vr_debug_cell_flags: needs data and a transfer function");
     if (!cells_supported(v)) return fail(v, VR_ERR_STATE, "vr_debug_cell_flags: macro-cells need the 4x4x2 layout and ghost >= 1");
-    const int rc = ensure_cells(v, 0);
+    const int rc = ensure_cells(v, true, 0);
     if (rc) return rc;
     for (int a = 0; a < 3; ++a) dims[a] = v->nc[a];
     if (!flags_out) return VR_OK;
@@ -607,8 +632,14 @@ extern "C" int vr_render(vr_volume* v, const float* view, const float* proj, int
     /* after an upload or a new transfer function only, and only if the table has a transparent range */
     const bool skipping = v->culling && v->tf_has_zero && mode == VR_ALPHA && cells_supported(v);
     if (skipping) {
-        rc = ensure_cells(v, st);
+        rc = ensure_cells(v, true, st);
         if (rc) return rc;
+    }
+    bool mip_skipping = false;
+    if (v->culling && mode == VR_MIP && cells_supported(v)) {
+        rc = decide_mip_skip(v, st);
+        if (rc) return rc;
+        mip_skipping = v->mip_skip_useful;
     }
     if (timing) VR_CUDA(v, cudaEventRecord(ev[0], st));
     rc = run_setup(v, view, proj, width, height, mode, v->culling, st);
@@ -626,6 +657,7 @@ extern "C" int vr_render(vr_volume* v, const float* view, const float* proj, int
     p.sub = v->d_sub;
     p.bitmap = NULL;
     p.cell_bits = skipping ? v->d_cell_bits : NULL;
+    p.cell_mm = mip_skipping ? v->d_cell_mm : NULL;
     p.nc[0] = v->nc[0]; p.nc[1] = v->nc[1]; p.nc[2] = v->nc[2];
     p.cell_words = v->cell_words;
     if (v->counting == 2) {

@@ -123,7 +123,9 @@ vr_fused_kernel(const VrRaycastParams prm, float4* __restrict__ frame) {
             Corners C;
             int pcx = INT_MIN, pcy = 0, pcz = 0;
             /* R19: samples based in a transparent macro-cell are skipped (see vr_raycast.cu) */
-            const unsigned* __restrict__ cbits = SKIP ? prm.cell_bits + (long long)b * prm.cell_words : NULL;
+            const unsigned* __restrict__ cbits = (SKIP && MODE == VR_ALPHA) ? prm.cell_bits + (long long)b * prm.cell_words : NULL;
+            const float2* __restrict__ cmm = (SKIP && MODE == VR_MIP) ? prm.cell_mm + (long long)b * (prm.nc[0] * prm.nc[1] * prm.nc[2]) : NULL;
+            float pbound = INFINITY;
             int pm = -1;
             bool ptransp = false;
             while (__any_sync(FULL_MASK, active)) {
@@ -133,11 +135,22 @@ vr_fused_kernel(const VrRaycastParams prm, float4* __restrict__ frame) {
                     if (!VR_REUSE || cx != pcx || cy != pcy || cz != pcz) {
                         if (SKIP) {
                             const int m = ((cz >> 3) * prm.nc[1] + (cy >> 3)) * prm.nc[0] + (cx >> 3);
-                            if (m != pm) {
-                                pm = m;
-                                ptransp = (__ldg(cbits + (m >> 5)) >> (m & 31)) & 1u;
+                            if (MODE == VR_ALPHA) {
+                                if (m != pm) {
+                                    pm = m;
+                                    ptransp = (__ldg(cbits + (m >> 5)) >> (m & 31)) & 1u;
+                                }
+                            } else {
+                                /* MIP: no sample based in this macro-cell can exceed its maximum (plus a rounding margin of the
+                                 * float32 interpolation); if that cannot raise the ray's maximum, the cell is stepped over */
+                                if (m != pm) {
+                                    pm = m;
+                                    const float cmax = __ldg(&cmm[m].y);
+                                    pbound = cmax + fabsf(cmax) * 1e-6f;
+                                }
+                                ptransp = pbound <= acc.r;
                             }
-                            if (ptransp) adv = -leap_steps(L, D, n); /* negative: a leap over transparent samples, nothing fetched */
+                            if (ptransp) adv = -leap_steps(L, D, n); /* negative: a leap over samples that cannot matter, nothing fetched */
                         }
                         if (adv > 0) {
                             fetch8<LAY, 0, CLAMP, COUNT>(brick, g, ext, L, prm.bitmap, (long long)b * g.slot, C);
@@ -244,8 +257,8 @@ static cudaError_t launch_fused_mode(const VrRaycastParams& p, float* frame, lon
         return clamp ? launch_fused<MODE, LAY_LINEAR, true, COUNT>(p, frame, items, st)
                      : launch_fused<MODE, LAY_LINEAR, false, COUNT>(p, frame, items, st);
     if (t442) {
-        if (MODE == VR_ALPHA && !clamp && p.cell_bits) /* R19: macro-cell skipping */
-            return launch_fused<MODE, LAY_TILE442, false, COUNT, MODE == VR_ALPHA>(p, frame, items, st);
+        if (!clamp && (MODE == VR_ALPHA ? p.cell_bits != NULL : p.cell_mm != NULL)) /* R19: macro-cell skipping */
+            return launch_fused<MODE, LAY_TILE442, false, COUNT, true>(p, frame, items, st);
         return clamp ? launch_fused<MODE, LAY_TILE442, true, COUNT>(p, frame, items, st)
                      : launch_fused<MODE, LAY_TILE442, false, COUNT>(p, frame, items, st);
     }

@@ -120,6 +120,7 @@ struct VrRaycastParams {
     void* sub;          /* float4[] (ALPHA) or float[] (MIP) */
     unsigned* bitmap;   /* counting variant only: one bit per brick-store cell, or NULL */
     const unsigned* cell_bits; /* R19: one bit per 8x8x8 macro-cell, 1 = transparent under the LUT; NULL = no skipping */
+    const float2* cell_mm; /* R19, MIP: (min, max) per macro-cell (a cell whose max cannot raise the ray's maximum is skipped); NULL = off */
     int nc[3];          /* macro-cells per axis of a brick slot */
     int cell_words;     /* 32-bit words of cell_bits per brick */
     VrLut lut;
@@ -145,6 +146,9 @@ cudaError_t vr_launch_setup(const VrGrid& grid, const VrMatrices& mats, int W, i
 cudaError_t vr_launch_minmax(const VrGrid& grid, const float* bricks, int2* enc, float2* table, cudaStream_t st);
 /* macro-cells (R19): per-cell (min, max) of the 4x4x2-tiled store; transparency bits for a LUT */
 cudaError_t vr_launch_cell_minmax(const VrGrid& grid, const float* bricks, float2* cell_mm, const int nc[3], cudaStream_t st);
+/* *count += macro-cells of the whole store whose (min, max) is exactly (lo, lo): empty space of a density cube */
+cudaError_t vr_launch_cell_count_empty(const float2* cell_mm, long long ncells, const float2* global_mm, unsigned long long* count,
+                                       cudaStream_t st);
 cudaError_t vr_launch_cell_flags(const float2* cell_mm, unsigned* bits, int nbricks, const int nc[3], int words_per_brick,
                                  const VrLut& lut, cudaStream_t st);
 /* items = work items of the view (sizes the persistent grid); sparse = the view samples the store at

@@ -230,3 +230,22 @@ cudaError_t vr_launch_cell_flags(const float2* cell_mm, unsigned* bits, int nbri
     vr_cell_flags_kernel<<<(unsigned)blocks, 256, 0, st>>>(cell_mm, bits, nbricks, nc[0], nc[1], nc[2], words_per_brick, lut);
     return cudaGetLastError();
 }
+
+__global__ void __launch_bounds__(256)
+vr_cell_count_empty_kernel(const float2* __restrict__ cell_mm, long long ncells, const float2* __restrict__ global_mm,
+                           unsigned long long* __restrict__ count) {
+    const float lo = global_mm->x;
+    unsigned c = 0;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < ncells; i += (long long)gridDim.x * blockDim.x) {
+        const float2 r = cell_mm[i];
+        c += (r.x == lo && r.y == lo) ? 1u : 0u;
+    }
+    for (int o = 16; o > 0; o >>= 1) c += __shfl_xor_sync(0xffffffffu, c, o);
+    if ((threadIdx.x & 31) == 0 && c) atomicAdd(count, (unsigned long long)c);
+}
+
+cudaError_t vr_launch_cell_count_empty(const float2* cell_mm, long long ncells, const float2* global_mm, unsigned long long* count,
+                                       cudaStream_t st) {
+    vr_cell_count_empty_kernel<<<148 * 8, 256, 0, st>>>(cell_mm, ncells, global_mm, count);
+    return cudaGetLastError();
+}

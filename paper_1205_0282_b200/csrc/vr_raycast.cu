@@ -140,7 +140,9 @@ vr_raycast_kernel(const VrRaycastParams prm) {
         int pcx = INT_MIN, pcy = 0, pcz = 0;
         /* R19: samples based in a macro-cell the transfer function makes transparent are skipped (their
          * opacity is exactly 0): no voxel is fetched. The flag is looked up when the macro-cell changes. */
-        const unsigned* __restrict__ cbits = SKIP ? prm.cell_bits + (long long)b * prm.cell_words : NULL;
+        const unsigned* __restrict__ cbits = (SKIP && MODE == VR_ALPHA) ? prm.cell_bits + (long long)b * prm.cell_words : NULL;
+        const float2* __restrict__ cmm = (SKIP && MODE == VR_MIP) ? prm.cell_mm + (long long)b * (prm.nc[0] * prm.nc[1] * prm.nc[2]) : NULL;
+        float pbound = INFINITY;
         int pm = -1;
         bool ptransp = false;
         while (__any_sync(FULL_MASK, active)) {
@@ -150,11 +152,22 @@ vr_raycast_kernel(const VrRaycastParams prm) {
                 if (!VR_REUSE || cx != pcx || cy != pcy || cz != pcz) {
                     if (SKIP) {
                         const int m = ((cz >> 3) * prm.nc[1] + (cy >> 3)) * prm.nc[0] + (cx >> 3);
-                        if (m != pm) {
-                            pm = m;
-                            ptransp = (__ldg(cbits + (m >> 5)) >> (m & 31)) & 1u;
+                        if (MODE == VR_ALPHA) {
+                            if (m != pm) {
+                                pm = m;
+                                ptransp = (__ldg(cbits + (m >> 5)) >> (m & 31)) & 1u;
+                            }
+                        } else {
+                            /* MIP: no sample based in this macro-cell can exceed its maximum (plus a rounding margin of the
+                             * float32 interpolation); if that cannot raise the ray's maximum, the cell is stepped over */
+                            if (m != pm) {
+                                pm = m;
+                                const float cmax = __ldg(&cmm[m].y);
+                                pbound = cmax + fabsf(cmax) * 1e-6f;
+                            }
+                            ptransp = pbound <= acc.r;
                         }
-                        if (ptransp) adv = -leap_steps(L, D, n); /* negative: a leap over transparent samples, nothing fetched */
+                        if (ptransp) adv = -leap_steps(L, D, n); /* negative: a leap over samples that cannot matter, nothing fetched */
                     }
                     if (adv > 0) {
                         fetch8<LAY, PT, CLAMP, COUNT>(brick, g, ext, L, prm.bitmap, (long long)b * g.slot, C);
@@ -271,8 +284,9 @@ static cudaError_t launch_mode(const VrRaycastParams& p, long long ctas, bool sp
         }
     }
     if (is_tile442(p.grid)) {
-        if (MODE == VR_ALPHA && !clamp && p.cell_bits) /* R19: macro-cell skipping, the transfer function has a transparent range */
-            return launch_variant<MODE, LAY_TILE442, 0, false, COUNT, MODE == VR_ALPHA>(p, ctas, sparse, st);
+        /* R19: macro-cell skipping - ALPHA when the transfer function has a transparent range, MIP when the cube has empty space */
+        if (!clamp && (MODE == VR_ALPHA ? p.cell_bits != NULL : p.cell_mm != NULL))
+            return launch_variant<MODE, LAY_TILE442, 0, false, COUNT, true>(p, ctas, sparse, st);
         return clamp ? launch_variant<MODE, LAY_TILE442, 0, true, COUNT>(p, ctas, sparse, st)
                      : launch_variant<MODE, LAY_TILE442, 0, false, COUNT>(p, ctas, sparse, st);
     }

@@ -427,6 +427,47 @@ def test_macro_cell_skipping_is_exact(vr):
     assert abs(g.debug_stats()["samples"] - int(ref["counts"][..., 0].sum())) <= 1e-4 * ref["counts"][..., 0].sum()
 
 
+def test_mip_steps_over_empty_space_exactly(vr):
+    """R19 for MIP (the paper's shipped mode) on a density cube with a zero background: macro-cells
+    that cannot raise a ray's maximum are stepped over; frames bit-identical with the feature off,
+    equal to the oracle's, far fewer samples, in both traversals."""
+    nx, ny, nz, B = 128, 96, 80, 32
+    cube = synth.Cube(33, nx, ny, nz, 3, kind=synth.NBODY)
+    data = cube.fill_host()
+    assert (data == 0.0).mean() > 0.3
+    tf = synth.tf_density()
+    g = vr.Volume(nx, ny, nz, B, 1)
+    g.upload(data)
+    o = oracle.Volume(nx, ny, nz, B, 1, data=data)
+    for v in (g, o):
+        v.set_transfer_function(tf, 0.0, synth.NBODY_VMAX)
+    W, H = 192, 144
+    fr = synth.Framing(nx, ny, nz, W, H)
+    view, proj = fr.seeded(9, 0), fr.proj(False)
+    ref = o.render(view, proj, W, H, 0.5, oracle.MIP)
+    g.set_counting(1)
+    for trav in (vr.SORT_LAST, vr.FUSED):
+        g.set_traversal(trav)
+        g.set_culling(True)
+        on = gpu_frame(g, view, proj, W, H, 0.5, vr.MIP)
+        n_on = g.debug_stats()["samples"]
+        g.set_culling(False)
+        off = gpu_frame(g, view, proj, W, H, 0.5, vr.MIP)
+        n_off = g.debug_stats()["samples"]
+        assert np.array_equal(on, off) and n_on < 0.6 * n_off
+        assert n_off == int(ref["counts"][..., 0].sum())
+        check_mip(on, ref["image"], "MIP over empty space")
+    # a noise cube has no empty space: the feature stays off and every sample is taken
+    noise = synth.Cube(34, 64, 48, 40, 2)
+    gn, on_ = make_pair(noise, 16, 1)
+    gn.set_counting(1)
+    r2 = on_.render(view, proj, 64, 48, 0.5, oracle.MIP)
+    fr2 = synth.Framing(64, 48, 40, 64, 48)
+    r2 = on_.render(fr2.seeded(1, 0), fr2.proj(False), 64, 48, 0.5, oracle.MIP)
+    check_mip(gpu_frame(gn, fr2.seeded(1, 0), fr2.proj(False), 64, 48, 0.5, vr.MIP), r2["image"], "noise MIP")
+    assert gn.debug_stats()["samples"] == int(r2["counts"][..., 0].sum())
+
+
 # --------------------------------------------------------------------------- f2 fused traversal (R17)
 @pytest.mark.parametrize("tau", [0.99, 2.0])
 @pytest.mark.parametrize("ortho", [False, True])
