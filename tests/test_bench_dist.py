@@ -66,3 +66,36 @@ def test_workloads_match_baseline_configs():
         w = bench.workload(name)
         assert (w["nx"], w["ny"], w["nz"]) == dims and w["brick"] == brick and (w["width"], w["height"]) == wh
         assert w["step"] == step and len(w["views"]) == 36 and w["tau"] == 0.99 and w["ghost"] == 1
+
+
+def test_reference_arm_prints_the_contract_line():
+    """`bench.py --impl reference` (the oracle timed on the host cores, this tier's reference arm) on the
+    smallest workload: one JSON line with the base contract's keys, no GPU involved."""
+    import json
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    r = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--impl", "reference", "--workload", "c0", "--steps", "2",
+                        "--warmup", "1"], capture_output=True, text=True, timeout=600, cwd=root)
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [l for l in r.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1
+    j = json.loads(lines[0])
+    for key in ("metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better", "scaling", "vs_baseline",
+                "dtype", "data", "config", "e2e", "cpu_baseline", "impl"):
+        assert key in j, key
+    assert j["impl"] == "reference" and j["unit"] == "frames/s" and j["value"] > 0 and j["steps"] == 2
+    assert j["cpu_baseline"]["kind"] == "oracle" and j["cpu_baseline"]["cores"] >= 1
+    assert j["e2e"]["h2d_bytes_per_step"] == 0 and j["e2e"]["d2h_bytes_per_step"] == 0 and j["vs_baseline"] is None
+
+
+def test_product_arm_refuses_to_run_without_a_gpu():
+    """No CPU fallback: without a CUDA device the product arm exits loudly instead of measuring something else."""
+    import subprocess
+    import sys
+    if torch.cuda.is_available():
+        pytest.skip("a GPU is present")
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    r = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--workload", "c0", "--steps", "1"], capture_output=True,
+                       text=True, timeout=600, cwd=root)
+    assert r.returncode != 0 and "no CUDA device" in (r.stderr + r.stdout)
