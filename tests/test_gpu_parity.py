@@ -551,6 +551,76 @@ def test_fused_traversal_edge_cases(vr):
     assert np.array_equal(gpu_frame(g1, fr.turntable(3), fr.proj(False), W, H, 0.5, vr.ALPHA), a)
 
 
+# --------------------------------------------------------------------------- state across calls
+def test_handle_state_survives_a_session(vr):
+    """Two handles alive at once; frame sizes that grow and shrink (scratch regrown), a sub-box
+    re-upload in the middle (range tables invalidated), transfer-function, traversal and culling
+    switches, device, host and pipelined host frames interleaved: every frame equals the frame a
+    FRESH handle renders from the same state, bit for bit."""
+    import torch
+    ca, cb = synth.Cube(81, 72, 60, 48, 5), synth.Cube(82, 40, 56, 64, 3, kind=synth.NBODY)
+    da, db = ca.fill_host(), cb.fill_host()
+    ga, gb = vr.Volume(72, 60, 48, 16, 1), vr.Volume(40, 56, 64, 32, 1)
+    ga.upload(da)
+    gb.upload(db)
+    tfs = {"ramp": (synth.tf_ramp(), synth.TF_VMIN, synth.TF_VMAX), "thr": (synth.tf_threshold(), synth.TF_VMIN, synth.TF_VMAX),
+           "dens": (synth.tf_density(), 0.0, synth.NBODY_VMAX)}
+    ga.set_transfer_function(*tfs["ramp"])
+    gb.set_transfer_function(*tfs["dens"])
+    state = {"a": dict(data=da, dims=(72, 60, 48), brick=16, tf="ramp", trav=vr.SORT_LAST, cull=True),
+             "b": dict(data=db, dims=(40, 56, 64), brick=32, tf="dens", trav=vr.SORT_LAST, cull=True)}
+    handles = {"a": ga, "b": gb}
+
+    def fresh(which, W, H, k, mode):
+        st = state[which]
+        g = vr.Volume(*st["dims"], st["brick"], 1)
+        g.upload(st["data"])
+        g.set_transfer_function(*tfs[st["tf"]])
+        g.set_traversal(st["trav"])
+        g.set_culling(st["cull"])
+        fr = synth.Framing(*st["dims"], W, H)
+        return gpu_frame(g, fr.seeded(3, k), fr.proj(k % 2 == 1), W, H, 0.5, mode)
+
+    def frame(which, W, H, k, mode, how):
+        g, st = handles[which], state[which]
+        fr = synth.Framing(*st["dims"], W, H)
+        view, proj = fr.seeded(3, k), fr.proj(k % 2 == 1)
+        if how == "device":
+            return gpu_frame(g, view, proj, W, H, 0.5, mode)
+        if how == "host":
+            return g.render_host(view, proj, W, H, 0.5, mode).astype(np.float64)
+        buf = torch.empty((H, W, 4), dtype=torch.float32).pin_memory()
+        g.render_host_async(view, proj, W, H, 0.5, mode, buf)
+        g.render_host_wait()
+        return buf.numpy().astype(np.float64)
+
+    script = [("a", 96, 64, 0, vr.ALPHA, "device"), ("b", 160, 120, 1, vr.MIP, "async"), ("a", 200, 150, 2, vr.MIP, "host"),
+              ("tf", "a", "thr"), ("a", 64, 48, 3, vr.ALPHA, "async"), ("b", 80, 60, 4, vr.ALPHA, "device"),
+              ("trav", "a", vr.FUSED), ("a", 120, 90, 5, vr.ALPHA, "device"), ("upload", "a"), ("a", 120, 90, 6, vr.ALPHA, "host"),
+              ("cull", "b", False), ("b", 160, 120, 7, vr.MIP, "device"), ("trav", "a", vr.SORT_LAST), ("tf", "a", "ramp"),
+              ("a", 210, 130, 8, vr.ALPHA, "device"), ("cull", "b", True), ("trav", "b", vr.FUSED), ("b", 33, 17, 9, vr.ALPHA, "async"),
+              ("a", 96, 64, 10, vr.MIP, "device")]
+    for op in script:
+        if op[0] == "tf":
+            handles[op[1]].set_transfer_function(*tfs[op[2]])
+            state[op[1]]["tf"] = op[2]
+        elif op[0] == "trav":
+            handles[op[1]].set_traversal(op[2])
+            state[op[1]]["trav"] = op[2]
+        elif op[0] == "cull":
+            handles[op[1]].set_culling(op[2])
+            state[op[1]]["cull"] = op[2]
+        elif op[0] == "upload":   # overwrite a box that straddles brick seams with bright values
+            box = np.full((20, 22, 24), 7.0, dtype=np.float32)
+            handles[op[1]].upload(box, origin=(10, 12, 14))
+            d = state[op[1]]["data"].copy()
+            d[14:34, 12:34, 10:34] = box
+            state[op[1]]["data"] = d
+        else:
+            which, W, H, k, mode, how = op
+            assert np.array_equal(frame(which, W, H, k, mode, how), fresh(which, W, H, k, mode)), op
+
+
 # --------------------------------------------------------------------------- edge cases
 def test_edge_cases(vr):
     import torch
