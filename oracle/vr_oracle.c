@@ -32,7 +32,8 @@
  * owned once, rectangle conservativeness, step-halving convergence, brute force against an
  * independent numpy renderer; data range: planted extremes incl. ghost-only cells, brute
  * force; transparent bricks: their sub-images are exactly zero. Parity unpinned (pure conventions): R1 row orientation,
- * R11 MIP alpha, R13 form of the relative tolerance, R14 NaN handling (excluded).
+ * R11 MIP alpha, R13 form of the relative tolerance. R14 (NaN = blanked voxel: samples that
+ * touch one are dropped) is pinned by a closed form on a homogeneous cube with a blanked slab.
  *
  * Build: gcc -O2 -std=c11 -ffp-contract=off -fopenmp -shared -fPIC (oracle/build.py).
  */
@@ -553,6 +554,10 @@ static void render_pixel(vro_volume* v, const vro_view* vw, const int* order, in
             int64_t lo[3], hi[3];
             brick_core(v, b, lo, hi);
             double val = trilinear(v, b, lo, hi, p);
+            /* R14: blanked voxels are NaN (the usual convention of radio cubes). A sample whose 2x2x2
+             * neighbourhood holds a NaN interpolates to NaN (also with weight 0) and is dropped: it is not
+             * taken, adds nothing in ALPHA and cannot be the maximum in MIP. */
+            if (isnan(val)) continue;
             B->count++;
             ++taken;
             if (mode == VRO_MIP) {

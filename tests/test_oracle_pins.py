@@ -665,3 +665,37 @@ def test_auto_step_is_one_sample_per_major_axis_voxel():
         L = (c[1] - c[0]) if c is not None else 0.0
         a32 = float(np.float32(0.05))                # the table holds float32 opacities
         assert L > 5 and abs(img[j, i, 3] - (1.0 - (1.0 - a32) ** L)) < 1e-12
+
+
+# --------------------------------------------------------------------------- blanked voxels (R14)
+def test_nan_voxels_drop_the_samples_that_touch_them():
+    """Radio cubes blank voxels with NaN. A sample whose 2x2x2 neighbourhood holds a NaN is dropped.
+    Closed form: homogeneous cube, axis-aligned orthographic rays through voxel centres, step 1,
+    a blanked slab of T planes: the samples in the slab AND the one just in front of it (it reads
+    the slab's first plane with weight 0) vanish, opacity = 1 - (1-a)^(n - T - 1); MIP of a
+    ramp-in-z cube is the largest plane value that survives; the data range ignores NaN;
+    a fully blanked cube renders nothing."""
+    n, T, z0 = 20, 4, 9
+    view, proj = ortho_along_z(n, n, n)
+    data = np.full((n, n, n), 2.0, dtype=np.float32)
+    data[z0:z0 + T] = np.nan
+    vol = oracle.Volume(n, n, n, 8, 1, data=data)
+    vol.set_transfer_function(const_tf((0.2, 0.5, 0.9), 0.05), -3, 10)
+    vol.set_early_termination(2.0)
+    r = vol.render(view, proj, n, n, 1.0, oracle.ALPHA)
+    a32 = float(np.float32(0.05))
+    assert np.abs(r["image"][..., 3] - (1.0 - (1.0 - a32) ** (n - T - 1))).max() < 1e-12
+    assert np.all(r["counts"][..., 0] == n - T - 1) and np.all(r["counts"][..., 1] == n)
+    ramp = np.broadcast_to(np.arange(n, dtype=np.float32)[:, None, None], (n, n, n)).copy()
+    ramp[n - 3:] = np.nan                               # the three brightest planes are blanked
+    volr = oracle.Volume(n, n, n, 8, 1, data=ramp)
+    tf = synth.tf_ramp()
+    volr.set_transfer_function(tf, 0.0, float(n))
+    m = volr.render(view, proj, n, n, 1.0, oracle.MIP)["image"]
+    expect = (n - 5) / float(n)                         # plane n-4 sits next to the blank: its sample is dropped too
+    assert np.abs(m[..., 0] - expect).max() < 1e-6 and np.all(m[..., 3] == 1.0)
+    assert volr.brick_minmax(-1) == (np.float32(0.0), np.float32(n - 4))
+    blank = oracle.Volume(n, n, n, 8, 1, data=np.full((n, n, n), np.nan, dtype=np.float32))
+    blank.set_transfer_function(tf, 0.0, 1.0)
+    for mode in (oracle.ALPHA, oracle.MIP):
+        assert not blank.render(view, proj, n, n, 1.0, mode)["image"].any()
