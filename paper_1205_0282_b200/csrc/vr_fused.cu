@@ -159,7 +159,7 @@ vr_fused_kernel(const VrRaycastParams prm, float4* __restrict__ frame) {
                     }
                     if (adv > 0) {
                         const float v = lerp8(C, L);
-                        if (COUNT) ++nsamples;
+                        if (COUNT) nsamples += (v == v) ? 1 : 0; /* R14: a sample that touches a blanked (NaN) voxel is dropped */
                         if (MODE == VR_MIP) {
                             acc.r = fmaxf(acc.r, v);
                             stopped = acc.r >= mip_stop;
@@ -187,7 +187,7 @@ vr_fused_kernel(const VrRaycastParams prm, float4* __restrict__ frame) {
                         L.q[a] = to_fixed(p - ((double)(blo[a] - g.ghost) + 0.5));
                     }
                     const float v = trilinear<LAY, 0, CLAMP, COUNT>(brick, g, ext, L, prm.bitmap, (long long)b * g.slot);
-                    if (COUNT) ++nsamples;
+                    if (COUNT) nsamples += (v == v) ? 1 : 0;
                     if (MODE == VR_MIP) {
                         acc.r = fmaxf(acc.r, v);
                         stopped = acc.r >= mip_stop;

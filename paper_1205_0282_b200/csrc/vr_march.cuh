@@ -457,7 +457,9 @@ __device__ __forceinline__ void shade_alpha(Accum& acc, float v, float w, const 
     const float4 e = lds128<0>(a), dl = lds128<16>(a);
     const float cr = fmaf(f, dl.x, e.x), cg = fmaf(f, dl.y, e.y), cb = fmaf(f, dl.z, e.z), ca = fmaf(f, dl.w, e.w);
     const float alpha = 1.0f - ex2_approx(w * lg2_approx(1.0f - ca));
-    const float ta = (1.0f - acc.a) * alpha;
+    /* R14: a sample that touches a blanked (NaN) voxel is dropped. NaN classifies harmlessly (the
+     * saturation maps it to entry 0); its opacity is forced to 0. MIP needs nothing: fmaxf ignores NaN. */
+    const float ta = (v == v) ? (1.0f - acc.a) * alpha : 0.0f;
     acc.r = fmaf(ta, cr, acc.r);
     acc.g = fmaf(ta, cg, acc.g);
     acc.b = fmaf(ta, cb, acc.b);

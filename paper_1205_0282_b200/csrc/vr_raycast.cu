@@ -176,7 +176,7 @@ vr_raycast_kernel(const VrRaycastParams prm) {
                 }
                 if (adv > 0) {
                     const float v = lerp8(C, L);
-                    if (COUNT) ++nsamples;
+                    if (COUNT) nsamples += (v == v) ? 1 : 0; /* R14: a sample that touches a blanked (NaN) voxel is dropped */
                     if (MODE == VR_MIP) {
                         acc.r = fmaxf(acc.r, v);
                         stopped = acc.r >= mip_stop;
@@ -212,7 +212,7 @@ vr_raycast_kernel(const VrRaycastParams prm) {
                     L.q[a] = to_fixed(p - ((double)(blo[a] - g.ghost) + 0.5));
                 }
                 const float v = trilinear<LAY, PT, CLAMP, COUNT>(brick, g, ext, L, prm.bitmap, (long long)b * g.slot);
-                if (COUNT) ++nsamples;
+                if (COUNT) nsamples += (v == v) ? 1 : 0;
                 if (MODE == VR_MIP) {
                     acc.r = fmaxf(acc.r, v);
                     stopped = acc.r >= mip_stop;

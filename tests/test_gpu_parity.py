@@ -551,6 +551,57 @@ def test_fused_traversal_edge_cases(vr):
     assert np.array_equal(gpu_frame(g1, fr.turntable(3), fr.proj(False), W, H, 0.5, vr.ALPHA), a)
 
 
+# --------------------------------------------------------------------------- blanked voxels (R14)
+def test_nan_voxels_are_blanked(vr):
+    """NaN voxels (blanked channels, masked edges: the usual state of a radio cube) drop exactly the
+    samples that touch them on both sides: parity in both modes and traversals, with the exact
+    sample count; the data range ignores them; culling and macro-cell skipping stay exact."""
+    nx, ny, nz, B = 90, 70, 52, 16
+    data = synth.Cube(91, nx, ny, nz, 8).fill_host()
+    data[:, :, :5] = np.nan                       # a masked edge
+    data[20:23] = np.nan                          # three blanked channels (across every brick column)
+    data[30:47, 10:35, 40:70] = np.nan            # a masked box straddling brick seams
+    rng = np.random.default_rng(5)
+    data[rng.random(data.shape) < 0.002] = np.nan  # isolated bad voxels
+    g = vr.Volume(nx, ny, nz, B, 1)
+    g.upload(data)
+    o = oracle.Volume(nx, ny, nz, B, 1, data=data)
+    one = oracle.Volume(nx, ny, nz, 128, 1, data=data)
+    assert g.minmax() == o.brick_minmax(-1) == (np.nanmin(data), np.nanmax(data))
+    mm = g.debug_brick_minmax()
+    for b in range(0, g.nbricks, 7):
+        assert tuple(mm[b]) == o.brick_minmax(b)
+    W, H = 180, 140
+    fr = synth.Framing(nx, ny, nz, W, H)
+    view, proj = fr.seeded(12, 0), fr.proj(False)
+    g.set_counting(1)
+    for tf_name, tf in (("translucent", synth.tf_translucent()), ("threshold", synth.tf_threshold())):
+        for v in (g, o, one):
+            v.set_transfer_function(tf, synth.TF_VMIN, synth.TF_VMAX)
+            v.set_early_termination(2.0)          # no early termination: sample counts are exact
+        for trav, orc in ((vr.SORT_LAST, o), (vr.FUSED, one)):
+            g.set_traversal(trav)
+            g.set_culling(False)
+            ref = orc.render(view, proj, W, H, 0.5, oracle.ALPHA)
+            img = gpu_frame(g, view, proj, W, H, 0.5, vr.ALPHA)
+            assert np.isfinite(img).all()
+            check_alpha(img, ref["image"], ref["flags"], 2.0, "NaN " + tf_name)
+            assert g.debug_stats()["samples"] == int(ref["counts"][..., 0].sum())
+            g.set_culling(True)
+            assert np.array_equal(gpu_frame(g, view, proj, W, H, 0.5, vr.ALPHA), img)
+            refm = orc.render(view, proj, W, H, 0.5, oracle.MIP)
+            imgm = gpu_frame(g, view, proj, W, H, 0.5, vr.MIP)
+            check_mip(imgm, refm["image"], "NaN MIP")
+            assert g.debug_stats()["samples"] == int(refm["counts"][..., 0].sum())
+    # a fully blanked volume renders nothing
+    gb = vr.Volume(24, 24, 24, 16, 1)
+    gb.upload(np.full((24, 24, 24), np.nan, dtype=np.float32))
+    gb.set_transfer_function(synth.tf_ramp(), synth.TF_VMIN, synth.TF_VMAX)
+    f2 = synth.Framing(24, 24, 24, 48, 48)
+    for mode in (vr.ALPHA, vr.MIP):
+        assert not gpu_frame(gb, f2.seeded(1, 0), f2.proj(False), 48, 48, 0.5, mode).any()
+
+
 # --------------------------------------------------------------------------- state across calls
 def test_handle_state_survives_a_session(vr):
     """Two handles alive at once; frame sizes that grow and shrink (scratch regrown), a sub-box
