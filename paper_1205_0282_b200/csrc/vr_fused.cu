@@ -66,12 +66,13 @@ vr_fused_kernel(const VrRaycastParams prm, float4* __restrict__ frame) {
         ray.K = 0;
         ray.step = step;
         if (in_frame) ray_setup(s_minv, W, H, pi, pj, g, step, ray);
-        const float stepf = (float)ray.step; /* path length a lattice sample stands for */
+        float stepf = (float)ray.step; /* path length a lattice sample stands for */
+        asm volatile("" : "+f"(stepf)); /* one register: not re-converted from the double in every loop trip */
 
         Accum acc;
         acc.r = (MODE == VR_MIP) ? -INFINITY : 0.0f;
         acc.g = acc.b = acc.a = 0.0f;
-        bool stopped = (MODE == VR_ALPHA) ? !(acc.a < tau) : false;
+        int stopped = (MODE == VR_ALPHA) ? !(acc.a < tau) : 0; /* int, not bool: no byte packing in the loop control */
         int k = 0; /* next sample of the ray's schedule */
 
         /* one trip per brick the ray crosses */
@@ -119,7 +120,7 @@ vr_fused_kernel(const VrRaycastParams prm, float4* __restrict__ frame) {
                 L.q[0] = L.q[1] = L.q[2] = 0;
                 D[0] = D[1] = D[2] = 0;
             }
-            bool active = n > 0 && !stopped;
+            int active = n > 0 && !stopped;
             Corners C;
             int pcx = INT_MIN, pcy = 0, pcz = 0;
             /* R19: samples based in a transparent macro-cell are skipped (see vr_raycast.cu) */

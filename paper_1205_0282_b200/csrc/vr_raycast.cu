@@ -117,7 +117,8 @@ vr_raycast_kernel(const VrRaycastParams prm) {
         acc.g = acc.b = acc.a = 0.0f;
         Lattice L;
         long long D[3];
-        const float stepf = (float)ray.step; /* path length a lattice sample stands for */
+        float stepf = (float)ray.step; /* path length a lattice sample stands for */
+        asm volatile("" : "+f"(stepf)); /* one register: not re-converted from the double in every loop trip */
         if (n > 0) {
             double s, w;
             sample_sw(ray, k_lo, s, w);
@@ -131,8 +132,8 @@ vr_raycast_kernel(const VrRaycastParams prm) {
             L.q[0] = L.q[1] = L.q[2] = 0;
             D[0] = D[1] = D[2] = 0;
         }
-        bool stopped = (MODE == VR_ALPHA) ? !(acc.a < tau) : false;
-        bool active = n > 0 && !stopped;
+        int stopped = (MODE == VR_ALPHA) ? !(acc.a < tau) : 0; /* int, not bool: no byte packing in the loop control */
+        int active = n > 0 && !stopped;
         /* With step < 1 consecutive samples of a ray often fall into the same cell: the 8
          * voxels stay in registers and only the weights change (fewer L1 wavefronts, the
          * bound of densely sampled views). */
