@@ -179,11 +179,12 @@ int vr_volume_minmax(vr_volume* v, float* vmin_out, float* vmax_out, void* strea
  * contributes exact zeros, so the frame is bit-identical with culling on or off. */
 int vr_set_culling(vr_volume* v, int enable);
 /* With culling on, VR_ALPHA frames also skip transparent space INSIDE bricks (R19; 4x4x2 layout,
- * ghost >= 1, and only when the transfer function has an entry with alpha == 0). The padded
+ * ghost >= 1, and only when the transfer function has at least three consecutive entries with
+ * alpha == 0 - fewer can never satisfy R16's rule, e.g. the lone zero of a linear ramp). The padded
  * cells of a brick are cut into 8x8x8 macro-cells; macro-cell m is transparent iff R16's rule
  * holds for the (min, max) of cells 8m .. 8m+8 per axis (the macro-cell plus one layer on its
- * high sides) - every voxel a sample based in m can interpolate between. Samples based in a transparent macro-cell
- * are not fetched: their opacity is exactly zero, so frames are bit-identical with culling on or
+ * high sides) - every voxel a sample based in m can interpolate between. Samples based in a
+ * transparent macro-cell are not fetched (a lane leaps to the macro-cell's exit): their opacity is exactly zero, so frames are bit-identical with culling on or
  * off. The per-cell ranges are computed once after an upload (one streaming pass, 8 bytes per 512
  * voxels of extra memory), the transparency bits once per transfer function.
  * VR_MIP frames use the same per-cell ranges where the cube has empty space (at least an eighth
