@@ -670,10 +670,13 @@ def main():
         # (row f2: one ray through all bricks, global early termination, no sub-images, no compositing)
         for vmode, vtf, vtrav in (("alpha", "translucent", "sort_last"), ("mip", "ramp", "sort_last"),
                                   ("alpha", "ramp", "fused"), ("alpha", "translucent", "fused"),
-                                  ("alpha", "threshold", "sort_last"), ("alpha", "threshold", "fused")):
+                                  ("alpha", "threshold", "sort_last"), ("alpha", "threshold", "fused"),
+                                  ("alpha", "ramp, early termination off", "sort_last")):
             if vtrav == "sort_last" and vmode == args.mode and vtf == args.tf:
                 vtf = "ramp"
-            g.set_transfer_function(pick_tf(wl, vtf), *tf_range(wl))
+            noert = vtf.endswith("early termination off")  # the paper's protocol: with and without
+            g.set_transfer_function(pick_tf(wl, "ramp" if noert else vtf), *tf_range(wl))
+            g.set_early_termination(2.0 if noert else wl["tau"])
             g.set_traversal(vr.FUSED if vtrav == "fused" else vr.SORT_LAST)
             v = measure(0 if vmode == "alpha" else 1, False, None)
             extra = {}
@@ -683,6 +686,7 @@ def main():
                 g.set_culling(True)
                 extra = {"frames_per_s_skipping_off": round(K / (ms_off * 1e-3), 3)}
             g.set_traversal(vr.SORT_LAST)
+            g.set_early_termination(wl["tau"])
             variants.append({"mode": vmode, "tf": vtf, "traversal": vtrav, "frames_per_s": round(K / (v["ms"] * 1e-3), 3), **extra,
                              "gsamples_per_s": round(v["samples"] / (v["ms"] * 1e-3) / 1e9, 3),
                              "samples_per_frame": int(v["samples"] / K),
