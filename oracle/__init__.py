@@ -12,7 +12,7 @@ import numpy as np
 from . import build as _build
 
 ALPHA, MIP = 0, 1
-FLAG_ERT_MARGIN, FLAG_OWNER_MARGIN, FLAG_LAST_SAMPLE, FLAG_GRAZING = 1, 2, 4, 8
+FLAG_ERT_MARGIN, FLAG_OWNER_MARGIN, FLAG_LAST_SAMPLE, FLAG_GRAZING, FLAG_NAN_MARGIN = 1, 2, 4, 8, 16
 
 _lib = None
 

@@ -32,8 +32,9 @@
  * owned once, rectangle conservativeness, step-halving convergence, brute force against an
  * independent numpy renderer; data range: planted extremes incl. ghost-only cells, brute
  * force; transparent bricks: their sub-images are exactly zero. Parity unpinned (pure conventions): R1 row orientation,
- * R11 MIP alpha, R13 form of the relative tolerance. R14 (NaN = blanked voxel: samples that
- * touch one are dropped) is pinned by a closed form on a homogeneous cube with a blanked slab.
+ * R11 MIP alpha, R13 form of the relative tolerance. R14 (NaN = blanked voxel: a sample with
+ * more than 1e-4 of its weight on NaN voxels is dropped, else the NaN corners are left out) is
+ * pinned by closed forms on a homogeneous cube with a blanked slab.
  *
  * Build: gcc -O2 -std=c11 -ffp-contract=off -fopenmp -shared -fPIC (oracle/build.py).
  */
@@ -49,6 +50,8 @@
 #define VRO_FLAG_OWNER_MARGIN 2 /* an owner decision within 1e-6 voxel, brick ERT'ed   (R12) */
 #define VRO_FLAG_LAST_SAMPLE 4  /* MIP: existence of the last sample is marginal       (R12) */
 #define VRO_FLAG_GRAZING 8      /* hit/miss of the volume decided by < 1e-9 voxel      (R10) */
+#define VRO_FLAG_NAN_MARGIN 16  /* a sample's NaN weight within a factor 2 of the limit (R14) */
+#define VRO_NAN_WEIGHT 1e-4     /* R14: tri-linear weight on NaN corners above which a sample is dropped */
 
 typedef float (*vro_voxel_fn)(const void* ctx, int64_t x, int64_t y, int64_t z);
 
@@ -248,7 +251,7 @@ static double brick_voxel(vro_volume* v, int b, const int64_t lo[3], const int64
 }
 
 /* R3: voxel (i,j,k) is centred at (i+1/2, j+1/2, k+1/2); tri-linear interpolation. */
-static double trilinear(vro_volume* v, int b, const int64_t lo[3], const int64_t hi[3], const double p[3]) {
+static double trilinear(vro_volume* v, int b, const int64_t lo[3], const int64_t hi[3], const double p[3], double* nan_weight) {
     int64_t i0[3];
     double f[3];
     for (int a = 0; a < 3; ++a) {
@@ -267,7 +270,25 @@ static double trilinear(vro_volume* v, int b, const int64_t lo[3], const int64_t
     double c11 = c[1][1][0] + f[0] * (c[1][1][1] - c[1][1][0]);
     double c0 = c00 + f[1] * (c01 - c00);
     double c1 = c10 + f[1] * (c11 - c10);
-    return c0 + f[2] * (c1 - c0);
+    double val = c0 + f[2] * (c1 - c0);
+    if (nan_weight) *nan_weight = 0.0;
+    if (isnan(val)) {
+        /* R14: blanked (NaN) voxels. N = the tri-linear weight that falls on NaN corners. N > 1e-4: the
+         * sample is dropped (NaN returned). Otherwise the NaN corners are left out and the rest
+         * renormalised: val = sum over valid corners of w_i v_i / (1 - N) - continuous where a sample sits
+         * on a cell boundary and a NaN neighbour has weight 0 (the paper's per-ray step puts whole rays there). */
+        double N = 0.0, acc = 0.0;
+        for (int dz = 0; dz < 2; ++dz)
+            for (int dy = 0; dy < 2; ++dy)
+                for (int dx = 0; dx < 2; ++dx) {
+                    double w = (dx ? f[0] : 1.0 - f[0]) * (dy ? f[1] : 1.0 - f[1]) * (dz ? f[2] : 1.0 - f[2]);
+                    if (isnan(c[dz][dy][dx])) N += w;
+                    else acc += w * c[dz][dy][dx];
+                }
+        if (nan_weight) *nan_weight = N;
+        val = (N > VRO_NAN_WEIGHT) ? NAN : acc / (1.0 - N);
+    }
+    return val;
 }
 
 /* ------------------------------------------------------------------ view (R1, R2, R9) */
@@ -553,10 +574,12 @@ static void render_pixel(vro_volume* v, const vro_view* vw, const int* order, in
             /* step 5: value from the brick's own padded copy (R3) */
             int64_t lo[3], hi[3];
             brick_core(v, b, lo, hi);
-            double val = trilinear(v, b, lo, hi, p);
-            /* R14: blanked voxels are NaN (the usual convention of radio cubes). A sample whose 2x2x2
-             * neighbourhood holds a NaN interpolates to NaN (also with weight 0) and is dropped: it is not
-             * taken, adds nothing in ALPHA and cannot be the maximum in MIP. */
+            double nanw;
+            double val = trilinear(v, b, lo, hi, p, &nanw);
+            /* R14: blanked voxels are NaN (the usual convention of radio cubes). A sample with more than
+             * 1e-4 of its tri-linear weight on NaN voxels is dropped: it is not taken, adds nothing in
+             * ALPHA and cannot be the maximum in MIP. */
+            if (nanw > 0.5 * VRO_NAN_WEIGHT && nanw < 2.0 * VRO_NAN_WEIGHT) fl |= VRO_FLAG_NAN_MARGIN;
             if (isnan(val)) continue;
             B->count++;
             ++taken;

@@ -602,6 +602,59 @@ def test_nan_voxels_are_blanked(vr):
         assert not gpu_frame(gb, f2.seeded(1, 0), f2.proj(False), 48, 48, 0.5, mode).any()
 
 
+# --------------------------------------------------------------------------- randomised configurations
+@pytest.mark.parametrize("case", range(int(__import__("os").environ.get("VR_RANDOM_CASES", "16"))))
+def test_randomised_configurations(vr, case):
+    """Seeded random volumes, bricks, ghosts, steps (incl. the per-ray step), cameras (incl. eyes
+    inside the volume), transfer functions, data kinds and blanked voxels, both modes and both
+    traversals, culling on: parity with the oracle every time."""
+    rng = np.random.default_rng(1000 + case)
+    nx, ny, nz = (int(v) for v in rng.integers(18, 75, 3))
+    brick = int(rng.choice([8, 12, 16, 20, 32, 64]))
+    ghost = int(rng.choice([1, 1, 2]))
+    kind = int(rng.choice([0, 0, 1]))
+    cube = synth.Cube(500 + case, nx, ny, nz, int(rng.integers(1, 8)), kind=kind)
+    data = cube.fill_host()
+    if rng.random() < 0.4:
+        data[rng.random(data.shape) < 0.01] = np.nan
+        a, b = sorted(int(v) for v in rng.integers(0, nz, 2))
+        data[a:b + 1, : ny // 3] = np.nan
+    if kind == 1:
+        tf, lo, hi = synth.tf_density(), 0.0, synth.NBODY_VMAX
+    else:
+        tf = [synth.tf_ramp, synth.tf_translucent, synth.tf_threshold][int(rng.integers(0, 3))]()
+        lo, hi = synth.TF_VMIN, synth.TF_VMAX
+    tau = float(rng.choice([0.99, 0.9, 2.0]))
+    step = float(rng.choice([0.0, 0.37, 0.5, 1.0, 1.63]))
+    W, H = int(rng.integers(40, 130)), int(rng.integers(30, 100))
+    fr = synth.Framing(nx, ny, nz, W, H)
+    if rng.random() < 0.25:   # an eye inside the volume, looking at a random corner
+        eye = (nx * rng.uniform(0.2, 0.8), ny * rng.uniform(0.2, 0.8), nz * rng.uniform(0.2, 0.8))
+        corner = (nx * float(rng.integers(0, 2)), ny * float(rng.integers(0, 2)), nz * float(rng.integers(0, 2)))
+        view, proj = synth.look_at(eye, corner, (0.0, 0.3, 1.0)), synth.perspective(60, W / H, 0.3, 400.0)
+    else:
+        view, proj = fr.seeded(700 + case, case), fr.proj(bool(rng.integers(0, 2)))
+    g = vr.Volume(nx, ny, nz, brick, ghost)
+    g.upload(data)
+    o = oracle.Volume(nx, ny, nz, brick, ghost, data=data)
+    one = oracle.Volume(nx, ny, nz, 128, 1, data=data)
+    for v in (g, o, one):
+        v.set_transfer_function(tf, lo, hi)
+        v.set_early_termination(tau)
+    assert np.array_equal(g.debug_brick_order(view, proj), o.brick_order(view, proj))
+    for trav, orc in ((vr.SORT_LAST, o), (vr.FUSED, one)):
+        g.set_traversal(trav)
+        ref = orc.render(view, proj, W, H, step, oracle.ALPHA)
+        check_alpha(gpu_frame(g, view, proj, W, H, step if step > 0 else vr.STEP_AUTO, vr.ALPHA), ref["image"], ref["flags"],
+                    tau, "case %d" % case)
+        refm = orc.render(view, proj, W, H, step, oracle.MIP)
+        got = gpu_frame(g, view, proj, W, H, step if step > 0 else vr.STEP_AUTO, vr.MIP)
+        lastm = (refm["flags"] & oracle.FLAG_LAST_SAMPLE) != 0     # R12: the marginal last sample may or may not exist in float
+        tol = MIP_TOL = 1e-5 * np.maximum(np.abs(got), np.abs(refm["image"])) + 1e-7
+        bad = (np.abs(got - refm["image"]) > tol).any(axis=-1) & ~lastm
+        assert not bad.any(), "case %d MIP: %d pixels off" % (case, int(bad.sum()))
+
+
 # --------------------------------------------------------------------------- state across calls
 def test_handle_state_survives_a_session(vr):
     """Two handles alive at once; frame sizes that grow and shrink (scratch regrown), a sub-box

@@ -668,32 +668,51 @@ def test_auto_step_is_one_sample_per_major_axis_voxel():
 
 
 # --------------------------------------------------------------------------- blanked voxels (R14)
-def test_nan_voxels_drop_the_samples_that_touch_them():
-    """Radio cubes blank voxels with NaN. A sample whose 2x2x2 neighbourhood holds a NaN is dropped.
-    Closed form: homogeneous cube, axis-aligned orthographic rays through voxel centres, step 1,
-    a blanked slab of T planes: the samples in the slab AND the one just in front of it (it reads
-    the slab's first plane with weight 0) vanish, opacity = 1 - (1-a)^(n - T - 1); MIP of a
-    ramp-in-z cube is the largest plane value that survives; the data range ignores NaN;
-    a fully blanked cube renders nothing."""
+def test_nan_voxels_drop_the_samples_that_rest_on_them():
+    """Radio cubes blank voxels with NaN. R14: a sample with more than 1e-4 of its tri-linear
+    weight on NaN voxels is dropped; otherwise the NaN corners are left out and the others
+    renormalised (so a NaN neighbour with weight 0 changes nothing - where the paper's per-ray
+    step puts whole rays). Closed forms: homogeneous cube, axis-aligned orthographic rays, step 1.
+    (i) rays through voxel centres, a blanked slab of T planes: exactly the T samples in the slab
+    vanish, opacity = 1 - (1-a)^(n - T); (ii) rays at quarter-voxel offsets, a blanked plane
+    x = m: the rays with |x - (m + 1/2)| < 1 lose every sample, the others none; (iii) MIP of a
+    z-ramp with its brightest planes blanked is the brightest surviving plane; the data range
+    ignores NaN; a fully blanked cube renders nothing."""
     n, T, z0 = 20, 4, 9
     view, proj = ortho_along_z(n, n, n)
+    a32 = float(np.float32(0.05))
     data = np.full((n, n, n), 2.0, dtype=np.float32)
     data[z0:z0 + T] = np.nan
     vol = oracle.Volume(n, n, n, 8, 1, data=data)
     vol.set_transfer_function(const_tf((0.2, 0.5, 0.9), 0.05), -3, 10)
     vol.set_early_termination(2.0)
     r = vol.render(view, proj, n, n, 1.0, oracle.ALPHA)
-    a32 = float(np.float32(0.05))
-    assert np.abs(r["image"][..., 3] - (1.0 - (1.0 - a32) ** (n - T - 1))).max() < 1e-12
-    assert np.all(r["counts"][..., 0] == n - T - 1) and np.all(r["counts"][..., 1] == n)
+    assert np.abs(r["image"][..., 3] - (1.0 - (1.0 - a32) ** (n - T))).max() < 1e-12
+    assert np.all(r["counts"][..., 0] == n - T) and np.all(r["counts"][..., 1] == n)
+    assert not (r["flags"] & oracle.FLAG_NAN_MARGIN).any()
+    # (ii) a blanked plane x = m seen at two pixels per voxel
+    m = 7
+    data2 = np.full((n, n, n), 2.0, dtype=np.float32)
+    data2[:, :, m] = np.nan
+    vol2 = oracle.Volume(n, n, n, 8, 1, data=data2)
+    vol2.set_transfer_function(const_tf((0.2, 0.5, 0.9), 0.05), -3, 10)
+    vol2.set_early_termination(2.0)
+    r2 = vol2.render(view, proj, 2 * n, n, 1.0, oracle.ALPHA)
+    taken = r2["counts"][0, :, 0]
+    xs = (np.arange(2 * n) + 0.5) / 2.0                       # pixel centres in voxel units (either orientation:
+    hit = np.abs(xs - (m + 0.5)) < 1.0                        # the test cube is symmetric under x -> n - x only if
+    hit_m = np.abs((n - xs) - (m + 0.5)) < 1.0                # mirrored, so accept the view's handedness)
+    assert (np.array_equal(taken == 0, hit) or np.array_equal(taken == 0, hit_m)) and set(np.unique(taken)) == {0, n}
+    full = 1.0 - (1.0 - a32) ** n
+    assert np.abs(r2["image"][0, taken == n, 3] - full).max() < 1e-12 and not r2["image"][0, taken == 0].any()
+    # (iii)
     ramp = np.broadcast_to(np.arange(n, dtype=np.float32)[:, None, None], (n, n, n)).copy()
-    ramp[n - 3:] = np.nan                               # the three brightest planes are blanked
+    ramp[n - 3:] = np.nan
     volr = oracle.Volume(n, n, n, 8, 1, data=ramp)
     tf = synth.tf_ramp()
     volr.set_transfer_function(tf, 0.0, float(n))
-    m = volr.render(view, proj, n, n, 1.0, oracle.MIP)["image"]
-    expect = (n - 5) / float(n)                         # plane n-4 sits next to the blank: its sample is dropped too
-    assert np.abs(m[..., 0] - expect).max() < 1e-6 and np.all(m[..., 3] == 1.0)
+    mimg = volr.render(view, proj, n, n, 1.0, oracle.MIP)["image"]
+    assert np.abs(mimg[..., 0] - (n - 4) / float(n)).max() < 1e-6 and np.all(mimg[..., 3] == 1.0)
     assert volr.brick_minmax(-1) == (np.float32(0.0), np.float32(n - 4))
     blank = oracle.Volume(n, n, n, 8, 1, data=np.full((n, n, n), np.nan, dtype=np.float32))
     blank.set_transfer_function(tf, 0.0, 1.0)
