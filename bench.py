@@ -314,7 +314,7 @@ def roofline_of(counts, stages, stage_views, peak_gbs, peak_src, traffic=None):
 # SASS instructions of one trip of the ray-cast kernel's sample loop (4x4x2 layout, timed instance;
 # counted with `cuobjdump -sass` between the loop head and the backward branch after VOTE.ANY:
 # DESIGN.md "Kernels" lists them by kind). One trip = one sample for each of the warp's 32 rays.
-LOOP_INSTRUCTIONS = {"alpha": 123, "mip": 97}
+LOOP_INSTRUCTIONS = {"alpha": 128, "mip": 102}
 SM_COUNT, SCHEDULERS_PER_SM = 148, 4
 
 

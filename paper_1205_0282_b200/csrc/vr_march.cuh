@@ -387,12 +387,37 @@ __device__ __forceinline__ float lerp8(const Corners& C, const Lattice& L) {
     return fmaf(fz, c1 - c0, c0);
 }
 
+/* R14, the rare path: lerp8 gave NaN, i.e. some of the 8 voxels are blanked. N = tri-linear weight on the
+ * NaN corners; N > 1e-4: the sample is dropped (NaN stays); otherwise the NaN corners are left out and the
+ * others renormalised - continuous where a sample sits on a cell boundary next to a blanked voxel. */
+static __device__ __forceinline__ float lerp8_blanked_values(float c0, float c1, float c2, float c3, float c4, float c5, float c6,
+                                                         float c7, float fx, float fy, float fz) {
+    const float c[8] = {c0, c1, c2, c3, c4, c5, c6, c7};
+    float N = 0.0f, acc = 0.0f;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+        const float w = ((i & 1) ? fx : 1.0f - fx) * ((i & 2) ? fy : 1.0f - fy) * ((i & 4) ? fz : 1.0f - fz);
+        if (c[i] != c[i]) N += w;
+        else acc = fmaf(w, c[i], acc);
+    }
+    return N > 1e-4f ? __int_as_float(0x7fc00000) : acc / (1.0f - N);
+}
+/* everything by value, in registers: a by-reference call would keep the lattice and the voxels in local memory */
+__device__ __forceinline__ float lerp8_blanked(const Corners& C, const Lattice& L) {
+    const float fx = __uint_as_float(0x3F800000u | ((unsigned)L.q[0] >> 9)) - 1.0f;
+    const float fy = __uint_as_float(0x3F800000u | ((unsigned)L.q[1] >> 9)) - 1.0f;
+    const float fz = __uint_as_float(0x3F800000u | ((unsigned)L.q[2] >> 9)) - 1.0f;
+    return lerp8_blanked_values(C.c000, C.c001, C.c010, C.c011, C.c100, C.c101, C.c110, C.c111, fx, fy, fz);
+}
+
 template <int LAY, int PT, bool CLAMP, bool COUNT>
 __device__ __forceinline__ float trilinear(const float* __restrict__ brick, const VrGrid& g, const int ext[3], const Lattice& L,
                                            unsigned* __restrict__ bitmap, long long brick_cell0) {
     Corners C;
     fetch8<LAY, PT, CLAMP, COUNT>(brick, g, ext, L, bitmap, brick_cell0, C);
-    return lerp8(C, L);
+    float v = lerp8(C, L);
+    if (v != v) v = lerp8_blanked(C, L); /* R14 */
+    return v;
 }
 
 /* R19: how many lattice steps (at least 1, at most n) can be taken from position L without leaving the
@@ -457,8 +482,8 @@ __device__ __forceinline__ void shade_alpha(Accum& acc, float v, float w, const 
     const float4 e = lds128<0>(a), dl = lds128<16>(a);
     const float cr = fmaf(f, dl.x, e.x), cg = fmaf(f, dl.y, e.y), cb = fmaf(f, dl.z, e.z), ca = fmaf(f, dl.w, e.w);
     const float alpha = 1.0f - ex2_approx(w * lg2_approx(1.0f - ca));
-    /* R14: a sample that touches a blanked (NaN) voxel is dropped. NaN classifies harmlessly (the
-     * saturation maps it to entry 0); its opacity is forced to 0. MIP needs nothing: fmaxf ignores NaN. */
+    /* R14: a dropped sample arrives as NaN. It classifies harmlessly (the saturation maps it to entry 0);
+     * its opacity is forced to 0. MIP needs nothing: fmaxf ignores NaN. */
     const float ta = (v == v) ? (1.0f - acc.a) * alpha : 0.0f;
     acc.r = fmaf(ta, cr, acc.r);
     acc.g = fmaf(ta, cg, acc.g);

@@ -176,8 +176,9 @@ vr_raycast_kernel(const VrRaycastParams prm) {
                     }
                 }
                 if (adv > 0) {
-                    const float v = lerp8(C, L);
-                    if (COUNT) nsamples += (v == v) ? 1 : 0; /* R14: a sample that touches a blanked (NaN) voxel is dropped */
+                    float v = lerp8(C, L);
+                    if (v != v) v = lerp8_blanked(C, L); /* R14: some of the 8 voxels are blanked (rare path) */
+                    if (COUNT) nsamples += (v == v) ? 1 : 0; /* R14: a dropped sample is NaN */
                     if (MODE == VR_MIP) {
                         acc.r = fmaxf(acc.r, v);
                         stopped = acc.r >= mip_stop;
