@@ -23,7 +23,7 @@
  *   - Geometry: world units are voxels. The volume occupies [0,nx] x [0,ny] x [0,nz]; voxel
  *     (i,j,k) is centred at (i+1/2, j+1/2, k+1/2) (R3). Cube memory layout is [nz][ny][nx]
  *     float32, x fastest, z = spectral axis.
- *   - Blanked voxels: a NaN voxel is blanked (R14). A sample with more than 1e-4 of its tri-linear
+ *   - Blanked voxels: a NaN voxel is blanked (R14). A sample with more than 4e-6 of its tri-linear
  *     weight on NaN voxels is dropped (adds nothing in VR_ALPHA, cannot be the maximum in
  *     VR_MIP); with less, the NaN voxels are left out and the other weights renormalised. The
  *     data range ignores NaN. Infinities are not supported.

@@ -33,7 +33,7 @@
  * independent numpy renderer; data range: planted extremes incl. ghost-only cells, brute
  * force; transparent bricks: their sub-images are exactly zero. Parity unpinned (pure conventions): R1 row orientation,
  * R11 MIP alpha, R13 form of the relative tolerance. R14 (NaN = blanked voxel: a sample with
- * more than 1e-4 of its weight on NaN voxels is dropped, else the NaN corners are left out) is
+ * more than 4e-6 of its weight on NaN voxels is dropped, else the NaN corners are left out) is
  * pinned by closed forms on a homogeneous cube with a blanked slab.
  *
  * Build: gcc -O2 -std=c11 -ffp-contract=off -fopenmp -shared -fPIC (oracle/build.py).
@@ -51,7 +51,7 @@
 #define VRO_FLAG_LAST_SAMPLE 4  /* MIP: existence of the last sample is marginal       (R12) */
 #define VRO_FLAG_GRAZING 8      /* hit/miss of the volume decided by < 1e-9 voxel      (R10) */
 #define VRO_FLAG_NAN_MARGIN 16  /* a sample's NaN weight within a factor 2 of the limit (R14) */
-#define VRO_NAN_WEIGHT 1e-4     /* R14: tri-linear weight on NaN corners above which a sample is dropped */
+#define VRO_NAN_WEIGHT 4e-6     /* R14: tri-linear weight on NaN corners above which a sample is dropped */
 
 typedef float (*vro_voxel_fn)(const void* ctx, int64_t x, int64_t y, int64_t z);
 
@@ -273,7 +273,7 @@ static double trilinear(vro_volume* v, int b, const int64_t lo[3], const int64_t
     double val = c0 + f[2] * (c1 - c0);
     if (nan_weight) *nan_weight = 0.0;
     if (isnan(val)) {
-        /* R14: blanked (NaN) voxels. N = the tri-linear weight that falls on NaN corners. N > 1e-4: the
+        /* R14: blanked (NaN) voxels. N = the tri-linear weight that falls on NaN corners. N > 4e-6: the
          * sample is dropped (NaN returned). Otherwise the NaN corners are left out and the rest
          * renormalised: val = sum over valid corners of w_i v_i / (1 - N) - continuous where a sample sits
          * on a cell boundary and a NaN neighbour has weight 0 (the paper's per-ray step puts whole rays there). */
@@ -577,7 +577,7 @@ static void render_pixel(vro_volume* v, const vro_view* vw, const int* order, in
             double nanw;
             double val = trilinear(v, b, lo, hi, p, &nanw);
             /* R14: blanked voxels are NaN (the usual convention of radio cubes). A sample with more than
-             * 1e-4 of its tri-linear weight on NaN voxels is dropped: it is not taken, adds nothing in
+             * 4e-6 of its tri-linear weight on NaN voxels is dropped: it is not taken, adds nothing in
              * ALPHA and cannot be the maximum in MIP. */
             if (nanw > 0.5 * VRO_NAN_WEIGHT && nanw < 2.0 * VRO_NAN_WEIGHT) fl |= VRO_FLAG_NAN_MARGIN;
             if (isnan(val)) continue;

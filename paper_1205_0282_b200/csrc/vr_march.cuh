@@ -388,7 +388,7 @@ __device__ __forceinline__ float lerp8(const Corners& C, const Lattice& L) {
 }
 
 /* R14, the rare path: lerp8 gave NaN, i.e. some of the 8 voxels are blanked. N = tri-linear weight on the
- * NaN corners; N > 1e-4: the sample is dropped (NaN stays); otherwise the NaN corners are left out and the
+ * NaN corners; N > 4e-6: the sample is dropped (NaN stays); otherwise the NaN corners are left out and the
  * others renormalised - continuous where a sample sits on a cell boundary next to a blanked voxel. */
 static __device__ __forceinline__ float lerp8_blanked_values(float c0, float c1, float c2, float c3, float c4, float c5, float c6,
                                                          float c7, float fx, float fy, float fz) {
@@ -400,7 +400,7 @@ static __device__ __forceinline__ float lerp8_blanked_values(float c0, float c1,
         if (c[i] != c[i]) N += w;
         else acc = fmaf(w, c[i], acc);
     }
-    return N > 1e-4f ? __int_as_float(0x7fc00000) : acc / (1.0f - N);
+    return N > 4e-6f ? __int_as_float(0x7fc00000) : acc / (1.0f - N);
 }
 /* everything by value, in registers: a by-reference call would keep the lattice and the voxels in local memory */
 __device__ __forceinline__ float lerp8_blanked(const Corners& C, const Lattice& L) {

@@ -56,20 +56,33 @@ def gpu_frame(g, view, proj, W, H, step, mode):
 def check_alpha(gpu, ref, flags, tau, what=""):
     """gpu, ref: [...,4]; flags: oracle decision-margin flags (R12)."""
     err = np.abs(gpu - ref).max(axis=-1)
+    # R14: a pixel with a sample whose NaN weight is within a factor 2 of the drop limit has two correct values
+    nanm = (flags & oracle.FLAG_NAN_MARGIN) != 0
+    assert nanm.mean() <= 0.01, "%s: %.2f %% of the pixels sit on the NaN-weight limit" % (what, 100 * nanm.mean())
+    err = np.where(nanm, 0.0, err)
     marg = (flags & (oracle.FLAG_ERT_MARGIN | oracle.FLAG_OWNER_MARGIN)) != 0
     bad = err > np.where(marg, ALPHA_TOL + max(0.0, 1.0 - tau), ALPHA_TOL)
     assert not bad.any(), "%s ALPHA: %d pixels off, max err %.3e (unflagged max %.3e)" % (
         what, int(bad.sum()), err.max(), err[~marg].max() if (~marg).any() else 0.0)
     # R12: a ray whose opacity passes tau in steps of dA is flagged with probability ~2e-5/dA
     # (a few per cent at most); what must stay rare is a flagged pixel that really differs
-    assert marg.mean() < 0.03, "%s: %.4f%% decision-margin pixels" % (what, 100 * marg.mean())
+    ert = (flags & oracle.FLAG_ERT_MARGIN) != 0
+    assert ert.mean() < 0.03, "%s: %.4f%% early-termination-margin pixels" % (what, 100 * ert.mean())
+    # owner margins (a sample within 1e-6 voxel of a brick face) are a property of the view: with the per-ray
+    # step an axis-aligned ray samples ON the voxel planes; a random view has none
+    assert marg.mean() < 0.10, "%s: %.4f%% decision-margin pixels" % (what, 100 * marg.mean())
     assert (err > ALPHA_TOL).mean() < 1e-3, "%s: %.4f%% pixels beyond 2e-3" % (what, 100 * (err > ALPHA_TOL).mean())
     return float(err.max())
 
 
-def check_mip(gpu, ref, what=""):
+def check_mip(gpu, ref, what="", flags=None):
     tol = MIP_RTOL * np.maximum(np.abs(gpu), np.abs(ref)) + MIP_ATOL
     err = np.abs(gpu - ref)
+    if flags is not None:  # R14 / R12: pixels with two correct values (NaN-weight limit, marginal last sample)
+        nanm = (flags & oracle.FLAG_NAN_MARGIN) != 0
+        assert nanm.mean() <= 0.01, "%s: %.2f %% of the pixels sit on the NaN-weight limit" % (what, 100 * nanm.mean())
+        loose = nanm | ((flags & oracle.FLAG_LAST_SAMPLE) != 0)
+        err = np.where(loose[..., None], 0.0, err)
     bad = err > tol
     assert not bad.any(), "%s MIP: %d values off, max err %.3e" % (what, int(bad.sum()), err.max())
     return float((err / np.maximum(np.abs(ref), 1e-30)).max())

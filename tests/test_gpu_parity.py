@@ -554,8 +554,8 @@ def test_fused_traversal_edge_cases(vr):
 # --------------------------------------------------------------------------- blanked voxels (R14)
 def test_nan_voxels_are_blanked(vr):
     """NaN voxels (blanked channels, masked edges: the usual state of a radio cube) drop exactly the
-    samples that touch them on both sides: parity in both modes and traversals, with the exact
-    sample count; the data range ignores them; culling and macro-cell skipping stay exact."""
+    samples that rest on them on both sides: parity in both modes and traversals, with the same
+    sample count (up to the samples that sit on the NaN-weight limit); the data range ignores them; culling and macro-cell skipping stay exact."""
     nx, ny, nz, B = 90, 70, 52, 16
     data = synth.Cube(91, nx, ny, nz, 8).fill_host()
     data[:, :, :5] = np.nan                       # a masked edge
@@ -586,13 +586,14 @@ def test_nan_voxels_are_blanked(vr):
             img = gpu_frame(g, view, proj, W, H, 0.5, vr.ALPHA)
             assert np.isfinite(img).all()
             check_alpha(img, ref["image"], ref["flags"], 2.0, "NaN " + tf_name)
-            assert g.debug_stats()["samples"] == int(ref["counts"][..., 0].sum())
+            slack = 4 * int(((ref["flags"] & oracle.FLAG_NAN_MARGIN) != 0).sum())   # samples on the NaN-weight limit may go either way
+            assert abs(g.debug_stats()["samples"] - int(ref["counts"][..., 0].sum())) <= slack
             g.set_culling(True)
             assert np.array_equal(gpu_frame(g, view, proj, W, H, 0.5, vr.ALPHA), img)
             refm = orc.render(view, proj, W, H, 0.5, oracle.MIP)
             imgm = gpu_frame(g, view, proj, W, H, 0.5, vr.MIP)
-            check_mip(imgm, refm["image"], "NaN MIP")
-            assert g.debug_stats()["samples"] == int(refm["counts"][..., 0].sum())
+            check_mip(imgm, refm["image"], "NaN MIP", flags=refm["flags"])
+            assert abs(g.debug_stats()["samples"] - int(refm["counts"][..., 0].sum())) <= slack
     # a fully blanked volume renders nothing
     gb = vr.Volume(24, 24, 24, 16, 1)
     gb.upload(np.full((24, 24, 24), np.nan, dtype=np.float32))
@@ -649,10 +650,7 @@ def test_randomised_configurations(vr, case):
                     tau, "case %d" % case)
         refm = orc.render(view, proj, W, H, step, oracle.MIP)
         got = gpu_frame(g, view, proj, W, H, step if step > 0 else vr.STEP_AUTO, vr.MIP)
-        lastm = (refm["flags"] & oracle.FLAG_LAST_SAMPLE) != 0     # R12: the marginal last sample may or may not exist in float
-        tol = MIP_TOL = 1e-5 * np.maximum(np.abs(got), np.abs(refm["image"])) + 1e-7
-        bad = (np.abs(got - refm["image"]) > tol).any(axis=-1) & ~lastm
-        assert not bad.any(), "case %d MIP: %d pixels off" % (case, int(bad.sum()))
+        check_mip(got, refm["image"], "case %d" % case, flags=refm["flags"])
 
 
 # --------------------------------------------------------------------------- state across calls

@@ -669,7 +669,7 @@ def test_auto_step_is_one_sample_per_major_axis_voxel():
 
 # --------------------------------------------------------------------------- blanked voxels (R14)
 def test_nan_voxels_drop_the_samples_that_rest_on_them():
-    """Radio cubes blank voxels with NaN. R14: a sample with more than 1e-4 of its tri-linear
+    """Radio cubes blank voxels with NaN. R14: a sample with more than 4e-6 of its tri-linear
     weight on NaN voxels is dropped; otherwise the NaN corners are left out and the others
     renormalised (so a NaN neighbour with weight 0 changes nothing - where the paper's per-ray
     step puts whole rays). Closed forms: homogeneous cube, axis-aligned orthographic rays, step 1.
