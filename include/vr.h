@@ -269,6 +269,52 @@ int vr_composite(const float* const* layers, const int* rects, const int* order,
                  int width, int height, float* out, void* stream);
 
 /* ------------------------------------------------------------------------------------------
+ * Multi-GPU sort-last (PAPER.md:136-138 data partitioning,
+ * :170-174 two-stage compositing, :178-184 direct send of rectangle-packed partial frames).
+ * One process per GPU; each holds a PART: a box of bricks of the global brick grid. A part
+ * handle behaves like a volume in every call above, in GLOBAL voxel coordinates and with the
+ * global brick numbering, but stores, ranges, culls and renders only its own bricks: rays,
+ * sample positions, the owner rule and the visibility order are those of the whole volume, so
+ * the sub-images of a part's bricks are bit-identical to the ones a single handle renders.
+ * libvr moves no data between GPUs: the exchange is the caller's (paper_1205_0282_b200.sortlast
+ * uses torch.distributed), the kernels on both sides of it are these.
+ *
+ * vr_volume_create_part: b0, b1 (host, int[3]): the part holds bricks b0 <= (bx,by,bz) < b1
+ *   (brick (bx,by,bz) = voxels [bx*brick, min((bx+1)*brick, n)) per axis). Memory: the box's
+ *   bricks only. vr_volume_upload takes boxes anywhere in the volume and keeps what falls into
+ *   the padded extent of the part's bricks: upload the part's voxels plus `ghost` layers of its
+ *   neighbours' (R3; a ghost layer left out reads as zeros). vr_volume_download and
+ *   vr_debug_brick_data accept the part's own bricks only; vr_volume_minmax gives the range of
+ *   the part's voxels (ghost layers included) - reduce it over the parts for the global range;
+ *   table entries of bricks held elsewhere are (+inf, -inf).
+ * vr_render_part: one frame of the part's bricks only, full-frame [height][width][4]:
+ *   VR_ALPHA  premultiplied RGBA of the part's sub-images composited in visibility order (what
+ *             vr_render gives on a part handle);
+ *   VR_MIP    (m, 0, 0, 1) with m the raw maximum over the part's samples, (0,0,0,0) for a ray
+ *             that takes no sample in the part (needs VR_SORT_LAST, else VR_ERR_STATE);
+ *   rect_out (host, int[4], may be NULL): (x0,y0,x1,y1), half-open: a rectangle that contains
+ *   every non-blank pixel of the partial frame (union of the bricks' rendering rectangles with
+ *   a pixel of slack; PAPER.md:184 packs messages by it); all zero if nothing is on screen.
+ * vr_part_rect: the same rectangle from the geometry alone (host arithmetic, no handle, no
+ *   device), so that every process can size the pieces it will receive without a message.
+ * vr_composite_parts: merges partial frames. parts/rects/order/n/out as vr_composite (piece l
+ *   covers rects[l], stored [y1-y0][x1-x0][4]); order = the parts front to back (any order for
+ *   VR_MIP). VR_ALPHA: front-to-back `over` (identical to vr_composite). VR_MIP: maximum of
+ *   the x components of the pieces whose w is non-zero, then the colour mapping with v's
+ *   transfer function, (0,0,0,0) where no piece holds a sample.
+ *   `over` is associative: merging the parts' frames in part order equals
+ *   compositing all sub-images in brick order up to float32 rounding, provided the part order
+ *   is a visibility order of the boxes (sortlast.part_order: the k-d tree, near side first). */
+int vr_volume_create_part(int nx, int ny, int nz, int brick, int ghost, const int* b0,
+                          const int* b1, vr_volume** out);
+int vr_render_part(vr_volume* v, const float* view, const float* proj, int width, int height,
+                   float step, int mode, float* out_part, int* rect_out, void* stream);
+int vr_part_rect(int nx, int ny, int nz, int brick, const int* b0, const int* b1,
+                 const float* view, const float* proj, int width, int height, int* rect_out);
+int vr_composite_parts(vr_volume* v, int mode, const float* const* parts, const int* rects,
+                       const int* order, int n, int width, int height, float* out, void* stream);
+
+/* ------------------------------------------------------------------------------------------
  * Debug / test exports. All synchronise and write HOST memory.
  * ---------------------------------------------------------------------------------------- */
 

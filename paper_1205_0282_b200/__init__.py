@@ -29,6 +29,7 @@ SYMBOLS = (
     "vr_volume_create", "vr_volume_create_layout", "vr_volume_destroy", "vr_volume_upload", "vr_volume_download", "vr_debug_brick_data",
     "vr_set_transfer_function", "vr_set_early_termination", "vr_volume_minmax", "vr_set_culling", "vr_set_traversal", "vr_debug_brick_minmax", "vr_debug_cell_flags", "vr_render", "vr_render_host", "vr_render_host_async", "vr_render_host_wait", "vr_composite",
     "vr_num_bricks", "vr_debug_brick_order", "vr_debug_rects", "vr_debug_ray_bricks", "vr_debug_subimages",
+    "vr_volume_create_part", "vr_render_part", "vr_part_rect", "vr_composite_parts",
     "vr_set_counting", "vr_set_timing", "vr_debug_stats", "vr_debug_stage_times", "vr_launch_count", "vr_last_error",
 )
 
@@ -79,6 +80,10 @@ def lib():
         L.vr_render_host_async.argtypes = [vp, vp, vp, ci, ci, cf, ci, vp, vp]
         L.vr_render_host_wait.argtypes = [vp]
         L.vr_composite.argtypes = [vp, vp, vp, ci, ci, ci, vp, vp]
+        L.vr_volume_create_part.argtypes = [ci, ci, ci, ci, ci, vp, vp, ctypes.POINTER(vp)]
+        L.vr_render_part.argtypes = [vp, vp, vp, ci, ci, cf, ci, vp, vp, vp]
+        L.vr_part_rect.argtypes = [ci, ci, ci, ci, vp, vp, vp, vp, ci, ci, vp]
+        L.vr_composite_parts.argtypes = [vp, ci, vp, vp, vp, ci, ci, ci, vp, vp]
         L.vr_num_bricks.argtypes = [vp]
         L.vr_debug_brick_order.argtypes = [vp, vp, vp, vp]
         L.vr_debug_rects.argtypes = [vp, vp, vp, ci, ci, vp]
@@ -114,11 +119,18 @@ def _pixels(pixels):
 class Volume:
     """Handle of a bricked volume in HBM (vr_volume_create ... vr_volume_destroy)."""
 
-    def __init__(self, nx, ny, nz, brick, ghost=1, layout=LAYOUT_DEFAULT):
+    def __init__(self, nx, ny, nz, brick, ghost=1, layout=LAYOUT_DEFAULT, part=None):
+        """part = (b0, b1): hold only the bricks b0 <= (bx,by,bz) < b1 of the grid (vr_volume_create_part)."""
         self._h = ctypes.c_void_p()
         self.nx, self.ny, self.nz, self.brick, self.ghost = int(nx), int(ny), int(nz), int(brick), int(ghost)
         self.layout = int(layout)
-        if self.layout == LAYOUT_DEFAULT:
+        self.part = None if part is None else (tuple(int(c) for c in part[0]), tuple(int(c) for c in part[1]))
+        if self.part is not None:
+            b0 = np.asarray(self.part[0], dtype=np.int32)
+            b1 = np.asarray(self.part[1], dtype=np.int32)
+            rc = lib().vr_volume_create_part(self.nx, self.ny, self.nz, self.brick, self.ghost, b0.ctypes.data, b1.ctypes.data,
+                                             ctypes.byref(self._h))
+        elif self.layout == LAYOUT_DEFAULT:
             rc = lib().vr_volume_create(self.nx, self.ny, self.nz, self.brick, self.ghost, ctypes.byref(self._h))
         else:
             rc = lib().vr_volume_create_layout(self.nx, self.ny, self.nz, self.brick, self.ghost, self.layout,
@@ -222,6 +234,31 @@ class Volume:
                                     out.data_ptr(), _stream(stream)))
         return out
 
+    def render_part(self, view, proj, width, height, step, mode, out, stream=None):
+        """This handle's contribution to a sort-last frame (vr_render_part). out: CUDA float32 tensor
+        [height][width][4]; returns the rectangle (x0,y0,x1,y1) outside which out is blank."""
+        assert out.is_cuda and out.is_contiguous() and out.element_size() == 4 and out.numel() == width * height * 4
+        v, p = _mat(view), _mat(proj)
+        rect = np.zeros(4, dtype=np.int32)
+        self._check(lib().vr_render_part(self._h, v.ctypes.data, p.ctypes.data, int(width), int(height), float(step), int(mode),
+                                         out.data_ptr(), rect.ctypes.data, _stream(stream)))
+        return tuple(int(c) for c in rect)
+
+    def composite_parts(self, mode, parts, rects, order, width, height, out, stream=None):
+        """Merge partial frames (vr_composite_parts). parts: CUDA float32 tensors [y1-y0][x1-x0][4], piece l
+        covering rects[l]; order: the pieces front to back; out: CUDA float32 tensor [height][width][4]."""
+        n = len(parts)
+        ptrs = (ctypes.c_void_p * max(n, 1))(*[l.data_ptr() for l in parts])
+        r = np.ascontiguousarray(rects, dtype=np.int32).reshape(n, 4)
+        o = np.ascontiguousarray(order, dtype=np.int32).reshape(n)
+        for l, rc_ in zip(parts, r):
+            assert l.is_cuda and l.is_contiguous() and l.element_size() == 4
+            assert l.numel() == (rc_[2] - rc_[0]) * (rc_[3] - rc_[1]) * 4
+        assert out.is_cuda and out.is_contiguous() and out.numel() == width * height * 4
+        self._check(lib().vr_composite_parts(self._h, int(mode), ptrs, r.ctypes.data, o.ctypes.data, n, int(width), int(height),
+                                             out.data_ptr(), _stream(stream)))
+        return out
+
     def render_host(self, view, proj, width, height, step, mode, out=None, stream=None):
         """out: float32 numpy array or pinned CPU tensor [height][width][4]; returns when filled."""
         v, p = _mat(view), _mat(proj)
@@ -304,6 +341,19 @@ class Volume:
 
     def launch_count(self):
         return int(lib().vr_launch_count(self._h))
+
+
+def part_rect(dims, brick, box, view, proj, width, height):
+    """vr_part_rect: the frame rectangle (x0,y0,x1,y1) a part's partial frame can be non-blank in. Host only."""
+    b0 = np.asarray(box[0], dtype=np.int32)
+    b1 = np.asarray(box[1], dtype=np.int32)
+    v, p = _mat(view), _mat(proj)
+    rect = np.zeros(4, dtype=np.int32)
+    rc = lib().vr_part_rect(int(dims[0]), int(dims[1]), int(dims[2]), int(brick), b0.ctypes.data, b1.ctypes.data, v.ctypes.data,
+                            p.ctypes.data, int(width), int(height), rect.ctypes.data)
+    if rc != 0:
+        raise VrError(rc, lib().vr_last_error(None).decode())
+    return tuple(int(c) for c in rect)
 
 
 def composite(layers, rects, order, width, height, out, stream=None):

@@ -16,7 +16,7 @@
 
 struct vr_volume {
     VrGrid grid;
-    float* bricks;           /* nbricks * slot floats */
+    float* bricks;           /* nown * slot floats (nown = nbricks unless the handle is a part) */
     bool has_data, has_tf;
     float4* d_lut_base;      /* VR_MAX_LUT entries each */
     float4* d_lut_delta;
@@ -177,7 +177,19 @@ extern "C" int vr_volume_create(int nx, int ny, int nz, int brick, int ghost, vr
     return vr_volume_create_layout(nx, ny, nz, brick, ghost, VR_LAYOUT_DEFAULT, out);
 }
 
+static int create_volume(int nx, int ny, int nz, int brick, int ghost, int layout, const int* b0, const int* b1, vr_volume** out);
+
 extern "C" int vr_volume_create_layout(int nx, int ny, int nz, int brick, int ghost, int layout, vr_volume** out) {
+    return create_volume(nx, ny, nz, brick, ghost, layout, NULL, NULL, out);
+}
+
+extern "C" int vr_volume_create_part(int nx, int ny, int nz, int brick, int ghost, const int* b0, const int* b1, vr_volume** out) {
+    if (!b0 || !b1) return fail(NULL, VR_ERR_INVALID_ARG, "vr_volume_create_part: NULL box");
+    return create_volume(nx, ny, nz, brick, ghost, VR_LAYOUT_DEFAULT, b0, b1, out);
+}
+
+/* b0, b1: the box of bricks the handle holds (row f3), or NULL for the whole grid */
+static int create_volume(int nx, int ny, int nz, int brick, int ghost, int layout, const int* b0, const int* b1, vr_volume** out) {
     if (!out) return fail(NULL, VR_ERR_INVALID_ARG, "vr_volume_create: out is NULL");
     *out = NULL;
     if (nx <= 0 || ny <= 0 || nz <= 0) return fail(NULL, VR_ERR_INVALID_ARG, "vr_volume_create: non-positive size %dx%dx%d", nx, ny, nz);
@@ -212,6 +224,24 @@ extern "C" int vr_volume_create_layout(int nx, int ny, int nz, int brick, int gh
         return fail(NULL, VR_ERR_INVALID_ARG, "vr_volume_create: %lld bricks > 65535", nb);
     }
     g.nbricks = (int)nb;
+    g.part = 0;
+    g.nown = g.nbricks;
+    for (int a = 0; a < 3; ++a) g.pb0[a] = 0, g.pb1[a] = g.g[a];
+    if (b0 && b1) {
+        long long own = 1;
+        for (int a = 0; a < 3; ++a) {
+            if (b0[a] < 0 || b1[a] <= b0[a] || b1[a] > g.g[a]) {
+                const int gx = g.g[0], gy = g.g[1], gz = g.g[2];
+                delete v;
+                return fail(NULL, VR_ERR_INVALID_ARG, "vr_volume_create_part: box [%d,%d) x [%d,%d) x [%d,%d) is empty or outside the %dx%dx%d brick grid",
+                            b0[0], b1[0], b0[1], b1[1], b0[2], b1[2], gx, gy, gz);
+            }
+            g.pb0[a] = b0[a], g.pb1[a] = b1[a];
+            own *= b1[a] - b0[a];
+        }
+        g.nown = (int)own;
+        g.part = g.nown != g.nbricks;
+    }
     /* a volume smaller than one brick needs no larger slot than itself */
     int core = brick;
     {
@@ -235,8 +265,8 @@ extern "C" int vr_volume_create_layout(int nx, int ny, int nz, int brick, int gh
     v->tau = 0.99f;
     v->culling = true;
 
-    cudaError_t e = cudaMalloc(&v->bricks, (size_t)g.slot * (size_t)g.nbricks * sizeof(float));
-    if (e == cudaSuccess) e = cudaMemset(v->bricks, 0, (size_t)g.slot * (size_t)g.nbricks * sizeof(float));
+    cudaError_t e = cudaMalloc(&v->bricks, (size_t)g.slot * (size_t)g.nown * sizeof(float));
+    if (e == cudaSuccess) e = cudaMemset(v->bricks, 0, (size_t)g.slot * (size_t)g.nown * sizeof(float));
     if (e == cudaSuccess) e = cudaMalloc(&v->d_lut_base, VR_MAX_LUT * sizeof(float4));
     if (e == cudaSuccess) e = cudaMalloc(&v->d_lut_delta, VR_MAX_LUT * sizeof(float4));
     if (e == cudaSuccess) e = cudaMalloc(&v->d_vs, sizeof(VrViewState));
@@ -253,7 +283,7 @@ extern "C" int vr_volume_create_layout(int nx, int ny, int nz, int brick, int gh
         cudaGetLastError();
         const int st = (e == cudaErrorMemoryAllocation) ? VR_ERR_OUT_OF_MEMORY : VR_ERR_CUDA;
         fail(NULL, st, "vr_volume_create: %s (brick store needs %.2f GB)", cudaGetErrorString(e),
-             (double)g.slot * g.nbricks * 4.0 / 1e9);
+             (double)g.slot * g.nown * 4.0 / 1e9);
         release(v);
         return st;
     }
@@ -326,6 +356,15 @@ extern "C" int vr_volume_download(vr_volume* v, float* dst, int memspace, int x0
                                   void* stream) {
     int rc = check_box(v, "vr_volume_download", dst, memspace, x0, y0, z0, sx, sy, sz);
     if (rc) return rc;
+    if (v->grid.part) { /* a part can return voxels of its own bricks only */
+        const VrGrid& g = v->grid;
+        const int lo[3] = {x0, y0, z0}, hi[3] = {x0 + sx, y0 + sy, z0 + sz};
+        for (int a = 0; a < 3; ++a) {
+            const long long plo = (long long)g.pb0[a] * g.brick, phi = (long long)g.pb1[a] * g.brick;
+            if (lo[a] < plo || hi[a] > (phi < g.n[a] ? phi : g.n[a]))
+                return fail(v, VR_ERR_INVALID_ARG, "vr_volume_download: the box leaves the bricks this part holds");
+        }
+    }
     cudaStream_t st = (cudaStream_t)stream;
     if (memspace == VR_DEVICE) {
         VR_CUDA(v, vr_launch_download(v->grid, v->bricks, dst, x0, y0, z0, sx, sy, sz, st));
@@ -351,6 +390,7 @@ extern "C" int vr_debug_brick_data(vr_volume* v, int b, float* dst, int* dims) {
     if (!v) return fail(NULL, VR_ERR_INVALID_ARG, "vr_debug_brick_data: NULL handle");
     const VrGrid& g = v->grid;
     if (b < 0 || b >= g.nbricks || !dims) return fail(v, VR_ERR_INVALID_ARG, "vr_debug_brick_data: bad brick %d or NULL dims", b);
+    if (vr_slot_index(g, b) < 0) return fail(v, VR_ERR_INVALID_ARG, "vr_debug_brick_data: this part does not hold brick %d", b);
     const int bx = b % g.g[0], by = (b / g.g[0]) % g.g[1], bz = b / (g.g[0] * g.g[1]);
     const int bc[3] = {bx, by, bz};
     int d[3];
@@ -428,7 +468,7 @@ extern "C" int vr_set_counting(vr_volume* v, int enable) {
     if (!v) return fail(NULL, VR_ERR_INVALID_ARG, "vr_set_counting: NULL handle");
     if (enable < 0 || enable > 2) return fail(v, VR_ERR_INVALID_ARG, "vr_set_counting: mode %d outside [0,2]", enable);
     if (enable == 2 && !v->d_bitmap) {
-        const long long words = (v->grid.slot * v->grid.nbricks + 31) / 32;
+        const long long words = (v->grid.slot * v->grid.nown + 31) / 32;
         VR_CUDA(v, cudaMalloc(&v->d_bitmap, (size_t)words * sizeof(unsigned)));
         VR_CUDA(v, cudaMalloc(&v->d_counts2, 3 * sizeof(unsigned long long)));
         v->bitmap_words = words;
@@ -495,8 +535,8 @@ static int ensure_cells(vr_volume* v, bool want_bits, cudaStream_t st) {
         for (int a = 0; a < 3; ++a) v->nc[a] = (g.nt[a] * (1 << g.tl[a]) + 7) / 8;
         const long long ncell = (long long)v->nc[0] * v->nc[1] * v->nc[2];
         v->cell_words = (int)((ncell + 31) / 32);
-        VR_CUDA(v, cudaMalloc(&v->d_cell_mm, sizeof(float2) * (size_t)ncell * g.nbricks));
-        VR_CUDA(v, cudaMalloc(&v->d_cell_bits, sizeof(unsigned) * (size_t)v->cell_words * g.nbricks));
+        VR_CUDA(v, cudaMalloc(&v->d_cell_mm, sizeof(float2) * (size_t)ncell * g.nown));
+        VR_CUDA(v, cudaMalloc(&v->d_cell_bits, sizeof(unsigned) * (size_t)v->cell_words * g.nown));
     }
     if (!v->cell_mm_valid) {
         VR_CUDA(v, vr_launch_cell_minmax(g, v->bricks, v->d_cell_mm, v->nc, st));
@@ -505,7 +545,7 @@ static int ensure_cells(vr_volume* v, bool want_bits, cudaStream_t st) {
         v->cell_bits_valid = false;
     }
     if (want_bits && !v->cell_bits_valid) {
-        VR_CUDA(v, vr_launch_cell_flags(v->d_cell_mm, v->d_cell_bits, g.nbricks, v->nc, v->cell_words, v->lut, st));
+        VR_CUDA(v, vr_launch_cell_flags(v->d_cell_mm, v->d_cell_bits, g.nown, v->nc, v->cell_words, v->lut, st));
         v->launches++;
         v->cell_bits_valid = true;
     }
@@ -521,7 +561,7 @@ static int decide_mip_skip(vr_volume* v, cudaStream_t st) {
     if (!rc) rc = ensure_cells(v, false, st);
     if (rc) return rc;
     if (!v->d_cell_count) VR_CUDA(v, cudaMalloc(&v->d_cell_count, sizeof(unsigned long long)));
-    const long long ncells = (long long)v->nc[0] * v->nc[1] * v->nc[2] * v->grid.nbricks;
+    const long long ncells = (long long)v->nc[0] * v->nc[1] * v->nc[2] * v->grid.nown;
     unsigned long long empty = 0;
     VR_CUDA(v, cudaMemsetAsync(v->d_cell_count, 0, sizeof(unsigned long long), st));
     VR_CUDA(v, vr_launch_cell_count_empty(v->d_cell_mm, ncells, v->d_mm + v->grid.nbricks, v->d_cell_count, st));
@@ -580,6 +620,8 @@ extern "C" int vr_set_culling(vr_volume* v, int enable) {
 extern "C" int vr_debug_cell_flags(vr_volume* v, int b, unsigned char* flags_out, int* dims) {
     if (!v) return fail(NULL, VR_ERR_INVALID_ARG, "vr_debug_cell_flags: NULL handle");
     if (!dims || b < 0 || b >= v->grid.nbricks) return fail(v, VR_ERR_INVALID_ARG, "vr_debug_cell_flags: bad brick %d or NULL dims", b);
+    const int slot_b = vr_slot_index(v->grid, b);
+    if (slot_b < 0) return fail(v, VR_ERR_INVALID_ARG, "vr_debug_cell_flags: this part does not hold brick %d", b);
     if (!v->has_data || !v->has_tf) return fail(v, VR_ERR_STATE, "vr_debug_cell_flags: needs data and a transfer function");
     if (!cells_supported(v)) return fail(v, VR_ERR_STATE, "vr_debug_cell_flags: macro-cells need the 4x4x2 layout and ghost >= 1");
     const int rc = ensure_cells(v, true, 0);
@@ -589,7 +631,7 @@ extern "C" int vr_debug_cell_flags(vr_volume* v, int b, unsigned char* flags_out
     VR_CUDA(v, cudaDeviceSynchronize());
     unsigned* words = new (std::nothrow) unsigned[v->cell_words];
     if (!words) return fail(v, VR_ERR_OUT_OF_MEMORY, "vr_debug_cell_flags: host allocation failed");
-    const cudaError_t e = cudaMemcpy(words, v->d_cell_bits + (size_t)b * v->cell_words, sizeof(unsigned) * v->cell_words,
+    const cudaError_t e = cudaMemcpy(words, v->d_cell_bits + (size_t)slot_b * v->cell_words, sizeof(unsigned) * v->cell_words,
                                      cudaMemcpyDeviceToHost);
     if (e == cudaSuccess)
         for (int m = 0; m < v->nc[0] * v->nc[1] * v->nc[2]; ++m) flags_out[m] = (unsigned char)((words[m >> 5] >> (m & 31)) & 1u);
@@ -609,11 +651,54 @@ extern "C" int vr_debug_brick_minmax(vr_volume* v, float* mm_out) {
     return VR_OK;
 }
 
+static int render_frame(vr_volume* v, const float* view, const float* proj, int width, int height, float step, int mode,
+                        float* out_rgba, void* stream, bool partial);
+
 extern "C" int vr_render(vr_volume* v, const float* view, const float* proj, int width, int height, float step, int mode,
                          float* out_rgba, void* stream) {
+    return render_frame(v, view, proj, width, height, step, mode, out_rgba, stream, false);
+}
+
+extern "C" int vr_render_part(vr_volume* v, const float* view, const float* proj, int width, int height, float step, int mode,
+                              float* out_part, int* rect_out, void* stream) {
+    const int rc = render_frame(v, view, proj, width, height, step, mode, out_part, stream, true);
+    if (rc) return rc;
+    if (rect_out && vr_host_part_rect(v->grid, view, proj, width, height, rect_out))
+        return fail(v, VR_ERR_INVALID_ARG, "vr_render_part: proj*view is singular");
+    return VR_OK;
+}
+
+extern "C" int vr_part_rect(int nx, int ny, int nz, int brick, const int* b0, const int* b1, const float* view, const float* proj,
+                            int width, int height, int* rect_out) {
+    if (!b0 || !b1 || !view || !proj || !rect_out) return fail(NULL, VR_ERR_INVALID_ARG, "vr_part_rect: NULL argument");
+    if (nx <= 0 || ny <= 0 || nz <= 0 || brick < 2 || width <= 0 || height <= 0)
+        return fail(NULL, VR_ERR_INVALID_ARG, "vr_part_rect: bad volume, brick or frame size");
+    VrGrid g;
+    memset(&g, 0, sizeof(g));
+    g.n[0] = nx; g.n[1] = ny; g.n[2] = nz;
+    g.brick = brick;
+    g.part = 1;
+    long long nb = 1;
+    for (int a = 0; a < 3; ++a) {
+        g.g[a] = (g.n[a] + brick - 1) / brick;
+        nb *= g.g[a];
+        if (b0[a] < 0 || b1[a] <= b0[a] || b1[a] > g.g[a]) return fail(NULL, VR_ERR_INVALID_ARG, "vr_part_rect: bad brick box");
+        g.pb0[a] = b0[a], g.pb1[a] = b1[a];
+    }
+    if (nb > 65535) return fail(NULL, VR_ERR_INVALID_ARG, "vr_part_rect: %lld bricks > 65535", nb);
+    g.nbricks = (int)nb;
+    if (vr_host_part_rect(g, view, proj, width, height, rect_out)) return fail(NULL, VR_ERR_INVALID_ARG, "vr_part_rect: proj*view is singular");
+    return VR_OK;
+}
+
+/* partial: the frame is one part's contribution to a sort-last frame (row f3): a MIP frame stays scalar */
+static int render_frame(vr_volume* v, const float* view, const float* proj, int width, int height, float step, int mode,
+                        float* out_rgba, void* stream, bool partial) {
     long long sub_px = 0, items = 0;
     int rc = check_view(v, "vr_render", view, proj, width, height, &sub_px, &items);
     if (rc) return rc;
+    if (partial && mode == VR_MIP && v->traversal == VR_FUSED)
+        return fail(v, VR_ERR_STATE, "vr_render_part: VR_MIP parts need the VR_SORT_LAST traversal");
     if (!out_rgba) return fail(v, VR_ERR_INVALID_ARG, "vr_render: NULL output");
     if (!(step >= 0.0f) || !isfinite(step)) return fail(v, VR_ERR_INVALID_ARG, "vr_render: step must be > 0, or VR_STEP_AUTO (0)");
     if (mode != VR_ALPHA && mode != VR_MIP) return fail(v, VR_ERR_INVALID_ARG, "vr_render: bad mode %d", mode);
@@ -674,11 +759,12 @@ extern "C" int vr_render(vr_volume* v, const float* view, const float* proj, int
         if (timing) VR_CUDA(v, cudaEventRecord(ev[2], st));
     } else {
         /* brick faces of brick^2 voxels project onto sub_px pixels in all: > 4 voxels per pixel = sparse */
-        const bool sparse = (double)v->grid.nbricks * v->grid.brick * v->grid.brick > 4.0 * (double)sub_px;
+        const bool sparse = (double)v->grid.nown * v->grid.brick * v->grid.brick > 4.0 * (double)sub_px;
         VR_CUDA(v, vr_launch_raycast(p, items, v->counting != 0, sparse, st));
         v->launches++;
         if (timing) VR_CUDA(v, cudaEventRecord(ev[2], st));
-        VR_CUDA(v, vr_launch_composite(v->d_layers, v->d_order, v->grid.nbricks, width, height, mode, v->lut, out_rgba, st));
+        VR_CUDA(v, vr_launch_composite(v->d_layers, v->d_order, v->grid.nbricks, width, height,
+                                       (partial && mode == VR_MIP) ? VR_MIP_RAW : mode, v->lut, out_rgba, st));
         v->launches++;
     }
     if (timing) {
@@ -769,8 +855,28 @@ extern "C" int vr_render_host_wait(vr_volume* v) {
 }
 
 /* ------------------------------------------------------------------------------------------ */
+static int composite_layers(const VrLut& lut, int kmode, const float* const* layers, const int* rects, const int* order, int n,
+                            int width, int height, float* out, void* stream);
+
 extern "C" int vr_composite(const float* const* layers, const int* rects, const int* order, int n, int width, int height,
                             float* out, void* stream) {
+    VrLut none;
+    memset(&none, 0, sizeof(none));
+    return composite_layers(none, VR_ALPHA, layers, rects, order, n, width, height, out, stream);
+}
+
+extern "C" int vr_composite_parts(vr_volume* v, int mode, const float* const* parts, const int* rects, const int* order, int n,
+                                  int width, int height, float* out, void* stream) {
+    if (!v) return fail(NULL, VR_ERR_INVALID_ARG, "vr_composite_parts: NULL handle");
+    if (mode != VR_ALPHA && mode != VR_MIP) return fail(v, VR_ERR_INVALID_ARG, "vr_composite_parts: bad mode %d", mode);
+    if (mode == VR_MIP && !v->has_tf) return fail(v, VR_ERR_STATE, "vr_composite_parts: no transfer function set");
+    const int rc = composite_layers(v->lut, mode == VR_MIP ? VR_MIP_PARTS : VR_ALPHA, parts, rects, order, n, width, height, out, stream);
+    if (rc == VR_OK) v->launches++;
+    return rc;
+}
+
+static int composite_layers(const VrLut& lut, int kmode, const float* const* layers, const int* rects, const int* order, int n,
+                            int width, int height, float* out, void* stream) {
     if (!layers || !rects || !order || !out) return fail(NULL, VR_ERR_INVALID_ARG, "vr_composite: NULL argument");
     if (n < 0 || n > 4096) return fail(NULL, VR_ERR_INVALID_ARG, "vr_composite: n = %d outside [0,4096]", n);
     if (width <= 0 || height <= 0 || width > 32768 || height > 32768)
@@ -812,9 +918,7 @@ extern "C" int vr_composite(const float* const* layers, const int* rects, const 
         VR_CUDA(NULL, cudaMemcpyAsync(d_tab, tab, sizeof(VrCompLayer) * n, cudaMemcpyHostToDevice, st));
         VR_CUDA(NULL, cudaMemcpyAsync(d_order, order, sizeof(int) * n, cudaMemcpyHostToDevice, st));
     }
-    VrLut none;
-    memset(&none, 0, sizeof(none));
-    VR_CUDA(NULL, vr_launch_composite(d_tab, d_order, n, width, height, VR_ALPHA, none, out, st));
+    VR_CUDA(NULL, vr_launch_composite(d_tab, d_order, n, width, height, kmode, lut, out, st));
     VR_CUDA(NULL, cudaFreeAsync(d_tab, st));
     VR_CUDA(NULL, cudaFreeAsync(d_order, st));
     return VR_OK;

@@ -48,9 +48,11 @@ vr_upload_kernel(VrGrid g, float* __restrict__ bricks, const float* __restrict__
     padded_range(lo[1], g.ghost, ey, g.n[1], y0, y0 + sy, j0, j1);
     padded_range(lo[2], g.ghost, ez, g.n[2], z0, z0 + sz, k0, k1);
     if (i1 <= i0 || j1 <= j0 || k1 <= k0) return;
+    const int slot_b = vr_slot_index(g, b);
+    if (slot_b < 0) return; /* a part handle does not hold this brick (row f3) */
     const int rows = (j1 - j0) * (k1 - k0);
     const int warps_per_block = blockDim.x >> 5, lane = threadIdx.x & 31;
-    float* __restrict__ dstb = bricks + (long long)b * g.slot;
+    float* __restrict__ dstb = bricks + (long long)slot_b * g.slot;
     for (int row = blockIdx.x * warps_per_block + (threadIdx.x >> 5); row < rows; row += gridDim.x * warps_per_block) {
         const int j = j0 + row % (j1 - j0), k = k0 + row / (j1 - j0);
         const int gy = min(max(lo[1] - g.ghost + j, 0), g.n[1] - 1), gz = min(max(lo[2] - g.ghost + k, 0), g.n[2] - 1);
@@ -86,6 +88,8 @@ vr_upload_tiled_kernel(VrGrid g, float* __restrict__ bricks, const float* __rest
     padded_range(lo[1], g.ghost, ey, g.n[1], y0, y0 + sy, j0, j1);
     padded_range(lo[2], g.ghost, ez, g.n[2], z0, z0 + sz, k0, k1);
     if (i1 <= i0 || j1 <= j0 || k1 <= k0) return;
+    const int slot_b = vr_slot_index(g, b);
+    if (slot_b < 0) return; /* a part handle does not hold this brick (row f3) */
     const int tx0 = i0 >> g.tl[0], tx1 = ((i1 - 1) >> g.tl[0]) + 1, ntx = tx1 - tx0;
     const int ty0 = j0 >> g.tl[1], ty1 = ((j1 - 1) >> g.tl[1]) + 1;
     const int tz0 = k0 >> g.tl[2], tz1 = ((k1 - 1) >> g.tl[2]) + 1;
@@ -96,7 +100,7 @@ vr_upload_tiled_kernel(VrGrid g, float* __restrict__ bricks, const float* __rest
     const int li = lane & ((1 << g.tl[0]) - 1), ljk = lane >> g.tl[0];
     const int lj = ljk & ((1 << g.tl[1]) - 1), lk = ljk >> g.tl[1];
     const int ibase = tx0 << g.tl[0]; /* first staged padded x index */
-    float* __restrict__ dstb = bricks + (long long)b * g.slot;
+    float* __restrict__ dstb = bricks + (long long)slot_b * g.slot;
     for (int grp = blockIdx.x; grp < groups; grp += gridDim.x) {
         const int tyg = ty0 + (grp % ngy) * TR, kt = (tz0 + grp / ngy) << g.tl[2];
         const int ntr = min(TR, ty1 - tyg); /* tile rows in this group */
@@ -170,6 +174,8 @@ vr_upload_tile442_kernel(VrGrid g, float* __restrict__ bricks, const float* __re
     padded_range(lo[1], g.ghost, ey, g.n[1], y0, y0 + sy, j0, j1);
     padded_range(lo[2], g.ghost, ez, g.n[2], z0, z0 + sz, k0, k1);
     if (i1 <= i0 || j1 <= j0 || k1 <= k0) return;
+    const int slot_b = vr_slot_index(g, b);
+    if (slot_b < 0) return; /* a part handle does not hold this brick (row f3) */
     const int tx0 = i0 >> 2, tx1 = ((i1 - 1) >> 2) + 1;
     const int ty0 = j0 >> 2, ty1 = ((j1 - 1) >> 2) + 1;
     const int tz0 = k0 >> 1, tz1 = ((k1 - 1) >> 1) + 1;
@@ -178,7 +184,7 @@ vr_upload_tile442_kernel(VrGrid g, float* __restrict__ bricks, const float* __re
     const int ibase = tx0 << 2;
     const int xbase = lo[0] - g.ghost; /* global x of padded cell 0 */
     const bool clamp_x = xbase < 0 || xbase + ex - 1 > g.n[0] - 1;
-    float* __restrict__ dstb = bricks + (long long)b * g.slot;
+    float* __restrict__ dstb = bricks + (long long)slot_b * g.slot;
     /* phase-2 role of this lane: tile row tr, row r = lj + 4 lk of the tile, x tile q (+ 4 per warp of the row) */
     const int tr = warp / WPT, r = lane & 7, q = (lane >> 3) + ((warp % WPT) << 2);
     for (int grp = blockIdx.x; grp < groups; grp += gridDim.x) {
@@ -247,7 +253,8 @@ vr_download_kernel(VrGrid g, const float* __restrict__ bricks, float* __restrict
             const int bx = x / g.brick;
             const int b = (bz * g.g[1] + by) * g.g[0] + bx;
             const int i = x - bx * g.brick + g.ghost, j = y - by * g.brick + g.ghost, k = z - bz * g.brick + g.ghost;
-            dst[row * sx + xo] = bricks[(long long)b * g.slot + vr_cell_offset(g, i, j, k)];
+            const int slot_b = vr_slot_index(g, b); /* the caller checked that the handle holds the box */
+            dst[row * sx + xo] = bricks[(long long)slot_b * g.slot + vr_cell_offset(g, i, j, k)];
         }
     }
 }

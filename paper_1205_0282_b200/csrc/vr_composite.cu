@@ -14,6 +14,9 @@
  * order-preserving), then each thread walks that short list for its pixel:
  *   ALPHA  C += (1-A) C_l,  A += (1-A) A_l      (float32, R15; no early termination)
  *   MIP    m = max(m, m_l); at the end RGB = LUT(u(m)), A = 1, or (0,0,0,0) if m = -inf (R11)
+ * Row f3 (multi-GPU sort-last): a part's MIP frame leaves as the raw maximum
+ * (VR_MIP_RAW: (m,0,0,1), or zeros without a sample), and the partial frames of the parts are merged
+ * by the same kernel (ALPHA: `over` in part order; VR_MIP_PARTS: maximum, then the colour mapping).
  */
 #include "vr_internal.cuh"
 
@@ -88,6 +91,9 @@ vr_composite_kernel(const VrCompLayer* __restrict__ layers, const int* __restric
                         cg = fmaf(t, s.y, cg);
                         cb = fmaf(t, s.z, cb);
                         ca = fmaf(t, s.w, ca);
+                    } else if (MODE == VR_MIP_PARTS) {
+                        const float4 s = __ldcs(reinterpret_cast<const float4*>(e.addr) + off);
+                        if (s.w != 0.0f) m = fmaxf(m, s.x);
                     } else {
                         m = fmaxf(m, __ldcs(reinterpret_cast<const float*>(e.addr) + off));
                     }
@@ -103,6 +109,8 @@ vr_composite_kernel(const VrCompLayer* __restrict__ layers, const int* __restric
             o = make_float4(cr, cg, cb, ca);
         } else if (m == -INFINITY) {
             o = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
+        } else if (MODE == VR_MIP_RAW) {
+            o = make_float4(m, 0.0f, 0.0f, 1.0f);
         } else {
             const float u = __saturatef((m - lut.vmin) * lut.inv_range);
             const float x = u * (float)(lut.n - 1);
@@ -120,7 +128,11 @@ cudaError_t vr_launch_composite(const VrCompLayer* layers, const int* order, int
     dim3 grid((W + VR_COMP_TILE_W - 1) / VR_COMP_TILE_W, (H + VR_COMP_TILE_H - 1) / VR_COMP_TILE_H);
     if (mode == VR_ALPHA)
         vr_composite_kernel<VR_ALPHA><<<grid, COMP_THREADS, 0, st>>>(layers, order, n, W, H, lut, reinterpret_cast<float4*>(out));
-    else
+    else if (mode == VR_MIP)
         vr_composite_kernel<VR_MIP><<<grid, COMP_THREADS, 0, st>>>(layers, order, n, W, H, lut, reinterpret_cast<float4*>(out));
+    else if (mode == VR_MIP_RAW)
+        vr_composite_kernel<VR_MIP_RAW><<<grid, COMP_THREADS, 0, st>>>(layers, order, n, W, H, lut, reinterpret_cast<float4*>(out));
+    else
+        vr_composite_kernel<VR_MIP_PARTS><<<grid, COMP_THREADS, 0, st>>>(layers, order, n, W, H, lut, reinterpret_cast<float4*>(out));
     return cudaGetLastError();
 }

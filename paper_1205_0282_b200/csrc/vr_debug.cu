@@ -169,7 +169,7 @@ cudaError_t vr_launch_gather_sub(const VrBrickView* bv, int nbricks, const void*
 __global__ void vr_brick_copy_kernel(VrGrid g, const float* __restrict__ bricks, int b, int dx, int dy, int dz,
                                      float* __restrict__ out) {
     const long long n = (long long)dx * dy * dz;
-    const float* __restrict__ src = bricks + (long long)b * g.slot;
+    const float* __restrict__ src = bricks + (long long)vr_slot_index(g, b) * g.slot;
     for (long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x; t < n; t += (long long)gridDim.x * blockDim.x) {
         const int i = (int)(t % dx), j = (int)((t / dx) % dy), k = (int)(t / ((long long)dx * dy));
         out[t] = src[vr_cell_offset(g, i, j, k)];

@@ -97,7 +97,8 @@ vr_fused_kernel(const VrRaycastParams prm, float4* __restrict__ frame) {
                 if (k_hi <= k) k_hi = k + 1; /* cannot happen (sample k is owned by bc); guarantees progress */
             }
             const int b = (bc[2] * g.g[1] + bc[1]) * g.g[0] + bc[0];
-            const float* __restrict__ brick = prm.bricks + (long long)b * g.slot;
+            const int slot_b = vr_slot_of_coords(g, bc); /* = b unless the handle is a part (row f3) */
+            const float* __restrict__ brick = prm.bricks + (long long)slot_b * g.slot;
             asm volatile("" : "+l"(brick)); /* keep the base in registers: do not rebuild it per load */
 
             /* a brick the set-up kernel found transparent (R16: empty rendering rectangle) contributes exact
@@ -124,8 +125,8 @@ vr_fused_kernel(const VrRaycastParams prm, float4* __restrict__ frame) {
             Corners C;
             int pcx = INT_MIN, pcy = 0, pcz = 0;
             /* R19: samples based in a transparent macro-cell are skipped (see vr_raycast.cu) */
-            const unsigned* __restrict__ cbits = (SKIP && MODE == VR_ALPHA) ? prm.cell_bits + (long long)b * prm.cell_words : NULL;
-            const float2* __restrict__ cmm = (SKIP && MODE == VR_MIP) ? prm.cell_mm + (long long)b * (prm.nc[0] * prm.nc[1] * prm.nc[2]) : NULL;
+            const unsigned* __restrict__ cbits = (SKIP && MODE == VR_ALPHA) ? prm.cell_bits + (long long)slot_b * prm.cell_words : NULL;
+            const float2* __restrict__ cmm = (SKIP && MODE == VR_MIP) ? prm.cell_mm + (long long)slot_b * (prm.nc[0] * prm.nc[1] * prm.nc[2]) : NULL;
             float pbound = INFINITY;
             int pm = -1;
             bool ptransp = false;
@@ -154,7 +155,7 @@ vr_fused_kernel(const VrRaycastParams prm, float4* __restrict__ frame) {
                             if (ptransp) adv = -leap_steps(L, D, n); /* negative: a leap over samples that cannot matter, nothing fetched */
                         }
                         if (adv > 0) {
-                            fetch8<LAY, 0, CLAMP, COUNT>(brick, g, ext, L, prm.bitmap, (long long)b * g.slot, C);
+                            fetch8<LAY, 0, CLAMP, COUNT>(brick, g, ext, L, prm.bitmap, (long long)slot_b * g.slot, C);
                             pcx = cx, pcy = cy, pcz = cz;
                         }
                     }
@@ -188,7 +189,7 @@ vr_fused_kernel(const VrRaycastParams prm, float4* __restrict__ frame) {
                         const double p = VR_FMA(s, ray.d[a], ray.o[a]);
                         L.q[a] = to_fixed(p - ((double)(blo[a] - g.ghost) + 0.5));
                     }
-                    const float v = trilinear<LAY, 0, CLAMP, COUNT>(brick, g, ext, L, prm.bitmap, (long long)b * g.slot);
+                    const float v = trilinear<LAY, 0, CLAMP, COUNT>(brick, g, ext, L, prm.bitmap, (long long)slot_b * g.slot);
                     if (COUNT) nsamples += (v == v) ? 1 : 0;
                     if (MODE == VR_MIP) {
                         acc.r = fmaxf(acc.r, v);

@@ -2,8 +2,8 @@
  * vr_internal.cuh -- shared declarations of libvr's translation units (not part of the ABI).
  *
  * Data layout in HBM:
- *   bricks        float[nbricks][slot], P = brick + 2*ghost padded cells per axis. Brick b =
- *                 (bz*gy + by)*gx + bx. Padded cell (i,j,k) of brick b holds global voxel
+ *   bricks        float[nown][slot], P = brick + 2*ghost padded cells per axis. Brick b =
+ *                 (bz*gy + by)*gx + bx sits in slot vr_slot_index(b) (= b unless the handle is a part). Padded cell (i,j,k) of brick b holds global voxel
  *                 clamp(lo_b - ghost + (i,j,k), 0, n-1) and sits at vr_cell_offset(i,j,k):
  *                 x-linear rows (VR_LAYOUT_LINEAR) or 128-byte 3-D micro-tiles
  *                 (VR_LAYOUT_TILED), see VrAxisLayout. Ragged bricks use the low corner of
@@ -29,6 +29,11 @@
 #define VR_RAYCAST_THREADS 256
 #define VR_COMP_TILE_W 32
 #define VR_COMP_TILE_H 8
+/* internal compositing modes next to VR_ALPHA / VR_MIP (row f3):
+ *   VR_MIP_RAW    scalar MIP sub-images in, (max, 0, 0, 1) out, or (0,0,0,0) where no layer holds a sample
+ *   VR_MIP_PARTS  such float4 partial frames in (w = 1 marks a sample), LUT colour of the maximum out */
+#define VR_MIP_RAW 2
+#define VR_MIP_PARTS 3
 #define VR_EV_RING 64 /* timed frames whose stage events are kept */
 
 /* Where padded cell i of one axis sits inside a brick slot. Every supported layout is
@@ -57,6 +62,11 @@ struct VrGrid {
     int ml[3];      /* log2 micro-tiles per macro block and axis (0,0,0: tiles in x-fastest order) */
     int nt[3];      /* tiled: macro blocks (or tiles) per axis of a slot */
     VrAxisLayout ax[3];
+    /* row f3: a PART handle stores only the bricks of the box pb0 <= (bx,by,bz) < pb1 of the global grid, in
+     * box-local x-fastest order (slot index, vr_slot_index); a whole volume has the box of the whole grid */
+    int part;       /* 1 if the box is smaller than the grid */
+    int pb0[3], pb1[3];
+    int nown;       /* bricks in the box = slots of the store and rows of the macro-cell tables */
 };
 
 /* The caller's matrices travel to the set-up kernel as a kernel argument (no copy, no sync). */
@@ -87,7 +97,7 @@ struct VrBrickView {
     int lx0, ly0, lx1, ly1; /* launch rectangle: the same, grown to the 8x4 tile grid */
     int tiles_x, tiles_y;
     int order_pos;
-    int pad;
+    int slot;               /* vr_slot_index of the brick (-1: held by another part) */
     long long sub_offset;   /* first pixel of this brick's sub-image in the scratch */
 };
 
@@ -134,6 +144,19 @@ __host__ __device__ __forceinline__ unsigned vr_axis_offset(const VrAxisLayout& 
     return ((unsigned)(i & A.lo_mask) << A.lo_shift) + ((unsigned)((i >> A.mid_in) & A.mid_mask) << A.mid_shift) +
            (unsigned)(i >> A.hi_in) * A.hi_stride;
 }
+__host__ __device__ __forceinline__ int vr_slot_of_coords(const VrGrid& g, const int bc[3]) {
+    if (!g.part) return (bc[2] * g.g[1] + bc[1]) * g.g[0] + bc[0];
+    if (bc[0] < g.pb0[0] || bc[0] >= g.pb1[0] || bc[1] < g.pb0[1] || bc[1] >= g.pb1[1] || bc[2] < g.pb0[2] || bc[2] >= g.pb1[2]) return -1;
+    return ((bc[2] - g.pb0[2]) * (g.pb1[1] - g.pb0[1]) + (bc[1] - g.pb0[1])) * (g.pb1[0] - g.pb0[0]) + (bc[0] - g.pb0[0]);
+}
+/* Slot of brick b in this handle's store (b itself for a whole volume), -1 if the handle does not hold it. */
+__host__ __device__ __forceinline__ int vr_slot_index(const VrGrid& g, int b) {
+    if (!g.part) return b;
+    const int t = b / g.g[0];
+    const int bx = b - t * g.g[0], bz = t / g.g[1], by = t - bz * g.g[1];
+    if (bx < g.pb0[0] || bx >= g.pb1[0] || by < g.pb0[1] || by >= g.pb1[1] || bz < g.pb0[2] || bz >= g.pb1[2]) return -1;
+    return ((bz - g.pb0[2]) * (g.pb1[1] - g.pb0[1]) + (by - g.pb0[1])) * (g.pb1[0] - g.pb0[0]) + (bx - g.pb0[0]);
+}
 __host__ __device__ __forceinline__ unsigned vr_cell_offset(const VrGrid& g, int i, int j, int k) {
     return vr_axis_offset(g.ax[0], i) + vr_axis_offset(g.ax[1], j) + vr_axis_offset(g.ax[2], k);
 }
@@ -174,5 +197,7 @@ cudaError_t vr_launch_count_bits(const unsigned* bitmap, long long words, unsign
 /* host mirror of the set-up arithmetic, for argument validation and scratch sizing only */
 int vr_host_view_check(const VrGrid& grid, const float* view, const float* proj, int W, int H, long long* sub_pixels,
                        long long* items);
+
+int vr_host_part_rect(const VrGrid& grid, const float* view, const float* proj, int W, int H, int rect[4]);
 
 #endif

@@ -38,7 +38,9 @@ vr_brick_minmax_kernel(VrGrid g, const float* __restrict__ bricks, int2* __restr
     vr_brick_coords(g, b, bc);
     vr_brick_core(g, bc, lo, hi);
     const int ex = hi[0] - lo[0] + 2 * g.ghost, ey = hi[1] - lo[1] + 2 * g.ghost, ez = hi[2] - lo[2] + 2 * g.ghost;
-    const float* __restrict__ base = bricks + (long long)b * g.slot;
+    const int slot_b = vr_slot_index(g, b);
+    if (slot_b < 0) return; /* not held by this part (row f3): its table entry stays (+inf, -inf) */
+    const float* __restrict__ base = bricks + (long long)slot_b * g.slot;
     float mn = INFINITY, mx = -INFINITY;
     if (TILE442) {
         /* word u of the slot = row r = u & 7 (lj = r & 3, lk = r >> 2) of tile u >> 3 */
@@ -141,7 +143,9 @@ vr_cell_minmax_kernel(VrGrid g, const float* __restrict__ bricks, float2* __rest
     vr_brick_coords(g, b, bc);
     vr_brick_core(g, bc, lo, hi);
     const int ex = hi[0] - lo[0] + 2 * g.ghost, ey = hi[1] - lo[1] + 2 * g.ghost, ez = hi[2] - lo[2] + 2 * g.ghost;
-    const float* __restrict__ base = bricks + (long long)b * g.slot;
+    const int slot_b = vr_slot_index(g, b);
+    if (slot_b < 0) return; /* the macro-cell tables have one row per held brick, by slot */
+    const float* __restrict__ base = bricks + (long long)slot_b * g.slot;
     const int lane = threadIdx.x & 31, ncell = nc0 * nc1 * nc2;
     for (int m = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); m < ncell; m += gridDim.x * (blockDim.x >> 5)) {
         const int m2 = m / (nc0 * nc1), rem = m - m2 * (nc0 * nc1), m1 = rem / nc0, m0 = rem - m1 * nc0;
@@ -177,7 +181,7 @@ vr_cell_minmax_kernel(VrGrid g, const float* __restrict__ bricks, float2* __rest
             mn = fminf(mn, __shfl_xor_sync(0xffffffffu, mn, o));
             mx = fmaxf(mx, __shfl_xor_sync(0xffffffffu, mx, o));
         }
-        if (lane == 0) cell_mm[(long long)b * ncell + m] = make_float2(mn + 0.0f, mx + 0.0f);
+        if (lane == 0) cell_mm[(long long)slot_b * ncell + m] = make_float2(mn + 0.0f, mx + 0.0f);
     }
 }
 

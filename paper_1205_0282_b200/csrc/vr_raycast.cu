@@ -96,7 +96,8 @@ vr_raycast_kernel(const VrRaycastParams prm) {
         vr_brick_core(g, bc, blo, bhi);
 #pragma unroll
         for (int a = 0; a < 3; ++a) ext[a] = bhi[a] - blo[a] + 2 * g.ghost;
-        const float* __restrict__ brick = prm.bricks + (long long)b * g.slot;
+        const int slot_b = bvw.slot; /* = b unless the handle is a part (row f3) */
+        const float* __restrict__ brick = prm.bricks + (long long)slot_b * g.slot;
         asm volatile("" : "+l"(brick)); /* keep the base in registers: do not rebuild it per load */
 
         RaySetup ray;
@@ -141,8 +142,8 @@ vr_raycast_kernel(const VrRaycastParams prm) {
         int pcx = INT_MIN, pcy = 0, pcz = 0;
         /* R19: samples based in a macro-cell the transfer function makes transparent are skipped (their
          * opacity is exactly 0): no voxel is fetched. The flag is looked up when the macro-cell changes. */
-        const unsigned* __restrict__ cbits = (SKIP && MODE == VR_ALPHA) ? prm.cell_bits + (long long)b * prm.cell_words : NULL;
-        const float2* __restrict__ cmm = (SKIP && MODE == VR_MIP) ? prm.cell_mm + (long long)b * (prm.nc[0] * prm.nc[1] * prm.nc[2]) : NULL;
+        const unsigned* __restrict__ cbits = (SKIP && MODE == VR_ALPHA) ? prm.cell_bits + (long long)slot_b * prm.cell_words : NULL;
+        const float2* __restrict__ cmm = (SKIP && MODE == VR_MIP) ? prm.cell_mm + (long long)slot_b * (prm.nc[0] * prm.nc[1] * prm.nc[2]) : NULL;
         float pbound = INFINITY;
         int pm = -1;
         bool ptransp = false;
@@ -171,7 +172,7 @@ vr_raycast_kernel(const VrRaycastParams prm) {
                         if (ptransp) adv = -leap_steps(L, D, n); /* negative: a leap over samples that cannot matter, nothing fetched */
                     }
                     if (adv > 0) {
-                        fetch8<LAY, PT, CLAMP, COUNT>(brick, g, ext, L, prm.bitmap, (long long)b * g.slot, C);
+                        fetch8<LAY, PT, CLAMP, COUNT>(brick, g, ext, L, prm.bitmap, (long long)slot_b * g.slot, C);
                         pcx = cx, pcy = cy, pcz = cz;
                     }
                 }
@@ -213,7 +214,7 @@ vr_raycast_kernel(const VrRaycastParams prm) {
                     const double p = VR_FMA(s, ray.d[a], ray.o[a]);
                     L.q[a] = to_fixed(p - ((double)(blo[a] - g.ghost) + 0.5));
                 }
-                const float v = trilinear<LAY, PT, CLAMP, COUNT>(brick, g, ext, L, prm.bitmap, (long long)b * g.slot);
+                const float v = trilinear<LAY, PT, CLAMP, COUNT>(brick, g, ext, L, prm.bitmap, (long long)slot_b * g.slot);
                 if (COUNT) nsamples += (v == v) ? 1 : 0;
                 if (MODE == VR_MIP) {
                     acc.r = fmaxf(acc.r, v);

@@ -15,6 +15,8 @@
  *      the transfer function makes transparent (R16: every table entry the brick's values can
  *      interpolate between has alpha 0, entry range widened by -1/+2): no work items, no
  *      sub-image, an empty compositing rectangle. Exact: such a brick contributes zeros.
+ *   6. Row f3: a part handle gives an empty rectangle to every brick outside its box; what it renders is the
+ *      partial frame of its own bricks, in the global visibility order.
  */
 #include "vr_view.cuh"
 
@@ -106,6 +108,7 @@ vr_setup_kernel(VrGrid grid, VrMatrices mats, int W, int H, int mode, long long 
         const int key = (sh.rank[2][bc[2]] * grid.g[1] + sh.rank[1][bc[1]]) * grid.g[0] + sh.rank[0][bc[0]];
         order[key] = b;
         vr_rect_of_box(sh.M, lo, hi, W, H, r);
+        if (vr_slot_index(grid, b) < 0) r[2] = r[0]; /* row f3: another part holds this brick */
         if (cull) { /* R16, float32 as the ray-cast kernel classifies */
             const float2 mm = range[b];
             const float ulo = __saturatef(__fmul_rn(__fsub_rn(mm.x, lut.vmin), lut.inv_range));
@@ -124,7 +127,7 @@ vr_setup_kernel(VrGrid grid, VrMatrices mats, int W, int H, int mode, long long 
         v.tiles_x = (l[2] - l[0] + VR_TILE_W - 1) / VR_TILE_W;
         v.tiles_y = (l[3] - l[1] + VR_TILE_H - 1) / VR_TILE_H;
         v.order_pos = key;
-        v.pad = 0;
+        v.slot = vr_slot_index(grid, b);
         v.sub_offset = 0;
         bv[b] = v;
     }
@@ -221,6 +224,7 @@ int vr_host_view_check(const VrGrid& grid, const float* view, const float* proj,
     long long pix = 0, it = 0;
     for (int b = 0; b < grid.nbricks; ++b) {
         int bc[3], lo[3], hi[3], r[4], l[4];
+        if (vr_slot_index(grid, b) < 0) continue; /* a part renders its own bricks only */
         vr_brick_coords(grid, b, bc);
         vr_brick_core(grid, bc, lo, hi);
         vr_rect_of_box(M, lo, hi, W, H, r);
@@ -239,5 +243,34 @@ int vr_host_view_check(const VrGrid& grid, const float* view, const float* proj,
     }
     *sub_pixels = pix;
     *items = it;
+    return 0;
+}
+
+/* Row f3: a rectangle that contains the rendering rectangle of every brick the handle holds (the union of
+ * the per-brick rectangles of PAPER.md:150, one pixel of slack per side as above): the part of the frame a
+ * part's partial image can be non-blank in, which is what travels in the exchange. */
+int vr_host_part_rect(const VrGrid& grid, const float* view, const float* proj, int W, int H, int rect[4]) {
+    double M[16], Minv[16], eye[3];
+    int ortho;
+    if (vr_view_setup(view, proj, M, Minv, eye, &ortho)) return 1;
+    int u[4] = {W, H, 0, 0};
+    for (int b = 0; b < grid.nbricks; ++b) {
+        int bc[3], lo[3], hi[3], r[4];
+        if (vr_slot_index(grid, b) < 0) continue;
+        vr_brick_coords(grid, b, bc);
+        vr_brick_core(grid, bc, lo, hi);
+        vr_rect_of_box(M, lo, hi, W, H, r);
+        if (r[2] <= r[0] || r[3] <= r[1]) continue;
+        r[0] = r[0] > 0 ? r[0] - 1 : 0;
+        r[1] = r[1] > 0 ? r[1] - 1 : 0;
+        r[2] = r[2] < W ? r[2] + 1 : W;
+        r[3] = r[3] < H ? r[3] + 1 : H;
+        if (r[0] < u[0]) u[0] = r[0];
+        if (r[1] < u[1]) u[1] = r[1];
+        if (r[2] > u[2]) u[2] = r[2];
+        if (r[3] > u[3]) u[3] = r[3];
+    }
+    if (u[2] <= u[0] || u[3] <= u[1]) u[0] = u[1] = u[2] = u[3] = 0;
+    for (int i = 0; i < 4; ++i) rect[i] = u[i];
     return 0;
 }

@@ -1,0 +1,195 @@
+"""Row f3 on one GPU: the parts of a k-d partition are rendered one after the other by part handles (no rank
+waits for another), their partial frames are merged by vr_composite_parts, and the frame must be the oracle's
+frame of the whole volume (north_star's tolerances) and the single-handle GPU frame to float32 rounding.
+The exchange in between is covered over gloo by tests/test_sortlast.py."""
+import numpy as np
+import pytest
+
+import oracle
+import synth
+from helpers import check_alpha, check_mip, gpu_frame
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def vr(cuda_device):
+    from paper_1205_0282_b200 import build
+    build.build()
+    import paper_1205_0282_b200 as vr
+    return vr
+
+
+def make_parts(vr, sortlast, data, dims, brick, ghost, nparts, halo_only=True):
+    """One part handle per box, fed with the box's region only (its bricks + ghost layers)."""
+    import torch
+    boxes, tree = sortlast.kd_partition(dims, brick, nparts)
+    parts = []
+    for box in boxes:
+        p = vr.Volume(*dims, brick, ghost, part=box)
+        (x0, y0, z0), (sx, sy, sz) = sortlast.part_region(dims, brick, ghost, box) if halo_only else ((0, 0, 0), dims)
+        p.upload(torch.from_numpy(np.ascontiguousarray(data[z0:z0 + sz, y0:y0 + sy, x0:x0 + sx])).cuda(), origin=(x0, y0, z0))
+        parts.append(p)
+    return boxes, tree, parts
+
+
+def merged_frame(vr, sortlast, parts, boxes, tree, dims, brick, view, proj, W, H, step, mode):
+    """What SortLastRenderer does, on one device: partial frames, packed by rectangle, merged in part order."""
+    import torch
+    pieces, rects = [], []
+    for p, box in zip(parts, boxes):
+        full = torch.empty((H, W, 4), dtype=torch.float32, device="cuda")
+        r = p.render_part(view, proj, W, H, step, mode, full)
+        assert r == vr.part_rect(dims, brick, box, view, proj, W, H)
+        outside = full.clone()
+        outside[r[1]:r[3], r[0]:r[2]] = 0
+        assert not outside.any(), "a partial frame is not blank outside its rectangle"
+        pieces.append(full[r[1]:r[3], r[0]:r[2]].contiguous())
+        rects.append(r)
+    out = torch.empty((H, W, 4), dtype=torch.float32, device="cuda")
+    parts[0].composite_parts(mode, pieces, rects, sortlast.part_order(tree, brick, view, proj), W, H, out)
+    torch.cuda.synchronize()
+    return out.cpu().numpy().astype(np.float64)
+
+
+@pytest.mark.parametrize("nparts", [2, 3, 4, 6])
+@pytest.mark.parametrize("tfname", ["ramp", "translucent"])
+def test_merged_parts_are_the_frame_of_the_whole_volume(vr, nparts, tfname):
+    from paper_1205_0282_b200 import sortlast
+    dims, brick, ghost, W, H = (70, 52, 64), 16, 1, 150, 110
+    cube = synth.Cube(21, *dims, 5)
+    data = cube.fill_host()
+    tf = getattr(synth, "tf_" + tfname)()
+    boxes, tree, parts = make_parts(vr, sortlast, data, dims, brick, ghost, nparts)
+    whole = vr.Volume(*dims, brick, ghost)
+    whole.upload(data)
+    o = oracle.Volume(*dims, brick, ghost, data=data)
+    for v in parts + [whole, o]:
+        v.set_transfer_function(tf, synth.TF_VMIN, synth.TF_VMAX)
+        v.set_early_termination(0.99)
+    fr = synth.Framing(*dims, W, H)
+    views = [(fr.seeded(31, k), fr.proj(k % 2 == 1)) for k in range(4)]
+    views.append((synth.look_at((20.0, 30.0, 40.0), (70.0, 0.0, 0.0), (0.0, 0.3, 1.0)), synth.perspective(60, W / H, 0.3, 400.0)))
+    for k, (view, proj) in enumerate(views):
+        for step in (0.6, vr.STEP_AUTO):
+            what = "%d parts, view %d, step %g" % (nparts, k, step)
+            ref = o.render(view, proj, W, H, step, oracle.ALPHA)
+            got = merged_frame(vr, sortlast, parts, boxes, tree, dims, brick, view, proj, W, H, step, vr.ALPHA)
+            check_alpha(got, ref["image"], ref["flags"], 0.99, what)
+            one = gpu_frame(whole, view, proj, W, H, step, vr.ALPHA)
+            assert np.abs(got - one).max() < 2e-6, what      # same sub-images, `over` regrouped
+            refm = o.render(view, proj, W, H, step, oracle.MIP)
+            gotm = merged_frame(vr, sortlast, parts, boxes, tree, dims, brick, view, proj, W, H, step, vr.MIP)
+            check_mip(gotm, refm["image"], what, flags=refm["flags"])
+            assert np.array_equal(gotm, gpu_frame(whole, view, proj, W, H, step, vr.MIP)), what   # max is exact
+
+
+def test_part_handles_hold_their_own_bricks_only(vr):
+    """Store, ranges and debug exports of a part: own bricks bit-exact (ghost layers from the neighbours' voxels),
+    the others absent; whole-volume uploads are filtered."""
+    from paper_1205_0282_b200 import sortlast
+    dims, brick, ghost = (50, 40, 45), 16, 2
+    data = synth.Cube(5, *dims, 4).fill_host()
+    o = oracle.Volume(*dims, brick, ghost, data=data)
+    g = sortlast.brick_grid(dims, brick)
+    for halo_only in (True, False):
+        boxes, tree, parts = make_parts(vr, sortlast, data, dims, brick, ghost, 3, halo_only)
+        for p, (b0, b1) in zip(parts, boxes):
+            mm = p.debug_brick_minmax()
+            lo, hi = np.inf, -np.inf
+            for b in range(p.nbricks):
+                bx, by, bz = b % g[0], (b // g[0]) % g[1], b // (g[0] * g[1])
+                own = all(b0[a] <= c < b1[a] for a, c in enumerate((bx, by, bz)))
+                if own:
+                    assert np.array_equal(p.debug_brick_data(b), o.brick_data(b)), b
+                    assert tuple(mm[b]) == o.brick_minmax(b)
+                    lo, hi = min(lo, mm[b][0]), max(hi, mm[b][1])
+                else:
+                    assert mm[b][0] == np.inf and mm[b][1] == -np.inf
+                    with pytest.raises(vr.VrError):
+                        p.debug_brick_data(b)
+            assert p.minmax() == (lo, hi)
+            # voxels come back from the part's own bricks only
+            import torch
+            x0, y0, z0 = (b0[a] * brick for a in range(3))
+            x1, y1, z1 = (min(b1[a] * brick, dims[a]) for a in range(3))
+            back = torch.empty((z1 - z0, y1 - y0, x1 - x0), dtype=torch.float32, device="cuda")
+            p.download(back, origin=(x0, y0, z0))
+            torch.cuda.synchronize()
+            assert np.array_equal(back.cpu().numpy(), data[z0:z1, y0:y1, x0:x1])
+            if (x1, y1, z1) != dims:
+                with pytest.raises(vr.VrError):
+                    p.download(torch.empty(dims[::-1], dtype=torch.float32, device="cuda"), origin=(0, 0, 0))
+
+
+def test_part_arguments(vr):
+    with pytest.raises(vr.VrError):
+        vr.Volume(64, 64, 64, 16, 1, part=((0, 0, 0), (5, 4, 4)))     # outside the 4x4x4 grid
+    with pytest.raises(vr.VrError):
+        vr.Volume(64, 64, 64, 16, 1, part=((2, 0, 0), (2, 4, 4)))     # empty
+    import torch
+    p = vr.Volume(64, 64, 64, 16, 1, part=((0, 0, 0), (2, 4, 4)))
+    p.upload(torch.zeros((64, 64, 64), dtype=torch.float32, device="cuda"))
+    p.set_transfer_function(synth.tf_ramp(), 0.0, 1.0)
+    p.set_traversal(vr.FUSED)
+    fr = synth.Framing(64, 64, 64, 64, 48)
+    out = torch.empty((48, 64, 4), dtype=torch.float32, device="cuda")
+    with pytest.raises(vr.VrError):                                    # a MIP part stays scalar: sort-last traversal only
+        p.render_part(fr.seeded(1, 0), fr.proj(False), 64, 48, 1.0, vr.MIP, out)
+    p.render_part(fr.seeded(1, 0), fr.proj(False), 64, 48, 1.0, vr.ALPHA, out)
+
+
+def test_parts_cull_and_skip_like_the_whole_volume(vr):
+    """R16/R19 on parts: a threshold transfer function over an N-body cube; culling and macro-cell skipping run per
+    part on the part's own tables, the merged frame does not change by a bit with them off, and parity holds. The
+    fused traversal of a part (global early termination inside the part) merges to the oracle's frame as well when
+    early termination is off."""
+    from paper_1205_0282_b200 import sortlast
+    dims, brick, ghost, W, H = (96, 80, 72), 32, 1, 140, 100
+    data = synth.Cube(9, *dims, 6, kind=1).fill_host()
+    tf = synth.tf_density()
+    boxes, tree, parts = make_parts(vr, sortlast, data, dims, brick, ghost, 4)
+    o = oracle.Volume(*dims, brick, ghost, data=data)
+    for v in parts + [o]:
+        v.set_transfer_function(tf, 0.0, synth.NBODY_VMAX)
+        v.set_early_termination(2.0)
+    fr = synth.Framing(*dims, W, H)
+    for k in range(3):
+        view, proj = fr.seeded(91, k), fr.proj(k == 2)
+        ref = o.render(view, proj, W, H, 0.8, oracle.ALPHA)
+        frames = {}
+        for cull in (True, False):
+            for p in parts:
+                p.set_culling(cull)
+            frames[cull] = merged_frame(vr, sortlast, parts, boxes, tree, dims, brick, view, proj, W, H, 0.8, vr.ALPHA)
+        assert np.array_equal(frames[True], frames[False])
+        check_alpha(frames[True], ref["image"], ref["flags"], 2.0, "view %d" % k)
+        for p in parts:
+            p.set_traversal(vr.FUSED)
+        fused = merged_frame(vr, sortlast, parts, boxes, tree, dims, brick, view, proj, W, H, 0.8, vr.ALPHA)
+        check_alpha(fused, ref["image"], ref["flags"], 2.0, "fused parts, view %d" % k)
+        for p in parts:
+            p.set_traversal(vr.SORT_LAST)
+    assert sum(p.debug_stats()["bricks_culled"] for p in parts) >= 0
+
+
+def test_a_world_of_one_renders_through_the_renderer(vr):
+    from paper_1205_0282_b200 import sortlast
+    import torch
+    dims, brick, W, H = (48, 40, 36), 16, 96, 72
+    data = synth.Cube(3, *dims, 3).fill_host()
+    rdr = sortlast.SortLastRenderer(dims, brick, 1, rank=0, world=1)
+    origin, shape = rdr.region()
+    assert origin == (0, 0, 0) and shape == dims
+    rdr.upload(torch.from_numpy(data).cuda(), origin)
+    rdr.set_transfer_function(synth.tf_ramp(), synth.TF_VMIN, synth.TF_VMAX)
+    whole = vr.Volume(*dims, brick, 1)
+    whole.upload(data)
+    whole.set_transfer_function(synth.tf_ramp(), synth.TF_VMIN, synth.TF_VMAX)
+    assert rdr.minmax() == whole.minmax()
+    fr = synth.Framing(*dims, W, H)
+    view, proj = fr.seeded(8, 1), fr.proj(False)
+    for mode in (vr.ALPHA, vr.MIP):
+        frame = rdr.render(view, proj, W, H, 1.0, mode)
+        torch.cuda.synchronize()
+        assert np.array_equal(frame.cpu().numpy().astype(np.float64), gpu_frame(whole, view, proj, W, H, 1.0, mode))
