@@ -176,6 +176,85 @@ def build_volume(vr, wl, tf):
     return g, cube
 
 
+def sortlast_report(vr, g, wl, cube, tf, nparts, order, K, Wm):
+    """Row f3 measured on ONE GPU, the parts one after the other (no rank waits for another): each part of the k-d
+    partition is created, filled with its region (bricks + ghost layers) and renders the K frames of the cycle as
+    partial frames (vr_render_part), one CUDA-event pair per frame; then the N partial frames of one view are merged
+    (vr_composite_parts, the work the N ranks share by stripes). The exchange itself needs N GPUs: its volume is
+    reported from the geometry (the paper's M + epsilon), not timed."""
+    import torch
+    from paper_1205_0282_b200 import sortlast
+    dims = (wl["nx"], wl["ny"], wl["nz"])
+    Wp, Hp = wl["width"], wl["height"]
+    boxes, tree = sortlast.kd_partition(dims, wl["brick"], nparts)
+    st = torch.cuda.current_stream().cuda_stream
+    out = torch.empty((Hp, Wp, 4), dtype=torch.float32, device="cuda")
+    K = min(K, 64)  # frames whose stage events the library keeps
+    frame_ms = np.zeros((nparts, K))
+    pieces, rects, store_gb, ray_ms = [], [], [], []
+    view0 = wl["views"][order[Wm % len(order)]]
+    for r, box in enumerate(boxes):
+        p = vr.Volume(*dims, wl["brick"], wl["ghost"], part=box)
+        (x0, y0, z0), (sx, sy, sz) = sortlast.part_region(dims, wl["brick"], wl["ghost"], box)
+        nzs = max(1, min(sz, (4 << 30) // (sx * sy * 4)))
+        buf = torch.empty((nzs, sy, sx), dtype=torch.float32, device="cuda")
+        for k0 in range(0, sz, nzs):
+            nk = min(nzs, sz - k0)
+            cube.fill_device(buf[:nk].data_ptr(), x0, y0, z0 + k0, sx, sy, nk, st)
+            p.upload(buf[:nk], origin=(x0, y0, z0 + k0))
+        torch.cuda.synchronize()
+        del buf
+        p.set_transfer_function(tf, *tf_range(wl))
+        p.set_early_termination(wl["tau"])
+        p.minmax()
+        for k in range(Wm):
+            p.render_part(wl["views"][order[k % len(order)]], wl["proj"], Wp, Hp, wl["step"], 0, out)
+        p.set_timing(1)  # the library's own stage events: device time of each frame's three kernels, no host gaps
+        torch.cuda.synchronize()
+        for k in range(K):
+            p.render_part(wl["views"][order[(Wm + k) % len(order)]], wl["proj"], Wp, Hp, wl["step"], 0, out)
+        torch.cuda.synchronize()
+        stg = p.debug_stage_times(K)
+        frame_ms[r] = stg.sum(axis=1)
+        ray_ms.append(round(float(stg[:, 1].mean()), 4))
+        p.set_timing(0)
+        rc = p.render_part(view0, wl["proj"], Wp, Hp, wl["step"], 0, out)
+        torch.cuda.synchronize()
+        pieces.append(out[rc[1]:rc[3], rc[0]:rc[2]].contiguous())
+        rects.append(rc)
+        nb = int(np.prod([box[1][a] - box[0][a] for a in range(3)]))
+        store_gb.append(round(nb * (wl["brick"] + 2 * wl["ghost"]) ** 3 * 4 / 1e9, 2))
+        p.close()
+        torch.cuda.empty_cache()
+    po = sortlast.part_order(tree, wl["brick"], view0, wl["proj"])
+    merged = torch.empty((Hp, Wp, 4), dtype=torch.float32, device="cuda")
+    for _ in range(3):
+        g.composite_parts(0, pieces, rects, po, Wp, Hp, merged)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(20):
+        g.composite_parts(0, pieces, rects, po, Wp, Hp, merged)
+    e1.record()
+    torch.cuda.synchronize()
+    merge_ms = e0.elapsed_time(e1) / 20
+    whole = torch.empty((Hp, Wp, 4), dtype=torch.float32, device="cuda")
+    g.render(view0, wl["proj"], Wp, Hp, wl["step"], 0, whole)
+    torch.cuda.synchronize()
+    rdr = sortlast.SortLastRenderer(dims, wl["brick"], wl["ghost"], backend=object(), rank=0, world=nparts)
+    moved = [rdr.exchange_bytes(wl["views"][v], wl["proj"], Wp, Hp) for v in sorted(set(order))]
+    slowest = frame_ms.max(axis=0)  # per frame: the part every other rank waits for
+    return {"parts": nparts, "boxes_bricks": [[b1[a] - b0[a] for a in range(3)] for b0, b1 in boxes], "store_gb_per_part": store_gb,
+            "part_frame_ms": {"mean": round(float(frame_ms.mean()), 4), "slowest_part_mean": round(float(slowest.mean()), 4),
+                              "per_part_mean": [round(float(x), 4) for x in frame_ms.mean(axis=1)], "per_part_raycast_mean": ray_ms},
+            "render_bound_frames_per_s": round(1e3 / float(slowest.mean()), 1),
+            "merge_ms_whole_frame": round(merge_ms, 4), "merge_launches": 1,
+            "merged_vs_single_handle_max_abs": float((merged - whole).abs().max()),
+            "exchange_bytes_per_frame": int(np.mean(moved)), "frame_bytes": Wp * Hp * 16,
+            "what": "one GPU, parts rendered one after the other; frame time of a part = device time of its set-up, ray-cast and "
+                    "stage-1 compositing kernels (stage events); render_bound_frames_per_s = 1 / mean over frames of the slowest "
+                    "part's frame time, before the exchange, which is not timed here"}
+
+
 def tf_range(wl):
     """Data range the transfer function spans: [-3, 10] sigma for the spectral cubes, [0, 20] for density cubes."""
     return (0.0, synth.NBODY_VMAX) if wl.get("kind", 0) == synth.NBODY else (synth.TF_VMIN, synth.TF_VMAX)
@@ -536,6 +615,8 @@ def main():
     ap.add_argument("--cells-every", type=int, default=6, help="count distinct cells on every n-th view of the cycle (0 = never)")
     ap.add_argument("--c4-part", default="both", choices=["both", "composite"],
                     help="--workload c4: `composite` runs only the compositing microbenchmark (profiling)")
+    ap.add_argument("--sortlast-parts", type=int, default=8,
+                    help="row f3 report: parts of the k-d partition rendered one after the other on this GPU (0 = skip)")
     ap.add_argument("--no-variants", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
@@ -697,6 +778,8 @@ def main():
                                                      traffic_of(args.workload, vmode, vtf + ("" if vtrav == "sort_last" else "/fused")))})
         g.set_transfer_function(tf, *tf_range(wl))
         line["variants"] = variants
+        if args.sortlast_parts > 1 and args.mode == "alpha":
+            line["sortlast"] = sortlast_report(vr, g, wl, cube, tf, args.sortlast_parts, order, K, Wm)
 
     if rank == 0 and not args.no_cpu_baseline and world == 1:
         g.close()
