@@ -176,6 +176,27 @@ def build_volume(vr, wl, tf):
     return g, cube
 
 
+def build_part(vr, wl, cube, tf, box):
+    """A part handle of the workload's cube (row f3), filled with its region (bricks + ghost layers) only."""
+    import torch
+    from paper_1205_0282_b200 import sortlast
+    dims = (wl["nx"], wl["ny"], wl["nz"])
+    st = torch.cuda.current_stream().cuda_stream
+    p = vr.Volume(*dims, wl["brick"], wl["ghost"], part=box)
+    (x0, y0, z0), (sx, sy, sz) = sortlast.part_region(dims, wl["brick"], wl["ghost"], box)
+    nzs = max(1, min(sz, (4 << 30) // (sx * sy * 4)))
+    buf = torch.empty((nzs, sy, sx), dtype=torch.float32, device="cuda")
+    for k0 in range(0, sz, nzs):
+        nk = min(nzs, sz - k0)
+        cube.fill_device(buf[:nk].data_ptr(), x0, y0, z0 + k0, sx, sy, nk, st)
+        p.upload(buf[:nk], origin=(x0, y0, z0 + k0))
+    torch.cuda.synchronize()
+    del buf
+    p.set_transfer_function(tf, *tf_range(wl))
+    p.set_early_termination(wl["tau"])
+    return p
+
+
 def sortlast_report(vr, g, wl, cube, tf, nparts, order, K, Wm):
     """Row f3 measured on ONE GPU, the parts one after the other (no rank waits for another): each part of the k-d
     partition is created, filled with its region (bricks + ghost layers) and renders the K frames of the cycle as
@@ -187,25 +208,13 @@ def sortlast_report(vr, g, wl, cube, tf, nparts, order, K, Wm):
     dims = (wl["nx"], wl["ny"], wl["nz"])
     Wp, Hp = wl["width"], wl["height"]
     boxes, tree = sortlast.kd_partition(dims, wl["brick"], nparts)
-    st = torch.cuda.current_stream().cuda_stream
     out = torch.empty((Hp, Wp, 4), dtype=torch.float32, device="cuda")
     K = min(K, 64)  # frames whose stage events the library keeps
     frame_ms = np.zeros((nparts, K))
     pieces, rects, store_gb, ray_ms = [], [], [], []
     view0 = wl["views"][order[Wm % len(order)]]
     for r, box in enumerate(boxes):
-        p = vr.Volume(*dims, wl["brick"], wl["ghost"], part=box)
-        (x0, y0, z0), (sx, sy, sz) = sortlast.part_region(dims, wl["brick"], wl["ghost"], box)
-        nzs = max(1, min(sz, (4 << 30) // (sx * sy * 4)))
-        buf = torch.empty((nzs, sy, sx), dtype=torch.float32, device="cuda")
-        for k0 in range(0, sz, nzs):
-            nk = min(nzs, sz - k0)
-            cube.fill_device(buf[:nk].data_ptr(), x0, y0, z0 + k0, sx, sy, nk, st)
-            p.upload(buf[:nk], origin=(x0, y0, z0 + k0))
-        torch.cuda.synchronize()
-        del buf
-        p.set_transfer_function(tf, *tf_range(wl))
-        p.set_early_termination(wl["tau"])
+        p = build_part(vr, wl, cube, tf, box)
         p.minmax()
         for k in range(Wm):
             p.render_part(wl["views"][order[k % len(order)]], wl["proj"], Wp, Hp, wl["step"], 0, out)
@@ -253,6 +262,79 @@ def sortlast_report(vr, g, wl, cube, tf, nparts, order, K, Wm):
             "what": "one GPU, parts rendered one after the other; frame time of a part = device time of its set-up, ray-cast and "
                     "stage-1 compositing kernels (stage events); render_bound_frames_per_s = 1 / mean over frames of the slowest "
                     "part's frame time, before the exchange, which is not timed here"}
+
+
+def run_bricks_sharded(args, vr, wl, tf, mode_id, rank, world, local_rank, dist, reduce_max):
+    """`--sharding bricks` (row f3): ONE cube over all ranks, every frame rendered by all of them (sort-last,
+    paper_1205_0282_b200.sortlast). Strong scaling: the cube and the frames are fixed as N grows. Each rank fills
+    only its own region (bricks + ghost layers) from the device generator. Timed like the frame-sharded arm:
+    barrier + synchronise on both sides, CUDA events, maximum over ranks. Not the default: north_star's bench line
+    is the one-GPU cube; every run of round 1 had one GPU, where this arm is the world of one."""
+    import torch
+    from paper_1205_0282_b200 import sortlast
+    dims = (wl["nx"], wl["ny"], wl["nz"])
+    cube = synth.Cube(wl["seed"], wl["nx"], wl["ny"], wl["nz"], wl["nsrc"], wl["ramp"], wl.get("kind", 0))
+    rdr = sortlast.SortLastRenderer(dims, wl["brick"], wl["ghost"], rank=rank, world=world)
+    (x0, y0, z0), (sx, sy, sz) = rdr.region()
+    st = torch.cuda.current_stream().cuda_stream
+    nzs = max(1, min(sz, (4 << 30) // (sx * sy * 4)))
+    buf = torch.empty((nzs, sy, sx), dtype=torch.float32, device="cuda")
+    for k0 in range(0, sz, nzs):
+        nk = min(nzs, sz - k0)
+        cube.fill_device(buf[:nk].data_ptr(), x0, y0, z0 + k0, sx, sy, nk, st)
+        rdr.upload(buf[:nk], (x0, y0, z0 + k0))
+    torch.cuda.synchronize()
+    del buf
+    rdr.set_transfer_function(tf, *tf_range(wl))
+    rdr.set_early_termination(wl["tau"])
+    lo, hi = rdr.minmax()
+    W, H, K, Wm = wl["width"], wl["height"], args.steps, args.warmup
+    nv = len(wl["views"])
+    sampler = ClockSampler(local_rank) if rank == 0 else None
+    for k in range(Wm):
+        rdr.render(wl["views"][k % nv], wl["proj"], W, H, wl["step"], mode_id)
+    if dist is not None:
+        dist.barrier()
+    torch.cuda.synchronize()
+    if sampler:
+        sampler.start()
+    l0 = rdr.backend.volume.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for k in range(K):
+        frame = rdr.render(wl["views"][(Wm + k) % nv], wl["proj"], W, H, wl["step"], mode_id)
+    e1.record()
+    torch.cuda.synchronize()
+    if dist is not None:
+        dist.barrier()
+    ms = reduce_max(e0.elapsed_time(e1))
+    clocks = sampler.stop() if sampler else None
+    launches = rdr.backend.volume.launch_count() - l0
+    # end to end: the finished frame also travels to pinned host memory on rank 0, every step
+    host = torch.empty((H, W, 4), dtype=torch.float32).pin_memory() if rank == 0 else None
+    if dist is not None:
+        dist.barrier()
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    for k in range(K):
+        frame = rdr.render(wl["views"][(Wm + k) % nv], wl["proj"], W, H, wl["step"], mode_id)
+        if rank == 0:
+            host.copy_(frame, non_blocking=True)
+    torch.cuda.synchronize()
+    if dist is not None:
+        dist.barrier()
+    e2e_ms = reduce_max((time.perf_counter() - t0) * 1e3)
+    moved = int(np.mean([rdr.exchange_bytes(wl["views"][(Wm + k) % nv], wl["proj"], W, H) for k in range(K)]))
+    cfg = config_of(wl, args)
+    cfg["sharding"] = "bricks: k-d partition into %d parts (row f3), one cube over all ranks, sort-last exchange" % world
+    return {"metric": METRIC, "value": round(K / (ms * 1e-3), 3), "unit": "frames/s", "n_gpus": world, "steps": K, "warmup": Wm,
+            "ms_per_step": round(ms / K, 4), "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f32",
+            "data": "synthetic", "config": cfg, "gpu_launches": int(launches),
+            "e2e": {"value": round(K / (e2e_ms * 1e-3), 3), "unit": "frames/s", "h2d_bytes_per_step": 128 * world,
+                    "d2h_bytes_per_step": W * H * 16,
+                    "what": "SortLastRenderer.render on every rank + the merged frame copied to pinned host memory on rank 0"},
+            "clocks": clocks, "exchange_bytes_per_frame": moved, "frame_bytes": W * H * 16,
+            "data_range": [float(lo), float(hi)], "roofline": None, "cpu_baseline": None}
 
 
 def tf_range(wl):
@@ -615,6 +697,9 @@ def main():
     ap.add_argument("--cells-every", type=int, default=6, help="count distinct cells on every n-th view of the cycle (0 = never)")
     ap.add_argument("--c4-part", default="both", choices=["both", "composite"],
                     help="--workload c4: `composite` runs only the compositing microbenchmark (profiling)")
+    ap.add_argument("--sharding", default="frames", choices=["frames", "bricks"],
+                    help="N > 1: frames = every rank holds the cube and renders its own frames (default, weak scaling); "
+                         "bricks = one cube over all ranks, sort-last (row f3, strong scaling)")
     ap.add_argument("--sortlast-parts", type=int, default=8,
                     help="row f3 report: parts of the k-d partition rendered one after the other on this GPU (0 = skip)")
     ap.add_argument("--no-variants", action="store_true")
@@ -663,6 +748,15 @@ def main():
             raise SystemExit("bench.py: --workload c4 is a single-GPU microbenchmark")
         peak, peak_src = measured_peak()
         print(json.dumps(run_c4(args, vr, peak, peak_src, ClockSampler(local_rank))), flush=True)
+        return 0
+
+    if args.sharding == "bricks":
+        line = run_bricks_sharded(args, vr, wl, tf, mode_id, rank, world, local_rank, dist, reduce_max)
+        if rank == 0:
+            print(json.dumps(line), flush=True)
+        if dist is not None:
+            dist.barrier()
+            dist.destroy_process_group()
         return 0
 
     t_build = time.perf_counter()

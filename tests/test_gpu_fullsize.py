@@ -172,3 +172,45 @@ def test_nbody_34GB_density_cube_with_culling(vr):
     assert culled == 0
     gpu_frame(g, wl["views"][13], wl["proj"], wl["width"], wl["height"], wl["step"], vr.ALPHA)
     assert g.debug_stats()["bricks_culled"] > 50
+
+
+def test_config3_in_eight_parts_merges_to_the_whole_frame(vr):
+    """Row f3 at full size: the 103 GB cube as the 8 parts of its k-d partition (13 GB each), rendered one after the
+    other, each filled with its own region only; the merged frame against the oracle on seeded pixels, against the
+    single handle everywhere, and one part's partial frame against the oracle's sub-images of that part's bricks."""
+    import torch
+    from paper_1205_0282_b200 import sortlast
+    tf = synth.tf_ramp()
+    wl, g, o, cube = pair(vr, "c3", tf)
+    W, H, dims = wl["width"], wl["height"], (wl["nx"], wl["ny"], wl["nz"])
+    boxes, tree = sortlast.kd_partition(dims, wl["brick"], 8)
+    gdim = sortlast.brick_grid(dims, wl["brick"])
+    vi = 6
+    view, proj = wl["views"][vi], wl["proj"]
+    pix = seeded_pixels(4000 + vi, W, H, 600)
+    ref = o.render(view, proj, W, H, wl["step"], oracle.ALPHA, pixels=pix, want_sub=True)
+    order = [int(b) for b in o.brick_order(view, proj)]
+    pieces, rects = [], []
+    full = torch.empty((H, W, 4), dtype=torch.float32, device="cuda")
+    for r, box in enumerate(boxes):
+        p = bench.build_part(vr, wl, cube, tf, box)
+        rc = p.render_part(view, proj, W, H, wl["step"], vr.ALPHA, full)
+        torch.cuda.synchronize()
+        own = set((bz * gdim[1] + by) * gdim[0] + bx for bz in range(box[0][2], box[1][2]) for by in range(box[0][1], box[1][1])
+                  for bx in range(box[0][0], box[1][0]))
+        acc = np.zeros((len(pix), 4))
+        for b in order:
+            if b in own:
+                acc += (1.0 - acc[:, 3:4]) * ref["sub"][:, b]
+        got = full.cpu().numpy().astype(np.float64)[pix[:, 1], pix[:, 0]]
+        check_alpha(got, acc, ref["flags"], wl["tau"], "c3 part %d" % r)
+        pieces.append(full[rc[1]:rc[3], rc[0]:rc[2]].contiguous())
+        rects.append(rc)
+        p.close()
+        torch.cuda.empty_cache()
+    merged = torch.empty((H, W, 4), dtype=torch.float32, device="cuda")
+    g.composite_parts(vr.ALPHA, pieces, rects, sortlast.part_order(tree, wl["brick"], view, proj), W, H, merged)
+    torch.cuda.synchronize()
+    m = merged.cpu().numpy().astype(np.float64)
+    check_alpha(m[pix[:, 1], pix[:, 0]], ref["image"], ref["flags"], wl["tau"], "c3 in 8 parts")
+    assert np.abs(m - gpu_frame(g, view, proj, W, H, wl["step"], vr.ALPHA)).max() < 2e-6

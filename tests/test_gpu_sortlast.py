@@ -193,3 +193,20 @@ def test_a_world_of_one_renders_through_the_renderer(vr):
         frame = rdr.render(view, proj, W, H, 1.0, mode)
         torch.cuda.synchronize()
         assert np.array_equal(frame.cpu().numpy().astype(np.float64), gpu_frame(whole, view, proj, W, H, 1.0, mode))
+
+
+def test_bench_brick_sharded_arm_as_a_world_of_one(vr):
+    """bench.py --sharding bricks on one GPU: the contract line, through SortLastRenderer."""
+    import json
+    import os
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    r = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--workload", "c0", "--sharding", "bricks", "--steps", "6",
+                        "--warmup", "3"], capture_output=True, text=True, timeout=600)
+    assert r.returncode == 0, r.stderr[-2000:]
+    line = json.loads(r.stdout.strip().splitlines()[-1])
+    assert line["metric"] == "frames_per_s" or line["unit"] == "frames/s"
+    assert line["n_gpus"] == 1 and line["scaling"] == "strong" and line["value"] > 0 and line["e2e"]["value"] > 0
+    assert line["gpu_launches"] == 6 * 4            # set-up, ray cast, stage-1 compositing, merge
+    assert line["exchange_bytes_per_frame"] == 0    # a world of one sends nothing
