@@ -174,24 +174,23 @@ def test_nbody_34GB_density_cube_with_culling(vr):
     assert g.debug_stats()["bricks_culled"] > 50
 
 
-def test_config3_in_eight_parts_merges_to_the_whole_frame(vr):
-    """Row f3 at full size: the 103 GB cube as the 8 parts of its k-d partition (13 GB each), rendered one after the
-    other, each filled with its own region only; the merged frame against the oracle on seeded pixels, against the
-    single handle everywhere, and one part's partial frame against the oracle's sub-images of that part's bricks."""
+def parts_against_oracle(vr, wl, cube, o, tf, nparts, vi, npix, whole=None):
+    """Row f3 at full size: the cube as the parts of its k-d partition, rendered one after the other, each filled with
+    its own region only. Every partial frame against the oracle's sub-images of that part's bricks, the merged frame
+    against the oracle's frame, on seeded pixels; against the single handle everywhere if there is one."""
     import torch
     from paper_1205_0282_b200 import sortlast
-    tf = synth.tf_ramp()
-    wl, g, o, cube = pair(vr, "c3", tf)
     W, H, dims = wl["width"], wl["height"], (wl["nx"], wl["ny"], wl["nz"])
-    boxes, tree = sortlast.kd_partition(dims, wl["brick"], 8)
+    boxes, tree = sortlast.kd_partition(dims, wl["brick"], nparts)
     gdim = sortlast.brick_grid(dims, wl["brick"])
-    vi = 6
     view, proj = wl["views"][vi], wl["proj"]
-    pix = seeded_pixels(4000 + vi, W, H, 600)
+    pix = seeded_pixels(4000 + vi, W, H, npix)
     ref = o.render(view, proj, W, H, wl["step"], oracle.ALPHA, pixels=pix, want_sub=True)
+    assert (ref["counts"][:, 0] > 0).mean() > 0.05
     order = [int(b) for b in o.brick_order(view, proj)]
     pieces, rects = [], []
     full = torch.empty((H, W, 4), dtype=torch.float32, device="cuda")
+    p = None
     for r, box in enumerate(boxes):
         p = bench.build_part(vr, wl, cube, tf, box)
         rc = p.render_part(view, proj, W, H, wl["step"], vr.ALPHA, full)
@@ -203,14 +202,47 @@ def test_config3_in_eight_parts_merges_to_the_whole_frame(vr):
             if b in own:
                 acc += (1.0 - acc[:, 3:4]) * ref["sub"][:, b]
         got = full.cpu().numpy().astype(np.float64)[pix[:, 1], pix[:, 0]]
-        check_alpha(got, acc, ref["flags"], wl["tau"], "c3 part %d" % r)
+        check_alpha(got, acc, ref["flags"], wl["tau"], "%s part %d of %d" % (wl["name"], r, nparts))
         pieces.append(full[rc[1]:rc[3], rc[0]:rc[2]].contiguous())
         rects.append(rc)
-        p.close()
-        torch.cuda.empty_cache()
+        if r + 1 < nparts:
+            p.close()
+            torch.cuda.empty_cache()
     merged = torch.empty((H, W, 4), dtype=torch.float32, device="cuda")
-    g.composite_parts(vr.ALPHA, pieces, rects, sortlast.part_order(tree, wl["brick"], view, proj), W, H, merged)
+    (whole or p).composite_parts(vr.ALPHA, pieces, rects, sortlast.part_order(tree, wl["brick"], view, proj), W, H, merged)
     torch.cuda.synchronize()
     m = merged.cpu().numpy().astype(np.float64)
-    check_alpha(m[pix[:, 1], pix[:, 0]], ref["image"], ref["flags"], wl["tau"], "c3 in 8 parts")
-    assert np.abs(m - gpu_frame(g, view, proj, W, H, wl["step"], vr.ALPHA)).max() < 2e-6
+    check_alpha(m[pix[:, 1], pix[:, 0]], ref["image"], ref["flags"], wl["tau"], "%s in %d parts" % (wl["name"], nparts))
+    if whole is not None:
+        assert np.abs(m - gpu_frame(whole, view, proj, W, H, wl["step"], vr.ALPHA)).max() < 2e-6
+    p.close()
+
+
+def test_config3_in_eight_parts_merges_to_the_whole_frame(vr):
+    """The 103 GB cube as the 8 parts (13 GB each) `bench.py`'s sortlast report times."""
+    tf = synth.tf_ramp()
+    wl, g, o, cube = pair(vr, "c3", tf)
+    parts_against_oracle(vr, wl, cube, o, tf, 8, 6, 600, whole=g)
+
+
+def test_a_206_gb_cube_as_two_parts_of_103_gb(vr):
+    """The paper's headline class (a 204 GB cube) does not fit one B200; its two parts do, one at a
+    time: config 3's recipe with twice the spectral axis (4096 x 4096 x 3072 float32 = 206 GB, 384 bricks of 512^3),
+    split by the k-d rule into two boxes of 192 bricks (104 GB of store each)."""
+    import gc
+    import torch
+    gc.collect()
+    torch.cuda.empty_cache()
+    if torch.cuda.mem_get_info()[0] < 125 * (1 << 30):
+        pytest.skip("needs 125 GB of free device memory")
+    tf = synth.tf_ramp()
+    wl = bench.workload("c3")
+    wl["nz"] *= 2
+    wl["name"] = "c3 x 2"
+    fr = synth.Framing(wl["nx"], wl["ny"], wl["nz"], wl["width"], wl["height"])
+    wl["views"], wl["proj"] = [fr.turntable(k) for k in range(36)], fr.proj(False)
+    cube = synth.Cube(wl["seed"], wl["nx"], wl["ny"], wl["nz"], wl["nsrc"], wl["ramp"], 0)
+    o = oracle.Volume(wl["nx"], wl["ny"], wl["nz"], wl["brick"], wl["ghost"], voxel_fn=cube.voxel_fn())
+    o.set_transfer_function(tf, *bench.tf_range(wl))
+    o.set_early_termination(wl["tau"])
+    parts_against_oracle(vr, wl, cube, o, tf, 2, 5, 500)
