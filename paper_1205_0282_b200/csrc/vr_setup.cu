@@ -43,34 +43,100 @@ vr_setup_kernel(VrGrid grid, VrMatrices mats, int W, int H, int mode, long long 
     __shared__ SetupShared sh;
     const int tid = threadIdx.x;
 
-    if (tid == 0) {
-        double Minv[16];
-        int ortho = 0;
-        const int bad = vr_view_setup(mats.view, mats.proj, sh.M, Minv, sh.eye, &ortho);
-        sh.ortho = ortho;
-        for (int i = 0; i < 16; ++i) {
-            vs->M[i] = sh.M[i];
-            vs->Minv[i] = Minv[i];
+    /* warp 0: M = P*V and its Gauss-Jordan inverse with one lane per entry of the augmented 4 x 8 matrix - the
+     * operations of vr_view_setup (vr_view.cuh), entry by entry and in the same order, so the same bits (R9, R10) */
+    if (tid < 32) {
+        const unsigned FULL = 0xffffffffu;
+        const int r = tid >> 3, c = tid & 7;
+        double m = 0.0;
+        if (tid < 16) { /* entry (row tid & 3, column tid >> 2) of M, column-major */
+            const int mr = tid & 3, mc = tid >> 2;
+            for (int k = 0; k < 4; ++k) m = VR_ADD(m, VR_MUL((double)mats.proj[k * 4 + mr], (double)mats.view[mc * 4 + k]));
+            sh.M[tid] = m;
+            vs->M[tid] = m;
         }
-        for (int a = 0; a < 3; ++a) vs->eye[a] = sh.eye[a];
-        vs->ortho = ortho;
-        vs->singular = bad;
-        vs->W = W;
-        vs->H = H;
-        vs->work_counter = 0u;
-        vs->samples = 0ull;
-        sh.carry_items = 0;
-        sh.carry_pix = 0;
-        sh.culled = 0;
-        vs->data_max = range ? range[grid.nbricks].y : INFINITY;
+        /* a = [M | I](r, c): M(r, c) lives in lane c * 4 + r */
+        double a = __shfl_sync(FULL, m, (c & 3) * 4 + r);
+        if (c >= 4) a = (r == c - 4) ? 1.0 : 0.0;
+        int bad = 0;
+        for (int col = 0; col < 4; ++col) {
+            int piv = col;
+            double best = fabs(__shfl_sync(FULL, a, col * 8 + col));
+            for (int rr = col + 1; rr < 4; ++rr) {
+                const double v = fabs(__shfl_sync(FULL, a, rr * 8 + col));
+                if (v > best) {
+                    best = v;
+                    piv = rr;
+                }
+            }
+            if (best == 0.0) {
+                bad = 1;
+                break;
+            }
+            const double from_piv = __shfl_sync(FULL, a, piv * 8 + c), from_col = __shfl_sync(FULL, a, col * 8 + c);
+            if (piv != col) {
+                if (r == col) a = from_piv;
+                else if (r == piv) a = from_col;
+            }
+            const double d = __shfl_sync(FULL, a, col * 8 + col);
+            if (r == col) a = VR_DIV(a, d);
+            const double f = __shfl_sync(FULL, a, r * 8 + col), pc = __shfl_sync(FULL, a, col * 8 + c);
+            if (r != col && f != 0.0) a = VR_SUB(a, VR_MUL(f, pc));
+        }
+        if (__any_sync(FULL, c >= 4 && !isfinite(a))) bad = 1;
+        if (c >= 4) vs->Minv[(c - 4) * 4 + r] = a;
+        /* homogeneous eye = third column of Minv: lanes r * 8 + 6 */
+        const double c0 = __shfl_sync(FULL, a, 6), c1 = __shfl_sync(FULL, a, 14), c2 = __shfl_sync(FULL, a, 22),
+                     c3 = __shfl_sync(FULL, a, 30);
+        if (tid == 0) {
+            int ortho = 0;
+            if (!bad) {
+                const double mag = VR_ADD(VR_ADD(fabs(c0), fabs(c1)), fabs(c2));
+                if (fabs(c3) < VR_MUL(1e-9, mag)) {
+                    ortho = 1;
+                    sh.eye[0] = c0; sh.eye[1] = c1; sh.eye[2] = c2;
+                } else {
+                    sh.eye[0] = VR_DIV(c0, c3); sh.eye[1] = VR_DIV(c1, c3); sh.eye[2] = VR_DIV(c2, c3);
+                }
+            } else {
+                sh.eye[0] = sh.eye[1] = sh.eye[2] = 0.0;
+            }
+            sh.ortho = ortho;
+            for (int i = 0; i < 3; ++i) vs->eye[i] = sh.eye[i];
+            vs->ortho = ortho;
+            vs->singular = bad;
+            vs->W = W;
+            vs->H = H;
+            vs->work_counter = 0u;
+            vs->samples = 0ull;
+            sh.carry_items = 0;
+            sh.carry_pix = 0;
+            sh.culled = 0;
+            vs->data_max = range ? range[grid.nbricks].y : INFINITY;
+        }
     }
     const bool cull = range != NULL && mode == VR_ALPHA && lut.base != NULL;
-    if (cull) { /* flags in parallel, then a serial prefix over at most 1024 entries of shared memory */
-        for (int i = tid; i < lut.n; i += SETUP_THREADS) sh.nz_prefix[i + 1] = lut.base[i].w != 0.0f ? 1 : 0;
+    if (cull) { /* block scan of the alpha != 0 flags: 4 consecutive entries per thread (n <= VR_MAX_LUT = 4 * 256) */
+        int f[4], t = 0;
+        for (int j = 0; j < 4; ++j) {
+            const int i = 4 * tid + j;
+            f[j] = (i < lut.n && lut.base[i].w != 0.0f) ? 1 : 0;
+            t += f[j];
+        }
+        int incl = t;
+        for (int o = 1; o < 32; o <<= 1) {
+            const int u = __shfl_up_sync(0xffffffffu, incl, o);
+            if ((tid & 31) >= o) incl += u;
+        }
+        if ((tid & 31) == 31) sh.warp_items[tid >> 5] = incl;
         __syncthreads();
-        if (tid == 0) {
-            sh.nz_prefix[0] = 0;
-            for (int i = 1; i <= lut.n; ++i) sh.nz_prefix[i] = (unsigned short)(sh.nz_prefix[i] + sh.nz_prefix[i - 1]);
+        int run = incl - t;
+        for (int w = 0; w < (tid >> 5); ++w) run += sh.warp_items[w];
+        if (tid == 0) sh.nz_prefix[0] = 0;
+        for (int j = 0; j < 4; ++j) {
+            const int i = 4 * tid + j;
+            run += f[j];
+            if (i < lut.n) sh.nz_prefix[i + 1] = (unsigned short)run;
         }
     }
     __syncthreads();
