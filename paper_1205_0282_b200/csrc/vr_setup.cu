@@ -33,6 +33,10 @@ struct SetupShared {
     double eye[3];
     int culled;
     unsigned short nz_prefix[VR_MAX_LUT + 1]; /* nz_prefix[i] = entries < i with alpha != 0 */
+    /* grids of up to SETUP_THREADS bricks keep their views and order here between the passes (the global
+     * copies are written once, complete, at the end): no global round trips inside the kernel */
+    VrBrickView bv[SETUP_THREADS];
+    int order[SETUP_THREADS];
 };
 
 __global__ void __launch_bounds__(SETUP_THREADS)
@@ -42,6 +46,12 @@ vr_setup_kernel(VrGrid grid, VrMatrices mats, int W, int H, int mode, long long 
                 const float2* __restrict__ range, VrLut lut) {
     __shared__ SetupShared sh;
     const int tid = threadIdx.x;
+    const bool small = grid.nbricks <= SETUP_THREADS;
+    const bool cull = range != NULL && mode == VR_ALPHA && lut.base != NULL;
+    /* the global reads the passes below wait for are issued first, ahead of the matrix inversion */
+    float2 mm0 = make_float2(0.0f, 0.0f);
+    if (cull && tid < grid.nbricks) mm0 = range[tid];
+    if (tid == 64) vs->data_max = range ? range[grid.nbricks].y : INFINITY;
 
     /* warp 0: M = P*V and its Gauss-Jordan inverse with one lane per entry of the augmented 4 x 8 matrix - the
      * operations of vr_view_setup (vr_view.cuh), entry by entry and in the same order, so the same bits (R9, R10) */
@@ -112,10 +122,8 @@ vr_setup_kernel(VrGrid grid, VrMatrices mats, int W, int H, int mode, long long 
             sh.carry_items = 0;
             sh.carry_pix = 0;
             sh.culled = 0;
-            vs->data_max = range ? range[grid.nbricks].y : INFINITY;
         }
     }
-    const bool cull = range != NULL && mode == VR_ALPHA && lut.base != NULL;
     if (cull) { /* block scan of the alpha != 0 flags: 4 consecutive entries per thread (n <= VR_MAX_LUT = 4 * 256) */
         int f[4], t = 0;
         for (int j = 0; j < 4; ++j) {
@@ -172,11 +180,12 @@ vr_setup_kernel(VrGrid grid, VrMatrices mats, int W, int H, int mode, long long 
         vr_brick_coords(grid, b, bc);
         vr_brick_core(grid, bc, lo, hi);
         const int key = (sh.rank[2][bc[2]] * grid.g[1] + sh.rank[1][bc[1]]) * grid.g[0] + sh.rank[0][bc[0]];
+        if (small) sh.order[key] = b;
         order[key] = b;
         vr_rect_of_box(sh.M, lo, hi, W, H, r);
         if (vr_slot_index(grid, b) < 0) r[2] = r[0]; /* row f3: another part holds this brick */
         if (cull) { /* R16, float32 as the ray-cast kernel classifies */
-            const float2 mm = range[b];
+            const float2 mm = (b == tid) ? mm0 : range[b];
             const float ulo = __saturatef(__fmul_rn(__fsub_rn(mm.x, lut.vmin), lut.inv_range));
             const float uhi = __saturatef(__fmul_rn(__fsub_rn(mm.y, lut.vmin), lut.inv_range));
             const int i0 = max(min((int)__fmul_rn(ulo, lut.scale), lut.nm2) - 1, 0);
@@ -195,7 +204,7 @@ vr_setup_kernel(VrGrid grid, VrMatrices mats, int W, int H, int mode, long long 
         v.order_pos = key;
         v.slot = vr_slot_index(grid, b);
         v.sub_offset = 0;
-        bv[b] = v;
+        *(small ? &sh.bv[b] : &bv[b]) = v;
     }
     __syncthreads();
     __threadfence_block();
@@ -208,10 +217,10 @@ vr_setup_kernel(VrGrid grid, VrMatrices mats, int W, int H, int mode, long long 
         long long pix = 0;
         int b = -1;
         if (q < grid.nbricks) {
-            b = order[q];
-            const VrBrickView v = bv[b];
-            items = v.tiles_x * v.tiles_y;
-            pix = (long long)(v.lx1 - v.lx0) * (long long)(v.ly1 - v.ly0);
+            b = small ? sh.order[q] : order[q];
+            const VrBrickView* v = small ? &sh.bv[b] : &bv[b];
+            items = v->tiles_x * v->tiles_y;
+            pix = (long long)(v->lx1 - v->lx0) * (long long)(v->ly1 - v->ly0);
         }
         int si = items;
         long long sp = pix;
@@ -236,7 +245,8 @@ vr_setup_kernel(VrGrid grid, VrMatrices mats, int W, int H, int mode, long long 
         }
         if (q < grid.nbricks) {
             item_prefix[q] = bi + si - items;
-            bv[b].sub_offset = bp + sp - pix;
+            if (small) sh.bv[b].sub_offset = bp + sp - pix;
+            else bv[b].sub_offset = bp + sp - pix;
         }
         __syncthreads();
         if (tid == SETUP_THREADS - 1) {
@@ -260,7 +270,8 @@ vr_setup_kernel(VrGrid grid, VrMatrices mats, int W, int H, int mode, long long 
     const unsigned long long px_bytes = (mode == VR_ALPHA) ? 16ull : 4ull;
     const bool over = sh.carry_pix > sub_capacity_px;
     for (int b = tid; b < grid.nbricks; b += SETUP_THREADS) {
-        const VrBrickView v = bv[b];
+        const VrBrickView v = *(small ? &sh.bv[b] : &bv[b]);
+        if (small) bv[b] = v;
         VrCompLayer L;
         L.x0 = v.rx0; L.y0 = v.ry0; L.x1 = over ? v.rx0 : v.rx1; L.y1 = v.ry1;
         L.sx0 = v.lx0; L.sy0 = v.ly0;
