@@ -764,7 +764,7 @@ static int render_frame(vr_volume* v, const float* view, const float* proj, int 
         v->launches++;
         if (timing) VR_CUDA(v, cudaEventRecord(ev[2], st));
         VR_CUDA(v, vr_launch_composite(v->d_layers, v->d_order, v->grid.nbricks, width, height,
-                                       (partial && mode == VR_MIP) ? VR_MIP_RAW : mode, v->lut, out_rgba, st));
+                                       (partial && mode == VR_MIP) ? VR_MIP_RAW : mode, v->lut, out_rgba, v->d_vs->bound, st));
         v->launches++;
     }
     if (timing) {
@@ -918,7 +918,7 @@ static int composite_layers(const VrLut& lut, int kmode, const float* const* lay
         VR_CUDA(NULL, cudaMemcpyAsync(d_tab, tab, sizeof(VrCompLayer) * n, cudaMemcpyHostToDevice, st));
         VR_CUDA(NULL, cudaMemcpyAsync(d_order, order, sizeof(int) * n, cudaMemcpyHostToDevice, st));
     }
-    VR_CUDA(NULL, vr_launch_composite(d_tab, d_order, n, width, height, kmode, lut, out, st));
+    VR_CUDA(NULL, vr_launch_composite(d_tab, d_order, n, width, height, kmode, lut, out, NULL, st));
     VR_CUDA(NULL, cudaFreeAsync(d_tab, st));
     VR_CUDA(NULL, cudaFreeAsync(d_order, st));
     return VR_OK;

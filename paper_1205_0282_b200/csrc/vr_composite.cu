@@ -37,7 +37,7 @@ struct CompEntry {
 template <int MODE>
 __global__ void __launch_bounds__(COMP_THREADS)
 vr_composite_kernel(const VrCompLayer* __restrict__ layers, const int* __restrict__ order, int n, int W, int H, VrLut lut,
-                    float4* __restrict__ out) {
+                    float4* __restrict__ out, const int* __restrict__ bound) {
     __shared__ CompEntry s_list[COMP_LIST];
     __shared__ int s_warp_cnt[COMP_THREADS / 32];
     __shared__ int s_count;
@@ -47,6 +47,15 @@ vr_composite_kernel(const VrCompLayer* __restrict__ layers, const int* __restric
     const int tx1 = min(tx0 + VR_COMP_TILE_W, W), ty1 = min(ty0 + VR_COMP_TILE_H, H);
     const int px = tx0 + (tid & (VR_COMP_TILE_W - 1)), py = ty0 + tid / VR_COMP_TILE_W;
     const bool live = px < W && py < H;
+    /* a tile outside the union of the layers' rectangles is blank: one load decides it, no table walk
+     * (c3: the cube covers 18 % of a 1080p frame) */
+    if (bound) {
+        const int bx0 = __ldg(bound), by0 = __ldg(bound + 1), bx1 = __ldg(bound + 2), by1 = __ldg(bound + 3);
+        if (!(bx0 < tx1 && bx1 > tx0 && by0 < ty1 && by1 > ty0)) {
+            if (live) __stcs(out + (long long)py * W + px, make_float4(0.0f, 0.0f, 0.0f, 0.0f));
+            return;
+        }
+    }
 
     float cr = 0.0f, cg = 0.0f, cb = 0.0f, ca = 0.0f;
     float m = -INFINITY;
@@ -124,15 +133,15 @@ vr_composite_kernel(const VrCompLayer* __restrict__ layers, const int* __restric
 }
 
 cudaError_t vr_launch_composite(const VrCompLayer* layers, const int* order, int n, int W, int H, int mode,
-                                const VrLut& lut, float* out, cudaStream_t st) {
+                                const VrLut& lut, float* out, const int* bound, cudaStream_t st) {
     dim3 grid((W + VR_COMP_TILE_W - 1) / VR_COMP_TILE_W, (H + VR_COMP_TILE_H - 1) / VR_COMP_TILE_H);
     if (mode == VR_ALPHA)
-        vr_composite_kernel<VR_ALPHA><<<grid, COMP_THREADS, 0, st>>>(layers, order, n, W, H, lut, reinterpret_cast<float4*>(out));
+        vr_composite_kernel<VR_ALPHA><<<grid, COMP_THREADS, 0, st>>>(layers, order, n, W, H, lut, reinterpret_cast<float4*>(out), bound);
     else if (mode == VR_MIP)
-        vr_composite_kernel<VR_MIP><<<grid, COMP_THREADS, 0, st>>>(layers, order, n, W, H, lut, reinterpret_cast<float4*>(out));
+        vr_composite_kernel<VR_MIP><<<grid, COMP_THREADS, 0, st>>>(layers, order, n, W, H, lut, reinterpret_cast<float4*>(out), bound);
     else if (mode == VR_MIP_RAW)
-        vr_composite_kernel<VR_MIP_RAW><<<grid, COMP_THREADS, 0, st>>>(layers, order, n, W, H, lut, reinterpret_cast<float4*>(out));
+        vr_composite_kernel<VR_MIP_RAW><<<grid, COMP_THREADS, 0, st>>>(layers, order, n, W, H, lut, reinterpret_cast<float4*>(out), bound);
     else
-        vr_composite_kernel<VR_MIP_PARTS><<<grid, COMP_THREADS, 0, st>>>(layers, order, n, W, H, lut, reinterpret_cast<float4*>(out));
+        vr_composite_kernel<VR_MIP_PARTS><<<grid, COMP_THREADS, 0, st>>>(layers, order, n, W, H, lut, reinterpret_cast<float4*>(out), bound);
     return cudaGetLastError();
 }

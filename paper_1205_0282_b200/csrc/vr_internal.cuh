@@ -90,6 +90,8 @@ struct VrViewState {
     unsigned long long samples;
     float data_max; /* global maximum of the data if known, else +inf (MIP stop) */
     int culled;     /* bricks skipped as transparent in this view (R16) */
+    int bound[4];   /* union of the non-empty rendering rectangles (x0, y0, x1, y1; zeros if none): the frame is
+                     * blank outside it, which the compositing kernel uses to leave early */
 };
 
 struct VrBrickView {
@@ -179,8 +181,9 @@ cudaError_t vr_launch_cell_flags(const float2* cell_mm, unsigned* bits, int nbri
 cudaError_t vr_launch_raycast(const VrRaycastParams& p, long long items, bool count, bool sparse, cudaStream_t st);
 /* fused traversal (row f2): one ray per frame pixel through all bricks, writes the frame */
 cudaError_t vr_launch_fused(const VrRaycastParams& p, float* frame, int W, int H, bool count, cudaStream_t st);
+/* bound: device int[4] as VrViewState::bound, or NULL (layers anywhere) */
 cudaError_t vr_launch_composite(const VrCompLayer* layers, const int* order, int n, int W, int H, int mode,
-                                const VrLut& lut, float* out, cudaStream_t st);
+                                const VrLut& lut, float* out, const int* bound, cudaStream_t st);
 cudaError_t vr_launch_upload(const VrGrid& grid, float* bricks, const float* src, int x0, int y0, int z0, int sx,
                              int sy, int sz, cudaStream_t st);
 cudaError_t vr_launch_download(const VrGrid& grid, const float* bricks, float* dst, int x0, int y0, int z0, int sx,

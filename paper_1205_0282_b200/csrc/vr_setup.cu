@@ -37,6 +37,7 @@ struct SetupShared {
      * copies are written once, complete, at the end): no global round trips inside the kernel */
     VrBrickView bv[SETUP_THREADS];
     int order[SETUP_THREADS];
+    int bound[4]; /* union of the non-empty rendering rectangles */
 };
 
 __global__ void __launch_bounds__(SETUP_THREADS)
@@ -122,6 +123,7 @@ vr_setup_kernel(VrGrid grid, VrMatrices mats, int W, int H, int mode, long long 
             sh.carry_items = 0;
             sh.carry_pix = 0;
             sh.culled = 0;
+            sh.bound[0] = W; sh.bound[1] = H; sh.bound[2] = 0; sh.bound[3] = 0;
         }
     }
     if (cull) { /* block scan of the alpha != 0 flags: 4 consecutive entries per thread (n <= VR_MAX_LUT = 4 * 256) */
@@ -195,6 +197,12 @@ vr_setup_kernel(VrGrid grid, VrMatrices mats, int W, int H, int mode, long long 
                 atomicAdd(&sh.culled, 1);
             }
         }
+        if (r[2] > r[0] && r[3] > r[1]) {
+            atomicMin(&sh.bound[0], r[0]);
+            atomicMin(&sh.bound[1], r[1]);
+            atomicMax(&sh.bound[2], r[2]);
+            atomicMax(&sh.bound[3], r[3]);
+        }
         vr_launch_rect(r, W, H, l);
         VrBrickView v;
         v.rx0 = r[0]; v.ry0 = r[1]; v.rx1 = r[2]; v.ry1 = r[3];
@@ -263,6 +271,8 @@ vr_setup_kernel(VrGrid grid, VrMatrices mats, int W, int H, int mode, long long 
         vs->total_sub_pixels = sh.carry_pix;
         vs->overflow = over;
         vs->culled = sh.culled;
+        const bool none = sh.bound[2] <= sh.bound[0] || sh.bound[3] <= sh.bound[1];
+        for (int i = 0; i < 4; ++i) vs->bound[i] = none ? 0 : sh.bound[i];
     }
     __syncthreads();
 
