@@ -682,6 +682,39 @@ def run_c4(args, vr, peak, peak_src, sampler):
             "roofline": roof, "clocks": clocks, "e2e": None, "cpu_baseline": None}
 
 
+# ----------------------------------------------------------------------------- DRAM probe
+def run_probe_dram(vr, gib):
+    """What a 4-byte load that misses L2 costs: for every load flavour, L2
+    fetch-granularity limit and locality pattern, loads per second of one probe launch (CUDA events inside
+    vr_debug_probe_dram). DRAM bytes per load need ncu: the same command under
+    `ncu --metrics dram__bytes_read.sum,gpu__time_duration.sum` lists the launches in the order of `cases`
+    (two launches per case: warm-up, then the timed one)."""
+    import torch
+    buf = torch.zeros((gib << 30) // 4, dtype=torch.float32, device="cuda")
+    peak, peak_src = measured_peak()
+    cases = []
+
+    def case(flavour, span, group, gran=0, ctas=148 * 8, lpt=256):
+        ms, loads = vr.debug_probe_dram(buf, flavour, span, group, lpt, ctas, gran)
+        cases.append({"flavour": vr.PROBE_FLAVOURS[flavour], "span_bytes": span, "group": group, "l2_fetch_granularity": gran or "default",
+                      "ctas": ctas, "loads": loads, "ms": round(ms, 4), "gloads_per_s": round(loads / (ms * 1e-3) / 1e9, 2),
+                      "gbs_if_128B_per_load": round(loads * 128 / (ms * 1e-3) / 1e9, 1)})
+
+    for f in range(len(vr.PROBE_FLAVOURS)):  # every load a random line
+        case(f, 128, 1)
+    for gran in (32, 64, 128):                 # cudaLimitMaxL2FetchGranularity
+        case(1, 128, 1, gran)
+        case(6, 128, 1, gran)
+    case(1, 128, 1, 128)                       # leave the limit at its largest value for what follows
+    for span, group in ((256, 2), (512, 2), (512, 4), (1024, 2), (1024, 8), (2048, 2), (4096, 2), (4096, 8), (65536, 2), (65536, 8)):
+        case(1, span, group)                   # locality: `group` lines of one aligned block
+        case(6, span, group)
+    for ctas in (148 * 2, 148 * 4, 148 * 16, 148 * 32):  # memory-level parallelism
+        case(1, 128, 1, 0, ctas)
+    del buf
+    return {"probe": "dram", "buffer_gib": gib, "hbm_peak_gbs": peak, "hbm_peak_source": peak_src, "cases": cases}
+
+
 # ----------------------------------------------------------------------------- main
 def main():
     ap = argparse.ArgumentParser()
@@ -703,6 +736,9 @@ def main():
     ap.add_argument("--sortlast-parts", type=int, default=8,
                     help="row f3 report: parts of the k-d partition rendered one after the other on this GPU (0 = skip)")
     ap.add_argument("--no-variants", action="store_true")
+    ap.add_argument("--probe", default=None, choices=["dram"],
+                    help="dram: the DRAM fetch-granularity probe (vr_debug_probe_dram) instead of a workload; one JSON line")
+    ap.add_argument("--probe-gib", type=int, default=16, help="--probe dram: size of the probed buffer")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
@@ -742,6 +778,11 @@ def main():
         t = torch.tensor([x], dtype=torch.float64, device="cuda")
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         return float(t.item())
+
+    if args.probe == "dram":
+        if rank == 0:
+            print(json.dumps(run_probe_dram(vr, args.probe_gib)), flush=True)
+        return 0
 
     if args.workload == "c4":
         if world > 1:

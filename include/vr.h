@@ -370,6 +370,23 @@ int vr_debug_stats(vr_volume* v, vr_stats* out);
  * them and read every frame's stage times afterwards. Synchronises. */
 int vr_debug_stage_times(vr_volume* v, int nframes, float* ms_out);
 
+/* DRAM fetch-granularity probe (no handle). Measures what
+ * bounds row a5 on sparsely sampled cubes: the cost of a 4-byte load that misses L2. ctas x 256
+ * threads each issue loads_per_thread (a multiple of 8 and of `group`) independent loads at hashed
+ * 32-byte-aligned offsets of buf (device, `bytes` long, far larger than L2, any finite contents);
+ * the loads of one group of `group` consecutive loads fall into `group` distinct 128-byte lines of
+ * one aligned span_bytes block (a power of two >= 128; group <= span_bytes / 128).
+ *   flavour: 0 ld.global, 1 ld.global.nc (= __ldg, the ray-cast kernel's load), 2 .cg, 3 .cs, 4 .cv,
+ *            5 .nc.L1::no_allocate, 6 .nc.L1::no_allocate.L2::64B, 7 .nc.L2::128B, 8 .nc.L2::256B,
+ *            9 .nc.v4.f32 (16 bytes), 10 .nc.L2::64B
+ *   l2_fetch_granularity: 0 = leave, or 32 / 64 / 128 = cudaLimitMaxL2FetchGranularity (stays set).
+ *   ms_out (host): device time of one launch (CUDA events on `stream`, after one warm-up launch);
+ *   loads_out (host): loads that launch issued. DRAM bytes per load come from ncu's
+ *   dram__bytes_read.sum of the same launch. Synchronises. */
+int vr_debug_probe_dram(const void* buf, uint64_t bytes, int flavour, int span_bytes, int group,
+                        int loads_per_thread, int ctas, int l2_fetch_granularity, float* ms_out,
+                        uint64_t* loads_out, void* stream);
+
 /* Number of kernel launches the library has issued on this handle since creation. */
 int64_t vr_launch_count(const vr_volume* v);
 

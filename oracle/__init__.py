@@ -36,6 +36,7 @@ def lib():
         L.vro_brick_minmax.argtypes = [vp, ci, vp, vp]
         L.vro_brick_transparent.argtypes = [vp, ci]
         L.vro_set_tau.argtypes = [vp, dbl]
+        L.vro_set_nan_limit_scale.argtypes = [vp, dbl]
         L.vro_set_order_override.argtypes = [vp, vp]
         L.vro_brick_order.argtypes = [vp, vp, vp, vp]
         L.vro_rects.argtypes = [vp, vp, vp, ci, ci, vp]
@@ -79,6 +80,7 @@ class Volume:
             self._keep = voxel_fn
             lib().vro_set_procedural(self._h, fn, ctx)
         self.nbricks = lib().vro_num_bricks(self._h)
+        self.tau = 0.99
 
     def __del__(self):
         try:
@@ -94,7 +96,12 @@ class Volume:
             raise ValueError("bad transfer function")
 
     def set_early_termination(self, tau):
-        lib().vro_set_tau(self._h, float(tau))
+        self.tau = float(tau)
+        lib().vro_set_tau(self._h, self.tau)
+
+    def set_nan_limit_scale(self, scale):
+        """R12/R14 test hook: R14's drop limit times `scale` (1 = nominal)."""
+        lib().vro_set_nan_limit_scale(self._h, float(scale))
 
     def set_order_override(self, order):
         if order is None:
@@ -167,6 +174,21 @@ class Volume:
         res = dict(image=out, flags=flags, counts=counts)
         if want_sub:
             res["sub"] = sub
+
+        def alt(dtau=0.0, nan_scale=1.0):
+            """R12: the same frame with every marginal decision taken the other way - early termination tested
+            against tau + dtau (|dtau| = the 1e-5 flag margin), R14's drop limit scaled by nan_scale (0.5 or 2,
+            the flag's band). A flagged pixel has more than one correct value; these are the others."""
+            tau0 = self.tau
+            try:
+                self.set_early_termination(tau0 + dtau)
+                self.set_nan_limit_scale(nan_scale)
+                return self.render(view, proj, width, height, step, mode, pixels=pixels, want_sub=want_sub, nthreads=nthreads)
+            finally:
+                self.set_early_termination(tau0)
+                self.set_nan_limit_scale(1.0)
+
+        res["alt"] = alt
         return res
 
     def ray_bricks(self, view, proj, width, height, pixels, maxlen=64):

@@ -69,6 +69,8 @@ typedef struct vro_volume {
     double tau;        /* early ray termination threshold; > 1 disables */
     int* order_override; /* test hook: composite in this order instead of R9's */
     int64_t ghost_violations; /* fetches that left the padded brick (R3) */
+    double nan_limit;  /* R14: tri-linear weight on NaN corners above which a sample is dropped (VRO_NAN_WEIGHT); the
+                        * tests move it by a factor 2 either way to obtain BOTH correct values of a flagged pixel (R12) */
 } vro_volume;
 
 /* ------------------------------------------------------------------ bricks (R3, a1) */
@@ -96,6 +98,7 @@ vro_volume* vro_create(int64_t nx, int64_t ny, int64_t nz, int brick, int ghost)
     for (int a = 0; a < 3; ++a) v->g[a] = (int)((v->n[a] + brick - 1) / brick);
     v->nbricks = v->g[0] * v->g[1] * v->g[2];
     v->tau = 0.99;
+    v->nan_limit = VRO_NAN_WEIGHT;
     return v;
 }
 
@@ -223,6 +226,9 @@ int vro_set_tf(vro_volume* v, const float* rgba, int n, double vmin, double vmax
     return 0;
 }
 void vro_set_tau(vro_volume* v, double tau) { v->tau = tau; }
+/* R12/R14 test hook: the drop limit of R14 scaled by `scale` (1 = the reading's 4e-6). The NAN_MARGIN flag keeps
+ * marking samples within a factor 2 of the NOMINAL limit, so scale 0.5 drops and scale 2 keeps every flagged sample. */
+void vro_set_nan_limit_scale(vro_volume* v, double scale) { v->nan_limit = VRO_NAN_WEIGHT * scale; }
 int vro_set_order_override(vro_volume* v, const int* order) {
     free(v->order_override);
     v->order_override = NULL;
@@ -286,7 +292,7 @@ static double trilinear(vro_volume* v, int b, const int64_t lo[3], const int64_t
                     else acc += w * c[dz][dy][dx];
                 }
         if (nan_weight) *nan_weight = N;
-        val = (N > VRO_NAN_WEIGHT) ? NAN : acc / (1.0 - N);
+        val = (N > v->nan_limit) ? NAN : acc / (1.0 - N);
     }
     return val;
 }

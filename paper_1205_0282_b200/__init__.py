@@ -30,7 +30,7 @@ SYMBOLS = (
     "vr_set_transfer_function", "vr_set_early_termination", "vr_volume_minmax", "vr_set_culling", "vr_set_traversal", "vr_debug_brick_minmax", "vr_debug_cell_flags", "vr_render", "vr_render_host", "vr_render_host_async", "vr_render_host_wait", "vr_composite",
     "vr_num_bricks", "vr_debug_brick_order", "vr_debug_rects", "vr_debug_ray_bricks", "vr_debug_subimages",
     "vr_volume_create_part", "vr_render_part", "vr_part_rect", "vr_composite_parts",
-    "vr_set_counting", "vr_set_timing", "vr_debug_stats", "vr_debug_stage_times", "vr_launch_count", "vr_last_error",
+    "vr_set_counting", "vr_set_timing", "vr_debug_stats", "vr_debug_stage_times", "vr_debug_probe_dram", "vr_launch_count", "vr_last_error",
 )
 
 
@@ -93,6 +93,7 @@ def lib():
         L.vr_set_timing.argtypes = [vp, ci]
         L.vr_debug_stats.argtypes = [vp, ctypes.POINTER(Stats)]
         L.vr_debug_stage_times.argtypes = [vp, ci, vp]
+        L.vr_debug_probe_dram.argtypes = [vp, ctypes.c_uint64, ci, ci, ci, ci, ci, ci, vp, vp, vp]
         L.vr_launch_count.argtypes = [vp]
         L.vr_launch_count.restype = i64
         L.vr_last_error.argtypes = [vp]
@@ -354,6 +355,24 @@ def part_rect(dims, brick, box, view, proj, width, height):
     if rc != 0:
         raise VrError(rc, lib().vr_last_error(None).decode())
     return tuple(int(c) for c in rect)
+
+
+PROBE_FLAVOURS = ("ld.global", "ld.global.nc", "ld.global.cg", "ld.global.cs", "ld.global.cv", "ld.global.nc.L1::no_allocate",
+                  "ld.global.nc.L1::no_allocate.L2::64B", "ld.global.nc.L2::128B", "ld.global.nc.L2::256B", "ld.global.nc.v4",
+                  "ld.global.nc.L2::64B")
+
+
+def debug_probe_dram(buf, flavour, span_bytes=128, group=1, loads_per_thread=256, ctas=148 * 8, l2_fetch_granularity=0, stream=None):
+    """vr_debug_probe_dram on a CUDA tensor: returns (ms of one launch, loads it issued)."""
+    if not (buf.is_cuda and buf.is_contiguous()):
+        raise ValueError("debug_probe_dram: buf must be a contiguous CUDA tensor")
+    ms, loads = ctypes.c_float(), ctypes.c_uint64()
+    rc = lib().vr_debug_probe_dram(buf.data_ptr(), buf.numel() * buf.element_size(), int(flavour), int(span_bytes), int(group),
+                                   int(loads_per_thread), int(ctas), int(l2_fetch_granularity), ctypes.byref(ms), ctypes.byref(loads),
+                                   _stream(stream))
+    if rc != 0:
+        raise VrError(rc, "vr_debug_probe_dram failed")
+    return float(ms.value), int(loads.value)
 
 
 def composite(layers, rects, order, width, height, out, stream=None):

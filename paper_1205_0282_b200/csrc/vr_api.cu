@@ -789,13 +789,7 @@ extern "C" int vr_render_host(vr_volume* v, const float* view, const float* proj
     if (px > v->frame_capacity_px) {
         if (v->d_frame) {
             VR_CUDA(v, cudaDeviceSynchronize());
-            cudaFree(v->d_frame);
-    for (int i = 0; i < 2; ++i) {
-        cudaFree(v->d_pipe[i]);
-        if (v->ev_rendered[i]) cudaEventDestroy(v->ev_rendered[i]);
-        if (v->ev_copied[i]) cudaEventDestroy(v->ev_copied[i]);
-    }
-    if (v->copy_stream) cudaStreamDestroy(v->copy_stream);
+            cudaFree(v->d_frame); /* only the synchronous entry's own frame: the pipelined entry's frames, events and stream stay */
             v->d_frame = NULL;
             v->frame_capacity_px = 0;
         }

@@ -53,39 +53,71 @@ def gpu_frame(g, view, proj, W, H, step, mode):
     return out.cpu().numpy().astype(np.float64)
 
 
-def check_alpha(gpu, ref, flags, tau, what=""):
-    """gpu, ref: [...,4]; flags: oracle decision-margin flags (R12)."""
-    err = np.abs(gpu - ref).max(axis=-1)
-    # R14: a pixel with a sample whose NaN weight is within a factor 2 of the drop limit has two correct values
-    nanm = (flags & oracle.FLAG_NAN_MARGIN) != 0
-    assert nanm.mean() <= 0.01, "%s: %.2f %% of the pixels sit on the NaN-weight limit" % (what, 100 * nanm.mean())
-    err = np.where(nanm, 0.0, err)
-    marg = (flags & (oracle.FLAG_ERT_MARGIN | oracle.FLAG_OWNER_MARGIN)) != 0
-    bad = err > np.where(marg, ALPHA_TOL + max(0.0, 1.0 - tau), ALPHA_TOL)
-    assert not bad.any(), "%s ALPHA: %d pixels off, max err %.3e (unflagged max %.3e)" % (
-        what, int(bad.sum()), err.max(), err[~marg].max() if (~marg).any() else 0.0)
-    # R12: a ray whose opacity passes tau in steps of dA is flagged with probability ~2e-5/dA
-    # (a few per cent at most); what must stay rare is a flagged pixel that really differs
+def _expand(mask, like):
+    return mask.reshape(mask.shape + (1,) * (like.ndim - mask.ndim))
+
+
+def _best_over_candidates(gpu, ref, key, errfn, want_ert, want_nan):
+    """R12: a decision-margin pixel has several correct values - the oracle's with each marginal decision taken
+    either way (early-termination tests within 1e-5 of tau: tau -/+ 1e-5; samples whose NaN weight is within a
+    factor 2 of R14's limit: limit x 0.5 / x 2). Returns, per pixel, the smallest error over those candidates;
+    the caller applies it to flagged pixels only and holds it to the NORMAL tolerance."""
+    best = errfn(gpu, ref[key])
+    for dtau in ((0.0, -1e-5, 1e-5) if want_ert else (0.0,)):
+        for ns in ((1.0, 0.5, 2.0) if want_nan else (1.0,)):
+            if dtau == 0.0 and ns == 1.0:
+                continue
+            best = np.minimum(best, errfn(gpu, ref["alt"](dtau, ns)[key]))
+    return best
+
+
+def check_alpha(gpu, ref, tau, what="", key="image"):
+    """gpu: [...,4]; ref: the oracle's result dict for the same pixels (image / sub, flags, alt)."""
+    flags = ref["flags"]
+    want = ref[key]
+    if want.ndim > flags.ndim + 1:          # sub-images [npix][nbricks][4]: the pixel's flags apply to each brick
+        flags = _expand(flags, want[..., 0])
+        flags = np.broadcast_to(flags, want.shape[:-1])
+
+    def errfn(a, b):
+        return np.abs(a - b).max(axis=-1)
+
+    err = errfn(gpu, want)
     ert = (flags & oracle.FLAG_ERT_MARGIN) != 0
+    nanm = (flags & oracle.FLAG_NAN_MARGIN) != 0
+    loose = ert | nanm
+    if loose.any():  # flagged pixels are CHECKED, against every candidate, at the normal tolerance (not excused)
+        err = np.where(loose, _best_over_candidates(gpu, ref, key, errfn, ert.any(), nanm.any()), err)
+    # owner-margin pixels (FLAG_OWNER_MARGIN) get no allowance: both sides take the owner decision in FP64 with the
+    # same operations (DESIGN.md "Set-up arithmetic"), so the sample sets are identical
+    bad = err > ALPHA_TOL
+    assert not bad.any(), "%s ALPHA: %d pixels off, max err %.3e (unflagged max %.3e)" % (
+        what, int(bad.sum()), err.max(), err[~loose].max() if (~loose).any() else 0.0)
+    # R12: a ray whose opacity passes tau in steps of dA is flagged with probability ~2e-5/dA (a few per cent at
+    # most on the ramp); R14: few samples sit on the NaN-weight limit
     assert ert.mean() < 0.03, "%s: %.4f%% early-termination-margin pixels" % (what, 100 * ert.mean())
-    # owner margins (a sample within 1e-6 voxel of a brick face) are a property of the view: with the per-ray
-    # step an axis-aligned ray samples ON the voxel planes; a random view has none
-    assert marg.mean() < 0.10, "%s: %.4f%% decision-margin pixels" % (what, 100 * marg.mean())
-    assert (err > ALPHA_TOL).mean() < 1e-3, "%s: %.4f%% pixels beyond 2e-3" % (what, 100 * (err > ALPHA_TOL).mean())
+    assert nanm.mean() <= 0.01, "%s: %.2f %% of the pixels sit on the NaN-weight limit" % (what, 100 * nanm.mean())
     return float(err.max())
 
 
-def check_mip(gpu, ref, what="", flags=None):
-    tol = MIP_RTOL * np.maximum(np.abs(gpu), np.abs(ref)) + MIP_ATOL
-    err = np.abs(gpu - ref)
-    if flags is not None:  # R14 / R12: pixels with two correct values (NaN-weight limit, marginal last sample)
-        nanm = (flags & oracle.FLAG_NAN_MARGIN) != 0
+def check_mip(gpu, ref, what="", key="image"):
+    """ref: the oracle's result dict, or a plain array (comparisons between two GPU frames)."""
+    want = ref[key] if isinstance(ref, dict) else ref
+
+    def errfn(a, b):
+        return (np.abs(a - b) - (MIP_RTOL * np.maximum(np.abs(a), np.abs(b)) + MIP_ATOL)).max(axis=-1)
+
+    excess = errfn(gpu, want)  # <= 0 where within R13's tolerance
+    if isinstance(ref, dict):
+        # FLAG_LAST_SAMPLE pixels get no allowance: the existence of the clipped last sample is decided in FP64 on both
+        # sides. R14: a sample on the NaN-weight limit may be kept or dropped - both candidates are tried.
+        nanm = (ref["flags"] & oracle.FLAG_NAN_MARGIN) != 0
         assert nanm.mean() <= 0.01, "%s: %.2f %% of the pixels sit on the NaN-weight limit" % (what, 100 * nanm.mean())
-        loose = nanm | ((flags & oracle.FLAG_LAST_SAMPLE) != 0)
-        err = np.where(loose[..., None], 0.0, err)
-    bad = err > tol
-    assert not bad.any(), "%s MIP: %d values off, max err %.3e" % (what, int(bad.sum()), err.max())
-    return float((err / np.maximum(np.abs(ref), 1e-30)).max())
+        if nanm.any():
+            excess = np.where(nanm, _best_over_candidates(gpu, ref, key, errfn, False, True), excess)
+    bad = excess > 0.0
+    assert not bad.any(), "%s MIP: %d pixels off, max excess over tolerance %.3e" % (what, int(bad.sum()), excess.max())
+    return float((np.abs(gpu - want) / np.maximum(np.abs(want), 1e-30)).max())
 
 
 def seeded_pixels(seed, W, H, n):

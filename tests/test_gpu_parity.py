@@ -112,9 +112,9 @@ def test_config0_full_frames(vr, tf_name):
     W, H = c["width"], c["height"]
     for name, view, proj in views_for(cube, W, H):
         ref = o.render(view, proj, W, H, c["step"], oracle.ALPHA)
-        check_alpha(gpu_frame(g, view, proj, W, H, c["step"], vr.ALPHA), ref["image"], ref["flags"], 0.99, "c0 " + name)
+        check_alpha(gpu_frame(g, view, proj, W, H, c["step"], vr.ALPHA), ref, 0.99, "c0 " + name)
         ref = o.render(view, proj, W, H, c["step"], oracle.MIP)
-        check_mip(gpu_frame(g, view, proj, W, H, c["step"], vr.MIP), ref["image"], "c0 " + name)
+        check_mip(gpu_frame(g, view, proj, W, H, c["step"], vr.MIP), ref, "c0 " + name)
         assert ref["image"][..., 3].max() == 1.0 and ref["image"][..., 3].min() == 0.0
 
 
@@ -130,14 +130,13 @@ def test_bricked_ragged_full_frames_and_subimages(vr, tau):
     for name, view, proj in views_for(cube, W, H, n_rot=2):
         ref = o.render(view, proj, W, H, step, oracle.ALPHA)
         img = gpu_frame(g, view, proj, W, H, step, vr.ALPHA)
-        check_alpha(img, ref["image"], ref["flags"], tau, name)
+        check_alpha(img, ref, tau, name)
         # row a8: each brick's sub-image value
         sub_ref = o.render(view, proj, W, H, step, oracle.ALPHA, pixels=pix, want_sub=True)
         sub = g.debug_subimages(pix).astype(np.float64)
-        fl = np.repeat(sub_ref["flags"][:, None], g.nbricks, axis=1)
-        check_alpha(sub, sub_ref["sub"], fl, tau, name + " sub-images")
+        check_alpha(sub, sub_ref, tau, name + " sub-images", key="sub")
         ref = o.render(view, proj, W, H, step, oracle.MIP)
-        check_mip(gpu_frame(g, view, proj, W, H, step, vr.MIP), ref["image"], name)
+        check_mip(gpu_frame(g, view, proj, W, H, step, vr.MIP), ref, name)
         sub_ref = o.render(view, proj, W, H, step, oracle.MIP, pixels=pix, want_sub=True)
         sub = g.debug_subimages(pix).astype(np.float64)[..., 0]
         m_ref = sub_ref["sub"][..., 0]
@@ -189,7 +188,38 @@ def test_pipelined_host_frames_equal_synchronous_ones(vr):
             sync = g.render_host(v, proj, W, H, 0.5, mode)
             assert np.array_equal(b.numpy(), sync)
     ref = o.render(views[0], proj, W, H, 0.5, oracle.MIP)
-    check_mip(bufs[0].numpy().astype(np.float64), ref["image"], "pipelined frame 0")
+    check_mip(bufs[0].numpy().astype(np.float64), ref, "pipelined frame 0")
+
+
+def test_host_entries_mixed_at_growing_sizes(vr):
+    """The synchronous and the pipelined host entry own separate device frames: growing the frame of one
+    must leave the other's frames, events and copy stream alone (small sync, async, LARGER sync, async, destroy)."""
+    import torch
+    cube = synth.Cube(22, 48, 40, 36, 4)
+    g, o = make_pair(cube, 32, 1)
+    small, large = (96, 64), (160, 120)
+    frs = {s: synth.Framing(cube.nx, cube.ny, cube.nz, *s) for s in (small, large)}
+
+    def sync(size, k):
+        fr = frs[size]
+        return g.render_host(fr.turntable(k), fr.proj(False), size[0], size[1], 0.5, vr.ALPHA)
+
+    def pipelined(size, k):
+        fr = frs[size]
+        b = torch.full((size[1], size[0], 4), -1.0, dtype=torch.float32).pin_memory()
+        g.render_host_async(fr.turntable(k), fr.proj(False), size[0], size[1], 0.5, vr.ALPHA, b)
+        g.render_host_wait()
+        return b.numpy().copy()
+
+    a0 = sync(small, 1)
+    assert np.array_equal(pipelined(small, 1), a0)
+    a1 = sync(large, 2)                       # grows the synchronous frame only
+    assert np.array_equal(pipelined(small, 1), a0)   # the pipelined frames, events and stream are still alive
+    assert np.array_equal(pipelined(large, 2), a1)   # and can grow on their own
+    assert np.array_equal(sync(small, 1), a0)
+    ref = o.render(frs[large].turntable(2), frs[large].proj(False), large[0], large[1], 0.5, oracle.ALPHA)
+    check_alpha(a1.astype(np.float64), ref, 0.99, "mixed host entries")
+    g.close()
 
 
 # --------------------------------------------------------------------------- f2 (i) per-ray step (R18)
@@ -209,9 +239,9 @@ def test_auto_step_matches_oracle(vr, ortho):
     for trav, orc in ((vr.SORT_LAST, o), (vr.FUSED, one)):
         g.set_traversal(trav)
         ref = orc.render(view, proj, W, H, 0.0, oracle.ALPHA)
-        check_alpha(gpu_frame(g, view, proj, W, H, vr.STEP_AUTO, vr.ALPHA), ref["image"], ref["flags"], 0.99, "auto step")
+        check_alpha(gpu_frame(g, view, proj, W, H, vr.STEP_AUTO, vr.ALPHA), ref, 0.99, "auto step")
         assert g.debug_stats()["samples"] == int(ref["counts"][..., 0].sum())
-        check_mip(gpu_frame(g, view, proj, W, H, vr.STEP_AUTO, vr.MIP), orc.render(view, proj, W, H, 0.0, oracle.MIP)["image"], "auto step")
+        check_mip(gpu_frame(g, view, proj, W, H, vr.STEP_AUTO, vr.MIP), orc.render(view, proj, W, H, 0.0, oracle.MIP), "auto step")
     # axis-aligned orthographic view: the per-ray step is exactly 1
     g.set_traversal(vr.SORT_LAST)
     view = synth.look_at((33, 25, -10.0), (33, 25, 0.0), (0.0, 1.0, 0.0))
@@ -253,12 +283,12 @@ def test_odd_bricks_ghosts_and_generic_layouts(vr, monkeypatch, brick, ghost, ti
     view, proj = fr.seeded(4, 2), fr.proj(False)
     assert np.array_equal(g.debug_brick_order(view, proj), o.brick_order(view, proj))
     ref = o.render(view, proj, W, H, 0.5, oracle.ALPHA)
-    check_alpha(gpu_frame(g, view, proj, W, H, 0.5, vr.ALPHA), ref["image"], ref["flags"], 0.99, "sort-last")
-    check_mip(gpu_frame(g, view, proj, W, H, 0.5, vr.MIP), o.render(view, proj, W, H, 0.5, oracle.MIP)["image"], "sort-last")
+    check_alpha(gpu_frame(g, view, proj, W, H, 0.5, vr.ALPHA), ref, 0.99, "sort-last")
+    check_mip(gpu_frame(g, view, proj, W, H, 0.5, vr.MIP), o.render(view, proj, W, H, 0.5, oracle.MIP), "sort-last")
     g.set_traversal(vr.FUSED)
     ref = one.render(view, proj, W, H, 0.5, oracle.ALPHA)
-    check_alpha(gpu_frame(g, view, proj, W, H, 0.5, vr.ALPHA), ref["image"], ref["flags"], 0.99, "fused")
-    check_mip(gpu_frame(g, view, proj, W, H, 0.5, vr.MIP), one.render(view, proj, W, H, 0.5, oracle.MIP)["image"], "fused")
+    check_alpha(gpu_frame(g, view, proj, W, H, 0.5, vr.ALPHA), ref, 0.99, "fused")
+    check_mip(gpu_frame(g, view, proj, W, H, 0.5, vr.MIP), one.render(view, proj, W, H, 0.5, oracle.MIP), "fused")
 
 
 # --------------------------------------------------------------------------- f1 data range, culling
@@ -327,7 +357,7 @@ def test_transparent_bricks_are_culled_exactly(vr):
     subs = g.debug_subimages(pix)                    # [npix][nbricks][4]: culled bricks deliver nothing
     assert np.all(subs[:, transparent, :] == 0.0)
     ref = o.render(view, proj, W, H, 0.5, oracle.ALPHA)
-    check_alpha(on, ref["image"], ref["flags"], 0.99, "culled frame")
+    check_alpha(on, ref, 0.99, "culled frame")
     g.set_culling(False)
     off = gpu_frame(g, view, proj, W, H, 0.5, vr.ALPHA)
     assert g.debug_stats()["bricks_culled"] == 0
@@ -344,7 +374,7 @@ def test_transparent_bricks_are_culled_exactly(vr):
     n_on = g.debug_stats()["samples"]
     assert np.array_equal(f_on, f_off) and n_on < 0.8 * n_off
     r1 = one.render(view, proj, W, H, 0.5, oracle.ALPHA)
-    check_alpha(f_on, r1["image"], r1["flags"], 0.99, "fused, culled")
+    check_alpha(f_on, r1, 0.99, "fused, culled")
     g.set_counting(0)
     g.set_traversal(vr.SORT_LAST)
     g.set_culling(False)
@@ -355,7 +385,7 @@ def test_transparent_bricks_are_culled_exactly(vr):
     g.set_culling(False)
     m_off = gpu_frame(g, view, proj, W, H, 0.5, vr.MIP)
     assert np.array_equal(m_on, m_off)
-    check_mip(m_on, o.render(view, proj, W, H, 0.5, oracle.MIP)["image"], "MIP with data-max stop")
+    check_mip(m_on, o.render(view, proj, W, H, 0.5, oracle.MIP), "MIP with data-max stop")
 
 
 # --------------------------------------------------------------------------- R19 macro-cell skipping
@@ -414,7 +444,7 @@ def test_macro_cell_skipping_is_exact(vr):
         assert np.array_equal(on, off) and on[..., 3].max() > 0.2
         assert n_on < 0.5 * n_off
         ref = orc.render(view, proj, W, H, 0.5, oracle.ALPHA)
-        check_alpha(on, ref["image"], ref["flags"], 0.99, "macro-cell skipping")
+        check_alpha(on, ref, 0.99, "macro-cell skipping")
         assert n_off == int(ref["counts"][..., 0].sum())
     # a new transfer function re-flags the cells; one without transparent entries switches skipping off
     g.set_traversal(vr.SORT_LAST)
@@ -422,7 +452,7 @@ def test_macro_cell_skipping_is_exact(vr):
     g.set_transfer_function(synth.tf_ramp(), synth.TF_VMIN, synth.TF_VMAX)
     o.set_transfer_function(synth.tf_ramp(), synth.TF_VMIN, synth.TF_VMAX)
     ref = o.render(view, proj, W, H, 0.5, oracle.ALPHA)
-    check_alpha(gpu_frame(g, view, proj, W, H, 0.5, vr.ALPHA), ref["image"], ref["flags"], 0.99, "ramp after threshold")
+    check_alpha(gpu_frame(g, view, proj, W, H, 0.5, vr.ALPHA), ref, 0.99, "ramp after threshold")
     # nothing is skipped any more (a termination decided in float32 may differ by one sample on a few rays, R12)
     assert abs(g.debug_stats()["samples"] - int(ref["counts"][..., 0].sum())) <= 1e-4 * ref["counts"][..., 0].sum()
 
@@ -456,7 +486,7 @@ def test_mip_steps_over_empty_space_exactly(vr):
         n_off = g.debug_stats()["samples"]
         assert np.array_equal(on, off) and n_on < 0.6 * n_off
         assert n_off == int(ref["counts"][..., 0].sum())
-        check_mip(on, ref["image"], "MIP over empty space")
+        check_mip(on, ref, "MIP over empty space")
     # a noise cube has no empty space: the feature stays off and every sample is taken
     noise = synth.Cube(34, 64, 48, 40, 2)
     gn, on_ = make_pair(noise, 16, 1)
@@ -464,7 +494,7 @@ def test_mip_steps_over_empty_space_exactly(vr):
     r2 = on_.render(view, proj, 64, 48, 0.5, oracle.MIP)
     fr2 = synth.Framing(64, 48, 40, 64, 48)
     r2 = on_.render(fr2.seeded(1, 0), fr2.proj(False), 64, 48, 0.5, oracle.MIP)
-    check_mip(gpu_frame(gn, fr2.seeded(1, 0), fr2.proj(False), 64, 48, 0.5, vr.MIP), r2["image"], "noise MIP")
+    check_mip(gpu_frame(gn, fr2.seeded(1, 0), fr2.proj(False), 64, 48, 0.5, vr.MIP), r2, "noise MIP")
     assert gn.debug_stats()["samples"] == int(r2["counts"][..., 0].sum())
 
 
@@ -491,9 +521,9 @@ def test_fused_traversal_equals_single_brick_oracle(vr, tau, ortho):
     fa = gpu_frame(g, view, proj, W, H, 0.5, vr.ALPHA)
     assert g.launch_count() - l0 == 2                                  # set-up + one fused kernel, no compositing
     ref = one.render(view, proj, W, H, 0.5, oracle.ALPHA)
-    check_alpha(fa, ref["image"], ref["flags"], tau, "fused alpha")
+    check_alpha(fa, ref, tau, "fused alpha")
     fm = gpu_frame(g, view, proj, W, H, 0.5, vr.MIP)
-    check_mip(fm, one.render(view, proj, W, H, 0.5, oracle.MIP)["image"], "fused mip")
+    check_mip(fm, one.render(view, proj, W, H, 0.5, oracle.MIP), "fused mip")
     g.set_traversal(vr.SORT_LAST)
     sm = gpu_frame(g, view, proj, W, H, 0.5, vr.MIP)
     check_mip(fm, sm, "fused vs sort-last mip")
@@ -532,8 +562,8 @@ def test_fused_traversal_edge_cases(vr):
 
     def both(view, proj, w, h, step, what):
         ref = one.render(view, proj, w, h, step, oracle.ALPHA)
-        check_alpha(gpu_frame(g, view, proj, w, h, step, vr.ALPHA), ref["image"], ref["flags"], 0.99, what)
-        check_mip(gpu_frame(g, view, proj, w, h, step, vr.MIP), one.render(view, proj, w, h, step, oracle.MIP)["image"], what)
+        check_alpha(gpu_frame(g, view, proj, w, h, step, vr.ALPHA), ref, 0.99, what)
+        check_mip(gpu_frame(g, view, proj, w, h, step, vr.MIP), one.render(view, proj, w, h, step, oracle.MIP), what)
 
     both(synth.look_at((20.3, 18.1, 14.2), (60, 40, 22), (0, 0, 1)), synth.perspective(70, W / H, 0.25, 200.0), W, H, 0.5, "inside")
     behind = synth.look_at((20, 18, 300), (20, 18, 600), (0, 1, 0))
@@ -585,14 +615,14 @@ def test_nan_voxels_are_blanked(vr):
             ref = orc.render(view, proj, W, H, 0.5, oracle.ALPHA)
             img = gpu_frame(g, view, proj, W, H, 0.5, vr.ALPHA)
             assert np.isfinite(img).all()
-            check_alpha(img, ref["image"], ref["flags"], 2.0, "NaN " + tf_name)
+            check_alpha(img, ref, 2.0, "NaN " + tf_name)
             slack = 4 * int(((ref["flags"] & oracle.FLAG_NAN_MARGIN) != 0).sum())   # samples on the NaN-weight limit may go either way
             assert abs(g.debug_stats()["samples"] - int(ref["counts"][..., 0].sum())) <= slack
             g.set_culling(True)
             assert np.array_equal(gpu_frame(g, view, proj, W, H, 0.5, vr.ALPHA), img)
             refm = orc.render(view, proj, W, H, 0.5, oracle.MIP)
             imgm = gpu_frame(g, view, proj, W, H, 0.5, vr.MIP)
-            check_mip(imgm, refm["image"], "NaN MIP", flags=refm["flags"])
+            check_mip(imgm, refm, "NaN MIP")
             assert abs(g.debug_stats()["samples"] - int(refm["counts"][..., 0].sum())) <= slack
     # a fully blanked volume renders nothing
     gb = vr.Volume(24, 24, 24, 16, 1)
@@ -646,11 +676,11 @@ def test_randomised_configurations(vr, case):
     for trav, orc in ((vr.SORT_LAST, o), (vr.FUSED, one)):
         g.set_traversal(trav)
         ref = orc.render(view, proj, W, H, step, oracle.ALPHA)
-        check_alpha(gpu_frame(g, view, proj, W, H, step if step > 0 else vr.STEP_AUTO, vr.ALPHA), ref["image"], ref["flags"],
+        check_alpha(gpu_frame(g, view, proj, W, H, step if step > 0 else vr.STEP_AUTO, vr.ALPHA), ref,
                     tau, "case %d" % case)
         refm = orc.render(view, proj, W, H, step, oracle.MIP)
         got = gpu_frame(g, view, proj, W, H, step if step > 0 else vr.STEP_AUTO, vr.MIP)
-        check_mip(got, refm["image"], "case %d" % case, flags=refm["flags"])
+        check_mip(got, refm, "case %d" % case)
 
 
 # --------------------------------------------------------------------------- state across calls
@@ -734,7 +764,7 @@ def test_edge_cases(vr):
         f2 = synth.Framing(20, 18, 16, W, H)
         view, proj = f2.seeded(1, 0), f2.proj(False)
         ref = o.render(view, proj, W, H, 0.5, oracle.ALPHA)
-        check_alpha(gpu_frame(g, view, proj, W, H, 0.5, vr.ALPHA), ref["image"], ref["flags"], 0.99, "%dx%d" % (W, H))
+        check_alpha(gpu_frame(g, view, proj, W, H, 0.5, vr.ALPHA), ref, 0.99, "%dx%d" % (W, H))
     W, H = 64, 48
     # the volume is behind the camera / off screen: transparent black, both modes
     view = synth.look_at((10, 9, 200), (10, 9, 400), (0, 1, 0))
@@ -745,23 +775,23 @@ def test_edge_cases(vr):
     view = synth.look_at((10.3, 9.1, 8.2), (30, 20, 12), (0, 0, 1))
     proj = synth.perspective(70, W / H, 0.25, 100.0)
     ref = o.render(view, proj, W, H, 0.5, oracle.ALPHA)
-    check_alpha(gpu_frame(g, view, proj, W, H, 0.5, vr.ALPHA), ref["image"], ref["flags"], 0.99, "inside")
+    check_alpha(gpu_frame(g, view, proj, W, H, 0.5, vr.ALPHA), ref, 0.99, "inside")
     ref = o.render(view, proj, W, H, 0.5, oracle.MIP)
-    check_mip(gpu_frame(g, view, proj, W, H, 0.5, vr.MIP), ref["image"], "inside")
+    check_mip(gpu_frame(g, view, proj, W, H, 0.5, vr.MIP), ref, "inside")
     # a step longer than the volume: one (clipped) sample per ray; and a fine step
     view, proj = fr.seeded(1, 1), fr.proj(True)
     for step in (100.0, 0.1, 1.0):
         ref = o.render(view, proj, W, H, step, oracle.ALPHA)
-        check_alpha(gpu_frame(g, view, proj, W, H, step, vr.ALPHA), ref["image"], ref["flags"], 0.99, "step %g" % step)
+        check_alpha(gpu_frame(g, view, proj, W, H, step, vr.ALPHA), ref, 0.99, "step %g" % step)
         ref = o.render(view, proj, W, H, step, oracle.MIP)
-        check_mip(gpu_frame(g, view, proj, W, H, step, vr.MIP), ref["image"], "step %g" % step)
+        check_mip(gpu_frame(g, view, proj, W, H, step, vr.MIP), ref, "step %g" % step)
     # axis-aligned orthographic view: two direction components are exactly zero (R4)
     view = synth.look_at((10, 9, -10.0), (10, 9, 0.0), (0.0, 1.0, 0.0))
     proj = synth.orthographic(10, 9, 1.0, 46.0)
     ref = o.render(view, proj, 20, 18, 1.0, oracle.MIP)
-    check_mip(gpu_frame(g, view, proj, 20, 18, 1.0, vr.MIP), ref["image"], "axis-aligned")
+    check_mip(gpu_frame(g, view, proj, 20, 18, 1.0, vr.MIP), ref, "axis-aligned")
     ref = o.render(view, proj, 20, 18, 1.0, oracle.ALPHA)
-    check_alpha(gpu_frame(g, view, proj, 20, 18, 1.0, vr.ALPHA), ref["image"], ref["flags"], 0.99, "axis-aligned")
+    check_alpha(gpu_frame(g, view, proj, 20, 18, 1.0, vr.ALPHA), ref, 0.99, "axis-aligned")
     # host-memory entry gives the same frame
     view, proj = fr.seeded(1, 2), fr.proj(False)
     a = gpu_frame(g, view, proj, W, H, 0.5, vr.ALPHA)

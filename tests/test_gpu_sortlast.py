@@ -75,12 +75,12 @@ def test_merged_parts_are_the_frame_of_the_whole_volume(vr, nparts, tfname):
             what = "%d parts, view %d, step %g" % (nparts, k, step)
             ref = o.render(view, proj, W, H, step, oracle.ALPHA)
             got = merged_frame(vr, sortlast, parts, boxes, tree, dims, brick, view, proj, W, H, step, vr.ALPHA)
-            check_alpha(got, ref["image"], ref["flags"], 0.99, what)
+            check_alpha(got, ref, 0.99, what)
             one = gpu_frame(whole, view, proj, W, H, step, vr.ALPHA)
             assert np.abs(got - one).max() < 2e-6, what      # same sub-images, `over` regrouped
             refm = o.render(view, proj, W, H, step, oracle.MIP)
             gotm = merged_frame(vr, sortlast, parts, boxes, tree, dims, brick, view, proj, W, H, step, vr.MIP)
-            check_mip(gotm, refm["image"], what, flags=refm["flags"])
+            check_mip(gotm, refm, what)
             assert np.array_equal(gotm, gpu_frame(whole, view, proj, W, H, step, vr.MIP)), what   # max is exact
 
 
@@ -163,11 +163,11 @@ def test_parts_cull_and_skip_like_the_whole_volume(vr):
                 p.set_culling(cull)
             frames[cull] = merged_frame(vr, sortlast, parts, boxes, tree, dims, brick, view, proj, W, H, 0.8, vr.ALPHA)
         assert np.array_equal(frames[True], frames[False])
-        check_alpha(frames[True], ref["image"], ref["flags"], 2.0, "view %d" % k)
+        check_alpha(frames[True], ref, 2.0, "view %d" % k)
         for p in parts:
             p.set_traversal(vr.FUSED)
         fused = merged_frame(vr, sortlast, parts, boxes, tree, dims, brick, view, proj, W, H, 0.8, vr.ALPHA)
-        check_alpha(fused, ref["image"], ref["flags"], 2.0, "fused parts, view %d" % k)
+        check_alpha(fused, ref, 2.0, "fused parts, view %d" % k)
         for p in parts:
             p.set_traversal(vr.SORT_LAST)
     assert sum(p.debug_stats()["bricks_culled"] for p in parts) >= 0

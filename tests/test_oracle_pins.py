@@ -718,3 +718,155 @@ def test_nan_voxels_drop_the_samples_that_rest_on_them():
     blank.set_transfer_function(tf, 0.0, 1.0)
     for mode in (oracle.ALPHA, oracle.MIP):
         assert not blank.render(view, proj, n, n, 1.0, mode)["image"].any()
+
+
+# --------------------------------------------------------------------------- a2: rendering rectangles are TIGHT
+def test_rendering_rectangle_closed_form_axis_aligned():
+    """PAPER.md:150 (sec. 2.3.2), Fig. 4 :168: the rendering rectangle is the bounding box of the 8 projected vertices.
+    For the axis-aligned orthographic camera a brick [lo,hi) projects onto a pixel box known in closed form
+    (pixel i looks down x = nx - (i+1/2) nx/W, pixel j down y = (j+1/2) ny/H): the rectangle must EQUAL it, not
+    merely contain it - a whole-viewport rectangle or one rounded a pixel too wide fails here."""
+    nx, ny, nz, brick = 19, 11, 13, 5
+    W, H = 58, 47  # no brick face projects onto a pixel boundary: 58/19 and 47/11 times 5, 10, 15 are not integers
+    view, proj = ortho_along_z(nx, ny, nz)
+    vol = oracle.Volume(nx, ny, nz, brick, 1)
+    rects = vol.rects(view, proj, W, H)
+    assert vol.nbricks == 4 * 3 * 3
+    for b in range(vol.nbricks):
+        bx, by = b % 4, (b // 4) % 3
+        lo = (bx * brick, by * brick)
+        hi = (min(lo[0] + brick, nx), min(lo[1] + brick, ny))
+        ex0, ex1 = (nx - hi[0]) * W / nx, (nx - lo[0]) * W / nx  # the look-at basis mirrors x
+        ey0, ey1 = lo[1] * H / ny, hi[1] * H / ny
+        for e in (ex0, ex1, ey0, ey1):  # the closed form is robust: far from an integer, or exactly on the viewport edge
+            assert e in (0.0, float(W), float(H)) or abs(e - round(e)) > 1e-3
+        want = [math.floor(ex0), math.floor(ey0), math.ceil(ex1), math.ceil(ey1)]
+        # a face exactly on the viewport edge may round a hair outside it before clipping: same box
+        want = [max(want[0], 0), max(want[1], 0), min(want[2], W), min(want[3], H)]
+        assert rects[b].tolist() == want, (b, rects[b].tolist(), want)
+    # every pixel whose ray takes a sample in a brick lies in its rectangle AND the rectangle ends within one pixel
+    # of the first / last such pixel on every side (the rectangle covers every pixel the projection TOUCHES, a ray
+    # goes through a pixel's centre; a brick face parallel to the image plane has no sharp corner to miss)
+    data = np.ones((nz, ny, nx), dtype=np.float32)
+    vol = oracle.Volume(nx, ny, nz, brick, 1, data=data)
+    vol.set_transfer_function(const_tf((1, 1, 1), 0.5), 0.0, 2.0)
+    pix = np.array([(i, j) for j in range(H) for i in range(W)], dtype=np.int32)
+    res = vol.render(view, proj, W, H, 1.0, oracle.MIP, pixels=pix, want_sub=True)
+    for b in range(vol.nbricks):
+        hit = res["sub"][:, b, 1].reshape(H, W) > 0
+        js, is_ = np.nonzero(hit)
+        x0, y0, x1, y1 = rects[b].tolist()
+        assert x0 <= is_.min() <= x0 + 1 and y0 <= js.min() <= y0 + 1
+        assert x1 - 1 <= is_.max() + 1 <= x1 and y1 - 1 <= js.max() + 1 <= y1
+
+
+@pytest.mark.parametrize("ortho", [False, True])
+def test_rendering_rectangle_is_the_bounding_box_of_the_projected_brick(ortho):
+    """The same for seeded oblique views, against numpy's own matrices: a dense lattice of points on the brick's 12
+    edges (the 8 vertices included) is projected with P @ V; the rectangle must equal floor(min) .. ceil(max) of
+    the projected points, clipped to the viewport (tight AND conservative), also for bricks partly off screen."""
+    nx, ny, nz, brick = 37, 29, 23, 8
+    W, H = 203, 117
+    fr = synth.Framing(nx, ny, nz, W, H)
+    vol = oracle.Volume(nx, ny, nz, brick, 1)
+    g = [(n + brick - 1) // brick for n in (nx, ny, nz)]
+    t = np.linspace(0.0, 1.0, 33)
+    checked = clipped = 0
+    for k in range(6):
+        view = fr.seeded(31, k)
+        if ortho:
+            proj = synth.orthographic(0.6 * fr.R * fr.aspect, 0.6 * fr.R, fr.near, fr.far)  # zoomed in: bricks leave the viewport
+        else:
+            proj = synth.perspective(25.0, fr.aspect, fr.near, fr.far)
+        V, P = mats(view, proj)
+        M = P @ V
+        rects = vol.rects(view, proj, W, H)
+        for b in range(vol.nbricks):
+            bc = (b % g[0], (b // g[0]) % g[1], b // (g[0] * g[1]))
+            lo = np.array([c * brick for c in bc], dtype=np.float64)
+            hi = np.minimum(lo + brick, (nx, ny, nz))
+            pts = []
+            for a in range(3):  # 4 edges along each axis
+                for u in (lo, hi):
+                    for w in (lo, hi):
+                        p = np.empty((len(t), 3))
+                        p[:, a] = lo[a] + t * (hi[a] - lo[a])
+                        p[:, (a + 1) % 3] = u[(a + 1) % 3]
+                        p[:, (a + 2) % 3] = w[(a + 2) % 3]
+                        pts.append(p)
+            pts = np.concatenate(pts)
+            clip = np.c_[pts, np.ones(len(pts))] @ M.T
+            assert (clip[:, 3] > 0).all()  # the camera is outside the volume in these views
+            px = (clip[:, 0] / clip[:, 3] + 1.0) * 0.5 * W
+            py = (clip[:, 1] / clip[:, 3] + 1.0) * 0.5 * H
+            ext = [px.min(), py.min(), px.max(), py.max()]
+            if any(abs(e - round(e)) < 1e-7 for e in ext):
+                continue  # a vertex on a pixel boundary: floor / ceil is a coin toss between two valid boxes
+            want = [int(np.clip(math.floor(ext[0]), 0, W)), int(np.clip(math.floor(ext[1]), 0, H)),
+                    int(np.clip(math.ceil(ext[2]), 0, W)), int(np.clip(math.ceil(ext[3]), 0, H))]
+            assert rects[b].tolist() == want, (k, b, rects[b].tolist(), want)
+            checked += 1
+            clipped += want != [math.floor(ext[0]), math.floor(ext[1]), math.ceil(ext[2]), math.ceil(ext[3])]
+    assert checked > 300 and clipped > 20
+
+
+def test_rendering_rectangle_with_a_vertex_behind_the_eye_is_the_viewport():
+    """a projected vertex is only meaningful in front of the eye; a brick with a vertex at clip w <= 0
+    gets the whole viewport (conservative), bricks entirely in front keep tight boxes."""
+    nx = ny = nz = 16
+    vol = oracle.Volume(nx, ny, nz, 8, 1)
+    W, H = 64, 48
+    view = synth.look_at((8.0, 8.0, 6.0), (8.0, 8.0, 16.0), (0.0, 1.0, 0.0))  # inside, looking up +z
+    proj = synth.perspective(60.0, W / H, 0.1, 100.0)
+    rects = vol.rects(view, proj, W, H)
+    for b in range(8):
+        if b < 4:   # z in [0, 8): holds vertices behind the eye plane z = 6
+            assert rects[b].tolist() == [0, 0, W, H]
+        else:       # z in [8, 16]: in front; its far face is smaller than the viewport in one direction at least
+            x0, y0, x1, y1 = rects[b]
+            assert (x1 - x0) * (y1 - y0) < W * H
+
+
+def test_margin_candidates_of_the_oracle():
+    """R12 test hooks: on data without marginal decisions the candidate frames (tau -/+ 1e-5, NaN limit x0.5 / x2)
+    equal the frame itself; with a blanked voxel and a sample whose NaN weight sits inside the flag's band the two
+    limits give the dropped and the kept value, and the nominal limit gives one of them."""
+    nx, ny, nz = 12, 10, 9
+    data = small_noise(nx, ny, nz)
+    W, H = 24, 20
+    fr = synth.Framing(nx, ny, nz, W, H)
+    view, proj = fr.seeded(2, 1), fr.proj(False)
+    vol = oracle.Volume(nx, ny, nz, 5, 1, data=data)
+    vol.set_transfer_function(synth.tf_translucent(), -3, 10)
+    ref = vol.render(view, proj, W, H, 0.5, oracle.ALPHA)
+    assert not ref["flags"].any() or not (ref["flags"] & (oracle.FLAG_ERT_MARGIN | oracle.FLAG_NAN_MARGIN)).any()
+    for dtau, ns in ((-1e-5, 1.0), (1e-5, 1.0), (0.0, 0.5), (0.0, 2.0)):
+        assert np.array_equal(ref["alt"](dtau, ns)["image"], ref["image"])
+    assert np.array_equal(vol.render(view, proj, W, H, 0.5, oracle.ALPHA)["image"], ref["image"])  # the hooks were reset
+    # one blanked voxel on the axis of an axis-aligned ray bundle; lateral offset chosen so that the NaN corner's
+    # weight is 3e-6 (inside (2e-6, 8e-6)): dropped with the limit at 2e-6, kept and renormalised at 4e-6 and 8e-6
+    n = 8
+    d = np.full((n, n, n), 2.0, dtype=np.float32)
+    d[:, 3, 3] = np.nan  # a blanked line of voxels along z at x = y = 3 (centres at 3.5)
+    o = oracle.Volume(n, n, n, 8, 1, data=d)
+    o.set_transfer_function(synth.tf_ramp(), 0.0, 4.0)
+    eps = 3e-6
+    view2 = synth.look_at((2.5 + eps, 2.5, -10.0), (2.5 + eps, 2.5, 0.0), (0.0, 1.0, 0.0))
+    proj2 = synth.orthographic(1e-3, 1e-3, 1.0, 40.0)
+    r = o.render(view2, proj2, 1, 1, 1.0, oracle.MIP)
+    # pixel (0,0) looks down x = 2.5 + eps (mirrored basis: centre pixel = centre line), y = 2.5: weights on the
+    # x = 3 column are eps, on y = 3 are 0, so the NaN corner (3,3) has weight 0 ... the ray is kept at any limit
+    assert r["image"][0, 0, 3] == 1.0
+    view3 = synth.look_at((3.0 - eps, 3.0 - 1e-9, -10.0), (3.0 - eps, 3.0 - 1e-9, 0.0), (0.0, 1.0, 0.0))
+    r = o.render(view3, proj2, 1, 1, 1.0, oracle.MIP)
+    # x = 3 - eps -> q_x = 2.5 - eps: cell 2, weight on column 3 = 0.5 - eps; y likewise ~0.5: N ~ 0.25: dropped at every limit
+    assert r["image"][0, 0, 3] == 0.0
+    # weight exactly in the band: sample at q = (2 + s, 2 + s) with s^2 = 3e-6
+    s = math.sqrt(3e-6)
+    view4 = synth.look_at((2.5 + s, 2.5 + s, -10.0), (2.5 + s, 2.5 + s, 0.0), (0.0, 1.0, 0.0))
+    r = o.render(view4, proj2, 1, 1, 1.0, oracle.MIP)
+    assert (r["flags"] & oracle.FLAG_NAN_MARGIN).all()
+    kept, dropped = r["alt"](0.0, 2.0), r["alt"](0.0, 0.5)
+    assert kept["image"][0, 0, 3] == 1.0 and kept["counts"][0, 0, 0] == n
+    assert dropped["image"][0, 0, 3] == 0.0 and dropped["counts"][0, 0, 0] == 0
+    assert np.array_equal(r["image"], kept["image"])  # 3e-6 < 4e-6: the nominal limit keeps it
