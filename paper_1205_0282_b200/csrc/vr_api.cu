@@ -30,6 +30,8 @@ struct vr_volume {
     VrCompLayer* d_layers;
     void* d_sub;             /* sub-image scratch, sub_capacity_px * 16 bytes */
     long long sub_capacity_px;
+    double2* d_rays;         /* the frame's ray table: VR_RAY_WORDS planes of ray_capacity_px entries */
+    long long ray_capacity_px;
     float* d_frame;          /* vr_render_host's device frame */
     long long frame_capacity_px;
     float* d_pipe[2];        /* vr_render_host_async: two device frames, ... */
@@ -102,6 +104,7 @@ static void release(vr_volume* v) {
     cudaFree(v->d_item_prefix);
     cudaFree(v->d_layers);
     cudaFree(v->d_sub);
+    cudaFree(v->d_rays);
     cudaFree(v->d_frame);
     for (int i = 0; i < 2; ++i) {
         cudaFree(v->d_pipe[i]);
@@ -512,6 +515,20 @@ static int ensure_sub(vr_volume* v, long long need_px) {
     return VR_OK;
 }
 
+/* The ray table of a W x H frame (vr_rays.cu). */
+static int ensure_rays(vr_volume* v, long long px) {
+    if (px <= v->ray_capacity_px) return VR_OK;
+    if (v->d_rays) {
+        VR_CUDA(v, cudaDeviceSynchronize());
+        cudaFree(v->d_rays);
+        v->d_rays = NULL;
+        v->ray_capacity_px = 0;
+    }
+    VR_CUDA(v, cudaMalloc(&v->d_rays, (size_t)px * VR_RAY_WORDS * sizeof(double2)));
+    v->ray_capacity_px = px;
+    return VR_OK;
+}
+
 /* Row f1: bring the range table up to date with the store (three launches, after an upload only). */
 static int ensure_minmax(vr_volume* v, cudaStream_t st) {
     if (v->mm_valid) return VR_OK;
@@ -706,6 +723,10 @@ static int render_frame(vr_volume* v, const float* view, const float* proj, int 
     if (!v->has_data) return fail(v, VR_ERR_STATE, "vr_render: nothing uploaded");
     rc = ensure_sub(v, sub_px);
     if (rc) return rc;
+    if (v->traversal == VR_SORT_LAST) {
+        rc = ensure_rays(v, (long long)width * height);
+        if (rc) return rc;
+    }
     cudaStream_t st = (cudaStream_t)stream;
     const bool timing = v->timing;
     cudaEvent_t* ev = v->ev[v->timed_frames % VR_EV_RING];
@@ -729,11 +750,17 @@ static int render_frame(vr_volume* v, const float* view, const float* proj, int 
     if (timing) VR_CUDA(v, cudaEventRecord(ev[0], st));
     rc = run_setup(v, view, proj, width, height, mode, v->culling, st);
     if (rc) return rc;
+    if (v->traversal == VR_SORT_LAST) { /* the per-ray part of row a4, once per pixel: part of the set-up stage */
+        VR_CUDA(v, vr_launch_rays(v->grid, v->d_vs, width, height, (double)step, v->d_rays, st));
+        v->launches++;
+    }
     if (timing) VR_CUDA(v, cudaEventRecord(ev[1], st));
 
     VrRaycastParams p;
     p.grid = v->grid;
     p.bricks = v->bricks;
+    p.rays = v->d_rays;
+    p.ray_plane = (long long)width * height;
     p.vs = v->d_vs;
     p.bv = v->d_bv;
     p.order = v->d_order;

@@ -18,6 +18,7 @@
 #define VR_INTERNAL_CUH
 
 #include <cuda_runtime.h>
+#include <stddef.h>
 #include <stdint.h>
 
 #include "../../include/vr.h"
@@ -94,6 +95,8 @@ struct VrViewState {
                      * blank outside it, which the compositing kernel uses to leave early */
 };
 
+static_assert(offsetof(VrViewState, bound) % 16 == 0, "VrViewState::bound is read as one int4");
+
 struct VrBrickView {
     int rx0, ry0, rx1, ry1; /* rendering rectangle, half-open, clipped */
     int lx0, ly0, lx1, ly1; /* launch rectangle: the same, grown to the 8x4 tile grid */
@@ -121,9 +124,19 @@ struct VrLut {
     float scale; /* n - 1 as float: u -> table coordinate */
 };
 
+/* Per-frame ray table ("each GPU kernel then starts by calculating its ray's start location,
+ * orientation" - once per RAY, not once per (ray, brick)): VR_RAY_WORDS double2 planes of W*H entries each,
+ * plane a at rays + a * (W*H), entry of pixel (i, j) at j*W + i:
+ *   0 (o0, o1)  1 (o2, d0)  2 (d1, d2)  3 (t0, t1)  4 (step, K as a double; 0 = the ray misses the volume)
+ *   5 (1/d0, 1/d1)  6 (1/d2, 1/step)      -- used for estimates only (brick_range)
+ * Written by vr_rays_kernel for the pixels inside VrViewState::bound, read by the ray-cast kernel. */
+#define VR_RAY_WORDS 7
+
 struct VrRaycastParams {
     VrGrid grid;
     const float* bricks;
+    const double2* rays; /* the frame's ray table */
+    long long ray_plane; /* entries per plane = W*H */
     const VrViewState* vs;
     const VrBrickView* bv;
     const int* order;
@@ -168,6 +181,8 @@ __host__ __device__ __forceinline__ unsigned vr_cell_offset(const VrGrid& g, int
 cudaError_t vr_launch_setup(const VrGrid& grid, const VrMatrices& mats, int W, int H, int mode,
                             long long sub_capacity_px, void* sub_base, VrViewState* vs, VrBrickView* bv, int* order,
                             int* item_prefix, VrCompLayer* layers, const float2* range, const VrLut& lut, cudaStream_t st);
+/* ray table of the frame whose set-up is in vs (row a4, the per-ray part) */
+cudaError_t vr_launch_rays(const VrGrid& grid, const VrViewState* vs, int W, int H, double step, double2* rays, cudaStream_t st);
 cudaError_t vr_launch_minmax(const VrGrid& grid, const float* bricks, int2* enc, float2* table, cudaStream_t st);
 /* macro-cells (R19): per-cell (min, max) of the 4x4x2-tiled store; transparency bits for a LUT */
 cudaError_t vr_launch_cell_minmax(const VrGrid& grid, const float* bricks, float2* cell_mm, const int nc[3], cudaStream_t st);

@@ -28,6 +28,7 @@ struct RaySetup {
     double t0, t1;
     double step; /* sample spacing along this ray (R5); per ray when the caller asks for the paper's rule (R18) */
     int K; /* number of scheduled samples; 0 = miss */
+    double inv_d[3], inv_step; /* 1/d_a (0 where d_a == 0) and 1/step: for the estimates of brick_range only */
 };
 
 /* R1, R2: pixel (i,j), centres at half-integers, row 0 at the bottom; ray from the near plane
@@ -86,6 +87,9 @@ __device__ __forceinline__ void ray_setup(const double* __restrict__ Minv, int W
             if (tb < tout) tout = tb;
         }
     }
+#pragma unroll
+    for (int a = 0; a < 3; ++a) r.inv_d[a] = r.d[a] == 0.0 ? 0.0 : 1.0 / r.d[a];
+    r.inv_step = 1.0 / step;
     r.K = 0;
     r.t0 = 0.0;
     r.t1 = 0.0;
@@ -99,6 +103,34 @@ __device__ __forceinline__ void ray_setup(const double* __restrict__ Minv, int W
             r.K = kd > 1073741824.0 ? 1073741824 : (int)kd;
         }
     }
+}
+
+/* The ray of pixel p = j*W + i from the frame's ray table (VrRaycastParams::rays): the values ray_setup computed,
+ * bit for bit. FULL = false loads only what the exit samples need (o, d, t0, t1, step). */
+template <bool FULL>
+__device__ __forceinline__ void ray_load(const double2* __restrict__ rays, long long plane, long long p, RaySetup& r) {
+    const double2 a0 = __ldg(rays + p), a1 = __ldg(rays + plane + p), a2 = __ldg(rays + 2 * plane + p),
+                  a3 = __ldg(rays + 3 * plane + p), a4 = __ldg(rays + 4 * plane + p);
+    r.o[0] = a0.x, r.o[1] = a0.y, r.o[2] = a1.x;
+    r.d[0] = a1.y, r.d[1] = a2.x, r.d[2] = a2.y;
+    r.t0 = a3.x, r.t1 = a3.y;
+    r.step = a4.x;
+    r.K = (int)a4.y;
+    if (FULL) {
+        const double2 a5 = __ldg(rays + 5 * plane + p), a6 = __ldg(rays + 6 * plane + p);
+        r.inv_d[0] = a5.x, r.inv_d[1] = a5.y, r.inv_d[2] = a6.x;
+        r.inv_step = a6.y;
+    }
+}
+
+__device__ __forceinline__ void ray_store(double2* __restrict__ rays, long long plane, long long p, const RaySetup& r) {
+    rays[p] = make_double2(r.o[0], r.o[1]);
+    rays[plane + p] = make_double2(r.o[2], r.d[0]);
+    rays[2 * plane + p] = make_double2(r.d[1], r.d[2]);
+    rays[3 * plane + p] = make_double2(r.t0, r.t1);
+    rays[4 * plane + p] = make_double2(r.step, (double)r.K);
+    rays[5 * plane + p] = make_double2(r.inv_d[0], r.inv_d[1]);
+    rays[6 * plane + p] = make_double2(r.inv_d[2], r.inv_step);
 }
 
 /* R5: sample k stands for the interval [t0 + k step, min(t0 + (k+1) step, t1)]: s = its
@@ -194,7 +226,7 @@ __device__ __forceinline__ void brick_range(const RaySetup& r, const VrGrid& g, 
         if (r.d[a] == 0.0) {
             if ((!first && r.o[a] < (double)lo[a] - 1e-6) || (!last && r.o[a] > (double)hi[a] + 1e-6)) miss = true;
         } else {
-            const double inv = 1.0 / r.d[a];
+            const double inv = r.inv_d[a];
             double ta = ((double)lo[a] - r.o[a]) * inv, tb = ((double)hi[a] - r.o[a]) * inv;
             const bool swap = ta > tb;
             if (swap) {
@@ -209,7 +241,7 @@ __device__ __forceinline__ void brick_range(const RaySetup& r, const VrGrid& g, 
         }
     }
     if (miss || tout < tin - 1e-6 * (1.0 + fabs(tin))) return;
-    const double inv_step = 1.0 / r.step;
+    const double inv_step = r.inv_step;
     const double e_lo = ceil((tin - r.t0) * inv_step - 0.5);
     const double e_hi = ceil((tout - r.t0) * inv_step - 0.5);
     const int est_lo = e_lo < 0.0 ? 0 : (e_lo > (double)r.K ? r.K : (int)e_lo);

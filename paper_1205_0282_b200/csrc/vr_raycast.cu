@@ -37,7 +37,6 @@ vr_raycast_kernel(const VrRaycastParams prm) {
     /* dynamic: 2 * lut.n float4 (ALPHA) - a 256-entry table takes 8 KB, not the 32 KB of the
      * largest one, and what it does not take stays L1 cache */
     extern __shared__ float4 s_lut[];
-    __shared__ double s_minv[16];
 
     const VrGrid& g = prm.grid;
     const int lane = threadIdx.x & 31;
@@ -47,13 +46,11 @@ vr_raycast_kernel(const VrRaycastParams prm) {
             s_lut[2 * i + 1] = prm.lut.delta[i];
         }
     }
-    if (threadIdx.x < 16) s_minv[threadIdx.x] = prm.vs->Minv[threadIdx.x];
     __syncthreads();
     if (prm.vs->singular) return;
 
     const int W = prm.vs->W, H = prm.vs->H;
     const int total = prm.vs->total_items;
-    const double step = prm.step;
     const float tau = prm.tau;
     LutView lut;
     lut.base = 0;
@@ -102,10 +99,11 @@ vr_raycast_kernel(const VrRaycastParams prm) {
 
         RaySetup ray;
         ray.K = 0;
-        ray.step = step;
+        ray.step = 1.0;
         int k_lo = 0, k_hi = 0;
+        const long long ray_p = (long long)pj * W + pi;
         if (in_rect) {
-            ray_setup(s_minv, W, H, pi, pj, g, step, ray);
+            ray_load<true>(prm.rays, prm.ray_plane, ray_p, ray);
             brick_range(ray, g, bc, blo, bhi, k_lo, k_hi);
         }
         /* lattice samples: k in [k_lo, k_lat); samples k >= K-2 (whose interval may be clipped
@@ -201,9 +199,9 @@ vr_raycast_kernel(const VrRaycastParams prm) {
         if (__any_sync(FULL_MASK, k_tail < k_hi && !stopped)) {
 #if VR_RECOMPUTE_TAIL
             if (k_tail < k_hi && !stopped) {
-                int qi = pi, qj = pj; /* opaque copies: the ray is rebuilt, not kept in registers */
-                asm volatile("" : "+r"(qi), "+r"(qj));
-                ray_setup(s_minv, W, H, qi, qj, g, step, ray);
+                long long q = ray_p; /* an opaque copy: the ray is read again, not kept in registers through the loop */
+                asm volatile("" : "+l"(q));
+                ray_load<false>(prm.rays, prm.ray_plane, q, ray);
             }
 #endif
             for (int k = k_tail; k < k_hi && !stopped; ++k) {

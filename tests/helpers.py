@@ -93,9 +93,10 @@ def check_alpha(gpu, ref, tau, what="", key="image"):
     bad = err > ALPHA_TOL
     assert not bad.any(), "%s ALPHA: %d pixels off, max err %.3e (unflagged max %.3e)" % (
         what, int(bad.sum()), err.max(), err[~loose].max() if (~loose).any() else 0.0)
-    # R12: a ray whose opacity passes tau in steps of dA is flagged with probability ~2e-5/dA (a few per cent at
-    # most on the ramp); R14: few samples sit on the NaN-weight limit
-    assert ert.mean() < 0.03, "%s: %.4f%% early-termination-margin pixels" % (what, 100 * ert.mean())
+    # R12: a (ray, brick) whose opacity passes tau in steps of dA is flagged with probability ~2e-5/dA (1-2 % on the
+    # ramp), a pixel if any of the bricks its ray saturates is (measured: up to 6.5 % of a block of c3 pixels that all hit
+    # the cube). Flagged pixels are checked above like the others, so this is a sanity bound on the flag, not an allowance.
+    assert ert.mean() < 0.10, "%s: %.4f%% early-termination-margin pixels" % (what, 100 * ert.mean())
     assert nanm.mean() <= 0.01, "%s: %.2f %% of the pixels sit on the NaN-weight limit" % (what, 100 * nanm.mean())
     return float(err.max())
 

@@ -208,5 +208,5 @@ def test_bench_brick_sharded_arm_as_a_world_of_one(vr):
     line = json.loads(r.stdout.strip().splitlines()[-1])
     assert line["metric"] == "frames_per_s" or line["unit"] == "frames/s"
     assert line["n_gpus"] == 1 and line["scaling"] == "strong" and line["value"] > 0 and line["e2e"]["value"] > 0
-    assert line["gpu_launches"] == 6 * 4            # set-up, ray cast, stage-1 compositing, merge
+    assert line["gpu_launches"] == 6 * 5            # set-up, ray table, ray cast, stage-1 compositing, merge
     assert line["exchange_bytes_per_frame"] == 0    # a world of one sends nothing
