@@ -591,7 +591,8 @@ def config_of(wl, args):
                         "early termination %.2f%s" % (
                             wl["name"], wl["nx"], wl["ny"], wl["nz"], what, wl["brick"], wl["ghost"], wl["width"], wl["height"],
                             wl["view_kind"], args.mode.upper(), wl["step"], args.tf, wl["tau"],
-                            ", fused traversal" if getattr(args, "traversal", "sort_last") == "fused" else ""),
+                            (", fused traversal" if getattr(args, "traversal", "sort_last") == "fused" else "") +
+                            (", texture sampler" if getattr(args, "sampler", "manual") == "texture" else "")),
             "baseline_config_index": int(wl["name"][1:]) if wl["name"][0] == "c" else None,
             "cube_gb": round(wl["nx"] * wl["ny"] * wl["nz"] * 4 / 1e9, 2),
             "l2_policy": "inputs larger than L2 (every frame streams a new view's share of the cube); no explicit flush",
@@ -647,6 +648,8 @@ def run_c4(args, vr, peak, peak_src, sampler):
     g = None
     if args.c4_part != "composite":
         g, _ = build_volume(vr, wl, synth.tf_ramp())
+        if args.sampler == "texture":
+            g.set_sampler(vr.SAMPLER_TEXTURE)
     for res in ((512, 1024, 2048, 4096) if g is not None else ()):
         w = dict(wl)
         w["width"] = w["height"] = res
@@ -735,6 +738,9 @@ def main():
                          "bricks = one cube over all ranks, sort-last (row f3, strong scaling)")
     ap.add_argument("--sortlast-parts", type=int, default=8,
                     help="row f3 report: parts of the k-d partition rendered one after the other on this GPU (0 = skip)")
+    ap.add_argument("--sampler", default="manual", choices=["manual", "texture"],
+                    help="row a5: hand-rolled float32 tri-linear from the tiled store (default) or the texture-object arm "
+                         "(ALPHA frames; a second copy of the bricks as 3-D CUDA arrays)")
     ap.add_argument("--no-variants", action="store_true")
     ap.add_argument("--probe", default=None, choices=["dram"],
                     help="dram: the DRAM fetch-granularity probe (vr_debug_probe_dram) instead of a workload; one JSON line")
@@ -803,6 +809,8 @@ def main():
     t_build = time.perf_counter()
     g, cube = build_volume(vr, wl, tf)
     t_build = time.perf_counter() - t_build
+    if args.sampler == "texture":
+        g.set_sampler(vr.SAMPLER_TEXTURE)
     W, H, K, Wm = wl["width"], wl["height"], args.steps, args.warmup
     out = torch.empty((H, W, 4), dtype=torch.float32, device="cuda")
     host_bufs = [torch.empty((H, W, 4), dtype=torch.float32).pin_memory() for _ in range(3)]

@@ -234,6 +234,24 @@ int vr_render(vr_volume* v, const float* view, const float* proj, int width, int
 #define VR_FUSED 1
 int vr_set_traversal(vr_volume* v, int traversal);
 
+/* Sampler of row a5 (north_star: bricks "either as 3D CUDA arrays behind texture objects or as a tiled linear
+ * layout with hand-rolled vectorised trilinear interpolation, whichever ncu shows is faster"; the paper's own
+ * design is the former, PAPER.md:150 sec. 2.3.2 "built-in tri-linear interpolation", :69).
+ * VR_SAMPLER_MANUAL (default): 8 float32 loads from the tiled store and 7 float32 FMA per sample.
+ * VR_SAMPLER_TEXTURE: VR_ALPHA frames of the VR_SORT_LAST traversal fetch each sample with one hardware-filtered
+ * texture read from a 3-D CUDA array per brick (float32 texels, linear filter, clamp addressing, unnormalised
+ * coordinates = R3's voxel-centre convention). The arrays are a SECOND copy of the handle's bricks, allocated
+ * by this call (VR_ERR_OUT_OF_MEMORY if they do not fit beside the store - the 103 GB cube - and the sampler
+ * stays as it was) and refilled from the store on the device by the first frame after an upload. The sample
+ * SET is unchanged (same FP64 set-up); the hardware's 8-bit interpolation weights perturb sample values by up
+ * to 2^-9 of the local voxel differences, which keeps VR_ALPHA inside its 2e-3 tolerance but moves early-
+ * termination decisions of rays whose opacity passes tau within ~1e-4 of it. VR_MIP frames (1e-5), fused
+ * frames and counting mode 2 always use the hand-rolled path; a sample whose filtered value is NaN (blanked
+ * voxels, R14) is re-evaluated from the float32 store by the exact rule. Needs the default (tiled) layout. */
+#define VR_SAMPLER_MANUAL 0
+#define VR_SAMPLER_TEXTURE 1
+int vr_set_sampler(vr_volume* v, int sampler);
+
 /* Same frame, delivered to HOST memory: renders into a library-owned device frame, copies it
  * to out_rgba_host ([height][width][4] float32; pinned memory makes the copy asynchronous
  * with respect to other streams) and waits for the copy. This is the end-to-end entry. */

@@ -37,6 +37,7 @@ def lib():
         L.vro_brick_transparent.argtypes = [vp, ci]
         L.vro_set_tau.argtypes = [vp, dbl]
         L.vro_set_nan_limit_scale.argtypes = [vp, dbl]
+        L.vro_set_ert_margin.argtypes = [vp, dbl]
         L.vro_set_order_override.argtypes = [vp, vp]
         L.vro_brick_order.argtypes = [vp, vp, vp, vp]
         L.vro_rects.argtypes = [vp, vp, vp, ci, ci, vp]
@@ -81,6 +82,7 @@ class Volume:
             lib().vro_set_procedural(self._h, fn, ctx)
         self.nbricks = lib().vro_num_bricks(self._h)
         self.tau = 0.99
+        self.ert_margin = 1e-5
 
     def __del__(self):
         try:
@@ -98,6 +100,11 @@ class Volume:
     def set_early_termination(self, tau):
         self.tau = float(tau)
         lib().vro_set_tau(self._h, self.tau)
+
+    def set_ert_margin(self, margin):
+        """R12 test hook: a termination test with |A_b - tau| < margin flags its pixel (default 1e-5)."""
+        self.ert_margin = float(margin)
+        lib().vro_set_ert_margin(self._h, self.ert_margin)
 
     def set_nan_limit_scale(self, scale):
         """R12/R14 test hook: R14's drop limit times `scale` (1 = nominal)."""
@@ -171,7 +178,7 @@ class Volume:
             out = out.reshape(height, width, 4)
             flags = flags.reshape(height, width)
             counts = counts.reshape(height, width, 2)
-        res = dict(image=out, flags=flags, counts=counts)
+        res = dict(image=out, flags=flags, counts=counts, ert_margin=self.ert_margin)
         if want_sub:
             res["sub"] = sub
 

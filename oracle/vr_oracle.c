@@ -69,6 +69,8 @@ typedef struct vro_volume {
     double tau;        /* early ray termination threshold; > 1 disables */
     int* order_override; /* test hook: composite in this order instead of R9's */
     int64_t ghost_violations; /* fetches that left the padded brick (R3) */
+    double ert_margin; /* R12: a termination test with |A_b - tau| below this flags the pixel (1e-5; the tests of the
+                        * texture sampler, whose 8-bit filter weights move A_b by ~1e-4, widen it) */
     double nan_limit;  /* R14: tri-linear weight on NaN corners above which a sample is dropped (VRO_NAN_WEIGHT); the
                         * tests move it by a factor 2 either way to obtain BOTH correct values of a flagged pixel (R12) */
 } vro_volume;
@@ -99,6 +101,7 @@ vro_volume* vro_create(int64_t nx, int64_t ny, int64_t nz, int brick, int ghost)
     v->nbricks = v->g[0] * v->g[1] * v->g[2];
     v->tau = 0.99;
     v->nan_limit = VRO_NAN_WEIGHT;
+    v->ert_margin = 1e-5;
     return v;
 }
 
@@ -228,6 +231,8 @@ int vro_set_tf(vro_volume* v, const float* rgba, int n, double vmin, double vmax
 void vro_set_tau(vro_volume* v, double tau) { v->tau = tau; }
 /* R12/R14 test hook: the drop limit of R14 scaled by `scale` (1 = the reading's 4e-6). The NAN_MARGIN flag keeps
  * marking samples within a factor 2 of the NOMINAL limit, so scale 0.5 drops and scale 2 keeps every flagged sample. */
+/* R12 test hook: width of the band around tau inside which a termination test flags its pixel (default 1e-5). */
+void vro_set_ert_margin(vro_volume* v, double margin) { v->ert_margin = margin; }
 void vro_set_nan_limit_scale(vro_volume* v, double scale) { v->nan_limit = VRO_NAN_WEIGHT * scale; }
 int vro_set_order_override(vro_volume* v, const int* order) {
     free(v->order_override);
@@ -574,7 +579,7 @@ static void render_pixel(vro_volume* v, const vro_view* vw, const int* order, in
             if (mode == VRO_ALPHA) {
                 /* step 7: brick-local early ray termination, tested before the sample (R8) */
                 if (B->stopped) continue;
-                if (fabs(B->A - v->tau) < 1e-5) fl |= VRO_FLAG_ERT_MARGIN;
+                if (fabs(B->A - v->tau) < v->ert_margin) fl |= VRO_FLAG_ERT_MARGIN;
                 if (B->A >= v->tau) { B->stopped = 1; any_stopped = 1; continue; }
             }
             /* step 5: value from the brick's own padded copy (R3) */

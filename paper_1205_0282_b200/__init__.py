@@ -15,6 +15,7 @@ import numpy as np
 
 ALPHA, MIP = 0, 1
 SORT_LAST, FUSED = 0, 1
+SAMPLER_MANUAL, SAMPLER_TEXTURE = 0, 1
 STEP_AUTO = 0.0  # vr_render step: the paper's per-ray step (R18)
 HOST, DEVICE = 0, 1
 LAYOUT_DEFAULT, LAYOUT_LINEAR, LAYOUT_TILED = 0, 1, 2
@@ -27,7 +28,7 @@ STATUS = {0: "VR_OK", 1: "VR_ERR_INVALID_ARG", 2: "VR_ERR_OUT_OF_MEMORY", 3: "VR
 # every symbol include/vr.h declares (tests check the library exports each of them)
 SYMBOLS = (
     "vr_volume_create", "vr_volume_create_layout", "vr_volume_destroy", "vr_volume_upload", "vr_volume_download", "vr_debug_brick_data",
-    "vr_set_transfer_function", "vr_set_early_termination", "vr_volume_minmax", "vr_set_culling", "vr_set_traversal", "vr_debug_brick_minmax", "vr_debug_cell_flags", "vr_render", "vr_render_host", "vr_render_host_async", "vr_render_host_wait", "vr_composite",
+    "vr_set_transfer_function", "vr_set_early_termination", "vr_volume_minmax", "vr_set_culling", "vr_set_traversal", "vr_set_sampler", "vr_debug_brick_minmax", "vr_debug_cell_flags", "vr_render", "vr_render_host", "vr_render_host_async", "vr_render_host_wait", "vr_composite",
     "vr_num_bricks", "vr_debug_brick_order", "vr_debug_rects", "vr_debug_ray_bricks", "vr_debug_subimages",
     "vr_volume_create_part", "vr_render_part", "vr_part_rect", "vr_composite_parts",
     "vr_set_counting", "vr_set_timing", "vr_debug_stats", "vr_debug_stage_times", "vr_debug_probe_dram", "vr_launch_count", "vr_last_error",
@@ -73,6 +74,7 @@ def lib():
         L.vr_volume_minmax.argtypes = [vp, vp, vp, vp]
         L.vr_set_culling.argtypes = [vp, ci]
         L.vr_set_traversal.argtypes = [vp, ci]
+        L.vr_set_sampler.argtypes = [vp, ci]
         L.vr_debug_brick_minmax.argtypes = [vp, vp]
         L.vr_debug_cell_flags.argtypes = [vp, ci, vp, vp]
         L.vr_render.argtypes = [vp, vp, vp, ci, ci, cf, ci, vp, vp]
@@ -219,6 +221,11 @@ class Volume:
     def set_traversal(self, traversal):
         """SORT_LAST (per-brick sub-images + compositing, the default) or FUSED (one ray through all bricks)."""
         self._check(lib().vr_set_traversal(self._h, int(traversal)))
+
+    def set_sampler(self, sampler):
+        """SAMPLER_MANUAL (hand-rolled float32 tri-linear, the default) or SAMPLER_TEXTURE (3-D CUDA arrays behind
+        texture objects for ALPHA frames; allocates a second copy of the bricks)."""
+        self._check(lib().vr_set_sampler(self._h, int(sampler)))
 
     def debug_brick_minmax(self):
         """[nbricks][2] float32: (min, max) per brick over its ghost-padded cells."""

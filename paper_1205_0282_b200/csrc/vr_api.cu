@@ -52,6 +52,9 @@ struct vr_volume {
     unsigned long long* d_cell_count;
     bool tf_has_zero;        /* the LUT has a run of >= 3 zero-alpha entries: skipping can do something */
     bool culling;
+    int sampler;             /* VR_SAMPLER_MANUAL or VR_SAMPLER_TEXTURE */
+    VrTexStore* tex;         /* texture arm of the store (allocated by vr_set_sampler) */
+    bool tex_valid;          /* the arrays hold the current contents of the store */
     int traversal;           /* VR_SORT_LAST or VR_FUSED */
     int counting;            /* 0 off, 1 samples, 2 samples + touched-cells bitmap */
     bool timing;
@@ -95,6 +98,7 @@ extern "C" int vr_num_bricks(const vr_volume* v) { return v ? v->grid.nbricks : 
 extern "C" int64_t vr_launch_count(const vr_volume* v) { return v ? v->launches : 0; }
 
 static void release(vr_volume* v) {
+    vr_tex_destroy(v->tex);
     cudaFree(v->bricks);
     cudaFree(v->d_lut_base);
     cudaFree(v->d_lut_delta);
@@ -349,6 +353,7 @@ extern "C" int vr_volume_upload(vr_volume* v, const float* src, int memspace, in
         }
     }
     v->has_data = true;
+    v->tex_valid = false;
     v->mm_valid = false;
     v->cell_mm_valid = v->cell_bits_valid = false;
     v->mip_skip_known = false;
@@ -628,6 +633,34 @@ extern "C" int vr_set_traversal(vr_volume* v, int traversal) {
     return VR_OK;
 }
 
+extern "C" int vr_set_sampler(vr_volume* v, int sampler) {
+    if (!v) return fail(NULL, VR_ERR_INVALID_ARG, "vr_set_sampler: NULL handle");
+    if (sampler != VR_SAMPLER_MANUAL && sampler != VR_SAMPLER_TEXTURE)
+        return fail(v, VR_ERR_INVALID_ARG, "vr_set_sampler: unknown sampler %d", sampler);
+    if (sampler == VR_SAMPLER_TEXTURE && !v->tex) {
+        const VrGrid& g = v->grid;
+        if (!(g.layout == VR_LAYOUT_TILED && g.tl[0] == 2 && g.tl[1] == 2 && g.tl[2] == 1 && g.ml[0] == 0 && g.ml[1] == 0 && g.ml[2] == 0))
+            return fail(v, VR_ERR_STATE, "vr_set_sampler: the texture arm is built beside the default (4x4x2 tiled) store only");
+        const cudaError_t e = vr_tex_create(g, &v->tex);
+        if (e != cudaSuccess)
+            return fail(v, e == cudaErrorMemoryAllocation ? VR_ERR_OUT_OF_MEMORY : VR_ERR_CUDA,
+                        "vr_set_sampler: 3-D arrays for %d bricks (%.2f GB beside the brick store): %s", g.nown,
+                        (double)g.slot * g.nown * 4.0 / 1e9, cudaGetErrorString(e));
+        v->tex_valid = false;
+    }
+    v->sampler = sampler;
+    return VR_OK;
+}
+
+/* texture arm: bring the arrays up to date with the store (one launch, after an upload only) */
+static int ensure_tex(vr_volume* v, cudaStream_t st) {
+    if (v->tex_valid) return VR_OK;
+    VR_CUDA(v, vr_launch_tex_fill(v->grid, v->bricks, v->tex, st));
+    v->launches++;
+    v->tex_valid = true;
+    return VR_OK;
+}
+
 extern "C" int vr_set_culling(vr_volume* v, int enable) {
     if (!v) return fail(NULL, VR_ERR_INVALID_ARG, "vr_set_culling: NULL handle");
     v->culling = enable != 0;
@@ -747,6 +780,11 @@ static int render_frame(vr_volume* v, const float* view, const float* proj, int 
         if (rc) return rc;
         mip_skipping = v->mip_skip_useful;
     }
+    const bool use_tex = v->sampler == VR_SAMPLER_TEXTURE && mode == VR_ALPHA && v->traversal == VR_SORT_LAST && v->counting != 2;
+    if (use_tex) { /* after an upload only */
+        rc = ensure_tex(v, st);
+        if (rc) return rc;
+    }
     if (timing) VR_CUDA(v, cudaEventRecord(ev[0], st));
     rc = run_setup(v, view, proj, width, height, mode, v->culling, st);
     if (rc) return rc;
@@ -768,6 +806,7 @@ static int render_frame(vr_volume* v, const float* view, const float* proj, int 
     p.vs_rw = v->d_vs;
     p.sub = v->d_sub;
     p.bitmap = NULL;
+    p.tex = use_tex ? vr_tex_table(v->tex) : NULL;
     p.cell_bits = skipping ? v->d_cell_bits : NULL;
     p.cell_mm = mip_skipping ? v->d_cell_mm : NULL;
     p.nc[0] = v->nc[0]; p.nc[1] = v->nc[1]; p.nc[2] = v->nc[2];

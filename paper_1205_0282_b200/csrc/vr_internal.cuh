@@ -143,6 +143,7 @@ struct VrRaycastParams {
     const int* item_prefix;
     VrViewState* vs_rw; /* work counter, sample counter */
     void* sub;          /* float4[] (ALPHA) or float[] (MIP) */
+    const cudaTextureObject_t* tex; /* texture arm (vr_texture.cu): one texture object per slot, or NULL = hand-rolled sampling */
     unsigned* bitmap;   /* counting variant only: one bit per brick-store cell, or NULL */
     const unsigned* cell_bits; /* R19: one bit per 8x8x8 macro-cell, 1 = transparent under the LUT; NULL = no skipping */
     const float2* cell_mm; /* R19, MIP: (min, max) per macro-cell (a cell whose max cannot raise the ray's maximum is skipped); NULL = off */
@@ -181,6 +182,12 @@ __host__ __device__ __forceinline__ unsigned vr_cell_offset(const VrGrid& g, int
 cudaError_t vr_launch_setup(const VrGrid& grid, const VrMatrices& mats, int W, int H, int mode,
                             long long sub_capacity_px, void* sub_base, VrViewState* vs, VrBrickView* bv, int* order,
                             int* item_prefix, VrCompLayer* layers, const float2* range, const VrLut& lut, cudaStream_t st);
+/* texture arm of the brick store (vr_texture.cu): one 3-D CUDA array + texture object per slot */
+struct VrTexStore;
+cudaError_t vr_tex_create(const VrGrid& grid, VrTexStore** out);
+void vr_tex_destroy(VrTexStore* t);
+const cudaTextureObject_t* vr_tex_table(const VrTexStore* t);
+cudaError_t vr_launch_tex_fill(const VrGrid& grid, const float* bricks, const VrTexStore* t, cudaStream_t st);
 /* ray table of the frame whose set-up is in vs (row a4, the per-ray part) */
 cudaError_t vr_launch_rays(const VrGrid& grid, const VrViewState* vs, int W, int H, double step, double2* rays, cudaStream_t st);
 cudaError_t vr_launch_minmax(const VrGrid& grid, const float* bricks, int2* enc, float2* table, cudaStream_t st);

@@ -1,0 +1,137 @@
+/*
+ * vr_texture.cu -- the texture-object arm of the brick store.
+ *
+ * PAPER.md:150 (sec. 2.3.2): the sub-cube is kept in the GPU's texture memory so that the
+ * built-in tri-linear interpolation can be used; :69 names the same facility. north_star asks
+ * for the bricks "either as 3D CUDA arrays behind texture objects or as a tiled linear layout with
+ * hand-rolled vectorised trilinear interpolation, whichever ncu shows is faster": this is the
+ * first arm.
+ *
+ * One 3-D CUDA array per brick of the handle, extent = the brick's ghost-padded extent, float32
+ * texels, behind a texture object with linear filtering, clamp addressing and unnormalised
+ * coordinates: texel i is centred at i + 1/2 and the hardware interpolates between the two nearest
+ * centres - R3's convention exactly, with the padded cell index as the texel index. The arrays
+ * are a second copy of the brick store, filled from it on the device through surface objects
+ * (vr_tex_fill_kernel) after an upload; the hand-rolled path keeps the float32 store, which
+ * VR_MIP always uses (the hardware filter's 8 fractional weight bits cannot meet MIP's 1e-5) and to
+ * which a VR_ALPHA sample falls back when the filter returns NaN (blanked voxels, R14).
+ */
+#include <string.h>
+
+#include <new>
+
+#include "vr_view.cuh"
+
+struct VrTexStore {
+    int n;                      /* bricks of the handle (slots) */
+    cudaArray_t* arr;
+    cudaTextureObject_t* tex;
+    cudaSurfaceObject_t* surf;
+    cudaTextureObject_t* d_tex; /* device copies of the two tables */
+    cudaSurfaceObject_t* d_surf;
+    int3* d_ext;                /* padded extent of every slot */
+};
+
+void vr_tex_destroy(VrTexStore* t) {
+    if (!t) return;
+    for (int s = 0; s < t->n; ++s) {
+        if (t->tex && t->tex[s]) cudaDestroyTextureObject(t->tex[s]);
+        if (t->surf && t->surf[s]) cudaDestroySurfaceObject(t->surf[s]);
+        if (t->arr && t->arr[s]) cudaFreeArray(t->arr[s]);
+    }
+    cudaFree(t->d_tex);
+    cudaFree(t->d_surf);
+    cudaFree(t->d_ext);
+    delete[] t->arr;
+    delete[] t->tex;
+    delete[] t->surf;
+    delete t;
+    cudaGetLastError();
+}
+
+/* brick held in slot s of the handle's store (the inverse of vr_slot_index) */
+static int brick_of_slot(const VrGrid& g, int s) {
+    const int w = g.pb1[0] - g.pb0[0], h = g.pb1[1] - g.pb0[1];
+    const int bx = g.pb0[0] + s % w, by = g.pb0[1] + (s / w) % h, bz = g.pb0[2] + s / (w * h);
+    return (bz * g.g[1] + by) * g.g[0] + bx;
+}
+
+cudaError_t vr_tex_create(const VrGrid& g, VrTexStore** out) {
+    *out = NULL;
+    VrTexStore* t = new (std::nothrow) VrTexStore();
+    if (!t) return cudaErrorMemoryAllocation;
+    memset(t, 0, sizeof(*t));
+    t->n = g.nown;
+    t->arr = new (std::nothrow) cudaArray_t[g.nown]();
+    t->tex = new (std::nothrow) cudaTextureObject_t[g.nown]();
+    t->surf = new (std::nothrow) cudaSurfaceObject_t[g.nown]();
+    int3* ext = new (std::nothrow) int3[g.nown];
+    cudaError_t e = (t->arr && t->tex && t->surf && ext) ? cudaSuccess : cudaErrorMemoryAllocation;
+    const cudaChannelFormatDesc fmt = cudaCreateChannelDesc<float>();
+    for (int s = 0; s < g.nown && e == cudaSuccess; ++s) {
+        int bc[3], lo[3], hi[3];
+        vr_brick_coords(g, brick_of_slot(g, s), bc);
+        vr_brick_core(g, bc, lo, hi);
+        ext[s] = make_int3(hi[0] - lo[0] + 2 * g.ghost, hi[1] - lo[1] + 2 * g.ghost, hi[2] - lo[2] + 2 * g.ghost);
+        e = cudaMalloc3DArray(&t->arr[s], &fmt, make_cudaExtent((size_t)ext[s].x, (size_t)ext[s].y, (size_t)ext[s].z),
+                              cudaArraySurfaceLoadStore);
+        if (e != cudaSuccess) break;
+        cudaResourceDesc res;
+        memset(&res, 0, sizeof(res));
+        res.resType = cudaResourceTypeArray;
+        res.res.array.array = t->arr[s];
+        cudaTextureDesc td;
+        memset(&td, 0, sizeof(td));
+        td.addressMode[0] = td.addressMode[1] = td.addressMode[2] = cudaAddressModeClamp;
+        td.filterMode = cudaFilterModeLinear;
+        td.readMode = cudaReadModeElementType;
+        td.normalizedCoords = 0;
+        e = cudaCreateTextureObject(&t->tex[s], &res, &td, NULL);
+        if (e == cudaSuccess) e = cudaCreateSurfaceObject(&t->surf[s], &res);
+    }
+    if (e == cudaSuccess) e = cudaMalloc(&t->d_tex, sizeof(cudaTextureObject_t) * g.nown);
+    if (e == cudaSuccess) e = cudaMalloc(&t->d_surf, sizeof(cudaSurfaceObject_t) * g.nown);
+    if (e == cudaSuccess) e = cudaMalloc(&t->d_ext, sizeof(int3) * g.nown);
+    if (e == cudaSuccess) e = cudaMemcpy(t->d_tex, t->tex, sizeof(cudaTextureObject_t) * g.nown, cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemcpy(t->d_surf, t->surf, sizeof(cudaSurfaceObject_t) * g.nown, cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemcpy(t->d_ext, ext, sizeof(int3) * g.nown, cudaMemcpyHostToDevice);
+    delete[] ext;
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        vr_tex_destroy(t);
+        return e;
+    }
+    *out = t;
+    return cudaSuccess;
+}
+
+const cudaTextureObject_t* vr_tex_table(const VrTexStore* t) { return t ? t->d_tex : NULL; }
+
+/* Padded cell (i, j, k) of slot s -> texel (i, j, k) of the slot's array. A CTA takes the 4 x 2 rows
+ * (j, k) of one row of micro-tiles, one row per warp, lanes along x, so the eight warps together consume
+ * whole 128-byte lines of the store (L1 serves a line's other rows to the neighbouring warps); the surface
+ * write is coalesced. Once per upload. */
+__global__ void __launch_bounds__(256)
+vr_tex_fill_kernel(VrGrid g, const float* __restrict__ bricks, const cudaSurfaceObject_t* __restrict__ surf,
+                   const int3* __restrict__ ext) {
+    const int s = blockIdx.y;
+    const int3 e = ext[s];
+    const cudaSurfaceObject_t su = surf[s];
+    const float* __restrict__ src = bricks + (long long)s * g.slot;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int nj = (e.y + 3) >> 2, nk = (e.z + 1) >> 1;
+    for (int blk = blockIdx.x; blk < nj * nk; blk += gridDim.x) {
+        const int j = ((blk % nj) << 2) + (warp & 3), k = ((blk / nj) << 1) + (warp >> 2);
+        if (j >= e.y || k >= e.z) continue;
+        const unsigned row = vr_axis_offset(g.ax[1], j) + vr_axis_offset(g.ax[2], k);
+        for (int i = lane; i < e.x; i += 32) surf3Dwrite(__ldcs(src + row + vr_axis_offset(g.ax[0], i)), su, i * 4, j, k);
+    }
+}
+
+cudaError_t vr_launch_tex_fill(const VrGrid& grid, const float* bricks, const VrTexStore* t, cudaStream_t st) {
+    const int nj = (grid.P + 3) >> 2, nk = (grid.P + 1) >> 1;
+    long long bx = (long long)nj * nk;
+    if (bx > 4096) bx = 4096;
+    vr_tex_fill_kernel<<<dim3((unsigned)bx, (unsigned)t->n), 256, 0, st>>>(grid, bricks, t->d_surf, t->d_ext);
+    return cudaGetLastError();
+}

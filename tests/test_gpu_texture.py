@@ -1,0 +1,135 @@
+"""GPU parity of the texture-object arm of rows a1 / a5 (vr_set_sampler(VR_SAMPLER_TEXTURE)
+"built-in tri-linear interpolation"): VR_ALPHA frames through hardware-filtered 3-D CUDA arrays against the same
+oracle at north_star's 2e-3. The sample SET is the hand-rolled path's (same FP64 set-up); the filter's 8-bit
+weights move a brick's accumulated opacity by up to ~1e-4, so a termination test within 2e-4 of tau may go either
+way: such pixels are flagged by the oracle (R12, margin widened to 2e-4) and must lie within 2e-3 of the interval
+between the oracle's frames for tau - 2e-4 and tau + 2e-4."""
+import numpy as np
+import pytest
+
+import oracle
+import synth
+from helpers import check_alpha, check_mip, gpu_frame, make_pair, seeded_pixels
+
+pytestmark = pytest.mark.gpu
+TEX_MARGIN = 2e-4
+
+
+@pytest.fixture(scope="module")
+def vr(cuda_device):
+    from paper_1205_0282_b200 import build
+    build.build()
+    import paper_1205_0282_b200 as vr
+    return vr
+
+
+def tex_pair(vr, cube, brick, ghost=1, tf=None, tau=0.99, data=None):
+    g, o = make_pair(cube, brick, ghost, tf=tf, tau=tau, data=data)
+    g.set_sampler(vr.SAMPLER_TEXTURE)
+    o.set_ert_margin(TEX_MARGIN)
+    return g, o
+
+
+@pytest.mark.parametrize("tf_name", ["ramp", "translucent"])
+def test_config0_full_frames_texture(vr, tf_name):
+    c = synth.CONFIGS["c0"]
+    cube = synth.config_cube("c0")
+    tf = synth.tf_ramp() if tf_name == "ramp" else synth.tf_translucent()
+    g, o = tex_pair(vr, cube, c["brick"], c["ghost"], tf=tf)
+    W, H = c["width"], c["height"]
+    fr = synth.Framing(cube.nx, cube.ny, cube.nz, W, H)
+    worst = 0.0
+    for ortho in (False, True):
+        for k in range(3):
+            view, proj = fr.seeded(77, k), fr.proj(ortho)
+            ref = o.render(view, proj, W, H, c["step"], oracle.ALPHA)
+            img = gpu_frame(g, view, proj, W, H, c["step"], vr.ALPHA)
+            worst = max(worst, check_alpha(img, ref, 0.99, "c0 texture %s %d" % (tf_name, k), envelope=True, max_flagged=1.0))
+            # unflagged pixels alone: the plain 2e-3 bound, and the filter's weights do show (not the manual path)
+            un = (ref["flags"] & oracle.FLAG_ERT_MARGIN) == 0
+            assert np.abs(img - ref["image"]).max(axis=-1)[un].max() <= 2e-3
+    g.set_sampler(vr.SAMPLER_MANUAL)
+    man = gpu_frame(g, view, proj, W, H, c["step"], vr.ALPHA)
+    assert 1e-7 < np.abs(man - img).max() < 0.02  # two different samplers, the same picture
+
+
+@pytest.mark.parametrize("ghost,tau", [(1, 0.99), (1, 2.0), (2, 0.99), (0, 2.0)])
+def test_bricked_ragged_texture_frames_subimages_and_counts(vr, ghost, tau):
+    """Ragged multi-brick volume: frames, each brick's sub-image, and - with early termination off - exactly the
+    hand-rolled path's sample count; ghost = 0 relies on the arrays' clamp addressing (seams as the oracle's)."""
+    cube = synth.Cube(11, 100, 90, 70, 12)
+    tf = synth.tf_translucent() if tau > 1 else synth.tf_ramp()
+    g, o = tex_pair(vr, cube, 32, ghost, tf=tf, tau=tau)
+    W, H = 203, 117
+    fr = synth.Framing(cube.nx, cube.ny, cube.nz, W, H)
+    pix = seeded_pixels(4, W, H, 300)
+    g.set_counting(1)
+    for k, ortho in ((0, False), (1, True)):
+        view, proj = fr.seeded(77, k), fr.proj(ortho)
+        ref = o.render(view, proj, W, H, 0.5, oracle.ALPHA)
+        img = gpu_frame(g, view, proj, W, H, 0.5, vr.ALPHA)
+        n_tex = g.debug_stats()["samples"]
+        check_alpha(img, ref, tau, "texture ghost %d view %d" % (ghost, k), envelope=True, max_flagged=1.0)
+        sub_ref = o.render(view, proj, W, H, 0.5, oracle.ALPHA, pixels=pix, want_sub=True)
+        check_alpha(g.debug_subimages(pix).astype(np.float64), sub_ref, tau, "texture sub-images", key="sub", envelope=True,
+                    max_flagged=1.0)
+        if tau > 1:
+            assert n_tex == int(ref["counts"][..., 0].sum())
+        # MIP frames keep the hand-rolled sampler (1e-5): bit-identical with the sampler switched back
+        m_tex = gpu_frame(g, view, proj, W, H, 0.5, vr.MIP)
+        g.set_sampler(vr.SAMPLER_MANUAL)
+        assert np.array_equal(gpu_frame(g, view, proj, W, H, 0.5, vr.MIP), m_tex)
+        g.set_sampler(vr.SAMPLER_TEXTURE)
+        check_mip(m_tex, o.render(view, proj, W, H, 0.5, oracle.MIP), "MIP beside the texture arm")
+
+
+def test_texture_arm_follows_uploads_and_blanked_voxels(vr):
+    """The arrays are refilled after an upload; NaN voxels (R14) go through the exact rule of the float32 store."""
+    import torch
+    cube = synth.Cube(31, 72, 40, 56, 6)
+    data = cube.fill_host()
+    g, o = tex_pair(vr, cube, 32, 1, tf=synth.tf_translucent(), tau=2.0, data=data)
+    W, H = 144, 100
+    fr = synth.Framing(cube.nx, cube.ny, cube.nz, W, H)
+    view, proj = fr.turntable(5), fr.proj(False)
+    check_alpha(gpu_frame(g, view, proj, W, H, 0.5, vr.ALPHA), o.render(view, proj, W, H, 0.5, oracle.ALPHA), 2.0, "first upload")
+    d2 = data.copy()
+    d2[10:30, 5:25, 20:50] = np.nan      # a blanked box across brick seams
+    d2[40:, :, :8] = np.nan              # a blanked edge
+    d2[3, 7, 60] = np.nan                # an isolated bad voxel
+    d2[31:34, 20:22, 30:33] += 4.0
+    g.upload(torch.from_numpy(d2).cuda())
+    o2 = oracle.Volume(cube.nx, cube.ny, cube.nz, 32, 1, data=d2)
+    o2.set_transfer_function(synth.tf_translucent(), synth.TF_VMIN, synth.TF_VMAX)
+    o2.set_early_termination(2.0)
+    g.set_counting(1)
+    ref = o2.render(view, proj, W, H, 0.5, oracle.ALPHA)
+    img = gpu_frame(g, view, proj, W, H, 0.5, vr.ALPHA)
+    assert np.isfinite(img).all()
+    check_alpha(img, ref, 2.0, "second upload, blanked voxels")
+    slack = 4 * int(((ref["flags"] & oracle.FLAG_NAN_MARGIN) != 0).sum())
+    assert abs(g.debug_stats()["samples"] - int(ref["counts"][..., 0].sum())) <= slack
+    assert np.abs(img - o.render(view, proj, W, H, 0.5, oracle.ALPHA)["image"]).max() > 1e-2  # not the first cube's frame
+
+
+def test_texture_arm_with_macro_cell_skipping_and_errors(vr):
+    """R19 beside the texture arm: frames bit-identical with skipping on / off; state errors."""
+    cube = synth.Cube(33, 96, 80, 64, 10)
+    g, o = tex_pair(vr, cube, 32, 1, tf=synth.tf_threshold())
+    W, H = 160, 120
+    fr = synth.Framing(cube.nx, cube.ny, cube.nz, W, H)
+    view, proj = fr.seeded(9, 0), fr.proj(False)
+    g.set_counting(1)
+    on = gpu_frame(g, view, proj, W, H, 0.5, vr.ALPHA)
+    n_on = g.debug_stats()["samples"]
+    g.set_culling(False)
+    off = gpu_frame(g, view, proj, W, H, 0.5, vr.ALPHA)
+    n_off = g.debug_stats()["samples"]
+    assert np.array_equal(on, off) and n_on < n_off
+    check_alpha(on, o.render(view, proj, W, H, 0.5, oracle.ALPHA), 0.99, "texture + skipping", envelope=True, max_flagged=1.0)
+    lin = vr.Volume(32, 32, 32, 16, 1, layout=vr.LAYOUT_LINEAR)
+    with pytest.raises(vr.VrError) as e:
+        lin.set_sampler(vr.SAMPLER_TEXTURE)
+    assert e.value.status == 4
+    with pytest.raises(vr.VrError):
+        g.set_sampler(7)
