@@ -246,8 +246,11 @@ int vr_set_traversal(vr_volume* v, int traversal);
  * SET is unchanged (same FP64 set-up); the hardware's 8-bit interpolation weights perturb sample values by up
  * to 2^-9 of the local voxel differences, which keeps VR_ALPHA inside its 2e-3 tolerance but moves early-
  * termination decisions of rays whose opacity passes tau within ~1e-4 of it. VR_MIP frames (1e-5), fused
- * frames and counting mode 2 always use the hand-rolled path; a sample whose filtered value is NaN (blanked
- * voxels, R14) is re-evaluated from the float32 store by the exact rule. Needs the default (tiled) layout. */
+ * frames and counting mode 2 always use the hand-rolled path, and so do (i) bricks that hold blanked (NaN) voxels -
+ * the filter cannot apply R14's rule - and (ii) frames whose transfer function has a step: two neighbouring entries
+ * further apart than 2.56/n in a channel (a threshold, a toe). The filter's value error is about one table entry on
+ * unit-sigma noise; across a step that is a wrong opacity, not 2e-3 (measured: 8e-2 on a threshold table).
+ * Needs the default (tiled) layout. */
 #define VR_SAMPLER_MANUAL 0
 #define VR_SAMPLER_TEXTURE 1
 int vr_set_sampler(vr_volume* v, int sampler);

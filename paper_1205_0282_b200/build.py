@@ -22,6 +22,10 @@ NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a",
               "-Xcompiler", "-fPIC,-ffp-contract=off", "-Xptxas", "-v"]
 
 
+# build-time experiments only (e.g. VR_NVCC_EXTRA="-DVR_TEX_CTAS=5"): never read at run time
+NVCC_FLAGS += os.environ.get("VR_NVCC_EXTRA", "").split()
+
+
 def _run(cmd, verbose):
     r = subprocess.run(cmd, capture_output=True, text=True)
     if r.returncode != 0:

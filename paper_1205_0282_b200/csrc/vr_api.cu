@@ -30,7 +30,7 @@ struct vr_volume {
     VrCompLayer* d_layers;
     void* d_sub;             /* sub-image scratch, sub_capacity_px * 16 bytes */
     long long sub_capacity_px;
-    double2* d_rays;         /* the frame's ray table: VR_RAY_WORDS planes of ray_capacity_px entries */
+    double2* d_rays;         /* the frame's ray table: VR_RAY_BYTES per pixel, ray_capacity_px pixels */
     long long ray_capacity_px;
     float* d_frame;          /* vr_render_host's device frame */
     long long frame_capacity_px;
@@ -50,6 +50,7 @@ struct vr_volume {
     bool cell_mm_valid, cell_bits_valid;
     bool mip_skip_known, mip_skip_useful; /* decided once per upload: does the cube have empty space (R19, MIP) */
     unsigned long long* d_cell_count;
+    bool tf_smooth;          /* no neighbouring LUT entries further apart than 2.56/n per channel (texture arm) */
     bool tf_has_zero;        /* the LUT has a run of >= 3 zero-alpha entries: skipping can do something */
     bool culling;
     int sampler;             /* VR_SAMPLER_MANUAL or VR_SAMPLER_TEXTURE */
@@ -460,6 +461,13 @@ extern "C" int vr_set_transfer_function(vr_volume* v, const float* rgba, int n, 
         run = rgba[4 * i + 3] == 0.0f ? run + 1 : 0;
         if (run >= 3) v->tf_has_zero = true;
     }
+    /* texture arm: the filter's 8-bit weights put a value error of up to ~3 * 2^-9 of the local voxel differences on a
+     * sample (about one table entry on noise of unit sigma over a 13-sigma, 256-entry table); 2e-3 per channel survives that
+     * only if neighbouring entries are close. Tables with steps (thresholds, toes) keep the hand-rolled sampler. */
+    v->tf_smooth = true;
+    for (int i = 0; i + 1 < n; ++i)
+        for (int c = 0; c < 4; ++c)
+            if (fabsf(rgba[4 * i + 4 + c] - rgba[4 * i + c]) > 2.56f / (float)n) v->tf_smooth = false;
     v->cell_bits_valid = false;
     v->has_tf = true;
     return VR_OK;
@@ -529,7 +537,7 @@ static int ensure_rays(vr_volume* v, long long px) {
         v->d_rays = NULL;
         v->ray_capacity_px = 0;
     }
-    VR_CUDA(v, cudaMalloc(&v->d_rays, (size_t)px * VR_RAY_WORDS * sizeof(double2)));
+    VR_CUDA(v, cudaMalloc(&v->d_rays, (size_t)px * VR_RAY_BYTES + 16));
     v->ray_capacity_px = px;
     return VR_OK;
 }
@@ -780,7 +788,8 @@ static int render_frame(vr_volume* v, const float* view, const float* proj, int 
         if (rc) return rc;
         mip_skipping = v->mip_skip_useful;
     }
-    const bool use_tex = v->sampler == VR_SAMPLER_TEXTURE && mode == VR_ALPHA && v->traversal == VR_SORT_LAST && v->counting != 2;
+    const bool use_tex = v->sampler == VR_SAMPLER_TEXTURE && mode == VR_ALPHA && v->traversal == VR_SORT_LAST && v->counting != 2 &&
+                         v->tf_smooth;
     if (use_tex) { /* after an upload only */
         rc = ensure_tex(v, st);
         if (rc) return rc;
@@ -807,6 +816,7 @@ static int render_frame(vr_volume* v, const float* view, const float* proj, int 
     p.sub = v->d_sub;
     p.bitmap = NULL;
     p.tex = use_tex ? vr_tex_table(v->tex) : NULL;
+    p.tex_nan = use_tex ? vr_tex_nan_table(v->tex) : NULL;
     p.cell_bits = skipping ? v->d_cell_bits : NULL;
     p.cell_mm = mip_skipping ? v->d_cell_mm : NULL;
     p.nc[0] = v->nc[0]; p.nc[1] = v->nc[1]; p.nc[2] = v->nc[2];

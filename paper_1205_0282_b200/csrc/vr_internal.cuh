@@ -125,12 +125,13 @@ struct VrLut {
 };
 
 /* Per-frame ray table ("each GPU kernel then starts by calculating its ray's start location,
- * orientation" - once per RAY, not once per (ray, brick)): VR_RAY_WORDS double2 planes of W*H entries each,
- * plane a at rays + a * (W*H), entry of pixel (i, j) at j*W + i:
- *   0 (o0, o1)  1 (o2, d0)  2 (d1, d2)  3 (t0, t1)  4 (step, K as a double; 0 = the ray misses the volume)
- *   5 (1/d0, 1/d1)  6 (1/d2, 1/step)      -- used for estimates only (brick_range)
- * Written by vr_rays_kernel for the pixels inside VrViewState::bound, read by the ray-cast kernel. */
-#define VR_RAY_WORDS 7
+ * orientation" - once per RAY, not once per (ray, brick)). Planes of W*H entries, entry of pixel (i, j) at j*W + i:
+ *   four double2 planes  (o0, o1) (o2, d0) (d1, d2) (t0, t1)                                 64 bytes per pixel
+ *   one int plane        K, the number of scheduled samples (0 = the ray misses the volume)    4
+ *   one double plane     the ray's step, written only for VR_STEP_AUTO (R18)                   8
+ * = VR_RAY_BYTES per pixel of scratch. Written by vr_rays_kernel for the pixels inside VrViewState::bound,
+ * read by the ray-cast kernel (64 to 76 bytes per (ray, brick) segment). */
+#define VR_RAY_BYTES 80 /* 76 rounded up: the planes stay 16-byte aligned for any W*H */
 
 struct VrRaycastParams {
     VrGrid grid;
@@ -144,12 +145,14 @@ struct VrRaycastParams {
     VrViewState* vs_rw; /* work counter, sample counter */
     void* sub;          /* float4[] (ALPHA) or float[] (MIP) */
     const cudaTextureObject_t* tex; /* texture arm (vr_texture.cu): one texture object per slot, or NULL = hand-rolled sampling */
+    const int* tex_nan;             /* 1 per slot that holds blanked voxels: sampled by hand also in the texture arm (R14) */
     unsigned* bitmap;   /* counting variant only: one bit per brick-store cell, or NULL */
     const unsigned* cell_bits; /* R19: one bit per 8x8x8 macro-cell, 1 = transparent under the LUT; NULL = no skipping */
     const float2* cell_mm; /* R19, MIP: (min, max) per macro-cell (a cell whose max cannot raise the ray's maximum is skipped); NULL = off */
     int nc[3];          /* macro-cells per axis of a brick slot */
     int cell_words;     /* 32-bit words of cell_bits per brick */
     VrLut lut;
+    int lut_copies; /* copies of the table in the ray-cast kernel's shared memory (vr_lut_copies) */
     double step; /* > 0: sample spacing in voxels; 0: per ray, 1 / max|d_a| (R18) */
     float tau;
     int mode;
@@ -187,6 +190,7 @@ struct VrTexStore;
 cudaError_t vr_tex_create(const VrGrid& grid, VrTexStore** out);
 void vr_tex_destroy(VrTexStore* t);
 const cudaTextureObject_t* vr_tex_table(const VrTexStore* t);
+const int* vr_tex_nan_table(const VrTexStore* t);
 cudaError_t vr_launch_tex_fill(const VrGrid& grid, const float* bricks, const VrTexStore* t, cudaStream_t st);
 /* ray table of the frame whose set-up is in vs (row a4, the per-ray part) */
 cudaError_t vr_launch_rays(const VrGrid& grid, const VrViewState* vs, int W, int H, double step, double2* rays, cudaStream_t st);

@@ -105,32 +105,38 @@ __device__ __forceinline__ void ray_setup(const double* __restrict__ Minv, int W
     }
 }
 
-/* The ray of pixel p = j*W + i from the frame's ray table (VrRaycastParams::rays): the values ray_setup computed,
- * bit for bit. FULL = false loads only what the exit samples need (o, d, t0, t1, step). */
+/* The ray of pixel p = j*W + i from the frame's ray table (VrRaycastParams::rays, layout in vr_internal.cuh): the values
+ * ray_setup computed, bit for bit. FULL also fills the reciprocals brick_range's ESTIMATES use, from float32
+ * reciprocals (relative error 1e-7: < 1e-3 voxel on the longest ray, a tenth of the margin of brick_range's early
+ * out; a wrong guess only costs a bisection). step_fixed > 0: the caller's spacing (not stored); 0: per ray (R18). */
+/* the int plane (K) and, 16-byte aligned behind it, the double plane (per-ray step) */
+__device__ __forceinline__ const int* ray_k_plane(const double2* rays, long long plane) { return reinterpret_cast<const int*>(rays + 4 * plane); }
+__device__ __forceinline__ const double* ray_step_plane(const double2* rays, long long plane) {
+    return reinterpret_cast<const double*>(reinterpret_cast<const char*>(rays + 4 * plane) + ((plane * 4 + 15) & ~15ll));
+}
+
 template <bool FULL>
-__device__ __forceinline__ void ray_load(const double2* __restrict__ rays, long long plane, long long p, RaySetup& r) {
-    const double2 a0 = __ldg(rays + p), a1 = __ldg(rays + plane + p), a2 = __ldg(rays + 2 * plane + p),
-                  a3 = __ldg(rays + 3 * plane + p), a4 = __ldg(rays + 4 * plane + p);
+__device__ __forceinline__ void ray_load(const double2* __restrict__ rays, long long plane, long long p, double step_fixed, RaySetup& r) {
+    const double2 a0 = __ldg(rays + p), a1 = __ldg(rays + plane + p), a2 = __ldg(rays + 2 * plane + p), a3 = __ldg(rays + 3 * plane + p);
+    r.K = __ldg(ray_k_plane(rays, plane) + p);
     r.o[0] = a0.x, r.o[1] = a0.y, r.o[2] = a1.x;
     r.d[0] = a1.y, r.d[1] = a2.x, r.d[2] = a2.y;
     r.t0 = a3.x, r.t1 = a3.y;
-    r.step = a4.x;
-    r.K = (int)a4.y;
+    r.step = step_fixed > 0.0 ? step_fixed : __ldg(ray_step_plane(rays, plane) + p);
     if (FULL) {
-        const double2 a5 = __ldg(rays + 5 * plane + p), a6 = __ldg(rays + 6 * plane + p);
-        r.inv_d[0] = a5.x, r.inv_d[1] = a5.y, r.inv_d[2] = a6.x;
-        r.inv_step = a6.y;
+#pragma unroll
+        for (int a = 0; a < 3; ++a) r.inv_d[a] = r.d[a] == 0.0 ? 0.0 : (double)__frcp_rn((float)r.d[a]);
+        r.inv_step = (double)__frcp_rn((float)r.step);
     }
 }
 
-__device__ __forceinline__ void ray_store(double2* __restrict__ rays, long long plane, long long p, const RaySetup& r) {
+__device__ __forceinline__ void ray_store(double2* __restrict__ rays, long long plane, long long p, bool step_fixed, const RaySetup& r) {
     rays[p] = make_double2(r.o[0], r.o[1]);
     rays[plane + p] = make_double2(r.o[2], r.d[0]);
     rays[2 * plane + p] = make_double2(r.d[1], r.d[2]);
     rays[3 * plane + p] = make_double2(r.t0, r.t1);
-    rays[4 * plane + p] = make_double2(r.step, (double)r.K);
-    rays[5 * plane + p] = make_double2(r.inv_d[0], r.inv_d[1]);
-    rays[6 * plane + p] = make_double2(r.inv_d[2], r.inv_step);
+    const_cast<int*>(ray_k_plane(rays, plane))[p] = r.K;
+    if (!step_fixed) const_cast<double*>(ray_step_plane(rays, plane))[p] = r.step;
 }
 
 /* R5: sample k stands for the interval [t0 + k step, min(t0 + (k+1) step, t1)]: s = its
@@ -480,8 +486,19 @@ struct Accum {
 /* The LUT as the kernel sees it: (entry, delta) pairs interleaved in shared memory, addressed
  * through one 32-bit shared-window address kept in a register. */
 struct LutView {
-    unsigned base; /* shared-memory byte address of pair 0 */
+    unsigned base;   /* shared-memory byte address of pair 0 (replicated layout: of this lane's copy of entry 0) */
+    unsigned stride; /* replicated layout: bytes from entry i to entry i + 1 of the same copy */
 };
+
+/* Replicated layout (the ray-cast kernel): a 128-bit shared load is served a quarter-warp (8 lanes x 16 bytes = all 32
+ * banks) at a time, and the lanes of a quarter read unrelated entries on noisy data: with one table, 8 lanes on 4 (pairs
+ * at 32-byte stride) bank groups cost 13.7 wavefronts per load instead of 4 (ncu, c1: 71 % of all shared wavefronts were
+ * conflicts). So the table is stored `copies` times, entry i of copy c at (i * copies + c) * 16 bytes, and lane l reads copy
+ * l mod copies - its own bank group: no conflicts at copies = 8. Only the entries are stored; the difference to the next
+ * entry is the same float32 subtraction the host made for the paired layout. copies = 8 for n <= 256 (32 KB), 4 / 2 above.
+ * Sparsely sampled views (the 103 GB cube: every sample misses L2, L1 capacity decides how often a ray finds its previous
+ * sample's lines again) keep ONE copy (4 KB): with 32 KB of table per CTA c3 lost 7 % (ramp) to 16 % (translucent). */
+__host__ __device__ __forceinline__ int vr_lut_copies(int n, bool sparse) { return sparse ? 1 : (n <= 256 ? 8 : (n <= 512 ? 4 : 2)); }
 
 template <int OFF>
 __device__ __forceinline__ float4 lds128(unsigned addr) {
@@ -505,13 +522,22 @@ __device__ __forceinline__ float ex2_approx(float x) {
 /* R7: classification and opacity of a sample standing for a path of length w; R8 blending.
  * alpha = 1 - (1-a)^w = 1 - 2^(w log2(1-a)) on the two MUFU approximations (2^-22 relative,
  * DESIGN.md "Tolerances"); a = 1 gives log2(0) = -inf and alpha = 1, a = 0 gives alpha = 0. */
+template <bool REP = false>
 __device__ __forceinline__ void shade_alpha(Accum& acc, float v, float w, const LutView& lut, const VrLut& P) {
     const float u = __saturatef((v - P.vmin) * P.inv_range);
     const float x = u * P.scale;
     const int i = min((int)x, P.nm2);
     const float f = x - (float)i;
-    const unsigned a = lut.base + 32u * (unsigned)i;
-    const float4 e = lds128<0>(a), dl = lds128<16>(a);
+    float4 e, dl;
+    if (REP) {
+        const unsigned a = lut.base + lut.stride * (unsigned)i;
+        e = lds128<0>(a);
+        const float4 e1 = lds128<0>(a + lut.stride);
+        dl = make_float4(e1.x - e.x, e1.y - e.y, e1.z - e.z, e1.w - e.w);
+    } else {
+        const unsigned a = lut.base + 32u * (unsigned)i;
+        e = lds128<0>(a), dl = lds128<16>(a);
+    }
     const float cr = fmaf(f, dl.x, e.x), cg = fmaf(f, dl.y, e.y), cb = fmaf(f, dl.z, e.z), ca = fmaf(f, dl.w, e.w);
     const float alpha = 1.0f - ex2_approx(w * lg2_approx(1.0f - ca));
     /* R14: a dropped sample arrives as NaN. It classifies harmlessly (the saturation maps it to entry 0);

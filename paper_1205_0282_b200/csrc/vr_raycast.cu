@@ -31,20 +31,27 @@
  */
 #include "vr_march.cuh"
 
+#ifndef VR_TEX_CTAS
+#define VR_TEX_CTAS 3 /* resident CTAs per SM the texture-arm instances are cut for */
+#endif
+#ifndef VR_TEX_DEPTH
+#define VR_TEX_DEPTH 4 /* texture fetches a lane keeps in flight */
+#endif
+#ifndef VR_TEX_COPIES
+#define VR_TEX_COPIES 8 /* copies of the table in the texture-arm instances (more CTAs per SM: less room for each) */
+#endif
+
 template <int MODE, int LAY, int PT, bool CLAMP, bool COUNT, bool SKIP, bool TEX>
-__global__ void __launch_bounds__(VR_RAYCAST_THREADS, VR_MIN_CTAS)
+__global__ void __launch_bounds__(VR_RAYCAST_THREADS, TEX ? VR_TEX_CTAS : VR_MIN_CTAS)
 vr_raycast_kernel(const VrRaycastParams prm) {
-    /* dynamic: 2 * lut.n float4 (ALPHA) - a 256-entry table takes 8 KB, not the 32 KB of the
-     * largest one, and what it does not take stays L1 cache */
+    /* dynamic (ALPHA): the table, `copies` times (vr_march.cuh): 32 KB at most; what it does not take stays L1 cache */
     extern __shared__ float4 s_lut[];
 
     const VrGrid& g = prm.grid;
     const int lane = threadIdx.x & 31;
+    const int copies = prm.lut_copies;
     if (MODE == VR_ALPHA) {
-        for (int i = threadIdx.x; i < prm.lut.n; i += blockDim.x) {
-            s_lut[2 * i] = prm.lut.base[i];
-            s_lut[2 * i + 1] = prm.lut.delta[i];
-        }
+        for (int i = threadIdx.x; i < prm.lut.n * copies; i += blockDim.x) s_lut[i] = prm.lut.base[i / copies];
     }
     __syncthreads();
     if (prm.vs->singular) return;
@@ -54,9 +61,10 @@ vr_raycast_kernel(const VrRaycastParams prm) {
     const float tau = prm.tau;
     LutView lut;
     lut.base = 0;
+    lut.stride = 16u * (unsigned)copies;
     if (MODE == VR_ALPHA) {
-        lut.base = (unsigned)__cvta_generic_to_shared(s_lut);
-        asm volatile("" : "+r"(lut.base)); /* one register, not rebuilt per sample */
+        lut.base = (unsigned)__cvta_generic_to_shared(s_lut) + 16u * (unsigned)(lane & (copies - 1));
+        asm volatile("" : "+r"(lut.base), "+r"(lut.stride)); /* two registers, not rebuilt per sample */
     }
     /* MIP may stop where the output saturates (vmax) or at the global maximum of the data when
      * it is known ("the maximum pixel value (defined by the global maximum of the data)") */
@@ -103,7 +111,7 @@ vr_raycast_kernel(const VrRaycastParams prm) {
         int k_lo = 0, k_hi = 0;
         const long long ray_p = (long long)pj * W + pi;
         if (in_rect) {
-            ray_load<true>(prm.rays, prm.ray_plane, ray_p, ray);
+            ray_load<true>(prm.rays, prm.ray_plane, ray_p, prm.step, ray);
             brick_range(ray, g, bc, blo, bhi, k_lo, k_hi);
         }
         /* lattice samples: k in [k_lo, k_lat); samples k >= K-2 (whose interval may be clipped
@@ -135,9 +143,9 @@ vr_raycast_kernel(const VrRaycastParams prm) {
          * step j = P0 + j * Df (one FFMA per axis; error < 1e-4 voxel, far below the filter's 2^-9 weight quantum) */
         cudaTextureObject_t tex = 0;
         float P0x = 0.0f, P0y = 0.0f, P0z = 0.0f, Dfx = 0.0f, Dfy = 0.0f, Dfz = 0.0f;
-        const Lattice L0 = L;
         const int n0 = n;
-        if (TEX) {
+        const bool use_tex = TEX && __ldg(prm.tex_nan + slot_b) == 0; /* warp-uniform: one brick per item */
+        if (use_tex) {
             tex = __ldg(prm.tex + slot_b);
             const double h = 1.0 / 4294967296.0;
             P0x = (float)((double)L.q[0] * h + 0.5), P0y = (float)((double)L.q[1] * h + 0.5), P0z = (float)((double)L.q[2] * h + 0.5);
@@ -159,7 +167,33 @@ vr_raycast_kernel(const VrRaycastParams prm) {
         float pbound = INFINITY;
         int pm = -1;
         bool ptransp = false;
-        while (TEX && __any_sync(FULL_MASK, active)) {
+        /* Without macro-cell look-ups a lane's next positions do not depend on anything it loads: VR_TEX_DEPTH samples are
+         * fetched back to back and then shaded in order, early termination tested between them as always (the values
+         * fetched beyond a termination are dropped: at most VR_TEX_DEPTH - 1 per ray segment). The texture arm is bound by
+         * the latency of its one fetch per sample at the 32 warps per SM its cache footprint allows (ncu: nothing above 40 %,
+         * 12.8 warps per issue waiting on the scoreboard); this keeps VR_TEX_DEPTH fetches per warp in flight instead of one. */
+        while (TEX && !SKIP && use_tex && __any_sync(FULL_MASK, active)) {
+            if (active) {
+                const float kf = (float)(n0 - n);
+                float vq[VR_TEX_DEPTH];
+#pragma unroll
+                for (int u = 0; u < VR_TEX_DEPTH; ++u) {
+                    const float ku = kf + (float)u;
+                    vq[u] = tex3D<float>(tex, fmaf(ku, Dfx, P0x), fmaf(ku, Dfy, P0y), fmaf(ku, Dfz, P0z));
+                }
+#pragma unroll
+                for (int u = 0; u < VR_TEX_DEPTH; ++u) {
+                    if (active) {
+                        if (COUNT) nsamples += (vq[u] == vq[u]) ? 1 : 0;
+                        shade_alpha<true>(acc, vq[u], stepf, lut, prm.lut);
+                        stopped = !(acc.a < tau);
+                        --n;
+                        active = n > 0 && !stopped;
+                    }
+                }
+            }
+        }
+        while (TEX && SKIP && use_tex && __any_sync(FULL_MASK, active)) {
             /* texture arm (built-in tri-linear interpolation): one TEX instead of 8 loads, the index
              * arithmetic and 7 FMA; the lattice is kept only where macro-cells are looked up (SKIP) */
             if (active) {
@@ -175,15 +209,9 @@ vr_raycast_kernel(const VrRaycastParams prm) {
                 }
                 if (adv > 0) {
                     const float kf = (float)(n0 - n);
-                    float v = tex3D<float>(tex, fmaf(kf, Dfx, P0x), fmaf(kf, Dfy, P0y), fmaf(kf, Dfz, P0z));
-                    if (v != v) { /* R14: blanked voxels among the 8 - the exact rule needs the float32 voxels (rare path) */
-                        Lattice Ls;
-                        const long long j = (long long)(n0 - n);
-                        Ls.q[0] = L0.q[0] + D[0] * j, Ls.q[1] = L0.q[1] + D[1] * j, Ls.q[2] = L0.q[2] + D[2] * j;
-                        v = trilinear<LAY, PT, CLAMP, false>(brick, g, ext, Ls, NULL, 0);
-                    }
+                    const float v = tex3D<float>(tex, fmaf(kf, Dfx, P0x), fmaf(kf, Dfy, P0y), fmaf(kf, Dfz, P0z));
                     if (COUNT) nsamples += (v == v) ? 1 : 0;
-                    shade_alpha(acc, v, stepf, lut, prm.lut);
+                    shade_alpha<true>(acc, v, stepf, lut, prm.lut);
                     stopped = !(acc.a < tau);
                     if (SKIP) L.q[0] += D[0], L.q[1] += D[1], L.q[2] += D[2];
                 } else {
@@ -194,7 +222,7 @@ vr_raycast_kernel(const VrRaycastParams prm) {
                 active = n > 0 && !stopped;
             }
         }
-        while (!TEX && __any_sync(FULL_MASK, active)) {
+        while (!(TEX && use_tex) && __any_sync(FULL_MASK, active)) {
             if (active) {
                 const int cx = (int)(L.q[0] >> 32), cy = (int)(L.q[1] >> 32), cz = (int)(L.q[2] >> 32);
                 int adv = 1; /* lattice steps this trip takes */
@@ -231,7 +259,7 @@ vr_raycast_kernel(const VrRaycastParams prm) {
                         acc.r = fmaxf(acc.r, v);
                         stopped = acc.r >= mip_stop;
                     } else {
-                        shade_alpha(acc, v, stepf, lut, prm.lut);
+                        shade_alpha<true>(acc, v, stepf, lut, prm.lut);
                         stopped = !(acc.a < tau);
                     }
                     L.q[0] += D[0], L.q[1] += D[1], L.q[2] += D[2];
@@ -250,7 +278,7 @@ vr_raycast_kernel(const VrRaycastParams prm) {
             if (k_tail < k_hi && !stopped) {
                 long long q = ray_p; /* an opaque copy: the ray is read again, not kept in registers through the loop */
                 asm volatile("" : "+l"(q));
-                ray_load<false>(prm.rays, prm.ray_plane, q, ray);
+                ray_load<false>(prm.rays, prm.ray_plane, q, prm.step, ray);
             }
 #endif
             for (int k = k_tail; k < k_hi && !stopped; ++k) {
@@ -267,7 +295,7 @@ vr_raycast_kernel(const VrRaycastParams prm) {
                     acc.r = fmaxf(acc.r, v);
                     stopped = acc.r >= mip_stop;
                 } else {
-                    shade_alpha(acc, v, (float)w, lut, prm.lut);
+                    shade_alpha<true>(acc, v, (float)w, lut, prm.lut);
                     stopped = !(acc.a < tau);
                 }
             }
@@ -291,21 +319,21 @@ vr_raycast_kernel(const VrRaycastParams prm) {
 /* Persistent grid: resident CTAs per SM (for this instance and its shared memory) x SMs,
  * but no more CTAs than there are groups of 8 work items. */
 template <int MODE, int LAY, int PT, bool CLAMP, bool COUNT, bool SKIP = false, bool TEX = false>
-static cudaError_t launch_variant(const VrRaycastParams& p, long long items, bool sparse, cudaStream_t st) {
-    static int sms = 0, cached_per_sm = 0;
-    static size_t cached_smem = (size_t)-1;
-    const size_t smem = MODE == VR_ALPHA ? 2 * sizeof(float4) * (size_t)p.lut.n : 0;
-    if (smem != cached_smem) {
-        int dev = 0;
-        cudaError_t e = cudaGetDevice(&dev);
-        if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-        if (e == cudaSuccess)
-            e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&cached_per_sm, vr_raycast_kernel<MODE, LAY, PT, CLAMP, COUNT, SKIP, TEX>,
-                                                              VR_RAYCAST_THREADS, smem);
-        if (e != cudaSuccess) return e;
-        if (cached_per_sm < 1) return cudaErrorLaunchOutOfResources;
-        cached_smem = smem;
-    }
+static cudaError_t launch_variant(const VrRaycastParams& p0, long long items, bool sparse, cudaStream_t st) {
+    VrRaycastParams p = p0;
+    p.lut_copies = vr_lut_copies(p.lut.n, sparse);
+    if (TEX && p.lut_copies > VR_TEX_COPIES) p.lut_copies = VR_TEX_COPIES;
+    const size_t smem = MODE == VR_ALPHA ? sizeof(float4) * (size_t)p.lut.n * p.lut_copies : 0;
+    /* asked of the runtime at every launch (a few microseconds): the current device's SM count and this instance's
+     * residency with this much shared memory - no process-wide cache to go stale across devices or threads */
+    int dev = 0, sms = 0, cached_per_sm = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    if (e == cudaSuccess)
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&cached_per_sm, vr_raycast_kernel<MODE, LAY, PT, CLAMP, COUNT, SKIP, TEX>,
+                                                          VR_RAYCAST_THREADS, smem);
+    if (e != cudaSuccess) return e;
+    if (cached_per_sm < 1) return cudaErrorLaunchOutOfResources;
     /* Sparse MIP frames (several voxels per pixel: every load is a DRAM line of its own) run faster with two
      * resident CTAs per SM than with three - the lighter MIP loop keeps more lines in flight than L1/L2 hold
      * (c3: 14.5 -> 12.3 ms); dense frames and ALPHA want all three. */

@@ -7,7 +7,7 @@
  * while a pixel's ray crosses several bricks (4.7 on c2, 7 on c3): they are computed here once per
  * pixel of the frame - 18 FP64 divisions and a square root, individually rounded (DESIGN.md
  * "Set-up arithmetic") - and kept in the frame's ray table (vr_internal.cuh), from which the
- * ray-cast kernel starts every (ray, brick) segment with seven 16-byte loads. Only the pixels
+ * ray-cast kernel starts every (ray, brick) segment with four 16-byte loads and one of 4 bytes. Only the pixels
  * inside the union of the rendering rectangles (VrViewState::bound) are touched.
  */
 #include "vr_march.cuh"
@@ -29,7 +29,7 @@ vr_rays_kernel(const VrGrid g, const VrViewState* __restrict__ vs, int W, int H,
     if (i < bound.x || i >= bound.z || j < bound.y || j >= bound.w) return;
     RaySetup r;
     ray_setup(s_minv, W, H, i, j, g, step, r);
-    ray_store(rays, (long long)W * H, (long long)j * W + i, r);
+    ray_store(rays, (long long)W * H, (long long)j * W + i, step > 0.0, r);
 }
 
 cudaError_t vr_launch_rays(const VrGrid& grid, const VrViewState* vs, int W, int H, double step, double2* rays, cudaStream_t st) {

@@ -13,8 +13,8 @@
  * centres - R3's convention exactly, with the padded cell index as the texel index. The arrays
  * are a second copy of the brick store, filled from it on the device through surface objects
  * (vr_tex_fill_kernel) after an upload; the hand-rolled path keeps the float32 store, which
- * VR_MIP always uses (the hardware filter's 8 fractional weight bits cannot meet MIP's 1e-5) and to
- * which a VR_ALPHA sample falls back when the filter returns NaN (blanked voxels, R14).
+ * VR_MIP always uses (the hardware filter's 8 fractional weight bits cannot meet MIP's 1e-5), and which
+ * VR_ALPHA keeps using for bricks that hold blanked (NaN) voxels: the filter cannot apply R14's rule.
  */
 #include <string.h>
 
@@ -30,6 +30,7 @@ struct VrTexStore {
     cudaTextureObject_t* d_tex; /* device copies of the two tables */
     cudaSurfaceObject_t* d_surf;
     int3* d_ext;                /* padded extent of every slot */
+    int* d_nan;                 /* 1 where the slot holds a NaN (blanked) voxel: such bricks are sampled by hand (R14) */
 };
 
 void vr_tex_destroy(VrTexStore* t) {
@@ -42,6 +43,7 @@ void vr_tex_destroy(VrTexStore* t) {
     cudaFree(t->d_tex);
     cudaFree(t->d_surf);
     cudaFree(t->d_ext);
+    cudaFree(t->d_nan);
     delete[] t->arr;
     delete[] t->tex;
     delete[] t->surf;
@@ -92,6 +94,7 @@ cudaError_t vr_tex_create(const VrGrid& g, VrTexStore** out) {
     if (e == cudaSuccess) e = cudaMalloc(&t->d_tex, sizeof(cudaTextureObject_t) * g.nown);
     if (e == cudaSuccess) e = cudaMalloc(&t->d_surf, sizeof(cudaSurfaceObject_t) * g.nown);
     if (e == cudaSuccess) e = cudaMalloc(&t->d_ext, sizeof(int3) * g.nown);
+    if (e == cudaSuccess) e = cudaMalloc(&t->d_nan, sizeof(int) * g.nown);
     if (e == cudaSuccess) e = cudaMemcpy(t->d_tex, t->tex, sizeof(cudaTextureObject_t) * g.nown, cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMemcpy(t->d_surf, t->surf, sizeof(cudaSurfaceObject_t) * g.nown, cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMemcpy(t->d_ext, ext, sizeof(int3) * g.nown, cudaMemcpyHostToDevice);
@@ -106,6 +109,7 @@ cudaError_t vr_tex_create(const VrGrid& g, VrTexStore** out) {
 }
 
 const cudaTextureObject_t* vr_tex_table(const VrTexStore* t) { return t ? t->d_tex : NULL; }
+const int* vr_tex_nan_table(const VrTexStore* t) { return t ? t->d_nan : NULL; }
 
 /* Padded cell (i, j, k) of slot s -> texel (i, j, k) of the slot's array. A CTA takes the 4 x 2 rows
  * (j, k) of one row of micro-tiles, one row per warp, lanes along x, so the eight warps together consume
@@ -113,25 +117,35 @@ const cudaTextureObject_t* vr_tex_table(const VrTexStore* t) { return t ? t->d_t
  * write is coalesced. Once per upload. */
 __global__ void __launch_bounds__(256)
 vr_tex_fill_kernel(VrGrid g, const float* __restrict__ bricks, const cudaSurfaceObject_t* __restrict__ surf,
-                   const int3* __restrict__ ext) {
+                   const int3* __restrict__ ext, int* __restrict__ has_nan) {
     const int s = blockIdx.y;
     const int3 e = ext[s];
     const cudaSurfaceObject_t su = surf[s];
     const float* __restrict__ src = bricks + (long long)s * g.slot;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int nj = (e.y + 3) >> 2, nk = (e.z + 1) >> 1;
+    bool nan_seen = false;
     for (int blk = blockIdx.x; blk < nj * nk; blk += gridDim.x) {
         const int j = ((blk % nj) << 2) + (warp & 3), k = ((blk / nj) << 1) + (warp >> 2);
         if (j >= e.y || k >= e.z) continue;
         const unsigned row = vr_axis_offset(g.ax[1], j) + vr_axis_offset(g.ax[2], k);
-        for (int i = lane; i < e.x; i += 32) surf3Dwrite(__ldcs(src + row + vr_axis_offset(g.ax[0], i)), su, i * 4, j, k);
+        for (int i = lane; i < e.x; i += 32) {
+            const float v = __ldcs(src + row + vr_axis_offset(g.ax[0], i));
+            nan_seen = nan_seen || v != v;
+            surf3Dwrite(v, su, i * 4, j, k);
+        }
     }
+    /* R14: the hardware filter cannot apply the blanking rule (it drops a NaN corner whose 8-bit weight rounds to
+     * zero, the rule drops the SAMPLE from a weight of 4e-6 on): bricks with blanked voxels keep the hand-rolled sampler */
+    if (__any_sync(0xffffffffu, nan_seen) && lane == 0) has_nan[s] = 1;
 }
 
 cudaError_t vr_launch_tex_fill(const VrGrid& grid, const float* bricks, const VrTexStore* t, cudaStream_t st) {
     const int nj = (grid.P + 3) >> 2, nk = (grid.P + 1) >> 1;
     long long bx = (long long)nj * nk;
     if (bx > 4096) bx = 4096;
-    vr_tex_fill_kernel<<<dim3((unsigned)bx, (unsigned)t->n), 256, 0, st>>>(grid, bricks, t->d_surf, t->d_ext);
+    cudaError_t e = cudaMemsetAsync(t->d_nan, 0, sizeof(int) * t->n, st);
+    if (e != cudaSuccess) return e;
+    vr_tex_fill_kernel<<<dim3((unsigned)bx, (unsigned)t->n), 256, 0, st>>>(grid, bricks, t->d_surf, t->d_ext, t->d_nan);
     return cudaGetLastError();
 }

@@ -112,13 +112,26 @@ def test_texture_arm_follows_uploads_and_blanked_voxels(vr):
     assert np.abs(img - o.render(view, proj, W, H, 0.5, oracle.ALPHA)["image"]).max() > 1e-2  # not the first cube's frame
 
 
-def test_texture_arm_with_macro_cell_skipping_and_errors(vr):
-    """R19 beside the texture arm: frames bit-identical with skipping on / off; state errors."""
+def test_texture_arm_keeps_stepped_tables_on_the_hand_rolled_path_and_errors(vr):
+    """A transfer function with a step (threshold, toe) is outside what 8-bit filter weights can render to 2e-3
+    (measured 8e-2): such frames keep the hand-rolled sampler, bit for bit, also with macro-cell skipping; a smooth
+    table with a transparent range (three zero entries, then a gentle ramp) does use the texture arm with skipping."""
     cube = synth.Cube(33, 96, 80, 64, 10)
     g, o = tex_pair(vr, cube, 32, 1, tf=synth.tf_threshold())
     W, H = 160, 120
     fr = synth.Framing(cube.nx, cube.ny, cube.nz, W, H)
     view, proj = fr.seeded(9, 0), fr.proj(False)
+    tex_frame = gpu_frame(g, view, proj, W, H, 0.5, vr.ALPHA)
+    g.set_sampler(vr.SAMPLER_MANUAL)
+    assert np.array_equal(gpu_frame(g, view, proj, W, H, 0.5, vr.ALPHA), tex_frame)
+    g.set_sampler(vr.SAMPLER_TEXTURE)
+    check_alpha(tex_frame, o.render(view, proj, W, H, 0.5, oracle.ALPHA), 0.99, "threshold table")
+    # smooth table with a transparent range: alpha = max(0, u - 0.55) (zero below 4.2 sigma, then the ramp's slope: no
+    # step), colours = u
+    tf = synth.tf_ramp()
+    tf[:, 3] = np.maximum(0.0, tf[:, 3] - 0.55)
+    for v in (g, o):
+        v.set_transfer_function(tf, synth.TF_VMIN, synth.TF_VMAX)
     g.set_counting(1)
     on = gpu_frame(g, view, proj, W, H, 0.5, vr.ALPHA)
     n_on = g.debug_stats()["samples"]
@@ -127,6 +140,8 @@ def test_texture_arm_with_macro_cell_skipping_and_errors(vr):
     n_off = g.debug_stats()["samples"]
     assert np.array_equal(on, off) and n_on < n_off
     check_alpha(on, o.render(view, proj, W, H, 0.5, oracle.ALPHA), 0.99, "texture + skipping", envelope=True, max_flagged=1.0)
+    g.set_sampler(vr.SAMPLER_MANUAL)
+    assert 1e-7 < np.abs(gpu_frame(g, view, proj, W, H, 0.5, vr.ALPHA) - off).max() < 0.02  # the texture arm was in use
     lin = vr.Volume(32, 32, 32, 16, 1, layout=vr.LAYOUT_LINEAR)
     with pytest.raises(vr.VrError) as e:
         lin.set_sampler(vr.SAMPLER_TEXTURE)
