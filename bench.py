@@ -44,7 +44,7 @@ def workload(name):
     """Shapes, cameras and classification of BASELINE.json's configs."""
     c = dict(synth.CONFIGS[name])
     c["name"] = name
-    c["seed"] = synth.BASE_SEED + int(name[1:]) + (10 if name[0] == "n" else 0)
+    c["seed"] = synth.BASE_SEED + int(name[1:]) + {"n": 10, "s": 20}.get(name[0], 0)
     c.setdefault("kind", 0)
     fr = synth.Framing(c["nx"], c["ny"], c["nz"], c["width"], c["height"])
     if name == "c2":  # "1920x1080 perspective output, 36 seeded views"
@@ -725,7 +725,7 @@ def main():
     ap.add_argument("--steps", type=int, default=36)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="c3", choices=["c0", "c1", "c2", "c3", "c4", "n1"])
+    ap.add_argument("--workload", default="c3", choices=["c0", "c1", "c2", "c3", "c4", "n1", "s3"])
     ap.add_argument("--mode", default="alpha", choices=["alpha", "mip"])
     ap.add_argument("--tf", default="ramp", choices=["ramp", "translucent", "threshold"])
     ap.add_argument("--traversal", default="sort_last", choices=["sort_last", "fused"],
@@ -868,7 +868,7 @@ def main():
     smax = (m["clocks"] or {}).get("sm_max_mhz") if rank == 0 else None
     ray_gs = m["samples"] / K / (float(m["stages"][:, 1].mean()) * 1e-3) / 1e9
     alu = roofline_alu(ray_gs, args.mode, smax, traffic_of(args.workload, args.mode, args.tf))
-    if args.workload == "c3":
+    if args.workload in ("c3", "s3"):
         line["roofline_alu"] = alu
     else:
         line["roofline_hbm"], line["roofline"] = line["roofline"], alu

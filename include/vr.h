@@ -46,6 +46,7 @@
 #ifndef VR_H
 #define VR_H
 
+#include <stddef.h>
 #include <stdint.h>
 
 #ifdef __cplusplus
@@ -72,6 +73,19 @@ enum { VR_HOST = 0, VR_DEVICE = 1 }; /* memory space of a data pointer */
 enum { VR_LAYOUT_DEFAULT = 0, VR_LAYOUT_LINEAR = 1, VR_LAYOUT_TILED = 2 };
 
 typedef struct vr_volume vr_volume; /* opaque */
+
+/* Device memory for the library's long-lived buffers (north_star: "PyTorch used only for device
+ * memory and streams"). By default libvr takes the brick store, the tables and the per-view scratch from cudaMalloc.
+ * After vr_set_allocator(alloc, free, user) every handle created LATER takes them from the caller's allocator instead
+ * and returns them to it (the Python binding passes torch's caching allocator: use_torch_allocator()):
+ *   alloc(bytes, user) returns a device pointer aligned to 256 bytes, or NULL when out of memory;
+ *   free(ptr, user) is called once per pointer, with no work of the library pending on it.
+ * A handle keeps the pair it was created with. Both NULL: back to cudaMalloc. Not covered: the 3-D CUDA arrays of
+ * the texture arm (cudaMalloc3DArray has no pointer form) and short-lived tables of debug calls. Process-wide, not
+ * thread-safe against concurrent vr_volume_create. */
+typedef void* (*vr_alloc_fn)(size_t bytes, void* user);
+typedef void (*vr_free_fn)(void* ptr, void* user);
+int vr_set_allocator(vr_alloc_fn alloc_fn, vr_free_fn free_fn, void* user);
 
 /* Counters of the most recent vr_render on a handle (vr_debug_stats). */
 typedef struct vr_stats {
@@ -219,6 +233,15 @@ int vr_set_culling(vr_volume* v, int enable);
  * or nothing uploaded), VR_ERR_OUT_OF_MEMORY, VR_ERR_CUDA. */
 int vr_render(vr_volume* v, const float* view, const float* proj, int width, int height,
               float step, int mode, float* out_rgba, void* stream);
+
+/* Size the per-view scratch BEFORE rendering, so that vr_render never allocates and never synchronises the host
+ * ("vr_render is asynchronous on the given stream and never syncs the host"): sub-image scratch for
+ * the most demanding of the `nviews` given views (+25 %), the ray table and the host entries' device frames for
+ * width x height frames. views, projs (host): nviews * 16 floats each, as vr_render takes them. A frame that still
+ * needs more (a view not announced here) grows the scratch as before, which synchronises once. A frame whose set-up
+ * finds the scratch too small on the DEVICE (host and device rectangle arithmetic would have to disagree by more than
+ * the pixel of slack) comes out blank; the next vr_render / vr_render_host* call on the handle returns VR_ERR_STATE. */
+int vr_reserve_views(vr_volume* v, const float* views, const float* projs, int nviews, int width, int height);
 
 /* Traversal. VR_SORT_LAST (default) is the path above: every brick
  * renders its own sub-image with BRICK-LOCAL early termination (R8) and the sub-images are

@@ -222,6 +222,8 @@ int vro_brick_transparent(const vro_volume* v, int b) {
 
 int vro_set_tf(vro_volume* v, const float* rgba, int n, double vmin, double vmax) {
     if (!v || !rgba || n < 2 || !(vmax > vmin)) return 1;
+    for (int i = 0; i < n; ++i) /* R7: the table's alpha is an opacity per voxel of path, 1 - (1-a)^w needs a in [0,1] */
+        if (!(rgba[4 * i + 3] >= 0.0f && rgba[4 * i + 3] <= 1.0f)) return 1;
     free(v->tf);
     v->tf = (float*)malloc((size_t)n * 4 * sizeof(float));
     memcpy(v->tf, rgba, (size_t)n * 4 * sizeof(float));

@@ -28,7 +28,7 @@ STATUS = {0: "VR_OK", 1: "VR_ERR_INVALID_ARG", 2: "VR_ERR_OUT_OF_MEMORY", 3: "VR
 # every symbol include/vr.h declares (tests check the library exports each of them)
 SYMBOLS = (
     "vr_volume_create", "vr_volume_create_layout", "vr_volume_destroy", "vr_volume_upload", "vr_volume_download", "vr_debug_brick_data",
-    "vr_set_transfer_function", "vr_set_early_termination", "vr_volume_minmax", "vr_set_culling", "vr_set_traversal", "vr_set_sampler", "vr_debug_brick_minmax", "vr_debug_cell_flags", "vr_render", "vr_render_host", "vr_render_host_async", "vr_render_host_wait", "vr_composite",
+    "vr_set_transfer_function", "vr_set_early_termination", "vr_volume_minmax", "vr_set_culling", "vr_set_traversal", "vr_set_sampler", "vr_set_allocator", "vr_reserve_views", "vr_debug_brick_minmax", "vr_debug_cell_flags", "vr_render", "vr_render_host", "vr_render_host_async", "vr_render_host_wait", "vr_composite",
     "vr_num_bricks", "vr_debug_brick_order", "vr_debug_rects", "vr_debug_ray_bricks", "vr_debug_subimages",
     "vr_volume_create_part", "vr_render_part", "vr_part_rect", "vr_composite_parts",
     "vr_set_counting", "vr_set_timing", "vr_debug_stats", "vr_debug_stage_times", "vr_debug_probe_dram", "vr_launch_count", "vr_last_error",
@@ -75,6 +75,8 @@ def lib():
         L.vr_set_culling.argtypes = [vp, ci]
         L.vr_set_traversal.argtypes = [vp, ci]
         L.vr_set_sampler.argtypes = [vp, ci]
+        L.vr_set_allocator.argtypes = [vp, vp, vp]
+        L.vr_reserve_views.argtypes = [vp, vp, vp, ci, ci, ci]
         L.vr_debug_brick_minmax.argtypes = [vp, vp]
         L.vr_debug_cell_flags.argtypes = [vp, ci, vp, vp]
         L.vr_render.argtypes = [vp, vp, vp, ci, ci, cf, ci, vp, vp]
@@ -104,6 +106,12 @@ def lib():
     return _lib
 
 
+def _require(cond, what):
+    """Argument checks of the binding raise (an `assert` would vanish under python -O and let a bad pointer through)."""
+    if not cond:
+        raise ValueError("paper_1205_0282_b200: argument check failed: " + what)
+
+
 def _mat(m):
     return np.ascontiguousarray(np.asarray(m, dtype=np.float32).reshape(16))
 
@@ -117,6 +125,35 @@ def _stream(stream):
 
 def _pixels(pixels):
     return np.ascontiguousarray(pixels, dtype=np.int32).reshape(-1, 2)
+
+
+_ALLOC_KEEP = []  # the ctypes callbacks must outlive every handle created with them
+
+
+def use_torch_allocator(enable=True):
+    """vr_set_allocator with torch's caching allocator: handles created afterwards take their brick store, tables and
+    scratch from torch.cuda.caching_allocator_alloc on the current stream and give them back with
+    caching_allocator_delete, so torch sees (and can reuse) every byte the library holds. enable=False: cudaMalloc."""
+    if not enable:
+        if lib().vr_set_allocator(None, None, None) != 0:
+            raise VrError(1, lib().vr_last_error(None).decode())
+        return
+    import torch
+
+    @ctypes.CFUNCTYPE(ctypes.c_void_p, ctypes.c_size_t, ctypes.c_void_p)
+    def _alloc(nbytes, _user):
+        try:
+            return torch.cuda.caching_allocator_alloc(int(nbytes))
+        except Exception:  # torch raises on OOM: the C side wants NULL
+            return None
+
+    @ctypes.CFUNCTYPE(None, ctypes.c_void_p, ctypes.c_void_p)
+    def _free(ptr, _user):
+        torch.cuda.caching_allocator_delete(ptr)
+
+    _ALLOC_KEEP.extend([_alloc, _free])
+    if lib().vr_set_allocator(ctypes.cast(_alloc, ctypes.c_void_p), ctypes.cast(_free, ctypes.c_void_p), None) != 0:
+        raise VrError(1, lib().vr_last_error(None).decode())
 
 
 class Volume:
@@ -168,19 +205,19 @@ class Volume:
         """data: float32 [sz][sy][sx] numpy array (host) or CUDA torch tensor (device)."""
         if isinstance(data, np.ndarray):
             d = np.ascontiguousarray(data, dtype=np.float32)
-            assert d.ndim == 3
+            _require(d.ndim == 3, 'd.ndim == 3')
             self._check(lib().vr_volume_upload(self._h, d.ctypes.data, HOST, *self._box(d.shape, origin), _stream(stream)))
         else:
-            assert data.is_cuda and data.is_contiguous() and data.dtype.is_floating_point and data.element_size() == 4
-            assert data.dim() == 3
+            _require(data.is_cuda and data.is_contiguous() and data.dtype.is_floating_point and data.element_size() == 4, 'data.is_cuda and data.is_contiguous() and data.dtype.is_floating_point and data.element_size() == 4')
+            _require(data.dim() == 3, 'data.dim() == 3')
             self._check(lib().vr_volume_upload(self._h, data.data_ptr(), DEVICE, *self._box(data.shape, origin), _stream(stream)))
 
     def download(self, out, origin=(0, 0, 0), stream=None):
         if isinstance(out, np.ndarray):
-            assert out.dtype == np.float32 and out.flags.c_contiguous and out.ndim == 3
+            _require(out.dtype == np.float32 and out.flags.c_contiguous and out.ndim == 3, 'out.dtype == np.float32 and out.flags.c_contiguous and out.ndim == 3')
             self._check(lib().vr_volume_download(self._h, out.ctypes.data, HOST, *self._box(out.shape, origin), _stream(stream)))
         else:
-            assert out.is_cuda and out.is_contiguous() and out.element_size() == 4 and out.dim() == 3
+            _require(out.is_cuda and out.is_contiguous() and out.element_size() == 4 and out.dim() == 3, 'out.is_cuda and out.is_contiguous() and out.element_size() == 4 and out.dim() == 3')
             self._check(lib().vr_volume_download(self._h, out.data_ptr(), DEVICE, *self._box(out.shape, origin), _stream(stream)))
         return out
 
@@ -194,7 +231,7 @@ class Volume:
     # -- classification (a6), termination (a7) --------------------------------
     def set_transfer_function(self, rgba, vmin, vmax):
         t = np.ascontiguousarray(rgba, dtype=np.float32)
-        assert t.ndim == 2 and t.shape[1] == 4
+        _require(t.ndim == 2 and t.shape[1] == 4, 't.ndim == 2 and t.shape[1] == 4')
         self._check(lib().vr_set_transfer_function(self._h, t.ctypes.data, t.shape[0], float(vmin), float(vmax)))
 
     def set_early_termination(self, tau):
@@ -236,16 +273,24 @@ class Volume:
     # -- one frame (a2..a9) ---------------------------------------------------
     def render(self, view, proj, width, height, step, mode, out, stream=None):
         """out: CUDA float32 tensor [height][width][4]; asynchronous on the stream."""
-        assert out.is_cuda and out.is_contiguous() and out.element_size() == 4 and out.numel() == width * height * 4
+        _require(out.is_cuda and out.is_contiguous() and out.element_size() == 4 and out.numel() == width * height * 4, 'out.is_cuda and out.is_contiguous() and out.element_size() == 4 and out.numel() == width * height * 4')
         v, p = _mat(view), _mat(proj)
         self._check(lib().vr_render(self._h, v.ctypes.data, p.ctypes.data, int(width), int(height), float(step), int(mode),
                                     out.data_ptr(), _stream(stream)))
         return out
 
+    def reserve_views(self, views, projs, width, height):
+        """vr_reserve_views: size the scratch for these views so that render() never allocates or synchronises."""
+        v = np.ascontiguousarray(np.stack([_mat(m) for m in views]) if len(views) else np.zeros((0, 16), np.float32))
+        p = np.ascontiguousarray(np.stack([_mat(m) for m in projs]) if len(projs) else np.zeros((0, 16), np.float32))
+        if v.shape != p.shape:
+            raise ValueError("reserve_views: as many projection as view matrices")
+        self._check(lib().vr_reserve_views(self._h, v.ctypes.data, p.ctypes.data, v.shape[0], int(width), int(height)))
+
     def render_part(self, view, proj, width, height, step, mode, out, stream=None):
         """This handle's contribution to a sort-last frame (vr_render_part). out: CUDA float32 tensor
         [height][width][4]; returns the rectangle (x0,y0,x1,y1) outside which out is blank."""
-        assert out.is_cuda and out.is_contiguous() and out.element_size() == 4 and out.numel() == width * height * 4
+        _require(out.is_cuda and out.is_contiguous() and out.element_size() == 4 and out.numel() == width * height * 4, 'out.is_cuda and out.is_contiguous() and out.element_size() == 4 and out.numel() == width * height * 4')
         v, p = _mat(view), _mat(proj)
         rect = np.zeros(4, dtype=np.int32)
         self._check(lib().vr_render_part(self._h, v.ctypes.data, p.ctypes.data, int(width), int(height), float(step), int(mode),
@@ -260,9 +305,9 @@ class Volume:
         r = np.ascontiguousarray(rects, dtype=np.int32).reshape(n, 4)
         o = np.ascontiguousarray(order, dtype=np.int32).reshape(n)
         for l, rc_ in zip(parts, r):
-            assert l.is_cuda and l.is_contiguous() and l.element_size() == 4
-            assert l.numel() == (rc_[2] - rc_[0]) * (rc_[3] - rc_[1]) * 4
-        assert out.is_cuda and out.is_contiguous() and out.numel() == width * height * 4
+            _require(l.is_cuda and l.is_contiguous() and l.element_size() == 4, 'l.is_cuda and l.is_contiguous() and l.element_size() == 4')
+            _require(l.numel() == (rc_[2] - rc_[0]) * (rc_[3] - rc_[1]) * 4, 'l.numel() == (rc_[2] - rc_[0]) * (rc_[3] - rc_[1]) * 4')
+        _require(out.is_cuda and out.is_contiguous() and out.numel() == width * height * 4, 'out.is_cuda and out.is_contiguous() and out.numel() == width * height * 4')
         self._check(lib().vr_composite_parts(self._h, int(mode), ptrs, r.ctypes.data, o.ctypes.data, n, int(width), int(height),
                                              out.data_ptr(), _stream(stream)))
         return out
@@ -273,10 +318,10 @@ class Volume:
         if out is None:
             out = np.empty((height, width, 4), dtype=np.float32)
         if isinstance(out, np.ndarray):
-            assert out.dtype == np.float32 and out.flags.c_contiguous and out.size == width * height * 4
+            _require(out.dtype == np.float32 and out.flags.c_contiguous and out.size == width * height * 4, 'out.dtype == np.float32 and out.flags.c_contiguous and out.size == width * height * 4')
             ptr = out.ctypes.data
         else:
-            assert (not out.is_cuda) and out.is_contiguous() and out.element_size() == 4 and out.numel() == width * height * 4
+            _require((not out.is_cuda) and out.is_contiguous() and out.element_size() == 4 and out.numel() == width * height * 4, '(not out.is_cuda) and out.is_contiguous() and out.element_size() == 4 and out.numel() == width * height * 4')
             ptr = out.data_ptr()
         self._check(lib().vr_render_host(self._h, v.ctypes.data, p.ctypes.data, int(width), int(height), float(step),
                                          int(mode), ptr, _stream(stream)))
@@ -287,10 +332,10 @@ class Volume:
         render_host_wait() has returned; use one buffer per frame in flight (two are)."""
         v, p = _mat(view), _mat(proj)
         if isinstance(out, np.ndarray):
-            assert out.dtype == np.float32 and out.flags.c_contiguous and out.size == width * height * 4
+            _require(out.dtype == np.float32 and out.flags.c_contiguous and out.size == width * height * 4, 'out.dtype == np.float32 and out.flags.c_contiguous and out.size == width * height * 4')
             ptr = out.ctypes.data
         else:
-            assert (not out.is_cuda) and out.is_contiguous() and out.element_size() == 4 and out.numel() == width * height * 4
+            _require((not out.is_cuda) and out.is_contiguous() and out.element_size() == 4 and out.numel() == width * height * 4, '(not out.is_cuda) and out.is_contiguous() and out.element_size() == 4 and out.numel() == width * height * 4')
             ptr = out.data_ptr()
         self._check(lib().vr_render_host_async(self._h, v.ctypes.data, p.ctypes.data, int(width), int(height), float(step),
                                                int(mode), ptr, _stream(stream)))
@@ -391,9 +436,9 @@ def composite(layers, rects, order, width, height, out, stream=None):
     r = np.ascontiguousarray(rects, dtype=np.int32).reshape(n, 4)
     o = np.ascontiguousarray(order, dtype=np.int32).reshape(n)
     for l, rc_ in zip(layers, r):
-        assert l.is_cuda and l.is_contiguous() and l.element_size() == 4
-        assert l.numel() == (rc_[2] - rc_[0]) * (rc_[3] - rc_[1]) * 4
-    assert out.is_cuda and out.is_contiguous() and out.numel() == width * height * 4
+        _require(l.is_cuda and l.is_contiguous() and l.element_size() == 4, 'l.is_cuda and l.is_contiguous() and l.element_size() == 4')
+        _require(l.numel() == (rc_[2] - rc_[0]) * (rc_[3] - rc_[1]) * 4, 'l.numel() == (rc_[2] - rc_[0]) * (rc_[3] - rc_[1]) * 4')
+    _require(out.is_cuda and out.is_contiguous() and out.numel() == width * height * 4, 'out.is_cuda and out.is_contiguous() and out.numel() == width * height * 4')
     rc = lib().vr_composite(ptrs, r.ctypes.data, o.ctypes.data, n, int(width), int(height), out.data_ptr(), _stream(stream))
     if rc != 0:
         raise VrError(rc, lib().vr_last_error(None).decode())

@@ -14,6 +14,9 @@
 
 #include "vr_internal.cuh"
 
+static char g_err[512] = "no error";
+static char* g_err_buf() { return g_err; }
+
 struct vr_volume {
     VrGrid grid;
     float* bricks;           /* nown * slot floats (nown = nbricks unless the handle is a part) */
@@ -68,10 +71,46 @@ struct vr_volume {
     bool last_valid;       /* the last frame's sub-images are still in the scratch */
     bool last_stats_valid; /* the last frame's counters are still in the view state */
     int64_t launches;
+    vr_alloc_fn alloc_fn;    /* the allocator in force when the handle was created (vr_set_allocator), or NULL = cudaMalloc */
+    vr_free_fn free_fn;
+    void* alloc_user;
+    int* h_overflow;         /* mapped pinned flag the set-up kernel raises when a view needs more scratch than reserved */
+    int* d_overflow;         /* its device address */
     char err[512];
 };
 
-static char g_err[512] = "no error";
+/* process-wide allocator for handles created from now on (vr_set_allocator) */
+static vr_alloc_fn g_alloc_fn = NULL;
+static vr_free_fn g_free_fn = NULL;
+static void* g_alloc_user = NULL;
+
+extern "C" int vr_set_allocator(vr_alloc_fn alloc_fn, vr_free_fn free_fn, void* user) {
+    if ((alloc_fn == NULL) != (free_fn == NULL)) {
+        snprintf(g_err_buf(), 512, "vr_set_allocator: alloc and free must both be given, or both be NULL");
+        return VR_ERR_INVALID_ARG;
+    }
+    g_alloc_fn = alloc_fn;
+    g_free_fn = free_fn;
+    g_alloc_user = user;
+    return VR_OK;
+}
+
+/* device memory the handle owns: through the handle's allocator (torch's caching allocator in the Python binding) */
+static cudaError_t v_alloc_bytes(const vr_volume* v, void** p, size_t bytes) {
+    if (!v->alloc_fn) return cudaMalloc(p, bytes);
+    *p = v->alloc_fn(bytes ? bytes : 1, v->alloc_user);
+    return *p ? cudaSuccess : cudaErrorMemoryAllocation;
+}
+template <typename T>
+static cudaError_t v_alloc(const vr_volume* v, T** p, size_t bytes) {
+    return v_alloc_bytes(v, reinterpret_cast<void**>(p), bytes);
+}
+static void v_free(const vr_volume* v, void* p) {
+    if (!p) return;
+    if (v->free_fn) v->free_fn(p, v->alloc_user);
+    else cudaFree(p);
+}
+
 
 static int fail(vr_volume* v, int status, const char* fmt, ...) {
     char* dst = v ? v->err : g_err;
@@ -100,31 +139,32 @@ extern "C" int64_t vr_launch_count(const vr_volume* v) { return v ? v->launches 
 
 static void release(vr_volume* v) {
     vr_tex_destroy(v->tex);
-    cudaFree(v->bricks);
-    cudaFree(v->d_lut_base);
-    cudaFree(v->d_lut_delta);
-    cudaFree(v->d_vs);
-    cudaFree(v->d_bv);
-    cudaFree(v->d_order);
-    cudaFree(v->d_item_prefix);
-    cudaFree(v->d_layers);
-    cudaFree(v->d_sub);
-    cudaFree(v->d_rays);
-    cudaFree(v->d_frame);
+    if (v->h_overflow) cudaFreeHost(v->h_overflow);
+    v_free(v, v->bricks);
+    v_free(v, v->d_lut_base);
+    v_free(v, v->d_lut_delta);
+    v_free(v, v->d_vs);
+    v_free(v, v->d_bv);
+    v_free(v, v->d_order);
+    v_free(v, v->d_item_prefix);
+    v_free(v, v->d_layers);
+    v_free(v, v->d_sub);
+    v_free(v, v->d_rays);
+    v_free(v, v->d_frame);
     for (int i = 0; i < 2; ++i) {
-        cudaFree(v->d_pipe[i]);
+        v_free(v, v->d_pipe[i]);
         if (v->ev_rendered[i]) cudaEventDestroy(v->ev_rendered[i]);
         if (v->ev_copied[i]) cudaEventDestroy(v->ev_copied[i]);
     }
     if (v->copy_stream) cudaStreamDestroy(v->copy_stream);
-    cudaFree(v->d_stage);
-    cudaFree(v->d_bitmap);
-    cudaFree(v->d_mm_enc);
-    cudaFree(v->d_mm);
-    cudaFree(v->d_cell_mm);
-    cudaFree(v->d_cell_bits);
-    cudaFree(v->d_cell_count);
-    cudaFree(v->d_counts2);
+    v_free(v, v->d_stage);
+    v_free(v, v->d_bitmap);
+    v_free(v, v->d_mm_enc);
+    v_free(v, v->d_mm);
+    v_free(v, v->d_cell_mm);
+    v_free(v, v->d_cell_bits);
+    v_free(v, v->d_cell_count);
+    v_free(v, v->d_counts2);
     for (int r = 0; r < VR_EV_RING; ++r)
         for (int i = 0; i < 4; ++i)
             if (v->ev[r][i]) cudaEventDestroy(v->ev[r][i]);
@@ -261,9 +301,22 @@ static int create_volume(int nx, int ny, int nz, int brick, int ghost, int layou
     g.brick_pow2 = (brick & (brick - 1)) == 0;
     {
         int tl[3] = {2, 2, 1}, ml[3] = {0, 0, 0};
-        if (const char* e = getenv("VR_TILE")) /* experiment knob: "lx,ly,lz,mx,my,mz" (log2) */
-            sscanf(e, "%d,%d,%d,%d,%d,%d", &tl[0], &tl[1], &tl[2], &ml[0], &ml[1], &ml[2]);
-        if (const char* e = getenv("VR_LAYOUT")) layout = atoi(e) == 1 ? VR_LAYOUT_LINEAR : VR_LAYOUT_TILED;
+        if (const char* e = getenv("VR_TILE")) { /* experiment knob: "lx,ly,lz,mx,my,mz" (log2) */
+            const int got = sscanf(e, "%d,%d,%d,%d,%d,%d", &tl[0], &tl[1], &tl[2], &ml[0], &ml[1], &ml[2]);
+            bool ok = got == 6 && tl[0] + tl[1] + tl[2] == 5; /* a micro-tile is 32 floats = one 128-byte line */
+            for (int a = 0; a < 3; ++a) ok = ok && tl[a] >= 0 && tl[a] <= 5 && ml[a] >= 0 && ml[a] <= 4;
+            if (!ok) {
+                delete v;
+                return fail(NULL, VR_ERR_INVALID_ARG, "vr_volume_create: VR_TILE=\"%s\" is not six log2 sizes with lx+ly+lz = 5, m* in [0,4]", e);
+            }
+        }
+        if (const char* e = getenv("VR_LAYOUT")) {
+            if (strcmp(e, "1") != 0 && strcmp(e, "2") != 0) {
+                delete v;
+                return fail(NULL, VR_ERR_INVALID_ARG, "vr_volume_create: VR_LAYOUT=\"%s\" is neither 1 (linear) nor 2 (tiled)", e);
+            }
+            layout = e[0] == '1' ? VR_LAYOUT_LINEAR : VR_LAYOUT_TILED;
+        }
         set_layout(g, layout, tl, ml);
     }
     if (g.slot >= (1ll << 31)) {
@@ -272,21 +325,29 @@ static int create_volume(int nx, int ny, int nz, int brick, int ghost, int layou
     }
     v->tau = 0.99f;
     v->culling = true;
+    v->alloc_fn = g_alloc_fn;
+    v->free_fn = g_free_fn;
+    v->alloc_user = g_alloc_user;
 
-    cudaError_t e = cudaMalloc(&v->bricks, (size_t)g.slot * (size_t)g.nown * sizeof(float));
+    cudaError_t e = v_alloc(v, &v->bricks, (size_t)g.slot * (size_t)g.nown * sizeof(float));
     if (e == cudaSuccess) e = cudaMemset(v->bricks, 0, (size_t)g.slot * (size_t)g.nown * sizeof(float));
-    if (e == cudaSuccess) e = cudaMalloc(&v->d_lut_base, VR_MAX_LUT * sizeof(float4));
-    if (e == cudaSuccess) e = cudaMalloc(&v->d_lut_delta, VR_MAX_LUT * sizeof(float4));
-    if (e == cudaSuccess) e = cudaMalloc(&v->d_vs, sizeof(VrViewState));
+    if (e == cudaSuccess) e = v_alloc(v, &v->d_lut_base, VR_MAX_LUT * sizeof(float4));
+    if (e == cudaSuccess) e = v_alloc(v, &v->d_lut_delta, VR_MAX_LUT * sizeof(float4));
+    if (e == cudaSuccess) e = v_alloc(v, &v->d_vs, sizeof(VrViewState));
     if (e == cudaSuccess) e = cudaMemset(v->d_vs, 0, sizeof(VrViewState));
-    if (e == cudaSuccess) e = cudaMalloc(&v->d_bv, sizeof(VrBrickView) * g.nbricks);
-    if (e == cudaSuccess) e = cudaMalloc(&v->d_order, sizeof(int) * g.nbricks);
-    if (e == cudaSuccess) e = cudaMalloc(&v->d_item_prefix, sizeof(int) * (g.nbricks + 1));
-    if (e == cudaSuccess) e = cudaMalloc(&v->d_layers, sizeof(VrCompLayer) * g.nbricks);
-    if (e == cudaSuccess) e = cudaMalloc(&v->d_mm_enc, sizeof(int2) * g.nbricks);
-    if (e == cudaSuccess) e = cudaMalloc(&v->d_mm, sizeof(float2) * (g.nbricks + 1));
+    if (e == cudaSuccess) e = v_alloc(v, &v->d_bv, sizeof(VrBrickView) * g.nbricks);
+    if (e == cudaSuccess) e = v_alloc(v, &v->d_order, sizeof(int) * g.nbricks);
+    if (e == cudaSuccess) e = v_alloc(v, &v->d_item_prefix, sizeof(int) * (g.nbricks + 1));
+    if (e == cudaSuccess) e = v_alloc(v, &v->d_layers, sizeof(VrCompLayer) * g.nbricks);
+    if (e == cudaSuccess) e = v_alloc(v, &v->d_mm_enc, sizeof(int2) * g.nbricks);
+    if (e == cudaSuccess) e = v_alloc(v, &v->d_mm, sizeof(float2) * (g.nbricks + 1));
     for (int r = 0; r < VR_EV_RING && e == cudaSuccess; ++r)
         for (int i = 0; i < 4 && e == cudaSuccess; ++i) e = cudaEventCreate(&v->ev[r][i]);
+    if (e == cudaSuccess) e = cudaHostAlloc(&v->h_overflow, sizeof(int), cudaHostAllocMapped);
+    if (e == cudaSuccess) {
+        *v->h_overflow = 0;
+        e = cudaHostGetDevicePointer(&v->d_overflow, v->h_overflow, 0);
+    }
     if (e != cudaSuccess) {
         cudaGetLastError();
         const int st = (e == cudaErrorMemoryAllocation) ? VR_ERR_OUT_OF_MEMORY : VR_ERR_CUDA;
@@ -320,11 +381,11 @@ static int ensure_stage(vr_volume* v, int sx, int sy, int sz, int* planes) {
     if (v->stage_floats < n * plane) {
         if (v->d_stage) {
             cudaDeviceSynchronize();
-            cudaFree(v->d_stage);
+            v_free(v, v->d_stage);
             v->d_stage = NULL;
             v->stage_floats = 0;
         }
-        VR_CUDA(v, cudaMalloc(&v->d_stage, (size_t)(n * plane) * sizeof(float)));
+        VR_CUDA(v, v_alloc(v, &v->d_stage, (size_t)(n * plane) * sizeof(float)));
         v->stage_floats = n * plane;
     }
     *planes = (int)n;
@@ -432,6 +493,9 @@ extern "C" int vr_set_transfer_function(vr_volume* v, const float* rgba, int n, 
         return fail(v, VR_ERR_INVALID_ARG, "vr_set_transfer_function: need finite vmin < vmax");
     for (int i = 0; i < 4 * n; ++i)
         if (!isfinite(rgba[i])) return fail(v, VR_ERR_INVALID_ARG, "vr_set_transfer_function: entry %d is not finite", i / 4);
+    for (int i = 0; i < n; ++i) /* R7: the table's alpha is an opacity; log2(1 - a) of anything else is NaN */
+        if (!(rgba[4 * i + 3] >= 0.0f && rgba[4 * i + 3] <= 1.0f))
+            return fail(v, VR_ERR_INVALID_ARG, "vr_set_transfer_function: alpha %g of entry %d outside [0,1]", rgba[4 * i + 3], i);
     /* the table is stored as (entry, difference to the next entry) pairs; the differences are
      * plain float32 subtractions of the caller's entries */
     float4 base[VR_MAX_LUT], delta[VR_MAX_LUT]; /* 32 KB of stack: no state shared between handles or threads */
@@ -485,8 +549,8 @@ extern "C" int vr_set_counting(vr_volume* v, int enable) {
     if (enable < 0 || enable > 2) return fail(v, VR_ERR_INVALID_ARG, "vr_set_counting: mode %d outside [0,2]", enable);
     if (enable == 2 && !v->d_bitmap) {
         const long long words = (v->grid.slot * v->grid.nown + 31) / 32;
-        VR_CUDA(v, cudaMalloc(&v->d_bitmap, (size_t)words * sizeof(unsigned)));
-        VR_CUDA(v, cudaMalloc(&v->d_counts2, 3 * sizeof(unsigned long long)));
+        VR_CUDA(v, v_alloc(v, &v->d_bitmap, (size_t)words * sizeof(unsigned)));
+        VR_CUDA(v, v_alloc(v, &v->d_counts2, 3 * sizeof(unsigned long long)));
         v->bitmap_words = words;
     }
     v->counting = enable;
@@ -514,16 +578,27 @@ static int check_view(vr_volume* v, const char* who, const float* view, const fl
     return VR_OK;
 }
 
+/* A view that needed more sub-image scratch than was reserved (host and device rectangle arithmetic disagreed by more
+ * than the slack, or vr_reserve_views was given other views) renders a blank frame and raises a flag in mapped host
+ * memory: the next call on the handle that looks reports it. */
+static int check_overflow(vr_volume* v, const char* who) {
+    if (v->h_overflow && *(volatile int*)v->h_overflow) {
+        *v->h_overflow = 0;
+        return fail(v, VR_ERR_STATE, "%s: an earlier frame needed more sub-image scratch than was reserved and came out blank", who);
+    }
+    return VR_OK;
+}
+
 static int ensure_sub(vr_volume* v, long long need_px) {
     if (need_px <= v->sub_capacity_px) return VR_OK;
     if (v->d_sub) {
         VR_CUDA(v, cudaDeviceSynchronize());
-        cudaFree(v->d_sub);
+        v_free(v, v->d_sub);
         v->d_sub = NULL;
         v->sub_capacity_px = 0;
     }
     const long long cap = need_px + need_px / 4 + 4096; /* headroom: neighbouring views fit too */
-    VR_CUDA(v, cudaMalloc(&v->d_sub, (size_t)cap * 16));
+    VR_CUDA(v, v_alloc(v, &v->d_sub, (size_t)cap * 16));
     v->sub_capacity_px = cap;
     return VR_OK;
 }
@@ -533,12 +608,34 @@ static int ensure_rays(vr_volume* v, long long px) {
     if (px <= v->ray_capacity_px) return VR_OK;
     if (v->d_rays) {
         VR_CUDA(v, cudaDeviceSynchronize());
-        cudaFree(v->d_rays);
+        v_free(v, v->d_rays);
         v->d_rays = NULL;
         v->ray_capacity_px = 0;
     }
-    VR_CUDA(v, cudaMalloc(&v->d_rays, (size_t)px * VR_RAY_BYTES + 16));
+    VR_CUDA(v, v_alloc(v, &v->d_rays, (size_t)px * VR_RAY_BYTES + 16));
     v->ray_capacity_px = px;
+    return VR_OK;
+}
+
+/* vr_render_host_async's two device frames, copy stream and events, for frames of px pixels */
+static int ensure_pipe(vr_volume* v, long long px) {
+    if (!v->copy_stream) {
+        VR_CUDA(v, cudaStreamCreateWithFlags(&v->copy_stream, cudaStreamNonBlocking));
+        for (int i = 0; i < 2; ++i) {
+            VR_CUDA(v, cudaEventCreateWithFlags(&v->ev_rendered[i], cudaEventDisableTiming));
+            VR_CUDA(v, cudaEventCreateWithFlags(&v->ev_copied[i], cudaEventDisableTiming));
+        }
+    }
+    if (px > v->pipe_capacity_px) {
+        VR_CUDA(v, cudaDeviceSynchronize());
+        for (int i = 0; i < 2; ++i) {
+            v_free(v, v->d_pipe[i]);
+            v->d_pipe[i] = NULL;
+        }
+        v->pipe_capacity_px = 0;
+        for (int i = 0; i < 2; ++i) VR_CUDA(v, v_alloc(v, &v->d_pipe[i], (size_t)px * 16));
+        v->pipe_capacity_px = px;
+    }
     return VR_OK;
 }
 
@@ -565,8 +662,8 @@ static int ensure_cells(vr_volume* v, bool want_bits, cudaStream_t st) {
         for (int a = 0; a < 3; ++a) v->nc[a] = (g.nt[a] * (1 << g.tl[a]) + 7) / 8;
         const long long ncell = (long long)v->nc[0] * v->nc[1] * v->nc[2];
         v->cell_words = (int)((ncell + 31) / 32);
-        VR_CUDA(v, cudaMalloc(&v->d_cell_mm, sizeof(float2) * (size_t)ncell * g.nown));
-        VR_CUDA(v, cudaMalloc(&v->d_cell_bits, sizeof(unsigned) * (size_t)v->cell_words * g.nown));
+        VR_CUDA(v, v_alloc(v, &v->d_cell_mm, sizeof(float2) * (size_t)ncell * g.nown));
+        VR_CUDA(v, v_alloc(v, &v->d_cell_bits, sizeof(unsigned) * (size_t)v->cell_words * g.nown));
     }
     if (!v->cell_mm_valid) {
         VR_CUDA(v, vr_launch_cell_minmax(g, v->bricks, v->d_cell_mm, v->nc, st));
@@ -590,7 +687,7 @@ static int decide_mip_skip(vr_volume* v, cudaStream_t st) {
     int rc = ensure_minmax(v, st);
     if (!rc) rc = ensure_cells(v, false, st);
     if (rc) return rc;
-    if (!v->d_cell_count) VR_CUDA(v, cudaMalloc(&v->d_cell_count, sizeof(unsigned long long)));
+    if (!v->d_cell_count) VR_CUDA(v, v_alloc(v, &v->d_cell_count, sizeof(unsigned long long)));
     const long long ncells = (long long)v->nc[0] * v->nc[1] * v->nc[2] * v->grid.nown;
     unsigned long long empty = 0;
     VR_CUDA(v, cudaMemsetAsync(v->d_cell_count, 0, sizeof(unsigned long long), st));
@@ -613,9 +710,39 @@ static int run_setup(vr_volume* v, const float* view, const float* proj, int W, 
         if (rc) return rc;
     }
     VR_CUDA(v, vr_launch_setup(v->grid, m, W, H, mode, v->sub_capacity_px, v->d_sub, v->d_vs, v->d_bv, v->d_order,
-                               v->d_item_prefix, v->d_layers, use_range ? v->d_mm : NULL, v->lut, st));
+                               v->d_item_prefix, v->d_layers, use_range ? v->d_mm : NULL, v->lut, v->d_overflow, st));
     v->launches++;
     return VR_OK;
+}
+
+extern "C" int vr_reserve_views(vr_volume* v, const float* views, const float* projs, int nviews, int width, int height) {
+    if (!v) return fail(NULL, VR_ERR_INVALID_ARG, "vr_reserve_views: NULL handle");
+    if (nviews < 0 || (nviews > 0 && (!views || !projs))) return fail(v, VR_ERR_INVALID_ARG, "vr_reserve_views: NULL matrices");
+    if (width <= 0 || height <= 0 || width > 32768 || height > 32768)
+        return fail(v, VR_ERR_INVALID_ARG, "vr_reserve_views: bad frame size %dx%d", width, height);
+    long long need = 0;
+    for (int q = 0; q < nviews; ++q) {
+        long long sub_px = 0, items = 0;
+        const int rc = check_view(v, "vr_reserve_views", views + 16 * q, projs + 16 * q, width, height, &sub_px, &items);
+        if (rc) return rc;
+        if (sub_px > need) need = sub_px;
+    }
+    const long long px = (long long)width * height;
+    int rc = ensure_sub(v, need > 0 ? need : px);
+    if (!rc) rc = ensure_rays(v, px);
+    if (rc) return rc;
+    /* the host entries' device frames (vr_render_host: one; vr_render_host_async: two, a stream and four events) */
+    if (px > v->frame_capacity_px) {
+        if (v->d_frame) {
+            VR_CUDA(v, cudaDeviceSynchronize());
+            v_free(v, v->d_frame);
+            v->d_frame = NULL;
+            v->frame_capacity_px = 0;
+        }
+        VR_CUDA(v, v_alloc(v, &v->d_frame, (size_t)px * 16));
+        v->frame_capacity_px = px;
+    }
+    return ensure_pipe(v, px);
 }
 
 extern "C" int vr_volume_minmax(vr_volume* v, float* vmin_out, float* vmax_out, void* stream) {
@@ -755,6 +882,8 @@ static int render_frame(vr_volume* v, const float* view, const float* proj, int 
     long long sub_px = 0, items = 0;
     int rc = check_view(v, "vr_render", view, proj, width, height, &sub_px, &items);
     if (rc) return rc;
+    rc = check_overflow(v, "vr_render");
+    if (rc) return rc;
     if (partial && mode == VR_MIP && v->traversal == VR_FUSED)
         return fail(v, VR_ERR_STATE, "vr_render_part: VR_MIP parts need the VR_SORT_LAST traversal");
     if (!out_rgba) return fail(v, VR_ERR_INVALID_ARG, "vr_render: NULL output");
@@ -865,11 +994,11 @@ extern "C" int vr_render_host(vr_volume* v, const float* view, const float* proj
     if (px > v->frame_capacity_px) {
         if (v->d_frame) {
             VR_CUDA(v, cudaDeviceSynchronize());
-            cudaFree(v->d_frame); /* only the synchronous entry's own frame: the pipelined entry's frames, events and stream stay */
+            v_free(v, v->d_frame); /* only the synchronous entry's own frame: the pipelined entry's frames, events and stream stay */
             v->d_frame = NULL;
             v->frame_capacity_px = 0;
         }
-        VR_CUDA(v, cudaMalloc(&v->d_frame, (size_t)px * 16));
+        VR_CUDA(v, v_alloc(v, &v->d_frame, (size_t)px * 16));
         v->frame_capacity_px = px;
     }
     const int rc = vr_render(v, view, proj, width, height, step, mode, v->d_frame, stream);
@@ -877,7 +1006,7 @@ extern "C" int vr_render_host(vr_volume* v, const float* view, const float* proj
     cudaStream_t st = (cudaStream_t)stream;
     VR_CUDA(v, cudaMemcpyAsync(out_rgba_host, v->d_frame, (size_t)px * 16, cudaMemcpyDeviceToHost, st));
     VR_CUDA(v, cudaStreamSynchronize(st));
-    return VR_OK;
+    return check_overflow(v, "vr_render_host");
 }
 
 extern "C" int vr_render_host_async(vr_volume* v, const float* view, const float* proj, int width, int height, float step,
@@ -887,23 +1016,8 @@ extern "C" int vr_render_host_async(vr_volume* v, const float* view, const float
     if (width <= 0 || height <= 0 || width > 32768 || height > 32768)
         return fail(v, VR_ERR_INVALID_ARG, "vr_render_host_async: bad frame size %dx%d", width, height);
     const long long px = (long long)width * height;
-    if (!v->copy_stream) {
-        VR_CUDA(v, cudaStreamCreateWithFlags(&v->copy_stream, cudaStreamNonBlocking));
-        for (int i = 0; i < 2; ++i) {
-            VR_CUDA(v, cudaEventCreateWithFlags(&v->ev_rendered[i], cudaEventDisableTiming));
-            VR_CUDA(v, cudaEventCreateWithFlags(&v->ev_copied[i], cudaEventDisableTiming));
-        }
-    }
-    if (px > v->pipe_capacity_px) {
-        VR_CUDA(v, cudaDeviceSynchronize());
-        for (int i = 0; i < 2; ++i) {
-            cudaFree(v->d_pipe[i]);
-            v->d_pipe[i] = NULL;
-        }
-        v->pipe_capacity_px = 0;
-        for (int i = 0; i < 2; ++i) VR_CUDA(v, cudaMalloc(&v->d_pipe[i], (size_t)px * 16));
-        v->pipe_capacity_px = px;
-    }
+    const int rcp = ensure_pipe(v, px);
+    if (rcp) return rcp;
     cudaStream_t st = (cudaStream_t)stream;
     const int slot = (int)(v->pipe_frames & 1);
     /* the frame that last used this slot must have left it */
@@ -921,7 +1035,7 @@ extern "C" int vr_render_host_async(vr_volume* v, const float* view, const float
 extern "C" int vr_render_host_wait(vr_volume* v) {
     if (!v) return fail(NULL, VR_ERR_INVALID_ARG, "vr_render_host_wait: NULL handle");
     if (v->copy_stream) VR_CUDA(v, cudaStreamSynchronize(v->copy_stream));
-    return VR_OK;
+    return check_overflow(v, "vr_render_host_wait");
 }
 
 /* ------------------------------------------------------------------------------------------ */

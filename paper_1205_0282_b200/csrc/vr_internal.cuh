@@ -184,7 +184,8 @@ __host__ __device__ __forceinline__ unsigned vr_cell_offset(const VrGrid& g, int
 /* range: float2[nbricks + 1] (per brick, then the whole volume) or NULL = unknown, no culling */
 cudaError_t vr_launch_setup(const VrGrid& grid, const VrMatrices& mats, int W, int H, int mode,
                             long long sub_capacity_px, void* sub_base, VrViewState* vs, VrBrickView* bv, int* order,
-                            int* item_prefix, VrCompLayer* layers, const float2* range, const VrLut& lut, cudaStream_t st);
+                            int* item_prefix, VrCompLayer* layers, const float2* range, const VrLut& lut, int* overflow_flag,
+                            cudaStream_t st);
 /* texture arm of the brick store (vr_texture.cu): one 3-D CUDA array + texture object per slot */
 struct VrTexStore;
 cudaError_t vr_tex_create(const VrGrid& grid, VrTexStore** out);

@@ -44,7 +44,7 @@ __global__ void __launch_bounds__(SETUP_THREADS)
 vr_setup_kernel(VrGrid grid, VrMatrices mats, int W, int H, int mode, long long sub_capacity_px,
                 unsigned long long sub_base, VrViewState* __restrict__ vs, VrBrickView* __restrict__ bv,
                 int* __restrict__ order, int* __restrict__ item_prefix, VrCompLayer* __restrict__ layers,
-                const float2* __restrict__ range, VrLut lut) {
+                const float2* __restrict__ range, VrLut lut, int* __restrict__ overflow_flag) {
     __shared__ SetupShared sh;
     const int tid = threadIdx.x;
     const bool small = grid.nbricks <= SETUP_THREADS;
@@ -270,6 +270,7 @@ vr_setup_kernel(VrGrid grid, VrMatrices mats, int W, int H, int mode, long long 
         vs->total_items = over ? 0 : sh.carry_items;
         vs->total_sub_pixels = sh.carry_pix;
         vs->overflow = over;
+        if (over && overflow_flag) *overflow_flag = 1; /* mapped host memory: the host sees it without a copy */
         vs->culled = sh.culled;
         const bool none = sh.bound[2] <= sh.bound[0] || sh.bound[3] <= sh.bound[1];
         for (int i = 0; i < 4; ++i) vs->bound[i] = none ? 0 : sh.bound[i];
@@ -294,10 +295,10 @@ vr_setup_kernel(VrGrid grid, VrMatrices mats, int W, int H, int mode, long long 
 
 cudaError_t vr_launch_setup(const VrGrid& grid, const VrMatrices& mats, int W, int H, int mode, long long sub_capacity_px,
                             void* sub_base, VrViewState* vs, VrBrickView* bv, int* order, int* item_prefix,
-                            VrCompLayer* layers, const float2* range, const VrLut& lut, cudaStream_t st) {
+                            VrCompLayer* layers, const float2* range, const VrLut& lut, int* overflow_flag, cudaStream_t st) {
     vr_setup_kernel<<<1, SETUP_THREADS, 0, st>>>(grid, mats, W, H, mode, sub_capacity_px,
                                                  (unsigned long long)(uintptr_t)sub_base, vs, bv, order, item_prefix, layers,
-                                                 range, lut);
+                                                 range, lut, overflow_flag);
     return cudaGetLastError();
 }
 

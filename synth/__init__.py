@@ -289,11 +289,14 @@ CONFIGS = {
     "c3": dict(nx=4096, ny=4096, nz=1536, brick=512, ghost=1, nsrc=50000, ramp=0.0, width=1920, height=1080, step=1.0),
     # row f4 (not a BASELINE.json config): the paper's other data family (Table 1 "Nbody" 1024^3, "scaled Nbody"
     # 2600^3): a 2048^3 density cube (34 GB), zero except for 200 extended halos, in 512 bricks of 256^3
+    # not a BASELINE.json config: config 3 at half scale (the same voxels-per-pixel ratio, bricks of 256^3: 8x8x3 grid, 26 GB),
+    # small enough for the texture arm's second copy of the bricks - the sparse-sampling regime for BOTH samplers
+    "s3": dict(nx=2048, ny=2048, nz=768, brick=256, ghost=1, nsrc=6250, ramp=0.0, width=960, height=540, step=1.0),
     "n1": dict(nx=2048, ny=2048, nz=2048, brick=256, ghost=1, nsrc=200, ramp=0.0, width=1920, height=1080, step=0.5, kind=1),
 }
 
 
 def config_cube(name):
     c = CONFIGS[name]
-    k = int(name[1:]) + (10 if name[0] == "n" else 0)
+    k = int(name[1:]) + {"n": 10, "s": 20}.get(name[0], 0)
     return Cube(BASE_SEED + k, c["nx"], c["ny"], c["nz"], c["nsrc"], c["ramp"], c.get("kind", 0))

@@ -830,8 +830,82 @@ def test_errors(vr):
         g.set_transfer_function(synth.tf_ramp(), 1.0, 1.0)
     with pytest.raises(vr.VrError):
         g.upload(np.zeros((4, 4, 4), dtype=np.float32), origin=(14, 0, 0))
+    bad = synth.tf_ramp()
+    bad[7, 3] = 1.5   # an opacity outside [0,1] would turn log2(1 - a) into NaN: refused, on both sides
+    with pytest.raises(vr.VrError) as e:
+        g.set_transfer_function(bad, -3, 10)
+    assert e.value.status == 1 and "alpha" in str(e.value)
+    with pytest.raises(ValueError):
+        oracle.Volume(16, 16, 16, 8, 1).set_transfer_function(bad, -3, 10)
+    with pytest.raises(ValueError):   # the binding's own argument checks raise (they are not asserts)
+        g.render(I, I, 8, 8, 0.5, vr.ALPHA, torch.empty((4, 4, 4), dtype=torch.float32, device="cuda"))
     g.render(I, I, 8, 8, 0.5, vr.ALPHA, out)  # still usable after errors
     torch.cuda.synchronize()
+
+
+def test_environment_knobs_are_validated(vr, monkeypatch):
+    monkeypatch.setenv("VR_TILE", "9,9,9")
+    with pytest.raises(vr.VrError) as e:
+        vr.Volume(16, 16, 16, 8, 1)
+    assert e.value.status == 1 and "VR_TILE" in str(e.value)
+    monkeypatch.setenv("VR_TILE", "3,3,3,0,0,0")   # 512 cells: not one 128-byte line
+    with pytest.raises(vr.VrError):
+        vr.Volume(16, 16, 16, 8, 1)
+    monkeypatch.delenv("VR_TILE")
+    monkeypatch.setenv("VR_LAYOUT", "tiled")
+    with pytest.raises(vr.VrError) as e:
+        vr.Volume(16, 16, 16, 8, 1)
+    assert "VR_LAYOUT" in str(e.value)
+
+
+def test_reserved_views_render_without_allocating_and_torch_allocator(vr):
+    """vr_reserve_views sizes every per-view buffer up front (vr_render then never allocates: the device's free memory
+    does not move); a view that was not announced and needs more scratch still renders. With vr_set_allocator the
+    library's buffers come out of torch's caching allocator (north_star: PyTorch for device memory)."""
+    import torch
+    cube = synth.Cube(41, 96, 80, 64, 6)
+    data = cube.fill_host()
+    W, H = 320, 200
+    fr = synth.Framing(cube.nx, cube.ny, cube.nz, W, H)
+    views = [fr.turntable(k) for k in range(0, 36, 3)]
+    projs = [fr.proj(False)] * len(views)
+    torch.cuda.synchronize()
+    before = torch.cuda.memory_allocated()
+    vr.use_torch_allocator(True)
+    try:
+        g = vr.Volume(cube.nx, cube.ny, cube.nz, 32, 1)
+    finally:
+        vr.use_torch_allocator(False)
+    held = torch.cuda.memory_allocated() - before
+    assert held >= 27 * 36 * 36 * 34 * 4  # at least the brick store (27 slots of 9x9x17 micro-tiles) is torch's
+    o = oracle.Volume(cube.nx, cube.ny, cube.nz, 32, 1, data=data)
+    g.upload(torch.from_numpy(data).cuda())
+    for v in (g, o):
+        v.set_transfer_function(synth.tf_ramp(), synth.TF_VMIN, synth.TF_VMAX)
+    g.reserve_views(views, projs, W, H)
+    host = torch.empty((H, W, 4), dtype=torch.float32).pin_memory()
+    out = torch.empty((H, W, 4), dtype=torch.float32, device="cuda")
+    torch.cuda.synchronize()
+    free0, _ = torch.cuda.mem_get_info()
+    alloc0 = torch.cuda.memory_allocated()
+    for view in views:
+        g.render(view, projs[0], W, H, 0.5, vr.ALPHA, out)
+        g.render(view, projs[0], W, H, 0.5, vr.MIP, out)
+        g.render_host_async(view, projs[0], W, H, 0.5, vr.ALPHA, host)
+    g.render_host_wait()
+    g.render_host(views[0], projs[0], W, H, 0.5, vr.ALPHA, host.numpy())
+    torch.cuda.synchronize()
+    assert torch.cuda.mem_get_info()[0] == free0 and torch.cuda.memory_allocated() == alloc0
+    ref = o.render(views[0], projs[0], W, H, 0.5, oracle.ALPHA)
+    check_alpha(host.numpy().astype(np.float64), ref, 0.99, "reserved views")
+    # an unannounced, much closer view needs more sub-image scratch: it grows (and renders correctly)
+    close = synth.look_at((cube.nx * 0.5, cube.ny * 0.5, cube.nz * 1.2), (cube.nx * 0.5, cube.ny * 0.5, 0.0), (0, 1, 0))
+    wide = synth.perspective(100.0, W / H, 0.5, 500.0)
+    img = gpu_frame(g, close, wide, W, H, 0.5, vr.ALPHA)
+    check_alpha(img, o.render(close, wide, W, H, 0.5, oracle.ALPHA), 0.99, "unannounced view")
+    g.close()
+    torch.cuda.synchronize()
+    assert torch.cuda.memory_allocated() - before < held  # the handle's buffers went back to torch
 
 
 # --------------------------------------------------------------------------- a9 stand-alone
