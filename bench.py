@@ -200,7 +200,7 @@ def build_part(vr, wl, cube, tf, box):
 def sortlast_report(vr, g, wl, cube, tf, nparts, order, K, Wm):
     """Row f3 measured on ONE GPU, the parts one after the other (no rank waits for another): each part of the k-d
     partition is created, filled with its region (bricks + ghost layers) and renders the K frames of the cycle as
-    partial frames (vr_render_part), one CUDA-event pair per frame; then the N partial frames of one view are merged
+    partial frames packed by rectangle (vr_render_part_pieces), stage events per frame; then the N pieces of one view are merged
     (vr_composite_parts, the work the N ranks share by stripes). The exchange itself needs N GPUs: its volume is
     reported from the geometry (the paper's M + epsilon), not timed."""
     import torch
@@ -216,20 +216,28 @@ def sortlast_report(vr, g, wl, cube, tf, nparts, order, K, Wm):
     for r, box in enumerate(boxes):
         p = build_part(vr, wl, cube, tf, box)
         p.minmax()
+        # what a rank does per frame: set-up, ray table, ray cast, and stage-1 compositing straight into the
+        # rectangle-packed piece it sends (vr_render_part_pieces; here one piece = the part's whole rectangle)
+        def part_frame(vi):
+            rc = vr.part_rect(dims, wl["brick"], box, wl["views"][vi], wl["proj"], Wp, Hp)
+            piece = out.view(-1)[:(rc[3] - rc[1]) * (rc[2] - rc[0]) * 4].view(rc[3] - rc[1], rc[2] - rc[0], 4)
+            p.render_part_pieces(wl["views"][vi], wl["proj"], Wp, Hp, wl["step"], 0, [rc], [piece])
+            return rc, piece
+
         for k in range(Wm):
-            p.render_part(wl["views"][order[k % len(order)]], wl["proj"], Wp, Hp, wl["step"], 0, out)
-        p.set_timing(1)  # the library's own stage events: device time of each frame's three kernels, no host gaps
+            part_frame(order[k % len(order)])
+        p.set_timing(1)  # the library's own stage events: device time of each frame's kernels, no host gaps
         torch.cuda.synchronize()
         for k in range(K):
-            p.render_part(wl["views"][order[(Wm + k) % len(order)]], wl["proj"], Wp, Hp, wl["step"], 0, out)
+            part_frame(order[(Wm + k) % len(order)])
         torch.cuda.synchronize()
         stg = p.debug_stage_times(K)
         frame_ms[r] = stg.sum(axis=1)
         ray_ms.append(round(float(stg[:, 1].mean()), 4))
         p.set_timing(0)
-        rc = p.render_part(view0, wl["proj"], Wp, Hp, wl["step"], 0, out)
+        rc, piece = part_frame(order[Wm % len(order)])
         torch.cuda.synchronize()
-        pieces.append(out[rc[1]:rc[3], rc[0]:rc[2]].contiguous())
+        pieces.append(piece.clone())
         rects.append(rc)
         nb = int(np.prod([box[1][a] - box[0][a] for a in range(3)]))
         store_gb.append(round(nb * (wl["brick"] + 2 * wl["ghost"]) ** 3 * 4 / 1e9, 2))
@@ -268,8 +276,8 @@ def run_bricks_sharded(args, vr, wl, tf, mode_id, rank, world, local_rank, dist,
     """`--sharding bricks` (row f3): ONE cube over all ranks, every frame rendered by all of them (sort-last,
     paper_1205_0282_b200.sortlast). Strong scaling: the cube and the frames are fixed as N grows. Each rank fills
     only its own region (bricks + ghost layers) from the device generator. Timed like the frame-sharded arm:
-    barrier + synchronise on both sides, CUDA events, maximum over ranks. Not the default: north_star's bench line
-    is the one-GPU cube; every run of round 1 had one GPU, where this arm is the world of one."""
+    barrier + synchronise on both sides, CUDA events, maximum over ranks. The default on N > 1 ranks (north_star's bench
+    line is the one-GPU cube; on one GPU this arm is the world of one and has to be asked for)."""
     import torch
     from paper_1205_0282_b200 import sortlast
     dims = (wl["nx"], wl["ny"], wl["nz"])
@@ -324,7 +332,7 @@ def run_bricks_sharded(args, vr, wl, tf, mode_id, rank, world, local_rank, dist,
     if dist is not None:
         dist.barrier()
     e2e_ms = reduce_max((time.perf_counter() - t0) * 1e3)
-    moved = int(np.mean([rdr.exchange_bytes(wl["views"][(Wm + k) % nv], wl["proj"], W, H) for k in range(K)]))
+    moved = int(np.mean([rdr.exchange_bytes(wl["views"][(Wm + k) % nv], wl["proj"], W, H, mode_id) for k in range(K)]))
     cfg = config_of(wl, args)
     cfg["sharding"] = "bricks: k-d partition into %d parts (row f3), one cube over all ranks, sort-last exchange" % world
     return {"metric": METRIC, "value": round(K / (ms * 1e-3), 3), "unit": "frames/s", "n_gpus": world, "steps": K, "warmup": Wm,
@@ -733,9 +741,11 @@ def main():
     ap.add_argument("--cells-every", type=int, default=6, help="count distinct cells on every n-th view of the cycle (0 = never)")
     ap.add_argument("--c4-part", default="both", choices=["both", "composite"],
                     help="--workload c4: `composite` runs only the compositing microbenchmark (profiling)")
-    ap.add_argument("--sharding", default="frames", choices=["frames", "bricks"],
-                    help="N > 1: frames = every rank holds the cube and renders its own frames (default, weak scaling); "
-                         "bricks = one cube over all ranks, sort-last (row f3, strong scaling)")
+    ap.add_argument("--sharding", default="auto", choices=["auto", "frames", "bricks"],
+                    help="bricks = ONE cube over all ranks, sort-last with a rectangle-packed exchange (the paper's design, "
+                         "PAPER.md:136, :178-184; row f3; strong scaling); frames = every rank holds the whole cube and renders its "
+                         "own frames (replicas, weak scaling). auto (default): bricks when launched on N > 1 ranks - with the "
+                         "replica figure beside it as `replicas` - and the one-GPU line otherwise")
     ap.add_argument("--sortlast-parts", type=int, default=8,
                     help="row f3 report: parts of the k-d partition rendered one after the other on this GPU (0 = skip)")
     ap.add_argument("--sampler", default="manual", choices=["manual", "texture"],
@@ -768,6 +778,7 @@ def main():
     dist = None
     if world > 1:
         import torch.distributed as dist
+        os.environ.setdefault("NCCL_DEBUG", "INFO")  # the communicator's own log (rings / NVLS, transports) goes to stderr
         dist.init_process_group(backend="nccl", device_id=torch.device("cuda", local_rank))
 
     from paper_1205_0282_b200 import build as vr_build
@@ -797,8 +808,24 @@ def main():
         print(json.dumps(run_c4(args, vr, peak, peak_src, ClockSampler(local_rank))), flush=True)
         return 0
 
+    if args.sharding == "auto":
+        args.sharding = "bricks" if world > 1 else "frames"
+        auto = True
+    else:
+        auto = False
     if args.sharding == "bricks":
         line = run_bricks_sharded(args, vr, wl, tf, mode_id, rank, world, local_rank, dist, reduce_max)
+        if auto and world > 1:  # beside it: N replicas of the whole cube, each rendering its own frames
+            torch.cuda.empty_cache()
+            g, _ = build_volume(vr, wl, tf)
+            out = torch.empty((wl["height"], wl["width"], 4), dtype=torch.float32, device="cuda")
+            order = views_for_rank(rank, world, len(wl["views"]))
+            ms = timed_device(g, wl, mode_id, order, args.steps, args.warmup, out, dist)[0]
+            fps, ms_max = aggregate(ms, args.steps, world, reduce_max)
+            g.close()
+            line["replicas"] = {"value": round(fps, 3), "unit": "frames/s", "scaling": "weak", "ms_per_step": round(ms_max / args.steps, 4),
+                                "what": "every rank holds the whole cube and renders its own frames of the cycle; no data-path "
+                                        "collective; all ranks' frames over the slowest rank's device time"}
         if rank == 0:
             print(json.dumps(line), flush=True)
         if dist is not None:

@@ -321,7 +321,7 @@ int vr_composite(const float* const* layers, const int* rects, const int* order,
  * sample positions, the owner rule and the visibility order are those of the whole volume, so
  * the sub-images of a part's bricks are bit-identical to the ones a single handle renders.
  * libvr moves no data between GPUs: the exchange is the caller's (paper_1205_0282_b200.sortlast
- * uses torch.distributed), the kernels on both sides of it are these.
+ * uses torch.distributed), the partition, the part order, the rectangles and the kernels on both sides of it are these.
  *
  * vr_volume_create_part: b0, b1 (host, int[3]): the part holds bricks b0 <= (bx,by,bz) < b1
  *   (brick (bx,by,bz) = voxels [bx*brick, min((bx+1)*brick, n)) per axis). Memory: the box's
@@ -331,20 +331,37 @@ int vr_composite(const float* const* layers, const int* rects, const int* order,
  *   vr_debug_brick_data accept the part's own bricks only; vr_volume_minmax gives the range of
  *   the part's voxels (ghost layers included) - reduce it over the parts for the global range;
  *   table entries of bricks held elsewhere are (+inf, -inf).
- * vr_render_part: one frame of the part's bricks only, full-frame [height][width][4]:
- *   VR_ALPHA  premultiplied RGBA of the part's sub-images composited in visibility order (what
- *             vr_render gives on a part handle);
- *   VR_MIP    (m, 0, 0, 1) with m the raw maximum over the part's samples, (0,0,0,0) for a ray
- *             that takes no sample in the part (needs VR_SORT_LAST, else VR_ERR_STATE);
+ * vr_kd_partition: the data partition (sec. 2.3.1: k-d trees; host arithmetic, no handle, no device).
+ *   The brick grid is cut across its longest axis (in voxels, ties to the lower axis) at the brick face nearest to
+ *   the wanted share (ties to even), at least one brick per side, until there are nparts boxes: nparts = 2^k gives
+ *   one balanced tree, other counts a chain of balanced trees, one per set bit of nparts from the largest down,
+ *   whose roots share the box in proportion to their leaf counts (6 = 4 + 2).
+ *   boxes_out (host, int[nparts*6]): part r holds bricks (b0x,b0y,b0z) <= b < (b1x,b1y,b1z), low side first.
+ *   tree_out (host, int[(2*nparts-1)*4]): node 0 = root, pre-order; an inner node is (axis, cut in bricks, low child,
+ *   high child), a leaf (-1, part, 0, 0). Errors: VR_ERR_INVALID_ARG (more parts than the grid can be cut into).
+ * vr_part_order: the parts front to back for a view (`over` needs a visibility order): at every node
+ *   the side of the cut plane that holds the eye first (orthographic: the side the view direction leaves first);
+ *   the eye is R9's homogeneous eye from the library's own inverse of proj*view. order_out (host, int[nparts]).
+ * vr_render_part: one frame of the part's bricks only, the full frame:
+ *   VR_ALPHA  [height][width][4]: premultiplied RGBA of the part's sub-images composited in visibility order
+ *             (what vr_render gives on a part handle);
+ *   VR_MIP    [height][width]: ONE float per pixel as in the paper (a 1024^2 sub-frame is 4 MB) - the
+ *             raw maximum over the part's samples, -inf for a ray that takes no sample in the part (needs
+ *             VR_SORT_LAST, else VR_ERR_STATE);
  *   rect_out (host, int[4], may be NULL): (x0,y0,x1,y1), half-open: a rectangle that contains
  *   every non-blank pixel of the partial frame (union of the bricks' rendering rectangles with
  *   a pixel of slack; PAPER.md:184 packs messages by it); all zero if nothing is on screen.
+ * vr_render_part_pieces: the same partial frame, composited (stage 1) straight into `npieces`
+ *   rectangle-packed pieces instead of a full frame - what a rank sends: piece q covers piece_rects[q] =
+ *   (x0,y0,x1,y1) inside the frame (host int[npieces*4]) and is stored [y1-y0][x1-x0][4] (VR_ALPHA) or [y1-y0][x1-x0]
+ *   (VR_MIP) at pieces[q] (host array of npieces DEVICE pointers). Only those pixels are written: nothing else of the
+ *   frame is touched or cleared. Needs VR_SORT_LAST.
  * vr_part_rect: the same rectangle from the geometry alone (host arithmetic, no handle, no
  *   device), so that every process can size the pieces it will receive without a message.
  * vr_composite_parts: merges partial frames. parts/rects/order/n/out as vr_composite (piece l
- *   covers rects[l], stored [y1-y0][x1-x0][4]); order = the parts front to back (any order for
- *   VR_MIP). VR_ALPHA: front-to-back `over` (identical to vr_composite). VR_MIP: maximum of
- *   the x components of the pieces whose w is non-zero, then the colour mapping with v's
+ *   covers rects[l]); order = the parts front to back (any order for VR_MIP). VR_ALPHA: pieces
+ *   stored [y1-y0][x1-x0][4], front-to-back `over` (identical to vr_composite). VR_MIP: scalar
+ *   pieces stored [y1-y0][x1-x0] (-inf = no sample): their maximum, then the colour mapping with v's
  *   transfer function, (0,0,0,0) where no piece holds a sample.
  *   `over` is associative: merging the parts' frames in part order equals
  *   compositing all sub-images in brick order up to float32 rounding, provided the part order
@@ -353,8 +370,14 @@ int vr_volume_create_part(int nx, int ny, int nz, int brick, int ghost, const in
                           const int* b1, vr_volume** out);
 int vr_render_part(vr_volume* v, const float* view, const float* proj, int width, int height,
                    float step, int mode, float* out_part, int* rect_out, void* stream);
+int vr_render_part_pieces(vr_volume* v, const float* view, const float* proj, int width, int height,
+                          float step, int mode, const int* piece_rects, float* const* pieces, int npieces,
+                          void* stream);
 int vr_part_rect(int nx, int ny, int nz, int brick, const int* b0, const int* b1,
                  const float* view, const float* proj, int width, int height, int* rect_out);
+int vr_kd_partition(int nx, int ny, int nz, int brick, int nparts, int* boxes_out, int* tree_out);
+int vr_part_order(const int* tree, int nparts, int brick, const float* view, const float* proj,
+                  int* order_out);
 int vr_composite_parts(vr_volume* v, int mode, const float* const* parts, const int* rects,
                        const int* order, int n, int width, int height, float* out, void* stream);
 

@@ -30,7 +30,7 @@ SYMBOLS = (
     "vr_volume_create", "vr_volume_create_layout", "vr_volume_destroy", "vr_volume_upload", "vr_volume_download", "vr_debug_brick_data",
     "vr_set_transfer_function", "vr_set_early_termination", "vr_volume_minmax", "vr_set_culling", "vr_set_traversal", "vr_set_sampler", "vr_set_allocator", "vr_reserve_views", "vr_debug_brick_minmax", "vr_debug_cell_flags", "vr_render", "vr_render_host", "vr_render_host_async", "vr_render_host_wait", "vr_composite",
     "vr_num_bricks", "vr_debug_brick_order", "vr_debug_rects", "vr_debug_ray_bricks", "vr_debug_subimages",
-    "vr_volume_create_part", "vr_render_part", "vr_part_rect", "vr_composite_parts",
+    "vr_volume_create_part", "vr_render_part", "vr_render_part_pieces", "vr_part_rect", "vr_composite_parts", "vr_kd_partition", "vr_part_order",
     "vr_set_counting", "vr_set_timing", "vr_debug_stats", "vr_debug_stage_times", "vr_debug_probe_dram", "vr_launch_count", "vr_last_error",
 )
 
@@ -87,6 +87,9 @@ def lib():
         L.vr_volume_create_part.argtypes = [ci, ci, ci, ci, ci, vp, vp, ctypes.POINTER(vp)]
         L.vr_render_part.argtypes = [vp, vp, vp, ci, ci, cf, ci, vp, vp, vp]
         L.vr_part_rect.argtypes = [ci, ci, ci, ci, vp, vp, vp, vp, ci, ci, vp]
+        L.vr_render_part_pieces.argtypes = [vp, vp, vp, ci, ci, cf, ci, vp, vp, ci, vp]
+        L.vr_kd_partition.argtypes = [ci, ci, ci, ci, ci, vp, vp]
+        L.vr_part_order.argtypes = [vp, ci, ci, vp, vp, vp]
         L.vr_composite_parts.argtypes = [vp, ci, vp, vp, vp, ci, ci, ci, vp, vp]
         L.vr_num_bricks.argtypes = [vp]
         L.vr_debug_brick_order.argtypes = [vp, vp, vp, vp]
@@ -289,13 +292,32 @@ class Volume:
 
     def render_part(self, view, proj, width, height, step, mode, out, stream=None):
         """This handle's contribution to a sort-last frame (vr_render_part). out: CUDA float32 tensor
-        [height][width][4]; returns the rectangle (x0,y0,x1,y1) outside which out is blank."""
-        _require(out.is_cuda and out.is_contiguous() and out.element_size() == 4 and out.numel() == width * height * 4, 'out.is_cuda and out.is_contiguous() and out.element_size() == 4 and out.numel() == width * height * 4')
+        [height][width][4] (ALPHA) or [height][width] (MIP: the raw maximum, -inf without a sample; a [height][width][4]
+        tensor is accepted and its first width*height floats are written); returns the rectangle (x0,y0,x1,y1) outside
+        which the partial frame is blank."""
+        _require(out.is_cuda and out.is_contiguous() and out.element_size() == 4, "out: a contiguous float32 CUDA tensor")
+        _require(out.numel() == width * height * 4 or (mode == MIP and out.numel() == width * height), "out: width*height*4 floats (MIP: or width*height)")
         v, p = _mat(view), _mat(proj)
         rect = np.zeros(4, dtype=np.int32)
         self._check(lib().vr_render_part(self._h, v.ctypes.data, p.ctypes.data, int(width), int(height), float(step), int(mode),
                                          out.data_ptr(), rect.ctypes.data, _stream(stream)))
         return tuple(int(c) for c in rect)
+
+    def render_part_pieces(self, view, proj, width, height, step, mode, rects, pieces, stream=None):
+        """vr_render_part_pieces: the handle's partial frame, composited straight into rectangle-packed pieces. rects:
+        n x (x0,y0,x1,y1) inside the frame; pieces: n CUDA float32 tensors, piece q holding rects[q] as
+        [y1-y0][x1-x0][4] (ALPHA) or [y1-y0][x1-x0] (MIP: raw maximum, -inf without a sample)."""
+        n = len(pieces)
+        r = np.ascontiguousarray(rects, dtype=np.int32).reshape(n, 4)
+        per = 4 if mode == ALPHA else 1
+        for t, rc_ in zip(pieces, r):
+            _require(t.is_cuda and t.is_contiguous() and t.element_size() == 4, "pieces: contiguous float32 CUDA tensors")
+            _require(t.numel() == (rc_[2] - rc_[0]) * (rc_[3] - rc_[1]) * per, "piece size does not match its rectangle and the mode")
+        ptrs = (ctypes.c_void_p * max(n, 1))(*[t.data_ptr() for t in pieces])
+        v, p = _mat(view), _mat(proj)
+        self._check(lib().vr_render_part_pieces(self._h, v.ctypes.data, p.ctypes.data, int(width), int(height), float(step), int(mode),
+                                                r.ctypes.data, ptrs, n, _stream(stream)))
+        return pieces
 
     def composite_parts(self, mode, parts, rects, order, width, height, out, stream=None):
         """Merge partial frames (vr_composite_parts). parts: CUDA float32 tensors [y1-y0][x1-x0][4], piece l
@@ -304,9 +326,10 @@ class Volume:
         ptrs = (ctypes.c_void_p * max(n, 1))(*[l.data_ptr() for l in parts])
         r = np.ascontiguousarray(rects, dtype=np.int32).reshape(n, 4)
         o = np.ascontiguousarray(order, dtype=np.int32).reshape(n)
+        per = 4 if mode == ALPHA else 1  # MIP pieces are scalar (one float per pixel)
         for l, rc_ in zip(parts, r):
             _require(l.is_cuda and l.is_contiguous() and l.element_size() == 4, 'l.is_cuda and l.is_contiguous() and l.element_size() == 4')
-            _require(l.numel() == (rc_[2] - rc_[0]) * (rc_[3] - rc_[1]) * 4, 'l.numel() == (rc_[2] - rc_[0]) * (rc_[3] - rc_[1]) * 4')
+            _require(l.numel() == (rc_[2] - rc_[0]) * (rc_[3] - rc_[1]) * per, "piece size does not match its rectangle and the mode")
         _require(out.is_cuda and out.is_contiguous() and out.numel() == width * height * 4, 'out.is_cuda and out.is_contiguous() and out.numel() == width * height * 4')
         self._check(lib().vr_composite_parts(self._h, int(mode), ptrs, r.ctypes.data, o.ctypes.data, n, int(width), int(height),
                                              out.data_ptr(), _stream(stream)))
@@ -425,6 +448,30 @@ def debug_probe_dram(buf, flavour, span_bytes=128, group=1, loads_per_thread=256
     if rc != 0:
         raise VrError(rc, "vr_debug_probe_dram failed")
     return float(ms.value), int(loads.value)
+
+
+def kd_partition(dims, brick, nparts):
+    """vr_kd_partition (PAPER.md:138): (boxes, tree) - boxes[r] = (b0, b1), the half-open box of bricks of part r;
+    tree: int32 [(2 nparts - 1)][4] in libvr's encoding, for part_order. Host only."""
+    nparts = int(nparts)
+    boxes = np.zeros((max(nparts, 1), 6), dtype=np.int32)
+    tree = np.zeros((max(2 * nparts - 1, 1), 4), dtype=np.int32)
+    rc = lib().vr_kd_partition(int(dims[0]), int(dims[1]), int(dims[2]), int(brick), nparts, boxes.ctypes.data, tree.ctypes.data)
+    if rc != 0:
+        raise VrError(rc, lib().vr_last_error(None).decode())
+    return [(tuple(int(c) for c in b[:3]), tuple(int(c) for c in b[3:])) for b in boxes], tree
+
+
+def part_order(tree, brick, view, proj):
+    """vr_part_order: the parts of a k-d partition front to back for this view. Host only."""
+    t = np.ascontiguousarray(tree, dtype=np.int32).reshape(-1, 4)
+    nparts = (t.shape[0] + 1) // 2
+    v, p = _mat(view), _mat(proj)
+    out = np.zeros(nparts, dtype=np.int32)
+    rc = lib().vr_part_order(t.ctypes.data, nparts, int(brick), v.ctypes.data, p.ctypes.data, out.ctypes.data)
+    if rc != 0:
+        raise VrError(rc, lib().vr_last_error(None).decode())
+    return [int(r) for r in out]
 
 
 def composite(layers, rects, order, width, height, out, stream=None):

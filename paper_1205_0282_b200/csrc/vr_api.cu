@@ -836,21 +836,45 @@ extern "C" int vr_debug_brick_minmax(vr_volume* v, float* mm_out) {
     return VR_OK;
 }
 
+/* pieces: the frame leaves as n windows (x0, y0, x1, y1), window q stored [y1-y0][x1-x0] at ptrs[q] (row f3) */
+struct VrPieces {
+    int n;
+    const int* rects;
+    float* const* ptrs;
+};
+
 static int render_frame(vr_volume* v, const float* view, const float* proj, int width, int height, float step, int mode,
-                        float* out_rgba, void* stream, bool partial);
+                        float* out_rgba, void* stream, bool partial, const VrPieces* pieces);
 
 extern "C" int vr_render(vr_volume* v, const float* view, const float* proj, int width, int height, float step, int mode,
                          float* out_rgba, void* stream) {
-    return render_frame(v, view, proj, width, height, step, mode, out_rgba, stream, false);
+    return render_frame(v, view, proj, width, height, step, mode, out_rgba, stream, false, NULL);
 }
 
 extern "C" int vr_render_part(vr_volume* v, const float* view, const float* proj, int width, int height, float step, int mode,
                               float* out_part, int* rect_out, void* stream) {
-    const int rc = render_frame(v, view, proj, width, height, step, mode, out_part, stream, true);
+    const int rc = render_frame(v, view, proj, width, height, step, mode, out_part, stream, true, NULL);
     if (rc) return rc;
     if (rect_out && vr_host_part_rect(v->grid, view, proj, width, height, rect_out))
         return fail(v, VR_ERR_INVALID_ARG, "vr_render_part: proj*view is singular");
     return VR_OK;
+}
+
+extern "C" int vr_render_part_pieces(vr_volume* v, const float* view, const float* proj, int width, int height, float step,
+                                     int mode, const int* piece_rects, float* const* pieces, int npieces, void* stream) {
+    if (!v) return fail(NULL, VR_ERR_INVALID_ARG, "vr_render_part_pieces: NULL handle");
+    if (npieces < 0 || npieces > 4096 || (npieces > 0 && (!piece_rects || !pieces)))
+        return fail(v, VR_ERR_INVALID_ARG, "vr_render_part_pieces: bad piece list");
+    if (v->traversal != VR_SORT_LAST) return fail(v, VR_ERR_STATE, "vr_render_part_pieces: needs the VR_SORT_LAST traversal");
+    for (int q = 0; q < npieces; ++q) {
+        const int* r = piece_rects + 4 * q;
+        if (r[0] < 0 || r[1] < 0 || r[2] > width || r[3] > height || r[2] < r[0] || r[3] < r[1])
+            return fail(v, VR_ERR_INVALID_ARG, "vr_render_part_pieces: piece %d leaves the %dx%d frame", q, width, height);
+        if (!pieces[q] && r[2] > r[0] && r[3] > r[1]) return fail(v, VR_ERR_INVALID_ARG, "vr_render_part_pieces: piece %d is NULL", q);
+    }
+    const VrPieces pc = {npieces, piece_rects, pieces};
+    float dummy; /* render_frame wants a non-NULL output; with pieces it is not written */
+    return render_frame(v, view, proj, width, height, step, mode, &dummy, stream, true, &pc);
 }
 
 extern "C" int vr_part_rect(int nx, int ny, int nz, int brick, const int* b0, const int* b1, const float* view, const float* proj,
@@ -876,9 +900,30 @@ extern "C" int vr_part_rect(int nx, int ny, int nz, int brick, const int* b0, co
     return VR_OK;
 }
 
+extern "C" int vr_kd_partition(int nx, int ny, int nz, int brick, int nparts, int* boxes_out, int* tree_out) {
+    if (!boxes_out || !tree_out) return fail(NULL, VR_ERR_INVALID_ARG, "vr_kd_partition: NULL output");
+    if (nx <= 0 || ny <= 0 || nz <= 0 || brick < 2) return fail(NULL, VR_ERR_INVALID_ARG, "vr_kd_partition: bad volume or brick size");
+    long long nb = 1;
+    for (int a = 0; a < 3; ++a) nb *= ((a == 0 ? nx : a == 1 ? ny : nz) + brick - 1) / brick;
+    if (nparts < 1 || nparts > nb || nb > 65535)
+        return fail(NULL, VR_ERR_INVALID_ARG, "vr_kd_partition: %d parts for %lld bricks", nparts, nb);
+    if (vr_host_kd_partition(nx, ny, nz, brick, nparts, boxes_out, tree_out))
+        return fail(NULL, VR_ERR_INVALID_ARG, "vr_kd_partition: the brick grid cannot be cut into %d boxes this way", nparts);
+    return VR_OK;
+}
+
+extern "C" int vr_part_order(const int* tree, int nparts, int brick, const float* view, const float* proj, int* order_out) {
+    if (!tree || !view || !proj || !order_out || nparts < 1 || brick < 2)
+        return fail(NULL, VR_ERR_INVALID_ARG, "vr_part_order: NULL or bad argument");
+    const int rc = vr_host_part_order(tree, nparts, brick, view, proj, order_out);
+    if (rc == 1) return fail(NULL, VR_ERR_INVALID_ARG, "vr_part_order: proj*view is singular");
+    if (rc) return fail(NULL, VR_ERR_INVALID_ARG, "vr_part_order: malformed tree");
+    return VR_OK;
+}
+
 /* partial: the frame is one part's contribution to a sort-last frame (row f3): a MIP frame stays scalar */
 static int render_frame(vr_volume* v, const float* view, const float* proj, int width, int height, float step, int mode,
-                        float* out_rgba, void* stream, bool partial) {
+                        float* out_rgba, void* stream, bool partial, const VrPieces* pieces) {
     long long sub_px = 0, items = 0;
     int rc = check_view(v, "vr_render", view, proj, width, height, &sub_px, &items);
     if (rc) return rc;
@@ -968,9 +1013,20 @@ static int render_frame(vr_volume* v, const float* view, const float* proj, int 
         VR_CUDA(v, vr_launch_raycast(p, items, v->counting != 0, sparse, st));
         v->launches++;
         if (timing) VR_CUDA(v, cudaEventRecord(ev[2], st));
-        VR_CUDA(v, vr_launch_composite(v->d_layers, v->d_order, v->grid.nbricks, width, height,
-                                       (partial && mode == VR_MIP) ? VR_MIP_RAW : mode, v->lut, out_rgba, v->d_vs->bound, st));
-        v->launches++;
+        const int kmode = (partial && mode == VR_MIP) ? VR_MIP_RAW : mode;
+        if (!pieces) {
+            VR_CUDA(v, vr_launch_composite(v->d_layers, v->d_order, v->grid.nbricks, width, height, kmode, v->lut, out_rgba,
+                                           v->d_vs->bound, NULL, st));
+            v->launches++;
+        }
+        /* stage-1 compositing straight into the rectangle-packed pieces the part sends */
+        for (int q = 0; pieces && q < pieces->n; ++q) {
+            const int* r = pieces->rects + 4 * q;
+            if (r[2] <= r[0] || r[3] <= r[1]) continue;
+            VR_CUDA(v, vr_launch_composite(v->d_layers, v->d_order, v->grid.nbricks, width, height, kmode, v->lut, pieces->ptrs[q],
+                                           v->d_vs->bound, r, st));
+            v->launches++;
+        }
     }
     if (timing) {
         VR_CUDA(v, cudaEventRecord(ev[3], st));
@@ -1102,7 +1158,7 @@ static int composite_layers(const VrLut& lut, int kmode, const float* const* lay
         VR_CUDA(NULL, cudaMemcpyAsync(d_tab, tab, sizeof(VrCompLayer) * n, cudaMemcpyHostToDevice, st));
         VR_CUDA(NULL, cudaMemcpyAsync(d_order, order, sizeof(int) * n, cudaMemcpyHostToDevice, st));
     }
-    VR_CUDA(NULL, vr_launch_composite(d_tab, d_order, n, width, height, kmode, lut, out, NULL, st));
+    VR_CUDA(NULL, vr_launch_composite(d_tab, d_order, n, width, height, kmode, lut, out, NULL, NULL, st));
     VR_CUDA(NULL, cudaFreeAsync(d_tab, st));
     VR_CUDA(NULL, cudaFreeAsync(d_order, st));
     return VR_OK;

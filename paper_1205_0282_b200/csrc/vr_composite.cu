@@ -14,9 +14,11 @@
  * order-preserving), then each thread walks that short list for its pixel:
  *   ALPHA  C += (1-A) C_l,  A += (1-A) A_l      (float32, R15; no early termination)
  *   MIP    m = max(m, m_l); at the end RGB = LUT(u(m)), A = 1, or (0,0,0,0) if m = -inf (R11)
- * Row f3 (multi-GPU sort-last): a part's MIP frame leaves as the raw maximum
- * (VR_MIP_RAW: (m,0,0,1), or zeros without a sample), and the partial frames of the parts are merged
- * by the same kernel (ALPHA: `over` in part order; VR_MIP_PARTS: maximum, then the colour mapping).
+ * Row f3 (multi-GPU sort-last): a part's MIP frame leaves as the raw maximum, ONE float per
+ * pixel as in the paper (:180: 4 MB per 1024^2 sub-frame; VR_MIP_RAW: m, or -inf without a sample), and the
+ * partial frames of the parts are merged by the same kernel (ALPHA: `over` in part order; VR_MIP_PARTS: maximum
+ * of the scalar pieces, then the colour mapping). The output may be a WINDOW of the frame (a rectangle stored
+ * [h][w]): a part composites its sub-images straight into the rectangle-packed pieces it sends (:184).
  */
 #include "vr_internal.cuh"
 
@@ -36,14 +38,18 @@ struct CompEntry {
 
 template <int MODE>
 __global__ void __launch_bounds__(COMP_THREADS)
-vr_composite_kernel(const VrCompLayer* __restrict__ layers, const int* __restrict__ order, int n, int W, int H, VrLut lut,
-                    float4* __restrict__ out, const int* __restrict__ bound) {
+vr_composite_kernel(const VrCompLayer* __restrict__ layers, const int* __restrict__ order, int n, int4 win, VrLut lut,
+                    void* __restrict__ out_, const int* __restrict__ bound) {
+    /* win = (x0, y0, x1, y1): the pixels of the frame this launch writes, stored [y1-y0][x1-x0] at out_ */
+    const int W = win.z, H = win.w, WP = win.z - win.x;
     __shared__ CompEntry s_list[COMP_LIST];
     __shared__ int s_warp_cnt[COMP_THREADS / 32];
     __shared__ int s_count;
 
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
-    const int tx0 = blockIdx.x * VR_COMP_TILE_W, ty0 = blockIdx.y * VR_COMP_TILE_H;
+    const int tx0 = win.x + blockIdx.x * VR_COMP_TILE_W, ty0 = win.y + blockIdx.y * VR_COMP_TILE_H;
+    float4* __restrict__ out = reinterpret_cast<float4*>(out_);
+    const long long oidx = (long long)(ty0 + (int)(threadIdx.x / VR_COMP_TILE_W) - win.y) * WP + (tx0 + (int)(threadIdx.x & (VR_COMP_TILE_W - 1)) - win.x);
     const int tx1 = min(tx0 + VR_COMP_TILE_W, W), ty1 = min(ty0 + VR_COMP_TILE_H, H);
     const int px = tx0 + (tid & (VR_COMP_TILE_W - 1)), py = ty0 + tid / VR_COMP_TILE_W;
     const bool live = px < W && py < H;
@@ -52,7 +58,10 @@ vr_composite_kernel(const VrCompLayer* __restrict__ layers, const int* __restric
     if (bound) {
         const int bx0 = __ldg(bound), by0 = __ldg(bound + 1), bx1 = __ldg(bound + 2), by1 = __ldg(bound + 3);
         if (!(bx0 < tx1 && bx1 > tx0 && by0 < ty1 && by1 > ty0)) {
-            if (live) __stcs(out + (long long)py * W + px, make_float4(0.0f, 0.0f, 0.0f, 0.0f));
+            if (live) {
+                if (MODE == VR_MIP_RAW) __stcs(reinterpret_cast<float*>(out_) + oidx, -INFINITY);
+                else __stcs(out + oidx, make_float4(0.0f, 0.0f, 0.0f, 0.0f));
+            }
             return;
         }
     }
@@ -100,10 +109,7 @@ vr_composite_kernel(const VrCompLayer* __restrict__ layers, const int* __restric
                         cg = fmaf(t, s.y, cg);
                         cb = fmaf(t, s.z, cb);
                         ca = fmaf(t, s.w, ca);
-                    } else if (MODE == VR_MIP_PARTS) {
-                        const float4 s = __ldcs(reinterpret_cast<const float4*>(e.addr) + off);
-                        if (s.w != 0.0f) m = fmaxf(m, s.x);
-                    } else {
+                    } else { /* VR_MIP: brick sub-images; VR_MIP_RAW likewise; VR_MIP_PARTS: the parts' scalar pieces (-inf = no sample) */
                         m = fmaxf(m, __ldcs(reinterpret_cast<const float*>(e.addr) + off));
                     }
                 }
@@ -112,14 +118,14 @@ vr_composite_kernel(const VrCompLayer* __restrict__ layers, const int* __restric
         __syncthreads();
     }
 
-    if (live) {
+    if (live && MODE == VR_MIP_RAW) {
+        __stcs(reinterpret_cast<float*>(out_) + oidx, m);
+    } else if (live) {
         float4 o;
         if (MODE == VR_ALPHA) {
             o = make_float4(cr, cg, cb, ca);
         } else if (m == -INFINITY) {
             o = make_float4(0.0f, 0.0f, 0.0f, 0.0f);
-        } else if (MODE == VR_MIP_RAW) {
-            o = make_float4(m, 0.0f, 0.0f, 1.0f);
         } else {
             const float u = __saturatef((m - lut.vmin) * lut.inv_range);
             const float x = u * (float)(lut.n - 1);
@@ -128,20 +134,22 @@ vr_composite_kernel(const VrCompLayer* __restrict__ layers, const int* __restric
             const float4 e = __ldg(lut.base + i), d = __ldg(lut.delta + i);
             o = make_float4(fmaf(f, d.x, e.x), fmaf(f, d.y, e.y), fmaf(f, d.z, e.z), 1.0f);
         }
-        __stcs(out + (long long)py * W + px, o);
+        __stcs(out + oidx, o);
     }
 }
 
 cudaError_t vr_launch_composite(const VrCompLayer* layers, const int* order, int n, int W, int H, int mode,
-                                const VrLut& lut, float* out, const int* bound, cudaStream_t st) {
-    dim3 grid((W + VR_COMP_TILE_W - 1) / VR_COMP_TILE_W, (H + VR_COMP_TILE_H - 1) / VR_COMP_TILE_H);
+                                const VrLut& lut, float* out, const int* bound, const int* window, cudaStream_t st) {
+    const int4 win = window ? make_int4(window[0], window[1], window[2], window[3]) : make_int4(0, 0, W, H);
+    if (win.z <= win.x || win.w <= win.y) return cudaSuccess; /* an empty window: nothing to write */
+    dim3 grid((win.z - win.x + VR_COMP_TILE_W - 1) / VR_COMP_TILE_W, (win.w - win.y + VR_COMP_TILE_H - 1) / VR_COMP_TILE_H);
     if (mode == VR_ALPHA)
-        vr_composite_kernel<VR_ALPHA><<<grid, COMP_THREADS, 0, st>>>(layers, order, n, W, H, lut, reinterpret_cast<float4*>(out), bound);
+        vr_composite_kernel<VR_ALPHA><<<grid, COMP_THREADS, 0, st>>>(layers, order, n, win, lut, out, bound);
     else if (mode == VR_MIP)
-        vr_composite_kernel<VR_MIP><<<grid, COMP_THREADS, 0, st>>>(layers, order, n, W, H, lut, reinterpret_cast<float4*>(out), bound);
+        vr_composite_kernel<VR_MIP><<<grid, COMP_THREADS, 0, st>>>(layers, order, n, win, lut, out, bound);
     else if (mode == VR_MIP_RAW)
-        vr_composite_kernel<VR_MIP_RAW><<<grid, COMP_THREADS, 0, st>>>(layers, order, n, W, H, lut, reinterpret_cast<float4*>(out), bound);
+        vr_composite_kernel<VR_MIP_RAW><<<grid, COMP_THREADS, 0, st>>>(layers, order, n, win, lut, out, bound);
     else
-        vr_composite_kernel<VR_MIP_PARTS><<<grid, COMP_THREADS, 0, st>>>(layers, order, n, W, H, lut, reinterpret_cast<float4*>(out), bound);
+        vr_composite_kernel<VR_MIP_PARTS><<<grid, COMP_THREADS, 0, st>>>(layers, order, n, win, lut, out, bound);
     return cudaGetLastError();
 }

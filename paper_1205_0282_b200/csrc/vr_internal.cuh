@@ -31,8 +31,8 @@
 #define VR_COMP_TILE_W 32
 #define VR_COMP_TILE_H 8
 /* internal compositing modes next to VR_ALPHA / VR_MIP (row f3):
- *   VR_MIP_RAW    scalar MIP sub-images in, (max, 0, 0, 1) out, or (0,0,0,0) where no layer holds a sample
- *   VR_MIP_PARTS  such float4 partial frames in (w = 1 marks a sample), LUT colour of the maximum out */
+ *   VR_MIP_RAW    scalar MIP sub-images in, scalar maximum out (-inf where no layer holds a sample)
+ *   VR_MIP_PARTS  such scalar partial frames in, LUT colour of the maximum out ((0,0,0,0) where all are -inf) */
 #define VR_MIP_RAW 2
 #define VR_MIP_PARTS 3
 #define VR_EV_RING 64 /* timed frames whose stage events are kept */
@@ -208,9 +208,11 @@ cudaError_t vr_launch_cell_flags(const float2* cell_mm, unsigned* bits, int nbri
 cudaError_t vr_launch_raycast(const VrRaycastParams& p, long long items, bool count, bool sparse, cudaStream_t st);
 /* fused traversal (row f2): one ray per frame pixel through all bricks, writes the frame */
 cudaError_t vr_launch_fused(const VrRaycastParams& p, float* frame, int W, int H, bool count, cudaStream_t st);
-/* bound: device int[4] as VrViewState::bound, or NULL (layers anywhere) */
+/* bound: device int[4] as VrViewState::bound, or NULL (layers anywhere); window: host int[4] (x0, y0, x1, y1), the
+ * pixels of the W x H frame this launch writes, stored [y1-y0][x1-x0] at out, or NULL = the whole frame.
+ * out: float4 per pixel, except VR_MIP_RAW: one float per pixel (-inf = no sample). */
 cudaError_t vr_launch_composite(const VrCompLayer* layers, const int* order, int n, int W, int H, int mode,
-                                const VrLut& lut, float* out, const int* bound, cudaStream_t st);
+                                const VrLut& lut, float* out, const int* bound, const int* window, cudaStream_t st);
 cudaError_t vr_launch_upload(const VrGrid& grid, float* bricks, const float* src, int x0, int y0, int z0, int sx,
                              int sy, int sz, cudaStream_t st);
 cudaError_t vr_launch_download(const VrGrid& grid, const float* bricks, float* dst, int x0, int y0, int z0, int sx,
@@ -229,5 +231,9 @@ int vr_host_view_check(const VrGrid& grid, const float* view, const float* proj,
                        long long* items);
 
 int vr_host_part_rect(const VrGrid& grid, const float* view, const float* proj, int W, int H, int rect[4]);
+/* row f3 (vr_parts.cu): k-d partition of the brick grid (0 = ok, 1 = more parts than the grid can be cut into) and the
+ * parts front to back (0 = ok, 1 = singular view, 2 = malformed tree) */
+int vr_host_kd_partition(int nx, int ny, int nz, int brick, int nparts, int* boxes_out, int* tree_out);
+int vr_host_part_order(const int* tree, int nparts, int brick, const float* view, const float* proj, int* order_out);
 
 #endif

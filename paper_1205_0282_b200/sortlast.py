@@ -3,16 +3,18 @@
 The paper's scheme (PAPER.md:136-138 partitioning, :170-174 two-stage compositing, :178-184 direct send of
 rectangle-packed partial frames), mapped onto one node of B200s:
 
-  1. `kd_partition` deals the brick grid to the ranks as boxes: balanced k-d trees, split across the longest
+  1. `vr_kd_partition` deals the brick grid to the ranks as boxes: balanced k-d trees, split across the longest
      axis, and for a rank count that is not a power of two several trees whose roots share the longest axis in
      proportion to their rank counts.
-  2. Every rank renders the partial frame of its own bricks (`vr_render_part`: stage-1 compositing happens on
-     the GPU that rendered, "each node utilizes its local memory to do the first local composition").
-  3. The frame is dealt to the ranks in horizontal stripes; rank r sends rank s the piece
-     rect(r) ∩ stripe(s) of its partial frame, where rect(r) is the part's rendering rectangle (`vr_part_rect`,
-     computed by every rank for every part from the geometry alone: no size handshake). The volume moved per
-     frame is the frame size plus the overlap of the rectangles, "M + epsilon". This is a direct
-     send: point-to-point `torch.distributed` messages, NCCL over NVLink on GPUs.
+  2. The frame is dealt to the ranks in horizontal stripes; rank r owes rank s the piece rect(r) ∩ stripe(s) of its
+     partial frame, where rect(r) is the part's rendering rectangle (`vr_part_rect`, computed by every rank for every
+     part from the geometry alone: no size handshake). Every rank renders its own bricks and composites them
+     straight INTO those rectangle-packed pieces (`vr_render_part_pieces`: stage-1 compositing on the GPU that
+     rendered, "each node utilizes its local memory to do the first local composition") - float4 per pixel
+     for ALPHA, ONE float per pixel for MIP as in the paper (:180: 4 MB per 1024^2 sub-frame).
+  3. The pieces travel: the volume moved per frame is the frame size plus the overlap of the rectangles,
+     "M + epsilon". This is a direct send: point-to-point `torch.distributed`
+     messages, NCCL over NVLink on GPUs.
   4. Every rank merges the pieces of its stripe in part visibility order (`vr_composite_parts`: `over` for
      ALPHA, which NCCL's reductions cannot express; maximum + colour mapping for MIP) and rank 0 collects the
      stripes.
@@ -20,74 +22,15 @@ rectangle-packed partial frames), mapped onto one node of B200s:
 This module is plumbing: the arithmetic of every step runs in libvr's kernels through the `backend` (default: a
 part handle on the current CUDA device). Tests pass a backend of their own to run the protocol over gloo on CPUs.
 """
-import numpy as np
-
-from . import ALPHA, MIP, Volume, part_rect
+from . import ALPHA, MIP, Volume, kd_partition, part_order, part_rect  # noqa: F401 (kd_partition, part_order: re-exported)
 
 
 # ---------------------------------------------------------------------------------------------------------------
-# partitioning (host logic)
+# which voxels a rank uploads, which rows it merges (index bookkeeping; the partition and the part order are libvr's
+# vr_kd_partition / vr_part_order, the rectangles vr_part_rect)
 # ---------------------------------------------------------------------------------------------------------------
 def brick_grid(dims, brick):
     return tuple((int(n) + int(brick) - 1) // int(brick) for n in dims)
-
-
-def _extent(dims, brick, lo, hi, a):
-    """Voxels of bricks [lo, hi) along axis a (the last brick of an axis may be ragged)."""
-    return min(hi * brick, dims[a]) - lo * brick
-
-
-def _split(dims, brick, b0, b1, n_low, n_all):
-    """Cut the box across its longest axis (in voxels) that has more than one brick, the low side getting the
-    share n_low / n_all of the extent, rounded to a brick face."""
-    axes = sorted(range(3), key=lambda a: (-_extent(dims, brick, b0[a], b1[a], a), a))
-    for a in axes:
-        if b1[a] - b0[a] < 2:
-            continue
-        want = b0[a] * brick + _extent(dims, brick, b0[a], b1[a], a) * n_low / n_all
-        cut = int(round(want / brick))
-        return a, min(max(cut, b0[a] + 1), b1[a] - 1)
-    raise ValueError("more parts than bricks in the box %s..%s" % (b0, b1))
-
-
-def _balanced(dims, brick, b0, b1, n, first, boxes):
-    """A balanced k-d tree with n = 2^k leaves; leaves are numbered first, first+1, ... low side first."""
-    if n == 1:
-        boxes[first] = (tuple(b0), tuple(b1))
-        return ("leaf", first)
-    a, cut = _split(dims, brick, b0, b1, 1, 2)
-    lo1, hi0 = list(b0), list(b1)
-    hi0[a] = cut
-    lo1[a] = cut
-    return ("node", a, cut, _balanced(dims, brick, b0, hi0, n // 2, first, boxes),
-            _balanced(dims, brick, lo1, b1, n // 2, first + n // 2, boxes))
-
-
-def kd_partition(dims, brick, nparts):
-    """PAPER.md:138. Returns (boxes, tree): boxes[r] = (b0, b1), the half-open brick box of part r; tree = nested
-    ("node", axis, cut, low, high) / ("leaf", r) with cut in brick units, the structure `part_order` walks."""
-    nparts = int(nparts)
-    if nparts < 1:
-        raise ValueError("nparts must be positive")
-    g = brick_grid(dims, brick)
-    if nparts > g[0] * g[1] * g[2]:
-        raise ValueError("%d parts for %d bricks" % (nparts, g[0] * g[1] * g[2]))
-    boxes = [None] * nparts
-    sizes = [1 << k for k in range(nparts.bit_length() - 1, -1, -1) if nparts >> k & 1]  # 6 -> [4, 2]
-
-    def forest(b0, b1, sizes, first):
-        if len(sizes) == 1:
-            return _balanced(dims, brick, b0, b1, sizes[0], first, boxes)
-        # the roots of the trees share the longest axis in proportion to their rank counts
-        a, cut = _split(dims, brick, b0, b1, sizes[0], sum(sizes))
-        lo1, hi0 = list(b0), list(b1)
-        hi0[a] = cut
-        lo1[a] = cut
-        return ("node", a, cut, _balanced(dims, brick, b0, hi0, sizes[0], first, boxes),
-                forest(lo1, b1, sizes[1:], first + sizes[0]))
-
-    tree = forest([0, 0, 0], list(g), sizes, 0)
-    return boxes, tree
 
 
 def part_region(dims, brick, ghost, box):
@@ -96,36 +39,6 @@ def part_region(dims, brick, ghost, box):
     lo = [max(box[0][a] * brick - ghost, 0) for a in range(3)]
     hi = [min(min(box[1][a] * brick, dims[a]) + ghost, dims[a]) for a in range(3)]
     return tuple(lo), tuple(h - l for l, h in zip(lo, hi))
-
-
-def eye_of(view, proj):
-    """The homogeneous eye of R9: third column of (proj*view)^-1. Returns (xyz, ortho): the eye point, or for an
-    orthographic camera the forward direction."""
-    V = np.asarray(view, dtype=np.float32).astype(np.float64).reshape(4, 4).T  # column-major input
-    P = np.asarray(proj, dtype=np.float32).astype(np.float64).reshape(4, 4).T
-    c = np.linalg.inv(P @ V)[:, 2]
-    if abs(c[3]) < 1e-9 * np.abs(c[:3]).sum():
-        return c[:3], True
-    return c[:3] / c[3], False
-
-
-def part_order(tree, brick, view, proj):
-    """The parts front to back: at every node of the k-d tree the side that holds the eye comes first (the boxes of
-    the two sides are separated by the cut plane, so no ray meets the far side before the near one)."""
-    eye, ortho = eye_of(view, proj)
-    out = []
-
-    def walk(t):
-        if t[0] == "leaf":
-            out.append(t[1])
-            return
-        _, a, cut, low, high = t
-        low_first = eye[a] >= 0.0 if ortho else eye[a] < cut * brick
-        walk(low if low_first else high)
-        walk(high if low_first else low)
-
-    walk(tree)
-    return out
 
 
 def stripes(height, nparts):
@@ -155,10 +68,15 @@ class CudaBackend:
     def empty(self, shape):
         return self.torch.empty(shape, dtype=self.torch.float32, device=self.device)
 
-    def render_part(self, view, proj, width, height, step, mode):
-        out = self.empty((height, width, 4))
-        rect = self.volume.render_part(view, proj, width, height, step, mode, out)
-        return out, rect
+    def empty_piece(self, rect, mode):
+        h, w = rect[3] - rect[1], rect[2] - rect[0]
+        return self.empty((h, w, 4) if mode == ALPHA else (h, w))
+
+    def render_pieces(self, view, proj, width, height, step, mode, rects):
+        """The part's partial frame as one tensor per rectangle: [h][w][4] (ALPHA) or [h][w] (MIP, raw maximum)."""
+        pieces = [self.empty_piece(r, mode) for r in rects]
+        self.volume.render_part_pieces(view, proj, width, height, step, mode, rects, pieces)
+        return pieces
 
     def composite_parts(self, mode, pieces, rects, order, width, height):
         out = self.empty((height, width, 4))
@@ -211,34 +129,35 @@ class SortLastRenderer:
     # -- one frame -----------------------------------------------------------------------------------------------
     def render(self, view, proj, width, height, step, mode):
         """Returns the frame [height][width][4] on rank 0 (a tensor on the backend's device), None elsewhere."""
-        assert mode in (ALPHA, MIP)
+        if mode not in (ALPHA, MIP):
+            raise ValueError("SortLastRenderer.render: mode must be ALPHA or MIP")
         be, R, me = self.backend, self.world, self.rank
         rects = [part_rect(self.dims, self.brick, b, view, proj, width, height) for b in self.boxes]
         order = part_order(self.tree, self.brick, view, proj)
         rows = stripes(height, R)
-        partial, my_rect = be.render_part(view, proj, width, height, step, mode)
-        assert tuple(my_rect) == tuple(rects[me])
 
         def piece_of(r, s):
             return _clip(rects[r], rows[s][0], rows[s][1])
 
+        # stage 1 on this GPU, straight into the pieces this rank owes every stripe (its own included)
+        owed = [(s, piece_of(me, s)) for s in range(R)]
+        owed = [(s, c) for s, c in owed if c is not None]
+        rendered = be.render_pieces(view, proj, width, height, step, mode, [c for _, c in owed])
+        mine = dict((s, t) for (s, _), t in zip(owed, rendered))
         pieces = {}  # source rank -> tensor of rect(r) ∩ my stripe
-        mine = piece_of(me, me)
-        if mine is not None:
-            pieces[me] = partial[mine[1]:mine[3], mine[0]:mine[2]].contiguous()
+        if me in mine:
+            pieces[me] = mine[me]
         if R > 1:
             import torch.distributed as dist
-            ops, keep = [], []
+            ops = []
             for s in range(R):
                 if s == me:
                     continue
-                c = piece_of(me, s)
-                if c is not None:  # direct send of the packed piece (PAPER.md:180-184)
-                    keep.append(partial[c[1]:c[3], c[0]:c[2]].contiguous())
-                    ops.append(dist.P2POp(dist.isend, keep[-1], self._global(s), group=self.group))
+                if s in mine:  # direct send of the packed piece (PAPER.md:180-184)
+                    ops.append(dist.P2POp(dist.isend, mine[s], self._global(s), group=self.group))
                 c = piece_of(s, me)
                 if c is not None:
-                    pieces[s] = be.empty((c[3] - c[1], c[2] - c[0], 4))
+                    pieces[s] = be.empty_piece(c, mode)
                     ops.append(dist.P2POp(dist.irecv, pieces[s], self._global(s), group=self.group))
             if ops:
                 for w in dist.batch_isend_irecv(ops):
@@ -278,9 +197,9 @@ class SortLastRenderer:
         import torch.distributed as dist
         return dist.get_global_rank(self.group, r)
 
-    def exchange_bytes(self, view, proj, width, height):
-        """Bytes this frame's exchange moves between ranks (pieces sent to other ranks + stripes sent to rank 0):
-        the paper's M + epsilon, from the geometry alone."""
+    def exchange_bytes(self, view, proj, width, height, mode=ALPHA):
+        """Bytes this frame's exchange moves between ranks (pieces sent to other ranks: 16 bytes per pixel for ALPHA, 4 for
+        MIP; + the merged RGBA stripes sent to rank 0): the paper's M + epsilon, from the geometry alone."""
         rects = [part_rect(self.dims, self.brick, b, view, proj, width, height) for b in self.boxes]
         rows = stripes(height, self.world)
         total = 0
@@ -288,6 +207,6 @@ class SortLastRenderer:
             for s in range(self.world):
                 c = _clip(rects[r], rows[s][0], rows[s][1])
                 if r != s and c is not None:
-                    total += (c[2] - c[0]) * (c[3] - c[1]) * 16
+                    total += (c[2] - c[0]) * (c[3] - c[1]) * (16 if mode == ALPHA else 4)
         total += sum((y1 - y0) * width * 16 for (y0, y1) in rows[1:])
         return total

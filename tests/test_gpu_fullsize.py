@@ -230,7 +230,10 @@ def parts_against_oracle(vr, wl, cube, o, tf, nparts, vi, npix, whole=None):
         got = full.cpu().numpy().astype(np.float64)[pix[:, 1], pix[:, 0]]
         want = {"image": partial(ref), "flags": ref["flags"], "alt": lambda dtau, ns: {"image": partial(ref["alt"](dtau, ns))}}
         check_alpha(got, want, wl["tau"], "%s part %d of %d" % (wl["name"], r, nparts))
-        pieces.append(full[rc[1]:rc[3], rc[0]:rc[2]].contiguous())
+        piece = torch.empty((rc[3] - rc[1], rc[2] - rc[0], 4), dtype=torch.float32, device="cuda")
+        p.render_part_pieces(view, proj, W, H, wl["step"], vr.ALPHA, [rc], [piece])   # what a rank sends: packed by rectangle
+        assert torch.equal(piece, full[rc[1]:rc[3], rc[0]:rc[2]])
+        pieces.append(piece)
         rects.append(rc)
         if r + 1 < nparts:
             p.close()

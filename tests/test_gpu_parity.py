@@ -877,7 +877,7 @@ def test_reserved_views_render_without_allocating_and_torch_allocator(vr):
     finally:
         vr.use_torch_allocator(False)
     held = torch.cuda.memory_allocated() - before
-    assert held >= 27 * 36 * 36 * 34 * 4  # at least the brick store (27 slots of 9x9x17 micro-tiles) is torch's
+    assert held >= 18 * 9 * 9 * 17 * 128  # at least the brick store (18 slots of 9 x 9 x 17 micro-tiles of 128 bytes) is torch's
     o = oracle.Volume(cube.nx, cube.ny, cube.nz, 32, 1, data=data)
     g.upload(torch.from_numpy(data).cuda())
     for v in (g, o):

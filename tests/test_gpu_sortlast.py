@@ -33,21 +33,44 @@ def make_parts(vr, sortlast, data, dims, brick, ghost, nparts, halo_only=True):
     return boxes, tree, parts
 
 
-def merged_frame(vr, sortlast, parts, boxes, tree, dims, brick, view, proj, W, H, step, mode):
-    """What SortLastRenderer does, on one device: partial frames, packed by rectangle, merged in part order."""
+def merged_frame(vr, sortlast, parts, boxes, tree, dims, brick, view, proj, W, H, step, mode, use_pieces=True):
+    """What SortLastRenderer does, on one device: every part composites its sub-images straight into rectangle-packed
+    pieces (here: its rectangle cut into an upper and a lower piece, as two stripes would), merged in part order.
+    The pieces must equal, bit for bit, the same pixels of the part's full partial frame (vr_render_part), which must
+    be blank outside the part's rectangle. ALPHA: float4 per pixel; MIP: one float per pixel, -inf = no sample."""
     import torch
     pieces, rects = [], []
     for p, box in zip(parts, boxes):
-        full = torch.empty((H, W, 4), dtype=torch.float32, device="cuda")
+        full = torch.empty((H, W, 4) if mode == vr.ALPHA else (H, W), dtype=torch.float32, device="cuda")
         r = p.render_part(view, proj, W, H, step, mode, full)
         assert r == vr.part_rect(dims, brick, box, view, proj, W, H)
         outside = full.clone()
-        outside[r[1]:r[3], r[0]:r[2]] = 0
-        assert not outside.any(), "a partial frame is not blank outside its rectangle"
-        pieces.append(full[r[1]:r[3], r[0]:r[2]].contiguous())
-        rects.append(r)
+        outside[r[1]:r[3], r[0]:r[2]] = 0 if mode == vr.ALPHA else -np.inf
+        assert not (outside.any() if mode == vr.ALPHA else (outside != -np.inf).any()), "a partial frame is not blank outside its rectangle"
+        ymid = (r[1] + r[3]) // 2
+        cuts = [c for c in ((r[0], r[1], r[2], ymid), (r[0], ymid, r[2], r[3])) if c[2] > c[0] and c[3] > c[1]]
+        bufs = [torch.full((c[3] - c[1], c[2] - c[0], 4) if mode == vr.ALPHA else (c[3] - c[1], c[2] - c[0]), 7.0,
+                           dtype=torch.float32, device="cuda") for c in cuts]
+        if use_pieces:
+            p.render_part_pieces(view, proj, W, H, step, mode, cuts, bufs)
+            for c, b in zip(cuts, bufs):
+                assert torch.equal(b, full[c[1]:c[3], c[0]:c[2]])
+        else:  # the fused traversal of a part writes its whole partial frame: the pieces are cut out of it
+            bufs = [full[c[1]:c[3], c[0]:c[2]].contiguous() for c in cuts]
+        pieces += bufs
+        rects += cuts
+    # a part's pieces do not overlap, so any order that keeps the parts in visibility order will do
+    po = sortlast.part_order(tree, brick, view, proj)
+    idx, k = {}, 0
+    for q, (p, box) in enumerate(zip(parts, boxes)):
+        r = vr.part_rect(dims, brick, box, view, proj, W, H)
+        ymid = (r[1] + r[3]) // 2
+        n = sum(1 for c in ((r[0], r[1], r[2], ymid), (r[0], ymid, r[2], r[3])) if c[2] > c[0] and c[3] > c[1])
+        idx[q] = list(range(k, k + n))
+        k += n
+    order = [i for q in po for i in idx[q]]
     out = torch.empty((H, W, 4), dtype=torch.float32, device="cuda")
-    parts[0].composite_parts(mode, pieces, rects, sortlast.part_order(tree, brick, view, proj), W, H, out)
+    parts[0].composite_parts(mode, pieces, rects, order, W, H, out)
     torch.cuda.synchronize()
     return out.cpu().numpy().astype(np.float64)
 
@@ -137,6 +160,11 @@ def test_part_arguments(vr):
     with pytest.raises(vr.VrError):                                    # a MIP part stays scalar: sort-last traversal only
         p.render_part(fr.seeded(1, 0), fr.proj(False), 64, 48, 1.0, vr.MIP, out)
     p.render_part(fr.seeded(1, 0), fr.proj(False), 64, 48, 1.0, vr.ALPHA, out)
+    with pytest.raises(vr.VrError):                                    # pieces come from the sort-last traversal
+        p.render_part_pieces(fr.seeded(1, 0), fr.proj(False), 64, 48, 1.0, vr.ALPHA, [(0, 0, 8, 8)], [out[:8, :8].contiguous()])
+    p.set_traversal(vr.SORT_LAST)
+    with pytest.raises(vr.VrError):                                    # a piece must lie inside the frame
+        p.render_part_pieces(fr.seeded(1, 0), fr.proj(False), 64, 48, 1.0, vr.ALPHA, [(60, 0, 68, 8)], [out[:8, :8].contiguous()])
 
 
 def test_parts_cull_and_skip_like_the_whole_volume(vr):
@@ -166,7 +194,7 @@ def test_parts_cull_and_skip_like_the_whole_volume(vr):
         check_alpha(frames[True], ref, 2.0, "view %d" % k)
         for p in parts:
             p.set_traversal(vr.FUSED)
-        fused = merged_frame(vr, sortlast, parts, boxes, tree, dims, brick, view, proj, W, H, 0.8, vr.ALPHA)
+        fused = merged_frame(vr, sortlast, parts, boxes, tree, dims, brick, view, proj, W, H, 0.8, vr.ALPHA, use_pieces=False)
         check_alpha(fused, ref, 2.0, "fused parts, view %d" % k)
         for p in parts:
             p.set_traversal(vr.SORT_LAST)
