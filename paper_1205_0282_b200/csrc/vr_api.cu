@@ -656,7 +656,8 @@ static bool cells_supported(const vr_volume* v) {
            g.ml[2] == 0 && g.ghost >= 1;
 }
 
-static int ensure_cells(vr_volume* v, bool want_bits, cudaStream_t st) {
+/* memory of the macro-cell tables (taken on first use, or ahead of it by vr_reserve_views) */
+static int alloc_cells(vr_volume* v) {
     const VrGrid& g = v->grid;
     if (!v->d_cell_mm) {
         for (int a = 0; a < 3; ++a) v->nc[a] = (g.nt[a] * (1 << g.tl[a]) + 7) / 8;
@@ -664,6 +665,16 @@ static int ensure_cells(vr_volume* v, bool want_bits, cudaStream_t st) {
         v->cell_words = (int)((ncell + 31) / 32);
         VR_CUDA(v, v_alloc(v, &v->d_cell_mm, sizeof(float2) * (size_t)ncell * g.nown));
         VR_CUDA(v, v_alloc(v, &v->d_cell_bits, sizeof(unsigned) * (size_t)v->cell_words * g.nown));
+    }
+    if (!v->d_cell_count) VR_CUDA(v, v_alloc(v, &v->d_cell_count, sizeof(unsigned long long)));
+    return VR_OK;
+}
+
+static int ensure_cells(vr_volume* v, bool want_bits, cudaStream_t st) {
+    const VrGrid& g = v->grid;
+    {
+        const int rc = alloc_cells(v);
+        if (rc) return rc;
     }
     if (!v->cell_mm_valid) {
         VR_CUDA(v, vr_launch_cell_minmax(g, v->bricks, v->d_cell_mm, v->nc, st));
@@ -687,7 +698,6 @@ static int decide_mip_skip(vr_volume* v, cudaStream_t st) {
     int rc = ensure_minmax(v, st);
     if (!rc) rc = ensure_cells(v, false, st);
     if (rc) return rc;
-    if (!v->d_cell_count) VR_CUDA(v, v_alloc(v, &v->d_cell_count, sizeof(unsigned long long)));
     const long long ncells = (long long)v->nc[0] * v->nc[1] * v->nc[2] * v->grid.nown;
     unsigned long long empty = 0;
     VR_CUDA(v, cudaMemsetAsync(v->d_cell_count, 0, sizeof(unsigned long long), st));
@@ -730,6 +740,7 @@ extern "C" int vr_reserve_views(vr_volume* v, const float* views, const float* p
     const long long px = (long long)width * height;
     int rc = ensure_sub(v, need > 0 ? need : px);
     if (!rc) rc = ensure_rays(v, px);
+    if (!rc && cells_supported(v)) rc = alloc_cells(v); /* R19's tables: filled by the first frame that uses them */
     if (rc) return rc;
     /* the host entries' device frames (vr_render_host: one; vr_render_host_async: two, a stream and four events) */
     if (px > v->frame_capacity_px) {
