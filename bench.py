@@ -164,14 +164,17 @@ def build_volume(vr, wl, tf):
     up_ms = sum(a.elapsed_time(b) for a, b in evs)
     g.upload_stats = {"kernel": "vr_upload_tile442_kernel", "launches": len(evs), "ms": round(up_ms, 3), "bytes": up_bytes,
                       "gb_per_s": round(up_bytes / (up_ms * 1e-3) / 1e9, 1)}
-    # row f1 (once per upload): one streaming read of the padded brick store
+    # every per-view buffer and table the frames below need, taken now: vr_render then never allocates or synchronises
+    g.reserve_views(wl["views"], [wl["proj"]] * len(wl["views"]), wl["width"], wl["height"])
+    torch.cuda.synchronize()
+    # rows f1 + R19 (once per upload): one streaming read of the padded brick store gives the per-brick and the macro-cell ranges
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record()
     lo, hi = g.minmax()
     e1.record()
     torch.cuda.synchronize()
     mm_ms = e0.elapsed_time(e1)
-    g.minmax_stats = {"kernel": "vr_brick_minmax_kernel", "ms": round(mm_ms, 3), "bytes": 4 * pad,
+    g.minmax_stats = {"kernel": "vr_range_kernel (+ init, decode, reduce: 4 launches)", "ms": round(mm_ms, 3), "bytes": 4 * pad,
                       "gb_per_s": round(4 * pad / (mm_ms * 1e-3) / 1e9, 1), "data_min": float(lo), "data_max": float(hi)}
     return g, cube
 

@@ -12,7 +12,7 @@
 
 #include <new>
 
-#include "vr_internal.cuh"
+#include "vr_view.cuh"
 
 static char g_err[512] = "no error";
 static char* g_err_buf() { return g_err; }
@@ -46,6 +46,7 @@ struct vr_volume {
     long long stage_floats;
     int2* d_mm_enc;          /* row f1: per-brick range, order-preserving integer encoding */
     float2* d_mm;            /* nbricks + 1 entries: per brick, then the whole volume */
+    int4* d_slot_ext;        /* nown entries: padded extent (x, y, z) of the brick in each slot */
     bool mm_valid;           /* d_mm describes the current contents of the store */
     float2* d_cell_mm;       /* R19: (min, max) per 8x8x8 macro-cell, nbricks * nc^3 (allocated on first use) */
     unsigned* d_cell_bits;   /* 1 = macro-cell transparent under the current LUT */
@@ -161,6 +162,7 @@ static void release(vr_volume* v) {
     v_free(v, v->d_bitmap);
     v_free(v, v->d_mm_enc);
     v_free(v, v->d_mm);
+    v_free(v, v->d_slot_ext);
     v_free(v, v->d_cell_mm);
     v_free(v, v->d_cell_bits);
     v_free(v, v->d_cell_count);
@@ -343,6 +345,21 @@ static int create_volume(int nx, int ny, int nz, int brick, int ghost, int layou
     if (e == cudaSuccess) e = v_alloc(v, &v->d_mm, sizeof(float2) * (g.nbricks + 1));
     for (int r = 0; r < VR_EV_RING && e == cudaSuccess; ++r)
         for (int i = 0; i < 4 && e == cudaSuccess; ++i) e = cudaEventCreate(&v->ev[r][i]);
+    if (e == cudaSuccess) e = v_alloc(v, &v->d_slot_ext, sizeof(int4) * g.nown);
+    if (e == cudaSuccess) {
+        int4* ext = new (std::nothrow) int4[g.nown];
+        if (!ext) e = cudaErrorMemoryAllocation;
+        for (int b = 0; ext && b < g.nbricks; ++b) {
+            const int s = vr_slot_index(g, b);
+            if (s < 0) continue;
+            int bc[3], lo[3], hi[3];
+            vr_brick_coords(g, b, bc);
+            vr_brick_core(g, bc, lo, hi);
+            ext[s] = make_int4(hi[0] - lo[0] + 2 * ghost, hi[1] - lo[1] + 2 * ghost, hi[2] - lo[2] + 2 * ghost, b);
+        }
+        if (ext) e = cudaMemcpy(v->d_slot_ext, ext, sizeof(int4) * g.nown, cudaMemcpyHostToDevice);
+        delete[] ext;
+    }
     if (e == cudaSuccess) e = cudaHostAlloc(&v->h_overflow, sizeof(int), cudaHostAllocMapped);
     if (e == cudaSuccess) {
         *v->h_overflow = 0;
@@ -640,10 +657,22 @@ static int ensure_pipe(vr_volume* v, long long px) {
 }
 
 /* Row f1: bring the range table up to date with the store (three launches, after an upload only). */
+static bool cells_supported(const vr_volume* v);
+static int alloc_cells(vr_volume* v);
+
 static int ensure_minmax(vr_volume* v, cudaStream_t st) {
     if (v->mm_valid) return VR_OK;
-    VR_CUDA(v, vr_launch_minmax(v->grid, v->bricks, v->d_mm_enc, v->d_mm, st));
-    v->launches += 3;
+    if (cells_supported(v)) { /* the macro-cell table (R19) comes out of the same read of the store */
+        const int rc = alloc_cells(v);
+        if (rc) return rc;
+        VR_CUDA(v, vr_launch_ranges(v->grid, v->bricks, v->d_mm_enc, v->d_mm, v->d_cell_mm, v->nc, v->d_slot_ext, st));
+        v->launches += 4;
+        v->cell_mm_valid = true;
+        v->cell_bits_valid = false;
+    } else {
+        VR_CUDA(v, vr_launch_minmax(v->grid, v->bricks, v->d_mm_enc, v->d_mm, st));
+        v->launches += 3;
+    }
     v->mm_valid = true;
     return VR_OK;
 }

@@ -196,6 +196,10 @@ cudaError_t vr_launch_tex_fill(const VrGrid& grid, const float* bricks, const Vr
 /* ray table of the frame whose set-up is in vs (row a4, the per-ray part) */
 cudaError_t vr_launch_rays(const VrGrid& grid, const VrViewState* vs, int W, int H, double step, double2* rays, cudaStream_t st);
 cudaError_t vr_launch_minmax(const VrGrid& grid, const float* bricks, int2* enc, float2* table, cudaStream_t st);
+/* rows f1 + R19 in one streaming read (4x4x2 layout, ghost >= 1): the per-brick table and the macro-cell table; 4 launches */
+/* slot_ext: device int4[nown], the padded extent (x, y, z) of the brick in each slot */
+cudaError_t vr_launch_ranges(const VrGrid& grid, const float* bricks, int2* enc, float2* table, float2* cell_mm, const int nc[3],
+                             const int4* slot_ext, cudaStream_t st);
 /* macro-cells (R19): per-cell (min, max) of the 4x4x2-tiled store; transparency bits for a LUT */
 cudaError_t vr_launch_cell_minmax(const VrGrid& grid, const float* bricks, float2* cell_mm, const int nc[3], cudaStream_t st);
 /* *count += macro-cells of the whole store whose (min, max) is exactly (lo, lo): empty space of a density cube */

@@ -218,6 +218,153 @@ vr_cell_flags_kernel(const float2* __restrict__ cell_mm, unsigned* __restrict__ 
     }
 }
 
+/* ------------------------------------------------------------------------------------------
+ * Both tables from ONE streaming read of the store (one min/max task after the data is loaded).
+ * A warp takes a macro-cell: its 16 micro-tiles = 128 float4 words, 4 per lane (lane -> tile column tx, tile row ty and
+ * row r of the micro-tile are fixed, the 4 words differ in tile layer tz). The 9x9x9 block R19 asks for is the macro-
+ * cell's own 8x8x8 cells plus the FIRST planes of its high-side neighbours; seen from the neighbour, its planes x = 0,
+ * y = 0, z = 0, their three common edges and the corner belong to the blocks of the macro-cells on its low sides. So a
+ * warp reduces eight ranges - own cells, three faces, three edges, corner - with REDUX on the order-preserving integer
+ * encoding (16 instructions) and merges each into the table entry of the macro-cell it belongs to with integer atomics
+ * (distinct addresses, absorbed by L2). The brick's range is the union of its macro-cells' own-cell ranges: kept in
+ * registers across a CTA's macro-cells, two atomics per CTA. No cell is read twice; the halo reads that cost the two-pass
+ * version 1.47x the store's bytes are gone.
+ * ---------------------------------------------------------------------------------------- */
+__global__ void vr_range_init_kernel(int2* __restrict__ cell_enc, long long ncells, int2* __restrict__ brick_enc, int nbricks) {
+    const int2 e = make_int2(mm_encode(INFINITY), mm_encode(-INFINITY));
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < ncells; i += (long long)gridDim.x * blockDim.x) cell_enc[i] = e;
+    if (blockIdx.x == 0)
+        for (int b = threadIdx.x; b < nbricks; b += blockDim.x) brick_enc[b] = e;
+}
+
+__device__ __forceinline__ void range_merge(int2* __restrict__ p, int mn, int mx) {
+    if (mn <= mx) {
+        atomicMin(&p->x, mn);
+        atomicMax(&p->y, mx);
+    }
+}
+
+__global__ void __launch_bounds__(256)
+vr_range_kernel(VrGrid g, const float* __restrict__ bricks, int2* __restrict__ cell_enc, const int4* __restrict__ slot_ext, int nc0,
+                int nc1, int nc2) {
+    /* grid (1, rows x layers of macro-cells, slots): a CTA takes one row of macro-cells, warp w the macro-cells
+     * m0 = w, w + 8, ... of it: the per-row index arithmetic is paid once per warp, the words of the next macro-cell are
+     * 16 float4 further on (the first version, a grid-stride loop over all macro-cells with two divisions per cell and
+     * eight predicated accumulators, was ALU-bound at 554 instructions per macro-cell) */
+    const int slot_b = blockIdx.z;
+    const int4 ext = __ldg(slot_ext + slot_b); /* padded extent of the brick in this slot (x, y, z) */
+    const int ex = ext.x, ey = ext.y, ez = ext.z;
+    const int lane = threadIdx.x & 31;
+    const int m2 = blockIdx.y / nc1, m1 = blockIdx.y - m2 * nc1;
+    const float4* __restrict__ base = reinterpret_cast<const float4*>(bricks + (long long)slot_b * g.slot);
+    const int tcol = (lane >> 3) & 1, trow = lane >> 4, r = lane & 7;
+    const int jl = (trow << 2) + (r & 3); /* the lane's y inside the macro-cell; x = 4 tcol .. 4 tcol + 3; z = 2 q + (r >> 2) */
+    const int ty = (m1 << 1) + trow;
+    const bool row_ok = ty < g.nt[1] && (m1 << 3) + jl < ey;
+    bool okz[4];
+#pragma unroll
+    for (int q = 0; q < 4; ++q) okz[q] = row_ok && (m2 << 2) + q < g.nt[2] && (((m2 << 2) + q) << 1) + (r >> 2) < ez;
+    const long long wrow = ((long long)(((m2 << 2) * g.nt[1] + ty) * g.nt[0]) << 3) + r, wz = (long long)g.nt[1] * g.nt[0] << 3;
+    const bool x0 = tcol == 0, y0 = jl == 0, z0 = r < 4;
+    const int E_HI = mm_encode(INFINITY), E_LO = mm_encode(-INFINITY);
+    int2* __restrict__ cells = cell_enc + (long long)slot_b * (nc0 * nc1 * nc2);
+    /* which range this lane merges (lanes 0..7: own, -x, -y, -z, -x-y, -x-z, -y-z, -x-y-z) and into which macro-cell */
+    const int dx = (0xB2 >> (lane & 7)) & 1, dy = (0xD4 >> (lane & 7)) & 1, dz = (0xE8 >> (lane & 7)) & 1;
+    const bool merges = lane < 8 && m1 - dy >= 0 && m2 - dz >= 0;
+    int2* __restrict__ target = cells + ((m2 - dz) * nc1 + (m1 - dy)) * nc0 - dx;
+    for (int m0 = threadIdx.x >> 5; m0 < nc0; m0 += blockDim.x >> 5) {
+        const int tx = (m0 << 1) + tcol, i = tx << 2;
+        const bool col_ok = tx < g.nt[0] && i < ex;
+        const float4* __restrict__ p = base + (wrow + ((long long)tx << 3));
+        float4 v[4];
+#pragma unroll
+        for (int q = 0; q < 4; ++q) /* all four loads first */
+            if (col_ok && okz[q]) v[q] = __ldcs(p + q * wz);
+        /* per lane: A = range of its words (own cells), B = range of their first elements (the column x = 4 tcol), and
+         * both restricted to the plane z = 0 (word q = 0 of the lanes with r < 4) */
+        float amn = INFINITY, amx = -INFINITY, bmn = INFINITY, bmx = -INFINITY, azmn = INFINITY, azmx = -INFINITY, bzmn = INFINITY,
+              bzmx = -INFINITY;
+        const bool full = i + 3 < ex;
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            if (!(col_ok && okz[q])) continue;
+            float wmn, wmx; /* cells beyond the brick's extent are left out */
+            if (full) {
+                wmn = fminf(fminf(v[q].x, v[q].y), fminf(v[q].z, v[q].w));
+                wmx = fmaxf(fmaxf(v[q].x, v[q].y), fmaxf(v[q].z, v[q].w));
+            } else {
+                wmn = wmx = v[q].x;
+                if (i + 1 < ex) wmn = fminf(wmn, v[q].y), wmx = fmaxf(wmx, v[q].y);
+                if (i + 2 < ex) wmn = fminf(wmn, v[q].z), wmx = fmaxf(wmx, v[q].z);
+            }
+            amn = fminf(amn, wmn), amx = fmaxf(amx, wmx);
+            bmn = fminf(bmn, v[q].x), bmx = fmaxf(bmx, v[q].x);
+            if (q == 0 && z0) /* through fminf / fmaxf: a NaN (blanked) cell must not become a bound (R14) */
+                azmn = fminf(azmn, wmn), azmx = fmaxf(azmx, wmx), bzmn = fminf(bzmn, v[q].x), bzmx = fmaxf(bzmx, v[q].x);
+        }
+        /* the eight ranges: 0 own cells, 1 x = 0, 2 y = 0, 3 z = 0, 4 x = y = 0, 5 x = z = 0, 6 y = z = 0, 7 corner; a lane
+         * contributes to a face only if it holds cells of it (lane-constant conditions). fminf / fmaxf ignored NaN
+         * voxels (R14); an untouched range stays (+inf, -inf) */
+        const int eamn = mm_encode(amn), eamx = mm_encode(amx), ebmn = mm_encode(bmn), ebmx = mm_encode(bmx);
+        const int eazmn = mm_encode(azmn), eazmx = mm_encode(azmx), ebzmn = mm_encode(bzmn), ebzmx = mm_encode(bzmx);
+        int smn = E_HI, smx = E_LO, t;
+#define VR_RANGE(c, vmn, vmx)                                        \
+    t = __reduce_min_sync(0xffffffffu, (vmn)); if (lane == (c)) smn = t; \
+    t = __reduce_max_sync(0xffffffffu, (vmx)); if (lane == (c)) smx = t;
+        VR_RANGE(0, eamn, eamx)
+        VR_RANGE(1, x0 ? ebmn : E_HI, x0 ? ebmx : E_LO)
+        VR_RANGE(2, y0 ? eamn : E_HI, y0 ? eamx : E_LO)
+        VR_RANGE(3, eazmn, eazmx)
+        VR_RANGE(4, x0 && y0 ? ebmn : E_HI, x0 && y0 ? ebmx : E_LO)
+        VR_RANGE(5, x0 ? ebzmn : E_HI, x0 ? ebzmx : E_LO)
+        VR_RANGE(6, y0 ? eazmn : E_HI, y0 ? eazmx : E_LO)
+        VR_RANGE(7, x0 && y0 ? ebzmn : E_HI, x0 && y0 ? ebzmx : E_LO)
+#undef VR_RANGE
+        if (merges && m0 - dx >= 0) range_merge(target + m0, smn, smx);
+    }
+}
+
+/* Decode the macro-cell table in place (int2 -> float2, -0 -> +0 as the two-pass version did) and reduce each brick's
+ * entries to the brick's range: the union of the 9x9x9 blocks of a brick's macro-cells is the brick's padded cells. */
+__global__ void __launch_bounds__(256)
+vr_range_finish_cells_kernel(VrGrid g, int2* __restrict__ cell_enc, int ncell, int2* __restrict__ brick_enc) {
+    const int b = blockIdx.y;
+    const int slot_b = vr_slot_index(g, b);
+    if (slot_b < 0) return;
+    int2* __restrict__ cells = cell_enc + (long long)slot_b * ncell;
+    int bmn = mm_encode(INFINITY), bmx = mm_encode(-INFINITY);
+    for (int m = blockIdx.x * blockDim.x + threadIdx.x; m < ncell; m += gridDim.x * blockDim.x) {
+        const int2 e = cells[m];
+        if (e.x <= e.y) bmn = min(bmn, e.x), bmx = max(bmx, e.y);
+        reinterpret_cast<float2*>(cells)[m] = make_float2(mm_decode(e.x), mm_decode(e.y));
+    }
+    bmn = __reduce_min_sync(0xffffffffu, bmn);
+    bmx = __reduce_max_sync(0xffffffffu, bmx);
+    __shared__ int s_mn[8], s_mx[8];
+    if ((threadIdx.x & 31) == 0) s_mn[threadIdx.x >> 5] = bmn, s_mx[threadIdx.x >> 5] = bmx;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int w = 1; w < (int)(blockDim.x >> 5); ++w) bmn = min(bmn, s_mn[w]), bmx = max(bmx, s_mx[w]);
+        range_merge(brick_enc + b, bmn, bmx);
+    }
+}
+
+cudaError_t vr_launch_ranges(const VrGrid& grid, const float* bricks, int2* enc, float2* table, float2* cell_mm, const int nc[3],
+                             const int4* slot_ext, cudaStream_t st) {
+    const int ncell = nc[0] * nc[1] * nc[2];
+    const long long total = (long long)ncell * grid.nown;
+    if ((long long)nc[1] * nc[2] > 65535 || grid.nbricks > 65535) return cudaErrorInvalidValue;
+    int2* cell_enc = reinterpret_cast<int2*>(cell_mm);
+    vr_range_init_kernel<<<148 * 8, 256, 0, st>>>(cell_enc, total, enc, grid.nbricks);
+    vr_range_kernel<<<dim3(1u, (unsigned)(nc[1] * nc[2]), (unsigned)grid.nown), 256, 0, st>>>(grid, bricks, cell_enc, slot_ext, nc[0],
+                                                                                               nc[1], nc[2]);
+    int fx = (ncell + 256 * 8 - 1) / (256 * 8);
+    if (fx > 64) fx = 64;
+    vr_range_finish_cells_kernel<<<dim3((unsigned)fx, (unsigned)grid.nbricks), 256, 0, st>>>(grid, cell_enc, ncell, enc);
+    vr_minmax_finish_kernel<<<1, 256, 0, st>>>(enc, grid.nbricks, table);
+    return cudaGetLastError();
+}
+
 cudaError_t vr_launch_cell_minmax(const VrGrid& grid, const float* bricks, float2* cell_mm, const int nc[3], cudaStream_t st) {
     const long long ncell = (long long)nc[0] * nc[1] * nc[2];
     long long bx = (ncell + 7) / 8;

@@ -869,6 +869,8 @@ def test_reserved_views_render_without_allocating_and_torch_allocator(vr):
     fr = synth.Framing(cube.nx, cube.ny, cube.nz, W, H)
     views = [fr.turntable(k) for k in range(0, 36, 3)]
     projs = [fr.proj(False)] * len(views)
+    import gc
+    gc.collect()
     torch.cuda.synchronize()
     before = torch.cuda.memory_allocated()
     vr.use_torch_allocator(True)
@@ -886,7 +888,9 @@ def test_reserved_views_render_without_allocating_and_torch_allocator(vr):
     host = torch.empty((H, W, 4), dtype=torch.float32).pin_memory()
     out = torch.empty((H, W, 4), dtype=torch.float32, device="cuda")
     torch.cuda.synchronize()
-    alloc0 = torch.cuda.memory_allocated()  # the handle allocates through torch: anything it took would show here
+    # the handle allocates through torch: any block it took would be counted here (a cumulative count of allocations:
+    # tensors of earlier tests being collected meanwhile cannot disturb it)
+    allocs0 = torch.cuda.memory_stats()["allocation.all.allocated"]
     for view in views:
         g.render(view, projs[0], W, H, 0.5, vr.ALPHA, out)
         g.render(view, projs[0], W, H, 0.5, vr.MIP, out)
@@ -894,7 +898,7 @@ def test_reserved_views_render_without_allocating_and_torch_allocator(vr):
     g.render_host_wait()
     g.render_host(views[0], projs[0], W, H, 0.5, vr.ALPHA, host.numpy())
     torch.cuda.synchronize()
-    assert torch.cuda.memory_allocated() == alloc0
+    assert torch.cuda.memory_stats()["allocation.all.allocated"] == allocs0
     ref = o.render(views[0], projs[0], W, H, 0.5, oracle.ALPHA)
     check_alpha(host.numpy().astype(np.float64), ref, 0.99, "reserved views")
     # an unannounced, much closer view needs more sub-image scratch: it grows (and renders correctly)
