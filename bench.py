@@ -442,11 +442,12 @@ def timed_e2e(g, wl, mode, order, K, W, host_bufs, dist=None, pipelined=True):
 
 def traffic_of(workload, mode, tf):
     """DRAM bytes (read + write) of ONE ray-cast launch from the committed `ncu --set full`
-    capture of this workload (profiles/r1_traffic.csv, written from the .ncu-rep files as
-    profiles/r1_traffic.md describes), or None. Quoted, not measured in this run."""
+    capture of this workload (profiles/r2_traffic.csv, written from the .ncu-rep files as
+    profiles/r2_traffic.md describes), or None. QUOTED from that capture of one view, not measured in this run
+    (the line says so: `traffic_source`)."""
     try:
         import csv
-        with open(os.path.join(ROOT, "profiles", "r1_traffic.csv")) as f:
+        with open(os.path.join(ROOT, "profiles", "r2_traffic.csv")) as f:
             for row in csv.DictReader(f):
                 if (row["workload"], row["mode"], row["tf"]) == (workload, mode, tf):
                     return int(row["dram_read_bytes"]) + int(row["dram_write_bytes"])
@@ -477,30 +478,35 @@ def roofline_of(counts, stages, stage_views, peak_gbs, peak_src, traffic=None):
     achieved = alg / (ms * 1e-3) / 1e9
     lines_gbs = lines / (ms * 1e-3) / 1e9
     return {"bound": "hbm", "kernel": "vr_raycast_kernel", "achieved": round(achieved, 1), "peak": peak_gbs, "unit": "GB/s",
-            "frac": round(achieved / peak_gbs, 4), "traffic": traffic, "peak_source": peak_src,
+            "frac": round(achieved / peak_gbs, 4), "traffic": traffic,
+            "traffic_source": "quoted: dram__bytes_read.sum + dram__bytes_write.sum of one launch in the committed ncu --set full capture "
+                              "(profiles/r2_traffic.csv), not measured in this run" if traffic else None,
+            "peak_source": peak_src,
             "algorithmic_bytes_per_launch": round(alg / n), "launch_ms": round(ms / n, 4), "views_counted": n,
             "lines_bytes_per_launch": round(lines / n), "lines_gbs": round(lines_gbs, 1),
             "lines_frac": round(lines_gbs / peak_gbs, 4)}
 
 
-# SASS instructions of one trip of the ray-cast kernel's sample loop (4x4x2 layout, timed instance;
-# counted with `cuobjdump -sass` between the loop head and the backward branch after VOTE.ANY:
-# DESIGN.md "Kernels" lists them by kind). One trip = one sample for each of the warp's 32 rays.
-LOOP_INSTRUCTIONS = {"alpha": 128, "mip": 102}
+# Issued instructions one sample NEEDS, whatever the kernel: ALPHA 8 loads + 7 lerp FMA + 7 differences
+# + 6 position adds + 3 weights + classification (scale, index, fraction, 2 shared loads, 4 FMA) + opacity (2 MUFU, 3 FP) +
+# blending (5 FP) + termination and loop control (~5) = 55; MIP drops classification, opacity and blending: 30.
+ALGORITHMIC_INSTRUCTIONS = {"alpha": 55, "mip": 30}
 SM_COUNT, SCHEDULERS_PER_SM = 148, 4
 
 
 def roofline_alu(gsamples_per_s, mode, sm_mhz, traffic=None):
-    """Issue-slot bound of the sample loop, the bound of DENSELY sampled views (configs 0, 1, 2, 4:
-    >= 0.6 samples per voxel, every line is reused from L1/L2 and DRAM idles): peak = SMs x 4
-    warp schedulers x SM clock issue slots per second, x 32 samples per loop trip / instructions
-    per trip. `frac` therefore = issue-slot utilisation x the fraction of lanes doing a sample."""
+    """Issue-slot bound of the sample loop, the bound of DENSELY sampled views (configs 0, 1, 2, 4: >= 0.6 samples per
+    voxel, every line is reused from L1/L2 and DRAM idles). The peak uses the ALGORITHMIC work of a sample (SURVEY.md sec.
+    8(d): 8 loads, 7 lerps, the position update, one LUT lerp with 2 shared loads, one pow on 2 MUFU, ~8 FMA of blending:
+    50-60 issued instructions; ALGORITHMIC_INSTRUCTIONS = 55 for ALPHA, 30 for MIP, which has no classification, opacity
+    or blending), NOT this kernel's own SASS count: peak = SMs x 4 warp schedulers x max SM clock x 32 lanes / that count.
+    `frac` is then the distance from what the method needs, whatever the sampler (the texture arm issues fewer)."""
     clock = (sm_mhz or 1965.0) * 1e6
-    peak = SM_COUNT * SCHEDULERS_PER_SM * clock * 32.0 / LOOP_INSTRUCTIONS[mode] / 1e9
+    peak = SM_COUNT * SCHEDULERS_PER_SM * clock * 32.0 / ALGORITHMIC_INSTRUCTIONS[mode] / 1e9
     return {"bound": "alu", "kernel": "vr_raycast_kernel", "achieved": round(gsamples_per_s, 2), "peak": round(peak, 1),
             "unit": "Gsamples/s", "frac": round(gsamples_per_s / peak, 4), "traffic": traffic,
-            "peak_source": "%d SMs x %d schedulers x %.0f MHz (max SM clock) x 32 lanes / %d SASS instructions per loop trip" % (
-                SM_COUNT, SCHEDULERS_PER_SM, clock / 1e6, LOOP_INSTRUCTIONS[mode])}
+            "peak_source": "%d SMs x %d schedulers x %.0f MHz (max SM clock) x 32 lanes / %d ALGORITHMIC instructions per sample "
+                           "(SURVEY.md 8(d): 50-60 for ALPHA)" % (SM_COUNT, SCHEDULERS_PER_SM, clock / 1e6, ALGORITHMIC_INSTRUCTIONS[mode])}
 
 
 def measured_peak():
@@ -709,6 +715,7 @@ def run_probe_dram(vr, gib):
     cases = []
 
     def case(flavour, span, group, gran=0, ctas=148 * 8, lpt=256):
+        nonlocal buf
         ms, loads = vr.debug_probe_dram(buf, flavour, span, group, lpt, ctas, gran)
         cases.append({"flavour": vr.PROBE_FLAVOURS[flavour], "span_bytes": span, "group": group, "l2_fetch_granularity": gran or "default",
                       "ctas": ctas, "loads": loads, "ms": round(ms, 4), "gloads_per_s": round(loads / (ms * 1e-3) / 1e9, 2),
@@ -725,6 +732,15 @@ def run_probe_dram(vr, gib):
         case(6, span, group)
     for ctas in (148 * 2, 148 * 4, 148 * 16, 148 * 32):  # memory-level parallelism
         case(1, 128, 1, 0, ctas)
+    # address range: does the miss rate depend on how many 2 MB pages the lines are spread over (TLB reach), beyond what the
+    # L2 hit rate of a smaller range explains? (sub-ranges of the same buffer)
+    whole = buf
+    for mib in (256, 512, 1024, 2048, 4096, 8192):
+        if mib << 20 < whole.numel() * 4:
+            buf = whole[:(mib << 20) // 4]
+            case(1, 128, 1, 0, 148 * 32)
+            cases[-1]["range_mib"] = mib
+    buf = whole
     del buf
     return {"probe": "dram", "buffer_gib": gib, "hbm_peak_gbs": peak, "hbm_peak_source": peak_src, "cases": cases}
 
@@ -922,12 +938,19 @@ def main():
         variants = []
         # sort-last (the headline path) with the other transfer function / mode, then the fused traversal
         # (row f2: one ray through all bricks, global early termination, no sub-images, no compositing)
-        for vmode, vtf, vtrav in (("alpha", "translucent", "sort_last"), ("mip", "ramp", "sort_last"),
-                                  ("alpha", "ramp", "fused"), ("alpha", "translucent", "fused"),
-                                  ("alpha", "threshold", "sort_last"), ("alpha", "threshold", "fused"),
-                                  ("alpha", "ramp, early termination off", "sort_last")):
-            if vtrav == "sort_last" and vmode == args.mode and vtf == args.tf:
+        other = "manual" if args.sampler == "texture" else "texture"  # the other arm of rows a1 / a5, on the same frames
+        for vmode, vtf, vtrav, vsamp in (("alpha", "translucent", "sort_last", args.sampler), ("mip", "ramp", "sort_last", args.sampler),
+                                         ("alpha", "ramp", "sort_last", other), ("alpha", "translucent", "sort_last", other),
+                                         ("alpha", "ramp", "fused", args.sampler), ("alpha", "translucent", "fused", args.sampler),
+                                         ("alpha", "threshold", "sort_last", args.sampler), ("alpha", "threshold", "fused", args.sampler),
+                                         ("alpha", "ramp, early termination off", "sort_last", args.sampler)):
+            if vtrav == "sort_last" and vmode == args.mode and vtf == args.tf and vsamp == args.sampler:
                 vtf = "ramp"
+            try:
+                g.set_sampler(vr.SAMPLER_TEXTURE if vsamp == "texture" else vr.SAMPLER_MANUAL)
+            except vr.VrError as e:  # the 103 GB cube: no room for a second copy of the bricks as 3-D arrays
+                variants.append({"mode": vmode, "tf": vtf, "traversal": vtrav, "sampler": vsamp, "unavailable": str(e)})
+                continue
             noert = vtf.endswith("early termination off")  # the paper's protocol: with and without
             g.set_transfer_function(pick_tf(wl, "ramp" if noert else vtf), *tf_range(wl))
             g.set_early_termination(2.0 if noert else wl["tau"])
@@ -941,7 +964,8 @@ def main():
                 extra = {"frames_per_s_skipping_off": round(K / (ms_off * 1e-3), 3)}
             g.set_traversal(vr.SORT_LAST)
             g.set_early_termination(wl["tau"])
-            variants.append({"mode": vmode, "tf": vtf, "traversal": vtrav, "frames_per_s": round(K / (v["ms"] * 1e-3), 3), **extra,
+            variants.append({"mode": vmode, "tf": vtf, "traversal": vtrav, "sampler": vsamp if vmode == "alpha" and vtrav == "sort_last" else "manual",
+                             "frames_per_s": round(K / (v["ms"] * 1e-3), 3), **extra,
                              "gsamples_per_s": round(v["samples"] / (v["ms"] * 1e-3) / 1e9, 3),
                              "samples_per_frame": int(v["samples"] / K),
                              "stage_ms": {"setup": round(float(v["stages"][:, 0].mean()), 4),
@@ -950,7 +974,16 @@ def main():
                              "roofline": roofline_of(v["counts"], v["stages"], v["stage_views"], peak, peak_src,
                                                      traffic_of(args.workload, vmode, vtf + ("" if vtrav == "sort_last" else "/fused")))})
         g.set_transfer_function(tf, *tf_range(wl))
+        g.set_sampler(vr.SAMPLER_TEXTURE if args.sampler == "texture" else vr.SAMPLER_MANUAL)
         line["variants"] = variants
+        # the workloads the paper's cubes look like (faint sources: PAPER.md:19, :206) beside the opaque ramp: the same
+        # fraction (algorithmic bytes of the ray-cast kernel over its time, of the measured HBM peak) for every variant
+        line["roofline_variants"] = [{"mode": args.mode, "tf": args.tf, "traversal": args.traversal, "sampler": args.sampler,
+                                      "frac": line.get("roofline_hbm", line["roofline"])["frac"],
+                                      "lines_frac": line.get("roofline_hbm", line["roofline"]).get("lines_frac"),
+                                      "frames_per_s": line["value"]}] + [
+            {"mode": v["mode"], "tf": v["tf"], "traversal": v["traversal"], "sampler": v["sampler"], "frac": v["roofline"]["frac"],
+             "lines_frac": v["roofline"].get("lines_frac"), "frames_per_s": v["frames_per_s"]} for v in variants if "roofline" in v]
         if args.sortlast_parts > 1 and args.mode == "alpha":
             line["sortlast"] = sortlast_report(vr, g, wl, cube, tf, args.sortlast_parts, order, K, Wm)
 

@@ -31,7 +31,7 @@ SYMBOLS = (
     "vr_set_transfer_function", "vr_set_early_termination", "vr_volume_minmax", "vr_set_culling", "vr_set_traversal", "vr_set_sampler", "vr_set_allocator", "vr_reserve_views", "vr_debug_brick_minmax", "vr_debug_cell_flags", "vr_render", "vr_render_host", "vr_render_host_async", "vr_render_host_wait", "vr_composite",
     "vr_num_bricks", "vr_debug_brick_order", "vr_debug_rects", "vr_debug_ray_bricks", "vr_debug_subimages",
     "vr_volume_create_part", "vr_render_part", "vr_render_part_pieces", "vr_part_rect", "vr_composite_parts", "vr_kd_partition", "vr_part_order",
-    "vr_set_counting", "vr_set_timing", "vr_debug_stats", "vr_debug_stage_times", "vr_debug_probe_dram", "vr_launch_count", "vr_last_error",
+    "vr_set_counting", "vr_set_timing", "vr_debug_stats", "vr_debug_stage_times", "vr_debug_probe_dram", "vr_debug_set_upload_path", "vr_launch_count", "vr_last_error",
 )
 
 
@@ -101,6 +101,7 @@ def lib():
         L.vr_debug_stats.argtypes = [vp, ctypes.POINTER(Stats)]
         L.vr_debug_stage_times.argtypes = [vp, ci, vp]
         L.vr_debug_probe_dram.argtypes = [vp, ctypes.c_uint64, ci, ci, ci, ci, ci, ci, vp, vp, vp]
+        L.vr_debug_set_upload_path.argtypes = [ci]
         L.vr_launch_count.argtypes = [vp]
         L.vr_launch_count.restype = i64
         L.vr_last_error.argtypes = [vp]
@@ -472,6 +473,12 @@ def part_order(tree, brick, view, proj):
     if rc != 0:
         raise VrError(rc, lib().vr_last_error(None).decode())
     return [int(r) for r in out]
+
+
+def debug_set_upload_path(path):
+    """vr_debug_set_upload_path: 0 = cp.async staging (default), 1 = TMA box loads."""
+    if lib().vr_debug_set_upload_path(int(path)) != 0:
+        raise VrError(1, lib().vr_last_error(None).decode())
 
 
 def composite(layers, rects, order, width, height, out, stream=None):

@@ -473,6 +473,12 @@ extern "C" int vr_volume_download(vr_volume* v, float* dst, int memspace, int x0
     return VR_OK;
 }
 
+extern "C" int vr_debug_set_upload_path(int path) {
+    if (path != 0 && path != 1) return fail(NULL, VR_ERR_INVALID_ARG, "vr_debug_set_upload_path: 0 (cp.async) or 1 (TMA)");
+    vr_set_upload_path(path);
+    return VR_OK;
+}
+
 extern "C" int vr_debug_brick_data(vr_volume* v, int b, float* dst, int* dims) {
     if (!v) return fail(NULL, VR_ERR_INVALID_ARG, "vr_debug_brick_data: NULL handle");
     const VrGrid& g = v->grid;

@@ -259,6 +259,13 @@ vr_download_kernel(VrGrid g, const float* __restrict__ bricks, float* __restrict
     }
 }
 
+static cudaError_t launch_upload_tma(const VrGrid& grid, float* bricks, const float* src, int x0, int y0, int z0, int sx, int sy, int sz,
+                                     int b0, unsigned nby, cudaStream_t st);
+/* 0 = cp.async staging (vr_upload_tile442_kernel, the default: 5.23 TB/s on c3), 1 = TMA box loads (vr_upload_tma442_kernel:
+ * 4.95 TB/s on c3, 4.30 against 4.83 TB/s on c2 - measured round 2, profiles/r2_upload.md); vr_debug_set_upload_path */
+static int g_upload_path = 0;
+void vr_set_upload_path(int path) { g_upload_path = path; }
+
 cudaError_t vr_launch_upload(const VrGrid& grid, float* bricks, const float* src, int x0, int y0, int z0, int sx, int sy,
                              int sz, cudaStream_t st) {
     /* nbricks <= 65535 (checked at create): bricks along grid.y - only those brick z-slabs whose padded
@@ -292,6 +299,11 @@ cudaError_t vr_launch_upload(const VrGrid& grid, float* bricks, const float* src
         }
         const bool t442 = grid.tl[0] == 2 && grid.tl[1] == 2 && grid.tl[2] == 1 && grid.ml[0] == 0 && grid.ml[1] == 0 &&
                           grid.ml[2] == 0;
+        if (t442 && g_upload_path == 1) {
+            const cudaError_t e = launch_upload_tma(grid, bricks, src, x0, y0, z0, sx, sy, sz, b0, nby, st);
+            if (e != cudaErrorNotSupported) return e;
+            cudaGetLastError();
+        }
         if (t442) {
             /* 32 staged rows while six CTAs of them fit an SM's shared memory, else 16 */
             const bool big = smem > 40 * 1024;
@@ -319,5 +331,167 @@ cudaError_t vr_launch_download(const VrGrid& grid, const float* bricks, float* d
     if (blocks > 148 * 32) blocks = 148 * 32;
     if (blocks < 1) blocks = 1;
     vr_download_kernel<<<(unsigned)blocks, 256, 0, st>>>(grid, bricks, dst, x0, y0, z0, sx, sy, sz);
+    return cudaGetLastError();
+}
+
+/* ------------------------------------------------------------------------------------------
+ * TILED 4x4x2, source boxes moved by the TMA unit (cp.async.bulk.tensor, sm_90+): the dense source is described by
+ * a 3-D tensor map; a CTA takes a group of 4 tile rows (16 source rows x 2 planes) of one brick and walks it in
+ * chunks of 128 cells: one elected thread asks for the next chunk's 132 x 16 x 2 box (16.5 KB, out-of-range
+ * coordinates are filled with zeros by the unit and never used) while all threads turn the previous chunk into
+ * micro-tiles, two shared-memory stages, one mbarrier each. Against the cp.async version: no address arithmetic and no
+ * 4-byte requests on the load side - but the unit wants every box to start on a 16-byte boundary of the source row
+ * (a box at x = -1 faults as an illegal instruction), so with one ghost layer the staged rows sit 3 cells askew and
+ * the 16-byte tile rows are gathered with four 4-byte shared loads. Measured (round 2): 5 % SLOWER than the cp.async
+ * kernel on c3 (41.9 against 39.7 ms for 207 GB), 11 % on c2: kept as the alternative behind vr_debug_set_upload_path,
+ * not the default. Needs sx % 4 == 0 and a 16-byte aligned source (the tensor map's strides), else the caller falls back.
+ * ---------------------------------------------------------------------------------------- */
+#include <cuda.h>
+
+#define TMA_BX 128 /* cells per chunk */
+#define TMA_BW (TMA_BX + 4) /* box width: the unit wants the box to start on a 16-byte boundary of the source row, so it starts
+                             * up to 3 cells early (a ghost layer of 1 puts padded cell 0 at voxel -1 mod 4) */
+#define TMA_TR 4   /* tile rows per group: 16 source rows */
+#define TMA_STAGE_FLOATS (TMA_BW * TMA_TR * 4 * 2)
+
+__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long* bar, int count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long* bar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity) {
+    unsigned done = 0;
+    while (!done)
+        asm volatile("{\n\t.reg .pred p;\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\tselp.u32 %0, 1, 0, p;\n\t}"
+                     : "=r"(done)
+                     : "r"(smem_u32(bar)), "r"(parity)
+                     : "memory");
+}
+__device__ __forceinline__ void tma_load_3d(float* dst, const CUtensorMap* tm, unsigned long long* bar, int x, int y, int z) {
+    asm volatile("cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];" ::"r"(
+                     smem_u32(dst)),
+                 "l"(tm), "r"(smem_u32(bar)), "r"(x), "r"(y), "r"(z)
+                 : "memory");
+}
+
+__global__ void __launch_bounds__(256)
+vr_upload_tma442_kernel(VrGrid g, float* __restrict__ bricks, const __grid_constant__ CUtensorMap tm, const float* __restrict__ src,
+                        int x0, int y0, int z0, int sx, int sy, int sz, int b0) {
+    extern __shared__ __align__(128) float s_box_raw[]; /* two stages of [2][16][128] floats, 128-byte aligned by hand */
+    __shared__ __align__(8) unsigned long long s_bar[2];
+    float* s_box = reinterpret_cast<float*>((reinterpret_cast<uintptr_t>(s_box_raw) + 127) & ~(uintptr_t)127);
+    const int b = blockIdx.y + b0;
+    int bc[3], lo[3], hi[3];
+    vr_brick_coords(g, b, bc);
+    vr_brick_core(g, bc, lo, hi);
+    const int ex = hi[0] - lo[0] + 2 * g.ghost, ey = hi[1] - lo[1] + 2 * g.ghost, ez = hi[2] - lo[2] + 2 * g.ghost;
+    int i0, i1, j0, j1, k0, k1;
+    padded_range(lo[0], g.ghost, ex, g.n[0], x0, x0 + sx, i0, i1);
+    padded_range(lo[1], g.ghost, ey, g.n[1], y0, y0 + sy, j0, j1);
+    padded_range(lo[2], g.ghost, ez, g.n[2], z0, z0 + sz, k0, k1);
+    if (i1 <= i0 || j1 <= j0 || k1 <= k0) return;
+    const int slot_b = vr_slot_index(g, b);
+    if (slot_b < 0) return;
+    const int tx0 = i0 >> 2, tx1 = ((i1 - 1) >> 2) + 1;
+    const int ty0 = j0 >> 2, ty1 = ((j1 - 1) >> 2) + 1;
+    const int tz0 = k0 >> 1, tz1 = ((k1 - 1) >> 1) + 1;
+    const int ngy = (ty1 - ty0 + TMA_TR - 1) / TMA_TR, groups = ngy * (tz1 - tz0);
+    const int nchunks = ((tx1 - tx0) * 4 + TMA_BX - 1) / TMA_BX;
+    const int xbase = lo[0] - g.ghost, ybase = lo[1] - g.ghost, zbase = lo[2] - g.ghost; /* global voxel of padded cell 0 */
+    float* __restrict__ dstb = bricks + (long long)slot_b * g.slot;
+    const int xskew = (xbase + (tx0 << 2) - x0) & 3; /* cells between the box's 16-byte aligned start and the chunk's first cell */
+    const int tid = threadIdx.x;
+    if (tid == 0) {
+        mbar_init(&s_bar[0], 1);
+        mbar_init(&s_bar[1], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    /* work units of this CTA: (group, chunk), group = blockIdx.x, blockIdx.x + gridDim.x, ... */
+    const int my_groups = groups > (int)blockIdx.x ? (groups - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x : 0;
+    const int units = my_groups * nchunks;
+    auto issue = [&](int u) {
+        const int grp = (int)blockIdx.x + (u / nchunks) * (int)gridDim.x, c = u % nchunks;
+        const int jf = (ty0 + (grp % ngy) * TMA_TR) << 2, kt = (tz0 + grp / ngy) << 1, ic = (tx0 << 2) + c * TMA_BX;
+        unsigned long long* bar = &s_bar[u & 1];
+        mbar_expect_tx(bar, TMA_STAGE_FLOATS * 4u);
+        tma_load_3d(s_box + (u & 1) * TMA_STAGE_FLOATS, &tm, bar, (xbase + ic - x0) & ~3, ybase + jf - y0, zbase + kt - z0);
+    };
+    if (tid == 0 && units > 0) issue(0);
+    for (int u = 0; u < units; ++u) {
+        if (tid == 0 && u + 1 < units) issue(u + 1); /* its stage was released by the barrier that ended unit u - 1 */
+        mbar_wait(&s_bar[u & 1], (unsigned)((u >> 1) & 1));
+        const int grp = (int)blockIdx.x + (u / nchunks) * (int)gridDim.x, c = u % nchunks;
+        const int tyg = ty0 + (grp % ngy) * TMA_TR, kt = (tz0 + grp / ngy) << 1, ic = (tx0 << 2) + c * TMA_BX;
+        const float* __restrict__ box = s_box + (u & 1) * TMA_STAGE_FLOATS;
+        /* 1024 sixteen-byte tile rows per unit, 4 per thread: a quarter-warp takes 8 consecutive tiles of one row
+         * (conflict-free 128-bit shared loads), a warp the four rows lj of one plane lk of those tiles */
+#pragma unroll
+        for (int n = 0; n < 4; ++n) {
+            const int idx = tid + 256 * n;
+            const int txl = (idx & 7) | (((idx >> 5) & 3) << 3), lj = (idx >> 3) & 3, lk = (idx >> 7) & 1, tr = idx >> 8;
+            const int tx = (ic >> 2) + txl, i = tx << 2, j = ((tyg + tr) << 2) + lj, k = kt + lk;
+            if (tx >= tx1 || tyg + tr >= ty1 || j < j0 || j >= j1 || k < k0 || k >= k1) continue;
+            const float* __restrict__ srow = box + (lk * (TMA_TR * 4) + tr * 4 + lj) * TMA_BW + (txl << 2) + xskew;
+            float* __restrict__ out = dstb + (vr_axis_offset(g.ax[1], j) + vr_axis_offset(g.ax[2], k)) + (tx << 5);
+            /* cells outside the volume replicate the edge voxel (R3): the unit filled them with zeros, so the few rows and
+             * columns on the volume's faces take the clamped voxel straight from the source (it lies in the box: padded_range) */
+            const int gy = ybase + j, gz = zbase + k, gx = xbase + i;
+            const bool edge = gy < 0 || gy >= g.n[1] || gz < 0 || gz >= g.n[2] || gx < 0 || gx + 3 >= g.n[0];
+            if (!edge && i >= i0 && i + 3 < i1) {
+                *reinterpret_cast<float4*>(out) = xskew ? make_float4(srow[0], srow[1], srow[2], srow[3]) : *reinterpret_cast<const float4*>(srow);
+            } else if (!edge) {
+#pragma unroll
+                for (int q = 0; q < 4; ++q)
+                    if (i + q >= i0 && i + q < i1) out[q] = srow[q];
+            } else {
+                const int cy = min(max(gy, 0), g.n[1] - 1), cz = min(max(gz, 0), g.n[2] - 1);
+                const float* __restrict__ grow = src + ((long long)(cz - z0) * sy + (cy - y0)) * sx - x0;
+#pragma unroll
+                for (int q = 0; q < 4; ++q)
+                    if (i + q >= i0 && i + q < i1) out[q] = __ldg(grow + min(max(gx + q, 0), g.n[0] - 1));
+            }
+        }
+        __syncthreads();
+    }
+}
+
+typedef CUresult (*vr_encode_tiled_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                       const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                       CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+/* Returns cudaErrorNotSupported when the source cannot be described by a tensor map (or the driver has no encoder): the
+ * caller then falls back to the cp.async kernel. */
+static cudaError_t launch_upload_tma(const VrGrid& grid, float* bricks, const float* src, int x0, int y0, int z0, int sx, int sy, int sz,
+                                     int b0, unsigned nby, cudaStream_t st) {
+    static vr_encode_tiled_fn encode = NULL;
+    static bool looked = false;
+    if (!looked) {
+        looked = true;
+        void* fn = NULL;
+        cudaDriverEntryPointQueryResult qr;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qr) == cudaSuccess && qr == cudaDriverEntryPointSuccess)
+            encode = (vr_encode_tiled_fn)fn;
+        cudaGetLastError();
+    }
+    if (!encode || (sx & 3) || (((uintptr_t)src) & 15)) return cudaErrorNotSupported;
+    CUtensorMap tm;
+    const cuuint64_t dims[3] = {(cuuint64_t)sx, (cuuint64_t)sy, (cuuint64_t)sz};
+    const cuuint64_t strides[2] = {(cuuint64_t)sx * 4, (cuuint64_t)sx * sy * 4};
+    const cuuint32_t box[3] = {TMA_BW, TMA_TR * 4, 2};
+    const cuuint32_t estr[3] = {1, 1, 1};
+    if (encode(&tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, (void*)src, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+               CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+        return cudaErrorNotSupported;
+    const size_t smem = 2 * TMA_STAGE_FLOATS * sizeof(float) + 128;
+    cudaError_t e = cudaFuncSetAttribute(vr_upload_tma442_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    const long long ty = (((long long)grid.P >> 2) + 1 + TMA_TR - 1) / TMA_TR;
+    const long long tz = (((long long)(sz < grid.P ? sz + 2 * grid.ghost : grid.P)) >> 1) + 2;
+    long long bx = ty * tz;
+    if (bx > 4096) bx = 4096;
+    vr_upload_tma442_kernel<<<dim3((unsigned)bx, nby), 256, smem, st>>>(grid, bricks, tm, src, x0, y0, z0, sx, sy, sz, b0);
     return cudaGetLastError();
 }

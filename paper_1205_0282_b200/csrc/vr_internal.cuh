@@ -219,6 +219,7 @@ cudaError_t vr_launch_composite(const VrCompLayer* layers, const int* order, int
                                 const VrLut& lut, float* out, const int* bound, const int* window, cudaStream_t st);
 cudaError_t vr_launch_upload(const VrGrid& grid, float* bricks, const float* src, int x0, int y0, int z0, int sx,
                              int sy, int sz, cudaStream_t st);
+void vr_set_upload_path(int path); /* 0 cp.async staging, 1 TMA box loads (default where it applies) */
 cudaError_t vr_launch_download(const VrGrid& grid, const float* bricks, float* dst, int x0, int y0, int z0, int sx,
                                int sy, int sz, cudaStream_t st);
 cudaError_t vr_launch_ray_bricks(const VrGrid& grid, const VrViewState* vs, const int* d_pixels, int npix,

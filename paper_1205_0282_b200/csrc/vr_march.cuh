@@ -297,6 +297,23 @@ struct Corners {
     float c000, c001, c010, c011, c100, c101, c110, c111;
 };
 
+/* The voxel load of the 4x4x2 path. VR_LDG_L2_64B (build-time experiment, profiles/r2_c3_experiments.md): the L2::64B
+ * prefetch-size hint halves the DRAM bytes of a miss (probe: 63.8 instead of 127.3 bytes per load) but not the rate at
+ * which misses are served, and the second half of a micro-tile then costs a request of its own. */
+__device__ __forceinline__ float vr_ldg(const float* p) {
+#ifdef VR_LDG_L2_64B
+    float v;
+    asm volatile("ld.global.nc.L1::no_allocate.L2::64B.f32 %0, [%1];" : "=f"(v) : "l"(p));
+    return v;
+#elif defined(VR_LDG_L2_64B_ALLOC)
+    float v;
+    asm volatile("ld.global.nc.L2::64B.f32 %0, [%1];" : "=f"(v) : "l"(p));
+    return v;
+#else
+    return __ldg(p);
+#endif
+}
+
 template <int LAY, int PT, bool CLAMP, bool COUNT>
 __device__ __forceinline__ void fetch8(const float* __restrict__ brick, const VrGrid& g, const int ext[3], const Lattice& L,
                                        unsigned* __restrict__ bitmap, long long brick_cell0, Corners& C) {
@@ -312,14 +329,14 @@ __device__ __forceinline__ void fetch8(const float* __restrict__ brick, const Vr
         const unsigned oy0 = (uy0 << 2) + (uy0 >> 2) * sy, oy1 = (uy1 << 2) + (uy1 >> 2) * sy;
         const unsigned oz0 = (uz0 << 4) + (uz0 >> 1) * sz, oz1 = (uz1 << 4) + (uz1 >> 1) * sz;
         const unsigned r00 = oz0 + oy0, r01 = oz0 + oy1, r10 = oz1 + oy0, r11 = oz1 + oy1;
-        c000 = __ldg(brick + (r00 + ox0));
-        c001 = __ldg(brick + (r00 + ox1));
-        c010 = __ldg(brick + (r01 + ox0));
-        c011 = __ldg(brick + (r01 + ox1));
-        c100 = __ldg(brick + (r10 + ox0));
-        c101 = __ldg(brick + (r10 + ox1));
-        c110 = __ldg(brick + (r11 + ox0));
-        c111 = __ldg(brick + (r11 + ox1));
+        c000 = vr_ldg(brick + (r00 + ox0));
+        c001 = vr_ldg(brick + (r00 + ox1));
+        c010 = vr_ldg(brick + (r01 + ox0));
+        c011 = vr_ldg(brick + (r01 + ox1));
+        c100 = vr_ldg(brick + (r10 + ox0));
+        c101 = vr_ldg(brick + (r10 + ox1));
+        c110 = vr_ldg(brick + (r11 + ox0));
+        c111 = vr_ldg(brick + (r11 + ox1));
         if (COUNT && bitmap) {
             const long long c0 = brick_cell0 + ox0, c1 = brick_cell0 + ox1;
             mark_cell(bitmap, c0 + r00);
