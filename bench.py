@@ -964,7 +964,9 @@ def main():
                 extra = {"frames_per_s_skipping_off": round(K / (ms_off * 1e-3), 3)}
             g.set_traversal(vr.SORT_LAST)
             g.set_early_termination(wl["tau"])
-            variants.append({"mode": vmode, "tf": vtf, "traversal": vtrav, "sampler": vsamp if vmode == "alpha" and vtrav == "sort_last" else "manual",
+            variants.append({"mode": vmode, "tf": vtf, "traversal": vtrav, "sampler": ("manual" if vmode != "alpha" or (vtf == "threshold" and vsamp == "texture") else vsamp) +
+                                        (" (MIP keeps the hand-rolled sampler)" if vmode != "alpha" and vsamp == "texture" else "") +
+                                        (" (a stepped table keeps the hand-rolled sampler)" if vtf == "threshold" and vsamp == "texture" else ""),
                              "frames_per_s": round(K / (v["ms"] * 1e-3), 3), **extra,
                              "gsamples_per_s": round(v["samples"] / (v["ms"] * 1e-3) / 1e9, 3),
                              "samples_per_frame": int(v["samples"] / K),

@@ -1008,8 +1008,7 @@ static int render_frame(vr_volume* v, const float* view, const float* proj, int 
         if (rc) return rc;
         mip_skipping = v->mip_skip_useful;
     }
-    const bool use_tex = v->sampler == VR_SAMPLER_TEXTURE && mode == VR_ALPHA && v->traversal == VR_SORT_LAST && v->counting != 2 &&
-                         v->tf_smooth;
+    const bool use_tex = v->sampler == VR_SAMPLER_TEXTURE && mode == VR_ALPHA && v->counting != 2 && v->tf_smooth;
     if (use_tex) { /* after an upload only */
         rc = ensure_tex(v, st);
         if (rc) return rc;

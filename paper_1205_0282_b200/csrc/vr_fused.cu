@@ -20,7 +20,11 @@
  */
 #include "vr_march.cuh"
 
-template <int MODE, int LAY, bool CLAMP, bool COUNT, bool SKIP>
+#ifndef VR_TEX_DEPTH
+#define VR_TEX_DEPTH 4 /* texture fetches a lane keeps in flight (as in vr_raycast.cu) */
+#endif
+
+template <int MODE, int LAY, bool CLAMP, bool COUNT, bool SKIP, bool TEX>
 __global__ void __launch_bounds__(VR_RAYCAST_THREADS, VR_MIN_CTAS)
 vr_fused_kernel(const VrRaycastParams prm, float4* __restrict__ frame) {
     extern __shared__ float4 s_lut[]; /* (entry, delta) pairs: shading (ALPHA), final colour map (MIP) */
@@ -122,6 +126,67 @@ vr_fused_kernel(const VrRaycastParams prm, float4* __restrict__ frame) {
                 D[0] = D[1] = D[2] = 0;
             }
             int active = n > 0 && !stopped;
+            /* texture arm (vr_set_sampler; vr_raycast.cu has the reasoning): the lanes whose brick holds no blanked voxel
+             * fetch through the brick's texture object - PER LANE here, the rays of a warp may be in different bricks
+             * (the hardware serves the distinct objects of a warp one after the other) - VR_TEX_DEPTH fetches in flight;
+             * the others fall through to the hand-rolled loop below */
+            if (TEX && MODE == VR_ALPHA) {
+                const bool use_tex = owned && __ldg(prm.tex_nan + slot_b) == 0;
+                const cudaTextureObject_t tex = use_tex ? __ldg(prm.tex + slot_b) : 0;
+                const double h = 1.0 / 4294967296.0;
+                float P0x = (float)((double)L.q[0] * h + 0.5), P0y = (float)((double)L.q[1] * h + 0.5), P0z = (float)((double)L.q[2] * h + 0.5);
+                float Dfx = (float)((double)D[0] * h), Dfy = (float)((double)D[1] * h), Dfz = (float)((double)D[2] * h);
+                asm volatile("" : "+f"(P0x), "+f"(P0y), "+f"(P0z), "+f"(Dfx), "+f"(Dfy), "+f"(Dfz));
+                const int n0 = n;
+                int tactive = active && use_tex;
+                const unsigned* __restrict__ tbits = SKIP ? prm.cell_bits + (long long)slot_b * prm.cell_words : NULL;
+                int tpm = -1;
+                bool ttransp = false;
+                while (__any_sync(FULL_MASK, tactive)) {
+                    if (tactive) {
+                        if (SKIP) { /* macro-cell look-ups need the lattice: one sample per trip */
+                            const int cx = (int)(L.q[0] >> 32), cy = (int)(L.q[1] >> 32), cz = (int)(L.q[2] >> 32);
+                            const int m = ((cz >> 3) * prm.nc[1] + (cy >> 3)) * prm.nc[0] + (cx >> 3);
+                            if (m != tpm) {
+                                tpm = m;
+                                ttransp = (__ldg(tbits + (m >> 5)) >> (m & 31)) & 1u;
+                            }
+                            int adv = 1;
+                            if (ttransp) {
+                                adv = leap_steps(L, D, n);
+                            } else {
+                                const float kf = (float)(n0 - n);
+                                const float v = tex3D<float>(tex, fmaf(kf, Dfx, P0x), fmaf(kf, Dfy, P0y), fmaf(kf, Dfz, P0z));
+                                if (COUNT) nsamples += (v == v) ? 1 : 0;
+                                shade_alpha(acc, v, stepf, lut, prm.lut);
+                                stopped = !(acc.a < tau);
+                            }
+                            L.q[0] += D[0] * adv, L.q[1] += D[1] * adv, L.q[2] += D[2] * adv;
+                            n -= adv;
+                            tactive = n > 0 && !stopped;
+                        } else {
+                            const float kf = (float)(n0 - n);
+                            float vq[VR_TEX_DEPTH];
+#pragma unroll
+                            for (int u = 0; u < VR_TEX_DEPTH; ++u) {
+                                const float ku = kf + (float)u;
+                                vq[u] = tex3D<float>(tex, fmaf(ku, Dfx, P0x), fmaf(ku, Dfy, P0y), fmaf(ku, Dfz, P0z));
+                            }
+#pragma unroll
+                            for (int u = 0; u < VR_TEX_DEPTH; ++u) {
+                                if (tactive) {
+                                    if (COUNT) nsamples += (vq[u] == vq[u]) ? 1 : 0;
+                                    shade_alpha(acc, vq[u], stepf, lut, prm.lut);
+                                    stopped = !(acc.a < tau);
+                                    --n;
+                                    tactive = n > 0 && !stopped;
+                                }
+                            }
+                        }
+                    }
+                }
+                if (use_tex) active = 0; /* done (n == 0 or stopped); the other lanes still have their samples to take */
+            }
             Corners C;
             int pcx = INT_MIN, pcy = 0, pcz = 0;
             /* R19: samples based in a transparent macro-cell are skipped (see vr_raycast.cu) */
@@ -227,26 +292,22 @@ vr_fused_kernel(const VrRaycastParams prm, float4* __restrict__ frame) {
     }
 }
 
-template <int MODE, int LAY, bool CLAMP, bool COUNT, bool SKIP = false>
+template <int MODE, int LAY, bool CLAMP, bool COUNT, bool SKIP = false, bool TEX = false>
 static cudaError_t launch_fused(const VrRaycastParams& p, float* frame, long long items, cudaStream_t st) {
-    static int sms = 0, cached_per_sm = 0;
-    static size_t cached_smem = (size_t)-1;
     const size_t smem = 2 * sizeof(float4) * (size_t)p.lut.n;
-    if (smem != cached_smem) {
-        int dev = 0;
-        cudaError_t e = cudaGetDevice(&dev);
-        if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-        if (e == cudaSuccess)
-            e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&cached_per_sm, vr_fused_kernel<MODE, LAY, CLAMP, COUNT, SKIP>,
-                                                              VR_RAYCAST_THREADS, smem);
-        if (e != cudaSuccess) return e;
-        if (cached_per_sm < 1) return cudaErrorLaunchOutOfResources;
-        cached_smem = smem;
-    }
+    /* asked of the runtime at every launch (a few microseconds): no process-wide cache to go stale across devices or threads */
+    int dev = 0, sms = 0, cached_per_sm = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+    if (e == cudaSuccess)
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&cached_per_sm, vr_fused_kernel<MODE, LAY, CLAMP, COUNT, SKIP, TEX>,
+                                                          VR_RAYCAST_THREADS, smem);
+    if (e != cudaSuccess) return e;
+    if (cached_per_sm < 1) return cudaErrorLaunchOutOfResources;
     long long ctas = (long long)sms * cached_per_sm;
     const long long want = (items + (VR_RAYCAST_THREADS / 32) - 1) / (VR_RAYCAST_THREADS / 32);
     if (ctas > want) ctas = want < 1 ? 1 : want;
-    vr_fused_kernel<MODE, LAY, CLAMP, COUNT, SKIP><<<(int)ctas, VR_RAYCAST_THREADS, smem, st>>>(p, reinterpret_cast<float4*>(frame));
+    vr_fused_kernel<MODE, LAY, CLAMP, COUNT, SKIP, TEX><<<(int)ctas, VR_RAYCAST_THREADS, smem, st>>>(p, reinterpret_cast<float4*>(frame));
     return cudaGetLastError();
 }
 
@@ -259,6 +320,11 @@ static cudaError_t launch_fused_mode(const VrRaycastParams& p, float* frame, lon
     if (g.layout == VR_LAYOUT_LINEAR)
         return clamp ? launch_fused<MODE, LAY_LINEAR, true, COUNT>(p, frame, items, st)
                      : launch_fused<MODE, LAY_LINEAR, false, COUNT>(p, frame, items, st);
+    if (t442 && MODE == VR_ALPHA && p.tex != NULL && p.bitmap == NULL) { /* texture arm (vr_set_sampler): VR_ALPHA only */
+        if (!clamp && p.cell_bits != NULL) return launch_fused<VR_ALPHA, LAY_TILE442, false, COUNT, true, true>(p, frame, items, st);
+        return clamp ? launch_fused<VR_ALPHA, LAY_TILE442, true, COUNT, false, true>(p, frame, items, st)
+                     : launch_fused<VR_ALPHA, LAY_TILE442, false, COUNT, false, true>(p, frame, items, st);
+    }
     if (t442) {
         if (!clamp && (MODE == VR_ALPHA ? p.cell_bits != NULL : p.cell_mm != NULL)) /* R19: macro-cell skipping */
             return launch_fused<MODE, LAY_TILE442, false, COUNT, true>(p, frame, items, st);

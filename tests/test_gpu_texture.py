@@ -148,3 +148,47 @@ def test_texture_arm_keeps_stepped_tables_on_the_hand_rolled_path_and_errors(vr)
     assert e.value.status == 4
     with pytest.raises(vr.VrError):
         g.set_sampler(7)
+
+
+@pytest.mark.parametrize("tau", [0.99, 2.0])
+def test_fused_traversal_through_the_texture_arm(vr, tau):
+    """Row f2 with the texture sampler: one ray through all bricks, per-lane texture objects (the rays of a warp may be
+    in different bricks), against the oracle holding the cube in ONE brick (R17); early termination off: exactly the
+    hand-rolled path's sample count. A brick with blanked voxels takes the hand-rolled loop inside the same kernel."""
+    import torch
+    cube = synth.Cube(51, 100, 90, 70, 12)
+    data = cube.fill_host()
+    tf = synth.tf_translucent() if tau > 1 else synth.tf_ramp()
+    g, _ = tex_pair(vr, cube, 32, 1, tf=tf, tau=tau, data=data)
+    one = oracle.Volume(cube.nx, cube.ny, cube.nz, 128, 1, data=data)
+    one.set_transfer_function(tf, synth.TF_VMIN, synth.TF_VMAX)
+    one.set_early_termination(tau)
+    one.set_ert_margin(TEX_MARGIN)
+    W, H = 203, 117
+    fr = synth.Framing(cube.nx, cube.ny, cube.nz, W, H)
+    g.set_traversal(vr.FUSED)
+    g.set_counting(1)
+    for k, ortho in ((0, False), (1, True)):
+        view, proj = fr.seeded(77, k), fr.proj(ortho)
+        ref = one.render(view, proj, W, H, 0.5, oracle.ALPHA)
+        img = gpu_frame(g, view, proj, W, H, 0.5, vr.ALPHA)
+        n_tex = g.debug_stats()["samples"]
+        check_alpha(img, ref, tau, "fused texture view %d" % k, envelope=True, max_flagged=1.0)
+        if tau > 1:
+            assert n_tex == int(ref["counts"][..., 0].sum())
+        g.set_sampler(vr.SAMPLER_MANUAL)
+        man = gpu_frame(g, view, proj, W, H, 0.5, vr.ALPHA)
+        g.set_sampler(vr.SAMPLER_TEXTURE)
+        assert 1e-7 < np.abs(man - img).max() < 0.02
+    # blanked voxels in two bricks: those bricks are sampled by hand, the rest through the arrays, in one frame
+    d2 = data.copy()
+    d2[5:20, 40:60, 10:30] = np.nan
+    g.upload(torch.from_numpy(d2).cuda())
+    one2 = oracle.Volume(cube.nx, cube.ny, cube.nz, 128, 1, data=d2)
+    one2.set_transfer_function(tf, synth.TF_VMIN, synth.TF_VMAX)
+    one2.set_early_termination(tau)
+    one2.set_ert_margin(TEX_MARGIN)
+    ref = one2.render(view, proj, W, H, 0.5, oracle.ALPHA)
+    img = gpu_frame(g, view, proj, W, H, 0.5, vr.ALPHA)
+    assert np.isfinite(img).all()
+    check_alpha(img, ref, tau, "fused texture, blanked box", envelope=True, max_flagged=1.0)
