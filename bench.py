@@ -906,7 +906,8 @@ def main():
                          "min": round(float(m["stages"].sum(axis=1).min()), 4),
                          "max": round(float(m["stages"].sum(axis=1).max()), 4), "views": int(len(m["stages"]))},
             "roofline": roofline_of(m["counts"], m["stages"], m["stage_views"], peak, peak_src,
-                                    traffic_of(args.workload, args.mode, args.tf + ("" if args.traversal == "sort_last" else "/fused"))),
+                                    traffic_of(args.workload, args.mode, args.tf + ("" if args.traversal == "sort_last" else "/fused") +
+                                               ("/texture" if args.sampler == "texture" and args.mode == "alpha" else ""))),
             "build_s": round(t_build, 1), "upload": dict(g.upload_stats, frac_of_hbm_peak=round(g.upload_stats["gb_per_s"] / peak, 4)),
             "minmax": dict(g.minmax_stats, frac_of_hbm_peak=round(g.minmax_stats["gb_per_s"] / peak, 4))}
     # which roofline bounds the ray-cast kernel: DRAM for the sparsely sampled 103 GB cube (0.03 samples per
@@ -974,7 +975,8 @@ def main():
                                           "raycast": round(float(v["stages"][:, 1].mean()), 4),
                                           "composite": round(float(v["stages"][:, 2].mean()), 4)},
                              "roofline": roofline_of(v["counts"], v["stages"], v["stage_views"], peak, peak_src,
-                                                     traffic_of(args.workload, vmode, vtf + ("" if vtrav == "sort_last" else "/fused")))})
+                                                     traffic_of(args.workload, vmode, vtf + ("" if vtrav == "sort_last" else "/fused") +
+                                                                ("/texture" if vsamp == "texture" and vmode == "alpha" and vtf != "threshold" else "")))})
         g.set_transfer_function(tf, *tf_range(wl))
         g.set_sampler(vr.SAMPLER_TEXTURE if args.sampler == "texture" else vr.SAMPLER_MANUAL)
         line["variants"] = variants
