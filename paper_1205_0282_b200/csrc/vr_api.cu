@@ -1016,7 +1016,10 @@ static int render_frame(vr_volume* v, const float* view, const float* proj, int 
     if (timing) VR_CUDA(v, cudaEventRecord(ev[0], st));
     rc = run_setup(v, view, proj, width, height, mode, v->culling, st);
     if (rc) return rc;
-    if (v->traversal == VR_SORT_LAST) { /* the per-ray part of row a4, once per pixel: part of the set-up stage */
+    /* brick faces of brick^2 voxels project onto sub_px pixels in all: > 4 voxels per pixel = sparse */
+    const bool sparse = (double)v->grid.nown * v->grid.brick * v->grid.brick > 4.0 * (double)sub_px;
+    const bool ray_table = v->traversal == VR_SORT_LAST && !sparse;
+    if (ray_table) { /* the per-ray part of row a4, once per pixel: part of the set-up stage (dense views only) */
         VR_CUDA(v, vr_launch_rays(v->grid, v->d_vs, width, height, (double)step, v->d_rays, st));
         v->launches++;
     }
@@ -1025,7 +1028,7 @@ static int render_frame(vr_volume* v, const float* view, const float* proj, int 
     VrRaycastParams p;
     p.grid = v->grid;
     p.bricks = v->bricks;
-    p.rays = v->d_rays;
+    p.rays = ray_table ? v->d_rays : NULL;
     p.ray_plane = (long long)width * height;
     p.vs = v->d_vs;
     p.bv = v->d_bv;
@@ -1053,8 +1056,6 @@ static int render_frame(vr_volume* v, const float* view, const float* proj, int 
         v->launches++;
         if (timing) VR_CUDA(v, cudaEventRecord(ev[2], st));
     } else {
-        /* brick faces of brick^2 voxels project onto sub_px pixels in all: > 4 voxels per pixel = sparse */
-        const bool sparse = (double)v->grid.nown * v->grid.brick * v->grid.brick > 4.0 * (double)sub_px;
         VR_CUDA(v, vr_launch_raycast(p, items, v->counting != 0, sparse, st));
         v->launches++;
         if (timing) VR_CUDA(v, cudaEventRecord(ev[2], st));

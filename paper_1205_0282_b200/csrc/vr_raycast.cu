@@ -41,7 +41,11 @@
 #define VR_TEX_COPIES 8 /* copies of the table in the texture-arm instances (more CTAs per SM: less room for each) */
 #endif
 
-template <int MODE, int LAY, int PT, bool CLAMP, bool COUNT, bool SKIP, bool TEX>
+/* RAYTAB: every (ray, brick) segment starts from the frame's ray table (vr_rays.cu) - the dense views' choice: a quarter
+ * of c2's instructions were the per-segment FP64 ray set-up. Sparse views (the 103 GB cube) are bound by DRAM requests,
+ * not by issue slots: there the table's kernel (0.017 ms) costs more than it saves (0.002 ms), so their instances keep
+ * the set-up inside (RAYTAB = false, prm.rays == NULL). The values are the same bit for bit either way. */
+template <int MODE, int LAY, int PT, bool CLAMP, bool COUNT, bool SKIP, bool TEX, bool RAYTAB>
 __global__ void __launch_bounds__(VR_RAYCAST_THREADS, TEX ? VR_TEX_CTAS : VR_MIN_CTAS)
 vr_raycast_kernel(const VrRaycastParams prm) {
     /* dynamic (ALPHA): the table, `copies` times (vr_march.cuh): 32 KB at most; what it does not take stays L1 cache */
@@ -49,6 +53,8 @@ vr_raycast_kernel(const VrRaycastParams prm) {
 
     const VrGrid& g = prm.grid;
     const int lane = threadIdx.x & 31;
+    __shared__ double s_minv[16];
+    if (!RAYTAB && threadIdx.x < 16) s_minv[threadIdx.x] = prm.vs->Minv[threadIdx.x];
     const int copies = prm.lut_copies;
     if (MODE == VR_ALPHA) {
         for (int i = threadIdx.x; i < prm.lut.n * copies; i += blockDim.x) s_lut[i] = prm.lut.base[i / copies];
@@ -111,7 +117,8 @@ vr_raycast_kernel(const VrRaycastParams prm) {
         int k_lo = 0, k_hi = 0;
         const long long ray_p = (long long)pj * W + pi;
         if (in_rect) {
-            ray_load<true>(prm.rays, prm.ray_plane, ray_p, prm.step, ray);
+            if (RAYTAB) ray_load<true>(prm.rays, prm.ray_plane, ray_p, prm.step, ray);
+            else ray_setup(s_minv, W, H, pi, pj, g, prm.step, ray);
             brick_range(ray, g, bc, blo, bhi, k_lo, k_hi);
         }
         /* lattice samples: k in [k_lo, k_lat); samples k >= K-2 (whose interval may be clipped
@@ -276,9 +283,15 @@ vr_raycast_kernel(const VrRaycastParams prm) {
         if (__any_sync(FULL_MASK, k_tail < k_hi && !stopped)) {
 #if VR_RECOMPUTE_TAIL
             if (k_tail < k_hi && !stopped) {
-                long long q = ray_p; /* an opaque copy: the ray is read again, not kept in registers through the loop */
-                asm volatile("" : "+l"(q));
-                ray_load<false>(prm.rays, prm.ray_plane, q, prm.step, ray);
+                if (RAYTAB) {
+                    long long q = ray_p; /* an opaque copy: the ray is read again, not kept in registers through the loop */
+                    asm volatile("" : "+l"(q));
+                    ray_load<false>(prm.rays, prm.ray_plane, q, prm.step, ray);
+                } else {
+                    int qi = pi, qj = pj; /* opaque copies: the ray is rebuilt, not kept in registers */
+                    asm volatile("" : "+r"(qi), "+r"(qj));
+                    ray_setup(s_minv, W, H, qi, qj, g, prm.step, ray);
+                }
             }
 #endif
             for (int k = k_tail; k < k_hi && !stopped; ++k) {
@@ -318,8 +331,17 @@ vr_raycast_kernel(const VrRaycastParams prm) {
 /* ------------------------------------------------------------------------------------------ */
 /* Persistent grid: resident CTAs per SM (for this instance and its shared memory) x SMs,
  * but no more CTAs than there are groups of 8 work items. */
+template <int MODE, int LAY, int PT, bool CLAMP, bool COUNT, bool SKIP, bool TEX, bool RAYTAB>
+static cudaError_t launch_instance(const VrRaycastParams& p0, long long items, bool sparse, cudaStream_t st);
+
 template <int MODE, int LAY, int PT, bool CLAMP, bool COUNT, bool SKIP = false, bool TEX = false>
-static cudaError_t launch_variant(const VrRaycastParams& p0, long long items, bool sparse, cudaStream_t st) {
+static cudaError_t launch_variant(const VrRaycastParams& p, long long items, bool sparse, cudaStream_t st) {
+    return p.rays ? launch_instance<MODE, LAY, PT, CLAMP, COUNT, SKIP, TEX, true>(p, items, sparse, st)
+                  : launch_instance<MODE, LAY, PT, CLAMP, COUNT, SKIP, TEX, false>(p, items, sparse, st);
+}
+
+template <int MODE, int LAY, int PT, bool CLAMP, bool COUNT, bool SKIP, bool TEX, bool RAYTAB>
+static cudaError_t launch_instance(const VrRaycastParams& p0, long long items, bool sparse, cudaStream_t st) {
     VrRaycastParams p = p0;
     p.lut_copies = vr_lut_copies(p.lut.n, sparse);
     if (TEX && p.lut_copies > VR_TEX_COPIES) p.lut_copies = VR_TEX_COPIES;
@@ -330,7 +352,7 @@ static cudaError_t launch_variant(const VrRaycastParams& p0, long long items, bo
     cudaError_t e = cudaGetDevice(&dev);
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     if (e == cudaSuccess)
-        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&cached_per_sm, vr_raycast_kernel<MODE, LAY, PT, CLAMP, COUNT, SKIP, TEX>,
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&cached_per_sm, vr_raycast_kernel<MODE, LAY, PT, CLAMP, COUNT, SKIP, TEX, RAYTAB>,
                                                           VR_RAYCAST_THREADS, smem);
     if (e != cudaSuccess) return e;
     if (cached_per_sm < 1) return cudaErrorLaunchOutOfResources;
@@ -341,7 +363,7 @@ static cudaError_t launch_variant(const VrRaycastParams& p0, long long items, bo
     long long ctas = (long long)sms * per_sm;
     const long long want = (items + (VR_RAYCAST_THREADS / 32) - 1) / (VR_RAYCAST_THREADS / 32);
     if (ctas > want) ctas = want < 1 ? 1 : want;
-    vr_raycast_kernel<MODE, LAY, PT, CLAMP, COUNT, SKIP, TEX><<<(int)ctas, VR_RAYCAST_THREADS, smem, st>>>(p);
+    vr_raycast_kernel<MODE, LAY, PT, CLAMP, COUNT, SKIP, TEX, RAYTAB><<<(int)ctas, VR_RAYCAST_THREADS, smem, st>>>(p);
     return cudaGetLastError();
 }
 
