@@ -70,7 +70,10 @@ enum { VR_HOST = 0, VR_DEVICE = 1 }; /* memory space of a data pointer */
  * neighbourhoods of consecutive samples of a ray fall into few lines. DEFAULT = TILED (the
  * faster one on every config measured, see DESIGN.md and profiles/). Results do not depend
  * on the layout. */
-enum { VR_LAYOUT_DEFAULT = 0, VR_LAYOUT_LINEAR = 1, VR_LAYOUT_TILED = 2 };
+enum { VR_LAYOUT_DEFAULT = 0, VR_LAYOUT_LINEAR = 1, VR_LAYOUT_TILED = 2,
+       /* TILED, with the store's memory mapped brick by brick (CUDA virtual memory management) so that
+        * vr_volume_release_store can hand it back; identical to TILED for every other call */
+       VR_LAYOUT_TILED_RELEASABLE = 3 };
 
 typedef struct vr_volume vr_volume; /* opaque */
 
@@ -277,6 +280,16 @@ int vr_set_traversal(vr_volume* v, int traversal);
 #define VR_SAMPLER_MANUAL 0
 #define VR_SAMPLER_TEXTURE 1
 int vr_set_sampler(vr_volume* v, int sampler);
+
+/* The texture arm for cubes whose second copy does not fit beside the store (the 103 GB cube).
+ * On a handle created with VR_LAYOUT_TILED_RELEASABLE and filled: computes the range tables (rows f1, R19) if they are
+ * stale, then, brick by brick, creates the brick's 3-D array, fills it from the float32 store and gives the brick's
+ * float32 cells back to the device (peak memory: the store plus one array). Bricks that hold blanked (NaN) voxels keep
+ * their float32 cells, because R14 needs them. Afterwards the handle renders VR_ALPHA frames (both traversals) through the
+ * texture arm only: vr_volume_upload / download, VR_MIP frames, counting mode 2 and transfer functions with a step
+ * return VR_ERR_STATE. Irreversible; synchronises. freed_bytes_out (host, may be NULL): device memory given back.
+ * Errors: VR_ERR_STATE (not a releasable handle, nothing uploaded, already released), VR_ERR_OUT_OF_MEMORY, VR_ERR_CUDA. */
+int vr_volume_release_store(vr_volume* v, int64_t* freed_bytes_out, void* stream);
 
 /* Same frame, delivered to HOST memory: renders into a library-owned device frame, copies it
  * to out_rgba_host ([height][width][4] float32; pinned memory makes the copy asynchronous

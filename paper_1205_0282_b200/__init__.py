@@ -18,7 +18,7 @@ SORT_LAST, FUSED = 0, 1
 SAMPLER_MANUAL, SAMPLER_TEXTURE = 0, 1
 STEP_AUTO = 0.0  # vr_render step: the paper's per-ray step (R18)
 HOST, DEVICE = 0, 1
-LAYOUT_DEFAULT, LAYOUT_LINEAR, LAYOUT_TILED = 0, 1, 2
+LAYOUT_DEFAULT, LAYOUT_LINEAR, LAYOUT_TILED, LAYOUT_TILED_RELEASABLE = 0, 1, 2, 3
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libvr.so")
@@ -28,7 +28,7 @@ STATUS = {0: "VR_OK", 1: "VR_ERR_INVALID_ARG", 2: "VR_ERR_OUT_OF_MEMORY", 3: "VR
 # every symbol include/vr.h declares (tests check the library exports each of them)
 SYMBOLS = (
     "vr_volume_create", "vr_volume_create_layout", "vr_volume_destroy", "vr_volume_upload", "vr_volume_download", "vr_debug_brick_data",
-    "vr_set_transfer_function", "vr_set_early_termination", "vr_volume_minmax", "vr_set_culling", "vr_set_traversal", "vr_set_sampler", "vr_set_allocator", "vr_reserve_views", "vr_debug_brick_minmax", "vr_debug_cell_flags", "vr_render", "vr_render_host", "vr_render_host_async", "vr_render_host_wait", "vr_composite",
+    "vr_set_transfer_function", "vr_set_early_termination", "vr_volume_minmax", "vr_set_culling", "vr_set_traversal", "vr_set_sampler", "vr_volume_release_store", "vr_set_allocator", "vr_reserve_views", "vr_debug_brick_minmax", "vr_debug_cell_flags", "vr_render", "vr_render_host", "vr_render_host_async", "vr_render_host_wait", "vr_composite",
     "vr_num_bricks", "vr_debug_brick_order", "vr_debug_rects", "vr_debug_ray_bricks", "vr_debug_subimages",
     "vr_volume_create_part", "vr_render_part", "vr_render_part_pieces", "vr_part_rect", "vr_composite_parts", "vr_kd_partition", "vr_part_order",
     "vr_set_counting", "vr_set_timing", "vr_debug_stats", "vr_debug_stage_times", "vr_debug_probe_dram", "vr_debug_set_upload_path", "vr_launch_count", "vr_last_error",
@@ -75,6 +75,7 @@ def lib():
         L.vr_set_culling.argtypes = [vp, ci]
         L.vr_set_traversal.argtypes = [vp, ci]
         L.vr_set_sampler.argtypes = [vp, ci]
+        L.vr_volume_release_store.argtypes = [vp, vp, vp]
         L.vr_set_allocator.argtypes = [vp, vp, vp]
         L.vr_reserve_views.argtypes = [vp, vp, vp, ci, ci, ci]
         L.vr_debug_brick_minmax.argtypes = [vp, vp]
@@ -267,6 +268,14 @@ class Volume:
         """SAMPLER_MANUAL (hand-rolled float32 tri-linear, the default) or SAMPLER_TEXTURE (3-D CUDA arrays behind
         texture objects for ALPHA frames; allocates a second copy of the bricks)."""
         self._check(lib().vr_set_sampler(self._h, int(sampler)))
+
+    def release_store(self, stream=None):
+        """vr_volume_release_store (handles created with layout=LAYOUT_TILED_RELEASABLE): the bricks become 3-D arrays one by
+        one and their float32 cells go back to the device; ALPHA frames through the texture arm only afterwards. Returns
+        the bytes given back."""
+        freed = ctypes.c_int64()
+        self._check(lib().vr_volume_release_store(self._h, ctypes.byref(freed), _stream(stream)))
+        return int(freed.value)
 
     def debug_brick_minmax(self):
         """[nbricks][2] float32: (min, max) per brick over its ghost-padded cells."""

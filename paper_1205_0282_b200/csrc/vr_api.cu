@@ -60,6 +60,8 @@ struct vr_volume {
     int sampler;             /* VR_SAMPLER_MANUAL or VR_SAMPLER_TEXTURE */
     VrTexStore* tex;         /* texture arm of the store (allocated by vr_set_sampler) */
     bool tex_valid;          /* the arrays hold the current contents of the store */
+    VrVmm* vmm;              /* VR_LAYOUT_TILED_RELEASABLE: the store's physical memory, one chunk per slot */
+    bool store_released;     /* vr_volume_release_store ran: only bricks with blanked voxels still have float32 cells */
     int traversal;           /* VR_SORT_LAST or VR_FUSED */
     int counting;            /* 0 off, 1 samples, 2 samples + touched-cells bitmap */
     bool timing;
@@ -141,7 +143,8 @@ extern "C" int64_t vr_launch_count(const vr_volume* v) { return v ? v->launches 
 static void release(vr_volume* v) {
     vr_tex_destroy(v->tex);
     if (v->h_overflow) cudaFreeHost(v->h_overflow);
-    v_free(v, v->bricks);
+    if (v->vmm) vr_vmm_destroy(v->vmm);
+    else v_free(v, v->bricks);
     v_free(v, v->d_lut_base);
     v_free(v, v->d_lut_delta);
     v_free(v, v->d_vs);
@@ -245,9 +248,11 @@ static int create_volume(int nx, int ny, int nz, int brick, int ghost, int layou
     if (nx <= 0 || ny <= 0 || nz <= 0) return fail(NULL, VR_ERR_INVALID_ARG, "vr_volume_create: non-positive size %dx%dx%d", nx, ny, nz);
     if (brick < 2) return fail(NULL, VR_ERR_INVALID_ARG, "vr_volume_create: brick %d < 2", brick);
     if (ghost < 0 || ghost > 8) return fail(NULL, VR_ERR_INVALID_ARG, "vr_volume_create: ghost %d outside [0,8]", ghost);
-    if (layout != VR_LAYOUT_DEFAULT && layout != VR_LAYOUT_LINEAR && layout != VR_LAYOUT_TILED)
+    if (layout != VR_LAYOUT_DEFAULT && layout != VR_LAYOUT_LINEAR && layout != VR_LAYOUT_TILED && layout != VR_LAYOUT_TILED_RELEASABLE)
         return fail(NULL, VR_ERR_INVALID_ARG, "vr_volume_create_layout: unknown layout %d", layout);
-    if (layout == VR_LAYOUT_DEFAULT) layout = VR_LAYOUT_TILED;
+    const bool releasable = layout == VR_LAYOUT_TILED_RELEASABLE;
+    if (layout == VR_LAYOUT_DEFAULT || releasable) layout = VR_LAYOUT_TILED;
+    if (releasable && g_alloc_fn) return fail(NULL, VR_ERR_STATE, "vr_volume_create_layout: a releasable store maps its own memory (vr_set_allocator is in force)");
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
         cudaGetLastError();
@@ -331,7 +336,17 @@ static int create_volume(int nx, int ny, int nz, int brick, int ghost, int layou
     v->free_fn = g_free_fn;
     v->alloc_user = g_alloc_user;
 
-    cudaError_t e = v_alloc(v, &v->bricks, (size_t)g.slot * (size_t)g.nown * sizeof(float));
+    cudaError_t e;
+    if (releasable) {
+        e = vr_vmm_create((size_t)g.slot * sizeof(float), g.nown, &v->vmm, &v->bricks);
+        if (e == cudaErrorNotSupported) {
+            cudaGetLastError();
+            delete v;
+            return fail(NULL, VR_ERR_CUDA, "vr_volume_create_layout: no CUDA virtual memory management on this device or driver");
+        }
+    } else {
+        e = v_alloc(v, &v->bricks, (size_t)g.slot * (size_t)g.nown * sizeof(float));
+    }
     if (e == cudaSuccess) e = cudaMemset(v->bricks, 0, (size_t)g.slot * (size_t)g.nown * sizeof(float));
     if (e == cudaSuccess) e = v_alloc(v, &v->d_lut_base, VR_MAX_LUT * sizeof(float4));
     if (e == cudaSuccess) e = v_alloc(v, &v->d_lut_delta, VR_MAX_LUT * sizeof(float4));
@@ -413,6 +428,7 @@ extern "C" int vr_volume_upload(vr_volume* v, const float* src, int memspace, in
                                 void* stream) {
     int rc = check_box(v, "vr_volume_upload", src, memspace, x0, y0, z0, sx, sy, sz);
     if (rc) return rc;
+    if (v->store_released) return fail(v, VR_ERR_STATE, "vr_volume_upload: the float32 store was released (vr_volume_release_store)");
     cudaStream_t st = (cudaStream_t)stream;
     if (memspace == VR_DEVICE) {
         VR_CUDA(v, vr_launch_upload(v->grid, v->bricks, src, x0, y0, z0, sx, sy, sz, st));
@@ -443,6 +459,7 @@ extern "C" int vr_volume_download(vr_volume* v, float* dst, int memspace, int x0
                                   void* stream) {
     int rc = check_box(v, "vr_volume_download", dst, memspace, x0, y0, z0, sx, sy, sz);
     if (rc) return rc;
+    if (v->store_released) return fail(v, VR_ERR_STATE, "vr_volume_download: the float32 store was released (vr_volume_release_store)");
     if (v->grid.part) { /* a part can return voxels of its own bricks only */
         const VrGrid& g = v->grid;
         const int lo[3] = {x0, y0, z0}, hi[3] = {x0 + sx, y0 + sy, z0 + sz};
@@ -484,6 +501,7 @@ extern "C" int vr_debug_brick_data(vr_volume* v, int b, float* dst, int* dims) {
     const VrGrid& g = v->grid;
     if (b < 0 || b >= g.nbricks || !dims) return fail(v, VR_ERR_INVALID_ARG, "vr_debug_brick_data: bad brick %d or NULL dims", b);
     if (vr_slot_index(g, b) < 0) return fail(v, VR_ERR_INVALID_ARG, "vr_debug_brick_data: this part does not hold brick %d", b);
+    if (v->store_released) return fail(v, VR_ERR_STATE, "vr_debug_brick_data: the float32 store was released (vr_volume_release_store)");
     const int bx = b % g.g[0], by = (b / g.g[0]) % g.g[1], bz = b / (g.g[0] * g.g[1]);
     const int bc[3] = {bx, by, bz};
     int d[3];
@@ -818,11 +836,13 @@ extern "C" int vr_set_sampler(vr_volume* v, int sampler) {
     if (!v) return fail(NULL, VR_ERR_INVALID_ARG, "vr_set_sampler: NULL handle");
     if (sampler != VR_SAMPLER_MANUAL && sampler != VR_SAMPLER_TEXTURE)
         return fail(v, VR_ERR_INVALID_ARG, "vr_set_sampler: unknown sampler %d", sampler);
+    if (v->store_released && sampler != VR_SAMPLER_TEXTURE)
+        return fail(v, VR_ERR_STATE, "vr_set_sampler: the float32 store was released, only the texture arm is left");
     if (sampler == VR_SAMPLER_TEXTURE && !v->tex) {
         const VrGrid& g = v->grid;
         if (!(g.layout == VR_LAYOUT_TILED && g.tl[0] == 2 && g.tl[1] == 2 && g.tl[2] == 1 && g.ml[0] == 0 && g.ml[1] == 0 && g.ml[2] == 0))
             return fail(v, VR_ERR_STATE, "vr_set_sampler: the texture arm is built beside the default (4x4x2 tiled) store only");
-        const cudaError_t e = vr_tex_create(g, &v->tex);
+        const cudaError_t e = vr_tex_create(g, &v->tex, true);
         if (e != cudaSuccess)
             return fail(v, e == cudaErrorMemoryAllocation ? VR_ERR_OUT_OF_MEMORY : VR_ERR_CUDA,
                         "vr_set_sampler: 3-D arrays for %d bricks (%.2f GB beside the brick store): %s", g.nown,
@@ -839,6 +859,44 @@ static int ensure_tex(vr_volume* v, cudaStream_t st) {
     VR_CUDA(v, vr_launch_tex_fill(v->grid, v->bricks, v->tex, st));
     v->launches++;
     v->tex_valid = true;
+    return VR_OK;
+}
+
+extern "C" int vr_volume_release_store(vr_volume* v, int64_t* freed_bytes_out, void* stream) {
+    if (!v) return fail(NULL, VR_ERR_INVALID_ARG, "vr_volume_release_store: NULL handle");
+    if (freed_bytes_out) *freed_bytes_out = 0;
+    if (!v->vmm) return fail(v, VR_ERR_STATE, "vr_volume_release_store: the handle was not created with VR_LAYOUT_TILED_RELEASABLE");
+    if (!v->has_data) return fail(v, VR_ERR_STATE, "vr_volume_release_store: nothing uploaded");
+    if (v->store_released) return fail(v, VR_ERR_STATE, "vr_volume_release_store: already released");
+    cudaStream_t st = (cudaStream_t)stream;
+    int rc = ensure_minmax(v, st); /* the range tables (rows f1, R19) are read from the store: last chance */
+    if (rc) return rc;
+    VR_CUDA(v, cudaDeviceSynchronize());
+    if (v->tex) { /* a second copy made by vr_set_sampler: start over, array by array */
+        vr_tex_destroy(v->tex);
+        v->tex = NULL;
+    }
+    cudaError_t e = vr_tex_create(v->grid, &v->tex, false);
+    if (e != cudaSuccess) return fail(v, e == cudaErrorMemoryAllocation ? VR_ERR_OUT_OF_MEMORY : VR_ERR_CUDA, "vr_volume_release_store: %s", cudaGetErrorString(e));
+    long long freed = 0;
+    for (int s = 0; s < v->grid.nown; ++s) {
+        int has_nan = 0;
+        e = vr_tex_convert_slot(v->grid, v->bricks, v->tex, s, &has_nan, st);
+        v->launches++;
+        if (e != cudaSuccess) {
+            cudaGetLastError();
+            /* the slots converted so far are gone from the store: the handle can only be destroyed */
+            v->store_released = true;
+            v->has_data = false;
+            return fail(v, e == cudaErrorMemoryAllocation ? VR_ERR_OUT_OF_MEMORY : VR_ERR_CUDA,
+                        "vr_volume_release_store: slot %d of %d: %s (the handle is no longer usable)", s, v->grid.nown, cudaGetErrorString(e));
+        }
+        if (!has_nan) freed += (long long)vr_vmm_release_slot(v->vmm, s); /* R14 needs the float32 cells of blanked bricks */
+    }
+    v->store_released = true;
+    v->tex_valid = true;
+    v->sampler = VR_SAMPLER_TEXTURE;
+    if (freed_bytes_out) *freed_bytes_out = freed;
     return VR_OK;
 }
 
@@ -982,6 +1040,11 @@ static int render_frame(vr_volume* v, const float* view, const float* proj, int 
     if (mode != VR_ALPHA && mode != VR_MIP) return fail(v, VR_ERR_INVALID_ARG, "vr_render: bad mode %d", mode);
     if (!v->has_tf) return fail(v, VR_ERR_STATE, "vr_render: no transfer function set");
     if (!v->has_data) return fail(v, VR_ERR_STATE, "vr_render: nothing uploaded");
+    if (v->store_released) {
+        if (mode != VR_ALPHA) return fail(v, VR_ERR_STATE, "vr_render: VR_MIP needs the float32 store, which was released");
+        if (!v->tf_smooth) return fail(v, VR_ERR_STATE, "vr_render: a transfer function with a step needs the float32 store, which was released");
+        if (v->counting == 2) return fail(v, VR_ERR_STATE, "vr_render: counting mode 2 needs the float32 store, which was released");
+    }
     rc = ensure_sub(v, sub_px);
     if (rc) return rc;
     if (v->traversal == VR_SORT_LAST) {

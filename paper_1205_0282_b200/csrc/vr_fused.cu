@@ -130,9 +130,11 @@ vr_fused_kernel(const VrRaycastParams prm, float4* __restrict__ frame) {
              * fetch through the brick's texture object - PER LANE here, the rays of a warp may be in different bricks
              * (the hardware serves the distinct objects of a warp one after the other) - VR_TEX_DEPTH fetches in flight;
              * the others fall through to the hand-rolled loop below */
+            bool use_tex = false;
+            cudaTextureObject_t tex = 0;
             if (TEX && MODE == VR_ALPHA) {
-                const bool use_tex = owned && __ldg(prm.tex_nan + slot_b) == 0;
-                const cudaTextureObject_t tex = use_tex ? __ldg(prm.tex + slot_b) : 0;
+                use_tex = owned && __ldg(prm.tex_nan + slot_b) == 0;
+                tex = use_tex ? __ldg(prm.tex + slot_b) : 0;
                 const double h = 1.0 / 4294967296.0;
                 float P0x = (float)((double)L.q[0] * h + 0.5), P0y = (float)((double)L.q[1] * h + 0.5), P0z = (float)((double)L.q[2] * h + 0.5);
                 float Dfx = (float)((double)D[0] * h), Dfy = (float)((double)D[1] * h), Dfz = (float)((double)D[2] * h);
@@ -254,7 +256,13 @@ vr_fused_kernel(const VrRaycastParams prm, float4* __restrict__ frame) {
                         const double p = VR_FMA(s, ray.d[a], ray.o[a]);
                         L.q[a] = to_fixed(p - ((double)(blo[a] - g.ghost) + 0.5));
                     }
-                    const float v = trilinear<LAY, 0, CLAMP, COUNT>(brick, g, ext, L, prm.bitmap, (long long)slot_b * g.slot);
+                    float v;
+                    if (TEX && use_tex) { /* the exit samples through the array as well: a released store has no float32 cells */
+                        const double h = 1.0 / 4294967296.0;
+                        v = tex3D<float>(tex, (float)((double)L.q[0] * h + 0.5), (float)((double)L.q[1] * h + 0.5), (float)((double)L.q[2] * h + 0.5));
+                    } else {
+                        v = trilinear<LAY, 0, CLAMP, COUNT>(brick, g, ext, L, prm.bitmap, (long long)slot_b * g.slot);
+                    }
                     if (COUNT) nsamples += (v == v) ? 1 : 0;
                     if (MODE == VR_MIP) {
                         acc.r = fmaxf(acc.r, v);

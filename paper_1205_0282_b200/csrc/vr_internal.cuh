@@ -188,7 +188,14 @@ cudaError_t vr_launch_setup(const VrGrid& grid, const VrMatrices& mats, int W, i
                             cudaStream_t st);
 /* texture arm of the brick store (vr_texture.cu): one 3-D CUDA array + texture object per slot */
 struct VrTexStore;
-cudaError_t vr_tex_create(const VrGrid& grid, VrTexStore** out);
+cudaError_t vr_tex_create(const VrGrid& grid, VrTexStore** out, bool all);
+cudaError_t vr_tex_convert_slot(const VrGrid& grid, const float* bricks, VrTexStore* t, int s, int* has_nan, cudaStream_t st);
+/* a store that can be handed back slot by slot (vr_vmm.cu: CUDA virtual memory management) */
+struct VrVmm;
+cudaError_t vr_vmm_create(size_t slot_bytes, int nslots, VrVmm** out, float** base_out);
+void vr_vmm_destroy(VrVmm* m);
+size_t vr_vmm_release_slot(VrVmm* m, int s);
+int vr_vmm_slot_released(const VrVmm* m, int s);
 void vr_tex_destroy(VrTexStore* t);
 const cudaTextureObject_t* vr_tex_table(const VrTexStore* t);
 const int* vr_tex_nan_table(const VrTexStore* t);

@@ -302,7 +302,13 @@ vr_raycast_kernel(const VrRaycastParams prm) {
                     const double p = VR_FMA(s, ray.d[a], ray.o[a]);
                     L.q[a] = to_fixed(p - ((double)(blo[a] - g.ghost) + 0.5));
                 }
-                const float v = trilinear<LAY, PT, CLAMP, COUNT>(brick, g, ext, L, prm.bitmap, (long long)slot_b * g.slot);
+                float v;
+                if (TEX && use_tex) { /* the exit samples through the array as well: a released store has no float32 cells */
+                    const double h = 1.0 / 4294967296.0;
+                    v = tex3D<float>(tex, (float)((double)L.q[0] * h + 0.5), (float)((double)L.q[1] * h + 0.5), (float)((double)L.q[2] * h + 0.5));
+                } else {
+                    v = trilinear<LAY, PT, CLAMP, COUNT>(brick, g, ext, L, prm.bitmap, (long long)slot_b * g.slot);
+                }
                 if (COUNT) nsamples += (v == v) ? 1 : 0;
                 if (MODE == VR_MIP) {
                     acc.r = fmaxf(acc.r, v);

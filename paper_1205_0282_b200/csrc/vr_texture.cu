@@ -58,7 +58,8 @@ static int brick_of_slot(const VrGrid& g, int s) {
     return (bz * g.g[1] + by) * g.g[0] + bx;
 }
 
-cudaError_t vr_tex_create(const VrGrid& g, VrTexStore** out) {
+/* the store's host tables and device tables, no array yet */
+static cudaError_t tex_alloc(const VrGrid& g, VrTexStore** out) {
     *out = NULL;
     VrTexStore* t = new (std::nothrow) VrTexStore();
     if (!t) return cudaErrorMemoryAllocation;
@@ -67,41 +68,58 @@ cudaError_t vr_tex_create(const VrGrid& g, VrTexStore** out) {
     t->arr = new (std::nothrow) cudaArray_t[g.nown]();
     t->tex = new (std::nothrow) cudaTextureObject_t[g.nown]();
     t->surf = new (std::nothrow) cudaSurfaceObject_t[g.nown]();
-    int3* ext = new (std::nothrow) int3[g.nown];
-    cudaError_t e = (t->arr && t->tex && t->surf && ext) ? cudaSuccess : cudaErrorMemoryAllocation;
-    const cudaChannelFormatDesc fmt = cudaCreateChannelDesc<float>();
-    for (int s = 0; s < g.nown && e == cudaSuccess; ++s) {
-        int bc[3], lo[3], hi[3];
-        vr_brick_coords(g, brick_of_slot(g, s), bc);
-        vr_brick_core(g, bc, lo, hi);
-        ext[s] = make_int3(hi[0] - lo[0] + 2 * g.ghost, hi[1] - lo[1] + 2 * g.ghost, hi[2] - lo[2] + 2 * g.ghost);
-        e = cudaMalloc3DArray(&t->arr[s], &fmt, make_cudaExtent((size_t)ext[s].x, (size_t)ext[s].y, (size_t)ext[s].z),
-                              cudaArraySurfaceLoadStore);
-        if (e != cudaSuccess) break;
-        cudaResourceDesc res;
-        memset(&res, 0, sizeof(res));
-        res.resType = cudaResourceTypeArray;
-        res.res.array.array = t->arr[s];
-        cudaTextureDesc td;
-        memset(&td, 0, sizeof(td));
-        td.addressMode[0] = td.addressMode[1] = td.addressMode[2] = cudaAddressModeClamp;
-        td.filterMode = cudaFilterModeLinear;
-        td.readMode = cudaReadModeElementType;
-        td.normalizedCoords = 0;
-        e = cudaCreateTextureObject(&t->tex[s], &res, &td, NULL);
-        if (e == cudaSuccess) e = cudaCreateSurfaceObject(&t->surf[s], &res);
-    }
+    cudaError_t e = (t->arr && t->tex && t->surf) ? cudaSuccess : cudaErrorMemoryAllocation;
     if (e == cudaSuccess) e = cudaMalloc(&t->d_tex, sizeof(cudaTextureObject_t) * g.nown);
     if (e == cudaSuccess) e = cudaMalloc(&t->d_surf, sizeof(cudaSurfaceObject_t) * g.nown);
     if (e == cudaSuccess) e = cudaMalloc(&t->d_ext, sizeof(int3) * g.nown);
     if (e == cudaSuccess) e = cudaMalloc(&t->d_nan, sizeof(int) * g.nown);
-    if (e == cudaSuccess) e = cudaMemcpy(t->d_tex, t->tex, sizeof(cudaTextureObject_t) * g.nown, cudaMemcpyHostToDevice);
-    if (e == cudaSuccess) e = cudaMemcpy(t->d_surf, t->surf, sizeof(cudaSurfaceObject_t) * g.nown, cudaMemcpyHostToDevice);
-    if (e == cudaSuccess) e = cudaMemcpy(t->d_ext, ext, sizeof(int3) * g.nown, cudaMemcpyHostToDevice);
-    delete[] ext;
+    if (e == cudaSuccess) e = cudaMemset(t->d_nan, 0, sizeof(int) * g.nown);
     if (e != cudaSuccess) {
         cudaGetLastError();
         vr_tex_destroy(t);
+        return e;
+    }
+    *out = t;
+    return cudaSuccess;
+}
+
+/* array, texture object and surface object of slot s; their handles and the slot's extent go to the device tables */
+static cudaError_t tex_create_slot(VrTexStore* t, const VrGrid& g, int s) {
+    int bc[3], lo[3], hi[3];
+    vr_brick_coords(g, brick_of_slot(g, s), bc);
+    vr_brick_core(g, bc, lo, hi);
+    const int3 ext = make_int3(hi[0] - lo[0] + 2 * g.ghost, hi[1] - lo[1] + 2 * g.ghost, hi[2] - lo[2] + 2 * g.ghost);
+    const cudaChannelFormatDesc fmt = cudaCreateChannelDesc<float>();
+    cudaError_t e = cudaMalloc3DArray(&t->arr[s], &fmt, make_cudaExtent((size_t)ext.x, (size_t)ext.y, (size_t)ext.z), cudaArraySurfaceLoadStore);
+    if (e != cudaSuccess) return e;
+    cudaResourceDesc res;
+    memset(&res, 0, sizeof(res));
+    res.resType = cudaResourceTypeArray;
+    res.res.array.array = t->arr[s];
+    cudaTextureDesc td;
+    memset(&td, 0, sizeof(td));
+    td.addressMode[0] = td.addressMode[1] = td.addressMode[2] = cudaAddressModeClamp;
+    td.filterMode = cudaFilterModeLinear;
+    td.readMode = cudaReadModeElementType;
+    td.normalizedCoords = 0;
+    e = cudaCreateTextureObject(&t->tex[s], &res, &td, NULL);
+    if (e == cudaSuccess) e = cudaCreateSurfaceObject(&t->surf[s], &res);
+    if (e == cudaSuccess) e = cudaMemcpy(t->d_tex + s, t->tex + s, sizeof(cudaTextureObject_t), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemcpy(t->d_surf + s, t->surf + s, sizeof(cudaSurfaceObject_t), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemcpy(t->d_ext + s, &ext, sizeof(int3), cudaMemcpyHostToDevice);
+    return e;
+}
+
+/* all = true: every slot's array at once (the second copy beside the store); false: tables only, the arrays come slot by
+ * slot (vr_tex_convert_slot: vr_volume_release_store) */
+cudaError_t vr_tex_create(const VrGrid& g, VrTexStore** out, bool all) {
+    VrTexStore* t = NULL;
+    cudaError_t e = tex_alloc(g, &t);
+    for (int s = 0; all && s < g.nown && e == cudaSuccess; ++s) e = tex_create_slot(t, g, s);
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        vr_tex_destroy(t);
+        *out = NULL;
         return e;
     }
     *out = t;
@@ -117,8 +135,8 @@ const int* vr_tex_nan_table(const VrTexStore* t) { return t ? t->d_nan : NULL; }
  * write is coalesced. Once per upload. */
 __global__ void __launch_bounds__(256)
 vr_tex_fill_kernel(VrGrid g, const float* __restrict__ bricks, const cudaSurfaceObject_t* __restrict__ surf,
-                   const int3* __restrict__ ext, int* __restrict__ has_nan) {
-    const int s = blockIdx.y;
+                   const int3* __restrict__ ext, int* __restrict__ has_nan, int slot0) {
+    const int s = blockIdx.y + slot0;
     const int3 e = ext[s];
     const cudaSurfaceObject_t su = surf[s];
     const float* __restrict__ src = bricks + (long long)s * g.slot;
@@ -140,12 +158,26 @@ vr_tex_fill_kernel(VrGrid g, const float* __restrict__ bricks, const cudaSurface
     if (__any_sync(0xffffffffu, nan_seen) && lane == 0) has_nan[s] = 1;
 }
 
-cudaError_t vr_launch_tex_fill(const VrGrid& grid, const float* bricks, const VrTexStore* t, cudaStream_t st) {
+static cudaError_t launch_fill(const VrGrid& grid, const float* bricks, const VrTexStore* t, int slot0, int nslots, cudaStream_t st) {
     const int nj = (grid.P + 3) >> 2, nk = (grid.P + 1) >> 1;
     long long bx = (long long)nj * nk;
     if (bx > 4096) bx = 4096;
-    cudaError_t e = cudaMemsetAsync(t->d_nan, 0, sizeof(int) * t->n, st);
+    cudaError_t e = cudaMemsetAsync(t->d_nan + slot0, 0, sizeof(int) * nslots, st);
     if (e != cudaSuccess) return e;
-    vr_tex_fill_kernel<<<dim3((unsigned)bx, (unsigned)t->n), 256, 0, st>>>(grid, bricks, t->d_surf, t->d_ext, t->d_nan);
+    vr_tex_fill_kernel<<<dim3((unsigned)bx, (unsigned)nslots), 256, 0, st>>>(grid, bricks, t->d_surf, t->d_ext, t->d_nan, slot0);
     return cudaGetLastError();
+}
+
+cudaError_t vr_launch_tex_fill(const VrGrid& grid, const float* bricks, const VrTexStore* t, cudaStream_t st) {
+    return launch_fill(grid, bricks, t, 0, t->n, st);
+}
+
+/* vr_volume_release_store, one slot: create the slot's array, fill it from the store, wait, and say whether the slot holds
+ * blanked voxels (then its float32 cells must stay: R14 needs them). */
+cudaError_t vr_tex_convert_slot(const VrGrid& grid, const float* bricks, VrTexStore* t, int s, int* has_nan, cudaStream_t st) {
+    cudaError_t e = tex_create_slot(t, grid, s);
+    if (e == cudaSuccess) e = launch_fill(grid, bricks, t, s, 1, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(has_nan, t->d_nan + s, sizeof(int), cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    return e;
 }

@@ -192,3 +192,67 @@ def test_fused_traversal_through_the_texture_arm(vr, tau):
     img = gpu_frame(g, view, proj, W, H, 0.5, vr.ALPHA)
     assert np.isfinite(img).all()
     check_alpha(img, ref, tau, "fused texture, blanked box", envelope=True, max_flagged=1.0)
+
+
+def test_released_store_renders_through_the_arrays_alone(vr):
+    """VR_LAYOUT_TILED_RELEASABLE + vr_volume_release_store (the texture arm for cubes whose second copy does not fit):
+    frames before the release (texture sampler, both stores present) and after it (float32 cells handed back) are
+    bit-identical, match the oracle, the device gets the memory back, bricks with blanked voxels keep their float32
+    cells and the exact R14 rule, and everything that needs the float32 store refuses."""
+    import torch
+    dims, brick = (160, 128, 96), 32
+    cube = synth.Cube(61, *dims, 10)
+    data = cube.fill_host()
+    data[70:90, 40:60, 100:120] = np.nan          # blanked voxels in a few bricks
+    W, H = 203, 117
+    fr = synth.Framing(*dims, W, H)
+    g = vr.Volume(*dims, brick, 1, layout=vr.LAYOUT_TILED_RELEASABLE)
+    g.upload(torch.from_numpy(data).cuda())
+    o = oracle.Volume(*dims, brick, 1, data=data)
+    one = oracle.Volume(*dims, 256, 1, data=data)
+    for v in (g, o, one):
+        v.set_transfer_function(synth.tf_ramp(), synth.TF_VMIN, synth.TF_VMAX)
+        v.set_early_termination(0.99)
+    o.set_ert_margin(TEX_MARGIN)
+    one.set_ert_margin(TEX_MARGIN)
+    mip_before = gpu_frame(g, fr.seeded(3, 0), fr.proj(False), W, H, 0.5, vr.MIP)
+    check_mip(mip_before, o.render(fr.seeded(3, 0), fr.proj(False), W, H, 0.5, oracle.MIP), "releasable handle, MIP before the release")
+    g.set_sampler(vr.SAMPLER_TEXTURE)
+    views = [(fr.seeded(3, k), fr.proj(k == 1)) for k in range(2)]
+    before = [gpu_frame(g, v, p, W, H, 0.5, vr.ALPHA) for v, p in views]
+    lo, hi = g.minmax()
+    torch.cuda.synchronize()
+    free0 = torch.cuda.mem_get_info()[0]
+    freed = g.release_store()
+    torch.cuda.synchronize()
+    store_bytes = g.nbricks * 9 * 9 * 17 * 128
+    assert freed > 0.6 * store_bytes                                   # all but the blanked bricks (and the shared granules)
+    assert torch.cuda.mem_get_info()[0] > free0 - 0.5 * store_bytes    # a second copy was NOT needed at any time ...
+    assert g.minmax() == (lo, hi)                                      # ... and the range tables survive
+    for (v, p), b in zip(views, before):
+        after = gpu_frame(g, v, p, W, H, 0.5, vr.ALPHA)
+        assert np.array_equal(after, b)
+        check_alpha(after, o.render(v, p, W, H, 0.5, oracle.ALPHA), 0.99, "released store", envelope=True, max_flagged=1.0)
+    g.set_traversal(vr.FUSED)
+    fused = gpu_frame(g, *views[0], W, H, 0.5, vr.ALPHA)
+    check_alpha(fused, one.render(*views[0], W, H, 0.5, oracle.ALPHA), 0.99, "released store, fused", envelope=True, max_flagged=1.0)
+    g.set_traversal(vr.SORT_LAST)
+    out = torch.empty((H, W, 4), dtype=torch.float32, device="cuda")
+    for call in (lambda: g.render(*views[0], W, H, 0.5, vr.MIP, out),
+                 lambda: g.upload(torch.from_numpy(data).cuda()),
+                 lambda: g.download(np.empty((4, 4, 4), dtype=np.float32)),
+                 lambda: g.debug_brick_data(0),
+                 lambda: g.set_sampler(vr.SAMPLER_MANUAL),
+                 lambda: g.release_store()):
+        with pytest.raises(vr.VrError) as e:
+            call()
+        assert e.value.status == 4
+    g.set_transfer_function(synth.tf_threshold(), synth.TF_VMIN, synth.TF_VMAX)
+    with pytest.raises(vr.VrError):
+        g.render(*views[0], W, H, 0.5, vr.ALPHA, out)                 # a stepped table needs the float32 store
+    g.set_transfer_function(synth.tf_ramp(), synth.TF_VMIN, synth.TF_VMAX)
+    assert np.array_equal(gpu_frame(g, *views[0], W, H, 0.5, vr.ALPHA), before[0])
+    plain = vr.Volume(32, 32, 32, 16, 1)
+    plain.upload(np.zeros((32, 32, 32), dtype=np.float32))
+    with pytest.raises(vr.VrError):
+        plain.release_store()
