@@ -136,7 +136,14 @@ def build_volume(vr, wl, tf):
     toy.minmax()
     toy.close()
     cube = synth.Cube(wl["seed"], wl["nx"], wl["ny"], wl["nz"], wl["nsrc"], wl["ramp"], wl.get("kind", 0))
-    g = vr.Volume(wl["nx"], wl["ny"], wl["nz"], wl["brick"], wl["ghost"])
+    # the store is mapped brick by brick (VR_LAYOUT_TILED_RELEASABLE: the same tiled layout for every kernel), so that the
+    # LAST variant can hand it back array by array and render through the texture arm alone (vr_volume_release_store)
+    try:
+        g = vr.Volume(wl["nx"], wl["ny"], wl["nz"], wl["brick"], wl["ghost"], layout=vr.LAYOUT_TILED_RELEASABLE)
+        g.releasable = True
+    except vr.VrError:
+        g = vr.Volume(wl["nx"], wl["ny"], wl["nz"], wl["brick"], wl["ghost"])
+        g.releasable = False
     plane = wl["nx"] * wl["ny"] * 4
     nzs = max(1, min(wl["nz"], (4 << 30) // plane))  # 4 GiB slabs: 64 planes of config 3
     buf = torch.empty((nzs, wl["ny"], wl["nx"]), dtype=torch.float32, device="cuda")
@@ -974,6 +981,7 @@ def main():
                              "stage_ms": {"setup": round(float(v["stages"][:, 0].mean()), 4),
                                           "raycast": round(float(v["stages"][:, 1].mean()), 4),
                                           "composite": round(float(v["stages"][:, 2].mean()), 4)},
+                             "counts_": v["counts"],
                              "roofline": roofline_of(v["counts"], v["stages"], v["stage_views"], peak, peak_src,
                                                      traffic_of(args.workload, vmode, vtf + ("" if vtrav == "sort_last" else "/fused") +
                                                                 ("/texture" if vsamp == "texture" and vmode == "alpha" and vtf != "threshold" else "")))})
@@ -990,6 +998,29 @@ def main():
              "lines_frac": v["roofline"].get("lines_frac"), "frames_per_s": v["frames_per_s"]} for v in variants if "roofline" in v]
         if args.sortlast_parts > 1 and args.mode == "alpha":
             line["sortlast"] = sortlast_report(vr, g, wl, cube, tf, args.sortlast_parts, order, K, Wm)
+        # LAST (irreversible): the texture arm on THIS cube even where a second copy of the bricks does not fit - the bricks
+        # become 3-D arrays one by one and their float32 cells go back to the device; the same frames again. Sample sets are
+        # the hand-rolled path's, so the counting passes above supply the algorithmic bytes.
+        if getattr(g, "releasable", False):
+            transl = [v for v in variants if v["tf"] == "translucent" and v["traversal"] == "sort_last" and "counts_" in v]
+            try:
+                t0 = time.perf_counter()
+                freed = g.release_store()
+                rel = {"what": "vr_volume_release_store: float32 store handed back brick by brick, ALPHA frames through 3-D CUDA "
+                               "arrays only (8-bit filter weights: inside 2e-3 on these tables, tests/test_gpu_texture.py)",
+                       "freed_gb": round(freed / 1e9, 2), "convert_s": round(time.perf_counter() - t0, 2)}
+                for vtf, cnts in (("ramp", m["counts"] if args.tf == "ramp" and args.mode == "alpha" else None),
+                                  ("translucent", transl[0]["counts_"] if transl else None)):
+                    g.set_transfer_function(pick_tf(wl, vtf), *tf_range(wl))
+                    ms_r, _, st_r, sv_r = timed_device(g, wl, 0, order, K, Wm, out, dist)
+                    rel[vtf] = {"frames_per_s": round(K / (ms_r * 1e-3), 3), "raycast_ms": round(float(st_r[:, 1].mean()), 4)}
+                    if cnts is not None:
+                        rel[vtf]["roofline"] = roofline_of(cnts, st_r, sv_r, peak, peak_src, None)
+                line["texture_released"] = rel
+            except vr.VrError as e:
+                line["texture_released"] = {"unavailable": str(e)}
+        for v in variants:
+            v.pop("counts_", None)
 
     if rank == 0 and not args.no_cpu_baseline and world == 1:
         g.close()
