@@ -777,6 +777,9 @@ def main():
     ap.add_argument("--sampler", default="manual", choices=["manual", "texture"],
                     help="row a5: hand-rolled float32 tri-linear from the tiled store (default) or the texture-object arm "
                          "(ALPHA frames; a second copy of the bricks as 3-D CUDA arrays)")
+    ap.add_argument("--release-store", action="store_true",
+                    help="profiling: hand the float32 store back right after the build (vr_volume_release_store) and render the main "
+                         "arm through the texture arm alone; implies --sampler texture --no-variants --cells-every 0")
     ap.add_argument("--no-variants", action="store_true")
     ap.add_argument("--probe", default=None, choices=["dram"],
                     help="dram: the DRAM fetch-granularity probe (vr_debug_probe_dram) instead of a workload; one JSON line")
@@ -862,7 +865,10 @@ def main():
     t_build = time.perf_counter()
     g, cube = build_volume(vr, wl, tf)
     t_build = time.perf_counter() - t_build
-    if args.sampler == "texture":
+    if args.release_store:
+        g.release_store()
+        args.sampler, args.no_variants, args.cells_every = "texture", True, 0
+    elif args.sampler == "texture":
         g.set_sampler(vr.SAMPLER_TEXTURE)
     W, H, K, Wm = wl["width"], wl["height"], args.steps, args.warmup
     out = torch.empty((H, W, 4), dtype=torch.float32, device="cuda")
