@@ -616,7 +616,7 @@ def config_of(wl, args):
                             wl["name"], wl["nx"], wl["ny"], wl["nz"], what, wl["brick"], wl["ghost"], wl["width"], wl["height"],
                             wl["view_kind"], args.mode.upper(), wl["step"], args.tf, wl["tau"],
                             (", fused traversal" if getattr(args, "traversal", "sort_last") == "fused" else "") +
-                            (", texture sampler" if getattr(args, "sampler", "manual") == "texture" else "")),
+                            (", texture sampler" if getattr(args, "sampler_asked", "auto") == "texture" else "")),
             "baseline_config_index": int(wl["name"][1:]) if wl["name"][0] == "c" else None,
             "cube_gb": round(wl["nx"] * wl["ny"] * wl["nz"] * 4 / 1e9, 2),
             "l2_policy": "inputs larger than L2 (every frame streams a new view's share of the cube); no explicit flush",
@@ -672,8 +672,9 @@ def run_c4(args, vr, peak, peak_src, sampler):
     g = None
     if args.c4_part != "composite":
         g, _ = build_volume(vr, wl, synth.tf_ramp())
-        if args.sampler == "texture":
+        if args.sampler in ("auto", "texture"):  # auto: the faster arm on this cube (ALPHA, ramp TF; the second copy fits)
             g.set_sampler(vr.SAMPLER_TEXTURE)
+            args.sampler = "texture"
     for res in ((512, 1024, 2048, 4096) if g is not None else ()):
         w = dict(wl)
         w["width"] = w["height"] = res
@@ -774,9 +775,13 @@ def main():
                          "replica figure beside it as `replicas` - and the one-GPU line otherwise")
     ap.add_argument("--sortlast-parts", type=int, default=8,
                     help="row f3 report: parts of the k-d partition rendered one after the other on this GPU (0 = skip)")
-    ap.add_argument("--sampler", default="manual", choices=["manual", "texture"],
-                    help="row a5: hand-rolled float32 tri-linear from the tiled store (default) or the texture-object arm "
-                         "(ALPHA frames; a second copy of the bricks as 3-D CUDA arrays)")
+    ap.add_argument("--sampler", default="auto", choices=["auto", "manual", "texture"],
+                    help="row a5: manual = hand-rolled float32 tri-linear from the tiled store; texture = the texture-object arm "
+                         "(ALPHA frames; a second copy of the bricks as 3-D CUDA arrays). auto (default): 'whichever ncu shows is "
+                         "faster' (north_star; DESIGN.md section 9) - the texture arm for ALPHA frames with a smooth table, on a "
+                         "second copy where it fits beside the store, else on the RELEASED store (vr_volume_release_store, the "
+                         "run's last leg, which then supplies the headline with the hand-rolled figures beside it as "
+                         "`hand_rolled`); manual for MIP, stepped tables and the fused traversal's default")
     ap.add_argument("--release-store", action="store_true",
                     help="profiling: hand the float32 store back right after the build (vr_volume_release_store) and render the main "
                          "arm through the texture arm alone; implies --sampler texture --no-variants --cells-every 0")
@@ -786,6 +791,7 @@ def main():
     ap.add_argument("--probe-gib", type=int, default=16, help="--probe dram: size of the probed buffer")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
+    args.sampler_asked = args.sampler  # `config` names the sampler only when the caller chose it (both arms print the same config)
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
 
     rank = int(os.environ.get("RANK", "0"))
@@ -865,6 +871,15 @@ def main():
     t_build = time.perf_counter()
     g, cube = build_volume(vr, wl, tf)
     t_build = time.perf_counter() - t_build
+    promote = False  # auto: the texture arm on the released store becomes the headline (the run's last leg)
+    if args.sampler == "auto":
+        args.sampler = "manual"
+        if args.mode == "alpha" and args.traversal == "sort_last" and args.tf in ("ramp", "translucent") and not args.release_store:
+            free_b = torch.cuda.mem_get_info()[0]
+            if free_b > 1.15 * wl["nx"] * wl["ny"] * wl["nz"] * 4:  # a second copy fits (c0 - c2, n1)
+                args.sampler = "texture"
+            else:
+                promote = bool(getattr(g, "releasable", False)) and not args.no_variants and world == 1
     if args.release_store:
         g.release_store()
         args.sampler, args.no_variants, args.cells_every = "texture", True, 0
@@ -910,6 +925,9 @@ def main():
                     "synchronous_value": round(e2e_sync_fps, 3),
                     "synchronous_what": "vr_render_host: the caller waits for each frame's copy before queueing the next"},
             "clocks": m["clocks"],
+            "sampler": ("texture: 3-D CUDA arrays behind texture objects, a second copy beside the store" if args.sampler == "texture" and args.mode == "alpha"
+                        else "manual: hand-rolled float32 tri-linear from the 4x4x2 micro-tiled store") +
+                       (" (chosen by --sampler auto)" if args.sampler_asked == "auto" else ""),
             "stage_ms": {"setup": round(float(m["stages"][:, 0].mean()), 4), "raycast": round(float(m["stages"][:, 1].mean()), 4),
                          "composite": round(float(m["stages"][:, 2].mean()), 4)},
             # the paper's estimator: frame time per rotation angle, then its 75th percentile
@@ -1018,11 +1036,41 @@ def main():
                 for vtf, cnts in (("ramp", m["counts"] if args.tf == "ramp" and args.mode == "alpha" else None),
                                   ("translucent", transl[0]["counts_"] if transl else None)):
                     g.set_transfer_function(pick_tf(wl, vtf), *tf_range(wl))
-                    ms_r, _, st_r, sv_r = timed_device(g, wl, 0, order, K, Wm, out, dist)
+                    main = promote and vtf == args.tf and cnts is not None
+                    cl = ClockSampler(local_rank) if main else None
+                    if cl:
+                        cl.start()
+                    ms_r, la_r, st_r, sv_r = timed_device(g, wl, 0, order, K, Wm, out, dist)
                     rel[vtf] = {"frames_per_s": round(K / (ms_r * 1e-3), 3), "raycast_ms": round(float(st_r[:, 1].mean()), 4)}
                     if cnts is not None:
-                        rel[vtf]["roofline"] = roofline_of(cnts, st_r, sv_r, peak, peak_src, None)
+                        rel[vtf]["roofline"] = roofline_of(cnts, st_r, sv_r, peak, peak_src, traffic_of(args.workload, "alpha", vtf + "/texture"))
+                    if main:  # the headline: this arm is the faster one on this cube (profiles/r2_raycast_c3_ramp_tex.md)
+                        e2e_r = timed_e2e(g, wl, 0, order, K, Wm, host_bufs, dist, True)
+                        e2e_sync_r = timed_e2e(g, wl, 0, order, K, Wm, host_bufs, dist, False)
+                        keep = ("value", "ms_per_step", "gsamples_per_s", "gpu_launches", "e2e", "clocks", "stage_ms", "frame_ms", "roofline")
+                        hand = {k: line[k] for k in keep if k in line}
+                        hand["e2e"] = {k: line["e2e"][k] for k in ("value", "synchronous_value")}
+                        hand["sampler"] = "manual: hand-rolled float32 tri-linear from the 4x4x2 micro-tiled store (the same frames, before the store was handed back)"
+                        line["hand_rolled"] = hand
+                        frame_r = st_r.sum(axis=1)
+                        line.update({"value": round(K / (ms_r * 1e-3), 3), "ms_per_step": round(ms_r / K, 4),
+                                     "gsamples_per_s": round(m["samples"] / (ms_r * 1e-3) / 1e9, 3), "gpu_launches": int(la_r),
+                                     "clocks": cl.stop(),
+                                     "stage_ms": {"setup": round(float(st_r[:, 0].mean()), 4), "raycast": round(float(st_r[:, 1].mean()), 4),
+                                                  "composite": round(float(st_r[:, 2].mean()), 4)},
+                                     "frame_ms": {"p50": round(float(np.percentile(frame_r, 50)), 4), "p75": round(float(np.percentile(frame_r, 75)), 4),
+                                                  "min": round(float(frame_r.min()), 4), "max": round(float(frame_r.max()), 4), "views": int(len(st_r))},
+                                     "roofline": rel[vtf]["roofline"]})
+                        line["e2e"] = dict(line["e2e"], value=round(K / (e2e_r * 1e-3), 3), synchronous_value=round(K / (e2e_sync_r * 1e-3), 3))
+                        line["sampler"] = ("auto -> texture: 3-D CUDA arrays behind texture objects after vr_volume_release_store (the faster arm on "
+                                                     "this cube: profiles/r2_raycast_c3_ramp_tex.md against r2_raycast_c3_ramp.md); `hand_rolled` holds "
+                                                     "the same measurements of the hand-rolled sampler")
+                        rel["headline"] = True
                 line["texture_released"] = rel
+                line["roofline_variants"] += [{"mode": "alpha", "tf": vtf, "traversal": "sort_last", "sampler": "texture (released store)",
+                                               "frac": rel[vtf]["roofline"]["frac"], "lines_frac": rel[vtf]["roofline"].get("lines_frac"),
+                                               "frames_per_s": rel[vtf]["frames_per_s"]}
+                                              for vtf in ("ramp", "translucent") if "roofline" in rel.get(vtf, {})]
             except vr.VrError as e:
                 line["texture_released"] = {"unavailable": str(e)}
         for v in variants:

@@ -365,7 +365,10 @@ static cudaError_t launch_instance(const VrRaycastParams& p0, long long items, b
     /* Sparse MIP frames (several voxels per pixel: every load is a DRAM line of its own) run faster with two
      * resident CTAs per SM than with three - the lighter MIP loop keeps more lines in flight than L1/L2 hold
      * (c3: 14.5 -> 12.3 ms); dense frames and ALPHA want all three. */
-    const int per_sm = (MODE == VR_MIP && sparse && cached_per_sm > 2) ? 2 : cached_per_sm;
+    int per_sm = (MODE == VR_MIP && sparse && cached_per_sm > 2) ? 2 : cached_per_sm;
+#ifdef VR_EXP_SPARSE_TEX_PER_SM /* experiment knob (profiles/r2_c3_experiments.md): resident CTAs of the texture arm on sparse views */
+    if (TEX && sparse && per_sm > VR_EXP_SPARSE_TEX_PER_SM) per_sm = VR_EXP_SPARSE_TEX_PER_SM;
+#endif
     long long ctas = (long long)sms * per_sm;
     const long long want = (items + (VR_RAYCAST_THREADS / 32) - 1) / (VR_RAYCAST_THREADS / 32);
     if (ctas > want) ctas = want < 1 ? 1 : want;
