@@ -729,7 +729,7 @@ def run_probe_dram(vr, gib):
                       "ctas": ctas, "loads": loads, "ms": round(ms, 4), "gloads_per_s": round(loads / (ms * 1e-3) / 1e9, 2),
                       "gbs_if_128B_per_load": round(loads * 128 / (ms * 1e-3) / 1e9, 1)})
 
-    for f in range(len(vr.PROBE_FLAVOURS)):  # every load a random line
+    for f in range(11):  # every load a random line (the ld.global flavours; the texture unit's are `--probe tex`)
         case(f, 128, 1)
     for gran in (32, 64, 128):                 # cudaLimitMaxL2FetchGranularity
         case(1, 128, 1, gran)
@@ -751,6 +751,21 @@ def run_probe_dram(vr, gib):
     buf = whole
     del buf
     return {"probe": "dram", "buffer_gib": gib, "hbm_peak_gbs": peak, "hbm_peak_source": peak_src, "cases": cases}
+
+
+def run_probe_tex(vr):
+    """The same question for the texture unit (profiles/r2_probe_dram.md, second part): random fetches through texture
+    objects - tex1Dfetch over linear memory (4 and 16 bytes), tex3D point fetches of float4 texels and linear-filtered
+    float fetches from a 3-D CUDA array the probe allocates - beside ld.global.nc, over 4 GiB, at two grid sizes."""
+    import torch
+    buf = torch.zeros((4 << 30) // 4, dtype=torch.float32, device="cuda")
+    cases = []
+    for ctas in (148 * 8, 148 * 32):
+        for f in (1, 11, 12, 13, 14):
+            ms, loads = vr.debug_probe_dram(buf, f, 128, 1, 256, ctas, 0)
+            cases.append({"flavour": vr.PROBE_FLAVOURS[f], "ctas": ctas, "loads": loads, "ms": round(ms, 4),
+                          "gloads_per_s": round(loads / (ms * 1e-3) / 1e9, 2)})
+    return {"probe": "tex", "buffer_gib": 4, "cases": cases}
 
 
 # ----------------------------------------------------------------------------- main
@@ -786,8 +801,9 @@ def main():
                     help="profiling: hand the float32 store back right after the build (vr_volume_release_store) and render the main "
                          "arm through the texture arm alone; implies --sampler texture --no-variants --cells-every 0")
     ap.add_argument("--no-variants", action="store_true")
-    ap.add_argument("--probe", default=None, choices=["dram"],
-                    help="dram: the DRAM fetch-granularity probe (vr_debug_probe_dram) instead of a workload; one JSON line")
+    ap.add_argument("--probe", default=None, choices=["dram", "tex"],
+                    help="dram: the DRAM fetch-granularity probe (vr_debug_probe_dram) instead of a workload; tex: the same for "
+                         "fetches through texture objects; one JSON line")
     ap.add_argument("--probe-gib", type=int, default=16, help="--probe dram: size of the probed buffer")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
@@ -831,9 +847,9 @@ def main():
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         return float(t.item())
 
-    if args.probe == "dram":
+    if args.probe:
         if rank == 0:
-            print(json.dumps(run_probe_dram(vr, args.probe_gib)), flush=True)
+            print(json.dumps(run_probe_dram(vr, args.probe_gib) if args.probe == "dram" else run_probe_tex(vr)), flush=True)
         return 0
 
     if args.workload == "c4":

@@ -458,7 +458,12 @@ int vr_debug_stage_times(vr_volume* v, int nframes, float* ms_out);
  * one aligned span_bytes block (a power of two >= 128; group <= span_bytes / 128).
  *   flavour: 0 ld.global, 1 ld.global.nc (= __ldg, the ray-cast kernel's load), 2 .cg, 3 .cs, 4 .cv,
  *            5 .nc.L1::no_allocate, 6 .nc.L1::no_allocate.L2::64B, 7 .nc.L2::128B, 8 .nc.L2::256B,
- *            9 .nc.v4.f32 (16 bytes), 10 .nc.L2::64B
+ *            9 .nc.v4.f32 (16 bytes), 10 .nc.L2::64B;
+ *            through texture objects: 11 tex1Dfetch<float> and 12 tex1Dfetch<float4> over the head of buf as linear
+ *            memory (as far as the device's 1-D linear texture limit reaches); 13 tex3D<float4> point fetches and
+ *            14 tex3D<float> linear-filtered fetches (the texture arm's) at hashed positions of a 3-D CUDA array of
+ *            1024 x 1024 x (bytes / texel / 2^20, at most 2048) texels which the call allocates and frees (buf may be
+ *            NULL; span_bytes / group are ignored)
  *   l2_fetch_granularity: 0 = leave, or 32 / 64 / 128 = cudaLimitMaxL2FetchGranularity (stays set).
  *   ms_out (host): device time of one launch (CUDA events on `stream`, after one warm-up launch);
  *   loads_out (host): loads that launch issued. DRAM bytes per load come from ncu's

@@ -444,7 +444,8 @@ def part_rect(dims, brick, box, view, proj, width, height):
 
 PROBE_FLAVOURS = ("ld.global", "ld.global.nc", "ld.global.cg", "ld.global.cs", "ld.global.cv", "ld.global.nc.L1::no_allocate",
                   "ld.global.nc.L1::no_allocate.L2::64B", "ld.global.nc.L2::128B", "ld.global.nc.L2::256B", "ld.global.nc.v4",
-                  "ld.global.nc.L2::64B")
+                  "ld.global.nc.L2::64B", "tex1Dfetch.f32 (linear memory)", "tex1Dfetch.v4.f32 (linear memory)",
+                  "tex3D.v4.f32 point (3-D array)", "tex3D.f32 linear (3-D array)")
 
 
 def debug_probe_dram(buf, flavour, span_bytes=128, group=1, loads_per_thread=256, ctas=148 * 8, l2_fetch_granularity=0, stream=None):

@@ -15,6 +15,7 @@
  * DRAM bytes per load = dram__bytes_read.sum of the launch (ncu) / loads; rate = loads / time.
  */
 #include <stdio.h>
+#include <string.h>
 
 #include "vr_internal.cuh"
 
@@ -30,12 +31,21 @@ enum {
     PF_NC_L2_256,     /* ld.global.nc.L2::256B */
     PF_NC_V4,         /* ld.global.nc.v4.f32: 16 bytes per load */
     PF_NC_L2_64_ONLY, /* ld.global.nc.L2::64B (L1 allocates) */
+    PF_TEX_F32,       /* tex1Dfetch<float> through a texture object over the (linear) buffer: the texture unit's path */
+    PF_TEX_V4,        /* tex1Dfetch<float4>: 16 bytes per fetch */
+    PF_ARR_V4_POINT,  /* tex3D<float4>, point sampling, from a 3-D CUDA array (block-linear; the probe allocates it, buf is not read) */
+    PF_ARR_F32_LINEAR,/* tex3D<float>, linear filter, random position in a 3-D CUDA array: the texture arm's fetch */
     PF_COUNT
 };
 
 template <int F>
-__device__ __forceinline__ float probe_load(const float* p) {
+__device__ __forceinline__ float probe_load(const float* p, const float* base, cudaTextureObject_t tex) {
     float v, v1, v2, v3;
+    if (F == PF_TEX_F32) return tex1Dfetch<float>(tex, (int)(p - base));
+    if (F == PF_TEX_V4) {
+        const float4 q = tex1Dfetch<float4>(tex, (int)((p - base) >> 2));
+        return q.x + q.y + q.z + q.w;
+    }
     if (F == PF_LD) asm volatile("ld.global.f32 %0, [%1];" : "=f"(v) : "l"(p));
     else if (F == PF_NC) asm volatile("ld.global.nc.f32 %0, [%1];" : "=f"(v) : "l"(p));
     else if (F == PF_CG) asm volatile("ld.global.cg.f32 %0, [%1];" : "=f"(v) : "l"(p));
@@ -69,7 +79,7 @@ __device__ __forceinline__ unsigned long long probe_mix(unsigned long long x) {
 template <int F>
 __global__ void __launch_bounds__(256) vr_probe_dram_kernel(const float* __restrict__ buf, unsigned long long nblocks, int lines,
                                                             int span_floats, int group, int loads_per_thread, unsigned seed,
-                                                            float* __restrict__ sink) {
+                                                            float* __restrict__ sink, cudaTextureObject_t tex) {
     const unsigned long long tid = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
     float acc = 0.0f;
     for (int i0 = 0; i0 < loads_per_thread; i0 += 8) {
@@ -84,16 +94,46 @@ __global__ void __launch_bounds__(256) vr_probe_dram_kernel(const float* __restr
             p[u] = buf + blk * (unsigned long long)span_floats + line * 32u + sector * 8u;
         }
 #pragma unroll
-        for (int u = 0; u < 8; ++u) acc += probe_load<F>(p[u]);
+        for (int u = 0; u < 8; ++u) acc += probe_load<F>(p[u], buf, tex);
     }
     if (acc == 1.2345e-30f) sink[0] = acc; /* keeps the loads alive; never true for the zero / finite data used */
 }
 
-typedef void (*probe_fn)(const float*, unsigned long long, int, int, int, int, unsigned, float*);
+/* 3-D array flavours: every fetch at a hashed texel (point sampling: its centre; linear filter: anywhere in its cell) */
+template <int F>
+__global__ void __launch_bounds__(256) vr_probe_array_kernel(cudaTextureObject_t tex, int ex, int ey, int ez, int loads_per_thread,
+                                                             unsigned seed, float* __restrict__ sink) {
+    const unsigned long long tid = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x;
+    float acc = 0.0f;
+    for (int i0 = 0; i0 < loads_per_thread; i0 += 8) {
+        float x[8], y[8], z[8];
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+            const unsigned long long h = probe_mix((tid << 24) ^ (unsigned long long)(i0 + u) ^ ((unsigned long long)seed << 48));
+            const float f = F == PF_ARR_F32_LINEAR ? (float)((h >> 56) & 255u) * (1.0f / 256.0f) : 0.5f;
+            x[u] = (float)(unsigned)(h % (unsigned)ex) + f;
+            y[u] = (float)(unsigned)((h >> 20) % (unsigned)ey) + f;
+            z[u] = (float)(unsigned)((h >> 40) % (unsigned)ez) + f;
+        }
+#pragma unroll
+        for (int u = 0; u < 8; ++u) {
+            if (F == PF_ARR_V4_POINT) {
+                const float4 q = tex3D<float4>(tex, x[u], y[u], z[u]);
+                acc += q.x + q.y + q.z + q.w;
+            } else {
+                acc += tex3D<float>(tex, x[u], y[u], z[u]);
+            }
+        }
+    }
+    if (acc == 1.2345e-30f) sink[0] = acc;
+}
+
+typedef void (*probe_fn)(const float*, unsigned long long, int, int, int, int, unsigned, float*, cudaTextureObject_t);
 
 extern "C" int vr_debug_probe_dram(const void* buf, uint64_t bytes, int flavour, int span_bytes, int group, int loads_per_thread,
                                    int ctas, int l2_fetch_granularity, float* ms_out, uint64_t* loads_out, void* stream) {
-    if (!buf || !ms_out || !loads_out) return VR_ERR_INVALID_ARG;
+    if (!ms_out || !loads_out) return VR_ERR_INVALID_ARG;
+    if (!buf && flavour != PF_ARR_V4_POINT && flavour != PF_ARR_F32_LINEAR) return VR_ERR_INVALID_ARG;
     if (flavour < 0 || flavour >= PF_COUNT) return VR_ERR_INVALID_ARG;
     if (span_bytes < 128 || (span_bytes & (span_bytes - 1)) || group < 1 || group > span_bytes / 128) return VR_ERR_INVALID_ARG;
     if (loads_per_thread < 8 || (loads_per_thread % 8) || (loads_per_thread % group) || ctas < 1) return VR_ERR_INVALID_ARG;
@@ -102,7 +142,7 @@ extern "C" int vr_debug_probe_dram(const void* buf, uint64_t bytes, int flavour,
         vr_probe_dram_kernel<PF_LD>, vr_probe_dram_kernel<PF_NC>, vr_probe_dram_kernel<PF_CG>, vr_probe_dram_kernel<PF_CS>,
         vr_probe_dram_kernel<PF_CV>, vr_probe_dram_kernel<PF_NC_NOALLOC>, vr_probe_dram_kernel<PF_NC_L2_64>,
         vr_probe_dram_kernel<PF_NC_L2_128>, vr_probe_dram_kernel<PF_NC_L2_256>, vr_probe_dram_kernel<PF_NC_V4>,
-        vr_probe_dram_kernel<PF_NC_L2_64_ONLY>};
+        vr_probe_dram_kernel<PF_NC_L2_64_ONLY>, vr_probe_dram_kernel<PF_TEX_F32>, vr_probe_dram_kernel<PF_TEX_V4>, NULL, NULL};
     cudaStream_t st = (cudaStream_t)stream;
     if (l2_fetch_granularity == 32 || l2_fetch_granularity == 64 || l2_fetch_granularity == 128) {
         if (cudaDeviceSetLimit(cudaLimitMaxL2FetchGranularity, (size_t)l2_fetch_granularity) != cudaSuccess) {
@@ -117,12 +157,71 @@ extern "C" int vr_debug_probe_dram(const void* buf, uint64_t bytes, int flavour,
     cudaError_t e = cudaMalloc(&sink, sizeof(float));
     if (e == cudaSuccess) e = cudaEventCreate(&e0);
     if (e == cudaSuccess) e = cudaEventCreate(&e1);
+    /* texture flavours: a texture object over the buffer's head, as far as a linear-memory texture reaches (a device limit
+     * in ELEMENTS: float4 texels reach four times as far as float ones); the probed range shrinks to it */
+    cudaTextureObject_t tex = 0;
+    if (e == cudaSuccess && (flavour == PF_TEX_F32 || flavour == PF_TEX_V4)) {
+        const size_t el = flavour == PF_TEX_V4 ? 16 : 4;
+        int dev = 0, max_el = 0;
+        e = cudaGetDevice(&dev);
+        if (e == cudaSuccess) e = cudaDeviceGetAttribute(&max_el, cudaDevAttrMaxTexture1DLinearWidth, dev);
+        if (e == cudaSuccess) {
+            if (bytes > (uint64_t)max_el * el) bytes = (uint64_t)max_el * el;
+            if (bytes > ((uint64_t)1 << 31) * el / 1) bytes = ((uint64_t)1 << 31) * el; /* int texel index */
+            cudaResourceDesc res;
+            memset(&res, 0, sizeof(res));
+            res.resType = cudaResourceTypeLinear;
+            res.res.linear.devPtr = const_cast<void*>(buf);
+            res.res.linear.desc = flavour == PF_TEX_V4 ? cudaCreateChannelDesc<float4>() : cudaCreateChannelDesc<float>();
+            res.res.linear.sizeInBytes = (size_t)bytes;
+            cudaTextureDesc td;
+            memset(&td, 0, sizeof(td));
+            td.readMode = cudaReadModeElementType;
+            e = cudaCreateTextureObject(&tex, &res, &td, NULL);
+        }
+    }
+    cudaArray_t arr = NULL;
+    int ex = 0, ey = 0, ez = 0;
+    if (e == cudaSuccess && (flavour == PF_ARR_V4_POINT || flavour == PF_ARR_F32_LINEAR)) {
+        const size_t el = flavour == PF_ARR_V4_POINT ? 16 : 4;
+        ex = ey = 1024;
+        uint64_t slices = bytes / (el * 1024 * 1024);
+        ez = (int)(slices > 2048 ? 2048 : (slices < 1 ? 1 : slices));
+        const cudaChannelFormatDesc fmt = flavour == PF_ARR_V4_POINT ? cudaCreateChannelDesc<float4>() : cudaCreateChannelDesc<float>();
+        e = cudaMalloc3DArray(&arr, &fmt, make_cudaExtent((size_t)ex, (size_t)ey, (size_t)ez), 0);
+        if (e == cudaSuccess) {
+            cudaResourceDesc res;
+            memset(&res, 0, sizeof(res));
+            res.resType = cudaResourceTypeArray;
+            res.res.array.array = arr;
+            cudaTextureDesc td;
+            memset(&td, 0, sizeof(td));
+            td.addressMode[0] = td.addressMode[1] = td.addressMode[2] = cudaAddressModeClamp;
+            td.filterMode = flavour == PF_ARR_F32_LINEAR ? cudaFilterModeLinear : cudaFilterModePoint;
+            td.readMode = cudaReadModeElementType;
+            e = cudaCreateTextureObject(&tex, &res, &td, NULL);
+        }
+    }
     const unsigned long long nblocks = bytes / (uint64_t)span_bytes;
     const int lines = span_bytes / 128;
-    if (e == cudaSuccess) { /* one untimed launch (different addresses), then the timed one */
-        table[flavour]<<<ctas, 256, 0, st>>>((const float*)buf, nblocks, lines, span_bytes / 4, group, loads_per_thread, 1u, sink);
+    if (e == cudaSuccess && arr) {
+        if (flavour == PF_ARR_V4_POINT) {
+            vr_probe_array_kernel<PF_ARR_V4_POINT><<<ctas, 256, 0, st>>>(tex, ex, ey, ez, loads_per_thread, 1u, sink);
+            e = cudaEventRecord(e0, st);
+            vr_probe_array_kernel<PF_ARR_V4_POINT><<<ctas, 256, 0, st>>>(tex, ex, ey, ez, loads_per_thread, 2u, sink);
+        } else {
+            vr_probe_array_kernel<PF_ARR_F32_LINEAR><<<ctas, 256, 0, st>>>(tex, ex, ey, ez, loads_per_thread, 1u, sink);
+            e = cudaEventRecord(e0, st);
+            vr_probe_array_kernel<PF_ARR_F32_LINEAR><<<ctas, 256, 0, st>>>(tex, ex, ey, ez, loads_per_thread, 2u, sink);
+        }
+        if (e == cudaSuccess) e = cudaEventRecord(e1, st);
+        if (e == cudaSuccess) e = cudaGetLastError();
+        if (e == cudaSuccess) e = cudaEventSynchronize(e1);
+        if (e == cudaSuccess) e = cudaEventElapsedTime(ms_out, e0, e1);
+    } else if (e == cudaSuccess) { /* one untimed launch (different addresses), then the timed one */
+        table[flavour]<<<ctas, 256, 0, st>>>((const float*)buf, nblocks, lines, span_bytes / 4, group, loads_per_thread, 1u, sink, tex);
         e = cudaEventRecord(e0, st);
-        table[flavour]<<<ctas, 256, 0, st>>>((const float*)buf, nblocks, lines, span_bytes / 4, group, loads_per_thread, 2u, sink);
+        table[flavour]<<<ctas, 256, 0, st>>>((const float*)buf, nblocks, lines, span_bytes / 4, group, loads_per_thread, 2u, sink, tex);
         if (e == cudaSuccess) e = cudaEventRecord(e1, st);
         if (e == cudaSuccess) e = cudaGetLastError();
         if (e == cudaSuccess) e = cudaEventSynchronize(e1);
@@ -131,6 +230,8 @@ extern "C" int vr_debug_probe_dram(const void* buf, uint64_t bytes, int flavour,
     *loads_out = (uint64_t)ctas * 256ull * (uint64_t)loads_per_thread;
     if (e0) cudaEventDestroy(e0);
     if (e1) cudaEventDestroy(e1);
+    if (tex) cudaDestroyTextureObject(tex);
+    if (arr) cudaFreeArray(arr);
     cudaFree(sink);
     if (e != cudaSuccess) {
         cudaGetLastError();
