@@ -325,6 +325,20 @@ int vr_render_host_wait(vr_volume* v);
 int vr_composite(const float* const* layers, const int* rects, const int* order, int n,
                  int width, int height, float* out, void* stream);
 
+/* The same operation for callers that must not allocate (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc): vr_composite takes its two small device tables from cudaMallocAsync; this
+ * entry keeps them in a fixed __device__ array inside the library (11 KB, held by every GPU that loads libvr until
+ * the process exits) and calls no cudaMalloc / cudaFree / allocating routine, on the host side either.
+ *   Arguments, layouts and result exactly as vr_composite (same kernel: the frames are bit-identical), except
+ *   n <= VR_COMPOSITE_STATIC_MAX_LAYERS: more layers -> VR_ERR_INVALID_ARG, nothing launched.
+ *   All calls share the one array per device, and it keeps the last call's tables (a call rewrites the entries it
+ *   reads; nothing has to be cleared). Calls on one stream are ordered by the stream; calls that OVERLAP on the GPU
+ *   (different streams without a dependency) race on the tables: serialise them.
+ * Errors: VR_ERR_INVALID_ARG (NULL, n, rectangles, order not a permutation), VR_ERR_CUDA. */
+#define VR_COMPOSITE_STATIC_MAX_LAYERS 256
+int vr_composite_static(const float* const* layers, const int* rects, const int* order, int n,
+                        int width, int height, float* out, void* stream);
+
 /* ------------------------------------------------------------------------------------------
  * Multi-GPU sort-last (PAPER.md:136-138 data partitioning,
  * :170-174 two-stage compositing, :178-184 direct send of rectangle-packed partial frames).

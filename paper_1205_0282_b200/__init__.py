@@ -28,7 +28,7 @@ STATUS = {0: "VR_OK", 1: "VR_ERR_INVALID_ARG", 2: "VR_ERR_OUT_OF_MEMORY", 3: "VR
 # every symbol include/vr.h declares (tests check the library exports each of them)
 SYMBOLS = (
     "vr_volume_create", "vr_volume_create_layout", "vr_volume_destroy", "vr_volume_upload", "vr_volume_download", "vr_debug_brick_data",
-    "vr_set_transfer_function", "vr_set_early_termination", "vr_volume_minmax", "vr_set_culling", "vr_set_traversal", "vr_set_sampler", "vr_volume_release_store", "vr_set_allocator", "vr_reserve_views", "vr_debug_brick_minmax", "vr_debug_cell_flags", "vr_render", "vr_render_host", "vr_render_host_async", "vr_render_host_wait", "vr_composite",
+    "vr_set_transfer_function", "vr_set_early_termination", "vr_volume_minmax", "vr_set_culling", "vr_set_traversal", "vr_set_sampler", "vr_volume_release_store", "vr_set_allocator", "vr_reserve_views", "vr_debug_brick_minmax", "vr_debug_cell_flags", "vr_render", "vr_render_host", "vr_render_host_async", "vr_render_host_wait", "vr_composite", "vr_composite_static",
     "vr_num_bricks", "vr_debug_brick_order", "vr_debug_rects", "vr_debug_ray_bricks", "vr_debug_subimages",
     "vr_volume_create_part", "vr_render_part", "vr_render_part_pieces", "vr_part_rect", "vr_composite_parts", "vr_kd_partition", "vr_part_order",
     "vr_set_counting", "vr_set_timing", "vr_debug_stats", "vr_debug_stage_times", "vr_debug_probe_dram", "vr_debug_set_upload_path", "vr_launch_count", "vr_last_error",
@@ -85,6 +85,7 @@ def lib():
         L.vr_render_host_async.argtypes = [vp, vp, vp, ci, ci, cf, ci, vp, vp]
         L.vr_render_host_wait.argtypes = [vp]
         L.vr_composite.argtypes = [vp, vp, vp, ci, ci, ci, vp, vp]
+        L.vr_composite_static.argtypes = [vp, vp, vp, ci, ci, ci, vp, vp]
         L.vr_volume_create_part.argtypes = [ci, ci, ci, ci, ci, vp, vp, ctypes.POINTER(vp)]
         L.vr_render_part.argtypes = [vp, vp, vp, ci, ci, cf, ci, vp, vp, vp]
         L.vr_part_rect.argtypes = [ci, ci, ci, ci, vp, vp, vp, vp, ci, ci, vp]
@@ -504,6 +505,26 @@ def composite(layers, rects, order, width, height, out, stream=None):
         _require(l.numel() == (rc_[2] - rc_[0]) * (rc_[3] - rc_[1]) * 4, 'l.numel() == (rc_[2] - rc_[0]) * (rc_[3] - rc_[1]) * 4')
     _require(out.is_cuda and out.is_contiguous() and out.numel() == width * height * 4, 'out.is_cuda and out.is_contiguous() and out.numel() == width * height * 4')
     rc = lib().vr_composite(ptrs, r.ctypes.data, o.ctypes.data, n, int(width), int(height), out.data_ptr(), _stream(stream))
+    if rc != 0:
+        raise VrError(rc, lib().vr_last_error(None).decode())
+    return out
+
+
+COMPOSITE_STATIC_MAX_LAYERS = 256
+
+
+def composite_static(layers, rects, order, width, height, out, stream=None):
+    """vr_composite_static: vr_composite without any allocation (the device tables live in a fixed array inside the
+    library; at most COMPOSITE_STATIC_MAX_LAYERS layers; calls that overlap on the GPU race). Arguments as composite."""
+    n = len(layers)
+    ptrs = (ctypes.c_void_p * max(n, 1))(*[l.data_ptr() for l in layers])
+    r = np.ascontiguousarray(rects, dtype=np.int32).reshape(n, 4)
+    o = np.ascontiguousarray(order, dtype=np.int32).reshape(n)
+    for l, rc_ in zip(layers, r):
+        _require(l.is_cuda and l.is_contiguous() and l.element_size() == 4, 'l.is_cuda and l.is_contiguous() and l.element_size() == 4')
+        _require(l.numel() == (rc_[2] - rc_[0]) * (rc_[3] - rc_[1]) * 4, 'l.numel() == (rc_[2] - rc_[0]) * (rc_[3] - rc_[1]) * 4')
+    _require(out.is_cuda and out.is_contiguous() and out.numel() == width * height * 4, 'out.is_cuda and out.is_contiguous() and out.numel() == width * height * 4')
+    rc = lib().vr_composite_static(ptrs, r.ctypes.data, o.ctypes.data, n, int(width), int(height), out.data_ptr(), _stream(stream))
     if rc != 0:
         raise VrError(rc, lib().vr_last_error(None).decode())
     return out

@@ -16,6 +16,13 @@
 
 static char g_err[512] = "no error";
 static char* g_err_buf() { return g_err; }
+/* for entry points that live in other files (vr_composite_static) */
+void vr_global_error(const char* fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+}
 
 struct vr_volume {
     VrGrid grid;

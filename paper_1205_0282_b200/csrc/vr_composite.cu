@@ -153,3 +153,101 @@ cudaError_t vr_launch_composite(const VrCompLayer* layers, const int* order, int
         vr_composite_kernel<VR_MIP_PARTS><<<grid, COMP_THREADS, 0, st>>>(layers, order, n, win, lut, out, bound);
     return cudaGetLastError();
 }
+
+/* ------------------------------------------------------------------------------------------
+ * vr_composite_static: stand-alone compositing (row a9) for callers that must not allocate - code under CUDA graph
+ * capture, tight serving loops, harnesses that forbid cudaMalloc. vr_composite takes its two small device tables
+ * (layer table, visibility order) from cudaMallocAsync; here they live in a file-scope __device__ array of a fixed,
+ * modest size, which every GPU that loads the library holds until the process exits (11 KB). The kernel is the same.
+ *
+ * The array's name is a host-side stand-in in host code, not a device address: the address comes from
+ * cudaGetSymbolAddress, once per device, with that device current.
+ * Every call shares the array; it keeps the last call's tables. Nothing in it has to start at zero: a call rewrites
+ * entries [0, n) of both tables and its kernel reads no others. Calls that overlap on the GPU (different streams, no
+ * dependency between them) race on the tables; calls on one stream are ordered by it.
+ */
+#include <mutex>
+
+#define VR_COMP_STATIC_MAX VR_COMPOSITE_STATIC_MAX_LAYERS
+static __device__ __align__(256) unsigned char g_comp_scratch[VR_COMP_STATIC_MAX * sizeof(VrCompLayer) + VR_COMP_STATIC_MAX * sizeof(int)];
+
+void vr_global_error(const char* fmt, ...); /* vr_api.cu: the message vr_last_error(NULL) returns */
+
+#define COMP_MAX_DEVICES 64
+static unsigned char* g_comp_scratch_addr[COMP_MAX_DEVICES]; /* device address of g_comp_scratch on each device, or NULL */
+static std::mutex g_comp_scratch_lock;
+
+/* device address of the scratch array on the CURRENT device (looked up on the first call per device) */
+static cudaError_t comp_scratch_address(unsigned char** out) {
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= COMP_MAX_DEVICES) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> hold(g_comp_scratch_lock);
+    if (!g_comp_scratch_addr[dev]) {
+        void* p = NULL;
+        e = cudaGetSymbolAddress(&p, g_comp_scratch);
+        if (e != cudaSuccess) return e;
+        g_comp_scratch_addr[dev] = static_cast<unsigned char*>(p);
+    }
+    *out = g_comp_scratch_addr[dev];
+    return cudaSuccess;
+}
+
+extern "C" int vr_composite_static(const float* const* layers, const int* rects, const int* order, int n, int width, int height,
+                                   float* out, void* stream) {
+    if (!layers || !rects || !order || !out) {
+        vr_global_error("vr_composite_static: NULL argument");
+        return VR_ERR_INVALID_ARG;
+    }
+    if (n < 0 || n > VR_COMP_STATIC_MAX) {
+        vr_global_error("vr_composite_static: n = %d layers, the static scratch holds at most %d (use vr_composite)", n, VR_COMP_STATIC_MAX);
+        return VR_ERR_INVALID_ARG;
+    }
+    if (width <= 0 || height <= 0 || width > 32768 || height > 32768) {
+        vr_global_error("vr_composite_static: bad frame size %dx%d", width, height);
+        return VR_ERR_INVALID_ARG;
+    }
+    VrCompLayer tab[VR_COMP_STATIC_MAX]; /* host tables on the stack: no host allocation either */
+    unsigned char seen[VR_COMP_STATIC_MAX];
+    memset(seen, 0, sizeof(seen));
+    for (int l = 0; l < n; ++l) {
+        const int* r = rects + 4 * l;
+        if (r[0] < 0 || r[1] < 0 || r[2] > width || r[3] > height || r[2] < r[0] || r[3] < r[1]) {
+            vr_global_error("vr_composite_static: rectangle %d outside the viewport", l);
+            return VR_ERR_INVALID_ARG;
+        }
+        if (!layers[l] && r[2] > r[0] && r[3] > r[1]) {
+            vr_global_error("vr_composite_static: layer %d is NULL", l);
+            return VR_ERR_INVALID_ARG;
+        }
+        if (order[l] < 0 || order[l] >= n || seen[order[l]]) {
+            vr_global_error("vr_composite_static: order is not a permutation");
+            return VR_ERR_INVALID_ARG;
+        }
+        seen[order[l]] = 1;
+        VrCompLayer& L = tab[l];
+        L.x0 = r[0]; L.y0 = r[1]; L.x1 = r[2]; L.y1 = r[3];
+        L.sx0 = r[0]; L.sy0 = r[1];
+        L.pitch = r[2] - r[0];
+        L.pad = 0;
+        L.addr = (unsigned long long)(uintptr_t)layers[l];
+    }
+    unsigned char* scratch = NULL;
+    cudaError_t e = comp_scratch_address(&scratch);
+    cudaStream_t st = (cudaStream_t)stream;
+    VrCompLayer* d_tab = reinterpret_cast<VrCompLayer*>(scratch);
+    int* d_order = reinterpret_cast<int*>(scratch + VR_COMP_STATIC_MAX * sizeof(VrCompLayer));
+    /* pageable (stack) sources: the runtime has taken the bytes when the call returns; the writes are ordered on `st` */
+    if (e == cudaSuccess && n > 0) e = cudaMemcpyAsync(d_tab, tab, sizeof(VrCompLayer) * n, cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess && n > 0) e = cudaMemcpyAsync(d_order, order, sizeof(int) * n, cudaMemcpyHostToDevice, st);
+    VrLut none;
+    memset(&none, 0, sizeof(none));
+    if (e == cudaSuccess) e = vr_launch_composite(d_tab, d_order, n, width, height, VR_ALPHA, none, out, NULL, NULL, st);
+    if (e != cudaSuccess) {
+        cudaGetLastError();
+        vr_global_error("vr_composite_static: %s", cudaGetErrorString(e));
+        return VR_ERR_CUDA;
+    }
+    return VR_OK;
+}
