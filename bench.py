@@ -890,9 +890,11 @@ def main():
     promote = False  # auto: the texture arm on the released store becomes the headline (the run's last leg)
     if args.sampler == "auto":
         args.sampler = "manual"
+        fits = torch.cuda.mem_get_info()[0] > 1.15 * wl["nx"] * wl["ny"] * wl["nz"] * 4  # a second copy fits (c0 - c2, n1)
+        if args.mode == "mip" and args.traversal == "sort_last" and fits and not args.release_store:
+            args.sampler = "texture"  # exact MIP: the arrays rule samples out, the float32 store supplies the values
         if args.mode == "alpha" and args.traversal == "sort_last" and args.tf in ("ramp", "translucent") and not args.release_store:
-            free_b = torch.cuda.mem_get_info()[0]
-            if free_b > 1.15 * wl["nx"] * wl["ny"] * wl["nz"] * 4:  # a second copy fits (c0 - c2, n1)
+            if fits:
                 args.sampler = "texture"
             else:
                 promote = bool(getattr(g, "releasable", False)) and not args.no_variants and world == 1
@@ -941,7 +943,7 @@ def main():
                     "synchronous_value": round(e2e_sync_fps, 3),
                     "synchronous_what": "vr_render_host: the caller waits for each frame's copy before queueing the next"},
             "clocks": m["clocks"],
-            "sampler": ("texture: 3-D CUDA arrays behind texture objects, a second copy beside the store" if args.sampler == "texture" and args.mode == "alpha"
+            "sampler": ("texture: 3-D CUDA arrays behind texture objects, a second copy beside the store" if args.sampler == "texture"
                         else "manual: hand-rolled float32 tri-linear from the 4x4x2 micro-tiled store") +
                        (" (chosen by --sampler auto)" if args.sampler_asked == "auto" else ""),
             "stage_ms": {"setup": round(float(m["stages"][:, 0].mean()), 4), "raycast": round(float(m["stages"][:, 1].mean()), 4),
@@ -954,7 +956,7 @@ def main():
                          "max": round(float(m["stages"].sum(axis=1).max()), 4), "views": int(len(m["stages"]))},
             "roofline": roofline_of(m["counts"], m["stages"], m["stage_views"], peak, peak_src,
                                     traffic_of(args.workload, args.mode, args.tf + ("" if args.traversal == "sort_last" else "/fused") +
-                                               ("/texture" if args.sampler == "texture" and args.mode == "alpha" else ""))),
+                                               ("/texture" if args.sampler == "texture" else ""))),
             "build_s": round(t_build, 1), "upload": dict(g.upload_stats, frac_of_hbm_peak=round(g.upload_stats["gb_per_s"] / peak, 4)),
             "minmax": dict(g.minmax_stats, frac_of_hbm_peak=round(g.minmax_stats["gb_per_s"] / peak, 4))}
     # which roofline bounds the ray-cast kernel: DRAM for the sparsely sampled 103 GB cube (0.03 samples per
@@ -1012,8 +1014,8 @@ def main():
                 extra = {"frames_per_s_skipping_off": round(K / (ms_off * 1e-3), 3)}
             g.set_traversal(vr.SORT_LAST)
             g.set_early_termination(wl["tau"])
-            variants.append({"mode": vmode, "tf": vtf, "traversal": vtrav, "sampler": ("manual" if vmode != "alpha" or (vtf == "threshold" and vsamp == "texture") else vsamp) +
-                                        (" (MIP keeps the hand-rolled sampler)" if vmode != "alpha" and vsamp == "texture" else "") +
+            variants.append({"mode": vmode, "tf": vtf, "traversal": vtrav, "sampler": ("manual" if (vtf == "threshold" and vsamp == "texture") else vsamp) +
+                                        (" (MIP: the arrays as an exact filter in front of the hand-rolled sampler)" if vmode != "alpha" and vsamp == "texture" else "") +
                                         (" (a stepped table keeps the hand-rolled sampler)" if vtf == "threshold" and vsamp == "texture" else ""),
                              "frames_per_s": round(K / (v["ms"] * 1e-3), 3), **extra,
                              "gsamples_per_s": round(v["samples"] / (v["ms"] * 1e-3) / 1e9, 3),
@@ -1024,7 +1026,7 @@ def main():
                              "counts_": v["counts"],
                              "roofline": roofline_of(v["counts"], v["stages"], v["stage_views"], peak, peak_src,
                                                      traffic_of(args.workload, vmode, vtf + ("" if vtrav == "sort_last" else "/fused") +
-                                                                ("/texture" if vsamp == "texture" and vmode == "alpha" and vtf != "threshold" else "")))})
+                                                                ("/texture" if vsamp == "texture" and vtf != "threshold" else "")))})
         g.set_transfer_function(tf, *tf_range(wl))
         g.set_sampler(vr.SAMPLER_TEXTURE if args.sampler == "texture" else vr.SAMPLER_MANUAL)
         line["variants"] = variants

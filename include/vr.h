@@ -271,8 +271,15 @@ int vr_set_traversal(vr_volume* v, int traversal);
  * stays as it was) and refilled from the store on the device by the first frame after an upload. The sample
  * SET is unchanged (same FP64 set-up); the hardware's 8-bit interpolation weights perturb sample values by up
  * to 2^-9 of the local voxel differences, which keeps VR_ALPHA inside its 2e-3 tolerance but moves early-
- * termination decisions of rays whose opacity passes tau within ~1e-4 of it. VR_MIP frames (1e-5), fused
- * frames and counting mode 2 always use the hand-rolled path, and so do (i) bricks that hold blanked (NaN) voxels -
+ * termination decisions of rays whose opacity passes tau within ~1e-4 of it.
+ * VR_MIP frames (1e-5) of the VR_SORT_LAST traversal use the arrays as an EXACT filter: a filtered fetch is within
+ * range / 64 (+ 2^-14 of the largest magnitude) of the hand-rolled value for every sample of a brick (the brick's
+ * range: row f1), so only samples whose filtered value lies within twice that of the largest one seen on their ray
+ * segment can be the segment's maximum; only those are evaluated - by the hand-rolled float32 sampler from the store.
+ * The frame is bit-identical to VR_SAMPLER_MANUAL's (a maximum does not depend on the order of its operands); it
+ * needs both copies (not a released store) and is not combined with stepping over empty macro-cells (R19: where
+ * that pays, it is used instead). Fused MIP frames
+ * and counting mode 2 always use the hand-rolled path, and so do (i) bricks that hold blanked (NaN) voxels -
  * the filter cannot apply R14's rule - and (ii) frames whose transfer function has a step: two neighbouring entries
  * further apart than 2.56/n in a channel (a threshold, a toe). The filter's value error is about one table entry on
  * unit-sigma noise; across a step that is a wrong opacity, not 2e-3 (measured: 8e-2 on a threshold table).

@@ -1078,9 +1078,19 @@ static int render_frame(vr_volume* v, const float* view, const float* proj, int 
         if (rc) return rc;
         mip_skipping = v->mip_skip_useful;
     }
-    const bool use_tex = v->sampler == VR_SAMPLER_TEXTURE && mode == VR_ALPHA && v->counting != 2 && v->tf_smooth;
+    /* texture arm: ALPHA frames with a smooth table take their values from the arrays; MIP frames use the arrays as an exact
+     * filter in front of the hand-rolled sampler (needs the float32 store and the bricks' ranges; where stepping over empty
+     * macro-cells pays, that stays) */
+    const bool tex_alpha = v->sampler == VR_SAMPLER_TEXTURE && mode == VR_ALPHA && v->counting != 2 && v->tf_smooth;
+    const bool tex_mip = v->sampler == VR_SAMPLER_TEXTURE && mode == VR_MIP && v->counting != 2 && !v->store_released &&
+                         v->traversal == VR_SORT_LAST && !mip_skipping;
+    const bool use_tex = tex_alpha || tex_mip;
     if (use_tex) { /* after an upload only */
         rc = ensure_tex(v, st);
+        if (rc) return rc;
+    }
+    if (tex_mip) {
+        rc = ensure_minmax(v, st);
         if (rc) return rc;
     }
     if (timing) VR_CUDA(v, cudaEventRecord(ev[0], st));
@@ -1109,6 +1119,7 @@ static int render_frame(vr_volume* v, const float* view, const float* proj, int 
     p.bitmap = NULL;
     p.tex = use_tex ? vr_tex_table(v->tex) : NULL;
     p.tex_nan = use_tex ? vr_tex_nan_table(v->tex) : NULL;
+    p.brick_mm = tex_mip ? v->d_mm : NULL;
     p.cell_bits = skipping ? v->d_cell_bits : NULL;
     p.cell_mm = mip_skipping ? v->d_cell_mm : NULL;
     p.nc[0] = v->nc[0]; p.nc[1] = v->nc[1]; p.nc[2] = v->nc[2];

@@ -146,6 +146,7 @@ struct VrRaycastParams {
     void* sub;          /* float4[] (ALPHA) or float[] (MIP) */
     const cudaTextureObject_t* tex; /* texture arm (vr_texture.cu): one texture object per slot, or NULL = hand-rolled sampling */
     const int* tex_nan;             /* 1 per slot that holds blanked voxels: sampled by hand also in the texture arm (R14) */
+    const float2* brick_mm;         /* texture arm, MIP: (min, max) of every brick's padded cells (row f1), indexed by brick */
     unsigned* bitmap;   /* counting variant only: one bit per brick-store cell, or NULL */
     const unsigned* cell_bits; /* R19: one bit per 8x8x8 macro-cell, 1 = transparent under the LUT; NULL = no skipping */
     const float2* cell_mm; /* R19, MIP: (min, max) per macro-cell (a cell whose max cannot raise the ray's maximum is skipped); NULL = off */

@@ -37,6 +37,12 @@
 #ifndef VR_TEX_DEPTH
 #define VR_TEX_DEPTH 4 /* texture fetches a lane keeps in flight */
 #endif
+#ifndef VR_TEX_MIP_EPS
+#define VR_TEX_MIP_EPS (1.0f / 64.0f) /* bound of |filtered - exact| in units of the brick's data range (see the MIP loop) */
+#endif
+#ifndef VR_MIP_QUEUE
+#define VR_MIP_QUEUE 4 /* candidate samples a lane queues before the warp evaluates them by hand */
+#endif
 #ifndef VR_TEX_COPIES
 #define VR_TEX_COPIES 8 /* copies of the table in the texture-arm instances (more CTAs per SM: less room for each) */
 #endif
@@ -151,7 +157,15 @@ vr_raycast_kernel(const VrRaycastParams prm) {
         cudaTextureObject_t tex = 0;
         float P0x = 0.0f, P0y = 0.0f, P0z = 0.0f, Dfx = 0.0f, Dfy = 0.0f, Dfz = 0.0f;
         const int n0 = n;
-        const bool use_tex = TEX && __ldg(prm.tex_nan + slot_b) == 0; /* warp-uniform: one brick per item */
+        bool use_tex = TEX && __ldg(prm.tex_nan + slot_b) == 0; /* warp-uniform: one brick per item */
+        /* MIP through the arrays (below): eps bounds |filtered - exact| for every sample of this brick */
+        float mip_eps = 0.0f;
+        if (TEX && MODE == VR_MIP && use_tex) {
+            const float2 bmm = __ldg(prm.brick_mm + b);
+            /* + the float32 rounding of either filter, which scales with the magnitude, not the range */
+            mip_eps = (bmm.y - bmm.x) * VR_TEX_MIP_EPS + fmaxf(fabsf(bmm.x), fabsf(bmm.y)) * (1.0f / 16384.0f);
+            use_tex = mip_eps >= 0.0f && mip_eps < INFINITY; /* a brick without finite voxels keeps the hand-rolled loop */
+        }
         if (use_tex) {
             tex = __ldg(prm.tex + slot_b);
             const double h = 1.0 / 4294967296.0;
@@ -179,7 +193,7 @@ vr_raycast_kernel(const VrRaycastParams prm) {
          * fetched beyond a termination are dropped: at most VR_TEX_DEPTH - 1 per ray segment). The texture arm is bound by
          * the latency of its one fetch per sample at the 32 warps per SM its cache footprint allows (ncu: nothing above 40 %,
          * 12.8 warps per issue waiting on the scoreboard); this keeps VR_TEX_DEPTH fetches per warp in flight instead of one. */
-        while (TEX && !SKIP && use_tex && __any_sync(FULL_MASK, active)) {
+        while (TEX && MODE == VR_ALPHA && !SKIP && use_tex && __any_sync(FULL_MASK, active)) {
             if (active) {
                 const float kf = (float)(n0 - n);
                 float vq[VR_TEX_DEPTH];
@@ -200,7 +214,7 @@ vr_raycast_kernel(const VrRaycastParams prm) {
                 }
             }
         }
-        while (TEX && SKIP && use_tex && __any_sync(FULL_MASK, active)) {
+        while (TEX && MODE == VR_ALPHA && SKIP && use_tex && __any_sync(FULL_MASK, active)) {
             /* texture arm (built-in tri-linear interpolation): one TEX instead of 8 loads, the index
              * arithmetic and 7 FMA; the lattice is kept only where macro-cells are looked up (SKIP) */
             if (active) {
@@ -228,6 +242,76 @@ vr_raycast_kernel(const VrRaycastParams prm) {
                 n -= adv;
                 active = n > 0 && !stopped;
             }
+        }
+        /* MIP through the arrays, EXACT (bit for bit the hand-rolled result): the filtered fetch serves as a bound, not as the
+         * value. |filtered - exact| <= eps for every sample of the brick (the unit quantises the three weights to 8 fractional
+         * bits: at most 3/256 of the largest difference between the 8 voxels, itself at most the brick's range; the float32 texel
+         * coordinate adds < 3e-4 of it; eps = range / 64 + 2^-14 of the largest magnitude for the filters' own rounding),
+         * so with hmax = the largest filtered value so far the segment's exact maximum is >= hmax - eps, and a sample whose
+         * filtered value is below hmax - 2 eps cannot be it: only the others (the CANDIDATES: a few per cent on noise, the
+         * records of the running maximum and their near misses) are evaluated by hand, in float32 from the tiled store, at the
+         * same lattice position q0 + j D the hand-rolled loop reaches by repeated addition. A maximum does not depend on the
+         * order of its operands. Candidates wait in a queue of VR_MIP_QUEUE (step, filtered value) pairs per lane; the warp
+         * empties all queues when one is full, so the hand-rolled evaluations run with most lanes busy. */
+        if (TEX && MODE == VR_MIP && use_tex) {
+            int qj[VR_MIP_QUEUE];
+            float qv[VR_MIP_QUEUE];
+            int qn = 0;
+            float hmax = -INFINITY;
+            const float eps2 = mip_eps + mip_eps;
+            const long long q0x = L.q[0], q0y = L.q[1], q0z = L.q[2];
+            int j = 0; /* next lattice step of this lane */
+            while (__any_sync(FULL_MASK, active || qn > 0)) {
+                /* empty the queues: at the end of the segment, when a lane's queue is full, or when a lane may have
+                 * reached the value at which MIP stops */
+                const bool want = qn > 0 && (!active || qn == VR_MIP_QUEUE || hmax - mip_eps >= mip_stop);
+                if (__any_sync(FULL_MASK, want)) {
+#pragma unroll
+                    for (int q = 0; q < VR_MIP_QUEUE; ++q) {
+                        if (q < qn && qv[q] + mip_eps > acc.r && qv[q] >= hmax - eps2) {
+                            Lattice Lj;
+                            Lj.q[0] = q0x + D[0] * qj[q], Lj.q[1] = q0y + D[1] * qj[q], Lj.q[2] = q0z + D[2] * qj[q];
+                            acc.r = fmaxf(acc.r, trilinear<LAY, PT, CLAMP, false>(brick, g, ext, Lj, prm.bitmap, (long long)slot_b * g.slot));
+                        }
+                    }
+                    qn = 0;
+                    stopped = acc.r >= mip_stop;
+                    active = j < n0 && !stopped;
+                }
+                if (active) {
+                    const float kf = (float)j;
+                    float vq[VR_TEX_DEPTH];
+#pragma unroll
+                    for (int u = 0; u < VR_TEX_DEPTH; ++u) {
+                        const float ku = kf + (float)u;
+                        vq[u] = tex3D<float>(tex, fmaf(ku, Dfx, P0x), fmaf(ku, Dfy, P0y), fmaf(ku, Dfz, P0z));
+                    }
+#pragma unroll
+                    for (int u = 0; u < VR_TEX_DEPTH; ++u) {
+                        if (j < n0) {
+                            const float v = vq[u];
+                            if (COUNT) ++nsamples; /* a brick seen through its array has no blanked voxel */
+                            if (v >= hmax - eps2 && v + mip_eps > acc.r) {
+                                if (qn < VR_MIP_QUEUE) {
+#pragma unroll
+                                    for (int q = 0; q < VR_MIP_QUEUE; ++q)
+                                        if (q == qn) qj[q] = j, qv[q] = v;
+                                    ++qn;
+                                } else { /* no room (several candidates in one batch of fetches): evaluated at once */
+                                    Lattice Lj;
+                                    Lj.q[0] = q0x + D[0] * j, Lj.q[1] = q0y + D[1] * j, Lj.q[2] = q0z + D[2] * j;
+                                    acc.r = fmaxf(acc.r, trilinear<LAY, PT, CLAMP, false>(brick, g, ext, Lj, prm.bitmap, (long long)slot_b * g.slot));
+                                }
+                            }
+                            hmax = fmaxf(hmax, v);
+                            ++j;
+                        }
+                    }
+                    active = j < n0;
+                }
+            }
+            n = 0;
+            stopped = acc.r >= mip_stop;
         }
         while (!(TEX && use_tex) && __any_sync(FULL_MASK, active)) {
             if (active) {
@@ -303,7 +387,7 @@ vr_raycast_kernel(const VrRaycastParams prm) {
                     L.q[a] = to_fixed(p - ((double)(blo[a] - g.ghost) + 0.5));
                 }
                 float v;
-                if (TEX && use_tex) { /* the exit samples through the array as well: a released store has no float32 cells */
+                if (TEX && MODE == VR_ALPHA && use_tex) { /* the exit samples through the array as well: a released store has no float32 cells */
                     const double h = 1.0 / 4294967296.0;
                     v = tex3D<float>(tex, (float)((double)L.q[0] * h + 0.5), (float)((double)L.q[1] * h + 0.5), (float)((double)L.q[2] * h + 0.5));
                 } else {
@@ -397,6 +481,11 @@ static cudaError_t launch_mode(const VrRaycastParams& p, long long ctas, bool sp
         if (!clamp && p.cell_bits != NULL) return launch_variant<VR_ALPHA, LAY_TILE442, 0, false, COUNT, true, true>(p, ctas, sparse, st);
         return clamp ? launch_variant<VR_ALPHA, LAY_TILE442, 0, true, COUNT, false, true>(p, ctas, sparse, st)
                      : launch_variant<VR_ALPHA, LAY_TILE442, 0, false, COUNT, false, true>(p, ctas, sparse, st);
+    }
+    if (is_tile442(p.grid) && p.tex != NULL && MODE == VR_MIP && p.bitmap == NULL && p.brick_mm != NULL && p.cell_mm == NULL) {
+        /* texture arm, MIP: the arrays as an exact filter in front of the hand-rolled sampler (the MIP loop of the kernel) */
+        return clamp ? launch_variant<VR_MIP, LAY_TILE442, 0, true, COUNT, false, true>(p, ctas, sparse, st)
+                     : launch_variant<VR_MIP, LAY_TILE442, 0, false, COUNT, false, true>(p, ctas, sparse, st);
     }
     if (is_tile442(p.grid)) {
         /* R19: macro-cell skipping - ALPHA when the transfer function has a transparent range, MIP when the cube has empty space */

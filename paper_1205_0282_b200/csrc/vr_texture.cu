@@ -13,7 +13,8 @@
  * centres - R3's convention exactly, with the padded cell index as the texel index. The arrays
  * are a second copy of the brick store, filled from it on the device through surface objects
  * (vr_tex_fill_kernel) after an upload; the hand-rolled path keeps the float32 store, which
- * VR_MIP always uses (the hardware filter's 8 fractional weight bits cannot meet MIP's 1e-5), and which
+ * VR_MIP needs for its values (the hardware filter's 8 fractional weight bits cannot meet MIP's 1e-5: MIP frames use
+ * the arrays only to rule out the samples that cannot be a ray's maximum, vr_raycast.cu), and which
  * VR_ALPHA keeps using for bricks that hold blanked (NaN) voxels: the filter cannot apply R14's rule.
  */
 #include <string.h>

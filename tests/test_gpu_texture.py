@@ -75,7 +75,7 @@ def test_bricked_ragged_texture_frames_subimages_and_counts(vr, ghost, tau):
                     max_flagged=1.0)
         if tau > 1:
             assert n_tex == int(ref["counts"][..., 0].sum())
-        # MIP frames keep the hand-rolled sampler (1e-5): bit-identical with the sampler switched back
+        # MIP frames are exact through the arrays too (candidates re-evaluated by hand): bit-identical with the sampler switched back
         m_tex = gpu_frame(g, view, proj, W, H, 0.5, vr.MIP)
         g.set_sampler(vr.SAMPLER_MANUAL)
         assert np.array_equal(gpu_frame(g, view, proj, W, H, 0.5, vr.MIP), m_tex)
@@ -256,3 +256,57 @@ def test_released_store_renders_through_the_arrays_alone(vr):
     plain.upload(np.zeros((32, 32, 32), dtype=np.float32))
     with pytest.raises(vr.VrError):
         plain.release_store()
+
+
+def _mip_both_samplers(vr, g, view, proj, W, H, step, pix):
+    """MIP frame, sub-images at `pix` and sample count with the hand-rolled sampler and through the arrays."""
+    out = []
+    for s in (vr.SAMPLER_MANUAL, vr.SAMPLER_TEXTURE):
+        g.set_sampler(s)
+        img = gpu_frame(g, view, proj, W, H, step, vr.MIP)
+        out.append((img, g.debug_subimages(pix), g.debug_stats()["samples"]))
+    return out
+
+
+@pytest.mark.parametrize("case", ["noise", "checkerboard", "outlier", "constant", "offset", "blanked", "ghost0", "ghost2"])
+def test_mip_through_the_arrays_is_exact(vr, case):
+    """VR_MIP with the texture sampler: the filtered fetch only decides which samples CAN be the maximum (bound: range / 64
+    of the brick); those are evaluated by the hand-rolled float32 sampler. The frame, every brick's scalar sub-image and
+    the sample count must equal the hand-rolled path's bit for bit - also where the bound is tight (a checkerboard: cells
+    span the brick's range), useless (one huge voxel), zero (constant data), dominated by rounding (a small range on a
+    large offset) or not applicable (blanked bricks)."""
+    rng = np.random.default_rng(5)
+    cube = synth.Cube(19, 100, 90, 70, 10)
+    data = cube.fill_host()
+    ghost = {"ghost0": 0, "ghost2": 2}.get(case, 1)
+    if case == "checkerboard":
+        z, y, x = np.indices(data.shape)
+        data = (((x + y + z) & 1) * 2.0 - 1.0).astype(np.float32) * rng.uniform(0.5, 8.0, size=data.shape).astype(np.float32)
+    elif case == "outlier":
+        data[33, 41, 57] = 3.0e6
+    elif case == "constant":
+        data[:] = 2.5
+        data[:, :, 64:] = -1.0   # two constant halves: bricks with range 0 and bricks with a step
+    elif case == "offset":
+        data = (data * 1e-3 - 4000.0).astype(np.float32)  # range 0.02 at magnitude 4000: float32 rounding of the filters shows
+    elif case == "blanked":
+        data[10:30, 5:25, 20:50] = np.nan
+        data[3, 7, 60] = np.nan
+    g, o = make_pair(cube, 32, ghost, data=data)
+    W, H = 203, 117
+    fr = synth.Framing(cube.nx, cube.ny, cube.nz, W, H)
+    pix = seeded_pixels(9, W, H, 400)
+    g.set_counting(1)
+    for k, ortho, step in ((0, False, 0.5), (1, True, 0.5), (2, False, 1.0)):
+        view, proj = fr.seeded(31, k), fr.proj(ortho)
+        (m_img, m_sub, m_n), (t_img, t_sub, t_n) = _mip_both_samplers(vr, g, view, proj, W, H, step, pix)
+        assert np.array_equal(m_img, t_img, equal_nan=True), "%s view %d: frames differ by %g" % (case, k, np.nanmax(np.abs(m_img - t_img)))
+        # a ray may stop once its maximum saturates the colour map (vmax): beyond that the scalar is not unique
+        assert np.array_equal(np.minimum(m_sub, synth.TF_VMAX), np.minimum(t_sub, synth.TF_VMAX), equal_nan=True), \
+            "%s view %d: sub-images differ" % (case, k)
+        if np.nanmax(data) < synth.TF_VMAX:
+            assert m_n == t_n   # no ray stops early: the same samples
+        else:
+            assert t_n >= m_n   # a saturated ray is noticed when its queue is emptied, a few samples later
+        if k == 0 and case in ("noise", "checkerboard", "blanked"):
+            check_mip(t_img, o.render(view, proj, W, H, step, oracle.MIP), "%s through the arrays" % case)
