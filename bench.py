@@ -753,6 +753,10 @@ def run_probe_dram(vr, gib):
     return {"probe": "dram", "buffer_gib": gib, "hbm_peak_gbs": peak, "hbm_peak_source": peak_src, "cases": cases}
 
 
+def sampler_id(vr, name):
+    return {"manual": vr.SAMPLER_MANUAL, "texture": vr.SAMPLER_TEXTURE, "texture_half": vr.SAMPLER_TEXTURE_HALF, "texture_byte": vr.SAMPLER_TEXTURE_BYTE}[name]
+
+
 def run_probe_tex(vr):
     """The same question for the texture unit (profiles/r2_probe_dram.md, second part): random fetches through texture
     objects - tex1Dfetch over linear memory (4 and 16 bytes), tex3D point fetches of float4 texels and linear-filtered
@@ -790,7 +794,7 @@ def main():
                          "replica figure beside it as `replicas` - and the one-GPU line otherwise")
     ap.add_argument("--sortlast-parts", type=int, default=8,
                     help="row f3 report: parts of the k-d partition rendered one after the other on this GPU (0 = skip)")
-    ap.add_argument("--sampler", default="auto", choices=["auto", "manual", "texture"],
+    ap.add_argument("--sampler", default="auto", choices=["auto", "manual", "texture", "texture_half", "texture_byte"],
                     help="row a5: manual = hand-rolled float32 tri-linear from the tiled store; texture = the texture-object arm "
                          "(ALPHA frames; a second copy of the bricks as 3-D CUDA arrays). auto (default): 'whichever ncu shows is "
                          "faster' (north_star; DESIGN.md section 9) - the texture arm for ALPHA frames with a smooth table, on a "
@@ -891,18 +895,23 @@ def main():
     if args.sampler == "auto":
         args.sampler = "manual"
         fits = torch.cuda.mem_get_info()[0] > 1.15 * wl["nx"] * wl["ny"] * wl["nz"] * 4  # a second copy fits (c0 - c2, n1)
-        if args.mode == "mip" and args.traversal == "sort_last" and fits and not args.release_store:
-            args.sampler = "texture"  # exact MIP: the arrays rule samples out, the float32 store supplies the values
+        fits_byte = torch.cuda.mem_get_info()[0] > 0.3 * wl["nx"] * wl["ny"] * wl["nz"] * 4  # byte arrays fit (c3 too)
+        if args.mode == "mip" and args.traversal == "sort_last" and fits_byte and not args.release_store:
+            args.sampler = "texture_byte"  # exact MIP: byte arrays rule samples out, the float32 store supplies the values
         if args.mode == "alpha" and args.traversal == "sort_last" and args.tf in ("ramp", "translucent") and not args.release_store:
             if fits:
                 args.sampler = "texture"
             else:
                 promote = bool(getattr(g, "releasable", False)) and not args.no_variants and world == 1
     if args.release_store:
+        if args.sampler == "texture_half":
+            g.set_sampler(vr.SAMPLER_TEXTURE_HALF)  # the store is turned into float16 arrays
+        else:
+            args.sampler = "texture"
         g.release_store()
-        args.sampler, args.no_variants, args.cells_every = "texture", True, 0
-    elif args.sampler == "texture":
-        g.set_sampler(vr.SAMPLER_TEXTURE)
+        args.no_variants, args.cells_every = True, 0
+    elif args.sampler != "manual":
+        g.set_sampler(sampler_id(vr, args.sampler))
     W, H, K, Wm = wl["width"], wl["height"], args.steps, args.warmup
     out = torch.empty((H, W, 4), dtype=torch.float32, device="cuda")
     host_bufs = [torch.empty((H, W, 4), dtype=torch.float32).pin_memory() for _ in range(3)]
@@ -943,7 +952,9 @@ def main():
                     "synchronous_value": round(e2e_sync_fps, 3),
                     "synchronous_what": "vr_render_host: the caller waits for each frame's copy before queueing the next"},
             "clocks": m["clocks"],
-            "sampler": ("texture: 3-D CUDA arrays behind texture objects, a second copy beside the store" if args.sampler == "texture"
+            "sampler": ("texture_byte: 8-bit 3-D CUDA arrays as the exact MIP filter in front of the hand-rolled sampler" if args.sampler == "texture_byte"
+                        else "texture_half: float16 copies of the float32 voxels in 3-D CUDA arrays (sampling only; ALPHA inside 2e-3, MIP exact)" if args.sampler == "texture_half"
+                        else "texture: 3-D CUDA arrays behind texture objects, a second copy beside the store" if args.sampler == "texture"
                         else "manual: hand-rolled float32 tri-linear from the 4x4x2 micro-tiled store") +
                        (" (chosen by --sampler auto)" if args.sampler_asked == "auto" else ""),
             "stage_ms": {"setup": round(float(m["stages"][:, 0].mean()), 4), "raycast": round(float(m["stages"][:, 1].mean()), 4),
@@ -956,7 +967,7 @@ def main():
                          "max": round(float(m["stages"].sum(axis=1).max()), 4), "views": int(len(m["stages"]))},
             "roofline": roofline_of(m["counts"], m["stages"], m["stage_views"], peak, peak_src,
                                     traffic_of(args.workload, args.mode, args.tf + ("" if args.traversal == "sort_last" else "/fused") +
-                                               ("/texture" if args.sampler == "texture" else ""))),
+                                               ("/" + args.sampler if args.sampler != "manual" else ""))),
             "build_s": round(t_build, 1), "upload": dict(g.upload_stats, frac_of_hbm_peak=round(g.upload_stats["gb_per_s"] / peak, 4)),
             "minmax": dict(g.minmax_stats, frac_of_hbm_peak=round(g.minmax_stats["gb_per_s"] / peak, 4))}
     # which roofline bounds the ray-cast kernel: DRAM for the sparsely sampled 103 GB cube (0.03 samples per
@@ -989,15 +1000,28 @@ def main():
         # sort-last (the headline path) with the other transfer function / mode, then the fused traversal
         # (row f2: one ray through all bricks, global early termination, no sub-images, no compositing)
         other = "manual" if args.sampler == "texture" else "texture"  # the other arm of rows a1 / a5, on the same frames
-        for vmode, vtf, vtrav, vsamp in (("alpha", "translucent", "sort_last", args.sampler), ("mip", "ramp", "sort_last", args.sampler),
+        # MIP: 8-bit arrays as the exact filter (they fit beside the 103 GB cube too), and the hand-rolled sampler beside it
+        mip_s = "texture_byte" if args.sampler_asked == "auto" else args.sampler
+        for vmode, vtf, vtrav, vsamp in (("alpha", "translucent", "sort_last", args.sampler), ("mip", "ramp", "sort_last", mip_s),
+                                         ("mip", "ramp", "sort_last", "manual"),
+                                         # float16 copies of the voxels for sampling (half the fetched bytes; fits beside the 103 GB cube)
+                                         ("alpha", "ramp", "sort_last", "texture_half"), ("alpha", "translucent", "sort_last", "texture_half"),
                                          ("alpha", "ramp", "sort_last", other), ("alpha", "translucent", "sort_last", other),
                                          ("alpha", "ramp", "fused", args.sampler), ("alpha", "translucent", "fused", args.sampler),
                                          ("alpha", "threshold", "sort_last", args.sampler), ("alpha", "threshold", "fused", args.sampler),
                                          ("alpha", "ramp, early termination off", "sort_last", args.sampler)):
             if vtrav == "sort_last" and vmode == args.mode and vtf == args.tf and vsamp == args.sampler:
+                if vmode == "mip":
+                    continue  # the main arm itself
                 vtf = "ramp"
+            if vmode == "mip" and vsamp == "manual" and mip_s == "manual":
+                continue
+            if vsamp == "texture_half" and args.sampler == "texture_half":
+                continue  # the main arm and its first variant already
+            if vmode == "alpha" and vsamp == "texture_byte":
+                vsamp = "manual"  # byte arrays serve MIP only
             try:
-                g.set_sampler(vr.SAMPLER_TEXTURE if vsamp == "texture" else vr.SAMPLER_MANUAL)
+                g.set_sampler(sampler_id(vr, vsamp))
             except vr.VrError as e:  # the 103 GB cube: no room for a second copy of the bricks as 3-D arrays
                 variants.append({"mode": vmode, "tf": vtf, "traversal": vtrav, "sampler": vsamp, "unavailable": str(e)})
                 continue
@@ -1015,7 +1039,7 @@ def main():
             g.set_traversal(vr.SORT_LAST)
             g.set_early_termination(wl["tau"])
             variants.append({"mode": vmode, "tf": vtf, "traversal": vtrav, "sampler": ("manual" if (vtf == "threshold" and vsamp == "texture") else vsamp) +
-                                        (" (MIP: the arrays as an exact filter in front of the hand-rolled sampler)" if vmode != "alpha" and vsamp == "texture" else "") +
+                                        (" (MIP: the arrays as an exact filter in front of the hand-rolled sampler)" if vmode != "alpha" and vsamp != "manual" else "") +
                                         (" (a stepped table keeps the hand-rolled sampler)" if vtf == "threshold" and vsamp == "texture" else ""),
                              "frames_per_s": round(K / (v["ms"] * 1e-3), 3), **extra,
                              "gsamples_per_s": round(v["samples"] / (v["ms"] * 1e-3) / 1e9, 3),
@@ -1026,9 +1050,9 @@ def main():
                              "counts_": v["counts"],
                              "roofline": roofline_of(v["counts"], v["stages"], v["stage_views"], peak, peak_src,
                                                      traffic_of(args.workload, vmode, vtf + ("" if vtrav == "sort_last" else "/fused") +
-                                                                ("/texture" if vsamp == "texture" and vtf != "threshold" else "")))})
+                                                                ("/" + vsamp if vsamp != "manual" and vtf != "threshold" else "")))})
         g.set_transfer_function(tf, *tf_range(wl))
-        g.set_sampler(vr.SAMPLER_TEXTURE if args.sampler == "texture" else vr.SAMPLER_MANUAL)
+        g.set_sampler(sampler_id(vr, args.sampler))
         line["variants"] = variants
         # the workloads the paper's cubes look like (faint sources: PAPER.md:19, :206) beside the opaque ramp: the same
         # fraction (algorithmic bytes of the ray-cast kernel over its time, of the measured HBM peak) for every variant

@@ -283,9 +283,22 @@ int vr_set_traversal(vr_volume* v, int traversal);
  * the filter cannot apply R14's rule - and (ii) frames whose transfer function has a step: two neighbouring entries
  * further apart than 2.56/n in a channel (a threshold, a toe). The filter's value error is about one table entry on
  * unit-sigma noise; across a step that is a wrong opacity, not 2e-3 (measured: 8e-2 on a threshold table).
+ * VR_SAMPLER_TEXTURE_HALF: arrays of float16 texels (half the memory and half the fetched bytes), used ONLY as that
+ * exact VR_MIP filter: rounding a voxel to float16 (to nearest) moves it by at most 2^-11 of its magnitude, which the
+ * bound carries (range / 64 + 2^-9 of the brick's largest magnitude); bricks holding a magnitude above 60000 (float16
+ * ends at 65504) keep the hand-rolled loop. VR_MIP frames stay bit-identical to VR_SAMPLER_MANUAL's; VR_ALPHA frames
+ * use the hand-rolled sampler (float16 values would not keep 2e-3). This is the arm that fits beside the 103 GB cube
+ * (105 GB store + 53 GB arrays).
+ * VR_SAMPLER_TEXTURE_BYTE: the same filter with 8-bit texels, q = round(255 (v - min) / (max - min)) with the brick's own
+ * range (row f1's table, computed first): a quarter of the float32 arrays' memory and the fewest fetched bytes; the
+ * bound grows by half a byte step (range / 64 + range / 500 + 2^-12 of the largest magnitude). Frames bit-identical
+ * to VR_SAMPLER_MANUAL's as well.
+ * Switching to VR_SAMPLER_MANUAL, or between texel widths, frees the arrays (synchronises the device).
  * Needs the default (tiled) layout. */
 #define VR_SAMPLER_MANUAL 0
 #define VR_SAMPLER_TEXTURE 1
+#define VR_SAMPLER_TEXTURE_HALF 2
+#define VR_SAMPLER_TEXTURE_BYTE 3
 int vr_set_sampler(vr_volume* v, int sampler);
 
 /* The texture arm for cubes whose second copy does not fit beside the store (the 103 GB cube).

@@ -15,7 +15,7 @@ import numpy as np
 
 ALPHA, MIP = 0, 1
 SORT_LAST, FUSED = 0, 1
-SAMPLER_MANUAL, SAMPLER_TEXTURE = 0, 1
+SAMPLER_MANUAL, SAMPLER_TEXTURE, SAMPLER_TEXTURE_HALF, SAMPLER_TEXTURE_BYTE = 0, 1, 2, 3
 STEP_AUTO = 0.0  # vr_render step: the paper's per-ray step (R18)
 HOST, DEVICE = 0, 1
 LAYOUT_DEFAULT, LAYOUT_LINEAR, LAYOUT_TILED, LAYOUT_TILED_RELEASABLE = 0, 1, 2, 3

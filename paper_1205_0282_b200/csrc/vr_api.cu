@@ -841,19 +841,27 @@ extern "C" int vr_set_traversal(vr_volume* v, int traversal) {
 
 extern "C" int vr_set_sampler(vr_volume* v, int sampler) {
     if (!v) return fail(NULL, VR_ERR_INVALID_ARG, "vr_set_sampler: NULL handle");
-    if (sampler != VR_SAMPLER_MANUAL && sampler != VR_SAMPLER_TEXTURE)
+    if (sampler != VR_SAMPLER_MANUAL && sampler != VR_SAMPLER_TEXTURE && sampler != VR_SAMPLER_TEXTURE_HALF && sampler != VR_SAMPLER_TEXTURE_BYTE)
         return fail(v, VR_ERR_INVALID_ARG, "vr_set_sampler: unknown sampler %d", sampler);
-    if (v->store_released && sampler != VR_SAMPLER_TEXTURE)
-        return fail(v, VR_ERR_STATE, "vr_set_sampler: the float32 store was released, only the texture arm is left");
-    if (sampler == VR_SAMPLER_TEXTURE && !v->tex) {
+    if (v->store_released && sampler != v->sampler)
+        return fail(v, VR_ERR_STATE, "vr_set_sampler: the float32 store was released, only the arrays it was turned into are left");
+    const int texel = sampler == VR_SAMPLER_TEXTURE_HALF ? VR_TEXEL_HALF : sampler == VR_SAMPLER_TEXTURE_BYTE ? VR_TEXEL_BYTE : VR_TEXEL_FLOAT;
+    if (v->tex && !v->store_released && (sampler == VR_SAMPLER_MANUAL || vr_tex_texel(v->tex) != texel)) {
+        /* the arrays of the other texel width, or arrays nobody uses any more: their memory goes back */
+        VR_CUDA(v, cudaDeviceSynchronize());
+        vr_tex_destroy(v->tex);
+        v->tex = NULL;
+        v->tex_valid = false;
+    }
+    if (sampler != VR_SAMPLER_MANUAL && !v->tex) {
         const VrGrid& g = v->grid;
         if (!(g.layout == VR_LAYOUT_TILED && g.tl[0] == 2 && g.tl[1] == 2 && g.tl[2] == 1 && g.ml[0] == 0 && g.ml[1] == 0 && g.ml[2] == 0))
             return fail(v, VR_ERR_STATE, "vr_set_sampler: the texture arm is built beside the default (4x4x2 tiled) store only");
-        const cudaError_t e = vr_tex_create(g, &v->tex, true);
+        const cudaError_t e = vr_tex_create(g, &v->tex, true, texel);
         if (e != cudaSuccess)
             return fail(v, e == cudaErrorMemoryAllocation ? VR_ERR_OUT_OF_MEMORY : VR_ERR_CUDA,
                         "vr_set_sampler: 3-D arrays for %d bricks (%.2f GB beside the brick store): %s", g.nown,
-                        (double)g.slot * g.nown * 4.0 / 1e9, cudaGetErrorString(e));
+                        (double)g.slot * g.nown * (texel == VR_TEXEL_FLOAT ? 4.0 : texel == VR_TEXEL_HALF ? 2.0 : 1.0) / 1e9, cudaGetErrorString(e));
         v->tex_valid = false;
     }
     v->sampler = sampler;
@@ -863,7 +871,11 @@ extern "C" int vr_set_sampler(vr_volume* v, int sampler) {
 /* texture arm: bring the arrays up to date with the store (one launch, after an upload only) */
 static int ensure_tex(vr_volume* v, cudaStream_t st) {
     if (v->tex_valid) return VR_OK;
-    VR_CUDA(v, vr_launch_tex_fill(v->grid, v->bricks, v->tex, st));
+    if (vr_tex_texel(v->tex) == VR_TEXEL_BYTE) { /* byte texels are scaled with the bricks' ranges (row f1) */
+        const int rc = ensure_minmax(v, st);
+        if (rc) return rc;
+    }
+    VR_CUDA(v, vr_launch_tex_fill(v->grid, v->bricks, v->tex, v->d_mm, st));
     v->launches++;
     v->tex_valid = true;
     return VR_OK;
@@ -883,7 +895,8 @@ extern "C" int vr_volume_release_store(vr_volume* v, int64_t* freed_bytes_out, v
         vr_tex_destroy(v->tex);
         v->tex = NULL;
     }
-    cudaError_t e = vr_tex_create(v->grid, &v->tex, false);
+    const bool to_half = v->sampler == VR_SAMPLER_TEXTURE_HALF; /* the arrays take the texel width of the sampler in force */
+    cudaError_t e = vr_tex_create(v->grid, &v->tex, false, to_half ? VR_TEXEL_HALF : VR_TEXEL_FLOAT);
     if (e != cudaSuccess) return fail(v, e == cudaErrorMemoryAllocation ? VR_ERR_OUT_OF_MEMORY : VR_ERR_CUDA, "vr_volume_release_store: %s", cudaGetErrorString(e));
     long long freed = 0;
     for (int s = 0; s < v->grid.nown; ++s) {
@@ -902,7 +915,7 @@ extern "C" int vr_volume_release_store(vr_volume* v, int64_t* freed_bytes_out, v
     }
     v->store_released = true;
     v->tex_valid = true;
-    v->sampler = VR_SAMPLER_TEXTURE;
+    v->sampler = to_half ? VR_SAMPLER_TEXTURE_HALF : VR_SAMPLER_TEXTURE;
     if (freed_bytes_out) *freed_bytes_out = freed;
     return VR_OK;
 }
@@ -1081,8 +1094,8 @@ static int render_frame(vr_volume* v, const float* view, const float* proj, int 
     /* texture arm: ALPHA frames with a smooth table take their values from the arrays; MIP frames use the arrays as an exact
      * filter in front of the hand-rolled sampler (needs the float32 store and the bricks' ranges; where stepping over empty
      * macro-cells pays, that stays) */
-    const bool tex_alpha = v->sampler == VR_SAMPLER_TEXTURE && mode == VR_ALPHA && v->counting != 2 && v->tf_smooth;
-    const bool tex_mip = v->sampler == VR_SAMPLER_TEXTURE && mode == VR_MIP && v->counting != 2 && !v->store_released &&
+    const bool tex_alpha = (v->sampler == VR_SAMPLER_TEXTURE || v->sampler == VR_SAMPLER_TEXTURE_HALF) && mode == VR_ALPHA && v->counting != 2 && v->tf_smooth;
+    const bool tex_mip = v->sampler != VR_SAMPLER_MANUAL && mode == VR_MIP && v->counting != 2 && !v->store_released &&
                          v->traversal == VR_SORT_LAST && !mip_skipping;
     const bool use_tex = tex_alpha || tex_mip;
     if (use_tex) { /* after an upload only */
@@ -1120,6 +1133,11 @@ static int render_frame(vr_volume* v, const float* view, const float* proj, int 
     p.tex = use_tex ? vr_tex_table(v->tex) : NULL;
     p.tex_nan = use_tex ? vr_tex_nan_table(v->tex) : NULL;
     p.brick_mm = tex_mip ? v->d_mm : NULL;
+    const int texel = tex_mip ? vr_tex_texel(v->tex) : VR_TEXEL_FLOAT;
+    p.mip_range_eps = 1.0f / 64.0f + (texel == VR_TEXEL_BYTE ? 1.0f / 500.0f : 0.0f); /* half a byte step is range / 510 */
+    p.mip_mag_eps = texel == VR_TEXEL_HALF ? 1.0f / 512.0f : texel == VR_TEXEL_BYTE ? 1.0f / 4096.0f : 1.0f / 16384.0f;
+    p.mip_mag_max = texel == VR_TEXEL_HALF ? 60000.0f : INFINITY;
+    p.tex_byte = texel == VR_TEXEL_BYTE;
     p.cell_bits = skipping ? v->d_cell_bits : NULL;
     p.cell_mm = mip_skipping ? v->d_cell_mm : NULL;
     p.nc[0] = v->nc[0]; p.nc[1] = v->nc[1]; p.nc[2] = v->nc[2];

@@ -147,6 +147,10 @@ struct VrRaycastParams {
     const cudaTextureObject_t* tex; /* texture arm (vr_texture.cu): one texture object per slot, or NULL = hand-rolled sampling */
     const int* tex_nan;             /* 1 per slot that holds blanked voxels: sampled by hand also in the texture arm (R14) */
     const float2* brick_mm;         /* texture arm, MIP: (min, max) of every brick's padded cells (row f1), indexed by brick */
+    float mip_range_eps;            /* texture arm, MIP: the filter's error bound as a fraction of the brick's range (1/64; byte texels + 1/500) */
+    float mip_mag_eps;              /* ... and the part that scales with the magnitude (2^-14; float16 texels 2^-9; byte texels 2^-12) */
+    int tex_byte;                   /* byte texels: a fetch returns (v - min) / (max - min) of the brick */
+    float mip_mag_max;              /* bricks with a larger magnitude keep the hand-rolled loop (float16 texels: 60000; else inf) */
     unsigned* bitmap;   /* counting variant only: one bit per brick-store cell, or NULL */
     const unsigned* cell_bits; /* R19: one bit per 8x8x8 macro-cell, 1 = transparent under the LUT; NULL = no skipping */
     const float2* cell_mm; /* R19, MIP: (min, max) per macro-cell (a cell whose max cannot raise the ray's maximum is skipped); NULL = off */
@@ -189,7 +193,10 @@ cudaError_t vr_launch_setup(const VrGrid& grid, const VrMatrices& mats, int W, i
                             cudaStream_t st);
 /* texture arm of the brick store (vr_texture.cu): one 3-D CUDA array + texture object per slot */
 struct VrTexStore;
-cudaError_t vr_tex_create(const VrGrid& grid, VrTexStore** out, bool all);
+#define VR_TEXEL_FLOAT 0
+#define VR_TEXEL_HALF 1
+#define VR_TEXEL_BYTE 2
+cudaError_t vr_tex_create(const VrGrid& grid, VrTexStore** out, bool all, int texel);
 cudaError_t vr_tex_convert_slot(const VrGrid& grid, const float* bricks, VrTexStore* t, int s, int* has_nan, cudaStream_t st);
 /* a store that can be handed back slot by slot (vr_vmm.cu: CUDA virtual memory management) */
 struct VrVmm;
@@ -200,7 +207,8 @@ int vr_vmm_slot_released(const VrVmm* m, int s);
 void vr_tex_destroy(VrTexStore* t);
 const cudaTextureObject_t* vr_tex_table(const VrTexStore* t);
 const int* vr_tex_nan_table(const VrTexStore* t);
-cudaError_t vr_launch_tex_fill(const VrGrid& grid, const float* bricks, const VrTexStore* t, cudaStream_t st);
+int vr_tex_texel(const VrTexStore* t);
+cudaError_t vr_launch_tex_fill(const VrGrid& grid, const float* bricks, const VrTexStore* t, const float2* brick_mm, cudaStream_t st);
 /* ray table of the frame whose set-up is in vs (row a4, the per-ray part) */
 cudaError_t vr_launch_rays(const VrGrid& grid, const VrViewState* vs, int W, int H, double step, double2* rays, cudaStream_t st);
 cudaError_t vr_launch_minmax(const VrGrid& grid, const float* bricks, int2* enc, float2* table, cudaStream_t st);

@@ -37,9 +37,6 @@
 #ifndef VR_TEX_DEPTH
 #define VR_TEX_DEPTH 4 /* texture fetches a lane keeps in flight */
 #endif
-#ifndef VR_TEX_MIP_EPS
-#define VR_TEX_MIP_EPS (1.0f / 64.0f) /* bound of |filtered - exact| in units of the brick's data range (see the MIP loop) */
-#endif
 #ifndef VR_MIP_QUEUE
 #define VR_MIP_QUEUE 4 /* candidate samples a lane queues before the warp evaluates them by hand */
 #endif
@@ -159,12 +156,15 @@ vr_raycast_kernel(const VrRaycastParams prm) {
         const int n0 = n;
         bool use_tex = TEX && __ldg(prm.tex_nan + slot_b) == 0; /* warp-uniform: one brick per item */
         /* MIP through the arrays (below): eps bounds |filtered - exact| for every sample of this brick */
-        float mip_eps = 0.0f;
+        float mip_eps = 0.0f, dec_a = 1.0f, dec_b = 0.0f;
         if (TEX && MODE == VR_MIP && use_tex) {
             const float2 bmm = __ldg(prm.brick_mm + b);
             /* + the float32 rounding of either filter, which scales with the magnitude, not the range */
-            mip_eps = (bmm.y - bmm.x) * VR_TEX_MIP_EPS + fmaxf(fabsf(bmm.x), fabsf(bmm.y)) * (1.0f / 16384.0f);
-            use_tex = mip_eps >= 0.0f && mip_eps < INFINITY; /* a brick without finite voxels keeps the hand-rolled loop */
+            const float mag = fmaxf(fabsf(bmm.x), fabsf(bmm.y));
+            mip_eps = (bmm.y - bmm.x) * prm.mip_range_eps + mag * prm.mip_mag_eps;
+            if (prm.tex_byte) dec_a = bmm.y - bmm.x, dec_b = bmm.x; /* a byte fetch is (v - min) / (max - min) */
+            /* a brick without finite voxels, or with voxels float16 texels cannot hold, keeps the hand-rolled loop */
+            use_tex = mip_eps >= 0.0f && mip_eps < INFINITY && mag <= prm.mip_mag_max;
         }
         if (use_tex) {
             tex = __ldg(prm.tex + slot_b);
@@ -246,7 +246,8 @@ vr_raycast_kernel(const VrRaycastParams prm) {
         /* MIP through the arrays, EXACT (bit for bit the hand-rolled result): the filtered fetch serves as a bound, not as the
          * value. |filtered - exact| <= eps for every sample of the brick (the unit quantises the three weights to 8 fractional
          * bits: at most 3/256 of the largest difference between the 8 voxels, itself at most the brick's range; the float32 texel
-         * coordinate adds < 3e-4 of it; eps = range / 64 + 2^-14 of the largest magnitude for the filters' own rounding),
+         * coordinate adds < 3e-4 of it; eps = range / 64 + 2^-14 of the largest magnitude for the filters' own rounding - 2^-9 of it
+         * when the texels are float16 (VR_SAMPLER_TEXTURE_HALF: rounding to float16 is within 2^-11 of a value, the rest is margin)),
          * so with hmax = the largest filtered value so far the segment's exact maximum is >= hmax - eps, and a sample whose
          * filtered value is below hmax - 2 eps cannot be it: only the others (the CANDIDATES: a few per cent on noise, the
          * records of the running maximum and their near misses) are evaluated by hand, in float32 from the tiled store, at the
@@ -289,7 +290,7 @@ vr_raycast_kernel(const VrRaycastParams prm) {
 #pragma unroll
                     for (int u = 0; u < VR_TEX_DEPTH; ++u) {
                         if (j < n0) {
-                            const float v = vq[u];
+                            const float v = fmaf(vq[u], dec_a, dec_b); /* float32 / float16 texels: v * 1 + 0, exact */
                             if (COUNT) ++nsamples; /* a brick seen through its array has no blanked voxel */
                             if (v >= hmax - eps2 && v + mip_eps > acc.r) {
                                 if (qn < VR_MIP_QUEUE) {

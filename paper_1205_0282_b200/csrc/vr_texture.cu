@@ -17,6 +17,7 @@
  * the arrays only to rule out the samples that cannot be a ray's maximum, vr_raycast.cu), and which
  * VR_ALPHA keeps using for bricks that hold blanked (NaN) voxels: the filter cannot apply R14's rule.
  */
+#include <cuda_fp16.h>
 #include <string.h>
 
 #include <new>
@@ -32,6 +33,7 @@ struct VrTexStore {
     cudaSurfaceObject_t* d_surf;
     int3* d_ext;                /* padded extent of every slot */
     int* d_nan;                 /* 1 where the slot holds a NaN (blanked) voxel: such bricks are sampled by hand (R14) */
+    int texel;                  /* VR_TEXEL_FLOAT, or - the exact MIP filter only - VR_TEXEL_HALF / VR_TEXEL_BYTE */
 };
 
 void vr_tex_destroy(VrTexStore* t) {
@@ -53,19 +55,21 @@ void vr_tex_destroy(VrTexStore* t) {
 }
 
 /* brick held in slot s of the handle's store (the inverse of vr_slot_index) */
-static int brick_of_slot(const VrGrid& g, int s) {
+static __host__ __device__ int brick_of_slot(const VrGrid& g, int s) {
+    if (!g.part) return s;
     const int w = g.pb1[0] - g.pb0[0], h = g.pb1[1] - g.pb0[1];
     const int bx = g.pb0[0] + s % w, by = g.pb0[1] + (s / w) % h, bz = g.pb0[2] + s / (w * h);
     return (bz * g.g[1] + by) * g.g[0] + bx;
 }
 
 /* the store's host tables and device tables, no array yet */
-static cudaError_t tex_alloc(const VrGrid& g, VrTexStore** out) {
+static cudaError_t tex_alloc(const VrGrid& g, VrTexStore** out, int texel) {
     *out = NULL;
     VrTexStore* t = new (std::nothrow) VrTexStore();
     if (!t) return cudaErrorMemoryAllocation;
     memset(t, 0, sizeof(*t));
     t->n = g.nown;
+    t->texel = texel;
     t->arr = new (std::nothrow) cudaArray_t[g.nown]();
     t->tex = new (std::nothrow) cudaTextureObject_t[g.nown]();
     t->surf = new (std::nothrow) cudaSurfaceObject_t[g.nown]();
@@ -90,7 +94,8 @@ static cudaError_t tex_create_slot(VrTexStore* t, const VrGrid& g, int s) {
     vr_brick_coords(g, brick_of_slot(g, s), bc);
     vr_brick_core(g, bc, lo, hi);
     const int3 ext = make_int3(hi[0] - lo[0] + 2 * g.ghost, hi[1] - lo[1] + 2 * g.ghost, hi[2] - lo[2] + 2 * g.ghost);
-    const cudaChannelFormatDesc fmt = cudaCreateChannelDesc<float>();
+    const cudaChannelFormatDesc fmt = t->texel == VR_TEXEL_HALF ? cudaCreateChannelDescHalf()
+                                      : t->texel == VR_TEXEL_BYTE ? cudaCreateChannelDesc<unsigned char>() : cudaCreateChannelDesc<float>();
     cudaError_t e = cudaMalloc3DArray(&t->arr[s], &fmt, make_cudaExtent((size_t)ext.x, (size_t)ext.y, (size_t)ext.z), cudaArraySurfaceLoadStore);
     if (e != cudaSuccess) return e;
     cudaResourceDesc res;
@@ -101,7 +106,7 @@ static cudaError_t tex_create_slot(VrTexStore* t, const VrGrid& g, int s) {
     memset(&td, 0, sizeof(td));
     td.addressMode[0] = td.addressMode[1] = td.addressMode[2] = cudaAddressModeClamp;
     td.filterMode = cudaFilterModeLinear;
-    td.readMode = cudaReadModeElementType;
+    td.readMode = t->texel == VR_TEXEL_BYTE ? cudaReadModeNormalizedFloat : cudaReadModeElementType; /* byte q reads as q / 255 */
     td.normalizedCoords = 0;
     e = cudaCreateTextureObject(&t->tex[s], &res, &td, NULL);
     if (e == cudaSuccess) e = cudaCreateSurfaceObject(&t->surf[s], &res);
@@ -113,9 +118,9 @@ static cudaError_t tex_create_slot(VrTexStore* t, const VrGrid& g, int s) {
 
 /* all = true: every slot's array at once (the second copy beside the store); false: tables only, the arrays come slot by
  * slot (vr_tex_convert_slot: vr_volume_release_store) */
-cudaError_t vr_tex_create(const VrGrid& g, VrTexStore** out, bool all) {
+cudaError_t vr_tex_create(const VrGrid& g, VrTexStore** out, bool all, int texel) {
     VrTexStore* t = NULL;
-    cudaError_t e = tex_alloc(g, &t);
+    cudaError_t e = tex_alloc(g, &t, texel);
     for (int s = 0; all && s < g.nown && e == cudaSuccess; ++s) e = tex_create_slot(t, g, s);
     if (e != cudaSuccess) {
         cudaGetLastError();
@@ -129,15 +134,24 @@ cudaError_t vr_tex_create(const VrGrid& g, VrTexStore** out, bool all) {
 
 const cudaTextureObject_t* vr_tex_table(const VrTexStore* t) { return t ? t->d_tex : NULL; }
 const int* vr_tex_nan_table(const VrTexStore* t) { return t ? t->d_nan : NULL; }
+int vr_tex_texel(const VrTexStore* t) { return t ? t->texel : VR_TEXEL_FLOAT; }
 
 /* Padded cell (i, j, k) of slot s -> texel (i, j, k) of the slot's array. A CTA takes the 4 x 2 rows
  * (j, k) of one row of micro-tiles, one row per warp, lanes along x, so the eight warps together consume
  * whole 128-byte lines of the store (L1 serves a line's other rows to the neighbouring warps); the surface
  * write is coalesced. Once per upload. */
+template <int TEXEL>
 __global__ void __launch_bounds__(256)
 vr_tex_fill_kernel(VrGrid g, const float* __restrict__ bricks, const cudaSurfaceObject_t* __restrict__ surf,
-                   const int3* __restrict__ ext, int* __restrict__ has_nan, int slot0) {
+                   const int3* __restrict__ ext, int* __restrict__ has_nan, int slot0, const float2* __restrict__ brick_mm) {
     const int s = blockIdx.y + slot0;
+    /* byte texels: q = round(255 (v - min) / (max - min)) with the brick's range (row f1's table); a constant brick gets q = 0 */
+    float q_lo = 0.0f, q_scale = 0.0f;
+    if (TEXEL == VR_TEXEL_BYTE) {
+        const float2 mm = brick_mm[brick_of_slot(g, s)];
+        q_lo = mm.x;
+        q_scale = mm.y > mm.x ? 255.0f / (mm.y - mm.x) : 0.0f;
+    }
     const int3 e = ext[s];
     const cudaSurfaceObject_t su = surf[s];
     const float* __restrict__ src = bricks + (long long)s * g.slot;
@@ -151,7 +165,9 @@ vr_tex_fill_kernel(VrGrid g, const float* __restrict__ bricks, const cudaSurface
         for (int i = lane; i < e.x; i += 32) {
             const float v = __ldcs(src + row + vr_axis_offset(g.ax[0], i));
             nan_seen = nan_seen || v != v;
-            surf3Dwrite(v, su, i * 4, j, k);
+            if (TEXEL == VR_TEXEL_HALF) surf3Dwrite(__half_as_ushort(__float2half_rn(v)), su, i * 2, j, k); /* to nearest: |h - v| <= 2^-11 |v| + 2^-25 */
+            else if (TEXEL == VR_TEXEL_BYTE) surf3Dwrite((unsigned char)__float2uint_rn(fminf(fmaxf((v - q_lo) * q_scale, 0.0f), 255.0f)), su, i, j, k);
+            else surf3Dwrite(v, su, i * 4, j, k);
         }
     }
     /* R14: the hardware filter cannot apply the blanking rule (it drops a NaN corner whose 8-bit weight rounds to
@@ -159,25 +175,30 @@ vr_tex_fill_kernel(VrGrid g, const float* __restrict__ bricks, const cudaSurface
     if (__any_sync(0xffffffffu, nan_seen) && lane == 0) has_nan[s] = 1;
 }
 
-static cudaError_t launch_fill(const VrGrid& grid, const float* bricks, const VrTexStore* t, int slot0, int nslots, cudaStream_t st) {
+static cudaError_t launch_fill(const VrGrid& grid, const float* bricks, const VrTexStore* t, int slot0, int nslots, const float2* brick_mm,
+                               cudaStream_t st) {
     const int nj = (grid.P + 3) >> 2, nk = (grid.P + 1) >> 1;
     long long bx = (long long)nj * nk;
     if (bx > 4096) bx = 4096;
     cudaError_t e = cudaMemsetAsync(t->d_nan + slot0, 0, sizeof(int) * nslots, st);
     if (e != cudaSuccess) return e;
-    vr_tex_fill_kernel<<<dim3((unsigned)bx, (unsigned)nslots), 256, 0, st>>>(grid, bricks, t->d_surf, t->d_ext, t->d_nan, slot0);
+    const dim3 gr((unsigned)bx, (unsigned)nslots);
+    if (t->texel == VR_TEXEL_BYTE && !brick_mm) return cudaErrorInvalidValue;
+    if (t->texel == VR_TEXEL_HALF) vr_tex_fill_kernel<VR_TEXEL_HALF><<<gr, 256, 0, st>>>(grid, bricks, t->d_surf, t->d_ext, t->d_nan, slot0, brick_mm);
+    else if (t->texel == VR_TEXEL_BYTE) vr_tex_fill_kernel<VR_TEXEL_BYTE><<<gr, 256, 0, st>>>(grid, bricks, t->d_surf, t->d_ext, t->d_nan, slot0, brick_mm);
+    else vr_tex_fill_kernel<VR_TEXEL_FLOAT><<<gr, 256, 0, st>>>(grid, bricks, t->d_surf, t->d_ext, t->d_nan, slot0, brick_mm);
     return cudaGetLastError();
 }
 
-cudaError_t vr_launch_tex_fill(const VrGrid& grid, const float* bricks, const VrTexStore* t, cudaStream_t st) {
-    return launch_fill(grid, bricks, t, 0, t->n, st);
+cudaError_t vr_launch_tex_fill(const VrGrid& grid, const float* bricks, const VrTexStore* t, const float2* brick_mm, cudaStream_t st) {
+    return launch_fill(grid, bricks, t, 0, t->n, brick_mm, st);
 }
 
 /* vr_volume_release_store, one slot: create the slot's array, fill it from the store, wait, and say whether the slot holds
  * blanked voxels (then its float32 cells must stay: R14 needs them). */
 cudaError_t vr_tex_convert_slot(const VrGrid& grid, const float* bricks, VrTexStore* t, int s, int* has_nan, cudaStream_t st) {
     cudaError_t e = tex_create_slot(t, grid, s);
-    if (e == cudaSuccess) e = launch_fill(grid, bricks, t, s, 1, st);
+    if (e == cudaSuccess) e = launch_fill(grid, bricks, t, s, 1, NULL, st);
     if (e == cudaSuccess) e = cudaMemcpyAsync(has_nan, t->d_nan + s, sizeof(int), cudaMemcpyDeviceToHost, st);
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
     return e;

@@ -140,6 +140,23 @@ def _config3_checks(vr, wl, g, o, cube):
         box = np.empty((1, 1, 2 if x < 4095 else 1), dtype=np.float32)
         g.download(box, origin=(x, y, z))
         assert box[0, 0, 0] == np.float32(cube.voxel(x, y, z))
+    # narrow arrays BESIDE the 103 GB store (105 + 53 resp. 26 GB): float16 copies of the voxels for ALPHA sampling - same
+    # oracle, same 2e-3 -, and 8-bit arrays as the exact MIP filter: the whole frame bit-identical to the hand-rolled path's
+    W, H = wl["width"], wl["height"]
+    view, proj = wl["views"][14], wl["proj"]
+    mip_manual = gpu_frame(g, view, proj, W, H, wl["step"], vr.MIP)
+    g.set_sampler(vr.SAMPLER_TEXTURE_BYTE)
+    assert np.array_equal(gpu_frame(g, view, proj, W, H, wl["step"], vr.MIP), mip_manual)
+    check_views(vr, wl, g, o, (14,), 1000, (vr.MIP,), 0.99, tile=None)
+    g.set_sampler(vr.SAMPLER_TEXTURE_HALF)
+    assert np.array_equal(gpu_frame(g, view, proj, W, H, wl["step"], vr.MIP), mip_manual)
+    o.set_ert_margin(2e-4)
+    check_views(vr, wl, g, o, (30,), 1000, (vr.ALPHA,), 0.99, envelope=True, max_flagged=1.0)
+    for v in (g, o):
+        v.set_transfer_function(synth.tf_ramp(), synth.TF_VMIN, synth.TF_VMAX)
+    check_views(vr, wl, g, o, (9,), 1500, (vr.ALPHA,), 0.99, envelope=True, max_flagged=1.0)
+    g.set_sampler(vr.SAMPLER_MANUAL)
+    o.set_ert_margin(1e-5)
     # the texture arm on the 103 GB cube (bench.py's `texture_released`): the bricks become 3-D arrays one by one, their
     # float32 cells go back to the device, and the same frames are rendered through the arrays alone - same oracle, same
     # 2e-3, R12's band widened to the filter's error (R20)

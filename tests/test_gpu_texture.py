@@ -23,19 +23,23 @@ def vr(cuda_device):
     return vr
 
 
-def tex_pair(vr, cube, brick, ghost=1, tf=None, tau=0.99, data=None):
+TEXELS = ["float32", "float16"]  # the arrays ALPHA frames may take their values from
+
+
+def tex_pair(vr, cube, brick, ghost=1, tf=None, tau=0.99, data=None, texels="float32"):
     g, o = make_pair(cube, brick, ghost, tf=tf, tau=tau, data=data)
-    g.set_sampler(vr.SAMPLER_TEXTURE)
+    g.set_sampler(vr.SAMPLER_TEXTURE if texels == "float32" else vr.SAMPLER_TEXTURE_HALF)
     o.set_ert_margin(TEX_MARGIN)
     return g, o
 
 
+@pytest.mark.parametrize("texels", TEXELS)
 @pytest.mark.parametrize("tf_name", ["ramp", "translucent"])
-def test_config0_full_frames_texture(vr, tf_name):
+def test_config0_full_frames_texture(vr, tf_name, texels):
     c = synth.CONFIGS["c0"]
     cube = synth.config_cube("c0")
     tf = synth.tf_ramp() if tf_name == "ramp" else synth.tf_translucent()
-    g, o = tex_pair(vr, cube, c["brick"], c["ghost"], tf=tf)
+    g, o = tex_pair(vr, cube, c["brick"], c["ghost"], tf=tf, texels=texels)
     W, H = c["width"], c["height"]
     fr = synth.Framing(cube.nx, cube.ny, cube.nz, W, H)
     worst = 0.0
@@ -53,13 +57,14 @@ def test_config0_full_frames_texture(vr, tf_name):
     assert 1e-7 < np.abs(man - img).max() < 0.02  # two different samplers, the same picture
 
 
+@pytest.mark.parametrize("texels", TEXELS)
 @pytest.mark.parametrize("ghost,tau", [(1, 0.99), (1, 2.0), (2, 0.99), (0, 2.0)])
-def test_bricked_ragged_texture_frames_subimages_and_counts(vr, ghost, tau):
+def test_bricked_ragged_texture_frames_subimages_and_counts(vr, ghost, tau, texels):
     """Ragged multi-brick volume: frames, each brick's sub-image, and - with early termination off - exactly the
     hand-rolled path's sample count; ghost = 0 relies on the arrays' clamp addressing (seams as the oracle's)."""
     cube = synth.Cube(11, 100, 90, 70, 12)
     tf = synth.tf_translucent() if tau > 1 else synth.tf_ramp()
-    g, o = tex_pair(vr, cube, 32, ghost, tf=tf, tau=tau)
+    g, o = tex_pair(vr, cube, 32, ghost, tf=tf, tau=tau, texels=texels)
     W, H = 203, 117
     fr = synth.Framing(cube.nx, cube.ny, cube.nz, W, H)
     pix = seeded_pixels(4, W, H, 300)
@@ -79,7 +84,7 @@ def test_bricked_ragged_texture_frames_subimages_and_counts(vr, ghost, tau):
         m_tex = gpu_frame(g, view, proj, W, H, 0.5, vr.MIP)
         g.set_sampler(vr.SAMPLER_MANUAL)
         assert np.array_equal(gpu_frame(g, view, proj, W, H, 0.5, vr.MIP), m_tex)
-        g.set_sampler(vr.SAMPLER_TEXTURE)
+        g.set_sampler(vr.SAMPLER_TEXTURE if texels == "float32" else vr.SAMPLER_TEXTURE_HALF)
         check_mip(m_tex, o.render(view, proj, W, H, 0.5, oracle.MIP), "MIP beside the texture arm")
 
 
@@ -150,8 +155,9 @@ def test_texture_arm_keeps_stepped_tables_on_the_hand_rolled_path_and_errors(vr)
         g.set_sampler(7)
 
 
+@pytest.mark.parametrize("texels", TEXELS)
 @pytest.mark.parametrize("tau", [0.99, 2.0])
-def test_fused_traversal_through_the_texture_arm(vr, tau):
+def test_fused_traversal_through_the_texture_arm(vr, tau, texels):
     """Row f2 with the texture sampler: one ray through all bricks, per-lane texture objects (the rays of a warp may be
     in different bricks), against the oracle holding the cube in ONE brick (R17); early termination off: exactly the
     hand-rolled path's sample count. A brick with blanked voxels takes the hand-rolled loop inside the same kernel."""
@@ -159,7 +165,7 @@ def test_fused_traversal_through_the_texture_arm(vr, tau):
     cube = synth.Cube(51, 100, 90, 70, 12)
     data = cube.fill_host()
     tf = synth.tf_translucent() if tau > 1 else synth.tf_ramp()
-    g, _ = tex_pair(vr, cube, 32, 1, tf=tf, tau=tau, data=data)
+    g, _ = tex_pair(vr, cube, 32, 1, tf=tf, tau=tau, data=data, texels=texels)
     one = oracle.Volume(cube.nx, cube.ny, cube.nz, 128, 1, data=data)
     one.set_transfer_function(tf, synth.TF_VMIN, synth.TF_VMAX)
     one.set_early_termination(tau)
@@ -178,7 +184,7 @@ def test_fused_traversal_through_the_texture_arm(vr, tau):
             assert n_tex == int(ref["counts"][..., 0].sum())
         g.set_sampler(vr.SAMPLER_MANUAL)
         man = gpu_frame(g, view, proj, W, H, 0.5, vr.ALPHA)
-        g.set_sampler(vr.SAMPLER_TEXTURE)
+        g.set_sampler(vr.SAMPLER_TEXTURE if texels == "float32" else vr.SAMPLER_TEXTURE_HALF)
         assert 1e-7 < np.abs(man - img).max() < 0.02
     # blanked voxels in two bricks: those bricks are sampled by hand, the rest through the arrays, in one frame
     d2 = data.copy()
@@ -194,7 +200,8 @@ def test_fused_traversal_through_the_texture_arm(vr, tau):
     check_alpha(img, ref, tau, "fused texture, blanked box", envelope=True, max_flagged=1.0)
 
 
-def test_released_store_renders_through_the_arrays_alone(vr):
+@pytest.mark.parametrize("texels", TEXELS)
+def test_released_store_renders_through_the_arrays_alone(vr, texels):
     """VR_LAYOUT_TILED_RELEASABLE + vr_volume_release_store (the texture arm for cubes whose second copy does not fit):
     frames before the release (texture sampler, both stores present) and after it (float32 cells handed back) are
     bit-identical, match the oracle, the device gets the memory back, bricks with blanked voxels keep their float32
@@ -217,7 +224,7 @@ def test_released_store_renders_through_the_arrays_alone(vr):
     one.set_ert_margin(TEX_MARGIN)
     mip_before = gpu_frame(g, fr.seeded(3, 0), fr.proj(False), W, H, 0.5, vr.MIP)
     check_mip(mip_before, o.render(fr.seeded(3, 0), fr.proj(False), W, H, 0.5, oracle.MIP), "releasable handle, MIP before the release")
-    g.set_sampler(vr.SAMPLER_TEXTURE)
+    g.set_sampler(vr.SAMPLER_TEXTURE if texels == "float32" else vr.SAMPLER_TEXTURE_HALF)  # the released arrays take this width
     views = [(fr.seeded(3, k), fr.proj(k == 1)) for k in range(2)]
     before = [gpu_frame(g, v, p, W, H, 0.5, vr.ALPHA) for v, p in views]
     lo, hi = g.minmax()
@@ -258,18 +265,19 @@ def test_released_store_renders_through_the_arrays_alone(vr):
         plain.release_store()
 
 
-def _mip_both_samplers(vr, g, view, proj, W, H, step, pix):
+def _mip_both_samplers(vr, g, view, proj, W, H, step, pix, tex_sampler):
     """MIP frame, sub-images at `pix` and sample count with the hand-rolled sampler and through the arrays."""
     out = []
-    for s in (vr.SAMPLER_MANUAL, vr.SAMPLER_TEXTURE):
+    for s in (vr.SAMPLER_MANUAL, tex_sampler):
         g.set_sampler(s)
         img = gpu_frame(g, view, proj, W, H, step, vr.MIP)
         out.append((img, g.debug_subimages(pix), g.debug_stats()["samples"]))
     return out
 
 
-@pytest.mark.parametrize("case", ["noise", "checkerboard", "outlier", "constant", "offset", "blanked", "ghost0", "ghost2"])
-def test_mip_through_the_arrays_is_exact(vr, case):
+@pytest.mark.parametrize("texels", ["float32", "float16", "byte"])
+@pytest.mark.parametrize("case", ["noise", "checkerboard", "outlier", "constant", "offset", "tiny", "blanked", "ghost0", "ghost2"])
+def test_mip_through_the_arrays_is_exact(vr, case, texels):
     """VR_MIP with the texture sampler: the filtered fetch only decides which samples CAN be the maximum (bound: range / 64
     of the brick); those are evaluated by the hand-rolled float32 sampler. The frame, every brick's scalar sub-image and
     the sample count must equal the hand-rolled path's bit for bit - also where the bound is tight (a checkerboard: cells
@@ -289,9 +297,14 @@ def test_mip_through_the_arrays_is_exact(vr, case):
         data[:, :, 64:] = -1.0   # two constant halves: bricks with range 0 and bricks with a step
     elif case == "offset":
         data = (data * 1e-3 - 4000.0).astype(np.float32)  # range 0.02 at magnitude 4000: float32 rounding of the filters shows
+    elif case == "tiny":
+        data = (data * 1e-6).astype(np.float32)  # float16 subnormals (below 6e-5): texels keep 2^-25 absolute, not 2^-11 relative
     elif case == "blanked":
         data[10:30, 5:25, 20:50] = np.nan
         data[3, 7, 60] = np.nan
+    if case == "outlier" and texels == "float16":
+        data[60, 20, 10] = -7.0e4  # beyond float16: that brick keeps the hand-rolled loop
+    tex_sampler = {"float32": vr.SAMPLER_TEXTURE, "float16": vr.SAMPLER_TEXTURE_HALF, "byte": vr.SAMPLER_TEXTURE_BYTE}[texels]
     g, o = make_pair(cube, 32, ghost, data=data)
     W, H = 203, 117
     fr = synth.Framing(cube.nx, cube.ny, cube.nz, W, H)
@@ -299,7 +312,7 @@ def test_mip_through_the_arrays_is_exact(vr, case):
     g.set_counting(1)
     for k, ortho, step in ((0, False, 0.5), (1, True, 0.5), (2, False, 1.0)):
         view, proj = fr.seeded(31, k), fr.proj(ortho)
-        (m_img, m_sub, m_n), (t_img, t_sub, t_n) = _mip_both_samplers(vr, g, view, proj, W, H, step, pix)
+        (m_img, m_sub, m_n), (t_img, t_sub, t_n) = _mip_both_samplers(vr, g, view, proj, W, H, step, pix, tex_sampler)
         assert np.array_equal(m_img, t_img, equal_nan=True), "%s view %d: frames differ by %g" % (case, k, np.nanmax(np.abs(m_img - t_img)))
         # a ray may stop once its maximum saturates the colour map (vmax): beyond that the scalar is not unique
         assert np.array_equal(np.minimum(m_sub, synth.TF_VMAX), np.minimum(t_sub, synth.TF_VMAX), equal_nan=True), \
@@ -310,3 +323,32 @@ def test_mip_through_the_arrays_is_exact(vr, case):
             assert t_n >= m_n   # a saturated ray is noticed when its queue is emptied, a few samples later
         if k == 0 and case in ("noise", "checkerboard", "blanked"):
             check_mip(t_img, o.render(view, proj, W, H, step, oracle.MIP), "%s through the arrays" % case)
+
+
+def test_narrow_arrays_serve_mip_only_and_switching_replaces_them(vr):
+    """SAMPLER_TEXTURE_HALF / _BYTE: ALPHA frames keep the hand-rolled sampler bit for bit; switching samplers replaces the arrays."""
+    import torch
+    cube = synth.Cube(23, 96, 80, 64, 8)
+    g, o = make_pair(cube, 32, 1)
+    W, H = 160, 100
+    fr = synth.Framing(cube.nx, cube.ny, cube.nz, W, H)
+    view, proj = fr.seeded(5, 1), fr.proj(False)
+    a_man = gpu_frame(g, view, proj, W, H, 0.5, vr.ALPHA)
+    m_man = gpu_frame(g, view, proj, W, H, 0.5, vr.MIP)
+    for s in (vr.SAMPLER_TEXTURE_HALF, vr.SAMPLER_TEXTURE, vr.SAMPLER_TEXTURE_BYTE, vr.SAMPLER_TEXTURE_HALF, vr.SAMPLER_MANUAL,
+              vr.SAMPLER_TEXTURE_BYTE):
+        g.set_sampler(s)
+        assert np.array_equal(gpu_frame(g, view, proj, W, H, 0.5, vr.MIP), m_man)
+        a = gpu_frame(g, view, proj, W, H, 0.5, vr.ALPHA)
+        if s in (vr.SAMPLER_TEXTURE, vr.SAMPLER_TEXTURE_HALF):
+            assert 1e-7 < np.abs(a - a_man).max() < 0.02  # the arrays' filtered values
+        else:
+            assert np.array_equal(a, a_man)
+    # an upload is followed by the byte arrays too (their scale is the NEW range of each brick)
+    d2 = cube.fill_host()
+    d2[20:40, 30:50, 40:60] += 6.0
+    g.upload(torch.from_numpy(d2).cuda())
+    m_tex = gpu_frame(g, view, proj, W, H, 0.5, vr.MIP)
+    g.set_sampler(vr.SAMPLER_MANUAL)
+    m2 = gpu_frame(g, view, proj, W, H, 0.5, vr.MIP)
+    assert np.array_equal(m_tex, m2) and np.abs(m2 - m_man).max() > 1e-2
