@@ -283,16 +283,20 @@ int vr_set_traversal(vr_volume* v, int traversal);
  * the filter cannot apply R14's rule - and (ii) frames whose transfer function has a step: two neighbouring entries
  * further apart than 2.56/n in a channel (a threshold, a toe). The filter's value error is about one table entry on
  * unit-sigma noise; across a step that is a wrong opacity, not 2e-3 (measured: 8e-2 on a threshold table).
- * VR_SAMPLER_TEXTURE_HALF: arrays of float16 texels (half the memory and half the fetched bytes), used ONLY as that
- * exact VR_MIP filter: rounding a voxel to float16 (to nearest) moves it by at most 2^-11 of its magnitude, which the
- * bound carries (range / 64 + 2^-9 of the brick's largest magnitude); bricks holding a magnitude above 60000 (float16
- * ends at 65504) keep the hand-rolled loop. VR_MIP frames stay bit-identical to VR_SAMPLER_MANUAL's; VR_ALPHA frames
- * use the hand-rolled sampler (float16 values would not keep 2e-3). This is the arm that fits beside the 103 GB cube
- * (105 GB store + 53 GB arrays).
+ * VR_SAMPLER_TEXTURE_HALF: the same arm with arrays of float16 texels - float16 COPIES of the float32 voxels, made for
+ * sampling only (the store, the range tables, blanked bricks and every other path stay float32): half the memory and
+ * about three quarters of the fetched bytes. Rounding a voxel to float16 (to nearest) moves it by at most 2^-11 of its
+ * magnitude - for data of a few sigma a quarter of what the filter's 8-bit weights already move a sample (2^-9 of the
+ * local voxel differences) - so VR_ALPHA frames stay inside 2e-3 (measured against the oracle: the same error as with
+ * float32 texels to two digits, R22); use float32 texels for data whose magnitude is large against the
+ * transfer function's range. For VR_MIP the arrays are the exact filter described above, the bound carrying the
+ * rounding (range / 64 + 2^-9 of the brick's largest magnitude); bricks holding a magnitude above 60000 (float16
+ * ends at 65504) keep the hand-rolled loop: VR_MIP frames stay bit-identical to VR_SAMPLER_MANUAL's. These arrays fit
+ * beside the 103 GB cube (105 GB store + 53 GB).
  * VR_SAMPLER_TEXTURE_BYTE: the same filter with 8-bit texels, q = round(255 (v - min) / (max - min)) with the brick's own
  * range (row f1's table, computed first): a quarter of the float32 arrays' memory and the fewest fetched bytes; the
- * bound grows by half a byte step (range / 64 + range / 500 + 2^-12 of the largest magnitude). Frames bit-identical
- * to VR_SAMPLER_MANUAL's as well.
+ * bound grows by half a byte step (range / 64 + range / 500 + 2^-12 of the largest magnitude). VR_MIP frames
+ * bit-identical to VR_SAMPLER_MANUAL's as well; VR_ALPHA frames use the hand-rolled sampler (8 bits would not keep 2e-3).
  * Switching to VR_SAMPLER_MANUAL, or between texel widths, frees the arrays (synchronises the device).
  * Needs the default (tiled) layout. */
 #define VR_SAMPLER_MANUAL 0
@@ -305,7 +309,8 @@ int vr_set_sampler(vr_volume* v, int sampler);
  * On a handle created with VR_LAYOUT_TILED_RELEASABLE and filled: computes the range tables (rows f1, R19) if they are
  * stale, then, brick by brick, creates the brick's 3-D array, fills it from the float32 store and gives the brick's
  * float32 cells back to the device (peak memory: the store plus one array). Bricks that hold blanked (NaN) voxels keep
- * their float32 cells, because R14 needs them. Afterwards the handle renders VR_ALPHA frames (both traversals) through the
+ * their float32 cells, because R14 needs them. The arrays take the texel width of the sampler in force (float16 after
+ * vr_set_sampler(v, VR_SAMPLER_TEXTURE_HALF), else float32). Afterwards the handle renders VR_ALPHA frames (both traversals) through the
  * texture arm only: vr_volume_upload / download, VR_MIP frames, counting mode 2 and transfer functions with a step
  * return VR_ERR_STATE. Irreversible; synchronises. freed_bytes_out (host, may be NULL): device memory given back.
  * Errors: VR_ERR_STATE (not a releasable handle, nothing uploaded, already released), VR_ERR_OUT_OF_MEMORY, VR_ERR_CUDA. */

@@ -266,8 +266,9 @@ class Volume:
         self._check(lib().vr_set_traversal(self._h, int(traversal)))
 
     def set_sampler(self, sampler):
-        """SAMPLER_MANUAL (hand-rolled float32 tri-linear, the default) or SAMPLER_TEXTURE (3-D CUDA arrays behind
-        texture objects for ALPHA frames; allocates a second copy of the bricks)."""
+        """SAMPLER_MANUAL (hand-rolled float32 tri-linear, the default), SAMPLER_TEXTURE (3-D CUDA arrays behind texture
+        objects: a second copy of the bricks; ALPHA values, exact MIP filter), SAMPLER_TEXTURE_HALF (float16 copies: the
+        same at half the memory) or SAMPLER_TEXTURE_BYTE (8-bit arrays: the exact MIP filter only)."""
         self._check(lib().vr_set_sampler(self._h, int(sampler)))
 
     def release_store(self, stream=None):
