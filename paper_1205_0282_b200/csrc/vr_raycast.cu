@@ -37,6 +37,9 @@
 #ifndef VR_TEX_DEPTH
 #define VR_TEX_DEPTH 4 /* texture fetches a lane keeps in flight */
 #endif
+#ifndef VR_MIP_TEX_DEPTH
+#define VR_MIP_TEX_DEPTH 4 /* fetches a lane keeps in flight in the MIP filter loop */
+#endif
 #ifndef VR_MIP_QUEUE
 #define VR_MIP_QUEUE 4 /* candidate samples a lane queues before the warp evaluates them by hand */
 #endif
@@ -281,14 +284,14 @@ vr_raycast_kernel(const VrRaycastParams prm) {
                 }
                 if (active) {
                     const float kf = (float)j;
-                    float vq[VR_TEX_DEPTH];
+                    float vq[VR_MIP_TEX_DEPTH];
 #pragma unroll
-                    for (int u = 0; u < VR_TEX_DEPTH; ++u) {
+                    for (int u = 0; u < VR_MIP_TEX_DEPTH; ++u) {
                         const float ku = kf + (float)u;
                         vq[u] = tex3D<float>(tex, fmaf(ku, Dfx, P0x), fmaf(ku, Dfy, P0y), fmaf(ku, Dfz, P0z));
                     }
 #pragma unroll
-                    for (int u = 0; u < VR_TEX_DEPTH; ++u) {
+                    for (int u = 0; u < VR_MIP_TEX_DEPTH; ++u) {
                         if (j < n0) {
                             const float v = fmaf(vq[u], dec_a, dec_b); /* float32 / float16 texels: v * 1 + 0, exact */
                             if (COUNT) ++nsamples; /* a brick seen through its array has no blanked voxel */
