@@ -481,7 +481,7 @@ static cudaError_t launch_mode(const VrRaycastParams& p, long long ctas, bool sp
         }
     }
     if (is_tile442(p.grid) && p.tex != NULL && MODE == VR_ALPHA && p.bitmap == NULL) {
-        /* texture arm (vr_set_sampler): VR_ALPHA only; the touched-cells bitmap is the hand-rolled path's */
+        /* texture arm (vr_set_sampler), VR_ALPHA values; the touched-cells bitmap is the hand-rolled path's */
         if (!clamp && p.cell_bits != NULL) return launch_variant<VR_ALPHA, LAY_TILE442, 0, false, COUNT, true, true>(p, ctas, sparse, st);
         return clamp ? launch_variant<VR_ALPHA, LAY_TILE442, 0, true, COUNT, false, true>(p, ctas, sparse, st)
                      : launch_variant<VR_ALPHA, LAY_TILE442, 0, false, COUNT, false, true>(p, ctas, sparse, st);
