@@ -1054,6 +1054,28 @@ def main():
         g.set_transfer_function(tf, *tf_range(wl))
         g.set_sampler(sampler_id(vr, args.sampler))
         line["variants"] = variants
+
+        def brief(v):
+            r = v.get("roofline") or {}
+            return {"frames_per_s": v.get("frames_per_s"), "gsamples_per_s": v.get("gsamples_per_s"), "raycast_ms": (v.get("stage_ms") or {}).get("raycast"),
+                    "frac": r.get("frac"), "traffic": r.get("traffic"),
+                    "traffic_over_algorithmic": round(r["traffic"] / r["algorithmic_bytes_per_launch"], 2) if r.get("traffic") and r.get("algorithmic_bytes_per_launch") else None}
+        # the narrow copies in one place (they are variants above): NOT the headline, which keeps float32 texels
+        nt = {}
+        for v in variants:
+            if v.get("frames_per_s") is None or v["traversal"] != "sort_last":
+                continue
+            if v["mode"] == "alpha" and v["sampler"].startswith("texture_half") and v["tf"] in ("ramp", "translucent"):
+                nt["alpha_%s_float16_texels" % v["tf"]] = brief(v)
+            if v["mode"] == "mip" and v["sampler"].startswith("texture_byte"):
+                nt["mip_8bit_exact_filter"] = brief(v)
+            if v["mode"] == "mip" and v["sampler"].startswith("manual"):
+                nt["mip_hand_rolled"] = brief(v)
+        if nt:
+            nt["what"] = ("float16 copies of the float32 voxels for ALPHA sampling (inside north_star's 2e-3 with the float32 arrays' error to two "
+                          "digits: DESIGN.md R22; tests/test_gpu_texture.py, tests/test_gpu_fullsize.py) and 8-bit arrays as an exact MIP filter "
+                          "(frames bit-identical to the hand-rolled path: R23); the headline `value` uses float32 texels")
+            line["narrow_texels"] = nt
         # the workloads the paper's cubes look like (faint sources: PAPER.md:19, :206) beside the opaque ramp: the same
         # fraction (algorithmic bytes of the ray-cast kernel over its time, of the measured HBM peak) for every variant
         line["roofline_variants"] = [{"mode": args.mode, "tf": args.tf, "traversal": args.traversal, "sampler": args.sampler,
