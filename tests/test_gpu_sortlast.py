@@ -238,3 +238,37 @@ def test_bench_brick_sharded_arm_as_a_world_of_one(vr):
     assert line["n_gpus"] == 1 and line["scaling"] == "strong" and line["value"] > 0 and line["e2e"]["value"] > 0
     assert line["gpu_launches"] == 6 * 5            # set-up, ray table, ray cast, stage-1 compositing, merge
     assert line["exchange_bytes_per_frame"] == 0    # a world of one sends nothing
+
+
+@pytest.mark.parametrize("sampler", ["texture", "texture_half", "texture_byte"])
+def test_parts_through_the_texture_arrays(vr, sampler):
+    """Part handles with the texture arm (arrays of the part's own bricks only; 8-bit texels scaled with the ranges of the
+    bricks the part holds): merged MIP frames bit-identical to the hand-rolled single handle's, merged ALPHA frames inside
+    the tolerance (float32 / float16 values) or untouched (8-bit arrays serve MIP only)."""
+    from paper_1205_0282_b200 import sortlast
+    dims, brick, ghost, W, H = (70, 52, 64), 16, 1, 150, 110
+    data = synth.Cube(21, *dims, 5).fill_host()
+    boxes, tree, parts = make_parts(vr, sortlast, data, dims, brick, ghost, 3)
+    whole = vr.Volume(*dims, brick, ghost)
+    whole.upload(data)
+    o = oracle.Volume(*dims, brick, ghost, data=data)
+    o.set_ert_margin(2e-4)
+    sid = {"texture": vr.SAMPLER_TEXTURE, "texture_half": vr.SAMPLER_TEXTURE_HALF, "texture_byte": vr.SAMPLER_TEXTURE_BYTE}[sampler]
+    for v in parts + [whole, o]:
+        v.set_transfer_function(synth.tf_ramp(), synth.TF_VMIN, synth.TF_VMAX)
+        v.set_early_termination(0.99)
+    for p in parts:
+        p.set_sampler(sid)
+    fr = synth.Framing(*dims, W, H)
+    for k in range(3):
+        view, proj = fr.seeded(31, k), fr.proj(k % 2 == 1)
+        gotm = merged_frame(vr, sortlast, parts, boxes, tree, dims, brick, view, proj, W, H, 0.6, vr.MIP)
+        assert np.array_equal(gotm, gpu_frame(whole, view, proj, W, H, 0.6, vr.MIP)), (sampler, k)
+        got = merged_frame(vr, sortlast, parts, boxes, tree, dims, brick, view, proj, W, H, 0.6, vr.ALPHA)
+        one = gpu_frame(whole, view, proj, W, H, 0.6, vr.ALPHA)
+        if sampler == "texture_byte":
+            assert np.abs(got - one).max() < 2e-6
+        else:
+            assert 1e-7 < np.abs(got - one).max() < 0.02
+            check_alpha(got, o.render(view, proj, W, H, 0.6, oracle.ALPHA), 0.99, "parts, %s, view %d" % (sampler, k), envelope=True,
+                        max_flagged=1.0)
