@@ -286,8 +286,8 @@ int vr_set_traversal(vr_volume* v, int traversal);
  * VR_SAMPLER_TEXTURE_HALF: the same arm with arrays of float16 texels - float16 COPIES of the float32 voxels, made for
  * sampling only (the store, the range tables, blanked bricks and every other path stay float32): half the memory and
  * about three quarters of the fetched bytes. Rounding a voxel to float16 (to nearest) moves it by at most 2^-11 of its
- * magnitude - for data of a few sigma a quarter of what the filter's 8-bit weights already move a sample (2^-9 of the
- * local voxel differences) - so VR_ALPHA frames stay inside 2e-3 (measured against the oracle: the same error as with
+ * magnitude and the unit filters such texels at float16 precision (2^-10 in all) - for data of a few sigma half of what
+ * the filter's 8-bit weights already move a sample (2^-9 of the local voxel differences) - so VR_ALPHA frames stay inside 2e-3 (measured against the oracle: the same error as with
  * float32 texels to two digits, R22); use float32 texels for data whose magnitude is large against the
  * transfer function's range. For VR_MIP the arrays are the exact filter described above, the bound carrying the
  * rounding (range / 64 + 2^-9 of the brick's largest magnitude); bricks holding a magnitude above 60000 (float16
@@ -468,6 +468,13 @@ int vr_debug_cell_flags(vr_volume* v, int b, unsigned char* flags_out, int* dims
 
 /* mm_out (host): nbricks * 2 floats, (min, max) per brick over its ghost-padded cells. */
 int vr_debug_brick_minmax(vr_volume* v, float* mm_out);
+
+/* R23's constant, measured (test / measurement export): with a texture sampler in force, the largest
+ * |filtered fetch - exact tri-linear value| over n hashed sample positions inside brick b (the exact value in double
+ * from the float32 store; 8-bit fetches decoded with the brick's range), and the brick's range (max - min, row f1).
+ * The exact MIP filter relies on max_err <= range / 64 (+ the magnitude terms of vr_set_sampler's text).
+ * max_err_out, range_out: host. Synchronises. Errors: VR_ERR_STATE (manual sampler, released store, no data). */
+int vr_debug_tex_error(vr_volume* v, int b, int64_t n, unsigned seed, float* max_err_out, float* range_out);
 
 int vr_debug_subimages(vr_volume* v, const int* pixels, int npix, float* sub_out);
 

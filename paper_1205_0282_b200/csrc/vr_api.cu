@@ -949,6 +949,32 @@ extern "C" int vr_debug_cell_flags(vr_volume* v, int b, unsigned char* flags_out
     return VR_OK;
 }
 
+/* R23: measured error of the texture arm's filtered fetch in brick b (test / measurement export) */
+extern "C" int vr_debug_tex_error(vr_volume* v, int b, int64_t n, unsigned seed, float* max_err_out, float* range_out) {
+    if (!v) return fail(NULL, VR_ERR_INVALID_ARG, "vr_debug_tex_error: NULL handle");
+    if (!max_err_out || !range_out || n < 1 || b < 0 || b >= v->grid.nbricks) return fail(v, VR_ERR_INVALID_ARG, "vr_debug_tex_error: bad argument");
+    const int slot_b = vr_slot_index(v->grid, b);
+    if (slot_b < 0) return fail(v, VR_ERR_INVALID_ARG, "vr_debug_tex_error: this part does not hold brick %d", b);
+    if (!v->has_data || v->store_released || v->sampler == VR_SAMPLER_MANUAL || !v->tex)
+        return fail(v, VR_ERR_STATE, "vr_debug_tex_error: needs data, a texture sampler and the float32 store");
+    int rc = ensure_minmax(v, 0);
+    if (!rc) rc = ensure_tex(v, 0);
+    if (rc) return rc;
+    float2 mm;
+    VR_CUDA(v, cudaMemcpy(&mm, v->d_mm + b, sizeof(mm), cudaMemcpyDeviceToHost));
+    const bool byte = vr_tex_texel(v->tex) == VR_TEXEL_BYTE;
+    float* d_err = NULL;
+    VR_CUDA(v, cudaMalloc(&d_err, sizeof(float)));
+    cudaError_t e = cudaMemset(d_err, 0, sizeof(float));
+    if (e == cudaSuccess) e = vr_launch_tex_error(v->grid, v->bricks, v->tex, slot_b, n, seed, byte ? mm.y - mm.x : 1.0f, byte ? mm.x : 0.0f, d_err, 0);
+    if (e == cudaSuccess) e = cudaMemcpy(max_err_out, d_err, sizeof(float), cudaMemcpyDeviceToHost);
+    cudaFree(d_err);
+    VR_CUDA(v, e);
+    v->launches++;
+    *range_out = mm.y - mm.x;
+    return VR_OK;
+}
+
 extern "C" int vr_debug_brick_minmax(vr_volume* v, float* mm_out) {
     if (!v) return fail(NULL, VR_ERR_INVALID_ARG, "vr_debug_brick_minmax: NULL handle");
     if (!mm_out) return fail(v, VR_ERR_INVALID_ARG, "vr_debug_brick_minmax: NULL output");

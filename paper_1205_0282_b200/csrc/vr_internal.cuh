@@ -208,6 +208,8 @@ void vr_tex_destroy(VrTexStore* t);
 const cudaTextureObject_t* vr_tex_table(const VrTexStore* t);
 const int* vr_tex_nan_table(const VrTexStore* t);
 int vr_tex_texel(const VrTexStore* t);
+cudaError_t vr_launch_tex_error(const VrGrid& grid, const float* bricks, const VrTexStore* t, int s, long long n, unsigned seed, float dec_a,
+                                float dec_b, float* max_err, cudaStream_t st);
 cudaError_t vr_launch_tex_fill(const VrGrid& grid, const float* bricks, const VrTexStore* t, const float2* brick_mm, cudaStream_t st);
 /* ray table of the frame whose set-up is in vs (row a4, the per-ray part) */
 cudaError_t vr_launch_rays(const VrGrid& grid, const VrViewState* vs, int W, int H, double step, double2* rays, cudaStream_t st);

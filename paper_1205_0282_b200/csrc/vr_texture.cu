@@ -203,3 +203,54 @@ cudaError_t vr_tex_convert_slot(const VrGrid& grid, const float* bricks, VrTexSt
     if (e == cudaSuccess) e = cudaStreamSynchronize(st);
     return e;
 }
+
+/* R23's constant, measured: the largest |filtered fetch - exact tri-linear value| over n hashed positions inside slot s,
+ * the exact value in double from the float32 store. Positions are texel coordinates in [1/2, extent - 1/2): inside the
+ * volume of texel centres, as every sample of a frame is. dec_a / dec_b decode an 8-bit fetch ((max - min), min; else 1, 0). */
+__global__ void __launch_bounds__(256)
+vr_tex_error_kernel(VrGrid g, const float* __restrict__ bricks, const cudaTextureObject_t* __restrict__ tex, const int3* __restrict__ ext,
+                    int s, long long n, unsigned seed, float dec_a, float dec_b, float* __restrict__ max_err) {
+    const int3 e = ext[s];
+    const cudaTextureObject_t t = tex[s];
+    const float* __restrict__ src = bricks + (long long)s * g.slot;
+    float worst = 0.0f;
+    for (long long q = (long long)blockIdx.x * blockDim.x + threadIdx.x; q < n; q += (long long)gridDim.x * blockDim.x) {
+        unsigned long long h = ((unsigned long long)seed << 40) ^ (unsigned long long)q;
+        float p[3];
+        const int ee[3] = {e.x, e.y, e.z};
+        for (int a = 0; a < 3; ++a) {
+            h ^= h >> 33; h *= 0xff51afd7ed558ccdull; h ^= h >> 33; h *= 0xc4ceb9fe1a85ec53ull; h ^= h >> 33;
+            p[a] = 0.5f + (float)((double)(h >> 11) * (1.0 / 9007199254740992.0) * (double)(ee[a] - 1));
+            if (p[a] >= (float)ee[a] - 0.5f) p[a] = (float)ee[a] - 0.5f - 1e-3f;
+        }
+        const float f = fmaf(tex3D<float>(t, p[0], p[1], p[2]), dec_a, dec_b);
+        int c[3];
+        double w[3];
+        for (int a = 0; a < 3; ++a) {
+            const double u = (double)p[a] - 0.5;
+            c[a] = (int)floor(u);
+            if (c[a] > ee[a] - 2) c[a] = ee[a] - 2;
+            w[a] = u - (double)c[a];
+        }
+        double v[2][2][2];
+        for (int k = 0; k < 2; ++k)
+            for (int j = 0; j < 2; ++j)
+                for (int i = 0; i < 2; ++i)
+                    v[k][j][i] = (double)src[vr_axis_offset(g.ax[0], c[0] + i) + vr_axis_offset(g.ax[1], c[1] + j) + vr_axis_offset(g.ax[2], c[2] + k)];
+        double x[2][2];
+        for (int k = 0; k < 2; ++k)
+            for (int j = 0; j < 2; ++j) x[k][j] = v[k][j][0] + w[0] * (v[k][j][1] - v[k][j][0]);
+        const double y0 = x[0][0] + w[1] * (x[0][1] - x[0][0]), y1 = x[1][0] + w[1] * (x[1][1] - x[1][0]);
+        const double exact = y0 + w[2] * (y1 - y0);
+        const float err = (float)fabs((double)f - exact);
+        if (err == err) worst = fmaxf(worst, err);
+    }
+    for (int o = 16; o > 0; o >>= 1) worst = fmaxf(worst, __shfl_xor_sync(0xffffffffu, worst, o));
+    if ((threadIdx.x & 31) == 0) atomicMax(reinterpret_cast<int*>(max_err), __float_as_int(worst)); /* non-negative floats order as ints */
+}
+
+cudaError_t vr_launch_tex_error(const VrGrid& grid, const float* bricks, const VrTexStore* t, int s, long long n, unsigned seed, float dec_a,
+                                float dec_b, float* max_err, cudaStream_t st) {
+    vr_tex_error_kernel<<<148 * 4, 256, 0, st>>>(grid, bricks, t->d_tex, t->d_ext, s, n, seed, dec_a, dec_b, max_err);
+    return cudaGetLastError();
+}

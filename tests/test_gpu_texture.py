@@ -352,3 +352,31 @@ def test_narrow_arrays_serve_mip_only_and_switching_replaces_them(vr):
     g.set_sampler(vr.SAMPLER_MANUAL)
     m2 = gpu_frame(g, view, proj, W, H, 0.5, vr.MIP)
     assert np.array_equal(m_tex, m2) and np.abs(m2 - m_man).max() > 1e-2
+
+
+@pytest.mark.parametrize("texels", ["float32", "float16", "byte"])
+def test_filter_error_stays_inside_the_bound_the_mip_filter_relies_on(vr, texels):
+    """R23's constant, measured where it is largest: a +-1 checkerboard (every cell spans the brick's whole range along
+    every axis), noise, and noise on a large offset. The filtered fetch must stay within range / 64 (+ range / 500 for
+    8-bit texels) + the magnitude term of the exact value, with room to spare."""
+    sid = {"float32": vr.SAMPLER_TEXTURE, "float16": vr.SAMPLER_TEXTURE_HALF, "byte": vr.SAMPLER_TEXTURE_BYTE}[texels]
+    range_eps = 1.0 / 64 + (1.0 / 500 if texels == "byte" else 0.0)
+    mag_eps = {"float32": 2.0 ** -14, "float16": 2.0 ** -9, "byte": 2.0 ** -12}[texels]
+    cube = synth.Cube(7, 96, 96, 96, 6)
+    noise = cube.fill_host()
+    z, y, x = np.indices(noise.shape)
+    cases = {"checkerboard": (((x + y + z) & 1) * 2.0 - 1.0).astype(np.float32), "noise": noise,
+             "offset noise": (noise + 300.0).astype(np.float32)}
+    for name, data in cases.items():
+        g = vr.Volume(96, 96, 96, 32, 1)
+        g.upload(data)
+        g.set_sampler(sid)
+        worst = 0.0
+        for b in (0, 13, 26):
+            err, rng = g.debug_tex_error(b, 1 << 21, seed=b + 1)
+            mag = float(np.abs(data).max())
+            bound = rng * range_eps + mag * mag_eps
+            assert rng > 0 and err <= 0.85 * bound, (name, texels, b, err, rng, bound)
+            worst = max(worst, err / rng)
+        print("filter error / range, %s texels, %s: %.5f (bound %.5f)" % (texels, name, worst, range_eps))
+        g.close()
