@@ -701,6 +701,12 @@ def test_randomised_configurations(vr, case):
         refm = orc.render(view, proj, W, H, step, oracle.MIP)
         got = gpu_frame(g, view, proj, W, H, step if step > 0 else vr.STEP_AUTO, vr.MIP)
         check_mip(got, refm, "case %d" % case)
+    # R23: MIP through the texture arrays of any texel width is the hand-rolled frame, bit for bit
+    g.set_traversal(vr.SORT_LAST)
+    want = gpu_frame(g, view, proj, W, H, step if step > 0 else vr.STEP_AUTO, vr.MIP)
+    for s in (vr.SAMPLER_TEXTURE, vr.SAMPLER_TEXTURE_HALF, vr.SAMPLER_TEXTURE_BYTE):
+        g.set_sampler(s)
+        assert np.array_equal(gpu_frame(g, view, proj, W, H, step if step > 0 else vr.STEP_AUTO, vr.MIP), want), (case, s)
 
 
 # --------------------------------------------------------------------------- state across calls
