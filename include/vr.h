@@ -290,7 +290,7 @@ int vr_set_traversal(vr_volume* v, int traversal);
  * the filter's 8-bit weights already move a sample (2^-9 of the local voxel differences) - so VR_ALPHA frames stay inside 2e-3 (measured against the oracle: the same error as with
  * float32 texels to two digits, R22); use float32 texels for data whose magnitude is large against the
  * transfer function's range. For VR_MIP the arrays are the exact filter described above, the bound carrying the
- * rounding (range / 64 + 2^-9 of the brick's largest magnitude); bricks holding a magnitude above 60000 (float16
+ * rounding (range / 64 + 2^-9 of the brick's largest magnitude + 2^-23 for float16's subnormal grid); bricks holding a magnitude above 60000 (float16
  * ends at 65504) keep the hand-rolled loop: VR_MIP frames stay bit-identical to VR_SAMPLER_MANUAL's. These arrays fit
  * beside the 103 GB cube (105 GB store + 53 GB).
  * VR_SAMPLER_TEXTURE_BYTE: the same filter with 8-bit texels, q = round(255 (v - min) / (max - min)) with the brick's own

@@ -1163,6 +1163,7 @@ static int render_frame(vr_volume* v, const float* view, const float* proj, int 
     p.mip_range_eps = 1.0f / 64.0f + (texel == VR_TEXEL_BYTE ? 1.0f / 500.0f : 0.0f); /* half a byte step is range / 510 */
     p.mip_mag_eps = texel == VR_TEXEL_HALF ? 1.0f / 512.0f : texel == VR_TEXEL_BYTE ? 1.0f / 4096.0f : 1.0f / 16384.0f;
     p.mip_mag_max = texel == VR_TEXEL_HALF ? 60000.0f : INFINITY;
+    p.mip_abs_eps = texel == VR_TEXEL_HALF ? 1.1920929e-7f /* 2^-23: four half-steps of float16's subnormal grid */ : 2.4e-38f;
     p.tex_byte = texel == VR_TEXEL_BYTE;
     p.cell_bits = skipping ? v->d_cell_bits : NULL;
     p.cell_mm = mip_skipping ? v->d_cell_mm : NULL;

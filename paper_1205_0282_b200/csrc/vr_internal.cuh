@@ -149,6 +149,7 @@ struct VrRaycastParams {
     const float2* brick_mm;         /* texture arm, MIP: (min, max) of every brick's padded cells (row f1), indexed by brick */
     float mip_range_eps;            /* texture arm, MIP: the filter's error bound as a fraction of the brick's range (1/64; byte texels + 1/500) */
     float mip_mag_eps;              /* ... and the part that scales with the magnitude (2^-14; float16 texels 2^-9; byte texels 2^-12) */
+    float mip_abs_eps;              /* ... and the absolute part: float16 texels are 2^-24 apart below 2^-14 (subnormals), rounded twice */
     int tex_byte;                   /* byte texels: a fetch returns (v - min) / (max - min) of the brick */
     float mip_mag_max;              /* bricks with a larger magnitude keep the hand-rolled loop (float16 texels: 60000; else inf) */
     unsigned* bitmap;   /* counting variant only: one bit per brick-store cell, or NULL */

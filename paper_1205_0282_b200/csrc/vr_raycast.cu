@@ -164,7 +164,7 @@ vr_raycast_kernel(const VrRaycastParams prm) {
             const float2 bmm = __ldg(prm.brick_mm + b);
             /* + the float32 rounding of either filter, which scales with the magnitude, not the range */
             const float mag = fmaxf(fabsf(bmm.x), fabsf(bmm.y));
-            mip_eps = (bmm.y - bmm.x) * prm.mip_range_eps + mag * prm.mip_mag_eps;
+            mip_eps = (bmm.y - bmm.x) * prm.mip_range_eps + mag * prm.mip_mag_eps + prm.mip_abs_eps;
             if (prm.tex_byte) dec_a = bmm.y - bmm.x, dec_b = bmm.x; /* a byte fetch is (v - min) / (max - min) */
             /* a brick without finite voxels, or with voxels float16 texels cannot hold, keeps the hand-rolled loop */
             use_tex = mip_eps >= 0.0f && mip_eps < INFINITY && mag <= prm.mip_mag_max;

@@ -654,7 +654,7 @@ def test_nan_voxels_are_blanked(vr):
 
 
 # --------------------------------------------------------------------------- randomised configurations
-@pytest.mark.parametrize("case", range(int(__import__("os").environ.get("VR_RANDOM_CASES", "16"))))
+@pytest.mark.parametrize("case", range(int(__import__("os").environ.get("VR_RANDOM_CASES", "64"))))
 def test_randomised_configurations(vr, case):
     """Seeded random volumes, bricks, ghosts, steps (incl. the per-ray step), cameras (incl. eyes
     inside the volume), transfer functions, data kinds and blanked voxels, both modes and both

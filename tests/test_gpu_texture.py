@@ -276,7 +276,7 @@ def _mip_both_samplers(vr, g, view, proj, W, H, step, pix, tex_sampler):
 
 
 @pytest.mark.parametrize("texels", ["float32", "float16", "byte"])
-@pytest.mark.parametrize("case", ["noise", "checkerboard", "outlier", "constant", "offset", "tiny", "blanked", "ghost0", "ghost2"])
+@pytest.mark.parametrize("case", ["noise", "checkerboard", "outlier", "constant", "offset", "tiny", "tinier", "blanked", "ghost0", "ghost2"])
 def test_mip_through_the_arrays_is_exact(vr, case, texels):
     """VR_MIP with the texture sampler: the filtered fetch only decides which samples CAN be the maximum (bound: range / 64
     of the brick); those are evaluated by the hand-rolled float32 sampler. The frame, every brick's scalar sub-image and
@@ -299,6 +299,8 @@ def test_mip_through_the_arrays_is_exact(vr, case, texels):
         data = (data * 1e-3 - 4000.0).astype(np.float32)  # range 0.02 at magnitude 4000: float32 rounding of the filters shows
     elif case == "tiny":
         data = (data * 1e-6).astype(np.float32)  # float16 subnormals (below 6e-5): texels keep 2^-25 absolute, not 2^-11 relative
+    elif case == "tinier":
+        data = (np.abs(data) * 2e-8).astype(np.float32)  # a brick's whole range inside ONE step (6e-8) of float16's subnormal grid
     elif case == "blanked":
         data[10:30, 5:25, 20:50] = np.nan
         data[3, 7, 60] = np.nan
