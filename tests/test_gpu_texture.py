@@ -382,3 +382,32 @@ def test_filter_error_stays_inside_the_bound_the_mip_filter_relies_on(vr, texels
             worst = max(worst, err / rng)
         print("filter error / range, %s texels, %s: %.5f (bound %.5f)" % (texels, name, worst, range_eps))
         g.close()
+
+
+@pytest.mark.parametrize("case", range(int(__import__("os").environ.get("VR_SCALE_CASES", "24"))))
+def test_mip_exactness_over_scales_and_offsets(vr, case):
+    """R23 across magnitudes: the same noise cube scaled by 10^-12 .. 10^6 and shifted by up to 10^4 ranges (float16
+    subnormals and overflow, 8-bit steps far above the data's own spread, float32 rounding of the decode): MIP frames
+    through every texel width equal the hand-rolled frame."""
+    rng = np.random.default_rng(4000 + case)
+    dims = tuple(int(v) for v in rng.integers(24, 60, 3))
+    base = synth.Cube(900 + case, *dims, 3).fill_host()
+    scale = 10.0 ** rng.uniform(-12, 6)
+    offset = scale * float(rng.choice([0.0, 0.0, 1.0, -30.0, 1e3, -1e4]))
+    data = (base * scale + offset).astype(np.float32)
+    if rng.random() < 0.3:
+        data[tuple(int(v) for v in rng.integers(0, 20, 3))] = np.float32(scale * 1e4)  # one voxel far outside
+    brick = int(rng.choice([8, 16, 32]))
+    g = vr.Volume(*dims, brick, int(rng.choice([0, 1, 2])))
+    g.upload(data)
+    lo, hi = float(np.min(data)), float(np.max(data))
+    g.set_transfer_function(synth.tf_ramp(), lo, hi if hi > lo else lo + 1.0)
+    W, H = 96, 80
+    fr = synth.Framing(*dims, W, H)
+    view, proj = fr.seeded(50 + case, case), fr.proj(bool(case & 1))
+    step = float(rng.choice([0.5, 1.0, 0.37]))
+    want = gpu_frame(g, view, proj, W, H, step, vr.MIP)
+    for s in (vr.SAMPLER_TEXTURE, vr.SAMPLER_TEXTURE_HALF, vr.SAMPLER_TEXTURE_BYTE):
+        g.set_sampler(s)
+        got = gpu_frame(g, view, proj, W, H, step, vr.MIP)
+        assert np.array_equal(got, want), (case, s, scale, offset, float(np.abs(got - want).max()))
