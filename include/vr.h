@@ -288,8 +288,9 @@ int vr_set_traversal(vr_volume* v, int traversal);
  * about three quarters of the fetched bytes. Rounding a voxel to float16 (to nearest) moves it by at most 2^-11 of its
  * magnitude and the unit filters such texels at float16 precision (2^-10 in all) - for data of a few sigma half of what
  * the filter's 8-bit weights already move a sample (2^-9 of the local voxel differences) - so VR_ALPHA frames stay inside 2e-3 (measured against the oracle: the same error as with
- * float32 texels to two digits, R22); use float32 texels for data whose magnitude is large against the
- * transfer function's range. For VR_MIP the arrays are the exact filter described above, the bound carrying the
+ * float32 texels to two digits, R22). Guard: while the largest magnitude in the volume / 1024 exceeds 1.5e-3 of
+ * the transfer function's range, VR_ALPHA frames use the hand-rolled sampler instead (VR_ERR_STATE on a released store):
+ * float32 texels are for such data. For VR_MIP the arrays are the exact filter described above, the bound carrying the
  * rounding (range / 64 + 2^-9 of the brick's largest magnitude + 2^-23 for float16's subnormal grid); bricks holding a magnitude above 60000 (float16
  * ends at 65504) keep the hand-rolled loop: VR_MIP frames stay bit-identical to VR_SAMPLER_MANUAL's. These arrays fit
  * beside the 103 GB cube (105 GB store + 53 GB).

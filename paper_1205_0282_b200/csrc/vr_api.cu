@@ -60,6 +60,7 @@ struct vr_volume {
     int nc[3], cell_words;   /* macro-cells per axis of a slot; words of d_cell_bits per brick */
     bool cell_mm_valid, cell_bits_valid;
     bool mip_skip_known, mip_skip_useful; /* decided once per upload: does the cube have empty space (R19, MIP) */
+    bool half_alpha_known, half_alpha_ok;  /* decided per upload and transfer function: may ALPHA values come from float16 texels (R22) */
     unsigned long long* d_cell_count;
     bool tf_smooth;          /* no neighbouring LUT entries further apart than 2.56/n per channel (texture arm) */
     bool tf_has_zero;        /* the LUT has a run of >= 3 zero-alpha entries: skipping can do something */
@@ -459,6 +460,7 @@ extern "C" int vr_volume_upload(vr_volume* v, const float* src, int memspace, in
     v->mm_valid = false;
     v->cell_mm_valid = v->cell_bits_valid = false;
     v->mip_skip_known = false;
+    v->half_alpha_known = false;
     return VR_OK;
 }
 
@@ -577,6 +579,7 @@ extern "C" int vr_set_transfer_function(vr_volume* v, const float* rgba, int n, 
      * sample (about one table entry on noise of unit sigma over a 13-sigma, 256-entry table); 2e-3 per channel survives that
      * only if neighbouring entries are close. Tables with steps (thresholds, toes) keep the hand-rolled sampler. */
     v->tf_smooth = true;
+    v->half_alpha_known = false;
     for (int i = 0; i + 1 < n; ++i)
         for (int c = 0; c < 4; ++c)
             if (fabsf(rgba[4 * i + 4 + c] - rgba[4 * i + c]) > 2.56f / (float)n) v->tf_smooth = false;
@@ -767,6 +770,22 @@ static int decide_mip_skip(vr_volume* v, cudaStream_t st) {
     VR_CUDA(v, cudaStreamSynchronize(st));
     v->mip_skip_useful = empty * 8ull >= (unsigned long long)ncells;
     v->mip_skip_known = true;
+    return VR_OK;
+}
+
+/* R22: float16 texels move a value by up to 2^-10 of its magnitude (rounding + the unit's float16 filter). ALPHA frames
+ * take their values from such arrays only while that stays below 1.5e-3 of the transfer function's range for the
+ * largest magnitude in the volume (about a third of an entry of a 256-entry table); decided once per upload / table. */
+static int decide_half_alpha(vr_volume* v, cudaStream_t st) {
+    if (v->half_alpha_known) return VR_OK;
+    const int rc = ensure_minmax(v, st);
+    if (rc) return rc;
+    float2 mm;
+    VR_CUDA(v, cudaMemcpyAsync(&mm, v->d_mm + v->grid.nbricks, sizeof(mm), cudaMemcpyDeviceToHost, st));
+    VR_CUDA(v, cudaStreamSynchronize(st));
+    const float mag = fmaxf(fabsf(mm.x), fabsf(mm.y));
+    v->half_alpha_ok = mag * (1.0f / 1024.0f) <= 1.5e-3f * (v->lut.vmax - v->lut.vmin); /* false for NaN / inf too */
+    v->half_alpha_known = true;
     return VR_OK;
 }
 
@@ -1120,7 +1139,17 @@ static int render_frame(vr_volume* v, const float* view, const float* proj, int 
     /* texture arm: ALPHA frames with a smooth table take their values from the arrays; MIP frames use the arrays as an exact
      * filter in front of the hand-rolled sampler (needs the float32 store and the bricks' ranges; where stepping over empty
      * macro-cells pays, that stays) */
-    const bool tex_alpha = (v->sampler == VR_SAMPLER_TEXTURE || v->sampler == VR_SAMPLER_TEXTURE_HALF) && mode == VR_ALPHA && v->counting != 2 && v->tf_smooth;
+    bool tex_alpha = (v->sampler == VR_SAMPLER_TEXTURE || v->sampler == VR_SAMPLER_TEXTURE_HALF) && mode == VR_ALPHA && v->counting != 2 && v->tf_smooth;
+    if (tex_alpha && v->sampler == VR_SAMPLER_TEXTURE_HALF) { /* R22: only while float16 is fine enough for this data under this table */
+        rc = decide_half_alpha(v, st);
+        if (rc) return rc;
+        if (!v->half_alpha_ok) {
+            if (v->store_released)
+                return fail(v, VR_ERR_STATE, "vr_render: float16 texels are too coarse for this data under this transfer function (largest "
+                                             "magnitude / 1024 > 1.5e-3 of the table's range) and the float32 store was released");
+            tex_alpha = false; /* the hand-rolled sampler */
+        }
+    }
     const bool tex_mip = v->sampler != VR_SAMPLER_MANUAL && mode == VR_MIP && v->counting != 2 && !v->store_released &&
                          v->traversal == VR_SORT_LAST && !mip_skipping;
     const bool use_tex = tex_alpha || tex_mip;

@@ -346,6 +346,19 @@ def test_narrow_arrays_serve_mip_only_and_switching_replaces_them(vr):
             assert 1e-7 < np.abs(a - a_man).max() < 0.02  # the arrays' filtered values
         else:
             assert np.array_equal(a, a_man)
+    # R22's guard: data whose magnitude is large against the table's range is too coarse in float16 - ALPHA frames then
+    # come from the hand-rolled sampler (bit for bit) although the float16 arrays are in force; MIP stays exact either way
+    far = vr.Volume(cube.nx, cube.ny, cube.nz, 32, 1)
+    shifted = (cube.fill_host() + 300.0).astype(np.float32)
+    far.upload(shifted)
+    far.set_transfer_function(synth.tf_ramp(), synth.TF_VMIN + 300.0, synth.TF_VMAX + 300.0)
+    a_far, m_far = gpu_frame(far, view, proj, W, H, 0.5, vr.ALPHA), gpu_frame(far, view, proj, W, H, 0.5, vr.MIP)
+    far.set_sampler(vr.SAMPLER_TEXTURE_HALF)
+    assert np.array_equal(gpu_frame(far, view, proj, W, H, 0.5, vr.ALPHA), a_far)
+    assert np.array_equal(gpu_frame(far, view, proj, W, H, 0.5, vr.MIP), m_far)
+    far.set_sampler(vr.SAMPLER_TEXTURE)
+    assert 1e-7 < np.abs(gpu_frame(far, view, proj, W, H, 0.5, vr.ALPHA) - a_far).max() < 0.02  # float32 texels do serve it
+    far.close()
     # an upload is followed by the byte arrays too (their scale is the NEW range of each brick)
     d2 = cube.fill_host()
     d2[20:40, 30:50, 40:60] += 6.0
