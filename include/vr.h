@@ -268,7 +268,7 @@ int vr_set_traversal(vr_volume* v, int traversal);
  * texture read from a 3-D CUDA array per brick (float32 texels, linear filter, clamp addressing, unnormalised
  * coordinates = R3's voxel-centre convention). The arrays are a SECOND copy of the handle's bricks, allocated
  * by this call (VR_ERR_OUT_OF_MEMORY if they do not fit beside the store - the 103 GB cube - and the sampler
- * stays as it was) and refilled from the store on the device by the first frame after an upload. The sample
+ * is then VR_SAMPLER_MANUAL: arrays of another texel width were freed to make room) and refilled from the store on the device by the first frame after an upload. The sample
  * SET is unchanged (same FP64 set-up); the hardware's 8-bit interpolation weights perturb sample values by up
  * to 2^-9 of the local voxel differences, which keeps VR_ALPHA inside its 2e-3 tolerance but moves early-
  * termination decisions of rays whose opacity passes tau within ~1e-4 of it.

@@ -877,6 +877,7 @@ extern "C" int vr_set_sampler(vr_volume* v, int sampler) {
         if (!(g.layout == VR_LAYOUT_TILED && g.tl[0] == 2 && g.tl[1] == 2 && g.tl[2] == 1 && g.ml[0] == 0 && g.ml[1] == 0 && g.ml[2] == 0))
             return fail(v, VR_ERR_STATE, "vr_set_sampler: the texture arm is built beside the default (4x4x2 tiled) store only");
         const cudaError_t e = vr_tex_create(g, &v->tex, true, texel);
+        if (e != cudaSuccess) v->sampler = VR_SAMPLER_MANUAL; /* no arrays (any of another width were freed above): hand-rolled */
         if (e != cudaSuccess)
             return fail(v, e == cudaErrorMemoryAllocation ? VR_ERR_OUT_OF_MEMORY : VR_ERR_CUDA,
                         "vr_set_sampler: 3-D arrays for %d bricks (%.2f GB beside the brick store): %s", g.nown,

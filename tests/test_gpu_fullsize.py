@@ -155,7 +155,12 @@ def _config3_checks(vr, wl, g, o, cube):
     for v in (g, o):
         v.set_transfer_function(synth.tf_ramp(), synth.TF_VMIN, synth.TF_VMAX)
     check_views(vr, wl, g, o, (9,), 1500, (vr.ALPHA,), 0.99, envelope=True, max_flagged=1.0)
+    with pytest.raises(vr.VrError) as oom:
+        g.set_sampler(vr.SAMPLER_TEXTURE)   # 104 GB of float32 arrays do not fit beside the store ...
+    assert oom.value.status == 2
+    a_fallback = gpu_frame(g, wl["views"][9], proj, W, H, wl["step"], vr.ALPHA)   # ... and the handle is back on the hand-rolled sampler
     g.set_sampler(vr.SAMPLER_MANUAL)
+    assert np.array_equal(gpu_frame(g, wl["views"][9], proj, W, H, wl["step"], vr.ALPHA), a_fallback)
     o.set_ert_margin(1e-5)
     # the texture arm on the 103 GB cube (bench.py's `texture_released`): the bricks become 3-D arrays one by one, their
     # float32 cells go back to the device, and the same frames are rendered through the arrays alone - same oracle, same
