@@ -169,7 +169,7 @@ def build_volume(vr, wl, tf):
         pad *= n + 2 * wl["ghost"] * nb
     up_bytes = 4 * (wl["nx"] * wl["ny"] * wl["nz"] + pad)
     up_ms = sum(a.elapsed_time(b) for a, b in evs)
-    g.upload_stats = {"kernel": "vr_upload_tile442_kernel", "launches": len(evs), "ms": round(up_ms, 3), "bytes": up_bytes,
+    g.upload_stats = {"kernel": "vr_upload_tma442_kernel (TMA box loads; vr_upload_tile442_kernel where the source is not 16-byte aligned)", "launches": len(evs), "ms": round(up_ms, 3), "bytes": up_bytes,
                       "gb_per_s": round(up_bytes / (up_ms * 1e-3) / 1e9, 1)}
     # every per-view buffer and table the frames below need, taken now: vr_render then never allocates or synchronises
     g.reserve_views(wl["views"], [wl["proj"]] * len(wl["views"]), wl["width"], wl["height"])

@@ -519,10 +519,10 @@ int vr_debug_probe_dram(const void* buf, uint64_t bytes, int flavour, int span_b
                         int loads_per_thread, int ctas, int l2_fetch_granularity, float* ms_out,
                         uint64_t* loads_out, void* stream);
 
-/* Which kernel vr_volume_upload uses for the default (4x4x2) layout, process-wide: 0 (default) = cp.async staging,
- * 1 = source boxes loaded by the TMA unit (cp.async.bulk.tensor; needs sx % 4 == 0 and a 16-byte aligned source, else
- * falls back to 0). Both give the same store, bit for bit; the switch exists to measure one against the other
- * (round 2, c3: 5.23 TB/s against 4.95 TB/s, so the TMA kernel is not the default). */
+/* Which kernel vr_volume_upload uses for the default (4x4x2) layout, process-wide: 1 (default) = source boxes loaded by the
+ * TMA unit (cp.async.bulk.tensor; needs sx % 4 == 0 and a 16-byte aligned source, else falls back to 0), 0 = cp.async
+ * staging. Both give the same store, bit for bit; the switch exists to measure one against the other
+ * (round 2, c3: 5.58 TB/s against 5.23 TB/s). */
 int vr_debug_set_upload_path(int path);
 
 /* Number of kernel launches the library has issued on this handle since creation. */

@@ -261,9 +261,10 @@ vr_download_kernel(VrGrid g, const float* __restrict__ bricks, float* __restrict
 
 static cudaError_t launch_upload_tma(const VrGrid& grid, float* bricks, const float* src, int x0, int y0, int z0, int sx, int sy, int sz,
                                      int b0, unsigned nby, cudaStream_t st);
-/* 0 = cp.async staging (vr_upload_tile442_kernel, the default: 5.23 TB/s on c3), 1 = TMA box loads (vr_upload_tma442_kernel:
- * 4.95 TB/s on c3, 4.30 against 4.83 TB/s on c2 - measured round 2, profiles/r2_upload.md); vr_debug_set_upload_path */
-static int g_upload_path = 0;
+/* 1 (default) = TMA box loads (vr_upload_tma442_kernel: 5.58 TB/s on c3, 4.86 on c2) where the source allows it (sx % 4 == 0, 16-byte
+ * aligned), 0 = cp.async staging (vr_upload_tile442_kernel: 5.23 / 4.83 TB/s; also the fallback) - measured round 2,
+ * profiles/r2_upload.md; vr_debug_set_upload_path */
+static int g_upload_path = 1;
 void vr_set_upload_path(int path) { g_upload_path = path; }
 
 cudaError_t vr_launch_upload(const VrGrid& grid, float* bricks, const float* src, int x0, int y0, int z0, int sx, int sy,
@@ -341,18 +342,26 @@ cudaError_t vr_launch_download(const VrGrid& grid, const float* bricks, float* d
  * coordinates are filled with zeros by the unit and never used) while all threads turn the previous chunk into
  * micro-tiles, two shared-memory stages, one mbarrier each. Against the cp.async version: no address arithmetic and no
  * 4-byte requests on the load side - but the unit wants every box to start on a 16-byte boundary of the source row
- * (a box at x = -1 faults as an illegal instruction), so with one ghost layer the staged rows sit 3 cells askew and
- * the 16-byte tile rows are gathered with four 4-byte shared loads. Measured (round 2): 5 % SLOWER than the cp.async
- * kernel on c3 (41.9 against 39.7 ms for 207 GB), 11 % on c2: kept as the alternative behind vr_debug_set_upload_path,
- * not the default. Needs sx % 4 == 0 and a 16-byte aligned source (the tensor map's strides), else the caller falls back.
+ * (a box at x = -1 faults as an illegal instruction), so with one ghost layer the staged rows sit 3 cells askew: a
+ * 16-byte tile row is picked out of TWO aligned 128-bit shared loads. First version (four 4-byte shared loads per row,
+ * a warp store over eight half-lines): 5 % slower than the cp.async kernel on c3. With whole-line stores and aligned
+ * conflict-free loads (the lane mapping in the kernel): 37.15 against 39.65 ms for c3's 207 GB (5.58 against 5.23 TB/s),
+ * 1.787 against 1.799 ms on c2 - the default. Three or four stages (fewer CTAs per SM) and 8-row boxes are slower
+ * (profiles/r2_upload.md). Needs sx % 4 == 0 and a 16-byte aligned source (the tensor map's strides), else the caller
+ * falls back to the cp.async kernel.
  * ---------------------------------------------------------------------------------------- */
 #include <cuda.h>
 
 #define TMA_BX 128 /* cells per chunk */
 #define TMA_BW (TMA_BX + 4) /* box width: the unit wants the box to start on a 16-byte boundary of the source row, so it starts
                              * up to 3 cells early (a ghost layer of 1 puts padded cell 0 at voxel -1 mod 4) */
+#ifndef TMA_TR
 #define TMA_TR 4   /* tile rows per group: 16 source rows */
+#endif
 #define TMA_STAGE_FLOATS (TMA_BW * TMA_TR * 4 * 2)
+#ifndef VR_TMA_STAGES
+#define VR_TMA_STAGES 2 /* shared-memory stages (boxes in flight per CTA) */
+#endif
 
 __device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(unsigned long long* bar, int count) {
@@ -380,7 +389,7 @@ __global__ void __launch_bounds__(256)
 vr_upload_tma442_kernel(VrGrid g, float* __restrict__ bricks, const __grid_constant__ CUtensorMap tm, const float* __restrict__ src,
                         int x0, int y0, int z0, int sx, int sy, int sz, int b0) {
     extern __shared__ __align__(128) float s_box_raw[]; /* two stages of [2][16][128] floats, 128-byte aligned by hand */
-    __shared__ __align__(8) unsigned long long s_bar[2];
+    __shared__ __align__(8) unsigned long long s_bar[VR_TMA_STAGES];
     float* s_box = reinterpret_cast<float*>((reinterpret_cast<uintptr_t>(s_box_raw) + 127) & ~(uintptr_t)127);
     const int b = blockIdx.y + b0;
     int bc[3], lo[3], hi[3];
@@ -404,8 +413,7 @@ vr_upload_tma442_kernel(VrGrid g, float* __restrict__ bricks, const __grid_const
     const int xskew = (xbase + (tx0 << 2) - x0) & 3; /* cells between the box's 16-byte aligned start and the chunk's first cell */
     const int tid = threadIdx.x;
     if (tid == 0) {
-        mbar_init(&s_bar[0], 1);
-        mbar_init(&s_bar[1], 1);
+        for (int q = 0; q < VR_TMA_STAGES; ++q) mbar_init(&s_bar[q], 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
@@ -415,23 +423,27 @@ vr_upload_tma442_kernel(VrGrid g, float* __restrict__ bricks, const __grid_const
     auto issue = [&](int u) {
         const int grp = (int)blockIdx.x + (u / nchunks) * (int)gridDim.x, c = u % nchunks;
         const int jf = (ty0 + (grp % ngy) * TMA_TR) << 2, kt = (tz0 + grp / ngy) << 1, ic = (tx0 << 2) + c * TMA_BX;
-        unsigned long long* bar = &s_bar[u & 1];
+        unsigned long long* bar = &s_bar[u % VR_TMA_STAGES];
         mbar_expect_tx(bar, TMA_STAGE_FLOATS * 4u);
-        tma_load_3d(s_box + (u & 1) * TMA_STAGE_FLOATS, &tm, bar, (xbase + ic - x0) & ~3, ybase + jf - y0, zbase + kt - z0);
+        tma_load_3d(s_box + (u % VR_TMA_STAGES) * TMA_STAGE_FLOATS, &tm, bar, (xbase + ic - x0) & ~3, ybase + jf - y0, zbase + kt - z0);
     };
-    if (tid == 0 && units > 0) issue(0);
+    if (tid == 0)
+        for (int u = 0; u < VR_TMA_STAGES - 1 && u < units; ++u) issue(u);
     for (int u = 0; u < units; ++u) {
-        if (tid == 0 && u + 1 < units) issue(u + 1); /* its stage was released by the barrier that ended unit u - 1 */
-        mbar_wait(&s_bar[u & 1], (unsigned)((u >> 1) & 1));
+        if (tid == 0 && u + VR_TMA_STAGES - 1 < units) issue(u + VR_TMA_STAGES - 1); /* its stage was released by the barrier that ended unit u - 1 */
+        mbar_wait(&s_bar[u % VR_TMA_STAGES], (unsigned)((u / VR_TMA_STAGES) & 1));
         const int grp = (int)blockIdx.x + (u / nchunks) * (int)gridDim.x, c = u % nchunks;
         const int tyg = ty0 + (grp % ngy) * TMA_TR, kt = (tz0 + grp / ngy) << 1, ic = (tx0 << 2) + c * TMA_BX;
-        const float* __restrict__ box = s_box + (u & 1) * TMA_STAGE_FLOATS;
-        /* 1024 sixteen-byte tile rows per unit, 4 per thread: a quarter-warp takes 8 consecutive tiles of one row
-         * (conflict-free 128-bit shared loads), a warp the four rows lj of one plane lk of those tiles */
+        const float* __restrict__ box = s_box + (u % VR_TMA_STAGES) * TMA_STAGE_FLOATS;
+        /* 1024 sixteen-byte tile rows per unit (TMA_TR = 4), 4 per thread. A warp takes the 8 rows (lj, lk) of FOUR tiles, so its store
+         * covers four whole 128-byte lines; a quarter-warp (one 128-bit shared-load wavefront) takes the rows lj = 0..3 of one
+         * plane lk of the tiles t and t + 4: rows are 132 floats apart (4 banks), tiles 4 floats, so its eight 16-byte words
+         * fall into eight different bank groups - also one word further on (the second load of an askew row) */
 #pragma unroll
-        for (int n = 0; n < 4; ++n) {
-            const int idx = tid + 256 * n;
-            const int txl = (idx & 7) | (((idx >> 5) & 3) << 3), lj = (idx >> 3) & 3, lk = (idx >> 7) & 1, tr = idx >> 8;
+        for (int n = 0; n < TMA_TR; ++n) { /* 256 TMA_TR tile rows per unit */
+            const int idx = tid + 256 * n, w = idx >> 5;
+            const int lj = idx & 3, lk = (idx >> 3) & 1, tr = w >> 3;
+            const int txl = (w & 3) | (((idx >> 2) & 1) << 2) | (((idx >> 4) & 1) << 3) | (((w >> 2) & 1) << 4);
             const int tx = (ic >> 2) + txl, i = tx << 2, j = ((tyg + tr) << 2) + lj, k = kt + lk;
             if (tx >= tx1 || tyg + tr >= ty1 || j < j0 || j >= j1 || k < k0 || k >= k1) continue;
             const float* __restrict__ srow = box + (lk * (TMA_TR * 4) + tr * 4 + lj) * TMA_BW + (txl << 2) + xskew;
@@ -441,7 +453,14 @@ vr_upload_tma442_kernel(VrGrid g, float* __restrict__ bricks, const __grid_const
             const int gy = ybase + j, gz = zbase + k, gx = xbase + i;
             const bool edge = gy < 0 || gy >= g.n[1] || gz < 0 || gz >= g.n[2] || gx < 0 || gx + 3 >= g.n[0];
             if (!edge && i >= i0 && i + 3 < i1) {
-                *reinterpret_cast<float4*>(out) = xskew ? make_float4(srow[0], srow[1], srow[2], srow[3]) : *reinterpret_cast<const float4*>(srow);
+                /* an askew row: two aligned 128-bit loads and a pick (xskew is the same for the whole CTA) */
+                const float4 A = *reinterpret_cast<const float4*>(srow - xskew);
+                float4 v = A;
+                if (xskew) {
+                    const float4 B = *reinterpret_cast<const float4*>(srow - xskew + 4);
+                    v = xskew == 1 ? make_float4(A.y, A.z, A.w, B.x) : xskew == 2 ? make_float4(A.z, A.w, B.x, B.y) : make_float4(A.w, B.x, B.y, B.z);
+                }
+                *reinterpret_cast<float4*>(out) = v;
             } else if (!edge) {
 #pragma unroll
                 for (int q = 0; q < 4; ++q)
@@ -485,7 +504,7 @@ static cudaError_t launch_upload_tma(const VrGrid& grid, float* bricks, const fl
     if (encode(&tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, (void*)src, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
                CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
         return cudaErrorNotSupported;
-    const size_t smem = 2 * TMA_STAGE_FLOATS * sizeof(float) + 128;
+    const size_t smem = VR_TMA_STAGES * TMA_STAGE_FLOATS * sizeof(float) + 128;
     cudaError_t e = cudaFuncSetAttribute(vr_upload_tma442_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     const long long ty = (((long long)grid.P >> 2) + 1 + TMA_TR - 1) / TMA_TR;

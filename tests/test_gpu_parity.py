@@ -68,23 +68,27 @@ def test_brick_store_is_bit_exact(vr, ghost):
 
 
 def test_tma_upload_path_gives_the_same_store(vr):
-    """vr_debug_set_upload_path: the TMA box-load kernel (cp.async.bulk.tensor) and the cp.async staging kernel fill the
-    store identically, ragged bricks, volume faces (edge replication) and sub-box uploads included."""
+    """vr_debug_set_upload_path: the TMA box-load kernel (cp.async.bulk.tensor, the default) and the cp.async staging kernel
+    (its fallback) fill the store identically, ragged bricks, volume faces (edge replication), sub-box uploads and boxes
+    the tensor map cannot describe (a row length that is not a multiple of 4 cells) included."""
     import torch
-    for dims, brick, ghost in (((128, 96, 80), 32, 1), ((100, 72, 50), 32, 2), ((64, 64, 64), 64, 1)):
+    for dims, brick, ghost in (((128, 96, 80), 32, 1), ((100, 72, 50), 32, 2), ((64, 64, 64), 64, 1), ((101, 72, 50), 32, 1)):
         data = synth.Cube(6, *dims, 3).fill_host()
         o = oracle.Volume(*dims, brick, ghost, data=data)
         d = torch.from_numpy(data).cuda()
         try:
-            vr.debug_set_upload_path(1)
-            g = vr.Volume(*dims, brick, ghost)
-            for z0 in range(0, dims[2], 24):                   # z-slabs, then an interior sub-box written again
-                g.upload(d[z0:z0 + 24].contiguous(), origin=(0, 0, z0))
-            g.upload(d[8:40, 12:60, 20:84].contiguous(), origin=(20, 12, 8))
+            for path in (1, 0):
+                vr.debug_set_upload_path(path)
+                g = vr.Volume(*dims, brick, ghost)
+                for z0 in range(0, dims[2], 24):                   # z-slabs, then interior sub-boxes written again
+                    g.upload(d[z0:z0 + 24].contiguous(), origin=(0, 0, z0))
+                g.upload(d[8:40, 12:60, 20:84].contiguous(), origin=(20, 12, 8))
+                g.upload(d[3:30, 5:41, 7:70].contiguous(), origin=(7, 5, 3))     # 63 cells per row: the cp.async kernel either way
+                for b in range(g.nbricks):
+                    assert np.array_equal(g.debug_brick_data(b), o.brick_data(b)), (dims, b, path)
+                g.close()
         finally:
-            vr.debug_set_upload_path(0)
-        for b in range(g.nbricks):
-            assert np.array_equal(g.debug_brick_data(b), o.brick_data(b)), (dims, b)
+            vr.debug_set_upload_path(1)
 
 
 # --------------------------------------------------------------------------- a2, a3
