@@ -522,7 +522,7 @@ int vr_debug_probe_dram(const void* buf, uint64_t bytes, int flavour, int span_b
 /* Which kernel vr_volume_upload uses for the default (4x4x2) layout, process-wide: 1 (default) = source boxes loaded by the
  * TMA unit (cp.async.bulk.tensor; needs sx % 4 == 0 and a 16-byte aligned source, else falls back to 0), 0 = cp.async
  * staging. Both give the same store, bit for bit; the switch exists to measure one against the other
- * (round 2, c3: 5.58 TB/s against 5.23 TB/s). */
+ * (round 2, c3: 5.86 TB/s against 5.23 TB/s). */
 int vr_debug_set_upload_path(int path);
 
 /* Number of kernel launches the library has issued on this handle since creation. */

@@ -261,7 +261,7 @@ vr_download_kernel(VrGrid g, const float* __restrict__ bricks, float* __restrict
 
 static cudaError_t launch_upload_tma(const VrGrid& grid, float* bricks, const float* src, int x0, int y0, int z0, int sx, int sy, int sz,
                                      int b0, unsigned nby, cudaStream_t st);
-/* 1 (default) = TMA box loads (vr_upload_tma442_kernel: 5.58 TB/s on c3, 4.86 on c2) where the source allows it (sx % 4 == 0, 16-byte
+/* 1 (default) = TMA box loads (vr_upload_tma442_kernel: 5.86 TB/s on c3, 4.95 on c2) where the source allows it (sx % 4 == 0, 16-byte
  * aligned), 0 = cp.async staging (vr_upload_tile442_kernel: 5.23 / 4.83 TB/s; also the fallback) - measured round 2,
  * profiles/r2_upload.md; vr_debug_set_upload_path */
 static int g_upload_path = 1;
@@ -345,8 +345,8 @@ cudaError_t vr_launch_download(const VrGrid& grid, const float* bricks, float* d
  * (a box at x = -1 faults as an illegal instruction), so with one ghost layer the staged rows sit 3 cells askew: a
  * 16-byte tile row is picked out of TWO aligned 128-bit shared loads. First version (four 4-byte shared loads per row,
  * a warp store over eight half-lines): 5 % slower than the cp.async kernel on c3. With whole-line stores and aligned
- * conflict-free loads (the lane mapping in the kernel): 37.15 against 39.65 ms for c3's 207 GB (5.58 against 5.23 TB/s),
- * 1.787 against 1.799 ms on c2 - the default. Three or four stages (fewer CTAs per SM) and 8-row boxes are slower
+ * conflict-free loads (the lane mapping in the kernel), the per-unit tests hoisted and a narrow box for a row's ghost-cell tail:
+ * 35.41 against 39.65 ms for c3's 207 GB (5.86 against 5.23 TB/s), 1.754 against 1.799 ms on c2 - the default. Three or four stages (fewer CTAs per SM) and 8-row boxes are slower
  * (profiles/r2_upload.md). Needs sx % 4 == 0 and a 16-byte aligned source (the tensor map's strides), else the caller
  * falls back to the cp.async kernel.
  * ---------------------------------------------------------------------------------------- */
@@ -359,6 +359,8 @@ cudaError_t vr_launch_download(const VrGrid& grid, const float* bricks, float* d
 #define TMA_TR 4   /* tile rows per group: 16 source rows */
 #endif
 #define TMA_STAGE_FLOATS (TMA_BW * TMA_TR * 4 * 2)
+#define TMA_TW 8    /* box width of a brick row's TAIL: the last chunk of a 128 k + 2 ghost cells wide row holds 2 or 4 cells (+ up to 3 of skew);
+                     * a full-width box there would read 132 cells for them (c3: 660 cells read per row of 514) */
 #ifndef VR_TMA_STAGES
 #define VR_TMA_STAGES 2 /* shared-memory stages (boxes in flight per CTA) */
 #endif
@@ -386,7 +388,8 @@ __device__ __forceinline__ void tma_load_3d(float* dst, const CUtensorMap* tm, u
 }
 
 __global__ void __launch_bounds__(256)
-vr_upload_tma442_kernel(VrGrid g, float* __restrict__ bricks, const __grid_constant__ CUtensorMap tm, const float* __restrict__ src,
+vr_upload_tma442_kernel(VrGrid g, float* __restrict__ bricks, const __grid_constant__ CUtensorMap tm, const __grid_constant__ CUtensorMap tm_tail,
+                        const float* __restrict__ src,
                         int x0, int y0, int z0, int sx, int sy, int sz, int b0) {
     extern __shared__ __align__(128) float s_box_raw[]; /* two stages of [2][16][128] floats, 128-byte aligned by hand */
     __shared__ __align__(8) unsigned long long s_bar[VR_TMA_STAGES];
@@ -407,11 +410,16 @@ vr_upload_tma442_kernel(VrGrid g, float* __restrict__ bricks, const __grid_const
     const int ty0 = j0 >> 2, ty1 = ((j1 - 1) >> 2) + 1;
     const int tz0 = k0 >> 1, tz1 = ((k1 - 1) >> 1) + 1;
     const int ngy = (ty1 - ty0 + TMA_TR - 1) / TMA_TR, groups = ngy * (tz1 - tz0);
-    const int nchunks = ((tx1 - tx0) * 4 + TMA_BX - 1) / TMA_BX;
     const int xbase = lo[0] - g.ghost, ybase = lo[1] - g.ghost, zbase = lo[2] - g.ghost; /* global voxel of padded cell 0 */
     float* __restrict__ dstb = bricks + (long long)slot_b * g.slot;
     const int xskew = (xbase + (tx0 << 2) - x0) & 3; /* cells between the box's 16-byte aligned start and the chunk's first cell */
+    /* chunks of 128 cells; a last chunk of a few cells (the ghost layers of a 128 k wide brick) comes in a narrow box. (Letting it ride
+     * along with the last full chunk in a 140-cell box - one unit less per group - was 14 % slower: profiles/r2_upload.md) */
+    const int nchunks = (i1 - (tx0 << 2) + TMA_BX - 1) / TMA_BX;
     const int tid = threadIdx.x;
+    /* phase-2 role of this thread (see the loop): row lj of plane lk of the tile txl of a chunk */
+    const int lane_lj = tid & 3, lane_lk = (tid >> 3) & 1;
+    const int lane_txl = ((tid >> 5) & 3) | (((tid >> 2) & 1) << 2) | (((tid >> 4) & 1) << 3) | (((tid >> 7) & 1) << 4);
     if (tid == 0) {
         for (int q = 0; q < VR_TMA_STAGES; ++q) mbar_init(&s_bar[q], 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -424,8 +432,10 @@ vr_upload_tma442_kernel(VrGrid g, float* __restrict__ bricks, const __grid_const
         const int grp = (int)blockIdx.x + (u / nchunks) * (int)gridDim.x, c = u % nchunks;
         const int jf = (ty0 + (grp % ngy) * TMA_TR) << 2, kt = (tz0 + grp / ngy) << 1, ic = (tx0 << 2) + c * TMA_BX;
         unsigned long long* bar = &s_bar[u % VR_TMA_STAGES];
-        mbar_expect_tx(bar, TMA_STAGE_FLOATS * 4u);
-        tma_load_3d(s_box + (u % VR_TMA_STAGES) * TMA_STAGE_FLOATS, &tm, bar, (xbase + ic - x0) & ~3, ybase + jf - y0, zbase + kt - z0);
+        const bool tail = (i1 - ic) + xskew <= TMA_TW; /* the narrow box holds everything this chunk needs */
+        mbar_expect_tx(bar, (tail ? TMA_TW : TMA_BW) * (TMA_TR * 4 * 2) * 4u);
+        tma_load_3d(s_box + (u % VR_TMA_STAGES) * TMA_STAGE_FLOATS, tail ? &tm_tail : &tm, bar, (xbase + ic - x0) & ~3, ybase + jf - y0,
+                    zbase + kt - z0);
     };
     if (tid == 0)
         for (int u = 0; u < VR_TMA_STAGES - 1 && u < units; ++u) issue(u);
@@ -439,38 +449,47 @@ vr_upload_tma442_kernel(VrGrid g, float* __restrict__ bricks, const __grid_const
          * covers four whole 128-byte lines; a quarter-warp (one 128-bit shared-load wavefront) takes the rows lj = 0..3 of one
          * plane lk of the tiles t and t + 4: rows are 132 floats apart (4 banks), tiles 4 floats, so its eight 16-byte words
          * fall into eight different bank groups - also one word further on (the second load of an askew row) */
-#pragma unroll
-        for (int n = 0; n < TMA_TR; ++n) { /* 256 TMA_TR tile rows per unit */
-            const int idx = tid + 256 * n, w = idx >> 5;
-            const int lj = idx & 3, lk = (idx >> 3) & 1, tr = w >> 3;
-            const int txl = (w & 3) | (((idx >> 2) & 1) << 2) | (((idx >> 4) & 1) << 3) | (((w >> 2) & 1) << 4);
-            const int tx = (ic >> 2) + txl, i = tx << 2, j = ((tyg + tr) << 2) + lj, k = kt + lk;
-            if (tx >= tx1 || tyg + tr >= ty1 || j < j0 || j >= j1 || k < k0 || k >= k1) continue;
-            const float* __restrict__ srow = box + (lk * (TMA_TR * 4) + tr * 4 + lj) * TMA_BW + (txl << 2) + xskew;
-            float* __restrict__ out = dstb + (vr_axis_offset(g.ax[1], j) + vr_axis_offset(g.ax[2], k)) + (tx << 5);
+        /* idx = tid + 256 n: a thread keeps its row (lj, lk) and its tile txl (lane_* above) in every round; n is the tile row.
+         * What does not depend on n is tested once per unit. */
+        const int pitch = (i1 - ic) + xskew <= TMA_TW ? TMA_TW : TMA_BW; /* as issued */
+        const int txl = lane_txl;
+        const int tx = (ic >> 2) + txl, i = tx << 2, k = kt + lane_lk;
+        if (tx < tx1 && k >= k0 && k < k1) {
+            const int gz = zbase + k, gx = xbase + i;
             /* cells outside the volume replicate the edge voxel (R3): the unit filled them with zeros, so the few rows and
              * columns on the volume's faces take the clamped voxel straight from the source (it lies in the box: padded_range) */
-            const int gy = ybase + j, gz = zbase + k, gx = xbase + i;
-            const bool edge = gy < 0 || gy >= g.n[1] || gz < 0 || gz >= g.n[2] || gx < 0 || gx + 3 >= g.n[0];
-            if (!edge && i >= i0 && i + 3 < i1) {
-                /* an askew row: two aligned 128-bit loads and a pick (xskew is the same for the whole CTA) */
-                const float4 A = *reinterpret_cast<const float4*>(srow - xskew);
-                float4 v = A;
-                if (xskew) {
-                    const float4 B = *reinterpret_cast<const float4*>(srow - xskew + 4);
-                    v = xskew == 1 ? make_float4(A.y, A.z, A.w, B.x) : xskew == 2 ? make_float4(A.z, A.w, B.x, B.y) : make_float4(A.w, B.x, B.y, B.z);
+            const bool edge_xz = gz < 0 || gz >= g.n[2] || gx < 0 || gx + 3 >= g.n[0];
+            const bool whole = i >= i0 && i + 3 < i1;
+            const float* __restrict__ scol = box + (lane_lk * (TMA_TR * 4) + lane_lj) * pitch + (txl << 2);
+            float* __restrict__ ocol = dstb + vr_axis_offset(g.ax[2], k) + (tx << 5);
+#pragma unroll
+            for (int n = 0; n < TMA_TR; ++n) { /* 256 TMA_TR tile rows per unit */
+                const int j = ((tyg + n) << 2) + lane_lj;
+                if (tyg + n >= ty1 || j < j0 || j >= j1) continue;
+                const float* __restrict__ srow = scol + n * (4 * pitch); /* 16-byte aligned; the cells start xskew further on */
+                float* __restrict__ out = ocol + vr_axis_offset(g.ax[1], j);
+                const int gy = ybase + j;
+                const bool edge = edge_xz || gy < 0 || gy >= g.n[1];
+                if (!edge && whole) {
+                    /* an askew row: two aligned 128-bit loads and a pick (xskew is the same for the whole CTA) */
+                    const float4 A = *reinterpret_cast<const float4*>(srow);
+                    float4 v = A;
+                    if (xskew) {
+                        const float4 B = *reinterpret_cast<const float4*>(srow + 4);
+                        v = xskew == 1 ? make_float4(A.y, A.z, A.w, B.x) : xskew == 2 ? make_float4(A.z, A.w, B.x, B.y) : make_float4(A.w, B.x, B.y, B.z);
+                    }
+                    *reinterpret_cast<float4*>(out) = v;
+                } else if (!edge) {
+#pragma unroll
+                    for (int q = 0; q < 4; ++q)
+                        if (i + q >= i0 && i + q < i1) out[q] = srow[xskew + q];
+                } else {
+                    const int cy = min(max(gy, 0), g.n[1] - 1), cz = min(max(gz, 0), g.n[2] - 1);
+                    const float* __restrict__ grow = src + ((long long)(cz - z0) * sy + (cy - y0)) * sx - x0;
+#pragma unroll
+                    for (int q = 0; q < 4; ++q)
+                        if (i + q >= i0 && i + q < i1) out[q] = __ldg(grow + min(max(gx + q, 0), g.n[0] - 1));
                 }
-                *reinterpret_cast<float4*>(out) = v;
-            } else if (!edge) {
-#pragma unroll
-                for (int q = 0; q < 4; ++q)
-                    if (i + q >= i0 && i + q < i1) out[q] = srow[q];
-            } else {
-                const int cy = min(max(gy, 0), g.n[1] - 1), cz = min(max(gz, 0), g.n[2] - 1);
-                const float* __restrict__ grow = src + ((long long)(cz - z0) * sy + (cy - y0)) * sx - x0;
-#pragma unroll
-                for (int q = 0; q < 4; ++q)
-                    if (i + q >= i0 && i + q < i1) out[q] = __ldg(grow + min(max(gx + q, 0), g.n[0] - 1));
             }
         }
         __syncthreads();
@@ -504,6 +523,11 @@ static cudaError_t launch_upload_tma(const VrGrid& grid, float* bricks, const fl
     if (encode(&tm, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, (void*)src, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
                CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
         return cudaErrorNotSupported;
+    CUtensorMap tm_tail;
+    const cuuint32_t box_tail[3] = {TMA_TW, TMA_TR * 4, 2};
+    if (encode(&tm_tail, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 3, (void*)src, dims, strides, box_tail, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+               CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+        return cudaErrorNotSupported;
     const size_t smem = VR_TMA_STAGES * TMA_STAGE_FLOATS * sizeof(float) + 128;
     cudaError_t e = cudaFuncSetAttribute(vr_upload_tma442_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
@@ -511,6 +535,6 @@ static cudaError_t launch_upload_tma(const VrGrid& grid, float* bricks, const fl
     const long long tz = (((long long)(sz < grid.P ? sz + 2 * grid.ghost : grid.P)) >> 1) + 2;
     long long bx = ty * tz;
     if (bx > 4096) bx = 4096;
-    vr_upload_tma442_kernel<<<dim3((unsigned)bx, nby), 256, smem, st>>>(grid, bricks, tm, src, x0, y0, z0, sx, sy, sz, b0);
+    vr_upload_tma442_kernel<<<dim3((unsigned)bx, nby), 256, smem, st>>>(grid, bricks, tm, tm_tail, src, x0, y0, z0, sx, sy, sz, b0);
     return cudaGetLastError();
 }
