@@ -306,6 +306,16 @@ def run_bricks_sharded(args, vr, wl, tf, mode_id, rank, world, local_rank, dist,
     rdr.set_transfer_function(tf, *tf_range(wl))
     rdr.set_early_termination(wl["tau"])
     lo, hi = rdr.minmax()
+    # rows a1 / a5 on a part: the faster arm where it fits beside the part's store (a rank holds 1 / N of the cube) - float32
+    # arrays for ALPHA values, 8-bit arrays as the exact MIP filter; falls back to the hand-rolled sampler (tests/test_gpu_sortlast.py)
+    part_sampler = "manual"
+    want = {"auto": "texture" if mode_id == 0 else "texture_byte", "manual": None}.get(args.sampler, args.sampler)
+    if want and args.tf in ("ramp", "translucent"):
+        try:
+            rdr.backend.volume.set_sampler(sampler_id(vr, want))
+            part_sampler = want
+        except vr.VrError:
+            pass
     W, H, K, Wm = wl["width"], wl["height"], args.steps, args.warmup
     nv = len(wl["views"])
     sampler = ClockSampler(local_rank) if rank == 0 else None
@@ -351,7 +361,7 @@ def run_bricks_sharded(args, vr, wl, tf, mode_id, rank, world, local_rank, dist,
             "e2e": {"value": round(K / (e2e_ms * 1e-3), 3), "unit": "frames/s", "h2d_bytes_per_step": 128 * world,
                     "d2h_bytes_per_step": W * H * 16,
                     "what": "SortLastRenderer.render on every rank + the merged frame copied to pinned host memory on rank 0"},
-            "clocks": clocks, "exchange_bytes_per_frame": moved, "frame_bytes": W * H * 16,
+            "clocks": clocks, "exchange_bytes_per_frame": moved, "frame_bytes": W * H * 16, "sampler": part_sampler + " (rank 0's part)",
             "data_range": [float(lo), float(hi)], "roofline": None, "cpu_baseline": None}
 
 

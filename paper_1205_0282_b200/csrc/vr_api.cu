@@ -876,7 +876,13 @@ extern "C" int vr_set_sampler(vr_volume* v, int sampler) {
         const VrGrid& g = v->grid;
         if (!(g.layout == VR_LAYOUT_TILED && g.tl[0] == 2 && g.tl[1] == 2 && g.tl[2] == 1 && g.ml[0] == 0 && g.ml[1] == 0 && g.ml[2] == 0))
             return fail(v, VR_ERR_STATE, "vr_set_sampler: the texture arm is built beside the default (4x4x2 tiled) store only");
-        const cudaError_t e = vr_tex_create(g, &v->tex, true, texel);
+        /* ask first: creating ~100 arrays until one fails and freeing them again takes seconds and has been seen to leave the
+         * process with slow host copies afterwards (bench.py --sharding bricks on the 103 GB cube) */
+        size_t free_b = 0, total_b = 0;
+        const double need_b = (double)g.slot * g.nown * (texel == VR_TEXEL_FLOAT ? 4.0 : texel == VR_TEXEL_HALF ? 2.0 : 1.0);
+        cudaError_t e = cudaMemGetInfo(&free_b, &total_b);
+        if (e == cudaSuccess && (double)free_b < need_b * 1.01 + 64e6) e = cudaErrorMemoryAllocation;
+        if (e == cudaSuccess) e = vr_tex_create(g, &v->tex, true, texel);
         if (e != cudaSuccess) v->sampler = VR_SAMPLER_MANUAL; /* no arrays (any of another width were freed above): hand-rolled */
         if (e != cudaSuccess)
             return fail(v, e == cudaErrorMemoryAllocation ? VR_ERR_OUT_OF_MEMORY : VR_ERR_CUDA,
