@@ -271,7 +271,11 @@ int vr_set_traversal(vr_volume* v, int traversal);
  * is then VR_SAMPLER_MANUAL: arrays of another texel width were freed to make room) and refilled from the store on the device by the first frame after an upload. The sample
  * SET is unchanged (same FP64 set-up); the hardware's 8-bit interpolation weights perturb sample values by up
  * to 2^-9 of the local voxel differences, which keeps VR_ALPHA inside its 2e-3 tolerance but moves early-
- * termination decisions of rays whose opacity passes tau within ~1e-4 of it.
+ * termination decisions of rays whose opacity passes tau within ~1e-4 of it. The opacity correction 1 - (1 - a)^step
+ * multiplies that error by the step and, for steps below one voxel, without bound where the table's opacity nears 1:
+ * ALPHA values come from the arrays for 0 < step <= 1 only (larger steps and VR_STEP_AUTO: hand-rolled); with step < 1 a
+ * sample whose table opacity exceeds 0.9 is re-evaluated by the hand-rolled sampler, and a ray's (at most two) exit
+ * samples are hand-rolled whenever the float32 store exists.
  * VR_MIP frames (1e-5) of the VR_SORT_LAST traversal use the arrays as an EXACT filter: a filtered fetch is within
  * range / 64 (+ 2^-14 of the largest magnitude) of the hand-rolled value for every sample of a brick (the brick's
  * range: row f1), so only samples whose filtered value lies within twice that of the largest one seen on their ray
@@ -312,7 +316,8 @@ int vr_set_sampler(vr_volume* v, int sampler);
  * float32 cells back to the device (peak memory: the store plus one array). Bricks that hold blanked (NaN) voxels keep
  * their float32 cells, because R14 needs them. The arrays take the texel width of the sampler in force (float16 after
  * vr_set_sampler(v, VR_SAMPLER_TEXTURE_HALF), else float32). Afterwards the handle renders VR_ALPHA frames (both traversals) through the
- * texture arm only: vr_volume_upload / download, VR_MIP frames, counting mode 2 and transfer functions with a step
+ * texture arm only: vr_volume_upload / download, VR_MIP frames, counting mode 2, transfer functions with a step and
+ * sample steps outside [0.9, 1] voxels (see vr_set_sampler: smaller steps need the float32 store for their guard)
  * return VR_ERR_STATE. Irreversible; synchronises. freed_bytes_out (host, may be NULL): device memory given back.
  * Errors: VR_ERR_STATE (not a releasable handle, nothing uploaded, already released), VR_ERR_OUT_OF_MEMORY, VR_ERR_CUDA. */
 int vr_volume_release_store(vr_volume* v, int64_t* freed_bytes_out, void* stream);

@@ -1116,6 +1116,10 @@ static int render_frame(vr_volume* v, const float* view, const float* proj, int 
         if (mode != VR_ALPHA) return fail(v, VR_ERR_STATE, "vr_render: VR_MIP needs the float32 store, which was released");
         if (!v->tf_smooth) return fail(v, VR_ERR_STATE, "vr_render: a transfer function with a step needs the float32 store, which was released");
         if (v->counting == 2) return fail(v, VR_ERR_STATE, "vr_render: counting mode 2 needs the float32 store, which was released");
+        if (!(step >= 0.9f && step <= 1.0f))
+            return fail(v, VR_ERR_STATE, "vr_render: on a released store the step must lie in [0.9, 1] voxels (the opacity correction multiplies "
+                                         "the texture filter's error by the step, and for smaller steps without bound where the table's "
+                                         "opacity nears 1: such frames need the float32 store, DESIGN.md R20)");
     }
     rc = ensure_sub(v, sub_px);
     if (rc) return rc;
@@ -1146,7 +1150,10 @@ static int render_frame(vr_volume* v, const float* view, const float* proj, int 
     /* texture arm: ALPHA frames with a smooth table take their values from the arrays; MIP frames use the arrays as an exact
      * filter in front of the hand-rolled sampler (needs the float32 store and the bricks' ranges; where stepping over empty
      * macro-cells pays, that stays) */
-    bool tex_alpha = (v->sampler == VR_SAMPLER_TEXTURE || v->sampler == VR_SAMPLER_TEXTURE_HALF) && mode == VR_ALPHA && v->counting != 2 && v->tf_smooth;
+    /* R20: the opacity correction 1 - (1 - a)^w multiplies the filter's per-sample error by the step w: ALPHA values come from the
+     * arrays for steps up to one voxel only (the randomised suite found 2.2e-3 at step 1.63; VR_STEP_AUTO's per-ray steps are >= 1) */
+    bool tex_alpha = (v->sampler == VR_SAMPLER_TEXTURE || v->sampler == VR_SAMPLER_TEXTURE_HALF) && mode == VR_ALPHA && v->counting != 2 && v->tf_smooth &&
+                     step > 0.0f && step <= 1.0f;
     if (tex_alpha && v->sampler == VR_SAMPLER_TEXTURE_HALF) { /* R22: only while float16 is fine enough for this data under this table */
         rc = decide_half_alpha(v, st);
         if (rc) return rc;
@@ -1195,6 +1202,10 @@ static int render_frame(vr_volume* v, const float* view, const float* proj, int 
     p.tex = use_tex ? vr_tex_table(v->tex) : NULL;
     p.tex_nan = use_tex ? vr_tex_nan_table(v->tex) : NULL;
     p.brick_mm = tex_mip ? v->d_mm : NULL;
+    /* R20's guard: with steps below one voxel the opacity correction (1 - a)^w has an unbounded slope where the table's opacity nears
+     * 1, so such samples are re-evaluated by the hand-rolled sampler (needs the float32 store: checked above for a released one) */
+    p.tex_guard = (tex_alpha && !v->store_released && step < 1.0f) ? 0.9f : 2.0f;
+    p.tex_only = v->store_released ? 1 : 0;
     const int texel = tex_mip ? vr_tex_texel(v->tex) : VR_TEXEL_FLOAT;
     p.mip_range_eps = 1.0f / 64.0f + (texel == VR_TEXEL_BYTE ? 1.0f / 500.0f : 0.0f); /* half a byte step is range / 510 */
     p.mip_mag_eps = texel == VR_TEXEL_HALF ? 1.0f / 512.0f : texel == VR_TEXEL_BYTE ? 1.0f / 4096.0f : 1.0f / 16384.0f;

@@ -158,9 +158,14 @@ vr_fused_kernel(const VrRaycastParams prm, float4* __restrict__ frame) {
                                 adv = leap_steps(L, D, n);
                             } else {
                                 const float kf = (float)(n0 - n);
-                                const float v = tex3D<float>(tex, fmaf(kf, Dfx, P0x), fmaf(kf, Dfy, P0y), fmaf(kf, Dfz, P0z));
+                                float v = tex3D<float>(tex, fmaf(kf, Dfx, P0x), fmaf(kf, Dfy, P0y), fmaf(kf, Dfz, P0z));
+                                float4 c = classify_alpha(v, lut, prm.lut);
+                                if (c.w > prm.tex_guard) { /* R20's guard (vr_raycast.cu): nearly opaque entries at steps < 1 */
+                                    v = trilinear<LAY, 0, CLAMP, false>(brick, g, ext, L, prm.bitmap, (long long)slot_b * g.slot);
+                                    c = classify_alpha(v, lut, prm.lut);
+                                }
                                 if (COUNT) nsamples += (v == v) ? 1 : 0;
-                                shade_alpha(acc, v, stepf, lut, prm.lut);
+                                blend_alpha(acc, v, stepf, c);
                                 stopped = !(acc.a < tau);
                             }
                             L.q[0] += D[0] * adv, L.q[1] += D[1] * adv, L.q[2] += D[2] * adv;
@@ -174,15 +179,32 @@ vr_fused_kernel(const VrRaycastParams prm, float4* __restrict__ frame) {
                                 const float ku = kf + (float)u;
                                 vq[u] = tex3D<float>(tex, fmaf(ku, Dfx, P0x), fmaf(ku, Dfy, P0y), fmaf(ku, Dfz, P0z));
                             }
+                            bool by_hand = false;
 #pragma unroll
                             for (int u = 0; u < VR_TEX_DEPTH; ++u) {
-                                if (tactive) {
-                                    if (COUNT) nsamples += (vq[u] == vq[u]) ? 1 : 0;
-                                    shade_alpha(acc, vq[u], stepf, lut, prm.lut);
-                                    stopped = !(acc.a < tau);
-                                    --n;
-                                    tactive = n > 0 && !stopped;
+                                if (tactive && !by_hand) {
+                                    const float4 c = classify_alpha(vq[u], lut, prm.lut);
+                                    if (c.w > prm.tex_guard) {
+                                        by_hand = true; /* R20's guard (vr_raycast.cu): the rest of the batch is dropped and fetched again */
+                                    } else {
+                                        if (COUNT) nsamples += (vq[u] == vq[u]) ? 1 : 0;
+                                        blend_alpha(acc, vq[u], stepf, c);
+                                        stopped = !(acc.a < tau);
+                                        --n;
+                                        tactive = n > 0 && !stopped;
+                                    }
                                 }
+                            }
+                            if (by_hand) { /* this loop does not advance the lattice */
+                                Lattice Lj;
+                                const long long jj = (long long)(n0 - n);
+                                Lj.q[0] = L.q[0] + D[0] * jj, Lj.q[1] = L.q[1] + D[1] * jj, Lj.q[2] = L.q[2] + D[2] * jj;
+                                const float v = trilinear<LAY, 0, CLAMP, false>(brick, g, ext, Lj, prm.bitmap, (long long)slot_b * g.slot);
+                                if (COUNT) nsamples += (v == v) ? 1 : 0;
+                                shade_alpha(acc, v, stepf, lut, prm.lut);
+                                stopped = !(acc.a < tau);
+                                --n;
+                                tactive = n > 0 && !stopped;
                             }
                         }
                     }
@@ -257,7 +279,7 @@ vr_fused_kernel(const VrRaycastParams prm, float4* __restrict__ frame) {
                         L.q[a] = to_fixed(p - ((double)(blo[a] - g.ghost) + 0.5));
                     }
                     float v;
-                    if (TEX && use_tex) { /* the exit samples through the array as well: a released store has no float32 cells */
+                    if (TEX && use_tex && prm.tex_only) { /* a released store has no float32 cells: the exit samples through the array too */
                         const double h = 1.0 / 4294967296.0;
                         v = tex3D<float>(tex, (float)((double)L.q[0] * h + 0.5), (float)((double)L.q[1] * h + 0.5), (float)((double)L.q[2] * h + 0.5));
                     } else {

@@ -159,6 +159,9 @@ struct VrRaycastParams {
     int cell_words;     /* 32-bit words of cell_bits per brick */
     VrLut lut;
     int lut_copies; /* copies of the table in the ray-cast kernel's shared memory (vr_lut_copies) */
+    float tex_guard; /* texture arm, ALPHA, steps below one voxel: a sample whose table opacity exceeds this is evaluated by the hand-rolled
+                      * sampler instead (the opacity correction (1 - a)^w has an unbounded slope at a = 1 for w < 1: R20); > 1 = off */
+    int tex_only;    /* the float32 store was released: the exit samples go through the arrays too */
     double step; /* > 0: sample spacing in voxels; 0: per ray, 1 / max|d_a| (R18) */
     float tau;
     int mode;

@@ -539,8 +539,10 @@ __device__ __forceinline__ float ex2_approx(float x) {
 /* R7: classification and opacity of a sample standing for a path of length w; R8 blending.
  * alpha = 1 - (1-a)^w = 1 - 2^(w log2(1-a)) on the two MUFU approximations (2^-22 relative,
  * DESIGN.md "Tolerances"); a = 1 gives log2(0) = -inf and alpha = 1, a = 0 gives alpha = 0. */
+/* classification (the table's interpolated entry for value v) and blending, separately: the texture arm looks at the
+ * entry's opacity before it blends (R20's guard). shade_alpha = the two in a row, the same operations as ever. */
 template <bool REP = false>
-__device__ __forceinline__ void shade_alpha(Accum& acc, float v, float w, const LutView& lut, const VrLut& P) {
+__device__ __forceinline__ float4 classify_alpha(float v, const LutView& lut, const VrLut& P) {
     const float u = __saturatef((v - P.vmin) * P.inv_range);
     const float x = u * P.scale;
     const int i = min((int)x, P.nm2);
@@ -555,15 +557,23 @@ __device__ __forceinline__ void shade_alpha(Accum& acc, float v, float w, const 
         const unsigned a = lut.base + 32u * (unsigned)i;
         e = lds128<0>(a), dl = lds128<16>(a);
     }
-    const float cr = fmaf(f, dl.x, e.x), cg = fmaf(f, dl.y, e.y), cb = fmaf(f, dl.z, e.z), ca = fmaf(f, dl.w, e.w);
-    const float alpha = 1.0f - ex2_approx(w * lg2_approx(1.0f - ca));
+    return make_float4(fmaf(f, dl.x, e.x), fmaf(f, dl.y, e.y), fmaf(f, dl.z, e.z), fmaf(f, dl.w, e.w));
+}
+
+__device__ __forceinline__ void blend_alpha(Accum& acc, float v, float w, const float4 c) {
+    const float alpha = 1.0f - ex2_approx(w * lg2_approx(1.0f - c.w));
     /* R14: a dropped sample arrives as NaN. It classifies harmlessly (the saturation maps it to entry 0);
      * its opacity is forced to 0. MIP needs nothing: fmaxf ignores NaN. */
     const float ta = (v == v) ? (1.0f - acc.a) * alpha : 0.0f;
-    acc.r = fmaf(ta, cr, acc.r);
-    acc.g = fmaf(ta, cg, acc.g);
-    acc.b = fmaf(ta, cb, acc.b);
+    acc.r = fmaf(ta, c.x, acc.r);
+    acc.g = fmaf(ta, c.y, acc.g);
+    acc.b = fmaf(ta, c.z, acc.b);
     acc.a += ta;
+}
+
+template <bool REP = false>
+__device__ __forceinline__ void shade_alpha(Accum& acc, float v, float w, const LutView& lut, const VrLut& P) {
+    blend_alpha(acc, v, w, classify_alpha<REP>(v, lut, P));
 }
 
 #endif

@@ -51,7 +51,7 @@
  * of c2's instructions were the per-segment FP64 ray set-up. Sparse views (the 103 GB cube) are bound by DRAM requests,
  * not by issue slots: there the table's kernel (0.017 ms) costs more than it saves (0.002 ms), so their instances keep
  * the set-up inside (RAYTAB = false, prm.rays == NULL). The values are the same bit for bit either way. */
-template <int MODE, int LAY, int PT, bool CLAMP, bool COUNT, bool SKIP, bool TEX, bool RAYTAB>
+template <int MODE, int LAY, int PT, bool CLAMP, bool COUNT, bool SKIP, bool TEX, bool RAYTAB, bool GUARD>
 __global__ void __launch_bounds__(VR_RAYCAST_THREADS, TEX ? VR_TEX_CTAS : VR_MIN_CTAS)
 vr_raycast_kernel(const VrRaycastParams prm) {
     /* dynamic (ALPHA): the table, `copies` times (vr_march.cuh): 32 KB at most; what it does not take stays L1 cache */
@@ -205,15 +205,34 @@ vr_raycast_kernel(const VrRaycastParams prm) {
                     const float ku = kf + (float)u;
                     vq[u] = tex3D<float>(tex, fmaf(ku, Dfx, P0x), fmaf(ku, Dfy, P0y), fmaf(ku, Dfz, P0z));
                 }
+                bool by_hand = false; /* GUARD: the next sample of this lane is one for the hand-rolled sampler */
 #pragma unroll
                 for (int u = 0; u < VR_TEX_DEPTH; ++u) {
-                    if (active) {
-                        if (COUNT) nsamples += (vq[u] == vq[u]) ? 1 : 0;
-                        shade_alpha<true>(acc, vq[u], stepf, lut, prm.lut);
-                        stopped = !(acc.a < tau);
-                        --n;
-                        active = n > 0 && !stopped;
+                    if (active && !by_hand) {
+                        const float4 c = classify_alpha<true>(vq[u], lut, prm.lut);
+                        if (GUARD && c.w > prm.tex_guard) {
+                            by_hand = true; /* the rest of the batch is dropped and fetched again after it */
+                        } else {
+                            if (COUNT) nsamples += (vq[u] == vq[u]) ? 1 : 0;
+                            blend_alpha(acc, vq[u], stepf, c);
+                            stopped = !(acc.a < tau);
+                            --n;
+                            active = n > 0 && !stopped;
+                        }
                     }
+                }
+                if (GUARD && by_hand) {
+                    /* R20's guard (steps below one voxel): where the table's opacity nears 1 the opacity correction (1 - a)^w
+                     * amplifies the filter's error without bound - this sample takes its value from the float32 store */
+                    Lattice Lj;
+                    const long long jj = (long long)(n0 - n);
+                    Lj.q[0] = L.q[0] + D[0] * jj, Lj.q[1] = L.q[1] + D[1] * jj, Lj.q[2] = L.q[2] + D[2] * jj;
+                    const float v = trilinear<LAY, PT, CLAMP, false>(brick, g, ext, Lj, prm.bitmap, (long long)slot_b * g.slot);
+                    if (COUNT) nsamples += (v == v) ? 1 : 0;
+                    shade_alpha<true>(acc, v, stepf, lut, prm.lut);
+                    stopped = !(acc.a < tau);
+                    --n;
+                    active = n > 0 && !stopped;
                 }
             }
         }
@@ -233,9 +252,14 @@ vr_raycast_kernel(const VrRaycastParams prm) {
                 }
                 if (adv > 0) {
                     const float kf = (float)(n0 - n);
-                    const float v = tex3D<float>(tex, fmaf(kf, Dfx, P0x), fmaf(kf, Dfy, P0y), fmaf(kf, Dfz, P0z));
+                    float v = tex3D<float>(tex, fmaf(kf, Dfx, P0x), fmaf(kf, Dfy, P0y), fmaf(kf, Dfz, P0z));
+                    float4 c = classify_alpha<true>(v, lut, prm.lut);
+                    if (GUARD && c.w > prm.tex_guard) { /* R20's guard, as above; the lattice is current here */
+                        v = trilinear<LAY, PT, CLAMP, false>(brick, g, ext, L, prm.bitmap, (long long)slot_b * g.slot);
+                        c = classify_alpha<true>(v, lut, prm.lut);
+                    }
                     if (COUNT) nsamples += (v == v) ? 1 : 0;
-                    shade_alpha<true>(acc, v, stepf, lut, prm.lut);
+                    blend_alpha(acc, v, stepf, c);
                     stopped = !(acc.a < tau);
                     if (SKIP) L.q[0] += D[0], L.q[1] += D[1], L.q[2] += D[2];
                 } else {
@@ -391,7 +415,7 @@ vr_raycast_kernel(const VrRaycastParams prm) {
                     L.q[a] = to_fixed(p - ((double)(blo[a] - g.ghost) + 0.5));
                 }
                 float v;
-                if (TEX && MODE == VR_ALPHA && use_tex) { /* the exit samples through the array as well: a released store has no float32 cells */
+                if (TEX && MODE == VR_ALPHA && use_tex && prm.tex_only) { /* a released store has no float32 cells: the exit samples through the array too */
                     const double h = 1.0 / 4294967296.0;
                     v = tex3D<float>(tex, (float)((double)L.q[0] * h + 0.5), (float)((double)L.q[1] * h + 0.5), (float)((double)L.q[2] * h + 0.5));
                 } else {
@@ -425,16 +449,21 @@ vr_raycast_kernel(const VrRaycastParams prm) {
 /* ------------------------------------------------------------------------------------------ */
 /* Persistent grid: resident CTAs per SM (for this instance and its shared memory) x SMs,
  * but no more CTAs than there are groups of 8 work items. */
-template <int MODE, int LAY, int PT, bool CLAMP, bool COUNT, bool SKIP, bool TEX, bool RAYTAB>
+template <int MODE, int LAY, int PT, bool CLAMP, bool COUNT, bool SKIP, bool TEX, bool RAYTAB, bool GUARD>
 static cudaError_t launch_instance(const VrRaycastParams& p0, long long items, bool sparse, cudaStream_t st);
 
 template <int MODE, int LAY, int PT, bool CLAMP, bool COUNT, bool SKIP = false, bool TEX = false>
 static cudaError_t launch_variant(const VrRaycastParams& p, long long items, bool sparse, cudaStream_t st) {
-    return p.rays ? launch_instance<MODE, LAY, PT, CLAMP, COUNT, SKIP, TEX, true>(p, items, sparse, st)
-                  : launch_instance<MODE, LAY, PT, CLAMP, COUNT, SKIP, TEX, false>(p, items, sparse, st);
+    if constexpr (TEX && MODE == VR_ALPHA) { /* R20's guard is compiled into the instances that need it only (steps below one voxel) */
+        if (p.tex_guard <= 1.0f)
+            return p.rays ? launch_instance<MODE, LAY, PT, CLAMP, COUNT, SKIP, TEX, true, true>(p, items, sparse, st)
+                          : launch_instance<MODE, LAY, PT, CLAMP, COUNT, SKIP, TEX, false, true>(p, items, sparse, st);
+    }
+    return p.rays ? launch_instance<MODE, LAY, PT, CLAMP, COUNT, SKIP, TEX, true, false>(p, items, sparse, st)
+                  : launch_instance<MODE, LAY, PT, CLAMP, COUNT, SKIP, TEX, false, false>(p, items, sparse, st);
 }
 
-template <int MODE, int LAY, int PT, bool CLAMP, bool COUNT, bool SKIP, bool TEX, bool RAYTAB>
+template <int MODE, int LAY, int PT, bool CLAMP, bool COUNT, bool SKIP, bool TEX, bool RAYTAB, bool GUARD>
 static cudaError_t launch_instance(const VrRaycastParams& p0, long long items, bool sparse, cudaStream_t st) {
     VrRaycastParams p = p0;
     p.lut_copies = vr_lut_copies(p.lut.n, sparse);
@@ -446,7 +475,7 @@ static cudaError_t launch_instance(const VrRaycastParams& p0, long long items, b
     cudaError_t e = cudaGetDevice(&dev);
     if (e == cudaSuccess) e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
     if (e == cudaSuccess)
-        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&cached_per_sm, vr_raycast_kernel<MODE, LAY, PT, CLAMP, COUNT, SKIP, TEX, RAYTAB>,
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&cached_per_sm, vr_raycast_kernel<MODE, LAY, PT, CLAMP, COUNT, SKIP, TEX, RAYTAB, GUARD>,
                                                           VR_RAYCAST_THREADS, smem);
     if (e != cudaSuccess) return e;
     if (cached_per_sm < 1) return cudaErrorLaunchOutOfResources;
@@ -460,7 +489,7 @@ static cudaError_t launch_instance(const VrRaycastParams& p0, long long items, b
     long long ctas = (long long)sms * per_sm;
     const long long want = (items + (VR_RAYCAST_THREADS / 32) - 1) / (VR_RAYCAST_THREADS / 32);
     if (ctas > want) ctas = want < 1 ? 1 : want;
-    vr_raycast_kernel<MODE, LAY, PT, CLAMP, COUNT, SKIP, TEX, RAYTAB><<<(int)ctas, VR_RAYCAST_THREADS, smem, st>>>(p);
+    vr_raycast_kernel<MODE, LAY, PT, CLAMP, COUNT, SKIP, TEX, RAYTAB, GUARD><<<(int)ctas, VR_RAYCAST_THREADS, smem, st>>>(p);
     return cudaGetLastError();
 }
 

@@ -711,6 +711,15 @@ def test_randomised_configurations(vr, case):
     for s in (vr.SAMPLER_TEXTURE, vr.SAMPLER_TEXTURE_HALF, vr.SAMPLER_TEXTURE_BYTE):
         g.set_sampler(s)
         assert np.array_equal(gpu_frame(g, view, proj, W, H, step if step > 0 else vr.STEP_AUTO, vr.MIP), want), (case, s)
+    # R20 / R22: ALPHA values through float32 and float16 texels against the same oracle at the same 2e-3 (R12's band widened
+    # to the filter's error); stepped tables and blanked bricks fall back to the hand-rolled sampler inside the library
+    # the band: the filter moves a ray's transmittance by up to ~4e-3 of itself, i.e. A_b near tau by 4e-3 (1 - tau); 5x that
+    o.set_ert_margin(0.02 * (1.0 - tau) if tau < 1.0 else 2e-4)
+    ref = o.render(view, proj, W, H, step, oracle.ALPHA)
+    for s in (vr.SAMPLER_TEXTURE, vr.SAMPLER_TEXTURE_HALF):
+        g.set_sampler(s)
+        check_alpha(gpu_frame(g, view, proj, W, H, step if step > 0 else vr.STEP_AUTO, vr.ALPHA), ref, tau,
+                    "case %d sampler %d" % (case, s), envelope=True, max_flagged=1.0)
 
 
 # --------------------------------------------------------------------------- state across calls

@@ -203,8 +203,8 @@ def test_fused_traversal_through_the_texture_arm(vr, tau, texels):
 @pytest.mark.parametrize("texels", TEXELS)
 def test_released_store_renders_through_the_arrays_alone(vr, texels):
     """VR_LAYOUT_TILED_RELEASABLE + vr_volume_release_store (the texture arm for cubes whose second copy does not fit):
-    frames before the release (texture sampler, both stores present) and after it (float32 cells handed back) are
-    bit-identical, match the oracle, the device gets the memory back, bricks with blanked voxels keep their float32
+    frames before the release (texture sampler, both stores present) and after it (float32 cells handed back) agree
+    (only a ray's exit samples come from the float32 store while it exists), match the oracle, the device gets the memory back, bricks with blanked voxels keep their float32
     cells and the exact R14 rule, and everything that needs the float32 store refuses."""
     import torch
     dims, brick = (160, 128, 96), 32
@@ -226,7 +226,7 @@ def test_released_store_renders_through_the_arrays_alone(vr, texels):
     check_mip(mip_before, o.render(fr.seeded(3, 0), fr.proj(False), W, H, 0.5, oracle.MIP), "releasable handle, MIP before the release")
     g.set_sampler(vr.SAMPLER_TEXTURE if texels == "float32" else vr.SAMPLER_TEXTURE_HALF)  # the released arrays take this width
     views = [(fr.seeded(3, k), fr.proj(k == 1)) for k in range(2)]
-    before = [gpu_frame(g, v, p, W, H, 0.5, vr.ALPHA) for v, p in views]
+    before = [gpu_frame(g, v, p, W, H, 1.0, vr.ALPHA) for v, p in views]
     lo, hi = g.minmax()
     torch.cuda.synchronize()
     free0 = torch.cuda.mem_get_info()[0]
@@ -237,15 +237,19 @@ def test_released_store_renders_through_the_arrays_alone(vr, texels):
     assert torch.cuda.mem_get_info()[0] > free0 - 0.5 * store_bytes    # a second copy was NOT needed at any time ...
     assert g.minmax() == (lo, hi)                                      # ... and the range tables survive
     for (v, p), b in zip(views, before):
-        after = gpu_frame(g, v, p, W, H, 0.5, vr.ALPHA)
-        assert np.array_equal(after, b)
-        check_alpha(after, o.render(v, p, W, H, 0.5, oracle.ALPHA), 0.99, "released store", envelope=True, max_flagged=1.0)
+        after = gpu_frame(g, v, p, W, H, 1.0, vr.ALPHA)
+        # the same arrays before and after; only the (at most two) exit samples of a ray came from the float32 store before
+        assert np.abs(after - b).max() < 1e-3 and (after != b).mean() < 0.5
+        check_alpha(after, o.render(v, p, W, H, 1.0, oracle.ALPHA), 0.99, "released store", envelope=True, max_flagged=1.0)
     g.set_traversal(vr.FUSED)
-    fused = gpu_frame(g, *views[0], W, H, 0.5, vr.ALPHA)
-    check_alpha(fused, one.render(*views[0], W, H, 0.5, oracle.ALPHA), 0.99, "released store, fused", envelope=True, max_flagged=1.0)
+    fused = gpu_frame(g, *views[0], W, H, 1.0, vr.ALPHA)
+    check_alpha(fused, one.render(*views[0], W, H, 1.0, oracle.ALPHA), 0.99, "released store, fused", envelope=True, max_flagged=1.0)
     g.set_traversal(vr.SORT_LAST)
     out = torch.empty((H, W, 4), dtype=torch.float32, device="cuda")
     for call in (lambda: g.render(*views[0], W, H, 0.5, vr.MIP, out),
+                 lambda: g.render(*views[0], W, H, 0.5, vr.ALPHA, out),        # steps outside [0.9, 1] need the float32 store (R20)
+                 lambda: g.render(*views[0], W, H, 1.63, vr.ALPHA, out),
+                 lambda: g.render(*views[0], W, H, vr.STEP_AUTO, vr.ALPHA, out),
                  lambda: g.upload(torch.from_numpy(data).cuda()),
                  lambda: g.download(np.empty((4, 4, 4), dtype=np.float32)),
                  lambda: g.debug_brick_data(0),
@@ -256,9 +260,9 @@ def test_released_store_renders_through_the_arrays_alone(vr, texels):
         assert e.value.status == 4
     g.set_transfer_function(synth.tf_threshold(), synth.TF_VMIN, synth.TF_VMAX)
     with pytest.raises(vr.VrError):
-        g.render(*views[0], W, H, 0.5, vr.ALPHA, out)                 # a stepped table needs the float32 store
+        g.render(*views[0], W, H, 1.0, vr.ALPHA, out)                 # a stepped table needs the float32 store
     g.set_transfer_function(synth.tf_ramp(), synth.TF_VMIN, synth.TF_VMAX)
-    assert np.array_equal(gpu_frame(g, *views[0], W, H, 0.5, vr.ALPHA), before[0])
+    assert np.abs(gpu_frame(g, *views[0], W, H, 1.0, vr.ALPHA) - before[0]).max() < 1e-3
     plain = vr.Volume(32, 32, 32, 16, 1)
     plain.upload(np.zeros((32, 32, 32), dtype=np.float32))
     with pytest.raises(vr.VrError):
@@ -424,3 +428,23 @@ def test_mip_exactness_over_scales_and_offsets(vr, case):
         g.set_sampler(s)
         got = gpu_frame(g, view, proj, W, H, step, vr.MIP)
         assert np.array_equal(got, want), (case, s, scale, offset, float(np.abs(got - want).max()))
+
+
+def test_nearly_opaque_samples_at_small_steps_are_taken_by_hand(vr):
+    """R20's guard. With steps below one voxel the opacity correction 1 - (1 - a)^w has an unbounded slope where the table's
+    opacity nears 1: a source whose peak sits just around the top of the table (a -> 1) turned the filter's 1e-3 value error
+    into 7e-3 of the pixel (randomised case 1082). Such samples are re-evaluated by the hand-rolled sampler."""
+    dims = (40, 36, 32)
+    z, y, x = np.indices(dims[::-1]).astype(np.float32)
+    r2 = (x - 20.3) ** 2 + (y - 17.6) ** 2 + (z - 15.2) ** 2
+    data = (np.random.default_rng(3).normal(0, 0.3, dims[::-1]) + 10.9 * np.exp(-r2 / (2 * 2.2 ** 2))).astype(np.float32)  # peak just above vmax = 10
+    W, H = 120, 100
+    fr = synth.Framing(*dims, W, H)
+    for texels in TEXELS:
+        for tau in (0.9, 0.99, 2.0):
+            g, o = tex_pair(vr, synth.Cube(1, *dims, 1), 16, 1, tf=synth.tf_ramp(), tau=tau, data=data, texels=texels)
+            o.set_ert_margin(0.02 * (1.0 - tau) if tau < 1 else 2e-4)
+            for k, step in ((0, 0.5), (1, 0.37), (2, 0.25)):
+                view, proj = fr.seeded(9, k), fr.proj(False)
+                check_alpha(gpu_frame(g, view, proj, W, H, step, vr.ALPHA), o.render(view, proj, W, H, step, oracle.ALPHA), tau,
+                            "peak at the table's top, %s, tau %g, step %g" % (texels, tau, step), envelope=True, max_flagged=1.0)
