@@ -720,6 +720,12 @@ def test_randomised_configurations(vr, case):
         g.set_sampler(s)
         check_alpha(gpu_frame(g, view, proj, W, H, step if step > 0 else vr.STEP_AUTO, vr.ALPHA), ref, tau,
                     "case %d sampler %d" % (case, s), envelope=True, max_flagged=1.0)
+    # ... and the fused traversal through the float32 arrays (per-lane texture objects) against the one-brick oracle
+    one.set_ert_margin(0.02 * (1.0 - tau) if tau < 1.0 else 2e-4)
+    g.set_sampler(vr.SAMPLER_TEXTURE)
+    g.set_traversal(vr.FUSED)
+    check_alpha(gpu_frame(g, view, proj, W, H, step if step > 0 else vr.STEP_AUTO, vr.ALPHA), one.render(view, proj, W, H, step, oracle.ALPHA),
+                tau, "case %d fused through the arrays" % case, envelope=True, max_flagged=1.0)
 
 
 # --------------------------------------------------------------------------- state across calls
