@@ -100,6 +100,30 @@ def test_config1_512cube_8_bricks(vr):
     g.set_transfer_function(synth.tf_translucent(), synth.TF_VMIN, synth.TF_VMAX)
     o.set_transfer_function(synth.tf_translucent(), synth.TF_VMIN, synth.TF_VMAX)
     check_views(vr, wl, g, o, (13,), 2000, (vr.ALPHA, vr.MIP), 0.99)
+    _texture_arm_checks(vr, wl, g, o, (6, 25))
+
+
+def _texture_arm_checks(vr, wl, g, o, view_ids):
+    """What `bench.py --sampler auto` times on the cubes that leave room for a second copy: ALPHA values through float32
+    (and float16) arrays, step 0.5 with R20's guard, against the same oracle at the same 2e-3; MIP through the 8-bit
+    exact filter (the frame of one view equal to the hand-rolled one)."""
+    W, H = wl["width"], wl["height"]
+    o.set_ert_margin(2e-4)
+    for tf in (synth.tf_ramp(), synth.tf_translucent()):
+        for v in (g, o):
+            v.set_transfer_function(tf, synth.TF_VMIN, synth.TF_VMAX)
+        for s in (vr.SAMPLER_TEXTURE, vr.SAMPLER_TEXTURE_HALF):
+            g.set_sampler(s)
+            check_views(vr, wl, g, o, view_ids[:1] if s == vr.SAMPLER_TEXTURE_HALF else view_ids, 1500, (vr.ALPHA,), 0.99, envelope=True,
+                        max_flagged=1.0)
+    g.set_sampler(vr.SAMPLER_MANUAL)
+    view = wl["views"][view_ids[0]]
+    mip = gpu_frame(g, view, wl["proj"], W, H, wl["step"], vr.MIP)
+    g.set_sampler(vr.SAMPLER_TEXTURE_BYTE)
+    assert np.array_equal(gpu_frame(g, view, wl["proj"], W, H, wl["step"], vr.MIP), mip)
+    check_views(vr, wl, g, o, view_ids[:1], 1000, (vr.MIP,), 0.99, tile=None)
+    g.set_sampler(vr.SAMPLER_MANUAL)
+    o.set_ert_margin(1e-5)
 
 
 def test_config2_1024cube_64_bricks(vr):
@@ -114,6 +138,12 @@ def test_config2_1024cube_64_bricks(vr):
     w4["proj"] = fr.proj(False)
     w4["name"] = "c4@4096"
     check_views(vr, w4, g, o, (21,), 1000, (vr.ALPHA, vr.MIP), 0.99)
+    _texture_arm_checks(vr, wl, g, o, (8, 30))
+    g.set_sampler(vr.SAMPLER_TEXTURE)   # the resolution sweep of config 4 through the arrays
+    o.set_ert_margin(2e-4)
+    for v in (g, o):
+        v.set_transfer_function(synth.tf_ramp(), synth.TF_VMIN, synth.TF_VMAX)
+    check_views(vr, w4, g, o, (11,), 1000, (vr.ALPHA,), 0.99, envelope=True, max_flagged=1.0)
 
 
 def test_config3_103GB_cube_192_bricks(vr):
