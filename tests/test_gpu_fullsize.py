@@ -262,6 +262,11 @@ def test_nbody_34GB_density_cube_with_culling(vr):
     assert culled == 0
     gpu_frame(g, wl["views"][13], wl["proj"], wl["width"], wl["height"], wl["step"], vr.ALPHA)
     assert g.debug_stats()["bricks_culled"] > 50
+    # what bench.py --sampler auto times on this cube: ALPHA values through the float32 arrays (beside macro-cell skipping)
+    g.set_sampler(vr.SAMPLER_TEXTURE)
+    o.set_ert_margin(2e-4)
+    check_views(vr, wl, g, o, (22,), 1200, (vr.ALPHA, vr.MIP), 0.99, envelope=True, max_flagged=1.0)
+    g.close()
 
 
 def parts_against_oracle(vr, wl, cube, o, tf, nparts, vi, npix, whole=None):
