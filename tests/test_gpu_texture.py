@@ -448,3 +448,43 @@ def test_nearly_opaque_samples_at_small_steps_are_taken_by_hand(vr):
                 view, proj = fr.seeded(9, k), fr.proj(False)
                 check_alpha(gpu_frame(g, view, proj, W, H, step, vr.ALPHA), o.render(view, proj, W, H, step, oracle.ALPHA), tau,
                             "peak at the table's top, %s, tau %g, step %g" % (texels, tau, step), envelope=True, max_flagged=1.0)
+
+
+@pytest.mark.parametrize("case", range(int(__import__("os").environ.get("VR_RELEASE_CASES", "16"))))
+def test_randomised_released_stores(vr, case):
+    """Seeded random volumes on VR_LAYOUT_TILED_RELEASABLE handles, released to float32 or float16 arrays: both traversals
+    against the oracle (steps in [0.9, 1]: what a released store renders), blanked bricks keep their float32 cells."""
+    import torch
+    rng = np.random.default_rng(7000 + case)
+    dims = tuple(int(v) for v in rng.integers(20, 80, 3))
+    brick = int(rng.choice([8, 16, 32]))
+    ghost = int(rng.choice([1, 1, 2]))
+    data = synth.Cube(300 + case, *dims, int(rng.integers(1, 8))).fill_host()
+    if rng.random() < 0.4:
+        data[rng.random(data.shape) < 0.005] = np.nan
+    tf = [synth.tf_ramp, synth.tf_translucent][int(rng.integers(0, 2))]()
+    tau = float(rng.choice([0.99, 0.9, 2.0]))
+    step = float(rng.choice([1.0, 1.0, 0.9, 0.95]))
+    half = bool(rng.integers(0, 2))
+    W, H = int(rng.integers(40, 130)), int(rng.integers(30, 100))
+    fr = synth.Framing(*dims, W, H)
+    view, proj = fr.seeded(800 + case, case), fr.proj(bool(rng.integers(0, 2)))
+    g = vr.Volume(*dims, brick, ghost, layout=vr.LAYOUT_TILED_RELEASABLE)
+    g.upload(torch.from_numpy(data).cuda())
+    o = oracle.Volume(*dims, brick, ghost, data=data)
+    one = oracle.Volume(*dims, 128, 1, data=data)
+    for v in (g, o, one):
+        v.set_transfer_function(tf, synth.TF_VMIN, synth.TF_VMAX)
+        v.set_early_termination(tau)
+    band = 0.02 * (1.0 - tau) if tau < 1.0 else 2e-4
+    o.set_ert_margin(band)
+    one.set_ert_margin(band)
+    if half:
+        g.set_sampler(vr.SAMPLER_TEXTURE_HALF)
+    assert g.release_store() >= 0
+    for trav, orc in ((vr.SORT_LAST, o), (vr.FUSED, one)):
+        g.set_traversal(trav)
+        check_alpha(gpu_frame(g, view, proj, W, H, step, vr.ALPHA), orc.render(view, proj, W, H, step, oracle.ALPHA), tau,
+                    "released case %d (%s texels, traversal %d)" % (case, "float16" if half else "float32", trav), envelope=True,
+                    max_flagged=1.0)
+    g.close()
