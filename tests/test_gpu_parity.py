@@ -91,6 +91,41 @@ def test_tma_upload_path_gives_the_same_store(vr):
             vr.debug_set_upload_path(1)
 
 
+@pytest.mark.parametrize("case", range(int(__import__("os").environ.get("VR_UPLOAD_CASES", "24"))))
+def test_randomised_uploads(vr, case):
+    """Row a1 under random use: volumes with ragged bricks, ghost 0-2, bricks of 8-256 cells (rows of one to three 128-cell
+    chunks plus tails), a whole-volume upload followed by random sub-boxes of new data (row lengths and origins that the
+    tensor map can and cannot describe, device and host sources): every brick equals the oracle's copy of the final volume,
+    and the volume comes back unchanged."""
+    import torch
+    rng = np.random.default_rng(9000 + case)
+    brick = int(rng.choice([8, 16, 32, 64, 128, 256]))
+    dims = tuple(int(v) for v in rng.integers(max(9, brick // 2), min(300, 3 * brick + 40), 3))
+    if brick >= 128:  # keep the oracle's copies small: one long axis is enough to cross chunk boundaries
+        dims = (int(rng.integers(130, 420)), int(rng.integers(20, 70)), int(rng.integers(10, 40)))
+    ghost = int(rng.choice([0, 1, 1, 2]))
+    nx, ny, nz = dims
+    data = rng.standard_normal((nz, ny, nx)).astype(np.float32)
+    g = vr.Volume(nx, ny, nz, brick, ghost)
+    g.upload(torch.from_numpy(data).cuda() if case % 2 else data)
+    for k in range(int(rng.integers(1, 5))):
+        sx, sy, sz = (int(rng.integers(1, d + 1)) for d in dims)
+        if rng.random() < 0.5:
+            sx = max(4, sx & ~3)                      # a row length the tensor map can describe
+        sx = min(sx, nx)
+        x0, y0, z0 = int(rng.integers(0, nx - sx + 1)), int(rng.integers(0, ny - sy + 1)), int(rng.integers(0, nz - sz + 1))
+        patch = rng.standard_normal((sz, sy, sx)).astype(np.float32)
+        data[z0:z0 + sz, y0:y0 + sy, x0:x0 + sx] = patch
+        g.upload(torch.from_numpy(patch).cuda() if (case + k) % 3 else patch, origin=(x0, y0, z0))
+    o = oracle.Volume(nx, ny, nz, brick, ghost, data=data)
+    for b in range(g.nbricks):
+        assert np.array_equal(g.debug_brick_data(b), o.brick_data(b)), (case, dims, brick, ghost, b)
+    back = np.zeros_like(data)
+    g.download(back)
+    assert np.array_equal(back, data)
+    g.close()
+
+
 # --------------------------------------------------------------------------- a2, a3
 @pytest.mark.parametrize("dims,brick", [((64, 64, 64), 64), ((100, 90, 70), 32), ((37, 29, 23), 8)])
 def test_brick_order_and_rectangles_match_exactly(vr, dims, brick):
