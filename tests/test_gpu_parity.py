@@ -115,14 +115,20 @@ def test_randomised_uploads(vr, case):
         sx = min(sx, nx)
         x0, y0, z0 = int(rng.integers(0, nx - sx + 1)), int(rng.integers(0, ny - sy + 1)), int(rng.integers(0, nz - sz + 1))
         patch = rng.standard_normal((sz, sy, sx)).astype(np.float32)
+        if rng.random() < 0.3:
+            patch[rng.random(patch.shape) < 0.02] = np.nan   # blanked voxels (R14)
         data[z0:z0 + sz, y0:y0 + sy, x0:x0 + sx] = patch
         g.upload(torch.from_numpy(patch).cuda() if (case + k) % 3 else patch, origin=(x0, y0, z0))
     o = oracle.Volume(nx, ny, nz, brick, ghost, data=data)
     for b in range(g.nbricks):
-        assert np.array_equal(g.debug_brick_data(b), o.brick_data(b)), (case, dims, brick, ghost, b)
+        assert np.array_equal(g.debug_brick_data(b), o.brick_data(b), equal_nan=True), (case, dims, brick, ghost, b)
+    # row f1 after the last upload: the per-brick ranges (one streaming read, integer atomics) equal the oracle's, blanked voxels ignored
+    mm = g.debug_brick_minmax()
+    for b in range(g.nbricks):
+        assert tuple(mm[b]) == o.brick_minmax(b), (case, b)
     back = np.zeros_like(data)
     g.download(back)
-    assert np.array_equal(back, data)
+    assert np.array_equal(back, data, equal_nan=True)
     g.close()
 
 
