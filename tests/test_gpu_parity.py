@@ -998,6 +998,40 @@ def test_reserved_views_render_without_allocating_and_torch_allocator(vr):
 
 
 # --------------------------------------------------------------------------- a9 stand-alone
+@pytest.mark.parametrize("case", range(int(__import__("os").environ.get("VR_COMPOSITE_CASES", "16"))))
+def test_randomised_compositing(vr, case):
+    """Row a9 under random use: 0-40 layers with random rectangles (empty, one pixel, full frame, straddling tile borders),
+    random visibility orders, frames that are not multiples of the 32x8 tile: vr_composite and vr_composite_static against
+    the oracle (R15, 1e-5) and against each other (bit-identical)."""
+    import torch
+    rng = np.random.default_rng(11000 + case)
+    W, H = int(rng.integers(1, 300)), int(rng.integers(1, 200))
+    n = int(rng.integers(0, 41))
+    rects, layers_h = [], []
+    for l in range(n):
+        kind = rng.random()
+        if kind < 0.1:
+            x0, y0, x1, y1 = 0, 0, W, H
+        elif kind < 0.2:
+            x0 = x1 = int(rng.integers(0, W + 1)); y0, y1 = 0, H          # empty
+        else:
+            x0, y0 = int(rng.integers(0, W)), int(rng.integers(0, H))
+            x1, y1 = int(rng.integers(x0, W + 1)), int(rng.integers(y0, H + 1))
+        rects.append((x0, y0, x1, y1))
+        a = rng.random((y1 - y0, x1 - x0, 1)).astype(np.float32)
+        layers_h.append(np.concatenate([rng.random((y1 - y0, x1 - x0, 3)).astype(np.float32) * a, a], axis=-1))
+    order = rng.permutation(n).astype(np.int32)
+    ref = oracle.composite(layers_h, rects, order, W, H)
+    layers_d = [torch.from_numpy(l).cuda() if l.size else torch.empty((0, 0, 4), device="cuda") for l in layers_h]
+    out = torch.full((H, W, 4), 7.0, dtype=torch.float32, device="cuda")
+    out_s = torch.full((H, W, 4), -7.0, dtype=torch.float32, device="cuda")
+    vr.composite(layers_d, np.array(rects, dtype=np.int32).reshape(n, 4), order, W, H, out)
+    vr.composite_static(layers_d, np.array(rects, dtype=np.int32).reshape(n, 4), order, W, H, out_s)
+    torch.cuda.synchronize()
+    assert np.abs(out.cpu().numpy() - ref).max() < 1e-5, case
+    assert torch.equal(out, out_s), case
+
+
 def test_composite_matches_oracle(vr):
     import torch
     W, H, n = 97, 61, 9
