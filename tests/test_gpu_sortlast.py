@@ -272,3 +272,41 @@ def test_parts_through_the_texture_arrays(vr, sampler):
             assert 1e-7 < np.abs(got - one).max() < 0.02
             check_alpha(got, o.render(view, proj, W, H, 0.6, oracle.ALPHA), 0.99, "parts, %s, view %d" % (sampler, k), envelope=True,
                         max_flagged=1.0)
+
+
+@pytest.mark.parametrize("case", range(int(__import__("os").environ.get("VR_PARTS_CASES", "12"))))
+def test_randomised_partitions(vr, case):
+    """Row f3 under random use: random volumes, brick sizes, 1-9 parts (as far as the grid has bricks), both modes, the
+    hand-rolled sampler or one of the texture arms on the parts: the merged frame is the single handle's (MIP: bit for
+    bit whatever the sampler; ALPHA: the same sub-images regrouped, to float32 rounding, with the hand-rolled sampler)."""
+    from paper_1205_0282_b200 import sortlast
+    rng = np.random.default_rng(13000 + case)
+    brick = int(rng.choice([8, 16, 32]))
+    dims = tuple(int(v) for v in rng.integers(brick + 3, 5 * brick, 3))
+    ghost = int(rng.choice([1, 1, 2]))
+    grid = sortlast.brick_grid(dims, brick)
+    nparts = int(rng.integers(1, min(9, grid[0] * grid[1] * grid[2]) + 1))
+    data = synth.Cube(600 + case, *dims, int(rng.integers(1, 6))).fill_host()
+    boxes, tree, parts = make_parts(vr, sortlast, data, dims, brick, ghost, nparts)
+    whole = vr.Volume(*dims, brick, ghost)
+    whole.upload(data)
+    tf = [synth.tf_ramp, synth.tf_translucent][int(rng.integers(0, 2))]()
+    for v in parts + [whole]:
+        v.set_transfer_function(tf, synth.TF_VMIN, synth.TF_VMAX)
+        v.set_early_termination(0.99)
+    sampler = int(rng.choice([vr.SAMPLER_MANUAL, vr.SAMPLER_TEXTURE, vr.SAMPLER_TEXTURE_HALF, vr.SAMPLER_TEXTURE_BYTE]))
+    for p in parts:
+        p.set_sampler(sampler)
+    W, H = int(rng.integers(40, 160)), int(rng.integers(30, 120))
+    fr = synth.Framing(*dims, W, H)
+    view, proj = fr.seeded(40 + case, case), fr.proj(bool(rng.integers(0, 2)))
+    step = float(rng.choice([0.5, 1.0, 0.7]))
+    gotm = merged_frame(vr, sortlast, parts, boxes, tree, dims, brick, view, proj, W, H, step, vr.MIP)
+    assert np.array_equal(gotm, gpu_frame(whole, view, proj, W, H, step, vr.MIP)), (case, nparts, sampler)
+    got = merged_frame(vr, sortlast, parts, boxes, tree, dims, brick, view, proj, W, H, step, vr.ALPHA)
+    one = gpu_frame(whole, view, proj, W, H, step, vr.ALPHA)
+    if sampler in (vr.SAMPLER_MANUAL, vr.SAMPLER_TEXTURE_BYTE):
+        assert np.abs(got - one).max() < 2e-6, (case, nparts)
+    else:
+        whole.set_sampler(sampler)   # the same arrays on the single handle: the same sub-images regrouped
+        assert np.abs(got - gpu_frame(whole, view, proj, W, H, step, vr.ALPHA)).max() < 2e-6, (case, nparts, sampler)
