@@ -496,7 +496,7 @@ def roofline_of(counts, stages, stage_views, peak_gbs, peak_src, traffic=None):
     lines_gbs = lines / (ms * 1e-3) / 1e9
     return {"bound": "hbm", "kernel": "vr_raycast_kernel", "achieved": round(achieved, 1), "peak": peak_gbs, "unit": "GB/s",
             "frac": round(achieved / peak_gbs, 4), "traffic": traffic,
-            "traffic_source": "quoted: dram__bytes_read.sum + dram__bytes_write.sum of one launch in the committed ncu --set full capture "
+            "traffic_source": "quoted: dram__bytes_read.sum + dram__bytes_write.sum of one launch in the committed ncu capture "
                               "(profiles/r2_traffic.csv), not measured in this run" if traffic else None,
             "peak_source": peak_src,
             "algorithmic_bytes_per_launch": round(alg / n), "launch_ms": round(ms / n, 4), "views_counted": n,
