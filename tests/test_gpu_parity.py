@@ -707,7 +707,7 @@ def test_randomised_configurations(vr, case):
     rng = np.random.default_rng(1000 + case)
     nx, ny, nz = (int(v) for v in rng.integers(18, 75, 3))
     brick = int(rng.choice([8, 12, 16, 20, 32, 64]))
-    ghost = int(rng.choice([1, 1, 2]))
+    ghost = int(rng.choice([1, 1, 2])) if case % 7 else 0   # every seventh case without ghost cells (clamped fetches, seams as the oracle's)
     kind = int(rng.choice([0, 0, 1]))
     cube = synth.Cube(500 + case, nx, ny, nz, int(rng.integers(1, 8)), kind=kind)
     data = cube.fill_host()
@@ -738,7 +738,8 @@ def test_randomised_configurations(vr, case):
         v.set_transfer_function(tf, lo, hi)
         v.set_early_termination(tau)
     assert np.array_equal(g.debug_brick_order(view, proj), o.brick_order(view, proj))
-    for trav, orc in ((vr.SORT_LAST, o), (vr.FUSED, one)):
+    # the fused traversal has the one-brick oracle as its reference, which needs ghost cells (R17: no seams)
+    for trav, orc in ((vr.SORT_LAST, o), (vr.FUSED, one)) if ghost > 0 else ((vr.SORT_LAST, o),):
         g.set_traversal(trav)
         ref = orc.render(view, proj, W, H, step, oracle.ALPHA)
         check_alpha(gpu_frame(g, view, proj, W, H, step if step > 0 else vr.STEP_AUTO, vr.ALPHA), ref,
@@ -762,6 +763,8 @@ def test_randomised_configurations(vr, case):
         check_alpha(gpu_frame(g, view, proj, W, H, step if step > 0 else vr.STEP_AUTO, vr.ALPHA), ref, tau,
                     "case %d sampler %d" % (case, s), envelope=True, max_flagged=1.0)
     # ... and the fused traversal through the float32 arrays (per-lane texture objects) against the one-brick oracle
+    if ghost == 0:
+        return
     one.set_ert_margin(0.02 * (1.0 - tau) if tau < 1.0 else 2e-4)
     g.set_sampler(vr.SAMPLER_TEXTURE)
     g.set_traversal(vr.FUSED)
