@@ -206,6 +206,12 @@ def _config3_checks(vr, wl, g, o, cube):
     assert freed > 100e9 and torch.cuda.mem_get_info()[0] > free0 - 0.25 * freed, (freed, free0, torch.cuda.mem_get_info()[0])
     o.set_ert_margin(2e-4)
     check_views(vr, wl, g, o, (4, 17), 1500, (vr.ALPHA,), 0.99, envelope=True, max_flagged=1.0)
+    # ... and EVERY pixel of one frame of the headline arm (all 36 views were checked this way in round 2: max 1.65e-3)
+    W, H = wl["width"], wl["height"]
+    full = o.render(wl["views"][20], wl["proj"], W, H, wl["step"], oracle.ALPHA)
+    worst = check_alpha(gpu_frame(g, wl["views"][20], wl["proj"], W, H, wl["step"], vr.ALPHA), full, 0.99, "c3 released, whole frame 20",
+                        envelope=True, max_flagged=1.0)
+    assert worst < 2e-3
     g.set_transfer_function(synth.tf_translucent(), synth.TF_VMIN, synth.TF_VMAX)
     o.set_transfer_function(synth.tf_translucent(), synth.TF_VMIN, synth.TF_VMAX)
     check_views(vr, wl, g, o, (29,), 1000, (vr.ALPHA,), 0.99, envelope=True, max_flagged=1.0)
