@@ -285,8 +285,10 @@ int vr_set_traversal(vr_volume* v, int traversal);
  * that pays, it is used instead). Fused MIP frames
  * and counting mode 2 always use the hand-rolled path, and so do (i) bricks that hold blanked (NaN) voxels -
  * the filter cannot apply R14's rule - and (ii) frames whose transfer function has a step: two neighbouring entries
- * further apart than 2.56/n in a channel (a threshold, a toe). The filter's value error is about one table entry on
- * unit-sigma noise; across a step that is a wrong opacity, not 2e-3 (measured: 8e-2 on a threshold table).
+ * further apart than 1.1/n in a channel - anything steeper than a ramp over the table's whole range (a threshold, a toe,
+ * a ramp over half the range). The filter's value error is about one table entry on unit-sigma noise, so the frame's
+ * error grows with the table's slope: 1.4e-3 to 1.65e-3 at slope 1 (the ramp), 2.7e-3 at 1.5, 3.3e-3 at 2.5, 8e-2 on
+ * a threshold table (measured).
  * VR_SAMPLER_TEXTURE_HALF: the same arm with arrays of float16 texels - float16 COPIES of the float32 voxels, made for
  * sampling only (the store, the range tables, blanked bricks and every other path stay float32): half the memory and
  * about three quarters of the fetched bytes. Rounding a voxel to float16 (to nearest) moves it by at most 2^-11 of its

@@ -62,7 +62,7 @@ struct vr_volume {
     bool mip_skip_known, mip_skip_useful; /* decided once per upload: does the cube have empty space (R19, MIP) */
     bool half_alpha_known, half_alpha_ok;  /* decided per upload and transfer function: may ALPHA values come from float16 texels (R22) */
     unsigned long long* d_cell_count;
-    bool tf_smooth;          /* no neighbouring LUT entries further apart than 2.56/n per channel (texture arm) */
+    bool tf_smooth;          /* no neighbouring LUT entries further apart than 1.1/n per channel: no steeper than a full-range ramp (texture arm, R20) */
     bool tf_has_zero;        /* the LUT has a run of >= 3 zero-alpha entries: skipping can do something */
     bool culling;
     int sampler;             /* VR_SAMPLER_MANUAL or VR_SAMPLER_TEXTURE */
@@ -582,7 +582,7 @@ extern "C" int vr_set_transfer_function(vr_volume* v, const float* rgba, int n, 
     v->half_alpha_known = false;
     for (int i = 0; i + 1 < n; ++i)
         for (int c = 0; c < 4; ++c)
-            if (fabsf(rgba[4 * i + 4 + c] - rgba[4 * i + c]) > 2.56f / (float)n) v->tf_smooth = false;
+            if (fabsf(rgba[4 * i + 4 + c] - rgba[4 * i + c]) > 1.1f / (float)n) v->tf_smooth = false; /* R20 (ii): no steeper than a full-range ramp */
     v->cell_bits_valid = false;
     v->has_tf = true;
     return VR_OK;

@@ -488,3 +488,27 @@ def test_randomised_released_stores(vr, case):
                     "released case %d (%s texels, traversal %d)" % (case, "float16" if half else "float32", trav), envelope=True,
                     max_flagged=1.0)
     g.close()
+
+
+def test_tables_steeper_than_a_full_range_ramp_keep_the_hand_rolled_sampler(vr):
+    """R20 (ii): the frame's error through the arrays grows with the table's slope (2.7e-3 at 1.5 times the ramp's), so
+    only tables no steeper than a ramp over the whole range take their values from the arrays; a ramp over the top half of
+    the range renders exactly as with the hand-rolled sampler although the texture sampler is in force."""
+    c = synth.CONFIGS["c0"]
+    cube = synth.config_cube("c0")
+    W, H = 128, 128
+    fr = synth.Framing(cube.nx, cube.ny, cube.nz, W, H)
+    view, proj = fr.seeded(77, 0), fr.proj(False)
+    for slope, through_arrays in ((1.0, True), (1.05, True), (1.5, False), (2.0, False)):
+        tf = synth.tf_ramp()
+        n = tf.shape[0]
+        u = np.arange(n) / (n - 1)
+        tf[:, 3] = np.clip((u - (1 - 1 / slope)) * slope, 0, 1).astype(np.float32)
+        g, o = make_pair(cube, c["brick"], 1, tf=tf, tau=0.99)
+        o.set_ert_margin(2e-4)
+        man = gpu_frame(g, view, proj, W, H, 0.5, vr.ALPHA)
+        for s in (vr.SAMPLER_TEXTURE, vr.SAMPLER_TEXTURE_HALF):
+            g.set_sampler(s)
+            img = gpu_frame(g, view, proj, W, H, 0.5, vr.ALPHA)
+            assert (not np.array_equal(img, man)) == through_arrays, (slope, s)
+            check_alpha(img, o.render(view, proj, W, H, 0.5, oracle.ALPHA), 0.99, "slope %g" % slope, envelope=True, max_flagged=1.0)
