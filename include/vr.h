@@ -288,7 +288,10 @@ int vr_set_traversal(vr_volume* v, int traversal);
  * further apart than 1.1/n in a channel - anything steeper than a ramp over the table's whole range (a threshold, a toe,
  * a ramp over half the range). The filter's value error is about one table entry on unit-sigma noise, so the frame's
  * error grows with the table's slope: 1.4e-3 to 1.65e-3 at slope 1 (the ramp), 2.7e-3 at 1.5, 3.3e-3 at 2.5, 8e-2 on
- * a threshold table (measured).
+ * a threshold table (measured). (iii) For the same reason the data must be smooth enough against the table: with R = the
+ * mean range of the 8x8x8 macro-cells over the table's range (0.46-0.48 on the benchmark cubes), VR_ALPHA values come
+ * from the arrays only while 3.5e-3 x R x (table slope) <= 1.9e-3 (vr_debug_tex_alpha_guard); otherwise the frames use
+ * the hand-rolled sampler (VR_ERR_STATE on a released store). Needs ghost >= 1 (the macro-cell table).
  * VR_SAMPLER_TEXTURE_HALF: the same arm with arrays of float16 texels - float16 COPIES of the float32 voxels, made for
  * sampling only (the store, the range tables, blanked bricks and every other path stay float32): half the memory and
  * about three quarters of the fetched bytes. Rounding a voxel to float16 (to nearest) moves it by at most 2^-11 of its
@@ -476,6 +479,13 @@ int vr_debug_cell_flags(vr_volume* v, int b, unsigned char* flags_out, int* dims
 
 /* mm_out (host): nbricks * 2 floats, (min, max) per brick over its ghost-padded cells. */
 int vr_debug_brick_minmax(vr_volume* v, float* mm_out);
+
+/* The texture arm's data guard for VR_ALPHA values (R20 vii; test / measurement export): the mean range
+ * (max - min) of the handle's 8x8x8 macro-cells, the table's largest difference between neighbouring entries in units of
+ * 1/n, and whether 3.5e-3 x (mean range / table range) x slope <= 1.9e-3, i.e. whether VR_ALPHA frames may take their
+ * values from the arrays (else they use the hand-rolled sampler; VR_ERR_STATE on a released store). Outputs: host.
+ * Synchronises. Errors: VR_ERR_STATE (no data or no transfer function). */
+int vr_debug_tex_alpha_guard(vr_volume* v, float* mean_cell_range_out, float* table_slope_out, int* ok_out);
 
 /* R23's constant, measured (test / measurement export): with a texture sampler in force, the largest
  * |filtered fetch - exact tri-linear value| over n hashed sample positions inside brick b (the exact value in double

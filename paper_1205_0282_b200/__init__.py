@@ -28,7 +28,7 @@ STATUS = {0: "VR_OK", 1: "VR_ERR_INVALID_ARG", 2: "VR_ERR_OUT_OF_MEMORY", 3: "VR
 # every symbol include/vr.h declares (tests check the library exports each of them)
 SYMBOLS = (
     "vr_volume_create", "vr_volume_create_layout", "vr_volume_destroy", "vr_volume_upload", "vr_volume_download", "vr_debug_brick_data",
-    "vr_set_transfer_function", "vr_set_early_termination", "vr_volume_minmax", "vr_set_culling", "vr_set_traversal", "vr_set_sampler", "vr_volume_release_store", "vr_set_allocator", "vr_reserve_views", "vr_debug_brick_minmax", "vr_debug_tex_error", "vr_debug_cell_flags", "vr_render", "vr_render_host", "vr_render_host_async", "vr_render_host_wait", "vr_composite", "vr_composite_static",
+    "vr_set_transfer_function", "vr_set_early_termination", "vr_volume_minmax", "vr_set_culling", "vr_set_traversal", "vr_set_sampler", "vr_volume_release_store", "vr_set_allocator", "vr_reserve_views", "vr_debug_brick_minmax", "vr_debug_tex_error", "vr_debug_tex_alpha_guard", "vr_debug_cell_flags", "vr_render", "vr_render_host", "vr_render_host_async", "vr_render_host_wait", "vr_composite", "vr_composite_static",
     "vr_num_bricks", "vr_debug_brick_order", "vr_debug_rects", "vr_debug_ray_bricks", "vr_debug_subimages",
     "vr_volume_create_part", "vr_render_part", "vr_render_part_pieces", "vr_part_rect", "vr_composite_parts", "vr_kd_partition", "vr_part_order",
     "vr_set_counting", "vr_set_timing", "vr_debug_stats", "vr_debug_stage_times", "vr_debug_probe_dram", "vr_debug_set_upload_path", "vr_launch_count", "vr_last_error",
@@ -80,6 +80,7 @@ def lib():
         L.vr_reserve_views.argtypes = [vp, vp, vp, ci, ci, ci]
         L.vr_debug_brick_minmax.argtypes = [vp, vp]
         L.vr_debug_tex_error.argtypes = [vp, ci, ctypes.c_int64, ctypes.c_uint, vp, vp]
+        L.vr_debug_tex_alpha_guard.argtypes = [vp, vp, vp, vp]
         L.vr_debug_cell_flags.argtypes = [vp, ci, vp, vp]
         L.vr_render.argtypes = [vp, vp, vp, ci, ci, cf, ci, vp, vp]
         L.vr_render_host.argtypes = [vp, vp, vp, ci, ci, cf, ci, vp, vp]
@@ -285,6 +286,12 @@ class Volume:
         mm = np.empty((self.nbricks, 2), dtype=np.float32)
         self._check(lib().vr_debug_brick_minmax(self._h, mm.ctypes.data))
         return mm
+
+    def debug_tex_alpha_guard(self):
+        """(mean macro-cell range, table slope in units of 1/n, whether ALPHA values may come from the arrays): R20's data guard."""
+        rng, slope, ok = ctypes.c_float(), ctypes.c_float(), ctypes.c_int()
+        self._check(lib().vr_debug_tex_alpha_guard(self._h, ctypes.byref(rng), ctypes.byref(slope), ctypes.byref(ok)))
+        return float(rng.value), float(slope.value), bool(ok.value)
 
     def debug_tex_error(self, brick, n=1 << 20, seed=1):
         """(largest |filtered fetch - exact value| over n hashed positions of the brick, the brick's range): R23's constant."""

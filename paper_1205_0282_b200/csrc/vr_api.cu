@@ -60,6 +60,10 @@ struct vr_volume {
     int nc[3], cell_words;   /* macro-cells per axis of a slot; words of d_cell_bits per brick */
     bool cell_mm_valid, cell_bits_valid;
     bool mip_skip_known, mip_skip_useful; /* decided once per upload: does the cube have empty space (R19, MIP) */
+    bool tex_alpha_known, tex_alpha_ok; /* decided per upload and transfer function: may ALPHA values come from the arrays at all (R20 vii) */
+    float tf_slope;          /* largest difference between neighbouring table entries, in units of 1/n */
+    float mean_cell_range;   /* mean (max - min) of the macro-cells, valid with tex_alpha_known */
+    double* d_cell_stat;
     bool half_alpha_known, half_alpha_ok;  /* decided per upload and transfer function: may ALPHA values come from float16 texels (R22) */
     unsigned long long* d_cell_count;
     bool tf_smooth;          /* no neighbouring LUT entries further apart than 1.1/n per channel: no steeper than a full-range ramp (texture arm, R20) */
@@ -177,6 +181,7 @@ static void release(vr_volume* v) {
     v_free(v, v->d_cell_mm);
     v_free(v, v->d_cell_bits);
     v_free(v, v->d_cell_count);
+    v_free(v, v->d_cell_stat);
     v_free(v, v->d_counts2);
     for (int r = 0; r < VR_EV_RING; ++r)
         for (int i = 0; i < 4; ++i)
@@ -461,6 +466,7 @@ extern "C" int vr_volume_upload(vr_volume* v, const float* src, int memspace, in
     v->cell_mm_valid = v->cell_bits_valid = false;
     v->mip_skip_known = false;
     v->half_alpha_known = false;
+    v->tex_alpha_known = false;
     return VR_OK;
 }
 
@@ -579,10 +585,14 @@ extern "C" int vr_set_transfer_function(vr_volume* v, const float* rgba, int n, 
      * sample (about one table entry on noise of unit sigma over a 13-sigma, 256-entry table); 2e-3 per channel survives that
      * only if neighbouring entries are close. Tables with steps (thresholds, toes) keep the hand-rolled sampler. */
     v->tf_smooth = true;
+    v->tf_slope = 0.0f;
     v->half_alpha_known = false;
+    v->tex_alpha_known = false;
     for (int i = 0; i + 1 < n; ++i)
-        for (int c = 0; c < 4; ++c)
+        for (int c = 0; c < 4; ++c) {
+            v->tf_slope = fmaxf(v->tf_slope, fabsf(rgba[4 * i + 4 + c] - rgba[4 * i + c]) * (float)n);
             if (fabsf(rgba[4 * i + 4 + c] - rgba[4 * i + c]) > 1.1f / (float)n) v->tf_smooth = false; /* R20 (ii): no steeper than a full-range ramp */
+        }
     v->cell_bits_valid = false;
     v->has_tf = true;
     return VR_OK;
@@ -770,6 +780,35 @@ static int decide_mip_skip(vr_volume* v, cudaStream_t st) {
     VR_CUDA(v, cudaStreamSynchronize(st));
     v->mip_skip_useful = empty * 8ull >= (unsigned long long)ncells;
     v->mip_skip_known = true;
+    return VR_OK;
+}
+
+/* R20 (vii): the filter's error is proportional to the voxel-to-voxel differences against the table's range. The mean range of
+ * the 8x8x8 macro-cells stands for those differences; measured on the benchmark cubes (ratio R = mean cell range / table range =
+ * 0.46-0.48, ramp table: slope 1) the largest pixel error of a frame is 1.4e-3 to 1.65e-3, i.e. up to 3.5e-3 x R x slope. ALPHA values
+ * come from the arrays only while that estimate stays below 1.9e-3; decided once per upload / table. */
+static int decide_tex_alpha(vr_volume* v, cudaStream_t st) {
+    if (v->tex_alpha_known) return VR_OK;
+    v->tex_alpha_ok = false;
+    v->mean_cell_range = 0.0f;
+    if (cells_supported(v)) {
+        int rc = ensure_minmax(v, st);
+        if (rc) return rc;
+        if (!v->d_cell_stat) VR_CUDA(v, v_alloc(v, &v->d_cell_stat, 2 * sizeof(double)));
+        const long long ncells = (long long)v->nc[0] * v->nc[1] * v->nc[2] * v->grid.nown;
+        double stat[2] = {0.0, 0.0};
+        VR_CUDA(v, cudaMemsetAsync(v->d_cell_stat, 0, sizeof(stat), st));
+        VR_CUDA(v, vr_launch_cell_range_sum(v->d_cell_mm, ncells, v->d_cell_stat, st));
+        v->launches++;
+        VR_CUDA(v, cudaMemcpyAsync(stat, v->d_cell_stat, sizeof(stat), cudaMemcpyDeviceToHost, st));
+        VR_CUDA(v, cudaStreamSynchronize(st));
+        if (stat[1] > 0.0) {
+            v->mean_cell_range = (float)(stat[0] / stat[1]);
+            const float R = v->mean_cell_range / (v->lut.vmax - v->lut.vmin);
+            v->tex_alpha_ok = 3.5e-3f * R * v->tf_slope <= 1.9e-3f;
+        }
+    }
+    v->tex_alpha_known = true;
     return VR_OK;
 }
 
@@ -1001,6 +1040,19 @@ extern "C" int vr_debug_tex_error(vr_volume* v, int b, int64_t n, unsigned seed,
     return VR_OK;
 }
 
+/* R20 (vii): the quantities the texture arm's ALPHA guard is decided on (test / measurement export) */
+extern "C" int vr_debug_tex_alpha_guard(vr_volume* v, float* mean_cell_range_out, float* table_slope_out, int* ok_out) {
+    if (!v) return fail(NULL, VR_ERR_INVALID_ARG, "vr_debug_tex_alpha_guard: NULL handle");
+    if (!mean_cell_range_out || !table_slope_out || !ok_out) return fail(v, VR_ERR_INVALID_ARG, "vr_debug_tex_alpha_guard: NULL output");
+    if (!v->has_data || !v->has_tf) return fail(v, VR_ERR_STATE, "vr_debug_tex_alpha_guard: needs data and a transfer function");
+    const int rc = decide_tex_alpha(v, 0);
+    if (rc) return rc;
+    *mean_cell_range_out = v->mean_cell_range;
+    *table_slope_out = v->tf_slope;
+    *ok_out = v->tex_alpha_ok ? 1 : 0;
+    return VR_OK;
+}
+
 extern "C" int vr_debug_brick_minmax(vr_volume* v, float* mm_out) {
     if (!v) return fail(NULL, VR_ERR_INVALID_ARG, "vr_debug_brick_minmax: NULL handle");
     if (!mm_out) return fail(v, VR_ERR_INVALID_ARG, "vr_debug_brick_minmax: NULL output");
@@ -1154,6 +1206,17 @@ static int render_frame(vr_volume* v, const float* view, const float* proj, int 
      * arrays for steps up to one voxel only (the randomised suite found 2.2e-3 at step 1.63; VR_STEP_AUTO's per-ray steps are >= 1) */
     bool tex_alpha = (v->sampler == VR_SAMPLER_TEXTURE || v->sampler == VR_SAMPLER_TEXTURE_HALF) && mode == VR_ALPHA && v->counting != 2 && v->tf_smooth &&
                      step > 0.0f && step <= 1.0f;
+    if (tex_alpha) { /* R20 (vii): only while the data's voxel-to-voxel differences are small enough against this table */
+        rc = decide_tex_alpha(v, st);
+        if (rc) return rc;
+        if (!v->tex_alpha_ok) {
+            if (v->store_released)
+                return fail(v, VR_ERR_STATE, "vr_render: the texture filter is too coarse for this data under this transfer function (mean macro-cell "
+                                             "range %g against a table range of %g, table slope %g: DESIGN.md R20) and the float32 store was released",
+                            (double)v->mean_cell_range, (double)(v->lut.vmax - v->lut.vmin), (double)v->tf_slope);
+            tex_alpha = false; /* the hand-rolled sampler */
+        }
+    }
     if (tex_alpha && v->sampler == VR_SAMPLER_TEXTURE_HALF) { /* R22: only while float16 is fine enough for this data under this table */
         rc = decide_half_alpha(v, st);
         if (rc) return rc;

@@ -225,6 +225,7 @@ cudaError_t vr_launch_ranges(const VrGrid& grid, const float* bricks, int2* enc,
 /* macro-cells (R19): per-cell (min, max) of the 4x4x2-tiled store; transparency bits for a LUT */
 cudaError_t vr_launch_cell_minmax(const VrGrid& grid, const float* bricks, float2* cell_mm, const int nc[3], cudaStream_t st);
 /* *count += macro-cells of the whole store whose (min, max) is exactly (lo, lo): empty space of a density cube */
+cudaError_t vr_launch_cell_range_sum(const float2* cell_mm, long long ncells, double* stat, cudaStream_t st);
 cudaError_t vr_launch_cell_count_empty(const float2* cell_mm, long long ncells, const float2* global_mm, unsigned long long* count,
                                        cudaStream_t st);
 cudaError_t vr_launch_cell_flags(const float2* cell_mm, unsigned* bits, int nbricks, const int nc[3], int words_per_brick,

@@ -400,3 +400,26 @@ cudaError_t vr_launch_cell_count_empty(const float2* cell_mm, long long ncells, 
     vr_cell_count_empty_kernel<<<148 * 8, 256, 0, st>>>(cell_mm, ncells, global_mm, count);
     return cudaGetLastError();
 }
+
+
+/* R20 (vii): the mean range of the macro-cells that hold finite data - the scale of the voxel-to-voxel differences the
+ * texture filter's error is proportional to. stat[0] += sum of (max - min), stat[1] += number of such cells. */
+__global__ void __launch_bounds__(256)
+vr_cell_range_sum_kernel(const float2* __restrict__ cell_mm, long long ncells, double* __restrict__ stat) {
+    double sum = 0.0, cnt = 0.0;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < ncells; i += (long long)gridDim.x * blockDim.x) {
+        const float2 r = cell_mm[i];
+        const float d = r.y - r.x;
+        if (d >= 0.0f && d < INFINITY) sum += (double)d, cnt += 1.0;
+    }
+    for (int o = 16; o > 0; o >>= 1) sum += __shfl_xor_sync(0xffffffffu, sum, o), cnt += __shfl_xor_sync(0xffffffffu, cnt, o);
+    if ((threadIdx.x & 31) == 0 && cnt > 0.0) {
+        atomicAdd(stat, sum);
+        atomicAdd(stat + 1, cnt);
+    }
+}
+
+cudaError_t vr_launch_cell_range_sum(const float2* cell_mm, long long ncells, double* stat, cudaStream_t st) {
+    vr_cell_range_sum_kernel<<<148 * 8, 256, 0, st>>>(cell_mm, ncells, stat);
+    return cudaGetLastError();
+}

@@ -512,3 +512,32 @@ def test_tables_steeper_than_a_full_range_ramp_keep_the_hand_rolled_sampler(vr):
             img = gpu_frame(g, view, proj, W, H, 0.5, vr.ALPHA)
             assert (not np.array_equal(img, man)) == through_arrays, (slope, s)
             check_alpha(img, o.render(view, proj, W, H, 0.5, oracle.ALPHA), 0.99, "slope %g" % slope, envelope=True, max_flagged=1.0)
+
+
+def test_data_too_rough_for_the_table_keeps_the_hand_rolled_sampler(vr):
+    """R20 (vii): the filter's error scales with the voxel-to-voxel differences against the table's range. The same cube
+    three times as noisy under the same table (or the same cube under a table a third as wide) fails the guard and renders
+    exactly as with the hand-rolled sampler; the benchmark statistics pass it."""
+    c = synth.CONFIGS["c0"]
+    cube = synth.config_cube("c0")
+    data = cube.fill_host()
+    W, H = 128, 128
+    fr = synth.Framing(cube.nx, cube.ny, cube.nz, W, H)
+    view, proj = fr.seeded(77, 1), fr.proj(False)
+    for scale, lo, hi, through_arrays in ((1.0, synth.TF_VMIN, synth.TF_VMAX, True), (3.0, synth.TF_VMIN, synth.TF_VMAX, False),
+                                         (1.0, -1.0, 3.3, False), (0.3, synth.TF_VMIN, synth.TF_VMAX, True)):
+        d = (data * scale).astype(np.float32)
+        g = vr.Volume(cube.nx, cube.ny, cube.nz, c["brick"], 1)
+        g.upload(d)
+        o = oracle.Volume(cube.nx, cube.ny, cube.nz, c["brick"], 1, data=d)
+        for v in (g, o):
+            v.set_transfer_function(synth.tf_ramp(), lo, hi)
+            v.set_early_termination(0.99)
+        o.set_ert_margin(2e-4)
+        rng_, slope, ok = g.debug_tex_alpha_guard()
+        assert ok == through_arrays and abs(slope - 1.004) < 1e-3, (scale, lo, hi, rng_, slope, ok)
+        man = gpu_frame(g, view, proj, W, H, 0.5, vr.ALPHA)
+        g.set_sampler(vr.SAMPLER_TEXTURE)
+        img = gpu_frame(g, view, proj, W, H, 0.5, vr.ALPHA)
+        assert (not np.array_equal(img, man)) == through_arrays
+        check_alpha(img, o.render(view, proj, W, H, 0.5, oracle.ALPHA), 0.99, "roughness guard", envelope=True, max_flagged=1.0)
