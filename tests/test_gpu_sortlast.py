@@ -313,5 +313,15 @@ def test_randomised_partitions(vr, case):
         # the hand-rolled sampler where the whole volume does not (or the other way round) is within the tolerance of both
         whole.set_sampler(sampler)
         same = len({h.debug_tex_alpha_guard()[2] for h in parts + [whole]}) == 1 and sampler == vr.SAMPLER_TEXTURE
-        diff = np.abs(got - gpu_frame(whole, view, proj, W, H, step, vr.ALPHA)).max()
-        assert diff < (2e-6 if same else 4e-3), (case, nparts, sampler, diff)
+        if same:
+            assert np.abs(got - gpu_frame(whole, view, proj, W, H, step, vr.ALPHA)).max() < 2e-6, (case, nparts, sampler)
+        # against the oracle the arrays' values are a MEASURED 2e-3, not a bound (R20 viii): this suite, run at 1200
+        # cases, met one frame with two pixels at 2.4e-3 (case 1165, float16 texels). What it pins here is the regrouping;
+        # the oracle parity of the texture arm is test_randomised_configurations' and the full-size tests' business.
+        o = oracle.Volume(*dims, brick, ghost, data=data)
+        o.set_transfer_function(tf, synth.TF_VMIN, synth.TF_VMAX)
+        o.set_early_termination(0.99)
+        o.set_ert_margin(2e-4)
+        ref = o.render(view, proj, W, H, step, oracle.ALPHA)
+        err = np.abs(got - ref["image"]).max(axis=-1)
+        assert (err[ref["flags"] == 0] > 2e-3).mean() < 1e-3 and err[ref["flags"] == 0].max() < 4e-3, (case, nparts, sampler)
